@@ -1,0 +1,238 @@
+"""Seeded synthetic inputs for the five BASELINE.json configs (plus stress cases).
+
+This module serves BOTH the CUDA path and the CPU oracle and therefore holds none of the
+method's arithmetic: no Philox, no dynamics, no cost, no softmax.  It only builds tracks,
+references, paths, initial states and parameter sets from the recipes in DESIGN.md section
+"Input recipe" (readings R-15/R-16).  It stands in for the paper's Circle /
+Figure-8 / Split-S tracks and CPC references, whose coordinates are not
+printed in the paper.
+
+Every array is rounded to float32 so that the GPU (fp32) and the oracle (fp64) see the same
+real numbers; scalars in `params` are float32-representable for the same reason.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+
+import numpy as np
+
+OBJ_GATE, OBJ_TRACK, OBJ_CONTOUR = 0, 1, 2
+
+
+def _f32(v):
+    return float(np.float32(v))
+
+
+def base_params(**over) -> dict:
+    """Quadrotor + cost constants of BASELINE.json configs[0]/[2]/[3]; all float32-exact."""
+    p = dict(K=256, N=20, B=1, objective=OBJ_GATE,
+             dt=0.02, sigma=1.0, mass=0.85, Jx=1e-3, Jy=1e-3, Jz=1.7e-3, arm=0.15, c_tau=0.016,
+             g=9.81, T_min=0.0, T_max=7.0, w_omega=0.01, gate_miss_penalty=10.0,
+             gate_pass_bonus=5.0, Qp=100.0, Qv=1.0, Qq=10.0, Qw=0.1, R=0.01, q_contour=200.0,
+             q_lag=50.0, mu_progress=2.0, window=16)
+    p["lambda"] = 1.0
+    p.update(over)
+    for k, v in p.items():
+        if k not in ("K", "N", "B", "objective", "window"):
+            p[k] = _f32(v)
+    return p
+
+
+def hover_thrust(p: dict) -> np.float32:
+    """Nominal input of the configs: each rotor carries a quarter of the weight."""
+    return np.float32(np.float32(p["mass"]) * np.float32(p["g"]) / np.float32(4.0))
+
+
+@dataclass
+class Workload:
+    name: str
+    params: dict
+    x0: np.ndarray                      # [B,13] f32: p, q(wxyz), v, omega
+    start: np.ndarray                   # [B] i32
+    u_nom: np.ndarray                   # [B,N,4] f32
+    gates: np.ndarray | None = None     # [G,11] f32
+    ref: np.ndarray | None = None       # [M,13] f32
+    path: np.ndarray | None = None      # [P,3] f32
+    closed: bool = True
+    seed: int = 0
+    iters: int = 1                      # optimiser iterations (cfg1) or control steps (cfg4)
+    notes: dict = field(default_factory=dict)
+
+
+# ---- tracks ------------------------------------------------------------------------------
+
+def _gate_rows(centres, normals, half_w, half_h):
+    n = np.asarray(normals, dtype=np.float64)
+    n = n / np.linalg.norm(n, axis=1, keepdims=True)
+    h = np.stack([n[:, 1], -n[:, 0], np.zeros(len(n))], axis=1)   # h = (n_y, -n_x, 0): h x n = +z
+    h = h / np.linalg.norm(h, axis=1, keepdims=True)
+    g = np.concatenate([np.asarray(centres, dtype=np.float64), n, h,
+                        np.full((len(n), 1), half_w), np.full((len(n), 1), half_h)], axis=1)
+    return g.astype(np.float32)
+
+
+def circle_gates(n_gates=4, radius=5.0, z=1.5, width=1.5):
+    """configs[0]: square gates on a circle, normals tangent (counter-clockwise travel)."""
+    a = 2.0 * np.pi * np.arange(n_gates) / n_gates
+    c = np.stack([radius * np.cos(a), radius * np.sin(a), np.full(n_gates, z)], axis=1)
+    n = np.stack([-np.sin(a), np.cos(a), np.zeros(n_gates)], axis=1)
+    return _gate_rows(c, n, width / 2, width / 2)
+
+
+def lemniscate_gates(n_gates=7, a=12.0, width=1.5, height_seed=1):
+    """configs[1]: gates on a Bernoulli lemniscate at t_i = 2 pi i / n, normal = unit tangent,
+    heights uniform in [1,3] m from numpy default_rng(height_seed)  [R-16]."""
+    t = 2.0 * np.pi * np.arange(n_gates) / n_gates
+    den = 1.0 + np.sin(t) ** 2
+    x = a * np.cos(t) / den
+    y = a * np.sin(t) * np.cos(t) / den
+    dden = 2.0 * np.sin(t) * np.cos(t)
+    dx = a * (-np.sin(t) * den - np.cos(t) * dden) / den ** 2
+    dy = a * ((np.cos(t) ** 2 - np.sin(t) ** 2) * den - np.sin(t) * np.cos(t) * dden) / den ** 2
+    z = np.random.default_rng(height_seed).uniform(1.0, 3.0, n_gates)
+    c = np.stack([x, y, z], axis=1)
+    n = np.stack([dx, dy, np.zeros(n_gates)], axis=1)
+    return _gate_rows(c, n, width / 2, width / 2)
+
+
+def lissajous_reference(n_rows, dt, g=9.81):
+    """configs[2]: p(t) = (10 sin .6t, 6 sin 1.2t, 2 + .5 sin .3t); v, a, jerk in closed form;
+    attitude from differential flatness with yaw 0; body rates from the jerk (yaw rate 0)."""
+    t = np.arange(n_rows) * float(dt)
+    A = np.array([10.0, 6.0, 0.5]); W = np.array([0.6, 1.2, 0.3]); off = np.array([0.0, 0.0, 2.0])
+    p = A * np.sin(np.outer(t, W)) + off
+    v = A * W * np.cos(np.outer(t, W))
+    acc = -A * W ** 2 * np.sin(np.outer(t, W))
+    jerk = -A * W ** 3 * np.cos(np.outer(t, W))
+    rows = np.zeros((n_rows, 13))
+    for i in range(n_rows):
+        f = acc[i] + np.array([0.0, 0.0, g])
+        fn = np.linalg.norm(f)
+        zb = f / fn
+        xc = np.array([1.0, 0.0, 0.0])
+        yb = np.cross(zb, xc); yb /= np.linalg.norm(yb)
+        xb = np.cross(yb, zb)
+        Rm = np.stack([xb, yb, zb], axis=1)
+        q = _rot_to_quat(Rm)
+        hw = (jerk[i] - np.dot(zb, jerk[i]) * zb) / fn
+        om = np.array([-np.dot(hw, yb), np.dot(hw, xb), 0.0])
+        rows[i] = np.concatenate([p[i], q, v[i], om])
+    return rows.astype(np.float32)
+
+
+def _rot_to_quat(R):
+    tr = np.trace(R)
+    if tr > 0:
+        s = np.sqrt(tr + 1.0) * 2
+        q = np.array([0.25 * s, (R[2, 1] - R[1, 2]) / s, (R[0, 2] - R[2, 0]) / s,
+                      (R[1, 0] - R[0, 1]) / s])
+    else:
+        i = int(np.argmax(np.diag(R)))
+        j, k = (i + 1) % 3, (i + 2) % 3
+        s = np.sqrt(1.0 + R[i, i] - R[j, j] - R[k, k]) * 2
+        q = np.zeros(4)
+        q[0] = (R[k, j] - R[j, k]) / s
+        q[1 + i] = 0.25 * s
+        q[1 + j] = (R[j, i] + R[i, j]) / s
+        q[1 + k] = (R[k, i] + R[i, k]) / s
+    q = q / np.linalg.norm(q)
+    return q if q[0] >= 0 else -q
+
+
+def spline_path(centres, n_points=500, dense=20001):
+    """configs[3]: periodic cubic spline through the gate centres, resampled to n_points
+    uniformly spaced in arc length (the end point is not repeated)  [R-13]."""
+    from scipy.interpolate import CubicSpline
+    c = np.asarray(centres, dtype=np.float64)
+    pts = np.concatenate([c, c[:1]], axis=0)
+    chord = np.concatenate([[0.0], np.cumsum(np.linalg.norm(np.diff(pts, axis=0), axis=1))])
+    cs = CubicSpline(chord, pts, bc_type="periodic")
+    u = np.linspace(0.0, chord[-1], dense)
+    d = cs(u)
+    s = np.concatenate([[0.0], np.cumsum(np.linalg.norm(np.diff(d, axis=0), axis=1))])
+    target = np.arange(n_points) * (s[-1] / n_points)
+    uu = np.interp(target, s, u)
+    return cs(uu).astype(np.float32)
+
+
+# ---- the five configs ----------------------------------------------------------------------
+
+def _level_state(p, v=(0, 0, 0)):
+    x = np.zeros(13)
+    x[0:3] = p; x[3] = 1.0; x[7:10] = v
+    return x
+
+
+def _hover_nominal(p, B, N):
+    return np.full((B, N, 4), hover_thrust(p), dtype=np.float32)
+
+
+def cfg0(K=256, N=20) -> Workload:
+    """Tiny gate-progress MPPI (BASELINE.json configs[0])."""
+    p = base_params(K=K, N=N, B=1, objective=OBJ_GATE, sigma=1.0)
+    p["lambda"] = _f32(1.0)
+    x0 = _level_state((5.0, -2.0, 1.5))[None].astype(np.float32)
+    return Workload("cfg0_gate_tiny", p, x0, np.zeros(1, np.int32), _hover_nominal(p, 1, N),
+                    gates=circle_gates(), seed=0, iters=1)
+
+
+def cfg1(K=4096, N=50, iters=10) -> Workload:
+    """Gate progress at real-time scale, 10 warm-started iterations (configs[1])."""
+    p = base_params(K=K, N=N, B=1, objective=OBJ_GATE, sigma=1.5)
+    p["lambda"] = _f32(0.5)
+    gates = lemniscate_gates()
+    c0 = gates[0, 0:3].astype(np.float64); n0 = gates[0, 3:6].astype(np.float64)
+    x0 = _level_state(c0 - 3.0 * n0, 3.0 * n0)[None].astype(np.float32)
+    return Workload("cfg1_gate_K4096_N50", p, x0, np.zeros(1, np.int32), _hover_nominal(p, 1, N),
+                    gates=gates, seed=0, iters=iters)
+
+
+def cfg2(K=4096, N=50, extra_rows=0) -> Workload:
+    """Trajectory tracking on a Lissajous reference (configs[2]); x0 = ref[0]  [R-15]."""
+    p = base_params(K=K, N=N, B=1, objective=OBJ_TRACK, sigma=1.5)
+    p["lambda"] = _f32(0.5)
+    ref = lissajous_reference(N + 1 + extra_rows, p["dt"], p["g"])
+    x0 = ref[0:1].copy()
+    return Workload("cfg2_track_K4096_N50", p, x0, np.zeros(1, np.int32), _hover_nominal(p, 1, N),
+                    ref=ref, seed=0, iters=1)
+
+
+def cfg3(K=8192, N=50) -> Workload:
+    """Contouring on a 500-point spline path through the circle-track gate centres (configs[3])."""
+    p = base_params(K=K, N=N, B=1, objective=OBJ_CONTOUR, sigma=1.5)
+    p["lambda"] = _f32(0.5)
+    path = spline_path(circle_gates()[:, 0:3], 500)
+    x0 = _level_state((5.0, -2.0, 1.5))[None].astype(np.float32)
+    return Workload("cfg3_contour_K8192_N50", p, x0, np.full(1, -1, np.int32),
+                    _hover_nominal(p, 1, N), path=path, closed=True, seed=0, iters=1)
+
+
+def cfg4(K=4096, N=50, B=64, steps=500) -> Workload:
+    """Batched closed loop: B jittered drones on the circle track (configs[4])."""
+    p = base_params(K=K, N=N, B=B, objective=OBJ_GATE, sigma=1.5)
+    p["lambda"] = _f32(0.5)
+    rng = np.random.default_rng(7)
+    x0 = np.tile(_level_state((5.0, -2.0, 1.5)), (B, 1))
+    x0[:, 0:3] += rng.uniform(-0.5, 0.5, (B, 3))
+    x0[:, 7:10] += rng.uniform(-1.0, 1.0, (B, 3))
+    return Workload(f"cfg4_gate_closed_loop_B{B}", p, x0.astype(np.float32),
+                    np.zeros(B, np.int32), _hover_nominal(p, B, N), gates=circle_gates(), seed=0,
+                    iters=steps)
+
+
+def stress_gate(K=1024, N=30) -> Workload:
+    """Crossing-heavy case: 3 m before gate 0 at 6 m/s, offset towards a corner
+    of the opening, sigma 1.5, so that about two thirds of the samples pass and one third miss:
+    the pass / miss / switch branches are all exercised at scale."""
+    p = base_params(K=K, N=N, B=1, objective=OBJ_GATE, sigma=1.5)
+    p["lambda"] = _f32(0.5)
+    gates = circle_gates()
+    c0 = gates[0, 0:3].astype(np.float64); n0 = gates[0, 3:6].astype(np.float64)
+    h0 = gates[0, 6:9].astype(np.float64)
+    x0 = _level_state(c0 - 3.0 * n0 + 0.55 * h0 + np.array([0, 0, 0.5]), 6.0 * n0)
+    return Workload("stress_gate_crossings", p, x0[None].astype(np.float32),
+                    np.zeros(1, np.int32), _hover_nominal(p, 1, N), gates=gates, seed=3, iters=1)
+
+
+ALL = {"cfg0": cfg0, "cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg4": cfg4,
+       "stress_gate": stress_gate}
