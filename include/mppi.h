@@ -1,0 +1,209 @@
+/*
+ * mppi.h -- C ABI of libmppi: one MPPI iteration of the reference-free racing controller of
+ * arXiv 2509.14726 as hand-written sm_100a CUDA kernels.
+ *
+ * What one call computes (BASELINE.json:north_star; Alg. 1), for each of B
+ * independent controllers:
+ *   1. K perturbed rotor-thrust sequences U^k = clamp(U* + dU^k), dU ~ N(0, sigma^2 I), drawn in
+ *      the kernel from Philox4x32-10 with counter (sample k, step t, iter, controller b) and key
+ *      = seed                                                     (eq.(3))
+ *   2. each rolled out through RK4 quadrotor rigid-body dynamics over N steps of dt
+ *                                                                  (eq.(2))
+ *   3. each scored under one objective: gate progress with gate-plane crossing and target
+ *      switching (eq.(6)), full-state tracking (eq.(8)) or
+ *      contouring against an arc-length path (eq.(9))
+ *   4. weights w_k = softmax(-J_k / lambda) and U*_new = sum_k w_k U^k
+ *                                                     (eq.(4),(5))
+ * The exact readings of every point the paper leaves open are listed in DESIGN.md (R-1..R-22).
+ *
+ * Conventions
+ *   - Notation follows BASELINE.json: K samples, N horizon steps, B controllers (the paper
+ *     writes M samples, K steps).
+ *   - State x[13] = p(3), q(w,x,y,z) body->world, v(3) world, omega(3) body.  World z is up,
+ *     gravity (0,0,-g).  Inputs are the four rotor thrusts in newtons.
+ *   - All floating-point data is fp32, row-major, densely packed.  "device" pointers are CUDA
+ *     device memory owned by the caller (e.g. torch tensors); "host" pointers are ordinary host
+ *     memory, copied during the call.  The library never frees or keeps a caller pointer beyond
+ *     the call (mppi_step keeps them only until the work it enqueued has run).
+ *   - Every entry point returns MPPI_OK (0) or a negative mppi_status.  Nothing throws, aborts
+ *     or prints.  NaN/Inf in device inputs are not detected; they propagate to the outputs.
+ *   - A context is not thread-safe; distinct contexts are independent.  All device work is
+ *     enqueued on the cudaStream_t passed in (NULL = the legacy default stream) and is
+ *     asynchronous with respect to the host unless stated otherwise.
+ *   - There is no CPU fallback: without a CUDA device mppi_create fails with MPPI_E_CUDA.
+ */
+#ifndef MPPI_H_
+#define MPPI_H_
+
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define MPPI_API __attribute__((visibility("default")))
+#else
+#define MPPI_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mppi_ctx mppi_ctx; /* opaque, owned by the library */
+
+typedef enum {
+    MPPI_OBJ_GATE = 0,    /* J_gate,    eq.(6) PAPER.md:105-112 (BASELINE.json configs[0,1,4]) */
+    MPPI_OBJ_TRACK = 1,   /* J_track,   eq.(8) PAPER.md:139-147 (configs[2])                   */
+    MPPI_OBJ_CONTOUR = 2  /* J_contour, eq.(9) PAPER.md:149-161 (configs[3])                   */
+} mppi_objective;
+
+typedef enum {
+    MPPI_OK = 0,
+    MPPI_E_NULL = -1,     /* a required pointer is NULL                                        */
+    MPPI_E_PARAM = -2,    /* a parameter is out of range (see mppi_params)                     */
+    MPPI_E_NO_TRACK = -3, /* mppi_step before the mppi_set_* call the objective needs          */
+    MPPI_E_TRACK = -4,    /* track data rejected (see mppi_set_*)                              */
+    MPPI_E_RANGE = -5,    /* buffers overlap partially, or a count is out of range             */
+    MPPI_E_CUDA = -6,     /* a CUDA call failed; text from mppi_last_error                     */
+    MPPI_E_ALLOC = -7     /* host or device allocation failed                                  */
+} mppi_status;
+
+typedef enum {
+    MPPI_PIPE_FUSED = 0,   /* one kernel per iteration: rollout + cost + block-local softmax
+                              partials + last-block combine; the perturbations never leave the SM
+                              (they are re-derived from the counter-based stream where needed)  */
+    MPPI_PIPE_TWO_PASS = 1 /* rollout kernel stores dU [B][N][K][4] to HBM, a second fused
+                              min / exp-weight / weighted-sum kernel reads it back              */
+} mppi_pipeline;
+
+/* Parameters of Alg. 1 (samples, horizon, lambda, Sigma) plus the model and cost
+ * constants of BASELINE.json configs[0..3].  struct_size = sizeof(mppi_params) versions the ABI. */
+typedef struct {
+    uint32_t struct_size;
+    int32_t K;         /* samples per controller; > 0 and a multiple of 32                       */
+    int32_t N;         /* horizon steps; 1..MPPI_MAX_N                                           */
+    int32_t B;         /* independent controllers; >= 1                                          */
+    int32_t objective; /* mppi_objective                                                         */
+    float dt;          /* s, > 0                                                                 */
+    float lambda;      /* temperature of eq.(4), cost units, > 0                                 */
+    float sigma;       /* per-rotor noise std, N, >= 0 (Sigma = sigma^2 I, eq.(3))               */
+    float mass, Jx, Jy, Jz; /* kg, kg m^2 (diagonal inertia), all > 0                            */
+    float arm;         /* m; lever of PAPER.md:70 is arm / sqrt(2)                               */
+    float c_tau;       /* m; rotor torque coefficient of PAPER.md:70                             */
+    float g;           /* m/s^2                                                                  */
+    float T_min, T_max;/* per-rotor hard clamp, N, T_min <= T_max                                */
+    float w_omega;     /* body-rate weight of the gate and contouring objectives                 */
+    float gate_miss_penalty; /* added on a plane crossing outside the opening                    */
+    float gate_pass_bonus;   /* subtracted on a valid pass                                       */
+    float Qp, Qv, Qq, Qw, R; /* tracking weights of eq.(8); R acts on (T - m g / 4)              */
+    float q_contour, q_lag, mu_progress; /* contouring weights of eq.(9)                         */
+    int32_t window;    /* contouring nearest-vertex search half-width in points, 1..64           */
+    int32_t pipeline;  /* mppi_pipeline                                                          */
+    int32_t use_graph; /* 1: replay each step as a CUDA graph; 0: plain stream launches          */
+    int32_t block_threads; /* threads per block of the rollout kernel: 0 = auto, else 32..256,
+                              a multiple of 32 that divides K                                    */
+    int32_t fast_math; /* 0: IEEE-accurate logf/sincospif/sqrtf/expf; 1: MUFU approximations for
+                          the Box-Muller transform (error budget)                 */
+    int32_t store_noise; /* 1: also keep dU of the last step for mppi_debug_noise (always kept
+                            in the TWO_PASS pipeline)                                            */
+} mppi_params;
+
+#define MPPI_MAX_N 256
+#define MPPI_MAX_GATES 64
+#define MPPI_MAX_PATH 2048
+#define MPPI_MAX_WINDOW 64
+
+/* Fills *p with struct_size and the constants of BASELINE.json configs[0] (K=256, N=20, B=1). */
+MPPI_API int mppi_default_params(mppi_params* p);
+
+/* Validates *p (MPPI_E_PARAM names the first offender through mppi_last_error(NULL)), creates the
+ * context on the current CUDA device and allocates its device scratch.  No kernel is launched. */
+MPPI_API int mppi_create(const mppi_params* p, mppi_ctx** out);
+MPPI_API int mppi_destroy(mppi_ctx* ctx); /* synchronises the device, frees everything; NULL is accepted */
+
+/* Waypoints W of Alg. 1.  host_gates [G][11]: centre c(3), unit normal n(3) = the
+ * direction of travel, unit in-plane axis h(3) with n.h = 0, half-width along h, half-height
+ * along v = h x n.  1 <= G <= MPPI_MAX_GATES.  MPPI_E_TRACK if |n|,|h| differ from 1 or n.h from
+ * 0 by more than 1e-4, or a half-size is <= 0.  Synchronous host->device copy. */
+MPPI_API int mppi_set_gates(mppi_ctx* ctx, const float* host_gates, int G);
+
+/* Reference trajectory tau_ref of Alg. 1.  host_ref [M][13], one full state per dt.  M >= N+1. */
+MPPI_API int mppi_set_reference(mppi_ctx* ctx, const float* host_ref, int M);
+
+/* Arc-length path P_arc of Alg. 1.  host_pts [P][3]; arc length s_i is the
+ * cumulative chord length, the tangent at i is the normalised central difference (periodic when
+ * closed != 0, one-sided at the ends otherwise)  [R-22].  2*window+1 <= P <= MPPI_MAX_PATH. */
+MPPI_API int mppi_set_path(mppi_ctx* ctx, const float* host_pts, int P, int closed);
+
+/* One MPPI iteration (Alg. 1 lines 3-17) for all B controllers, enqueued on cuda_stream.
+ *   d_x0      [B][13] device, in
+ *   d_start   [B]     device, in: gate objective: index of the current target gate (wrapped
+ *                     mod G); tracking: reference row t0 of the current time (clamped so that
+ *                     t0+N <= M-1); contouring: path index hint for the windowed search, or -1
+ *                     for a global nearest-vertex search
+ *   d_u_nom   [B][N][4] device, in: nominal thrust sequence U*
+ *   seed, iter  Philox key and counter word 2
+ *   d_u_new   [B][N][4] device, out; may equal d_u_nom exactly (in-place warm start); a partial
+ *                     overlap is rejected with MPPI_E_RANGE
+ *   d_cost    [B][K] device, out: trajectory costs J_k
+ *   d_weights [B][K] device, out: w_k of eq.(4), summing to 1 per controller
+ * Outputs are valid once the stream has reached the end of the enqueued work. */
+MPPI_API int mppi_step(mppi_ctx* ctx, const float* d_x0, const int32_t* d_start, const float* d_u_nom,
+              uint64_t seed, uint32_t iter, float* d_u_new, float* d_cost, float* d_weights,
+              void* cuda_stream);
+
+/* n_iters warm-started iterations at a fixed x0 (BASELINE.json configs[1]; [R-14]: no shift):
+ * iteration i uses counter word iter0+i and the nominal left by iteration i-1.  d_u [B][N][4] is
+ * updated in place; d_cost / d_weights hold the last iteration's values.  With use_graph the
+ * whole chain is one graph launch. */
+MPPI_API int mppi_optimize(mppi_ctx* ctx, const float* d_x0, const int32_t* d_start, float* d_u,
+                  uint64_t seed, uint32_t iter0, int n_iters, float* d_cost, float* d_weights,
+                  void* cuda_stream);
+
+/* Same as mppi_step with HOST buffers: copies x0, start, u_nom to the device, runs the
+ * iteration, copies u_new (and cost / weights when non-NULL) back and synchronises the stream.
+ * This is the end-to-end call a host-side control loop makes every cycle. */
+MPPI_API int mppi_step_host(mppi_ctx* ctx, const float* h_x0, const int32_t* h_start, const float* h_u_nom,
+                   uint64_t seed, uint32_t iter, float* h_u_new, float* h_cost, float* h_weights,
+                   void* cuda_stream);
+
+/* Closed-loop glue of BASELINE.json configs[4] (receding horizon): the plant
+ * (the same RK4 model) applies u_new[b][0] to d_x in place; d_start advances (gate: on a valid
+ * pass of the plant segment through the current gate; tracking: +1 row; contouring: windowed
+ * nearest vertex); d_u_nom_next[b][t] = d_u_new[b][min(t+1, N-1)].  d_u_nom_next may equal
+ * d_u_new. */
+MPPI_API int mppi_sim_step(mppi_ctx* ctx, float* d_x, int32_t* d_start, const float* d_u_new,
+                  float* d_u_nom_next, void* cuda_stream);
+
+/* Device pointer to dU [B][N][K][4] of the last step (parity debugging); NULL unless the
+ * context keeps it (TWO_PASS pipeline or store_noise). */
+MPPI_API const float* mppi_debug_noise(mppi_ctx* ctx);
+
+/* Static facts about the compiled kernels and the launch configuration of this context. */
+typedef struct {
+    uint32_t struct_size;
+    int32_t block_threads, grid_blocks, blocks_per_controller;
+    int32_t regs_per_thread, static_smem_bytes, dynamic_smem_bytes, local_bytes_per_thread;
+    int32_t max_blocks_per_sm, sm_count;
+    int32_t kernels_per_step; /* launches one mppi_step enqueues */
+    int32_t l2_bytes;
+    int64_t scratch_bytes;    /* device memory the context owns */
+} mppi_info;
+MPPI_API int mppi_get_info(mppi_ctx* ctx, mppi_info* out);
+
+/* Number of kernel launches this context has enqueued since creation. */
+MPPI_API int64_t mppi_launch_count(mppi_ctx* ctx);
+
+MPPI_API const char* mppi_error_string(int status);    /* static text for a status code              */
+MPPI_API const char* mppi_last_error(mppi_ctx* ctx);   /* detail of the last failure (NULL: of the last
+                                                 failed mppi_create / mppi_default_params)  */
+
+/* Roofline denominators measured on the device in use (bench.py).
+ * mppi_measure_fma_peak: dependent-chain-free FFMA loop on every SM; writes achieved TFLOP/s.
+ * mppi_measure_copy_bw:  device-to-device copy of `bytes`; writes read+write GB/s.
+ * Both synchronise and return the best of `reps` timings by CUDA events. */
+MPPI_API int mppi_measure_fma_peak(int reps, double* tflops, double* sm_clock_mhz);
+MPPI_API int mppi_measure_copy_bw(int64_t bytes, int reps, double* gbs);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MPPI_H_ */

@@ -1,0 +1,536 @@
+// mppi_api.cu -- host side of libmppi: the C ABI declared in include/mppi.h.
+// Parameter validation, track packing, scratch allocation, stream launches and CUDA-graph replay.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/mppi.h"
+#include "mppi_cost.cuh"
+#include "mppi_internal.h"
+
+using namespace mppi;
+
+struct GraphSlot {
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    std::vector<cudaGraphNode_t> rollout_nodes, reduce_nodes;
+    int n_iters = 0;
+};
+
+struct mppi_ctx {
+    mppi_params prm;
+    DevParams dp;
+    LaunchCfg cfg;
+    int device = 0, sm_count = 0, l2_bytes = 0;
+    bool have_gates = false, have_ref = false, have_path = false;
+    float4* d_gates = nullptr;
+    float4* d_ref = nullptr;
+    float4* d_path = nullptr;
+    float4* d_du = nullptr;
+    float* d_partials = nullptr;
+    unsigned* d_counters = nullptr;
+    // device staging for mppi_step_host
+    float* d_hx0 = nullptr; int* d_hstart = nullptr; float* d_hu = nullptr; float* d_hcost = nullptr;
+    float* d_hw = nullptr;
+    int64_t scratch_bytes = 0;
+    int64_t launches = 0;
+    GraphSlot g_step, g_opt;
+    std::string err;
+};
+
+static thread_local std::string g_create_err;
+
+static int fail(mppi_ctx* c, int code, const std::string& msg)
+{
+    if (c) c->err = msg; else g_create_err = msg;
+    return code;
+}
+static int cuda_fail(mppi_ctx* c, cudaError_t e, const char* what)
+{
+    return fail(c, MPPI_E_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CK(ctx, call)                                              \
+    do {                                                           \
+        cudaError_t e_ = (call);                                   \
+        if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);   \
+    } while (0)
+
+extern "C" const char* mppi_error_string(int s)
+{
+    switch (s) {
+        case MPPI_OK: return "ok";
+        case MPPI_E_NULL: return "null pointer";
+        case MPPI_E_PARAM: return "parameter out of range";
+        case MPPI_E_NO_TRACK: return "track data for this objective not set";
+        case MPPI_E_TRACK: return "track data rejected";
+        case MPPI_E_RANGE: return "buffer overlap or count out of range";
+        case MPPI_E_CUDA: return "CUDA error";
+        case MPPI_E_ALLOC: return "allocation failed";
+        default: return "unknown status";
+    }
+}
+
+extern "C" const char* mppi_last_error(mppi_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
+
+extern "C" int mppi_default_params(mppi_params* p)
+{
+    if (!p) return fail(nullptr, MPPI_E_NULL, "mppi_default_params: p is NULL");
+    std::memset(p, 0, sizeof *p);
+    p->struct_size = sizeof *p;
+    p->K = 256; p->N = 20; p->B = 1; p->objective = MPPI_OBJ_GATE;
+    p->dt = 0.02f; p->lambda = 1.0f; p->sigma = 1.0f;
+    p->mass = 0.85f; p->Jx = 1e-3f; p->Jy = 1e-3f; p->Jz = 1.7e-3f;
+    p->arm = 0.15f; p->c_tau = 0.016f; p->g = 9.81f;
+    p->T_min = 0.0f; p->T_max = 7.0f;
+    p->w_omega = 0.01f; p->gate_miss_penalty = 10.0f; p->gate_pass_bonus = 5.0f;
+    p->Qp = 100.0f; p->Qv = 1.0f; p->Qq = 10.0f; p->Qw = 0.1f; p->R = 0.01f;
+    p->q_contour = 200.0f; p->q_lag = 50.0f; p->mu_progress = 2.0f;
+    p->window = 16;
+    p->pipeline = MPPI_PIPE_FUSED; p->use_graph = 0; p->block_threads = 0; p->fast_math = 0;
+    p->store_noise = 0;
+    return MPPI_OK;
+}
+
+static bool finite_pos(float v) { return std::isfinite(v) && v > 0.0f; }
+
+static int validate(const mppi_params* p)
+{
+#define BAD(cond, msg) if (cond) return fail(nullptr, MPPI_E_PARAM, msg)
+    BAD(p->struct_size != sizeof(mppi_params), "struct_size does not match this library");
+    BAD(p->K <= 0 || p->K % 32 != 0, "K must be a positive multiple of 32");
+    BAD(p->N <= 0 || p->N > MPPI_MAX_N, "N must be in 1..MPPI_MAX_N");
+    BAD(p->B <= 0 || p->B > 65535, "B must be in 1..65535");
+    BAD(p->objective < 0 || p->objective > 2, "objective must be 0, 1 or 2");
+    BAD(!finite_pos(p->dt), "dt must be > 0");
+    BAD(!finite_pos(p->lambda), "lambda must be > 0");
+    BAD(!(std::isfinite(p->sigma) && p->sigma >= 0.0f), "sigma must be >= 0");
+    BAD(!finite_pos(p->mass) || !finite_pos(p->Jx) || !finite_pos(p->Jy) || !finite_pos(p->Jz),
+        "mass and inertia must be > 0");
+    BAD(!std::isfinite(p->arm) || !std::isfinite(p->c_tau) || !std::isfinite(p->g), "arm, c_tau, g must be finite");
+    BAD(!(std::isfinite(p->T_min) && std::isfinite(p->T_max) && p->T_min <= p->T_max), "need T_min <= T_max");
+    BAD(p->window < 1 || p->window > MPPI_MAX_WINDOW, "window must be in 1..MPPI_MAX_WINDOW");
+    BAD(p->pipeline != MPPI_PIPE_FUSED && p->pipeline != MPPI_PIPE_TWO_PASS, "unknown pipeline");
+    BAD(p->block_threads != 0 && (p->block_threads < 32 || p->block_threads > 256 || p->block_threads % 32 != 0 ||
+                                  p->K % p->block_threads != 0),
+        "block_threads must be 0 or a multiple of 32 in 32..256 that divides K");
+    BAD((int64_t)p->K / 32 > 65535, "K too large");
+#undef BAD
+    return MPPI_OK;
+}
+
+static int pick_block(const mppi_params* p, int sm_count)
+{
+    if (p->block_threads) return p->block_threads;
+    // Enough resident work to fill the chip -> 128-thread blocks (4 warps, one per scheduler);
+    // a lone controller is latency-bound: still 128 so that only K/128 partials meet in the
+    // last-block combine, unless K is too small to divide.
+    for (int tpb : {128, 64, 32})
+        if (p->K % tpb == 0) return tpb;
+    (void)sm_count;
+    return 32;
+}
+
+static void free_graph(GraphSlot& g)
+{
+    if (g.exec) cudaGraphExecDestroy(g.exec);
+    if (g.graph) cudaGraphDestroy(g.graph);
+    g = GraphSlot();
+}
+
+extern "C" int mppi_destroy(mppi_ctx* c)
+{
+    if (!c) return MPPI_OK;
+    cudaDeviceSynchronize();
+    free_graph(c->g_step); free_graph(c->g_opt);
+    cudaFree(c->d_gates); cudaFree(c->d_ref); cudaFree(c->d_path); cudaFree(c->d_du);
+    cudaFree(c->d_partials); cudaFree(c->d_counters);
+    cudaFree(c->d_hx0); cudaFree(c->d_hstart); cudaFree(c->d_hu); cudaFree(c->d_hcost); cudaFree(c->d_hw);
+    delete c;
+    return MPPI_OK;
+}
+
+template <typename T>
+static cudaError_t dev_alloc(mppi_ctx* c, T** p, size_t n)
+{
+    cudaError_t e = cudaMalloc(reinterpret_cast<void**>(p), n * sizeof(T));
+    if (e == cudaSuccess) c->scratch_bytes += (int64_t)(n * sizeof(T));
+    return e;
+}
+
+extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
+{
+    if (!p || !out) return fail(nullptr, MPPI_E_NULL, "mppi_create: NULL argument");
+    *out = nullptr;
+    int rc = validate(p);
+    if (rc != MPPI_OK) return rc;
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0)
+        return fail(nullptr, MPPI_E_CUDA, std::string("no CUDA device: ") + cudaGetErrorString(e));
+    mppi_ctx* c = new (std::nothrow) mppi_ctx();
+    if (!c) return fail(nullptr, MPPI_E_ALLOC, "host allocation failed");
+    c->prm = *p;
+    cudaGetDevice(&c->device);
+    cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device);
+    cudaDeviceGetAttribute(&c->l2_bytes, cudaDevAttrL2CacheSize, c->device);
+
+    // derived constants: computed in double from the fp32 parameters, rounded once
+    DevParams& d = c->dp;
+    std::memset(&d, 0, sizeof d);
+    d.K = p->K; d.N = p->N; d.B = p->B; d.window = p->window;
+    d.dt = p->dt; d.inv_lambda = (float)(1.0 / (double)p->lambda); d.sigma = p->sigma;
+    d.T_min = p->T_min; d.T_max = p->T_max;
+    d.inv_mass = (float)(1.0 / (double)p->mass); d.g = p->g;
+    d.hover = (float)((double)p->mass * (double)p->g / 4.0);
+    const double lever = (double)p->arm / std::sqrt(2.0);
+    d.ltx = (float)(lever / p->Jx); d.lty = (float)(lever / p->Jy); d.ltz = (float)((double)p->c_tau / p->Jz);
+    d.gyx = (float)(((double)p->Jy - p->Jz) / p->Jx);
+    d.gyy = (float)(((double)p->Jz - p->Jx) / p->Jy);
+    d.gyz = (float)(((double)p->Jx - p->Jy) / p->Jz);
+    d.w_omega = p->w_omega; d.miss = p->gate_miss_penalty; d.bonus = p->gate_pass_bonus;
+    d.Qp = p->Qp; d.Qv = p->Qv; d.Qq = p->Qq; d.Qw = p->Qw; d.R = p->R;
+    d.q_c = p->q_contour; d.q_l = p->q_lag; d.mu = p->mu_progress;
+
+    LaunchCfg& cfg = c->cfg;
+    cfg.objective = p->objective; cfg.fast_math = p->fast_math ? 1 : 0;
+    cfg.fused = p->pipeline == MPPI_PIPE_FUSED;
+    cfg.store_du = (!cfg.fused || p->store_noise) ? 1 : 0;
+    cfg.block_threads = pick_block(p, c->sm_count);
+    d.blocks_per_ctrl = p->K / cfg.block_threads;
+    cfg.smem_bytes = 0;   // fixed once the track is known
+
+    const size_t BN4 = (size_t)p->B * p->N * 4, BK = (size_t)p->B * p->K;
+#define CKC(call)                                                        \
+    do {                                                                 \
+        cudaError_t e2_ = (call);                                        \
+        if (e2_ != cudaSuccess) {                                        \
+            int r_ = cuda_fail(nullptr, e2_, #call);                     \
+            mppi_destroy(c);                                             \
+            return r_;                                                   \
+        }                                                                \
+    } while (0)
+    if (cfg.store_du) CKC(dev_alloc(c, &c->d_du, (size_t)p->B * p->N * p->K));
+    if (cfg.fused) {
+        CKC(dev_alloc(c, &c->d_partials, (size_t)p->B * d.blocks_per_ctrl * (4 * p->N + 4)));
+        CKC(dev_alloc(c, &c->d_counters, (size_t)p->B));
+        CKC(cudaMemset(c->d_counters, 0, (size_t)p->B * sizeof(unsigned)));
+    }
+    CKC(dev_alloc(c, &c->d_hx0, (size_t)p->B * 13));
+    CKC(dev_alloc(c, &c->d_hstart, (size_t)p->B));
+    CKC(dev_alloc(c, &c->d_hu, BN4));
+    CKC(dev_alloc(c, &c->d_hcost, BK));
+    CKC(dev_alloc(c, &c->d_hw, BK));
+#undef CKC
+    *out = c;
+    return MPPI_OK;
+}
+
+// ---- tracks -------------------------------------------------------------------------------------
+
+static int upload_f4(mppi_ctx* c, float4** dst, const std::vector<float4>& v)
+{
+    if (*dst) { cudaDeviceSynchronize(); cudaFree(*dst); *dst = nullptr; }
+    CK(c, dev_alloc(c, dst, v.size()));
+    CK(c, cudaMemcpy(*dst, v.data(), v.size() * sizeof(float4), cudaMemcpyHostToDevice));
+    free_graph(c->g_step); free_graph(c->g_opt);   // shared-memory size may have changed
+    return MPPI_OK;
+}
+
+extern "C" int mppi_set_gates(mppi_ctx* c, const float* g, int G)
+{
+    if (!c || !g) return fail(c, MPPI_E_NULL, "mppi_set_gates: NULL argument");
+    if (G < 1 || G > MPPI_MAX_GATES) return fail(c, MPPI_E_TRACK, "G must be in 1..MPPI_MAX_GATES");
+    std::vector<float4> v(4 * (size_t)G);
+    for (int i = 0; i < G; ++i) {
+        const float* r = g + 11 * i;
+        for (int j = 0; j < 11; ++j)
+            if (!std::isfinite(r[j])) return fail(c, MPPI_E_TRACK, "gate entry is not finite");
+        const double n[3] = {r[3], r[4], r[5]}, h[3] = {r[6], r[7], r[8]};
+        const double nn = std::sqrt(n[0] * n[0] + n[1] * n[1] + n[2] * n[2]);
+        const double hh = std::sqrt(h[0] * h[0] + h[1] * h[1] + h[2] * h[2]);
+        const double nh = n[0] * h[0] + n[1] * h[1] + n[2] * h[2];
+        if (std::fabs(nn - 1.0) > 1e-4 || std::fabs(hh - 1.0) > 1e-4 || std::fabs(nh) > 1e-4)
+            return fail(c, MPPI_E_TRACK, "gate normal / in-plane axis must be unit and orthogonal (1e-4)");
+        if (!(r[9] > 0.0f) || !(r[10] > 0.0f)) return fail(c, MPPI_E_TRACK, "gate half-sizes must be > 0");
+        const double vx = h[1] * n[2] - h[2] * n[1], vy = h[2] * n[0] - h[0] * n[2], vz = h[0] * n[1] - h[1] * n[0];
+        v[4 * i + 0] = make_float4(r[0], r[1], r[2], r[9]);
+        v[4 * i + 1] = make_float4(r[3], r[4], r[5], r[10]);
+        v[4 * i + 2] = make_float4(r[6], r[7], r[8], 0.0f);
+        v[4 * i + 3] = make_float4((float)vx, (float)vy, (float)vz, 0.0f);
+    }
+    int rc = upload_f4(c, &c->d_gates, v);
+    if (rc) return rc;
+    c->dp.G = G; c->dp.gates = c->d_gates; c->have_gates = true;
+    return MPPI_OK;
+}
+
+extern "C" int mppi_set_reference(mppi_ctx* c, const float* ref, int M)
+{
+    if (!c || !ref) return fail(c, MPPI_E_NULL, "mppi_set_reference: NULL argument");
+    if (M < c->prm.N + 1) return fail(c, MPPI_E_TRACK, "reference needs at least N+1 rows");
+    std::vector<float4> v(4 * (size_t)M);
+    for (int i = 0; i < M; ++i) {
+        const float* r = ref + 13 * i;
+        for (int j = 0; j < 13; ++j)
+            if (!std::isfinite(r[j])) return fail(c, MPPI_E_TRACK, "reference entry is not finite");
+        v[4 * i + 0] = make_float4(r[0], r[1], r[2], r[3]);
+        v[4 * i + 1] = make_float4(r[4], r[5], r[6], r[7]);
+        v[4 * i + 2] = make_float4(r[8], r[9], r[10], r[11]);
+        v[4 * i + 3] = make_float4(r[12], 0.0f, 0.0f, 0.0f);
+    }
+    int rc = upload_f4(c, &c->d_ref, v);
+    if (rc) return rc;
+    c->dp.M = M; c->dp.ref = c->d_ref; c->have_ref = true;
+    return MPPI_OK;
+}
+
+extern "C" int mppi_set_path(mppi_ctx* c, const float* pts, int P, int closed)
+{
+    if (!c || !pts) return fail(c, MPPI_E_NULL, "mppi_set_path: NULL argument");
+    if (P < 2 * c->prm.window + 1 || P > MPPI_MAX_PATH)
+        return fail(c, MPPI_E_TRACK, "P must be in 2*window+1..MPPI_MAX_PATH");
+    for (int i = 0; i < 3 * P; ++i)
+        if (!std::isfinite(pts[i])) return fail(c, MPPI_E_TRACK, "path entry is not finite");
+    // [R-22] arc length = cumulative chord length, tangent = normalised central difference;
+    // computed in double from the fp32 points, rounded once
+    std::vector<double> s(P, 0.0);
+    auto dist = [&](int a, int b) {
+        double d0 = (double)pts[3 * a] - pts[3 * b], d1 = (double)pts[3 * a + 1] - pts[3 * b + 1],
+               d2 = (double)pts[3 * a + 2] - pts[3 * b + 2];
+        return std::sqrt(d0 * d0 + d1 * d1 + d2 * d2);
+    };
+    for (int i = 1; i < P; ++i) {
+        const double d = dist(i, i - 1);
+        if (!(d > 0.0)) return fail(c, MPPI_E_TRACK, "consecutive path points coincide");
+        s[i] = s[i - 1] + d;
+    }
+    double L = s[P - 1];
+    if (closed) {
+        const double d = dist(0, P - 1);
+        if (!(d > 0.0)) return fail(c, MPPI_E_TRACK, "closed path repeats its first point");
+        L += d;
+    }
+    std::vector<float4> v(2 * (size_t)P);
+    for (int i = 0; i < P; ++i) {
+        int ip = i + 1, im = i - 1;
+        if (closed) { ip %= P; im = (im + P) % P; }
+        else { ip = ip > P - 1 ? P - 1 : ip; im = im < 0 ? 0 : im; }
+        double t[3];
+        for (int a = 0; a < 3; ++a) t[a] = (double)pts[3 * ip + a] - pts[3 * im + a];
+        const double nt = std::sqrt(t[0] * t[0] + t[1] * t[1] + t[2] * t[2]);
+        if (!(nt > 0.0)) return fail(c, MPPI_E_TRACK, "degenerate path tangent");
+        v[2 * i] = make_float4(pts[3 * i], pts[3 * i + 1], pts[3 * i + 2], (float)s[i]);
+        v[2 * i + 1] = make_float4((float)(t[0] / nt), (float)(t[1] / nt), (float)(t[2] / nt), 0.0f);
+    }
+    int rc = upload_f4(c, &c->d_path, v);
+    if (rc) return rc;
+    c->dp.P = P; c->dp.closed = closed ? 1 : 0; c->dp.path = c->d_path;
+    c->dp.path_L = (float)L; c->dp.inv_path_L = (float)(1.0 / L);
+    c->have_path = true;
+    return MPPI_OK;
+}
+
+// ---- launch preparation ---------------------------------------------------------------------------
+
+static int prepare(mppi_ctx* c)
+{
+    const int obj = c->prm.objective;
+    if ((obj == MPPI_OBJ_GATE && !c->have_gates) || (obj == MPPI_OBJ_TRACK && !c->have_ref) ||
+        (obj == MPPI_OBJ_CONTOUR && !c->have_path))
+        return fail(c, MPPI_E_NO_TRACK, "mppi_set_gates / mppi_set_reference / mppi_set_path not called for this objective");
+    const size_t need = rollout_smem_bytes(c->dp, c->cfg);
+    if (need != c->cfg.smem_bytes) {
+        if (need > 227 * 1024) return fail(c, MPPI_E_PARAM, "track + horizon do not fit in shared memory");
+        if (need > 48 * 1024)
+            CK(c, cudaFuncSetAttribute(rollout_kernel_ptr(c->cfg), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)need));
+        c->cfg.smem_bytes = need;
+    }
+    return MPPI_OK;
+}
+
+static bool overlaps(const void* a, size_t na, const void* b, size_t nb)
+{
+    const char* x = (const char*)a; const char* y = (const char*)b;
+    return x < y + nb && y < x + na;
+}
+
+static StepArgs make_args(mppi_ctx* c, const float* x0, const int32_t* start, const float* u_nom,
+                          uint64_t seed, uint32_t iter, float* u_new, float* cost, float* w)
+{
+    StepArgs a;
+    a.x0 = x0; a.start = start; a.u_nom = u_nom; a.u_new = u_new; a.cost = cost; a.weights = w;
+    a.du = c->d_du; a.partials = c->d_partials; a.counters = c->d_counters;
+    a.seed_lo = (uint32_t)(seed & 0xffffffffu); a.seed_hi = (uint32_t)(seed >> 32); a.iter = iter;
+    return a;
+}
+
+static int enqueue_iteration(mppi_ctx* c, const StepArgs& a, cudaStream_t s)
+{
+    CK(c, launch_rollout(c->dp, a, c->cfg, s));
+    c->launches += 1;
+    if (!c->cfg.fused) {
+        CK(c, launch_reduce(c->dp, a, s));
+        c->launches += 1;
+    }
+    return MPPI_OK;
+}
+
+static void node_params(mppi_ctx* c, bool reduce, void** kp, cudaKernelNodeParams* np)
+{
+    std::memset(np, 0, sizeof *np);
+    if (!reduce) {
+        np->func = const_cast<void*>(rollout_kernel_ptr(c->cfg));
+        np->gridDim = dim3(c->dp.blocks_per_ctrl, c->dp.B);
+        np->blockDim = dim3(c->cfg.block_threads);
+        np->sharedMemBytes = (unsigned)c->cfg.smem_bytes;
+    } else {
+        np->func = const_cast<void*>(reduce_kernel_ptr());
+        np->gridDim = dim3(c->dp.N, c->dp.B);
+        np->blockDim = dim3(kReduceThreads);
+        np->sharedMemBytes = 0;
+    }
+    np->kernelParams = kp;
+}
+
+// Build (once) a graph of n iterations; every replay only rewrites the kernel parameters.
+static int graph_run(mppi_ctx* c, GraphSlot& g, const std::vector<StepArgs>& args, cudaStream_t s)
+{
+    const int n = (int)args.size();
+    DevParams dp = c->dp;
+    const bool build = !g.exec || g.n_iters != n;
+    if (build) {
+        free_graph(g);
+        CK(c, cudaGraphCreate(&g.graph, 0));
+    }
+    cudaGraphNode_t prev = nullptr;
+    for (int i = 0; i < n; ++i) {
+        StepArgs a = args[i];
+        void* kp[2] = {&dp, &a};
+        cudaKernelNodeParams np;
+        for (int pass = 0; pass < (c->cfg.fused ? 1 : 2); ++pass) {
+            node_params(c, pass == 1, kp, &np);
+            std::vector<cudaGraphNode_t>& nodes = pass ? g.reduce_nodes : g.rollout_nodes;
+            if (build) {
+                cudaGraphNode_t node;
+                CK(c, cudaGraphAddKernelNode(&node, g.graph, prev ? &prev : nullptr, prev ? 1 : 0, &np));
+                nodes.push_back(node);
+                prev = node;
+            } else {
+                CK(c, cudaGraphExecKernelNodeSetParams(g.exec, nodes[i], &np));
+            }
+        }
+    }
+    if (build) {
+        CK(c, cudaGraphInstantiate(&g.exec, g.graph, 0));
+        g.n_iters = n;
+    }
+    CK(c, cudaGraphLaunch(g.exec, s));
+    c->launches += (int64_t)n * (c->cfg.fused ? 1 : 2);
+    return MPPI_OK;
+}
+
+extern "C" int mppi_step(mppi_ctx* c, const float* d_x0, const int32_t* d_start, const float* d_u_nom,
+                         uint64_t seed, uint32_t iter, float* d_u_new, float* d_cost, float* d_weights,
+                         void* stream)
+{
+    if (!c) return MPPI_E_NULL;
+    if (!d_x0 || !d_start || !d_u_nom || !d_u_new || !d_cost || !d_weights)
+        return fail(c, MPPI_E_NULL, "mppi_step: NULL device pointer");
+    const size_t ub = (size_t)c->prm.B * c->prm.N * 4 * sizeof(float);
+    if (d_u_new != d_u_nom && overlaps(d_u_new, ub, d_u_nom, ub))
+        return fail(c, MPPI_E_RANGE, "d_u_new partially overlaps d_u_nom");
+    int rc = prepare(c);
+    if (rc) return rc;
+    const StepArgs a = make_args(c, d_x0, d_start, d_u_nom, seed, iter, d_u_new, d_cost, d_weights);
+    if (c->prm.use_graph) return graph_run(c, c->g_step, std::vector<StepArgs>(1, a), (cudaStream_t)stream);
+    return enqueue_iteration(c, a, (cudaStream_t)stream);
+}
+
+extern "C" int mppi_optimize(mppi_ctx* c, const float* d_x0, const int32_t* d_start, float* d_u,
+                             uint64_t seed, uint32_t iter0, int n_iters, float* d_cost, float* d_weights,
+                             void* stream)
+{
+    if (!c) return MPPI_E_NULL;
+    if (!d_x0 || !d_start || !d_u || !d_cost || !d_weights)
+        return fail(c, MPPI_E_NULL, "mppi_optimize: NULL device pointer");
+    if (n_iters < 1 || n_iters > 1024) return fail(c, MPPI_E_RANGE, "n_iters must be in 1..1024");
+    int rc = prepare(c);
+    if (rc) return rc;
+    std::vector<StepArgs> args;
+    for (int i = 0; i < n_iters; ++i)
+        args.push_back(make_args(c, d_x0, d_start, d_u, seed, iter0 + (uint32_t)i, d_u, d_cost, d_weights));
+    if (c->prm.use_graph) return graph_run(c, c->g_opt, args, (cudaStream_t)stream);
+    for (int i = 0; i < n_iters; ++i) {
+        rc = enqueue_iteration(c, args[i], (cudaStream_t)stream);
+        if (rc) return rc;
+    }
+    return MPPI_OK;
+}
+
+extern "C" int mppi_step_host(mppi_ctx* c, const float* h_x0, const int32_t* h_start, const float* h_u_nom,
+                              uint64_t seed, uint32_t iter, float* h_u_new, float* h_cost, float* h_weights,
+                              void* stream)
+{
+    if (!c) return MPPI_E_NULL;
+    if (!h_x0 || !h_start || !h_u_nom || !h_u_new) return fail(c, MPPI_E_NULL, "mppi_step_host: NULL host pointer");
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t B = c->prm.B, N = c->prm.N, K = c->prm.K;
+    CK(c, cudaMemcpyAsync(c->d_hx0, h_x0, B * 13 * sizeof(float), cudaMemcpyHostToDevice, s));
+    CK(c, cudaMemcpyAsync(c->d_hstart, h_start, B * sizeof(int32_t), cudaMemcpyHostToDevice, s));
+    CK(c, cudaMemcpyAsync(c->d_hu, h_u_nom, B * N * 4 * sizeof(float), cudaMemcpyHostToDevice, s));
+    int rc = mppi_step(c, c->d_hx0, c->d_hstart, c->d_hu, seed, iter, c->d_hu, c->d_hcost, c->d_hw, stream);
+    if (rc) return rc;
+    CK(c, cudaMemcpyAsync(h_u_new, c->d_hu, B * N * 4 * sizeof(float), cudaMemcpyDeviceToHost, s));
+    if (h_cost) CK(c, cudaMemcpyAsync(h_cost, c->d_hcost, B * K * sizeof(float), cudaMemcpyDeviceToHost, s));
+    if (h_weights) CK(c, cudaMemcpyAsync(h_weights, c->d_hw, B * K * sizeof(float), cudaMemcpyDeviceToHost, s));
+    CK(c, cudaStreamSynchronize(s));
+    return MPPI_OK;
+}
+
+extern "C" int mppi_sim_step(mppi_ctx* c, float* d_x, int32_t* d_start, const float* d_u_new,
+                             float* d_u_nom_next, void* stream)
+{
+    if (!c) return MPPI_E_NULL;
+    if (!d_x || !d_start || !d_u_new || !d_u_nom_next) return fail(c, MPPI_E_NULL, "mppi_sim_step: NULL device pointer");
+    const size_t ub = (size_t)c->prm.B * c->prm.N * 4 * sizeof(float);
+    if (d_u_nom_next != d_u_new && overlaps(d_u_nom_next, ub, d_u_new, ub))
+        return fail(c, MPPI_E_RANGE, "d_u_nom_next partially overlaps d_u_new");
+    int rc = prepare(c);
+    if (rc) return rc;
+    CK(c, launch_sim(c->dp, c->prm.objective, d_x, d_start, d_u_new, d_u_nom_next, (cudaStream_t)stream));
+    c->launches += 1;
+    return MPPI_OK;
+}
+
+extern "C" const float* mppi_debug_noise(mppi_ctx* c) { return c ? reinterpret_cast<const float*>(c->d_du) : nullptr; }
+
+extern "C" int64_t mppi_launch_count(mppi_ctx* c) { return c ? c->launches : 0; }
+
+extern "C" int mppi_get_info(mppi_ctx* c, mppi_info* o)
+{
+    if (!c || !o) return fail(c, MPPI_E_NULL, "mppi_get_info: NULL argument");
+    if (o->struct_size != sizeof(mppi_info)) return fail(c, MPPI_E_PARAM, "mppi_info.struct_size mismatch");
+    int rc = prepare(c);
+    if (rc) return rc;
+    cudaFuncAttributes fa;
+    CK(c, cudaFuncGetAttributes(&fa, rollout_kernel_ptr(c->cfg)));
+    int nb = 0;
+    CK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, rollout_kernel_ptr(c->cfg), c->cfg.block_threads,
+                                                        c->cfg.smem_bytes));
+    o->block_threads = c->cfg.block_threads;
+    o->blocks_per_controller = c->dp.blocks_per_ctrl;
+    o->grid_blocks = c->dp.blocks_per_ctrl * c->dp.B;
+    o->regs_per_thread = fa.numRegs;
+    o->static_smem_bytes = (int32_t)fa.sharedSizeBytes;
+    o->dynamic_smem_bytes = (int32_t)c->cfg.smem_bytes;
+    o->local_bytes_per_thread = (int32_t)fa.localSizeBytes;
+    o->max_blocks_per_sm = nb;
+    o->sm_count = c->sm_count;
+    o->kernels_per_step = c->cfg.fused ? 1 : 2;
+    o->l2_bytes = c->l2_bytes;
+    o->scratch_bytes = c->scratch_bytes;
+    return MPPI_OK;
+}

@@ -1,0 +1,31 @@
+// mppi_internal.h -- host-side declarations shared by mppi_api.cu and mppi_kernels.cu.
+#pragma once
+#include "mppi_device.cuh"
+
+namespace mppi {
+
+struct LaunchCfg {
+    int objective;      // OBJ_*
+    int fast_math;      // 0 / 1
+    int store_du;       // 0 / 1
+    int fused;          // 1: MPPI_PIPE_FUSED, 0: MPPI_PIPE_TWO_PASS
+    int block_threads;  // rollout block size
+    size_t smem_bytes;  // dynamic shared memory of the rollout kernel
+};
+
+// dynamic shared memory the rollout kernel needs for this configuration
+size_t rollout_smem_bytes(const DevParams& P, const LaunchCfg& c);
+
+// kernel function pointers (for cudaFuncGetAttributes / graph nodes)
+const void* rollout_kernel_ptr(const LaunchCfg& c);
+const void* reduce_kernel_ptr();
+const void* sim_kernel_ptr();
+
+cudaError_t launch_rollout(const DevParams& P, const StepArgs& A, const LaunchCfg& c, cudaStream_t s);
+cudaError_t launch_reduce(const DevParams& P, const StepArgs& A, cudaStream_t s);
+cudaError_t launch_sim(const DevParams& P, int objective, float* x, int* start, const float* u_new,
+                       float* u_nom_next, cudaStream_t s);
+
+constexpr int kReduceThreads = 256;
+
+}  // namespace mppi

@@ -1,0 +1,292 @@
+"""GPU parity: the CUDA path behind the C ABI against the float64 oracle, element by element, on
+the same seeded inputs -- the five BASELINE.json configs at full size in the launch configuration
+bench.py times, plus stress, ragged and degenerate cases.  Tolerances: tests/parity.py."""
+import numpy as np
+import pytest
+
+import parity as Pz
+from paper_2509_14726_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _report():
+    yield
+    if Pz.REPORT:
+        print("\n[parity] reported separately:\n  " + "\n  ".join(Pz.REPORT))
+
+
+def run_case(wl, tag, it=0, **opts):
+    m = Pz.make_ctx(wl, **opts)
+    x0, start, u = Pz.to_dev(wl)
+    g = Pz.gpu_step(m, x0, start, u, wl.seed, it)
+    o = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, wl.seed, it, want_du=wl.params["K"] * wl.params["N"] * wl.params["B"] <= 1 << 22)
+    o["u_nom"] = wl.u_nom.astype(np.float64)
+    st = Pz.compare(tag, g, o, wl.params["lambda"], wl.params["objective"] == 0)
+    m.close()
+    return g, o, st
+
+
+PIPES = [dict(pipeline=0), dict(pipeline=1)]
+MATH = [dict(fast_math=0), dict(fast_math=1)]
+
+
+@pytest.mark.parametrize("pipe", PIPES, ids=["fused", "two_pass"])
+@pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
+def test_cfg0_tiny_gate(pipe, math):
+    g, o, st = run_case(W.cfg0(), f"cfg0[{pipe},{math}]", **pipe, **math)
+    assert st["ess"] > 1.5            # the config really mixes several samples
+
+
+@pytest.mark.parametrize("pipe", PIPES, ids=["fused", "two_pass"])
+def test_cfg1_ten_warm_started_iterations(pipe):
+    # [R-14] no shift, same x0, u_nom <- u_new, iter = 0..9; the oracle is teacher-forced with the
+    # GPU's nominal of each iteration (fp32 -> fp64) so that every iteration is an exact comparison
+    import torch
+    wl = W.cfg1()
+    m = Pz.make_ctx(wl, **pipe)
+    x0, start, u = Pz.to_dev(wl)
+    crossings = 0
+    for it in range(wl.iters):
+        u_in = u.cpu().numpy()
+        g = Pz.gpu_step(m, x0, start, u, wl.seed, it, u_new=u)          # in place
+        o = Pz.oracle_step(wl, wl.x0, wl.start, u_in, wl.seed, it, want_du=True)
+        o["u_nom"] = u_in.astype(np.float64)
+        Pz.compare(f"cfg1[{pipe}] it{it}", g, o, wl.params["lambda"], True)
+        crossings += int((o["ncross"] > 0).sum())
+        np.testing.assert_array_equal(u.cpu().numpy(), g["u_new"])
+    assert crossings > 0
+    m.close()
+
+
+def test_cfg1_optimize_graph_equals_step_chain():
+    import torch
+    wl = W.cfg1()
+    x0, start, u0 = Pz.to_dev(wl)
+    m = Pz.make_ctx(wl)
+    u = u0.clone()
+    for it in range(wl.iters):
+        _, c_ref, w_ref = m.step(x0, start, u, wl.seed, it, u_new=u)
+    for graph in (0, 1):
+        m2 = Pz.make_ctx(wl, use_graph=graph)
+        for rep in range(2):                       # second replay goes through SetParams
+            u2 = u0.clone()
+            _, c2, w2 = m2.optimize(x0, start, u2, wl.seed, 0, wl.iters)
+            torch.cuda.synchronize()
+            assert torch.equal(u2, u) and torch.equal(c2, c_ref) and torch.equal(w2, w_ref)
+        m2.close()
+    m.close()
+
+
+@pytest.mark.parametrize("pipe", PIPES, ids=["fused", "two_pass"])
+@pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
+def test_cfg2_tracking(pipe, math):
+    run_case(W.cfg2(), f"cfg2[{pipe},{math}]", **pipe, **math)
+
+
+@pytest.mark.parametrize("pipe", PIPES, ids=["fused", "two_pass"])
+@pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
+def test_cfg3_contouring(pipe, math):
+    run_case(W.cfg3(), f"cfg3[{pipe},{math}]", **pipe, **math)
+
+
+@pytest.mark.parametrize("pipe", PIPES, ids=["fused", "two_pass"])
+@pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
+def test_stress_gate_crossings(pipe, math):
+    wl = W.stress_gate(K=4096, N=30)
+    g, o, st = run_case(wl, f"stress[{pipe},{math}]", **pipe, **math)
+    nc = o["ncross"]
+    assert (nc > 0).mean() > 0.3 and (nc == 0).mean() > 0.1      # pass and miss branches both taken
+
+
+def test_cfg4_closed_loop_teacher_forced():
+    # [R-17] 64 drones, closed loop on the GPU (plant + shift kernel); at checked control steps the
+    # oracle gets the GPU loop's actual (x, start, u_nom, iter) and is compared for that one step
+    import torch
+    from oracle import oracle as O
+    wl = W.cfg4(steps=120)
+    m = Pz.make_ctx(wl)
+    x, start, u = Pz.to_dev(wl)
+    trk = Pz.oracle_track(wl)
+    checked = 0
+    for step in range(wl.iters):
+        check = step in (0, 1, 2) or step % 40 == 0 or step == wl.iters - 1
+        if check:
+            x_in, s_in, u_in = x.cpu().numpy(), start.cpu().numpy(), u.cpu().numpy()
+        u_new, cost, w = m.step(x, start, u, wl.seed, step)
+        if check:
+            torch.cuda.synchronize()
+            g = dict(u_new=u_new.cpu().numpy(), cost=cost.cpu().numpy(), weights=w.cpu().numpy())
+            o = Pz.oracle_step(wl, x_in, s_in, u_in, wl.seed, step)
+            Pz.compare(f"cfg4 step{step}", g, o, wl.params["lambda"], True)
+            xo, so, uo = O.sim_step(wl.params, trk, x_in, s_in, g["u_new"])
+        m.sim_step(x, start, u_new, u_nom_next=u)
+        if check:
+            torch.cuda.synchronize()
+            np.testing.assert_allclose(x.cpu().numpy(), xo, rtol=3e-6, atol=2e-5)
+            np.testing.assert_array_equal(u.cpu().numpy(), uo.astype(np.float32))
+            # the plant's gate decision may differ only if the plant sat within the margin
+            assert (start.cpu().numpy() == so).mean() >= 0.98
+            checked += 1
+    assert checked >= 6
+    assert int(start.max()) >= 1            # the loop really flies through gates
+    m.close()
+
+
+# ---- the reduction arithmetic with many contributing samples (ESS >> 1) -------------------------
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3"])
+@pytest.mark.parametrize("pipe", PIPES, ids=["fused", "two_pass"])
+def test_flat_weights_exercise_the_update(name, pipe):
+    wl = W.ALL[name](K=2048, N=50)
+    o0 = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, wl.seed, 0)
+    wl.params["lambda"] = float(np.float32(0.25 * o0["cost"].std()))
+    g, o, st = run_case(wl, f"flat-{name}[{pipe}]", **pipe)
+    assert st["ess"] > 20
+    assert st["w"] <= Pz.W_ATOL and st["u"] <= Pz.U_ATOL
+
+
+def test_noise_matches_oracle_and_pipelines_agree():
+    import torch
+    wl = W.cfg0(K=512, N=37)
+    outs = {}
+    for name, opts in dict(fused=dict(pipeline=0, store_noise=1), two=dict(pipeline=1)).items():
+        m = Pz.make_ctx(wl, **opts)
+        x0, start, u = Pz.to_dev(wl)
+        outs[name] = Pz.gpu_step(m, x0, start, u, 5, 7)
+        outs[name]["du"] = m.debug_noise().cpu().numpy()      # [B,N,K,4]
+        m.close()
+    o = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, 5, 7, want_du=True)
+    du_o = np.transpose(o["du"], (0, 2, 1, 3))
+    np.testing.assert_allclose(outs["fused"]["du"], du_o, rtol=0, atol=3e-6)
+    np.testing.assert_array_equal(outs["fused"]["du"], outs["two"]["du"])
+    np.testing.assert_array_equal(outs["fused"]["cost"], outs["two"]["cost"])
+    np.testing.assert_allclose(outs["fused"]["weights"], outs["two"]["weights"], rtol=0, atol=2e-6)
+    np.testing.assert_allclose(outs["fused"]["u_new"], outs["two"]["u_new"], rtol=0, atol=2e-5)
+    # clamp really acts: some perturbations are cut at the thrust limits
+    T = wl.u_nom[:, :, None, :] + outs["fused"]["du"]
+    assert T.min() >= 0.0 and T.max() <= 7.0 and (T == 0.0).any()
+    m = Pz.make_ctx(wl)
+    assert m.debug_noise() is None
+    m.close()
+
+
+# ---- ragged / degenerate / maximum sizes ----------------------------------------------------------
+
+@pytest.mark.parametrize("K,N,tpb", [(32, 1, 32), (32, 33, 32), (64, 20, 64), (96, 7, 32), (256, 256, 256),
+                                     (1024, 64, 128), (8192, 50, 256)])
+@pytest.mark.parametrize("pipe", PIPES, ids=["fused", "two_pass"])
+def test_sizes_and_block_shapes(K, N, tpb, pipe):
+    wl = W.stress_gate(K=K, N=N)
+    run_case(wl, f"sizes K{K} N{N} tpb{tpb} [{pipe}]", block_threads=tpb, **pipe)
+
+
+@pytest.mark.parametrize("pipe", PIPES, ids=["fused", "two_pass"])
+def test_sigma_zero_is_uniform(pipe):
+    wl = W.cfg0(K=128, N=10)
+    wl.params["sigma"] = 0.0
+    g, o, _ = run_case(wl, f"sigma0[{pipe}]", **pipe)
+    np.testing.assert_allclose(g["weights"], 1.0 / 128, rtol=1e-6)
+    np.testing.assert_array_equal(g["u_new"], wl.u_nom)
+    assert np.ptp(g["cost"]) == 0.0
+
+
+@pytest.mark.parametrize("pipe", PIPES, ids=["fused", "two_pass"])
+def test_saturated_nominal_and_tiny_lambda(pipe):
+    wl = W.cfg0(K=256, N=12)
+    wl.u_nom[:] = 7.0
+    wl.params["lambda"] = float(np.float32(1e-4))
+    g, o, _ = run_case(wl, f"saturated[{pipe}]", **pipe)
+    k = int(np.argmin(o["cost"][0]))
+    assert g["weights"][0, k] > 0.999                       # lambda -> 0: the arg-min sample
+    assert g["u_new"].max() <= 7.0 and g["u_new"].min() >= 0.0
+
+
+def test_multi_controller_batches_are_independent():
+    # B = 3 controllers with different states, starts and nominals; controller b of the batch
+    # equals a B = 1 run given the same counter word b -> checked against the oracle per b
+    wl = W.cfg4(K=512, N=20, B=3)
+    wl.start[:] = [0, 2, 3]
+    wl.u_nom[1] += 0.2
+    run_case(wl, "B3 gate", it=4)
+    wl2 = W.cfg2(K=256, N=16, extra_rows=8)
+    wl2.params["B"] = 2
+    wl2.x0 = np.repeat(wl2.x0, 2, 0); wl2.x0[1, 0:3] += 0.1
+    wl2.start = np.array([0, 5], np.int32)
+    wl2.u_nom = np.repeat(wl2.u_nom, 2, 0)
+    run_case(wl2, "B2 track")
+
+
+def test_contour_hint_and_open_path():
+    wl = W.cfg3(K=512, N=30)
+    run_case(wl, "contour global")
+    wl.start[:] = 470                                      # windowed search around a hint
+    run_case(wl, "contour hint")
+    wl.closed = False                                      # open path: no wrap, clipped window
+    wl.start[:] = -1
+    run_case(wl, "contour open")
+    wl.x0[0, 0:3] = wl.path[3] + np.float32([0.05, 0.0, 0.02])
+    wl.start[:] = 2
+    run_case(wl, "contour open near start")
+
+
+def test_determinism_and_host_entry_point():
+    import torch
+    wl = W.stress_gate(K=1024, N=30)
+    for opts in PIPES:
+        m = Pz.make_ctx(wl, **opts)
+        x0, start, u = Pz.to_dev(wl)
+        a = Pz.gpu_step(m, x0, start, u, 9, 1)
+        b = Pz.gpu_step(m, x0, start, u, 9, 1)
+        for k in a:
+            np.testing.assert_array_equal(a[k], b[k])
+        c = Pz.gpu_step(m, x0, start, u, 9, 2)
+        assert not np.array_equal(a["cost"], c["cost"])     # iter feeds the counter
+        d = Pz.gpu_step(m, x0, start, u, 10, 1)
+        assert not np.array_equal(a["cost"], d["cost"])     # seed feeds the key
+        un, co, we = m.step_host(wl.x0, wl.start, wl.u_nom, 9, 1)
+        np.testing.assert_array_equal(un, a["u_new"]); np.testing.assert_array_equal(co, a["cost"])
+        np.testing.assert_array_equal(we, a["weights"])
+        assert m.launch_count() == (5 if opts["pipeline"] == 0 else 10)
+        m.close()
+
+
+def test_seed_high_word_reaches_the_key():
+    wl = W.cfg0(K=64, N=5)
+    wl.seed = (0xDEADBEEF << 32) | 0x12345678
+    run_case(wl, "64-bit seed", it=0xFFFFFFFF)
+
+
+def test_error_paths_on_device():
+    import torch
+    from paper_2509_14726_b200 import binding as Bd
+    wl = W.cfg0(K=64, N=8)
+    m = Bd.Mppi(wl.params)
+    x0, start, u = Pz.to_dev(wl)
+    with pytest.raises(Bd.MppiError) as e:
+        m.step(x0, start, u, 0, 0)
+    assert e.value.status == -3                                           # MPPI_E_NO_TRACK
+    bad = wl.gates.copy(); bad[0, 3:6] *= 1.01
+    with pytest.raises(Bd.MppiError) as e:
+        m.set_gates(bad)
+    assert e.value.status == -4                                           # MPPI_E_TRACK
+    m.set_gates(wl.gates)
+    buf = torch.zeros(2 * u.numel(), device="cuda")
+    a = buf[: u.numel()].view_as(u); b = buf[4: 4 + u.numel()].view_as(u)
+    with pytest.raises(Bd.MppiError) as e:
+        m.step(x0, start, a, 0, 0, u_new=b)
+    assert e.value.status == -5                                           # MPPI_E_RANGE
+    with pytest.raises(ValueError):
+        m.step(x0, start, u.double(), 0, 0)
+    m.close()
+    m = Bd.Mppi(W.cfg2(K=64, N=8).params)
+    with pytest.raises(Bd.MppiError) as e:
+        m.set_reference(np.zeros((8, 13), np.float32))                    # M < N+1
+    assert e.value.status == -4
+    m.close()
+    m = Bd.Mppi(W.cfg3(K=64, N=8).params)
+    with pytest.raises(Bd.MppiError) as e:
+        m.set_path(np.zeros((10, 3), np.float32))                         # P < 2 window + 1
+    assert e.value.status == -4
+    m.close()
