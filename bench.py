@@ -1,0 +1,379 @@
+#!/usr/bin/env python
+"""bench.py -- MPPI sample-steps/s and iteration latency on B200 (BASELINE.json:metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+One "step" = one MPPI iteration of the whole hot path (noise -> clamp -> RK4 rollout -> cost ->
+softmax weights -> update) on the workload BASELINE.json's metric is quoted on: configs[1],
+gate progress, K=4096 samples, N=50 steps, one controller, warm-started in place.  The timed
+region has its inputs resident in HBM; L2 is flushed between timed iterations (a 256 MiB write,
+outside the events).  Rank 0 prints ONE JSON line.  Multi-GPU: the path does not shard
+(north_star: one GPU, no collectives) -> N independent replicas, value = N * units / max time.
+
+--impl reference times the float64 CPU oracle (oracle/) as it stands on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+METRIC = "mppi_sample_steps_per_sec"
+UNIT = "sample-steps/s"
+# Algorithmic FP32 work per sample-step of the gate objective (
+# SURVEY.md 8(d)): add/sub/mul = 1, FMA = 2, MUFU = 1, integer / min / max / compare = 0.
+FLOPS_PER_SAMPLE_STEP = {0: 417.0, 1: 449.0, 2: 685.0}
+FP32_LANES_PER_SM = 128
+L2_FLUSH_BYTES = 256 << 20
+
+
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def reduce_max_ms(ms: float, world: int, backend_device=None) -> float:
+    """max over ranks of a duration (the contract's multi-GPU timing rule)."""
+    if world == 1:
+        return ms
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=backend_device or "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(units_per_rank: float, world: int, max_ms: float) -> float:
+    """whole-job throughput of N independent replicas: all ranks' units / the slowest rank's time."""
+    return units_per_rank * world / (max_ms * 1e-3)
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int, period_s: float = 0.005):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period_s
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._halt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    _NAMES = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+              0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+              0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        while not self._halt.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in self._NAMES.items():
+                    if r & bit and name != "gpu_idle":
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._halt.wait(self.period)
+
+    def finish(self) -> dict:
+        self._halt.set()
+        if self.is_alive():
+            self.join(timeout=1.0)
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["nvml unavailable"], "samples": 0}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ---------------------------------------------------------------------------------------------
+# the reference arm / cpu_baseline: the oracle as it stands, on the host cores
+# ---------------------------------------------------------------------------------------------
+
+def time_oracle(wl, budget_s: float, max_iters: int, sample_K: int | None = None):
+    """Runs full oracle iterations of `wl` (optionally on the first sample_K samples) until the
+    budget or max_iters is reached.  Returns (sample-steps/s, seconds per iteration, iterations, threads)."""
+    from oracle import oracle as O
+    p = dict(wl.params)
+    if sample_K:
+        p["K"] = int(sample_K)
+    trk = O.Track(gates=wl.gates, ref=wl.ref, path=wl.path, closed=wl.closed)
+    u = wl.u_nom.astype(np.float64)
+    O.step(p, trk, wl.x0, wl.start, u, wl.seed, 0, want_diag=False)           # build + warm
+    t0 = time.perf_counter()
+    n = 0
+    while n < max_iters and (time.perf_counter() - t0 < budget_s or n == 0):
+        r = O.step(p, trk, wl.x0, wl.start, u, wl.seed, n, want_diag=False)
+        u = r["u_new"]
+        n += 1
+    dt = time.perf_counter() - t0
+    units = p["K"] * p["N"] * p["B"] * n
+    return units / dt, dt / n, n, O.num_threads()
+
+
+def run_reference(args):
+    from paper_2509_14726_b200 import workloads as W
+    rank, _, world = dist_env()
+    if rank != 0:
+        return 0
+    wl = W.cfg1()
+    from oracle import oracle as O
+    # size the per-step sample so that steps+warmup steps end within ~2 minutes
+    rate, s_iter, _, threads = time_oracle(wl, 1.0, 3)
+    total = args.steps + args.warmup
+    sample_K = wl.params["K"]
+    while sample_K > 32 and s_iter * sample_K / wl.params["K"] * total > 120.0:
+        sample_K //= 2
+    p = dict(wl.params); p["K"] = sample_K
+    trk = O.Track(gates=wl.gates, ref=wl.ref, path=wl.path, closed=wl.closed)
+    u = wl.u_nom.astype(np.float64)
+    for i in range(args.warmup):
+        u = O.step(p, trk, wl.x0, wl.start, u, wl.seed, i, want_diag=False)["u_new"]
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        u = O.step(p, trk, wl.x0, wl.start, u, wl.seed, args.warmup + i, want_diag=False)["u_new"]
+    dt = time.perf_counter() - t0
+    units = sample_K * wl.params["N"] * args.steps
+    value = units / dt
+    sample = (f"{args.steps} iterations of {wl.name} restricted to the first {sample_K} of {wl.params['K']} samples"
+              if sample_K != wl.params["K"] else f"{args.steps} full iterations of {wl.name}")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": wl.name, "K": wl.params["K"], "N": wl.params["N"], "B": 1,
+                       "objective": "gate", "sample_K": sample_K},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------
+
+def _events(n):
+    import torch
+    return [torch.cuda.Event(enable_timing=True) for _ in range(n)]
+
+
+def time_steps(step_fn, flush_fn, steps, warmup):
+    """W untimed steps, then exactly `steps` steps, each bracketed by CUDA events on the launching
+    stream with an L2 flush before it (outside the events).  Returns per-step ms (numpy)."""
+    import torch
+    for _ in range(warmup):
+        flush_fn(); step_fn()
+    torch.cuda.synchronize()
+    e0, e1 = _events(steps), _events(steps)
+    for i in range(steps):
+        flush_fn()
+        e0[i].record()
+        step_fn()
+        e1[i].record()
+    torch.cuda.synchronize()
+    return np.array([a.elapsed_time(b) for a, b in zip(e0, e1)])
+
+
+def time_back_to_back(step_fn, steps, warmup):
+    import torch
+    for _ in range(warmup):
+        step_fn()
+    torch.cuda.synchronize()
+    a, b = _events(2)
+    a.record()
+    for _ in range(steps):
+        step_fn()
+    b.record()
+    torch.cuda.synchronize()
+    return a.elapsed_time(b) / steps
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2509_14726_b200 import binding as Bd
+    from paper_2509_14726_b200 import workloads as W
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank % torch.cuda.device_count())
+    dev = torch.device("cuda", torch.cuda.current_device())
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    wl = W.cfg1()
+    P = wl.params
+    units = P["K"] * P["N"] * P["B"]
+    m = Bd.Mppi(P, fast_math=args.fast_math, pipeline=args.pipeline, use_graph=args.graph)
+    m.set_track(wl)
+    x0 = torch.from_numpy(wl.x0).to(dev); start = torch.from_numpy(wl.start).to(dev)
+    u = torch.from_numpy(wl.u_nom).to(dev)
+    cost = torch.empty((P["B"], P["K"]), device=dev); w = torch.empty_like(cost)
+    flush_buf = torch.empty(L2_FLUSH_BYTES // 4, dtype=torch.float32, device=dev)
+    it = [0]
+
+    def step():
+        m.step(x0, start, u, wl.seed, it[0], u_new=u, cost=cost, weights=w)     # warm start in place
+        it[0] += 1
+
+    def flush():
+        flush_buf.fill_(float(it[0] & 7))
+
+    # roofline denominators measured live on this device
+    fma_tflops, clock_attr_mhz = Bd.measure_fma_peak(3)
+    info = m.info()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(torch.cuda.current_device())
+    barrier()
+    l0 = m.launch_count()
+    sampler.start()
+    ms = time_steps(step, flush, args.steps, args.warmup)
+    clocks = sampler.finish()
+    barrier()
+    launches = m.launch_count() - l0 - args.warmup * info["kernels_per_step"]
+    my_ms = float(ms.sum())
+    max_ms = reduce_max_ms(my_ms, world, dev)
+    ms_per_step = max_ms / args.steps
+    value = aggregate_value(units * args.steps, world, max_ms)
+
+    line = None
+    if rank == 0:
+        hot_ms = time_back_to_back(step, args.steps, args.warmup)
+
+        # ---- e2e: the same iteration through mppi_step_host with pinned HOST buffers
+        hx0 = torch.from_numpy(wl.x0).pin_memory(); hstart = torch.from_numpy(wl.start).pin_memory()
+        hu = torch.from_numpy(wl.u_nom.copy()).pin_memory()
+        hout = torch.empty_like(hu).pin_memory()
+        n_e2e = min(args.steps, 2000)
+
+        def host_step(i):
+            m.step_host(hx0.numpy(), hstart.numpy(), hu.numpy(), wl.seed, i, u_new=hout.numpy(), want_cost=False)
+        for i in range(max(args.warmup, 3)):
+            host_step(i)
+        lat = np.empty(n_e2e)
+        t_all = time.perf_counter()
+        for i in range(n_e2e):
+            t0 = time.perf_counter()
+            host_step(i)
+            lat[i] = time.perf_counter() - t0
+        t_all = time.perf_counter() - t_all
+        h2d = hx0.numel() * 4 + hstart.numel() * 4 + hu.numel() * 4
+        d2h = hout.numel() * 4
+
+        # ---- the batched configuration (configs[4] shape): where the FP32 roofline is reachable
+        wl4 = W.cfg4()
+        P4 = wl4.params
+        m4 = Bd.Mppi(P4, fast_math=args.fast_math, pipeline=args.pipeline)
+        m4.set_track(wl4)
+        x4 = torch.from_numpy(wl4.x0).to(dev); s4 = torch.from_numpy(wl4.start).to(dev)
+        u4 = torch.from_numpy(wl4.u_nom).to(dev); un4 = torch.empty_like(u4)
+        c4 = torch.empty((P4["B"], P4["K"]), device=dev); w4 = torch.empty_like(c4)
+        j = [0]
+
+        def step4():
+            m4.step(x4, s4, u4, 0, j[0], u_new=un4, cost=c4, weights=w4); j[0] += 1
+        ms4 = time_steps(step4, flush, 30, 5)
+        units4 = P4["K"] * P4["N"] * P4["B"]
+        flops = FLOPS_PER_SAMPLE_STEP[0]
+        sm = info["sm_count"]
+        peak_tf = sm * FP32_LANES_PER_SM * 2 * (clocks["sm_max_mhz"] or clock_attr_mhz) * 1e6 / 1e12
+        ach = units * flops / (float(ms.mean()) * 1e-3) / 1e12
+        ach4 = units4 * flops / (float(ms4.mean()) * 1e-3) / 1e12
+
+        # ---- cpu_baseline: the oracle on this host's cores, bounded sample
+        from oracle import oracle as O   # noqa: F401  (cpu_baseline leg only)
+        cpu_rate, cpu_s_iter, cpu_n, cpu_threads = time_oracle(wl, args.cpu_budget, 400)
+
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": wl.name, "K": P["K"], "N": P["N"], "B": P["B"], "objective": "gate",
+                       "dt": P["dt"], "sigma": P["sigma"], "lambda": P["lambda"], "warm_start": "in place, iter = step",
+                       "l2": "flushed between timed iterations (256 MiB write outside the events)",
+                       "pipeline": "fused" if args.pipeline == 0 else "two_pass", "fast_math": args.fast_math,
+                       "cuda_graph": bool(args.graph), "block_threads": info["block_threads"],
+                       "grid_blocks": info["grid_blocks"], "replicas": world},
+            "clocks": clocks,
+            "latency_us": {"p50": float(np.median(ms) * 1e3), "p99": float(np.percentile(ms, 99) * 1e3),
+                           "mean": float(ms.mean() * 1e3), "back_to_back_no_flush": hot_ms * 1e3},
+            "e2e": {"value": units * n_e2e / t_all, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                    "d2h_bytes_per_step": int(d2h), "latency_us_p50": float(np.median(lat) * 1e6),
+                    "latency_us_p99": float(np.percentile(lat, 99) * 1e6),
+                    "timer": "host perf_counter around mppi_step_host (H2D + kernel + D2H + sync), pinned buffers"},
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
+                         "traffic": None, "kernel": "rollout_kernel<gate>" + (" (fused update)" if args.pipeline == 0 else ""),
+                         "flops_per_sample_step": flops, "units_per_launch": units,
+                         "peak_how": f"{sm} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 x clocks.max.sm (B200_PROFILING.md)",
+                         "peak_measured_ffma_tflops": fma_tflops, "frac_of_measured_ffma": ach / fma_tflops,
+                         "regs_per_thread": info["regs_per_thread"], "spill_bytes": info["local_bytes_per_thread"],
+                         "note": "K=4096 is 128 warps on 148 SMs: latency-bound by construction; see 'batched'"},
+            "batched": {"workload": wl4.name, "K": P4["K"], "N": P4["N"], "B": P4["B"],
+                        "value": units4 / (float(ms4.mean()) * 1e-3), "unit": UNIT, "ms_per_step": float(ms4.mean()),
+                        "roofline": {"bound": "alu", "achieved": ach4, "peak": peak_tf, "unit": "TFLOP/s",
+                                     "frac": ach4 / peak_tf, "frac_of_measured_ffma": ach4 / fma_tflops}},
+            "cpu_baseline": {"value": cpu_rate, "unit": UNIT, "cores": cpu_threads, "kind": "oracle",
+                             "sample": f"{cpu_n} full iterations of {wl.name} ({cpu_s_iter * 1e3:.1f} ms each), float64, OpenMP over samples"},
+        }
+        m4.close()
+    m.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if line is not None:
+        print(json.dumps(line), flush=True)
+    return 0
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=1000)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--pipeline", type=int, default=0, help="0 fused (default), 1 two-pass")
+    ap.add_argument("--fast-math", dest="fast_math", type=int, default=1)
+    ap.add_argument("--graph", type=int, default=0)
+    ap.add_argument("--cpu-budget", dest="cpu_budget", type=float, default=10.0)
+    args = ap.parse_args(argv)
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
