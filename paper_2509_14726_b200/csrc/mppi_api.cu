@@ -181,6 +181,11 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     DevParams& d = c->dp;
     std::memset(&d, 0, sizeof d);
     d.K = p->K; d.N = p->N; d.B = p->B; d.window = p->window;
+    {
+        const double h = (double)p->dt;
+        d.h2 = (float)(h / 2); d.h3 = (float)(h / 3); d.h4 = (float)(h / 4); d.h6 = (float)(h / 6);
+        d.h12 = (float)(h / 12); d.hh2 = (float)(h * h / 2); d.hh3 = (float)(h * h / 3);
+    }
     d.dt = p->dt; d.inv_lambda = (float)(1.0 / (double)p->lambda); d.sigma = p->sigma;
     d.T_min = p->T_min; d.T_max = p->T_max;
     d.inv_mass = (float)(1.0 / (double)p->mass); d.g = p->g;
@@ -364,6 +369,10 @@ static StepArgs make_args(mppi_ctx* c, const float* x0, const int32_t* start, co
     a.x0 = x0; a.start = start; a.u_nom = u_nom; a.u_new = u_new; a.cost = cost; a.weights = w;
     a.du = c->d_du; a.partials = c->d_partials; a.counters = c->d_counters;
     a.seed_lo = (uint32_t)(seed & 0xffffffffu); a.seed_hi = (uint32_t)(seed >> 32); a.iter = iter;
+    for (uint32_t r = 0; r < 10; ++r) {          // Philox key schedule (Weyl sequence), hoisted out of the kernel
+        a.rk[2 * r] = a.seed_lo + r * 0x9E3779B9u;
+        a.rk[2 * r + 1] = a.seed_hi + r * 0xBB67AE85u;
+    }
     return a;
 }
 

@@ -9,51 +9,75 @@ enum { OBJ_GATE = 0, OBJ_TRACK = 1, OBJ_CONTOUR = 2 };
 
 // ---- gate progress: eq.(6) PAPER.md:105-110 with un-squared distances [D-2], in-horizon target
 // switching PAPER.md:112, geometric pass test [R-9],[R-10]; constants BASELINE.json configs[0].
+//
+// The progress sum telescopes while the target does not change: sum_t (d_t - d_{t-1}) = d_end -
+// d_begin of each constant-target segment.  Only the signed plane distance s = n.(p - c) is needed
+// every step (the crossing test); the distances are taken at a target switch and at the horizon end.
+// The body-rate term accumulates sum |omega|^2 and is scaled once at the end.
 struct GateCost {
     int gate;                 // current target
-    float rx, ry, rz;         // p_{t-1} - c
-    float d_prev, s_prev;     // |p_{t-1} - c|, n . (p_{t-1} - c)
+    float d0;                 // |p - c| where the current segment began
+    float s_prev;             // n . (p_{t-1} - c)
+    float ppx, ppy, ppz;      // p_{t-1}
+    float J;                  // pass bonuses / miss penalties / finished segments
+    float w2;                 // sum_t |omega_t|^2
 
+    template <int MATH>
+    __device__ __forceinline__ static float norm3(float x, float y, float z)
+    {
+        const float r2 = fmaf(z, z, fmaf(y, y, x * x));
+        return MATH == 0 ? sqrtf(r2) : mufu_sqrt(r2);
+    }
+    template <int MATH>
     __device__ __forceinline__ void retarget(const float4* s_gates, float px, float py, float pz)
     {
         const float4 c = s_gates[4 * gate], n = s_gates[4 * gate + 1];
-        rx = px - c.x; ry = py - c.y; rz = pz - c.z;
-        d_prev = sqrtf(rx * rx + ry * ry + rz * rz);
-        s_prev = n.x * rx + n.y * ry + n.z * rz;
+        const float rx = px - c.x, ry = py - c.y, rz = pz - c.z;
+        d0 = norm3<MATH>(rx, ry, rz);
+        s_prev = fmaf(n.z, rz, fmaf(n.y, ry, n.x * rx));
     }
-    __device__ __forceinline__ void init(const DevParams& P, const float4* s_gates, int start,
-                                         const State& x)
+    template <int MATH>
+    __device__ __forceinline__ void init(const DevParams& P, const float4* s_gates, int start, const State& x)
     {
         gate = wrap_index(start, P.G);
-        retarget(s_gates, x.px, x.py, x.pz);
+        J = 0.0f; w2 = 0.0f;
+        ppx = x.px; ppy = x.py; ppz = x.pz;
+        retarget<MATH>(s_gates, x.px, x.py, x.pz);
     }
-    // post-step state x_{t+1}; returns the step cost
-    __device__ __forceinline__ float step(const DevParams& P, const float4* s_gates, const State& x)
+    // post-step state x_{t+1}
+    template <int MATH>
+    __device__ __forceinline__ void step(const DevParams& P, const float4* s_gates, const State& x)
     {
         const float4 c = s_gates[4 * gate], n = s_gates[4 * gate + 1];
         const float ax = x.px - c.x, ay = x.py - c.y, az = x.pz - c.z;
-        const float d = sqrtf(ax * ax + ay * ay + az * az);
-        const float s = n.x * ax + n.y * ay + n.z * az;
-        float J = d - d_prev;
+        const float s = fmaf(n.z, az, fmaf(n.y, ay, n.x * ax));
         if (s_prev < 0.0f && s >= 0.0f) {                 // front -> back through the plane
             const float4 h = s_gates[4 * gate + 2], v = s_gates[4 * gate + 3];
             const float alpha = s_prev / (s_prev - s);
-            const float hx = fmaf(alpha, ax - rx, rx), hy = fmaf(alpha, ay - ry, ry),
-                        hz = fmaf(alpha, az - rz, rz);
-            const float y = h.x * hx + h.y * hy + h.z * hz;
-            const float z = v.x * hx + v.y * hy + v.z * hz;
+            const float rx = ppx - c.x, ry = ppy - c.y, rz = ppz - c.z;
+            const float hx = fmaf(alpha, ax - rx, rx), hy = fmaf(alpha, ay - ry, ry), hz = fmaf(alpha, az - rz, rz);
+            const float y = fmaf(h.z, hz, fmaf(h.y, hy, h.x * hx));
+            const float z = fmaf(v.z, hz, fmaf(v.y, hy, v.x * hx));
             if (fabsf(y) <= c.w && fabsf(z) <= n.w) {     // inside the opening: pass + switch
-                J -= P.bonus;
+                J += (norm3<MATH>(ax, ay, az) - d0) - P.bonus;        // close the segment
                 gate = (gate + 1 == P.G) ? 0 : gate + 1;
-                retarget(s_gates, x.px, x.py, x.pz);      // the new target applies from the next step
+                retarget<MATH>(s_gates, x.px, x.py, x.pz);            // new target from the next step on
             } else {                                      // miss: target unchanged
                 J += P.miss;
-                rx = ax; ry = ay; rz = az; d_prev = d; s_prev = s;
+                s_prev = s;
             }
         } else {
-            rx = ax; ry = ay; rz = az; d_prev = d; s_prev = s;
+            s_prev = s;
         }
-        return fmaf(P.w_omega, x.ox * x.ox + x.oy * x.oy + x.oz * x.oz, J);
+        ppx = x.px; ppy = x.py; ppz = x.pz;
+        w2 = fmaf(x.oz, x.oz, fmaf(x.oy, x.oy, fmaf(x.ox, x.ox, w2)));
+    }
+    template <int MATH>
+    __device__ __forceinline__ float finish(const DevParams& P, const float4* s_gates, const State& x) const
+    {
+        const float4 c = s_gates[4 * gate];
+        const float d = norm3<MATH>(x.px - c.x, x.py - c.y, x.pz - c.z);
+        return fmaf(P.w_omega, w2, J + (d - d0));
     }
 };
 

@@ -15,6 +15,7 @@ struct DevParams {
     int G, M, P, closed, window;      // gates, reference rows, path points
     int blocks_per_ctrl;               // rollout blocks per controller = K / blockDim.x
     float dt, inv_lambda, sigma, T_min, T_max;
+    float h2, h3, h4, h6, h12, hh2, hh3;   // dt/2, dt/3, dt/4, dt/6, dt/12, dt^2/2, dt^2/3
     float inv_mass, g, hover;
     float ltx, lty, ltz;               // (arm/sqrt2)/Jx, (arm/sqrt2)/Jy, c_tau/Jz
     float gyx, gyy, gyz;               // (Jy-Jz)/Jx, (Jz-Jx)/Jy, (Jx-Jy)/Jz   (omega x J omega)
@@ -38,24 +39,25 @@ struct StepArgs {
     float* partials;       // [B][blocks_per_ctrl][4N+4]  (fused pipeline)
     unsigned int* counters;// [B]                         (fused pipeline)
     uint32_t seed_lo, seed_hi, iter;
+    uint32_t rk[20];       // Philox round keys: rk[2r] = seed_lo + r W0, rk[2r+1] = seed_hi + r W1
 };
 
 // ---- Philox4x32-10, counter-based (Salmon et al., SC'11) [R-1] -----------------------------
 // eq.(3) PAPER.md:78-82 asks for independent Gaussian perturbations; north_star fixes the
 // generator and its keying: counter = (sample k, step t, iter, controller b), key = seed.
+// The ten round keys depend only on the seed: the host puts them in the kernel-argument constant
+// bank (StepArgs::rk), so a round is 2 IMAD.WIDE + 2 LOP3 and holds no key registers.
 __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
-                                               uint32_t k0, uint32_t k1)
+                                               const uint32_t (&rk)[20])
 {
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
         const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
         const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
-        c0 = hi1 ^ c1 ^ k0;
+        c0 = hi1 ^ c1 ^ rk[2 * r];
         c1 = lo1;
-        c2 = hi0 ^ c3 ^ k1;
+        c2 = hi0 ^ c3 ^ rk[2 * r + 1];
         c3 = lo0;
-        k0 += 0x9E3779B9u;
-        k1 += 0xBB67AE85u;
     }
     return make_uint4(c0, c1, c2, c3);
 }
@@ -67,44 +69,57 @@ __device__ __forceinline__ float u01(uint32_t r)
     return __uint_as_float(0x3f800000u | (r >> 9)) - 0.99999994f;
 }
 
-// [R-3] Box-Muller pair.  MATH = 0: IEEE-accurate library functions.  MATH = 1: MUFU
-// approximations (lg2 / rsq / sin / cos), see DESIGN.md "error budget".
+// MUFU approximations with flush-to-zero forms (no denormal fix-up code: every argument below is a
+// normal number by construction).
+__device__ __forceinline__ float mufu_lg2(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_rsq(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_sqrt(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_sin(float x) { float y; asm("sin.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_cos(float x) { float y; asm("cos.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_ex2(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
+// [R-3] Box-Muller pair scaled by sigma, added to the nominal: (a, b) = (una, unb) + sigma (z0, z1),
+// z0 = rad cos(2 pi u2), z1 = rad sin(2 pi u2), rad = sqrt(-2 ln u1).
+// MATH = 0: IEEE-accurate library functions, in the oracle's operation order.
+// MATH = 1: MUFU lg2 / rsq / sin / cos.  The angle is taken as 2 pi (u2 - 1/2) in [-pi, pi), where the
+// MUFU error bound holds, and the sign flip cos(x - pi) = -cos x is folded into the radius.
 template <int MATH>
-__device__ __forceinline__ void box_muller(uint32_t ra, uint32_t rb, float& z0, float& z1)
+__device__ __forceinline__ void perturb_pair(uint32_t ra, uint32_t rb, float sigma, float una, float unb,
+                                             float& a, float& b)
 {
-    const float u1 = u01(ra), u2 = u01(rb);
     if (MATH == 0) {
+        const float u1 = u01(ra), u2 = u01(rb);
         const float rad = sqrtf(-2.0f * logf(u1));
         float s, c;
         sincospif(2.0f * u2, &s, &c);
-        z0 = rad * c;
-        z1 = rad * s;
+        a = fmaf(sigma, rad * c, una);
+        b = fmaf(sigma, rad * s, unb);
     } else {
-        // -2 ln u = (-2 ln 2) log2 u
-        const float rad = sqrtf(-1.3862943611198906f * __log2f(u1));
-        float s, c;
-        __sincosf(6.283185307179586f * u2, &s, &c);
-        z0 = rad * c;
-        z1 = rad * s;
+        const float u1 = u01(ra);
+        const float t = -1.3862943611198906f * mufu_lg2(u1);          // -2 ln u1 > 0
+        const float nrad = (t * -sigma) * mufu_rsq(t);                // -sigma sqrt(t)
+        const float w = __uint_as_float(0x3f800000u | (rb >> 9)) - 1.5f;   // u2 - 1/2 - 2^-24, exact
+        const float ang = fmaf(w, 6.283185307179586f, 3.7450704e-7f);      // 2 pi (u2 - 1/2) in [-pi, pi)
+        a = fmaf(nrad, mufu_cos(ang), una);
+        b = fmaf(nrad, mufu_sin(ang), unb);
     }
 }
 
-// Perturbed, clamped rotor thrusts of one (sample, step) and the perturbation actually applied
-// [R-8]: T = clamp(u_nom + sigma z), dU = T - u_nom.
+// Perturbed, clamped rotor thrusts of one (sample, step) [R-8]: T = clamp(u_nom + sigma z).
+// The perturbation actually applied is dU = T - u_nom (formed by the callers that need it).
 template <int MATH>
-__device__ __forceinline__ void sample_thrust(const DevParams& P, uint32_t seed_lo, uint32_t seed_hi,
-                                              uint32_t k, uint32_t t, uint32_t iter, uint32_t b,
-                                              const float4 un, float4& T, float4& du)
+__device__ __forceinline__ float4 sample_thrust(const DevParams& P, const uint32_t (&rk)[20], uint32_t k,
+                                                uint32_t t, uint32_t iter, uint32_t b, const float4 un)
 {
-    const uint4 r = philox4x32_10(k, t, iter, b, seed_lo, seed_hi);
-    float z0, z1, z2, z3;
-    box_muller<MATH>(r.x, r.y, z0, z1);
-    box_muller<MATH>(r.z, r.w, z2, z3);
-    T.x = fminf(fmaxf(fmaf(P.sigma, z0, un.x), P.T_min), P.T_max);
-    T.y = fminf(fmaxf(fmaf(P.sigma, z1, un.y), P.T_min), P.T_max);
-    T.z = fminf(fmaxf(fmaf(P.sigma, z2, un.z), P.T_min), P.T_max);
-    T.w = fminf(fmaxf(fmaf(P.sigma, z3, un.w), P.T_min), P.T_max);
-    du = make_float4(T.x - un.x, T.y - un.y, T.z - un.z, T.w - un.w);
+    const uint4 r = philox4x32_10(k, t, iter, b, rk);
+    float4 T;
+    perturb_pair<MATH>(r.x, r.y, P.sigma, un.x, un.y, T.x, T.y);
+    perturb_pair<MATH>(r.z, r.w, P.sigma, un.z, un.w, T.z, T.w);
+    T.x = fminf(fmaxf(T.x, P.T_min), P.T_max);
+    T.y = fminf(fmaxf(T.y, P.T_min), P.T_max);
+    T.z = fminf(fmaxf(T.z, P.T_min), P.T_max);
+    T.w = fminf(fmaxf(T.w, P.T_min), P.T_max);
+    return T;
 }
 
 // ---- quadrotor state and dynamics, eq.(2) PAPER.md:65-72 -------------------------------------
@@ -115,72 +130,85 @@ struct State {
     float ox, oy, oz;
 };
 
-// The part of f_dyn that depends on the state: q_dot, v_dot, omega_dot (p_dot = v is used
-// directly).  Per-step constants (thrust-derived) are hoisted by the caller:
-//   c2 = 2 S/m, cz0 = S/m - g, (ax, ay, az) = J^-1 tau.
-struct Deriv { float qw, qx, qy, qz, vx, vy, vz, ox, oy, oz; };
-
-__device__ __forceinline__ Deriv f_dyn(const DevParams& P, float qw, float qx, float qy, float qz,
-                                       float ox, float oy, float oz, float c2, float cz0, float ax,
-                                       float ay, float az)
-{
-    Deriv d;
-    // q_dot = 1/2 q (x) (0, omega)                              (Hamilton product, body rates)
-    d.qw = 0.5f * (-qx * ox - qy * oy - qz * oz);
-    d.qx = 0.5f * (qw * ox + qy * oz - qz * oy);
-    d.qy = 0.5f * (qw * oy + qz * ox - qx * oz);
-    d.qz = 0.5f * (qw * oz + qx * oy - qy * ox);
-    // v_dot = g + R(q) [0 0 S]^T / m : third column of R(q)
-    d.vx = c2 * (qx * qz + qw * qy);
-    d.vy = c2 * (qy * qz - qw * qx);
-    d.vz = cz0 - c2 * (qx * qx + qy * qy);
-    // omega_dot = J^-1 (tau - omega x J omega), diagonal J
-    d.ox = fmaf(P.gyx, oy * oz, ax);
-    d.oy = fmaf(P.gyy, oz * ox, ay);
-    d.oz = fmaf(P.gyz, ox * oy, az);
-    return d;
-}
-
 // x <- RK4(f_dyn, x, T, dt), then q <- q / |q|   [R-4],[R-5]; input held over the step.
+//
+// f_dyn (eq.(2)) has a triangular structure that the step exploits to cut the instruction count:
+//   omega_dot depends on omega only           -> its four stages form their own chain
+//   q_dot = 1/2 G(q, omega), G = q (x) (0,w)  -> the 1/2 is folded into the step constants
+//   v_dot = (c2 r_x, c2 r_y, cz0 - c2 r_z), r(q) = (qx qz + qw qy, qy qz - qw qx, qx^2 + qy^2),
+//           c2 = 2 S/m, cz0 = S/m - g         -> only r(q_i) is evaluated per stage
+//   p_dot = v                                 -> p_new = p + h v + h^2/6 (a1 + a2 + a3),
+//                                                v_new = v + h/6 (a1 + 2 a2 + 2 a3 + a4)
+// which is the classical RK4 written out (the v stages never need to be formed).
 __device__ __forceinline__ void rk4_step(const DevParams& P, State& x, const float4 T)
 {
-    const float S = (T.x + T.y) + (T.z + T.w);
-    const float c = S * P.inv_mass;
-    const float c2 = 2.0f * c, cz0 = c - P.g;
-    const float ax = P.ltx * ((T.x + T.y) - (T.z + T.w));     // tau_x / Jx
-    const float ay = P.lty * ((T.y + T.z) - (T.x + T.w));     // tau_y / Jy
-    const float az = P.ltz * ((T.x + T.z) - (T.y + T.w));     // tau_z / Jz
-    const float h = P.dt, h2 = 0.5f * P.dt, h6 = P.dt * (1.0f / 6.0f);
+    const float s01 = T.x + T.y, s23 = T.z + T.w;
+    const float c = (s01 + s23) * P.inv_mass;                  // S / m
+    const float ax = P.ltx * (s01 - s23);                      // tau_x / Jx
+    const float ay = P.lty * ((T.y + T.z) - (T.x + T.w));      // tau_y / Jy
+    const float az = P.ltz * ((T.x + T.z) - (T.y + T.w));      // tau_z / Jz
+    const float cz0 = c - P.g;
+    const float kp = c * P.hh3, kv = c * P.h3;                 // h^2/6 c2, h/6 c2
 
-    const Deriv k1 = f_dyn(P, x.qw, x.qx, x.qy, x.qz, x.ox, x.oy, x.oz, c2, cz0, ax, ay, az);
-    const float v2x = fmaf(h2, k1.vx, x.vx), v2y = fmaf(h2, k1.vy, x.vy), v2z = fmaf(h2, k1.vz, x.vz);
-    const Deriv k2 = f_dyn(P, fmaf(h2, k1.qw, x.qw), fmaf(h2, k1.qx, x.qx), fmaf(h2, k1.qy, x.qy),
-                           fmaf(h2, k1.qz, x.qz), fmaf(h2, k1.ox, x.ox), fmaf(h2, k1.oy, x.oy),
-                           fmaf(h2, k1.oz, x.oz), c2, cz0, ax, ay, az);
-    const float v3x = fmaf(h2, k2.vx, x.vx), v3y = fmaf(h2, k2.vy, x.vy), v3z = fmaf(h2, k2.vz, x.vz);
-    const Deriv k3 = f_dyn(P, fmaf(h2, k2.qw, x.qw), fmaf(h2, k2.qx, x.qx), fmaf(h2, k2.qy, x.qy),
-                           fmaf(h2, k2.qz, x.qz), fmaf(h2, k2.ox, x.ox), fmaf(h2, k2.oy, x.oy),
-                           fmaf(h2, k2.oz, x.oz), c2, cz0, ax, ay, az);
-    const float v4x = fmaf(h, k3.vx, x.vx), v4y = fmaf(h, k3.vy, x.vy), v4z = fmaf(h, k3.vz, x.vz);
-    const Deriv k4 = f_dyn(P, fmaf(h, k3.qw, x.qw), fmaf(h, k3.qx, x.qx), fmaf(h, k3.qy, x.qy),
-                           fmaf(h, k3.qz, x.qz), fmaf(h, k3.ox, x.ox), fmaf(h, k3.oy, x.oy),
-                           fmaf(h, k3.oz, x.oz), c2, cz0, ax, ay, az);
+    // ---- stage 1 (state x)
+    float kox = fmaf(P.gyx, x.oy * x.oz, ax), koy = fmaf(P.gyy, x.oz * x.ox, ay), koz = fmaf(P.gyz, x.ox * x.oy, az);
+    float gw = fmaf(-x.qz, x.oz, fmaf(-x.qy, x.oy, -x.qx * x.ox));
+    float gx = fmaf(-x.qz, x.oy, fmaf(x.qy, x.oz, x.qw * x.ox));
+    float gy = fmaf(-x.qx, x.oz, fmaf(x.qz, x.ox, x.qw * x.oy));
+    float gz = fmaf(-x.qy, x.ox, fmaf(x.qx, x.oy, x.qw * x.oz));
+    const float r1x = fmaf(x.qw, x.qy, x.qx * x.qz), r1y = fmaf(-x.qw, x.qx, x.qy * x.qz),
+                r1z = fmaf(x.qy, x.qy, x.qx * x.qx);
+    float no_x = fmaf(P.h6, kox, x.ox), no_y = fmaf(P.h6, koy, x.oy), no_z = fmaf(P.h6, koz, x.oz);
+    float nw = fmaf(P.h12, gw, x.qw), nx = fmaf(P.h12, gx, x.qx), ny = fmaf(P.h12, gy, x.qy), nz = fmaf(P.h12, gz, x.qz);
+    float ox = fmaf(P.h2, kox, x.ox), oy = fmaf(P.h2, koy, x.oy), oz = fmaf(P.h2, koz, x.oz);
+    float qw = fmaf(P.h4, gw, x.qw), qx = fmaf(P.h4, gx, x.qx), qy = fmaf(P.h4, gy, x.qy), qz = fmaf(P.h4, gz, x.qz);
 
-    // x + dt/6 (k1 + 2 k2 + 2 k3 + k4); p_dot stage values are v, v2, v3, v4
-    x.px = fmaf(h6, (x.vx + v4x) + 2.0f * (v2x + v3x), x.px);
-    x.py = fmaf(h6, (x.vy + v4y) + 2.0f * (v2y + v3y), x.py);
-    x.pz = fmaf(h6, (x.vz + v4z) + 2.0f * (v2z + v3z), x.pz);
-    x.vx = fmaf(h6, (k1.vx + k4.vx) + 2.0f * (k2.vx + k3.vx), x.vx);
-    x.vy = fmaf(h6, (k1.vy + k4.vy) + 2.0f * (k2.vy + k3.vy), x.vy);
-    x.vz = fmaf(h6, (k1.vz + k4.vz) + 2.0f * (k2.vz + k3.vz), x.vz);
-    x.ox = fmaf(h6, (k1.ox + k4.ox) + 2.0f * (k2.ox + k3.ox), x.ox);
-    x.oy = fmaf(h6, (k1.oy + k4.oy) + 2.0f * (k2.oy + k3.oy), x.oy);
-    x.oz = fmaf(h6, (k1.oz + k4.oz) + 2.0f * (k2.oz + k3.oz), x.oz);
-    const float nw = fmaf(h6, (k1.qw + k4.qw) + 2.0f * (k2.qw + k3.qw), x.qw);
-    const float nx = fmaf(h6, (k1.qx + k4.qx) + 2.0f * (k2.qx + k3.qx), x.qx);
-    const float ny = fmaf(h6, (k1.qy + k4.qy) + 2.0f * (k2.qy + k3.qy), x.qy);
-    const float nz = fmaf(h6, (k1.qz + k4.qz) + 2.0f * (k2.qz + k3.qz), x.qz);
-    const float inv = rsqrtf(nw * nw + nx * nx + ny * ny + nz * nz);
+    // ---- stage 2
+    kox = fmaf(P.gyx, oy * oz, ax); koy = fmaf(P.gyy, oz * ox, ay); koz = fmaf(P.gyz, ox * oy, az);
+    gw = fmaf(-qz, oz, fmaf(-qy, oy, -qx * ox));
+    gx = fmaf(-qz, oy, fmaf(qy, oz, qw * ox));
+    gy = fmaf(-qx, oz, fmaf(qz, ox, qw * oy));
+    gz = fmaf(-qy, ox, fmaf(qx, oy, qw * oz));
+    const float r2x = fmaf(qw, qy, qx * qz), r2y = fmaf(-qw, qx, qy * qz), r2z = fmaf(qy, qy, qx * qx);
+    no_x = fmaf(P.h3, kox, no_x); no_y = fmaf(P.h3, koy, no_y); no_z = fmaf(P.h3, koz, no_z);
+    nw = fmaf(P.h6, gw, nw); nx = fmaf(P.h6, gx, nx); ny = fmaf(P.h6, gy, ny); nz = fmaf(P.h6, gz, nz);
+    ox = fmaf(P.h2, kox, x.ox); oy = fmaf(P.h2, koy, x.oy); oz = fmaf(P.h2, koz, x.oz);
+    qw = fmaf(P.h4, gw, x.qw); qx = fmaf(P.h4, gx, x.qx); qy = fmaf(P.h4, gy, x.qy); qz = fmaf(P.h4, gz, x.qz);
+
+    // ---- stage 3
+    kox = fmaf(P.gyx, oy * oz, ax); koy = fmaf(P.gyy, oz * ox, ay); koz = fmaf(P.gyz, ox * oy, az);
+    gw = fmaf(-qz, oz, fmaf(-qy, oy, -qx * ox));
+    gx = fmaf(-qz, oy, fmaf(qy, oz, qw * ox));
+    gy = fmaf(-qx, oz, fmaf(qz, ox, qw * oy));
+    gz = fmaf(-qy, ox, fmaf(qx, oy, qw * oz));
+    const float r3x = fmaf(qw, qy, qx * qz), r3y = fmaf(-qw, qx, qy * qz), r3z = fmaf(qy, qy, qx * qx);
+    no_x = fmaf(P.h3, kox, no_x); no_y = fmaf(P.h3, koy, no_y); no_z = fmaf(P.h3, koz, no_z);
+    nw = fmaf(P.h6, gw, nw); nx = fmaf(P.h6, gx, nx); ny = fmaf(P.h6, gy, ny); nz = fmaf(P.h6, gz, nz);
+    ox = fmaf(P.dt, kox, x.ox); oy = fmaf(P.dt, koy, x.oy); oz = fmaf(P.dt, koz, x.oz);
+    qw = fmaf(P.h2, gw, x.qw); qx = fmaf(P.h2, gx, x.qx); qy = fmaf(P.h2, gy, x.qy); qz = fmaf(P.h2, gz, x.qz);
+
+    // ---- stage 4
+    kox = fmaf(P.gyx, oy * oz, ax); koy = fmaf(P.gyy, oz * ox, ay); koz = fmaf(P.gyz, ox * oy, az);
+    gw = fmaf(-qz, oz, fmaf(-qy, oy, -qx * ox));
+    gx = fmaf(-qz, oy, fmaf(qy, oz, qw * ox));
+    gy = fmaf(-qx, oz, fmaf(qz, ox, qw * oy));
+    gz = fmaf(-qy, ox, fmaf(qx, oy, qw * oz));
+    const float r4x = fmaf(qw, qy, qx * qz), r4y = fmaf(-qw, qx, qy * qz), r4z = fmaf(qy, qy, qx * qx);
+    x.ox = fmaf(P.h6, kox, no_x); x.oy = fmaf(P.h6, koy, no_y); x.oz = fmaf(P.h6, koz, no_z);
+    nw = fmaf(P.h12, gw, nw); nx = fmaf(P.h12, gx, nx); ny = fmaf(P.h12, gy, ny); nz = fmaf(P.h12, gz, nz);
+
+    // ---- translation: A = r1 + r2 + r3, Bv = r1 + 2 r2 + 2 r3 + r4
+    const float mx = r2x + r3x, my = r2y + r3y, mz = r2z + r3z;
+    const float Ax = r1x + mx, Ay = r1y + my, Az = r1z + mz;
+    x.px = fmaf(kp, Ax, fmaf(P.dt, x.vx, x.px));
+    x.py = fmaf(kp, Ay, fmaf(P.dt, x.vy, x.py));
+    x.pz = fmaf(-kp, Az, fmaf(P.hh2, cz0, fmaf(P.dt, x.vz, x.pz)));
+    x.vx = fmaf(kv, (Ax + mx) + r4x, x.vx);
+    x.vy = fmaf(kv, (Ay + my) + r4y, x.vy);
+    x.vz = fmaf(-kv, (Az + mz) + r4z, fmaf(P.dt, cz0, x.vz));
+
+    // ---- renormalise once per step [R-5]
+    const float inv = rsqrtf(fmaf(nz, nz, fmaf(ny, ny, fmaf(nx, nx, nw * nw))));
     x.qw = nw * inv; x.qx = nx * inv; x.qy = ny * inv; x.qz = nz * inv;
 }
 

@@ -112,7 +112,7 @@ __global__ void rollout_kernel(const DevParams P, const StepArgs A)
     float J = 0.0f;
     GateCost gc;
     ContourCost cc;
-    if (OBJ == OBJ_GATE) gc.init(P, s_trk, start, x);
+    if (OBJ == OBJ_GATE) gc.init<MATH>(P, s_trk, start, x);
     if (OBJ == OBJ_CONTOUR) {
         int i0;
         if (start < 0) {
@@ -151,15 +151,16 @@ __global__ void rollout_kernel(const DevParams P, const StepArgs A)
     // ---- the horizon: noise -> clamp -> RK4 -> cost, all in registers (Alg. 1 lines 6-13) ----
     float4* du_out = STORE_DU ? A.du + (size_t)b * N * P.K + k : nullptr;
     for (int t = 0; t < N; ++t) {
-        float4 T, du;
-        sample_thrust<MATH>(P, A.seed_lo, A.seed_hi, (uint32_t)k, (uint32_t)t, A.iter, (uint32_t)b,
-                            s_unom[t], T, du);
-        if (STORE_DU) du_out[(size_t)t * P.K] = du;       // one coalesced 16-B store per thread
+        const float4 un = s_unom[t];
+        const float4 T = sample_thrust<MATH>(P, A.rk, (uint32_t)k, (uint32_t)t, A.iter, (uint32_t)b, un);
+        if (STORE_DU)                                      // one coalesced 16-B store per thread
+            du_out[(size_t)t * P.K] = make_float4(T.x - un.x, T.y - un.y, T.z - un.z, T.w - un.w);
         if (OBJ == OBJ_TRACK) J += track_stage(P, s_trk + 4 * t, x, T);
         rk4_step(P, x, T);
-        if (OBJ == OBJ_GATE) J += gc.step(P, s_trk, x);
+        if (OBJ == OBJ_GATE) gc.step<MATH>(P, s_trk, x);
         if (OBJ == OBJ_CONTOUR) J += cc.step(P, s_trk, x);
     }
+    if (OBJ == OBJ_GATE) J = gc.finish<MATH>(P, s_trk, x);
     if (OBJ == OBJ_TRACK) J += track_state_term(P, s_trk + 4 * N, x);
     A.cost[(size_t)b * P.K + k] = J;
 
@@ -184,11 +185,9 @@ __global__ void rollout_kernel(const DevParams P, const StepArgs A)
                 const int l = __ffs(mm) - 1;
                 mm &= mm - 1;
                 const float el = __shfl_sync(kFull, e, l);
-                float4 T, du;
-                sample_thrust<MATH>(P, A.seed_lo, A.seed_hi, kbase + l, (uint32_t)t, A.iter,
-                                    (uint32_t)b, un, T, du);
-                acc.x = fmaf(el, du.x, acc.x); acc.y = fmaf(el, du.y, acc.y);
-                acc.z = fmaf(el, du.z, acc.z); acc.w = fmaf(el, du.w, acc.w);
+                const float4 T = sample_thrust<MATH>(P, A.rk, kbase + l, (uint32_t)t, A.iter, (uint32_t)b, un);
+                acc.x = fmaf(el, T.x - un.x, acc.x); acc.y = fmaf(el, T.y - un.y, acc.y);
+                acc.z = fmaf(el, T.z - un.z, acc.z); acc.w = fmaf(el, T.w - un.w, acc.w);
             }
             if (t < N) s_acc[warp * N + t] = acc;
         }
@@ -304,9 +303,9 @@ __global__ void sim_kernel(const DevParams P, float* __restrict__ xs, int* __res
         const float4 T = reinterpret_cast<const float4*>(u_new)[(size_t)b * N];
         if (OBJ == OBJ_GATE) {
             GateCost gc;
-            gc.init(P, P.gates, start[b], x);
+            gc.init<0>(P, P.gates, start[b], x);
             rk4_step(P, x, T);
-            (void)gc.step(P, P.gates, x);
+            gc.step<0>(P, P.gates, x);
             start[b] = gc.gate;
         } else if (OBJ == OBJ_TRACK) {
             rk4_step(P, x, T);

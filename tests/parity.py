@@ -14,6 +14,7 @@ W_ATOL = 1e-5
 U_ATOL = 1e-4
 MARGIN = 1e-5
 
+STATS: list[str] = []           # one line per compared iteration: achieved errors
 REPORT: list[str] = []          # "reported separately" lines, printed at the end of the session
 
 
@@ -85,5 +86,7 @@ def compare(tag, g, o, lam, gate_objective):
             assert np.abs(g["u_new"] - u_self).max() <= U_ATOL, f"{tag}: u_new inconsistent with its weights"
         REPORT.append(f"{tag}: near-tied minimum (sensitivity {sens:.2e}, flagged-decided {decided_by_flagged}): "
                       f"weights err {werr:.2e}, u_new err {uerr:.2e} reported separately")
-    return dict(cost_rel=float(err[~flagged].max()) if (~flagged).any() else 0.0, w=werr, u=uerr,
-                flagged=n_flag, ess=float(1.0 / (wo ** 2).sum(-1).min()))
+    st = dict(cost_rel=float(err[~flagged].max()) if (~flagged).any() else 0.0, w=werr, u=uerr,
+              flagged=n_flag, ess=float(1.0 / (wo ** 2).sum(-1).min()))
+    STATS.append(f"{tag}: cost rel {st['cost_rel']:.2e}  weights {werr:.2e}  u_new {uerr:.2e}  ESS {st['ess']:.1f}  flagged {n_flag}")
+    return st

@@ -13,6 +13,11 @@ pytestmark = pytest.mark.gpu
 @pytest.fixture(scope="module", autouse=True)
 def _report():
     yield
+    import os
+    out = os.path.join(os.path.dirname(__file__), "..", "gpurun_out")
+    if os.path.isdir(out) and Pz.STATS:
+        with open(os.path.join(out, "parity_stats.txt"), "w") as f:
+            f.write("\n".join(Pz.STATS + ["", "reported separately:"] + Pz.REPORT) + "\n")
     if Pz.REPORT:
         print("\n[parity] reported separately:\n  " + "\n  ".join(Pz.REPORT))
 
