@@ -74,6 +74,14 @@ typedef enum {
                               min / exp-weight / weighted-sum kernel reads it back              */
 } mppi_pipeline;
 
+typedef enum {
+    MPPI_VARIANT_AUTO = 0,       /* latency kernel when B*K/32 warps cannot fill the chip, else throughput */
+    MPPI_VARIANT_THROUGHPUT = 1, /* one sample per thread, noise drawn inside the horizon loop; block_threads
+                                    samples per block                                                      */
+    MPPI_VARIANT_LATENCY = 2     /* 256-thread blocks: all warps draw the noise of 32 C samples into shared
+                                    memory first, then C warps (C = 1, 2 or 4) roll out; fused pipeline only */
+} mppi_variant;
+
 /* Parameters of Alg. 1 (samples, horizon, lambda, Sigma) plus the model and cost
  * constants of BASELINE.json configs[0..3].  struct_size = sizeof(mppi_params) versions the ABI. */
 typedef struct {
@@ -104,6 +112,7 @@ typedef struct {
                           the Box-Muller transform (error budget)                 */
     int32_t store_noise; /* 1: also keep dU of the last step for mppi_debug_noise (always kept
                             in the TWO_PASS pipeline)                                            */
+    int32_t variant;   /* mppi_variant: which rollout kernel the fused pipeline launches          */
 } mppi_params;
 
 #define MPPI_MAX_N 256

@@ -16,6 +16,7 @@ LIB_PATH = _HERE / "libmppi.so"
 
 OBJ_GATE, OBJ_TRACK, OBJ_CONTOUR = 0, 1, 2
 PIPE_FUSED, PIPE_TWO_PASS = 0, 1
+VARIANT_AUTO, VARIANT_THROUGHPUT, VARIANT_LATENCY = 0, 1, 2
 
 EXPORTS = ["mppi_default_params", "mppi_create", "mppi_destroy", "mppi_set_gates",
            "mppi_set_reference", "mppi_set_path", "mppi_step", "mppi_optimize", "mppi_step_host",
@@ -35,7 +36,7 @@ class MppiParams(C.Structure):
                 ("R", C.c_float), ("q_contour", C.c_float), ("q_lag", C.c_float),
                 ("mu_progress", C.c_float), ("window", C.c_int32), ("pipeline", C.c_int32),
                 ("use_graph", C.c_int32), ("block_threads", C.c_int32), ("fast_math", C.c_int32),
-                ("store_noise", C.c_int32)]
+                ("store_noise", C.c_int32), ("variant", C.c_int32)]
 
 
 class MppiInfo(C.Structure):

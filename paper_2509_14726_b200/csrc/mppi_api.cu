@@ -90,7 +90,7 @@ extern "C" int mppi_default_params(mppi_params* p)
     p->q_contour = 200.0f; p->q_lag = 50.0f; p->mu_progress = 2.0f;
     p->window = 16;
     p->pipeline = MPPI_PIPE_FUSED; p->use_graph = 0; p->block_threads = 0; p->fast_math = 0;
-    p->store_noise = 0;
+    p->store_noise = 0; p->variant = MPPI_VARIANT_AUTO;
     return MPPI_OK;
 }
 
@@ -117,20 +117,34 @@ static int validate(const mppi_params* p)
                                   p->K % p->block_threads != 0),
         "block_threads must be 0 or a multiple of 32 in 32..256 that divides K");
     BAD((int64_t)p->K / 32 > 65535, "K too large");
+    BAD(p->variant < 0 || p->variant > 2, "unknown variant");
+    BAD(p->variant == MPPI_VARIANT_LATENCY && p->pipeline != MPPI_PIPE_FUSED, "the latency variant needs the fused pipeline");
 #undef BAD
     return MPPI_OK;
 }
 
-static int pick_block(const mppi_params* p, int sm_count)
+// Launch shape.  Latency variant: C rollout warps per 256-thread block, the smallest C in {1,2,4}
+// that brings the grid down to one block per SM (so every rollout warp owns a scheduler).
+// Throughput variant: 256-thread blocks when the grid still covers the chip several times, else 128.
+static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, int* lat_consumers)
 {
-    if (p->block_threads) return p->block_threads;
-    // Enough resident work to fill the chip -> 128-thread blocks (4 warps, one per scheduler);
-    // a lone controller is latency-bound: still 128 so that only K/128 partials meet in the
-    // last-block combine, unless K is too small to divide.
+    const int64_t warps = (int64_t)p->B * p->K / 32;
+    *lat_consumers = 0;
+    const bool lat_ok = p->pipeline == MPPI_PIPE_FUSED && p->block_threads == 0;
+    if (lat_ok && (p->variant == MPPI_VARIANT_LATENCY || (p->variant == MPPI_VARIANT_AUTO && warps <= 4 * (int64_t)sm_count))) {
+        int best = 0;
+        for (int c : {1, 2, 4})
+            if (p->K % (32 * c) == 0) {
+                best = c;
+                if (warps / c <= sm_count) break;
+            }
+        if (best) { *lat_consumers = best; *block_threads = 256; return; }
+    }
+    if (p->block_threads) { *block_threads = p->block_threads; return; }
+    if (p->K % 256 == 0 && warps >= 16 * (int64_t)sm_count) { *block_threads = 256; return; }
     for (int tpb : {128, 64, 32})
-        if (p->K % tpb == 0) return tpb;
-    (void)sm_count;
-    return 32;
+        if (p->K % tpb == 0) { *block_threads = tpb; return; }
+    *block_threads = 32;
 }
 
 static void free_graph(GraphSlot& g)
@@ -203,8 +217,8 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     cfg.objective = p->objective; cfg.fast_math = p->fast_math ? 1 : 0;
     cfg.fused = p->pipeline == MPPI_PIPE_FUSED;
     cfg.store_du = (!cfg.fused || p->store_noise) ? 1 : 0;
-    cfg.block_threads = pick_block(p, c->sm_count);
-    d.blocks_per_ctrl = p->K / cfg.block_threads;
+    pick_shape(p, c->sm_count, &cfg.block_threads, &cfg.lat_consumers);
+    d.blocks_per_ctrl = cfg.lat_consumers ? p->K / (32 * cfg.lat_consumers) : p->K / cfg.block_threads;
     cfg.smem_bytes = 0;   // fixed once the track is known
 
     const size_t BN4 = (size_t)p->B * p->N * 4, BK = (size_t)p->B * p->K;
@@ -417,7 +431,8 @@ static int graph_run(mppi_ctx* c, GraphSlot& g, const std::vector<StepArgs>& arg
     cudaGraphNode_t prev = nullptr;
     for (int i = 0; i < n; ++i) {
         StepArgs a = args[i];
-        void* kp[2] = {&dp, &a};
+        int lat_c = c->cfg.lat_consumers;
+        void* kp[3] = {&dp, &a, &lat_c};
         cudaKernelNodeParams np;
         for (int pass = 0; pass < (c->cfg.fused ? 1 : 2); ++pass) {
             node_params(c, pass == 1, kp, &np);

@@ -1,81 +1,52 @@
 // mppi_kernels.cu -- the sm_100a kernels of the MPPI hot path.
 //
-//   rollout_kernel<OBJ, MATH, STORE_DU, FUSED>   SURVEY.md 8(a) steps 1-4 (+5-7 when FUSED)
+//   rollout_kernel<OBJ, MATH, STORE_DU, FUSED>   SURVEY.md 8(a) steps 1-4 (+5-7 when FUSED), one sample
+//                                                per thread, noise drawn in the horizon loop (throughput)
+//   rollout_lat_kernel<OBJ, MATH, STORE_DU>      the same iteration for a lone controller (latency):
+//                                                all warps draw the noise first, few warps roll out
 //   reduce_kernel                                steps 5-7 of the TWO_PASS pipeline
 //   sim_kernel                                   step 8 (closed-loop glue)
 //
-// Thread mapping: one sample per thread, block = blockDim.x consecutive samples of ONE
-// controller, grid = (K / blockDim.x, B).  No tensor cores: nothing here is a contraction.
-#include "mppi_cost.cuh"
+// No tensor cores: nothing here is a contraction.
 #include "mppi_internal.h"
+#include "mppi_rollout.cuh"
 
 namespace mppi {
 
-constexpr unsigned kFull = 0xffffffffu;
-
-__device__ __forceinline__ float warp_min(float v)
-{
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(kFull, v, o));
-    return v;
-}
-__device__ __forceinline__ float warp_sum(float v)
-{
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
-    return v;
-}
-
-template <int MATH>
-__device__ __forceinline__ float exp_weight(float x)   // exp(x), x <= 0
-{
-    return MATH == 0 ? expf(x) : __expf(x);
-}
-
-// block-wide min / sum over blockDim.x threads through s_red[0..31]; every thread gets the result
-__device__ __forceinline__ float block_min(float v, float* s_red)
-{
-    v = warp_min(v);
-    __syncthreads();
-    if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = v;
-    __syncthreads();
-    const int nw = blockDim.x >> 5;
-    float r = s_red[0];
-    for (int w = 1; w < nw; ++w) r = fminf(r, s_red[w]);
-    return r;
-}
-__device__ __forceinline__ float block_sum(float v, float* s_red)
-{
-    v = warp_sum(v);
-    __syncthreads();
-    if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = v;
-    __syncthreads();
-    const int nw = blockDim.x >> 5;
-    float r = s_red[0];
-    for (int w = 1; w < nw; ++w) r += s_red[w];      // fixed order: deterministic
-    return r;
-}
-
-// Shared-memory carve-up of the rollout kernel (units: float4).
+// Shared-memory carve-up of rollout_kernel (units: float4).
 //   [0, N)                         nominal thrusts u_nom[b]
 //   [N, N + trk)                   track data of the objective
 //   then 16 float4                 reduction scratch (64 floats)
 //   FUSED: nwarps * N float4       per-warp weighted-noise accumulators
-//   FUSED: ceil(nblk/4) float4     per-block rescale factors of the last-block combine
-__host__ __device__ inline int track_f4(const DevParams& P, int objective)
-{
-    return objective == OBJ_GATE ? 4 * P.G : objective == OBJ_TRACK ? 4 * (P.N + 1) : 2 * P.P;
-}
-
+//   FUSED: ceil(2 nblk / 4) float4 (min, Z) pairs / rescale factors of the last-block combine
 size_t rollout_smem_bytes(const DevParams& P, const LaunchCfg& c)
 {
     size_t f4 = (size_t)P.N + track_f4(P, c.objective) + 16;
-    if (c.fused) f4 += (size_t)(c.block_threads / 32) * P.N + (P.blocks_per_ctrl + 3) / 4;
+    if (c.lat_consumers > 0) {
+        f4 += (size_t)P.N * (32 * c.lat_consumers + 1) + 32 + (2 * P.blocks_per_ctrl + 3) / 4;
+        return f4 * sizeof(float4);
+    }
+    if (c.fused) f4 += (size_t)(c.block_threads / 32) * P.N + (2 * P.blocks_per_ctrl + 3) / 4;
     return f4 * sizeof(float4);
 }
 
+// thrust source of the throughput kernel: draw (k, t) in place
+template <int MATH, bool STORE_DU>
+struct DrawThrust {
+    const DevParams& P; const StepArgs& A; const float4* s_unom; uint32_t k, b; float4* du_out;
+    __device__ __forceinline__ float4 operator()(int t) const
+    {
+        const float4 un = s_unom[t];
+        const float4 T = sample_thrust<MATH>(P, A.rk, k, (uint32_t)t, A.iter, b, un);
+        if (STORE_DU)                                      // one coalesced 16-B store per thread
+            du_out[(size_t)t * P.K] = make_float4(T.x - un.x, T.y - un.y, T.z - un.z, T.w - un.w);
+        return T;
+    }
+};
+
 // ---------------------------------------------------------------------------------------------
-// rollout + cost (+ fused softmax partials and last-block combine)
+// throughput variant: rollout + cost (+ fused softmax partials and last-block combine)
+// grid = (K / blockDim.x, B), one sample per thread
 // ---------------------------------------------------------------------------------------------
 template <int OBJ, int MATH, bool STORE_DU, bool FUSED>
 __global__ void rollout_kernel(const DevParams P, const StepArgs A)
@@ -90,78 +61,17 @@ __global__ void rollout_kernel(const DevParams P, const StepArgs A)
     float4* s_trk = smem + N;
     float* s_red = reinterpret_cast<float*>(s_trk + track_f4(P, OBJ));   // 64 floats
     float4* s_acc = reinterpret_cast<float4*>(s_red + 64);
-    float* s_scale = reinterpret_cast<float*>(s_acc + (blockDim.x >> 5) * N);
+    float* s_pair = reinterpret_cast<float*>(s_acc + (blockDim.x >> 5) * N);
 
-    // ---- stage the nominal sequence and the track in shared memory ----
     const int start = A.start[b];
-    {
-        const float4* un = reinterpret_cast<const float4*>(A.u_nom) + (size_t)b * N;
-        for (int t = tid; t < N; t += blockDim.x) s_unom[t] = un[t];
-        if (OBJ == OBJ_GATE) {
-            for (int i = tid; i < 4 * P.G; i += blockDim.x) s_trk[i] = P.gates[i];
-        } else if (OBJ == OBJ_TRACK) {
-            const int t0 = min(max(start, 0), P.M - 1 - N);
-            for (int i = tid; i < 4 * (N + 1); i += blockDim.x) s_trk[i] = P.ref[4 * t0 + i];
-        } else {
-            for (int i = tid; i < 2 * P.P; i += blockDim.x) s_trk[i] = P.path[i];
-        }
-    }
+    stage_inputs<OBJ>(P, A, b, start, s_unom, s_trk);
     __syncthreads();
 
-    State x = load_state(A.x0 + 13 * b);
-    float J = 0.0f;
-    GateCost gc;
-    ContourCost cc;
-    if (OBJ == OBJ_GATE) gc.init<MATH>(P, s_trk, start, x);
-    if (OBJ == OBJ_CONTOUR) {
-        int i0;
-        if (start < 0) {
-            // global nearest vertex, block-cooperative; ties -> smallest index (scan order)
-            float best = __int_as_float(0x7f800000);
-            int ib = 0x7fffffff;
-            for (int i = tid; i < P.P; i += blockDim.x) {
-                const float4 q = s_trk[2 * i];
-                const float dx = x.px - q.x, dy = x.py - q.y, dz = x.pz - q.z;
-                const float d2 = dx * dx + dy * dy + dz * dz;
-                if (d2 < best) { best = d2; ib = i; }
-            }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                const float ob = __shfl_xor_sync(kFull, best, o);
-                const int oi = __shfl_xor_sync(kFull, ib, o);
-                if (ob < best || (ob == best && oi < ib)) { best = ob; ib = oi; }
-            }
-            if (lane == 0) { s_red[warp] = best; reinterpret_cast<int*>(s_red)[32 + warp] = ib; }
-            __syncthreads();
-            best = s_red[0]; ib = reinterpret_cast<int*>(s_red)[32];
-            for (int w = 1; w < (int)(blockDim.x >> 5); ++w) {
-                const float ob = s_red[w];
-                const int oi = reinterpret_cast<int*>(s_red)[32 + w];
-                if (ob < best || (ob == best && oi < ib)) { best = ob; ib = oi; }
-            }
-            i0 = ib;
-            __syncthreads();
-        } else {
-            const int centre = P.closed ? wrap_index(start, P.P) : min(max(start, 0), P.P - 1);
-            i0 = ContourCost::nearest(P, s_trk, centre, x.px, x.py, x.pz);
-        }
-        cc.init(s_trk, i0, x);
-    }
-
-    // ---- the horizon: noise -> clamp -> RK4 -> cost, all in registers (Alg. 1 lines 6-13) ----
-    float4* du_out = STORE_DU ? A.du + (size_t)b * N * P.K + k : nullptr;
-    for (int t = 0; t < N; ++t) {
-        const float4 un = s_unom[t];
-        const float4 T = sample_thrust<MATH>(P, A.rk, (uint32_t)k, (uint32_t)t, A.iter, (uint32_t)b, un);
-        if (STORE_DU)                                      // one coalesced 16-B store per thread
-            du_out[(size_t)t * P.K] = make_float4(T.x - un.x, T.y - un.y, T.z - un.z, T.w - un.w);
-        if (OBJ == OBJ_TRACK) J += track_stage(P, s_trk + 4 * t, x, T);
-        rk4_step(P, x, T);
-        if (OBJ == OBJ_GATE) gc.step<MATH>(P, s_trk, x);
-        if (OBJ == OBJ_CONTOUR) J += cc.step(P, s_trk, x);
-    }
-    if (OBJ == OBJ_GATE) J = gc.finish<MATH>(P, s_trk, x);
-    if (OBJ == OBJ_TRACK) J += track_state_term(P, s_trk + 4 * N, x);
+    const State x0 = load_state(A.x0 + 13 * b);
+    const int i0 = OBJ == OBJ_CONTOUR ? contour_start_index(P, s_trk, start, x0, s_red) : 0;
+    DrawThrust<MATH, STORE_DU> src{P, A, s_unom, (uint32_t)k, (uint32_t)b,
+                                   STORE_DU ? A.du + (size_t)b * N * P.K + k : nullptr};
+    const float J = rollout_cost<OBJ, MATH>(P, s_trk, x0, start, i0, src);
     A.cost[(size_t)b * P.K + k] = J;
 
     if (!FUSED) return;
@@ -194,49 +104,96 @@ __global__ void rollout_kernel(const DevParams P, const StepArgs A)
     }
     __syncthreads();
     const int nw = blockDim.x >> 5;
-    const int stride = 4 * N + 4;
-    float* part = A.partials + ((size_t)b * P.blocks_per_ctrl + blockIdx.x) * stride;
+    float* part = A.partials + ((size_t)b * P.blocks_per_ctrl + blockIdx.x) * (4 * N + 4);
     for (int j = tid; j < 4 * N; j += blockDim.x) {
         float s = 0.0f;
         for (int w = 0; w < nw; ++w) s += reinterpret_cast<const float*>(s_acc)[w * 4 * N + j];
         part[j] = s;
     }
     if (tid == 0) { part[4 * N] = m; part[4 * N + 1] = Zb; }
+    publish_and_combine<MATH>(P, A, b, P.blocks_per_ctrl, s_unom, s_red, s_pair);
+}
 
-    // ---- last block of this controller combines the partials ("threadfence reduction") ----
-    __threadfence();
-    __syncthreads();
-    if (tid == 0) {
-        const unsigned ticket = atomicAdd(&A.counters[b], 1u);
-        reinterpret_cast<int*>(s_red)[40] = (ticket == (unsigned)(P.blocks_per_ctrl - 1));
-    }
-    __syncthreads();
-    if (!reinterpret_cast<int*>(s_red)[40]) return;
-    __threadfence();
+// ---------------------------------------------------------------------------------------------
+// latency variant (fused pipeline only): for a lone controller K = 4096 is 128 warps on 148 SMs,
+// and the iteration time is the dependent-issue latency of one warp.  The noise does not depend
+// on the state, so it is taken off that critical path:
+//   phase 1  all 8 warps of the block draw the clamped thrusts of its 32 C samples for the whole
+//            horizon into shared memory (N x (32C+1) float4, rows padded against bank conflicts)
+//   phase 2  C consumer warps (one per SM sub-partition) roll the samples out, reading T from smem
+//   phase 3  all threads form the block's softmax partial from the thrusts still in shared memory
+//            (nothing is re-derived or re-read from HBM), then the last block combines.
+// grid = (K / (32 C), B), block = 256 threads.
+// ---------------------------------------------------------------------------------------------
+struct SmemThrust {
+    const float4* col; int row_stride;
+    __device__ __forceinline__ float4 operator()(int t) const { return col[t * row_stride]; }
+};
 
-    const int nb = P.blocks_per_ctrl;
-    const float* pb = A.partials + (size_t)b * nb * stride;
-    float bm = __int_as_float(0x7f800000);
-    for (int j = tid; j < nb; j += blockDim.x) bm = fminf(bm, __ldcg(pb + (size_t)j * stride + 4 * N));
-    const float beta = block_min(bm, s_red);
-    float zz = 0.0f;
-    for (int j = tid; j < nb; j += blockDim.x) {
-        const float sc = exp_weight<MATH>((beta - __ldcg(pb + (size_t)j * stride + 4 * N)) * P.inv_lambda);
-        s_scale[j] = sc;
-        zz = fmaf(__ldcg(pb + (size_t)j * stride + 4 * N + 1), sc, zz);
+constexpr int kLatThreads = 256;
+
+template <int OBJ, int MATH, bool STORE_DU>
+__global__ void __launch_bounds__(kLatThreads) rollout_lat_kernel(const DevParams P, const StepArgs A, const int C)
+{
+    extern __shared__ float4 smem[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int b = blockIdx.y, N = P.N;
+    const int S = 32 * C, RS = S + 1, lgS = 5 + (C >> 1);             // C in {1, 2, 4}
+    const int kbase = blockIdx.x * S;
+
+    float4* s_unom = smem;
+    float4* s_trk = smem + N;
+    float* s_red = reinterpret_cast<float*>(s_trk + track_f4(P, OBJ));   // 64 floats
+    float4* s_T = reinterpret_cast<float4*>(s_red + 64);                 // [N][RS]
+    float* s_e = reinterpret_cast<float*>(s_T + (size_t)N * RS);         // 128 floats
+    float* s_pair = s_e + 128;
+
+    const int start = A.start[b];
+    stage_inputs<OBJ>(P, A, b, start, s_unom, s_trk);
+    __syncthreads();
+
+    // ---- phase 1: the whole block draws the noise (eq.(3)) ----
+#pragma unroll 2
+    for (int idx = tid; idx < N * S; idx += kLatThreads) {
+        const int t = idx >> lgS, l = idx & (S - 1);
+        const float4 un = s_unom[t];
+        const float4 T = sample_thrust<MATH>(P, A.rk, (uint32_t)(kbase + l), (uint32_t)t, A.iter, (uint32_t)b, un);
+        s_T[t * RS + l] = T;
+        if (STORE_DU)
+            A.du[((size_t)b * N + t) * P.K + kbase + l] = make_float4(T.x - un.x, T.y - un.y, T.z - un.z, T.w - un.w);
     }
-    const float Z = block_sum(zz, s_red);      // also orders the s_scale writes before the reads
-    const float invZ = 1.0f / Z;
-    for (int j = tid; j < 4 * N; j += blockDim.x) {
+    const State x0 = load_state(A.x0 + 13 * b);
+    const int i0 = OBJ == OBJ_CONTOUR ? contour_start_index(P, s_trk, start, x0, s_red) : 0;
+    __syncthreads();
+
+    // ---- phase 2: C warps roll out, one per scheduler ----
+    float J = __int_as_float(0x7f800000);
+    if (warp < C) {
+        SmemThrust src{s_T + tid, RS};
+        J = rollout_cost<OBJ, MATH>(P, s_trk, x0, start, i0, src);
+        A.cost[(size_t)b * P.K + kbase + tid] = J;
+    }
+    const float m = block_min(J, s_red);
+    const float e = warp < C ? exp_weight<MATH>((m - J) * P.inv_lambda) : 0.0f;
+    const float Zb = block_sum(e, s_red);
+    if (warp < C) s_e[tid] = e;
+    __syncthreads();
+
+    // ---- phase 3: S[t][i] = sum_l e_l (T_l[t][i] - u_nom[t][i]) from shared memory ----
+    float* part = A.partials + ((size_t)b * P.blocks_per_ctrl + blockIdx.x) * (4 * N + 4);
+    for (int j = tid; j < 4 * N; j += kLatThreads) {
+        const int t = j >> 2, i = j & 3;
+        const float un = reinterpret_cast<const float*>(s_unom)[j];
+        const float* row = reinterpret_cast<const float*>(s_T + t * RS) + i;
         float acc = 0.0f;
-        for (int q = 0; q < nb; ++q) acc = fmaf(__ldcg(pb + (size_t)q * stride + j), s_scale[q], acc);
-        A.u_new[(size_t)b * 4 * N + j] = fmaf(acc, invZ, reinterpret_cast<const float*>(s_unom)[j]);
+        for (int l = 0; l < S; ++l) {
+            const float el = s_e[l];                      // block-uniform
+            if (el != 0.0f) acc = fmaf(el, row[4 * l] - un, acc);
+        }
+        part[j] = acc;
     }
-    for (int kk = tid; kk < P.K; kk += blockDim.x) {
-        const float Jk = __ldcg(A.cost + (size_t)b * P.K + kk);
-        A.weights[(size_t)b * P.K + kk] = exp_weight<MATH>((beta - Jk) * P.inv_lambda) * invZ;
-    }
-    if (tid == 0) A.counters[b] = 0u;          // ready for the next launch
+    if (tid == 0) { part[4 * N] = m; part[4 * N + 1] = Zb; }
+    publish_and_combine<MATH>(P, A, b, P.blocks_per_ctrl, s_unom, s_red, s_pair);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -370,14 +327,35 @@ static RolloutFn pick(const LaunchCfg& c)
     }
 }
 
-const void* rollout_kernel_ptr(const LaunchCfg& c) { return reinterpret_cast<const void*>(pick(c)); }
+typedef void (*LatFn)(const DevParams, const StepArgs, const int);
+
+template <int OBJ>
+static LatFn pick_lat1(const LaunchCfg& c)
+{
+    if (c.fast_math) return c.store_du ? rollout_lat_kernel<OBJ, 1, true> : rollout_lat_kernel<OBJ, 1, false>;
+    return c.store_du ? rollout_lat_kernel<OBJ, 0, true> : rollout_lat_kernel<OBJ, 0, false>;
+}
+static LatFn pick_lat(const LaunchCfg& c)
+{
+    switch (c.objective) {
+        case OBJ_GATE: return pick_lat1<OBJ_GATE>(c);
+        case OBJ_TRACK: return pick_lat1<OBJ_TRACK>(c);
+        default: return pick_lat1<OBJ_CONTOUR>(c);
+    }
+}
+
+const void* rollout_kernel_ptr(const LaunchCfg& c)
+{
+    return c.lat_consumers > 0 ? reinterpret_cast<const void*>(pick_lat(c)) : reinterpret_cast<const void*>(pick(c));
+}
 const void* reduce_kernel_ptr() { return reinterpret_cast<const void*>(reduce_kernel); }
 const void* sim_kernel_ptr() { return reinterpret_cast<const void*>(sim_kernel<OBJ_GATE>); }
 
 cudaError_t launch_rollout(const DevParams& P, const StepArgs& A, const LaunchCfg& c, cudaStream_t s)
 {
     const dim3 grid(P.blocks_per_ctrl, P.B), block(c.block_threads);
-    pick(c)<<<grid, block, c.smem_bytes, s>>>(P, A);
+    if (c.lat_consumers > 0) pick_lat(c)<<<grid, block, c.smem_bytes, s>>>(P, A, c.lat_consumers);
+    else pick(c)<<<grid, block, c.smem_bytes, s>>>(P, A);
     return cudaGetLastError();
 }
 

@@ -1,0 +1,197 @@
+// mppi_rollout.cuh -- device functions shared by the two rollout kernels (throughput and latency
+// variants): block reductions, shared-memory staging, the horizon loop, and the last-block
+// combine of the fused softmax update.
+#pragma once
+#include "mppi_cost.cuh"
+
+namespace mppi {
+
+constexpr unsigned kFull = 0xffffffffu;
+
+__device__ __forceinline__ float warp_min(float v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(kFull, v, o));
+    return v;
+}
+__device__ __forceinline__ float warp_sum(float v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+    return v;
+}
+
+template <int MATH>
+__device__ __forceinline__ float exp_weight(float x)   // exp(x), x <= 0
+{
+    return MATH == 0 ? expf(x) : mufu_ex2(x * 1.4426950408889634f);
+}
+
+// block-wide min / sum over blockDim.x threads through s_red[0..31]; every thread gets the result
+__device__ __forceinline__ float block_min(float v, float* s_red)
+{
+    v = warp_min(v);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = v;
+    __syncthreads();
+    const int nw = blockDim.x >> 5;
+    float r = s_red[0];
+    for (int w = 1; w < nw; ++w) r = fminf(r, s_red[w]);
+    return r;
+}
+__device__ __forceinline__ float block_sum(float v, float* s_red)
+{
+    v = warp_sum(v);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = v;
+    __syncthreads();
+    const int nw = blockDim.x >> 5;
+    float r = s_red[0];
+    for (int w = 1; w < nw; ++w) r += s_red[w];      // fixed order: deterministic
+    return r;
+}
+
+__host__ __device__ inline int track_f4(const DevParams& P, int objective)
+{
+    return objective == OBJ_GATE ? 4 * P.G : objective == OBJ_TRACK ? 4 * (P.N + 1) : 2 * P.P;
+}
+
+// Stage the nominal sequence of controller b and the objective's track data in shared memory.
+template <int OBJ>
+__device__ __forceinline__ void stage_inputs(const DevParams& P, const StepArgs& A, int b, int start,
+                                             float4* s_unom, float4* s_trk)
+{
+    const int tid = threadIdx.x, N = P.N;
+    const float4* un = reinterpret_cast<const float4*>(A.u_nom) + (size_t)b * N;
+    for (int t = tid; t < N; t += blockDim.x) s_unom[t] = un[t];
+    if (OBJ == OBJ_GATE) {
+        for (int i = tid; i < 4 * P.G; i += blockDim.x) s_trk[i] = P.gates[i];
+    } else if (OBJ == OBJ_TRACK) {
+        const int t0 = min(max(start, 0), P.M - 1 - N);
+        for (int i = tid; i < 4 * (N + 1); i += blockDim.x) s_trk[i] = P.ref[4 * t0 + i];
+    } else {
+        for (int i = tid; i < 2 * P.P; i += blockDim.x) s_trk[i] = P.path[i];
+    }
+}
+
+// Contouring: initial path index of the block (all samples share x0).  start < 0: global nearest
+// vertex, block-cooperative, ties -> smallest index (= the oracle's scan order); otherwise the
+// windowed search around the hint.  Every thread of the block must call this.
+__device__ __forceinline__ int contour_start_index(const DevParams& P, const float4* s_path, int start,
+                                                   const State& x, float* s_red)
+{
+    if (start >= 0) {
+        const int centre = P.closed ? wrap_index(start, P.P) : min(max(start, 0), P.P - 1);
+        return ContourCost::nearest(P, s_path, centre, x.px, x.py, x.pz);
+    }
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    float best = __int_as_float(0x7f800000);
+    int ib = 0x7fffffff;
+    for (int i = tid; i < P.P; i += blockDim.x) {
+        const float4 q = s_path[2 * i];
+        const float dx = x.px - q.x, dy = x.py - q.y, dz = x.pz - q.z;
+        const float d2 = dx * dx + dy * dy + dz * dz;
+        if (d2 < best) { best = d2; ib = i; }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const float ob = __shfl_xor_sync(kFull, best, o);
+        const int oi = __shfl_xor_sync(kFull, ib, o);
+        if (ob < best || (ob == best && oi < ib)) { best = ob; ib = oi; }
+    }
+    int* s_idx = reinterpret_cast<int*>(s_red) + 32;
+    if (lane == 0) { s_red[warp] = best; s_idx[warp] = ib; }
+    __syncthreads();
+    best = s_red[0]; ib = s_idx[0];
+    for (int w = 1; w < (int)(blockDim.x >> 5); ++w) {
+        const float ob = s_red[w];
+        const int oi = s_idx[w];
+        if (ob < best || (ob == best && oi < ib)) { best = ob; ib = oi; }
+    }
+    __syncthreads();
+    return ib;
+}
+
+// The horizon of one sample: thrust -> RK4 -> cost, all in registers (Alg. 1 lines 6-13).
+// `thrust(t)` yields the clamped rotor thrusts of step t (drawn in place or read from smem).
+template <int OBJ, int MATH, class Thrust>
+__device__ __forceinline__ float rollout_cost(const DevParams& P, const float4* s_trk, State x, int start,
+                                              int contour_i0, Thrust thrust)
+{
+    const int N = P.N;
+    float J = 0.0f;
+    GateCost gc;
+    ContourCost cc;
+    if (OBJ == OBJ_GATE) gc.init<MATH>(P, s_trk, start, x);
+    if (OBJ == OBJ_CONTOUR) cc.init(s_trk, contour_i0, x);
+    for (int t = 0; t < N; ++t) {
+        const float4 T = thrust(t);
+        if (OBJ == OBJ_TRACK) J += track_stage(P, s_trk + 4 * t, x, T);
+        rk4_step(P, x, T);
+        if (OBJ == OBJ_GATE) gc.step<MATH>(P, s_trk, x);
+        if (OBJ == OBJ_CONTOUR) J += cc.step(P, s_trk, x);
+    }
+    if (OBJ == OBJ_GATE) J = gc.finish<MATH>(P, s_trk, x);
+    if (OBJ == OBJ_TRACK) J += track_state_term(P, s_trk + 4 * N, x);
+    return J;
+}
+
+// Fused softmax update, second half ("threadfence reduction").  Every block of controller b has
+// written its partial  part = { S[4N] = sum_k e_k dU_k, m = min_k J_k, Z = sum_k e_k }  with
+// e_k = exp(-(J_k - m)/lambda)  (online-softmax form of eq.(4),(5)).  The block that
+// takes the last ticket rescales the nb partials to the global minimum beta and writes
+//   u_new = u_nom + sum_q S_q exp(-(m_q - beta)/lambda) / Z_tot,   w_k = exp(-(J_k - beta)/lambda) / Z_tot.
+// Partials whose rescale factor underflows to 0 contribute exactly 0 and are not read.
+// s_pair: 2 nb floats of shared memory.  All threads of the block must call this.
+template <int MATH>
+__device__ __forceinline__ void publish_and_combine(const DevParams& P, const StepArgs& A, int b, int nb,
+                                                    const float4* s_unom, float* s_red, float* s_pair)
+{
+    const int tid = threadIdx.x, N = P.N, stride = 4 * N + 4;
+    int* s_flag = reinterpret_cast<int*>(s_red) + 48;
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) *s_flag = (atomicAdd(&A.counters[b], 1u) == (unsigned)(nb - 1));
+    __syncthreads();
+    if (!*s_flag) return;
+    __threadfence();
+
+    const float* pb = A.partials + (size_t)b * nb * stride;
+    float* s_scale = s_pair;
+    float* s_z = s_pair + nb;
+    float bm = __int_as_float(0x7f800000);
+    for (int j = tid; j < nb; j += blockDim.x) {
+        const float2 mz = __ldcg(reinterpret_cast<const float2*>(pb + (size_t)j * stride + 4 * N));
+        s_scale[j] = mz.x; s_z[j] = mz.y;
+        bm = fminf(bm, mz.x);
+    }
+    const float beta = block_min(bm, s_red);
+    float zz = 0.0f;
+    for (int j = tid; j < nb; j += blockDim.x) {
+        const float sc = exp_weight<MATH>((beta - s_scale[j]) * P.inv_lambda);
+        s_scale[j] = sc;
+        zz = fmaf(s_z[j], sc, zz);
+    }
+    const float Z = block_sum(zz, s_red);      // its barriers also order the s_scale writes
+    const float invZ = 1.0f / Z;
+    for (int j = tid; j < 4 * N; j += blockDim.x) {
+        float acc = 0.0f;
+        for (int q = 0; q < nb; ++q) {
+            const float sc = s_scale[q];       // block-uniform: no divergence
+            if (sc != 0.0f) acc = fmaf(__ldcg(pb + (size_t)q * stride + j), sc, acc);
+        }
+        A.u_new[(size_t)b * 4 * N + j] = fmaf(acc, invZ, reinterpret_cast<const float*>(s_unom)[j]);
+    }
+    const float4* c4 = reinterpret_cast<const float4*>(A.cost + (size_t)b * P.K);
+    float4* w4 = reinterpret_cast<float4*>(A.weights + (size_t)b * P.K);
+    const float nil = -P.inv_lambda;
+#pragma unroll 4
+    for (int i = tid; i < P.K / 4; i += blockDim.x) {
+        const float4 c = __ldcg(c4 + i);
+        w4[i] = make_float4(exp_weight<MATH>((c.x - beta) * nil) * invZ, exp_weight<MATH>((c.y - beta) * nil) * invZ,
+                            exp_weight<MATH>((c.z - beta) * nil) * invZ, exp_weight<MATH>((c.w - beta) * nil) * invZ);
+    }
+    if (tid == 0) A.counters[b] = 0u;          // ready for the next launch
+}
+
+}  // namespace mppi

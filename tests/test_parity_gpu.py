@@ -33,18 +33,18 @@ def run_case(wl, tag, it=0, **opts):
     return g, o, st
 
 
-PIPES = [dict(pipeline=0), dict(pipeline=1)]
+PIPES = [dict(pipeline=0, variant=2), dict(pipeline=0, variant=1), dict(pipeline=1)]
 MATH = [dict(fast_math=0), dict(fast_math=1)]
 
 
-@pytest.mark.parametrize("pipe", PIPES, ids=["fused", "two_pass"])
+@pytest.mark.parametrize("pipe", PIPES, ids=["fused_lat", "fused_thr", "two_pass"])
 @pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
 def test_cfg0_tiny_gate(pipe, math):
     g, o, st = run_case(W.cfg0(), f"cfg0[{pipe},{math}]", **pipe, **math)
     assert st["ess"] > 1.5            # the config really mixes several samples
 
 
-@pytest.mark.parametrize("pipe", PIPES, ids=["fused", "two_pass"])
+@pytest.mark.parametrize("pipe", PIPES, ids=["fused_lat", "fused_thr", "two_pass"])
 def test_cfg1_ten_warm_started_iterations(pipe):
     # [R-14] no shift, same x0, u_nom <- u_new, iter = 0..9; the oracle is teacher-forced with the
     # GPU's nominal of each iteration (fp32 -> fp64) so that every iteration is an exact comparison
@@ -84,19 +84,19 @@ def test_cfg1_optimize_graph_equals_step_chain():
     m.close()
 
 
-@pytest.mark.parametrize("pipe", PIPES, ids=["fused", "two_pass"])
+@pytest.mark.parametrize("pipe", PIPES, ids=["fused_lat", "fused_thr", "two_pass"])
 @pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
 def test_cfg2_tracking(pipe, math):
     run_case(W.cfg2(), f"cfg2[{pipe},{math}]", **pipe, **math)
 
 
-@pytest.mark.parametrize("pipe", PIPES, ids=["fused", "two_pass"])
+@pytest.mark.parametrize("pipe", PIPES, ids=["fused_lat", "fused_thr", "two_pass"])
 @pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
 def test_cfg3_contouring(pipe, math):
     run_case(W.cfg3(), f"cfg3[{pipe},{math}]", **pipe, **math)
 
 
-@pytest.mark.parametrize("pipe", PIPES, ids=["fused", "two_pass"])
+@pytest.mark.parametrize("pipe", PIPES, ids=["fused_lat", "fused_thr", "two_pass"])
 @pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
 def test_stress_gate_crossings(pipe, math):
     wl = W.stress_gate(K=4096, N=30)
@@ -142,7 +142,7 @@ def test_cfg4_closed_loop_teacher_forced():
 # ---- the reduction arithmetic with many contributing samples (ESS >> 1) -------------------------
 
 @pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3"])
-@pytest.mark.parametrize("pipe", PIPES, ids=["fused", "two_pass"])
+@pytest.mark.parametrize("pipe", PIPES, ids=["fused_lat", "fused_thr", "two_pass"])
 def test_flat_weights_exercise_the_update(name, pipe):
     wl = W.ALL[name](K=2048, N=50)
     o0 = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, wl.seed, 0)
@@ -177,17 +177,29 @@ def test_noise_matches_oracle_and_pipelines_agree():
     m.close()
 
 
+@pytest.mark.parametrize("K,N,B,consumers", [(32, 1, 1, 1), (64, 33, 1, 1), (4096, 50, 1, 1), (8192, 50, 1, 2),
+                                             (16384, 20, 1, 4), (512, 20, 3, 1), (4096, 256, 1, 1), (96, 7, 1, 1)])
+def test_latency_variant_shapes(K, N, B, consumers):
+    # the warp-specialised kernel: C rollout warps per 256-thread block, C picked from the grid size
+    wl = W.cfg4(K=K, N=N, B=B) if B > 1 else W.stress_gate(K=K, N=N)
+    m = Pz.make_ctx(wl, variant=2)
+    info = m.info()
+    assert info["block_threads"] == 256 and info["blocks_per_controller"] == K // (32 * consumers)
+    m.close()
+    run_case(wl, f"lat K{K} N{N} B{B}", variant=2)
+
+
 # ---- ragged / degenerate / maximum sizes ----------------------------------------------------------
 
 @pytest.mark.parametrize("K,N,tpb", [(32, 1, 32), (32, 33, 32), (64, 20, 64), (96, 7, 32), (256, 256, 256),
                                      (1024, 64, 128), (8192, 50, 256)])
-@pytest.mark.parametrize("pipe", PIPES, ids=["fused", "two_pass"])
+@pytest.mark.parametrize("pipe", PIPES, ids=["fused_lat", "fused_thr", "two_pass"])
 def test_sizes_and_block_shapes(K, N, tpb, pipe):
     wl = W.stress_gate(K=K, N=N)
     run_case(wl, f"sizes K{K} N{N} tpb{tpb} [{pipe}]", block_threads=tpb, **pipe)
 
 
-@pytest.mark.parametrize("pipe", PIPES, ids=["fused", "two_pass"])
+@pytest.mark.parametrize("pipe", PIPES, ids=["fused_lat", "fused_thr", "two_pass"])
 def test_sigma_zero_is_uniform(pipe):
     wl = W.cfg0(K=128, N=10)
     wl.params["sigma"] = 0.0
@@ -197,7 +209,7 @@ def test_sigma_zero_is_uniform(pipe):
     assert np.ptp(g["cost"]) == 0.0
 
 
-@pytest.mark.parametrize("pipe", PIPES, ids=["fused", "two_pass"])
+@pytest.mark.parametrize("pipe", PIPES, ids=["fused_lat", "fused_thr", "two_pass"])
 def test_saturated_nominal_and_tiny_lambda(pipe):
     wl = W.cfg0(K=256, N=12)
     wl.u_nom[:] = 7.0
