@@ -75,11 +75,15 @@ typedef enum {
 } mppi_pipeline;
 
 typedef enum {
-    MPPI_VARIANT_AUTO = 0,       /* latency kernel when B*K/32 warps cannot fill the chip, else throughput */
+    MPPI_VARIANT_AUTO = 0,       /* latency kernel when B*K/32 warps cannot fill the chip, else packed (K % 64
+                                    == 0) or scalar throughput                                             */
     MPPI_VARIANT_THROUGHPUT = 1, /* one sample per thread, noise drawn inside the horizon loop; block_threads
                                     samples per block                                                      */
-    MPPI_VARIANT_LATENCY = 2     /* 256-thread blocks: all warps draw the noise of 32 C samples into shared
+    MPPI_VARIANT_LATENCY = 2,    /* 256-thread blocks: all warps draw the noise of 32 C samples into shared
                                     memory first, then C warps (C = 1, 2 or 4) roll out; fused pipeline only */
+    MPPI_VARIANT_PACKED = 3      /* throughput kernel with TWO samples per thread held in packed fp32x2
+                                    registers (sm_100a FFMA2); needs K % 64 == 0; results are bit-identical
+                                    to MPPI_VARIANT_THROUGHPUT                                             */
 } mppi_variant;
 
 /* Parameters of Alg. 1 (samples, horizon, lambda, Sigma) plus the model and cost
@@ -107,7 +111,8 @@ typedef struct {
     int32_t pipeline;  /* mppi_pipeline                                                          */
     int32_t use_graph; /* 1: replay each step as a CUDA graph; 0: plain stream launches          */
     int32_t block_threads; /* threads per block of the rollout kernel: 0 = auto, else 32..256,
-                              a multiple of 32 that divides K                                    */
+                              a multiple of 32 that divides K (packed variant: 2*block_threads
+                              must divide K)                                                     */
     int32_t fast_math; /* 0: IEEE-accurate logf/sincospif/sqrtf/expf; 1: MUFU approximations for
                           the Box-Muller transform (error budget)                 */
     int32_t store_noise; /* 1: also keep dU of the last step for mppi_debug_noise (always kept
@@ -193,6 +198,8 @@ typedef struct {
     int32_t regs_per_thread, static_smem_bytes, dynamic_smem_bytes, local_bytes_per_thread;
     int32_t max_blocks_per_sm, sm_count;
     int32_t kernels_per_step; /* launches one mppi_step enqueues */
+    int32_t samples_per_thread; /* 2 for the packed fp32x2 rollout kernel, else 1 */
+    int32_t rollout_warps_per_block; /* latency variant: consumer warps C; else block_threads / 32 */
     int32_t l2_bytes;
     int64_t scratch_bytes;    /* device memory the context owns */
 } mppi_info;

@@ -16,7 +16,7 @@ LIB_PATH = _HERE / "libmppi.so"
 
 OBJ_GATE, OBJ_TRACK, OBJ_CONTOUR = 0, 1, 2
 PIPE_FUSED, PIPE_TWO_PASS = 0, 1
-VARIANT_AUTO, VARIANT_THROUGHPUT, VARIANT_LATENCY = 0, 1, 2
+VARIANT_AUTO, VARIANT_THROUGHPUT, VARIANT_LATENCY, VARIANT_PACKED = 0, 1, 2, 3
 
 EXPORTS = ["mppi_default_params", "mppi_create", "mppi_destroy", "mppi_set_gates",
            "mppi_set_reference", "mppi_set_path", "mppi_step", "mppi_optimize", "mppi_step_host",
@@ -44,7 +44,8 @@ class MppiInfo(C.Structure):
                 ("blocks_per_controller", C.c_int32), ("regs_per_thread", C.c_int32),
                 ("static_smem_bytes", C.c_int32), ("dynamic_smem_bytes", C.c_int32),
                 ("local_bytes_per_thread", C.c_int32), ("max_blocks_per_sm", C.c_int32),
-                ("sm_count", C.c_int32), ("kernels_per_step", C.c_int32), ("l2_bytes", C.c_int32),
+                ("sm_count", C.c_int32), ("kernels_per_step", C.c_int32), ("samples_per_thread", C.c_int32),
+                ("rollout_warps_per_block", C.c_int32), ("l2_bytes", C.c_int32),
                 ("scratch_bytes", C.c_int64)]
 
 

@@ -117,7 +117,9 @@ static int validate(const mppi_params* p)
                                   p->K % p->block_threads != 0),
         "block_threads must be 0 or a multiple of 32 in 32..256 that divides K");
     BAD((int64_t)p->K / 32 > 65535, "K too large");
-    BAD(p->variant < 0 || p->variant > 2, "unknown variant");
+    BAD(p->variant < 0 || p->variant > 3, "unknown variant");
+    BAD(p->variant == MPPI_VARIANT_PACKED && (p->K % 64 != 0 || (p->block_threads && p->K % (2 * p->block_threads) != 0)),
+        "the packed variant needs K % 64 == 0 and 2*block_threads dividing K");
     BAD(p->variant == MPPI_VARIANT_LATENCY && p->pipeline != MPPI_PIPE_FUSED, "the latency variant needs the fused pipeline");
 #undef BAD
     return MPPI_OK;
@@ -126,10 +128,11 @@ static int validate(const mppi_params* p)
 // Launch shape.  Latency variant: C rollout warps per 256-thread block, the smallest C in {1,2,4}
 // that brings the grid down to one block per SM (so every rollout warp owns a scheduler).
 // Throughput variant: 256-thread blocks when the grid still covers the chip several times, else 128.
-static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, int* lat_consumers)
+static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, int* lat_consumers, int* packed)
 {
     const int64_t warps = (int64_t)p->B * p->K / 32;
     *lat_consumers = 0;
+    *packed = 0;
     const bool lat_ok = p->pipeline == MPPI_PIPE_FUSED && p->block_threads == 0;
     if (lat_ok && (p->variant == MPPI_VARIANT_LATENCY || (p->variant == MPPI_VARIANT_AUTO && warps <= 4 * (int64_t)sm_count))) {
         int best = 0;
@@ -139,6 +142,14 @@ static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, i
                 if (warps / c <= sm_count) break;
             }
         if (best) { *lat_consumers = best; *block_threads = 256; return; }
+    }
+    // packed fp32x2 throughput kernel: two samples per thread
+    if (p->K % 64 == 0 && (p->variant == MPPI_VARIANT_PACKED ||
+                           (p->variant == MPPI_VARIANT_AUTO && (!p->block_threads || p->K % (2 * p->block_threads) == 0)))) {
+        *packed = 1;
+        if (p->block_threads) { *block_threads = p->block_threads; return; }
+        for (int tpb : {128, 64, 32})
+            if (p->K % (2 * tpb) == 0) { *block_threads = tpb; return; }
     }
     if (p->block_threads) { *block_threads = p->block_threads; return; }
     if (p->K % 256 == 0 && warps >= 16 * (int64_t)sm_count) { *block_threads = 256; return; }
@@ -217,8 +228,9 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     cfg.objective = p->objective; cfg.fast_math = p->fast_math ? 1 : 0;
     cfg.fused = p->pipeline == MPPI_PIPE_FUSED;
     cfg.store_du = (!cfg.fused || p->store_noise) ? 1 : 0;
-    pick_shape(p, c->sm_count, &cfg.block_threads, &cfg.lat_consumers);
-    d.blocks_per_ctrl = cfg.lat_consumers ? p->K / (32 * cfg.lat_consumers) : p->K / cfg.block_threads;
+    pick_shape(p, c->sm_count, &cfg.block_threads, &cfg.lat_consumers, &cfg.packed);
+    d.blocks_per_ctrl = cfg.lat_consumers ? p->K / (32 * cfg.lat_consumers)
+                                          : p->K / (cfg.block_threads * (cfg.packed ? 2 : 1));
     cfg.smem_bytes = 0;   // fixed once the track is known
 
     const size_t BN4 = (size_t)p->B * p->N * 4, BK = (size_t)p->B * p->K;
@@ -554,6 +566,8 @@ extern "C" int mppi_get_info(mppi_ctx* c, mppi_info* o)
     o->max_blocks_per_sm = nb;
     o->sm_count = c->sm_count;
     o->kernels_per_step = c->cfg.fused ? 1 : 2;
+    o->samples_per_thread = c->cfg.packed ? 2 : 1;
+    o->rollout_warps_per_block = c->cfg.lat_consumers ? c->cfg.lat_consumers : c->cfg.block_threads / 32;
     o->l2_bytes = c->l2_bytes;
     o->scratch_bytes = c->scratch_bytes;
     return MPPI_OK;

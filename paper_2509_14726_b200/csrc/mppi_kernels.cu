@@ -10,6 +10,7 @@
 // No tensor cores: nothing here is a contraction.
 #include "mppi_internal.h"
 #include "mppi_rollout.cuh"
+#include "mppi_packed.cuh"
 
 namespace mppi {
 
@@ -28,6 +29,123 @@ size_t rollout_smem_bytes(const DevParams& P, const LaunchCfg& c)
     }
     if (c.fused) f4 += (size_t)(c.block_threads / 32) * P.N + (2 * P.blocks_per_ctrl + 3) / 4;
     return f4 * sizeof(float4);
+}
+
+// ---------------------------------------------------------------------------------------------
+// packed throughput variant: two samples per thread in fp32x2 registers (mppi_packed.cuh).
+// grid = (K / (2 blockDim.x), B); thread j of the grid row owns samples 2j and 2j+1.
+// ---------------------------------------------------------------------------------------------
+template <int OBJ, int MATH>
+__device__ __forceinline__ void rollout_cost2(const DevParams& P, const StepArgs& A, const float4* s_unom,
+                                              const float4* s_trk, State2 x, int start, int contour_i0,
+                                              uint32_t k0, uint32_t b, float4* du_out, float& Ja, float& Jb)
+{
+    const int N = P.N;
+    Ja = 0.0f; Jb = 0.0f;
+    GateCost ga, gb;
+    ContourCost ca, cb;
+    if (OBJ == OBJ_GATE) { ga.init<MATH>(P, s_trk, start, lane_state<0>(x)); gb = ga; }
+    if (OBJ == OBJ_CONTOUR) { ca.init(s_trk, contour_i0, lane_state<0>(x)); cb = ca; }
+    for (int t = 0; t < N; ++t) {
+        const float4 un = s_unom[t];
+        const float4 Ta = sample_thrust<MATH>(P, A.rk, k0, (uint32_t)t, A.iter, b, un);
+        const float4 Tb = sample_thrust<MATH>(P, A.rk, k0 + 1u, (uint32_t)t, A.iter, b, un);
+        if (du_out) {
+            du_out[(size_t)t * P.K] = make_float4(Ta.x - un.x, Ta.y - un.y, Ta.z - un.z, Ta.w - un.w);
+            du_out[(size_t)t * P.K + 1] = make_float4(Tb.x - un.x, Tb.y - un.y, Tb.z - un.z, Tb.w - un.w);
+        }
+        if (OBJ == OBJ_TRACK) {
+            Ja += track_stage(P, s_trk + 4 * t, lane_state<0>(x), Ta);
+            Jb += track_stage(P, s_trk + 4 * t, lane_state<1>(x), Tb);
+        }
+        rk4_step2(P, x, Ta, Tb);
+        if (OBJ == OBJ_GATE) {
+            ga.step<MATH>(P, s_trk, lane_state<0>(x));
+            gb.step<MATH>(P, s_trk, lane_state<1>(x));
+        }
+        if (OBJ == OBJ_CONTOUR) {
+            Ja += ca.step(P, s_trk, lane_state<0>(x));
+            Jb += cb.step(P, s_trk, lane_state<1>(x));
+        }
+    }
+    if (OBJ == OBJ_GATE) {
+        Ja = ga.finish<MATH>(P, s_trk, lane_state<0>(x));
+        Jb = gb.finish<MATH>(P, s_trk, lane_state<1>(x));
+    }
+    if (OBJ == OBJ_TRACK) {
+        Ja += track_state_term(P, s_trk + 4 * N, lane_state<0>(x));
+        Jb += track_state_term(P, s_trk + 4 * N, lane_state<1>(x));
+    }
+}
+
+#ifndef MPPI_PK_THREADS
+#define MPPI_PK_THREADS 128     // max block size of the packed kernel
+#define MPPI_PK_MINB 4          // resident blocks per SM the register budget is sized for
+#endif
+template <int OBJ, int MATH, bool STORE_DU, bool FUSED>
+__global__ void __launch_bounds__(MPPI_PK_THREADS, MPPI_PK_MINB) rollout2_kernel(const DevParams P, const StepArgs A)
+{
+    extern __shared__ float4 smem[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int b = blockIdx.y;
+    const int k0 = 2 * (blockIdx.x * blockDim.x + tid);
+    const int N = P.N;
+
+    float4* s_unom = smem;
+    float4* s_trk = smem + N;
+    float* s_red = reinterpret_cast<float*>(s_trk + track_f4(P, OBJ));   // 64 floats
+    float4* s_acc = reinterpret_cast<float4*>(s_red + 64);
+    float* s_pair = reinterpret_cast<float*>(s_acc + (blockDim.x >> 5) * N);
+
+    const int start = A.start[b];
+    stage_inputs<OBJ>(P, A, b, start, s_unom, s_trk);
+    __syncthreads();
+
+    const State x0 = load_state(A.x0 + 13 * b);
+    const int i0 = OBJ == OBJ_CONTOUR ? contour_start_index(P, s_trk, start, x0, s_red) : 0;
+    float Ja, Jb;
+    rollout_cost2<OBJ, MATH>(P, A, s_unom, s_trk, splat_state(x0), start, i0, (uint32_t)k0, (uint32_t)b,
+                             STORE_DU ? A.du + (size_t)b * N * P.K + k0 : nullptr, Ja, Jb);
+    *reinterpret_cast<float2*>(A.cost + (size_t)b * P.K + k0) = make_float2(Ja, Jb);
+
+    if (!FUSED) return;
+
+    // ---- block-local softmax partial, as in rollout_kernel, over the block's 2 blockDim.x samples ----
+    const float m = block_min(fminf(Ja, Jb), s_red);
+    const float ea = exp_weight<MATH>((m - Ja) * P.inv_lambda), eb = exp_weight<MATH>((m - Jb) * P.inv_lambda);
+    const float Zb = block_sum(ea + eb, s_red);
+    {
+        const unsigned ca = __ballot_sync(kFull, ea > 0.0f), cb = __ballot_sync(kFull, eb > 0.0f);
+        const uint32_t kbase = (uint32_t)(2 * (blockIdx.x * blockDim.x + warp * 32));
+        for (int t0 = 0; t0 < N; t0 += 32) {
+            const int t = t0 + lane;
+            const float4 un = t < N ? s_unom[t] : make_float4(0.f, 0.f, 0.f, 0.f);
+            float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                unsigned mm = h ? cb : ca;
+                while (mm) {
+                    const int l = __ffs(mm) - 1;
+                    mm &= mm - 1;
+                    const float el = __shfl_sync(kFull, h ? eb : ea, l);
+                    const float4 T = sample_thrust<MATH>(P, A.rk, kbase + 2u * l + h, (uint32_t)t, A.iter, (uint32_t)b, un);
+                    acc.x = fmaf(el, T.x - un.x, acc.x); acc.y = fmaf(el, T.y - un.y, acc.y);
+                    acc.z = fmaf(el, T.z - un.z, acc.z); acc.w = fmaf(el, T.w - un.w, acc.w);
+                }
+            }
+            if (t < N) s_acc[warp * N + t] = acc;
+        }
+    }
+    __syncthreads();
+    const int nw = blockDim.x >> 5;
+    float* part = A.partials + ((size_t)b * P.blocks_per_ctrl + blockIdx.x) * (4 * N + 4);
+    for (int j = tid; j < 4 * N; j += blockDim.x) {
+        float s = 0.0f;
+        for (int w = 0; w < nw; ++w) s += reinterpret_cast<const float*>(s_acc)[w * 4 * N + j];
+        part[j] = s;
+    }
+    if (tid == 0) { part[4 * N] = m; part[4 * N + 1] = Zb; }
+    publish_and_combine<MATH>(P, A, b, P.blocks_per_ctrl, s_unom, s_red, s_pair);
 }
 
 // thrust source of the throughput kernel: draw (k, t) in place
@@ -310,6 +428,10 @@ typedef void (*RolloutFn)(const DevParams, const StepArgs);
 template <int OBJ, int MATH>
 static RolloutFn pick2(const LaunchCfg& c)
 {
+    if (c.packed) {
+        if (c.fused) return c.store_du ? rollout2_kernel<OBJ, MATH, true, true> : rollout2_kernel<OBJ, MATH, false, true>;
+        return rollout2_kernel<OBJ, MATH, true, false>;
+    }
     if (c.fused) return c.store_du ? rollout_kernel<OBJ, MATH, true, true> : rollout_kernel<OBJ, MATH, false, true>;
     return rollout_kernel<OBJ, MATH, true, false>;
 }

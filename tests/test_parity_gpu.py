@@ -33,18 +33,22 @@ def run_case(wl, tag, it=0, **opts):
     return g, o, st
 
 
-PIPES = [dict(pipeline=0, variant=2), dict(pipeline=0, variant=1), dict(pipeline=1)]
+# fused pipeline with the latency / scalar throughput / packed fp32x2 throughput kernels; two-pass
+# pipeline with the packed (AUTO picks it when K % 64 == 0) and the scalar rollout kernel
+PIPES = [dict(pipeline=0, variant=2), dict(pipeline=0, variant=1), dict(pipeline=0, variant=3), dict(pipeline=1),
+         dict(pipeline=1, variant=1)]
+PIPE_IDS = ["fused_lat", "fused_thr", "fused_pk", "two_pass", "two_pass_thr"]
 MATH = [dict(fast_math=0), dict(fast_math=1)]
 
 
-@pytest.mark.parametrize("pipe", PIPES, ids=["fused_lat", "fused_thr", "two_pass"])
+@pytest.mark.parametrize("pipe", PIPES, ids=PIPE_IDS)
 @pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
 def test_cfg0_tiny_gate(pipe, math):
     g, o, st = run_case(W.cfg0(), f"cfg0[{pipe},{math}]", **pipe, **math)
     assert st["ess"] > 1.5            # the config really mixes several samples
 
 
-@pytest.mark.parametrize("pipe", PIPES, ids=["fused_lat", "fused_thr", "two_pass"])
+@pytest.mark.parametrize("pipe", PIPES, ids=PIPE_IDS)
 def test_cfg1_ten_warm_started_iterations(pipe):
     # [R-14] no shift, same x0, u_nom <- u_new, iter = 0..9; the oracle is teacher-forced with the
     # GPU's nominal of each iteration (fp32 -> fp64) so that every iteration is an exact comparison
@@ -84,19 +88,19 @@ def test_cfg1_optimize_graph_equals_step_chain():
     m.close()
 
 
-@pytest.mark.parametrize("pipe", PIPES, ids=["fused_lat", "fused_thr", "two_pass"])
+@pytest.mark.parametrize("pipe", PIPES, ids=PIPE_IDS)
 @pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
 def test_cfg2_tracking(pipe, math):
     run_case(W.cfg2(), f"cfg2[{pipe},{math}]", **pipe, **math)
 
 
-@pytest.mark.parametrize("pipe", PIPES, ids=["fused_lat", "fused_thr", "two_pass"])
+@pytest.mark.parametrize("pipe", PIPES, ids=PIPE_IDS)
 @pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
 def test_cfg3_contouring(pipe, math):
     run_case(W.cfg3(), f"cfg3[{pipe},{math}]", **pipe, **math)
 
 
-@pytest.mark.parametrize("pipe", PIPES, ids=["fused_lat", "fused_thr", "two_pass"])
+@pytest.mark.parametrize("pipe", PIPES, ids=PIPE_IDS)
 @pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
 def test_stress_gate_crossings(pipe, math):
     wl = W.stress_gate(K=4096, N=30)
@@ -142,7 +146,7 @@ def test_cfg4_closed_loop_teacher_forced():
 # ---- the reduction arithmetic with many contributing samples (ESS >> 1) -------------------------
 
 @pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3"])
-@pytest.mark.parametrize("pipe", PIPES, ids=["fused_lat", "fused_thr", "two_pass"])
+@pytest.mark.parametrize("pipe", PIPES, ids=PIPE_IDS)
 def test_flat_weights_exercise_the_update(name, pipe):
     wl = W.ALL[name](K=2048, N=50)
     o0 = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, wl.seed, 0)
@@ -156,7 +160,9 @@ def test_noise_matches_oracle_and_pipelines_agree():
     import torch
     wl = W.cfg0(K=512, N=37)
     outs = {}
-    for name, opts in dict(fused=dict(pipeline=0, store_noise=1), two=dict(pipeline=1)).items():
+    for name, opts in dict(fused=dict(pipeline=0, store_noise=1), two=dict(pipeline=1),
+                           thr=dict(pipeline=0, variant=1, store_noise=1),
+                           pk=dict(pipeline=0, variant=3, store_noise=1)).items():
         m = Pz.make_ctx(wl, **opts)
         x0, start, u = Pz.to_dev(wl)
         outs[name] = Pz.gpu_step(m, x0, start, u, 5, 7)
@@ -166,6 +172,12 @@ def test_noise_matches_oracle_and_pipelines_agree():
     du_o = np.transpose(o["du"], (0, 2, 1, 3))
     np.testing.assert_allclose(outs["fused"]["du"], du_o, rtol=0, atol=3e-6)
     np.testing.assert_array_equal(outs["fused"]["du"], outs["two"]["du"])
+    # the packed fp32x2 kernel performs, per half, the scalar kernel's operations in the same order
+    for key in ("du", "cost"):
+        np.testing.assert_array_equal(outs["thr"][key], outs["pk"][key])
+    # (the update is summed over differently shaped blocks: equal up to the summation order)
+    np.testing.assert_allclose(outs["thr"]["weights"], outs["pk"]["weights"], rtol=0, atol=2e-6)
+    np.testing.assert_allclose(outs["thr"]["u_new"], outs["pk"]["u_new"], rtol=0, atol=2e-5)
     np.testing.assert_array_equal(outs["fused"]["cost"], outs["two"]["cost"])
     np.testing.assert_allclose(outs["fused"]["weights"], outs["two"]["weights"], rtol=0, atol=2e-6)
     np.testing.assert_allclose(outs["fused"]["u_new"], outs["two"]["u_new"], rtol=0, atol=2e-5)
@@ -193,13 +205,19 @@ def test_latency_variant_shapes(K, N, B, consumers):
 
 @pytest.mark.parametrize("K,N,tpb", [(32, 1, 32), (32, 33, 32), (64, 20, 64), (96, 7, 32), (256, 256, 256),
                                      (1024, 64, 128), (8192, 50, 256)])
-@pytest.mark.parametrize("pipe", PIPES, ids=["fused_lat", "fused_thr", "two_pass"])
+@pytest.mark.parametrize("pipe", PIPES, ids=PIPE_IDS)
 def test_sizes_and_block_shapes(K, N, tpb, pipe):
     wl = W.stress_gate(K=K, N=N)
+    if pipe.get("variant") == 3 and K % (2 * tpb) != 0:
+        from paper_2509_14726_b200 import binding as Bd
+        with pytest.raises(Bd.MppiError) as e:                 # two samples per thread: 2*tpb must divide K
+            Pz.make_ctx(wl, block_threads=tpb, **pipe)
+        assert e.value.status == -2
+        return
     run_case(wl, f"sizes K{K} N{N} tpb{tpb} [{pipe}]", block_threads=tpb, **pipe)
 
 
-@pytest.mark.parametrize("pipe", PIPES, ids=["fused_lat", "fused_thr", "two_pass"])
+@pytest.mark.parametrize("pipe", PIPES, ids=PIPE_IDS)
 def test_sigma_zero_is_uniform(pipe):
     wl = W.cfg0(K=128, N=10)
     wl.params["sigma"] = 0.0
@@ -209,7 +227,7 @@ def test_sigma_zero_is_uniform(pipe):
     assert np.ptp(g["cost"]) == 0.0
 
 
-@pytest.mark.parametrize("pipe", PIPES, ids=["fused_lat", "fused_thr", "two_pass"])
+@pytest.mark.parametrize("pipe", PIPES, ids=PIPE_IDS)
 def test_saturated_nominal_and_tiny_lambda(pipe):
     wl = W.cfg0(K=256, N=12)
     wl.u_nom[:] = 7.0
