@@ -75,14 +75,18 @@ typedef enum {
 } mppi_pipeline;
 
 typedef enum {
-    MPPI_VARIANT_AUTO = 0,       /* latency kernel when B*K/32 warps cannot fill the chip, else packed (K % 64
+    MPPI_VARIANT_AUTO = 0,       /* pipelined kernel when B*K/32 warps cannot fill the chip, else packed (K % 64
                                     == 0) or scalar throughput                                             */
     MPPI_VARIANT_THROUGHPUT = 1, /* one sample per thread, noise drawn inside the horizon loop; block_threads
                                     samples per block                                                      */
     MPPI_VARIANT_LATENCY = 2,    /* 256-thread blocks: all warps draw the noise of 32 C samples into shared
                                     memory first, then C warps (C = 1, 2 or 4) roll out; fused pipeline only */
+    MPPI_VARIANT_PIPELINED = 4,  /* latency kernel, 256-thread blocks of 32 samples: five warps draw the noise,
+                                    three warps on three SM sub-partitions carry the body-rate, attitude and
+                                    translation chains of the same rollouts, pipelined over the horizon steps
+                                    through shared-memory rings (mbarriers); fused pipeline only           */
     MPPI_VARIANT_PACKED = 3      /* throughput kernel with TWO samples per thread held in packed fp32x2
-                                    registers (sm_100a FFMA2); needs K % 64 == 0; results are bit-identical
+                                    registers (sm_100a FFMA2); needs K % 64 == 0; costs are bit-identical
                                     to MPPI_VARIANT_THROUGHPUT                                             */
 } mppi_variant;
 
@@ -111,8 +115,8 @@ typedef struct {
     int32_t pipeline;  /* mppi_pipeline                                                          */
     int32_t use_graph; /* 1: replay each step as a CUDA graph; 0: plain stream launches          */
     int32_t block_threads; /* threads per block of the rollout kernel: 0 = auto, else 32..256,
-                              a multiple of 32 that divides K (packed variant: 2*block_threads
-                              must divide K)                                                     */
+                              a multiple of 32 that divides K (packed variant: <= 128 and
+                              2*block_threads divides K)                                                   */
     int32_t fast_math; /* 0: IEEE-accurate logf/sincospif/sqrtf/expf; 1: MUFU approximations for
                           the Box-Muller transform (error budget)                 */
     int32_t store_noise; /* 1: also keep dU of the last step for mppi_debug_noise (always kept

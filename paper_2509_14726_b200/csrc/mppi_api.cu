@@ -117,10 +117,12 @@ static int validate(const mppi_params* p)
                                   p->K % p->block_threads != 0),
         "block_threads must be 0 or a multiple of 32 in 32..256 that divides K");
     BAD((int64_t)p->K / 32 > 65535, "K too large");
-    BAD(p->variant < 0 || p->variant > 3, "unknown variant");
-    BAD(p->variant == MPPI_VARIANT_PACKED && (p->K % 64 != 0 || (p->block_threads && p->K % (2 * p->block_threads) != 0)),
-        "the packed variant needs K % 64 == 0 and 2*block_threads dividing K");
-    BAD(p->variant == MPPI_VARIANT_LATENCY && p->pipeline != MPPI_PIPE_FUSED, "the latency variant needs the fused pipeline");
+    BAD(p->variant < 0 || p->variant > 4, "unknown variant");
+    BAD(p->variant == MPPI_VARIANT_PACKED &&
+            (p->K % 64 != 0 || (p->block_threads && (p->block_threads > 128 || p->K % (2 * p->block_threads) != 0))),
+        "the packed variant needs K % 64 == 0, block_threads <= 128 and 2*block_threads dividing K");
+    BAD((p->variant == MPPI_VARIANT_LATENCY || p->variant == MPPI_VARIANT_PIPELINED) && p->pipeline != MPPI_PIPE_FUSED,
+        "the latency variants need the fused pipeline");
 #undef BAD
     return MPPI_OK;
 }
@@ -128,13 +130,18 @@ static int validate(const mppi_params* p)
 // Launch shape.  Latency variant: C rollout warps per 256-thread block, the smallest C in {1,2,4}
 // that brings the grid down to one block per SM (so every rollout warp owns a scheduler).
 // Throughput variant: 256-thread blocks when the grid still covers the chip several times, else 128.
-static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, int* lat_consumers, int* packed)
+static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, int* lat_consumers, int* packed, int* pipe)
 {
     const int64_t warps = (int64_t)p->B * p->K / 32;
     *lat_consumers = 0;
     *packed = 0;
+    *pipe = 0;
     const bool lat_ok = p->pipeline == MPPI_PIPE_FUSED && p->block_threads == 0;
-    if (lat_ok && (p->variant == MPPI_VARIANT_LATENCY || (p->variant == MPPI_VARIANT_AUTO && warps <= 4 * (int64_t)sm_count))) {
+    if (lat_ok && (p->variant == MPPI_VARIANT_PIPELINED || (p->variant == MPPI_VARIANT_AUTO && warps <= 4 * (int64_t)sm_count))) {
+        *pipe = 1; *block_threads = 256;
+        return;
+    }
+    if (lat_ok && p->variant == MPPI_VARIANT_LATENCY) {
         int best = 0;
         for (int c : {1, 2, 4})
             if (p->K % (32 * c) == 0) {
@@ -145,7 +152,8 @@ static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, i
     }
     // packed fp32x2 throughput kernel: two samples per thread
     if (p->K % 64 == 0 && (p->variant == MPPI_VARIANT_PACKED ||
-                           (p->variant == MPPI_VARIANT_AUTO && (!p->block_threads || p->K % (2 * p->block_threads) == 0)))) {
+                           (p->variant == MPPI_VARIANT_AUTO &&
+                            (!p->block_threads || (p->block_threads <= 128 && p->K % (2 * p->block_threads) == 0))))) {
         *packed = 1;
         if (p->block_threads) { *block_threads = p->block_threads; return; }
         for (int tpb : {128, 64, 32})
@@ -228,8 +236,8 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     cfg.objective = p->objective; cfg.fast_math = p->fast_math ? 1 : 0;
     cfg.fused = p->pipeline == MPPI_PIPE_FUSED;
     cfg.store_du = (!cfg.fused || p->store_noise) ? 1 : 0;
-    pick_shape(p, c->sm_count, &cfg.block_threads, &cfg.lat_consumers, &cfg.packed);
-    d.blocks_per_ctrl = cfg.lat_consumers ? p->K / (32 * cfg.lat_consumers)
+    pick_shape(p, c->sm_count, &cfg.block_threads, &cfg.lat_consumers, &cfg.packed, &cfg.pipe);
+    d.blocks_per_ctrl = cfg.pipe ? p->K / 32 : cfg.lat_consumers ? p->K / (32 * cfg.lat_consumers)
                                           : p->K / (cfg.block_threads * (cfg.packed ? 2 : 1));
     cfg.smem_bytes = 0;   // fixed once the track is known
 
@@ -567,7 +575,7 @@ extern "C" int mppi_get_info(mppi_ctx* c, mppi_info* o)
     o->sm_count = c->sm_count;
     o->kernels_per_step = c->cfg.fused ? 1 : 2;
     o->samples_per_thread = c->cfg.packed ? 2 : 1;
-    o->rollout_warps_per_block = c->cfg.lat_consumers ? c->cfg.lat_consumers : c->cfg.block_threads / 32;
+    o->rollout_warps_per_block = c->cfg.pipe ? 3 : c->cfg.lat_consumers ? c->cfg.lat_consumers : c->cfg.block_threads / 32;
     o->l2_bytes = c->l2_bytes;
     o->scratch_bytes = c->scratch_bytes;
     return MPPI_OK;

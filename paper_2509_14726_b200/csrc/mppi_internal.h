@@ -11,6 +11,7 @@ struct LaunchCfg {
     int fused;          // 1: MPPI_PIPE_FUSED, 0: MPPI_PIPE_TWO_PASS
     int block_threads;  // rollout block size
     int packed;         // 1: rollout2_kernel, two samples per thread in fp32x2 registers
+    int pipe;           // 1: rollout_pipe_kernel, one rollout pipelined over three warps (32 samples per block)
     int lat_consumers;  // 0: throughput kernel; 1, 2 or 4: latency kernel with that many rollout warps per block
     size_t smem_bytes;  // dynamic shared memory of the rollout kernel
 };

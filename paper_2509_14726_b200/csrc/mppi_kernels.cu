@@ -11,6 +11,7 @@
 #include "mppi_internal.h"
 #include "mppi_rollout.cuh"
 #include "mppi_packed.cuh"
+#include "mppi_pipe.cuh"
 
 namespace mppi {
 
@@ -19,15 +20,16 @@ namespace mppi {
 //   [N, N + trk)                   track data of the objective
 //   then 16 float4                 reduction scratch (64 floats)
 //   FUSED: nwarps * N float4       per-warp weighted-noise accumulators
-//   FUSED: ceil(2 nblk / 4) float4 (min, Z) pairs / rescale factors of the last-block combine
+//   FUSED: ceil(3 nblk / 4) float4 (min, Z) pairs / rescale factors / index list of the last-block combine
 size_t rollout_smem_bytes(const DevParams& P, const LaunchCfg& c)
 {
     size_t f4 = (size_t)P.N + track_f4(P, c.objective) + 16;
+    if (c.pipe) return (f4 + pipe_extra_f4(P.N, P.blocks_per_ctrl)) * sizeof(float4);
     if (c.lat_consumers > 0) {
-        f4 += (size_t)P.N * (32 * c.lat_consumers + 1) + 32 + (2 * P.blocks_per_ctrl + 3) / 4;
+        f4 += (size_t)P.N * (32 * c.lat_consumers + 1) + 32 + (3 * P.blocks_per_ctrl + 3) / 4;
         return f4 * sizeof(float4);
     }
-    if (c.fused) f4 += (size_t)(c.block_threads / 32) * P.N + (2 * P.blocks_per_ctrl + 3) / 4;
+    if (c.fused) f4 += (size_t)(c.block_threads / 32) * P.N + (3 * P.blocks_per_ctrl + 3) / 4;
     return f4 * sizeof(float4);
 }
 
@@ -466,8 +468,25 @@ static LatFn pick_lat(const LaunchCfg& c)
     }
 }
 
+typedef void (*PipeFn)(const DevParams, const StepArgs);
+template <int OBJ>
+static PipeFn pick_pipe1(const LaunchCfg& c)
+{
+    if (c.fast_math) return c.store_du ? rollout_pipe_kernel<OBJ, 1, true> : rollout_pipe_kernel<OBJ, 1, false>;
+    return c.store_du ? rollout_pipe_kernel<OBJ, 0, true> : rollout_pipe_kernel<OBJ, 0, false>;
+}
+static PipeFn pick_pipe(const LaunchCfg& c)
+{
+    switch (c.objective) {
+        case OBJ_GATE: return pick_pipe1<OBJ_GATE>(c);
+        case OBJ_TRACK: return pick_pipe1<OBJ_TRACK>(c);
+        default: return pick_pipe1<OBJ_CONTOUR>(c);
+    }
+}
+
 const void* rollout_kernel_ptr(const LaunchCfg& c)
 {
+    if (c.pipe) return reinterpret_cast<const void*>(pick_pipe(c));
     return c.lat_consumers > 0 ? reinterpret_cast<const void*>(pick_lat(c)) : reinterpret_cast<const void*>(pick(c));
 }
 const void* reduce_kernel_ptr() { return reinterpret_cast<const void*>(reduce_kernel); }
@@ -476,7 +495,8 @@ const void* sim_kernel_ptr() { return reinterpret_cast<const void*>(sim_kernel<O
 cudaError_t launch_rollout(const DevParams& P, const StepArgs& A, const LaunchCfg& c, cudaStream_t s)
 {
     const dim3 grid(P.blocks_per_ctrl, P.B), block(c.block_threads);
-    if (c.lat_consumers > 0) pick_lat(c)<<<grid, block, c.smem_bytes, s>>>(P, A, c.lat_consumers);
+    if (c.pipe) pick_pipe(c)<<<grid, block, c.smem_bytes, s>>>(P, A);
+    else if (c.lat_consumers > 0) pick_lat(c)<<<grid, block, c.smem_bytes, s>>>(P, A, c.lat_consumers);
     else pick(c)<<<grid, block, c.smem_bytes, s>>>(P, A);
     return cudaGetLastError();
 }

@@ -136,57 +136,107 @@ __device__ __forceinline__ float rollout_cost(const DevParams& P, const float4* 
     return J;
 }
 
-// Fused softmax update, second half ("threadfence reduction").  Every block of controller b has
-// written its partial  part = { S[4N] = sum_k e_k dU_k, m = min_k J_k, Z = sum_k e_k }  with
+// Fused softmax update, second half ("last block done").  Every block of controller b has written
+// its partial  part = { S[4N] = sum_k e_k dU_k, m = min_k J_k, Z = sum_k e_k }  with
 // e_k = exp(-(J_k - m)/lambda)  (online-softmax form of eq.(4),(5)).  The block that
 // takes the last ticket rescales the nb partials to the global minimum beta and writes
 //   u_new = u_nom + sum_q S_q exp(-(m_q - beta)/lambda) / Z_tot,   w_k = exp(-(J_k - beta)/lambda) / Z_tot.
 // Partials whose rescale factor underflows to 0 contribute exactly 0 and are not read.
-// s_pair: 2 nb floats of shared memory.  All threads of the block must call this.
+//
+// This runs after the last rollout of the controller has finished, so it is on the critical path of
+// the iteration latency: the chain is kept to three L2 round trips -- ticket; (m, Z) pairs together
+// with the first costs; the S rows of the few partials that still count -- and the contributing
+// partials are compacted (deterministically, by index) so that nobody scans nb scale factors.
+// s_pair: 3 nb floats of shared memory.  All threads of the block must call this.
+__device__ __forceinline__ unsigned ticket_acq_rel(unsigned* ctr)
+{
+    unsigned old;
+    asm volatile("atom.add.acq_rel.gpu.global.u32 %0, [%1], 1;" : "=r"(old) : "l"(ctr) : "memory");
+    return old;
+}
+
 template <int MATH>
 __device__ __forceinline__ void publish_and_combine(const DevParams& P, const StepArgs& A, int b, int nb,
                                                     const float4* s_unom, float* s_red, float* s_pair)
 {
-    const int tid = threadIdx.x, N = P.N, stride = 4 * N + 4;
+    const int tid = threadIdx.x, lane = tid & 31, N = P.N, stride = 4 * N + 4, nthr = blockDim.x;
     int* s_flag = reinterpret_cast<int*>(s_red) + 48;
-    __threadfence();
-    __syncthreads();
-    if (tid == 0) *s_flag = (atomicAdd(&A.counters[b], 1u) == (unsigned)(nb - 1));
+    int* s_cnt = s_flag + 1;
+    __syncthreads();                               // the block's partial is written (CTA-scope order) ...
+    if (tid == 0) *s_flag = (ticket_acq_rel(&A.counters[b]) == (unsigned)(nb - 1));   // ... and released here
     __syncthreads();
     if (!*s_flag) return;
-    __threadfence();
 
     const float* pb = A.partials + (size_t)b * nb * stride;
     float* s_scale = s_pair;
     float* s_z = s_pair + nb;
+    int* s_list = reinterpret_cast<int*>(s_pair + 2 * nb);
+    // round trip 2: the (m, Z) pairs and this thread's first costs, all in flight together
+    const float4* c4 = reinterpret_cast<const float4*>(A.cost + (size_t)b * P.K);
+    const int n4 = P.K >> 2;
+    constexpr int PRE = 4;
+    float4 cpre[PRE];
+#pragma unroll
+    for (int r = 0; r < PRE; ++r)
+        cpre[r] = tid + r * nthr < n4 ? __ldcg(c4 + tid + r * nthr) : make_float4(0.f, 0.f, 0.f, 0.f);
     float bm = __int_as_float(0x7f800000);
-    for (int j = tid; j < nb; j += blockDim.x) {
+    for (int j = tid; j < nb; j += nthr) {
         const float2 mz = __ldcg(reinterpret_cast<const float2*>(pb + (size_t)j * stride + 4 * N));
         s_scale[j] = mz.x; s_z[j] = mz.y;
         bm = fminf(bm, mz.x);
     }
     const float beta = block_min(bm, s_red);
     float zz = 0.0f;
-    for (int j = tid; j < nb; j += blockDim.x) {
+    for (int j = tid; j < nb; j += nthr) {
         const float sc = exp_weight<MATH>((beta - s_scale[j]) * P.inv_lambda);
         s_scale[j] = sc;
         zz = fmaf(s_z[j], sc, zz);
     }
     const float Z = block_sum(zz, s_red);      // its barriers also order the s_scale writes
     const float invZ = 1.0f / Z;
-    for (int j = tid; j < 4 * N; j += blockDim.x) {
+    // deterministic compaction of the partials with a non-zero scale (warp 0, ascending index)
+    if (tid < 32) {
+        int cnt = 0;
+        for (int j0 = 0; j0 < nb; j0 += 32) {
+            const int j = j0 + lane;
+            const bool on = j < nb && s_scale[j] != 0.0f;
+            const unsigned msk = __ballot_sync(kFull, on);
+            if (on) s_list[cnt + __popc(msk & ((1u << lane) - 1u))] = j;
+            cnt += __popc(msk);
+        }
+        if (lane == 0) *s_cnt = cnt;
+    }
+    __syncthreads();
+    const int cnt = *s_cnt;
+    // round trip 3: S rows of the contributing partials
+    for (int j = tid; j < 4 * N; j += nthr) {
         float acc = 0.0f;
-        for (int q = 0; q < nb; ++q) {
-            const float sc = s_scale[q];       // block-uniform: no divergence
-            if (sc != 0.0f) acc = fmaf(__ldcg(pb + (size_t)q * stride + j), sc, acc);
+        int i = 0;
+        for (; i + 4 <= cnt; i += 4) {
+            const int q0 = s_list[i], q1 = s_list[i + 1], q2 = s_list[i + 2], q3 = s_list[i + 3];
+            const float v0 = __ldcg(pb + (size_t)q0 * stride + j), v1 = __ldcg(pb + (size_t)q1 * stride + j),
+                        v2 = __ldcg(pb + (size_t)q2 * stride + j), v3 = __ldcg(pb + (size_t)q3 * stride + j);
+            acc = fmaf(v0, s_scale[q0], acc); acc = fmaf(v1, s_scale[q1], acc);
+            acc = fmaf(v2, s_scale[q2], acc); acc = fmaf(v3, s_scale[q3], acc);
+        }
+        for (; i < cnt; ++i) {
+            const int q = s_list[i];
+            acc = fmaf(__ldcg(pb + (size_t)q * stride + j), s_scale[q], acc);
         }
         A.u_new[(size_t)b * 4 * N + j] = fmaf(acc, invZ, reinterpret_cast<const float*>(s_unom)[j]);
     }
-    const float4* c4 = reinterpret_cast<const float4*>(A.cost + (size_t)b * P.K);
     float4* w4 = reinterpret_cast<float4*>(A.weights + (size_t)b * P.K);
     const float nil = -P.inv_lambda;
+#pragma unroll
+    for (int r = 0; r < PRE; ++r) {
+        const int i = tid + r * nthr;
+        const float4 c = cpre[r];
+        if (i < n4)
+            w4[i] = make_float4(exp_weight<MATH>((c.x - beta) * nil) * invZ, exp_weight<MATH>((c.y - beta) * nil) * invZ,
+                                exp_weight<MATH>((c.z - beta) * nil) * invZ, exp_weight<MATH>((c.w - beta) * nil) * invZ);
+    }
 #pragma unroll 4
-    for (int i = tid; i < P.K / 4; i += blockDim.x) {
+    for (int i = tid + PRE * nthr; i < n4; i += nthr) {
         const float4 c = __ldcg(c4 + i);
         w4[i] = make_float4(exp_weight<MATH>((c.x - beta) * nil) * invZ, exp_weight<MATH>((c.y - beta) * nil) * invZ,
                             exp_weight<MATH>((c.z - beta) * nil) * invZ, exp_weight<MATH>((c.w - beta) * nil) * invZ);

@@ -35,9 +35,9 @@ def run_case(wl, tag, it=0, **opts):
 
 # fused pipeline with the latency / scalar throughput / packed fp32x2 throughput kernels; two-pass
 # pipeline with the packed (AUTO picks it when K % 64 == 0) and the scalar rollout kernel
-PIPES = [dict(pipeline=0, variant=2), dict(pipeline=0, variant=1), dict(pipeline=0, variant=3), dict(pipeline=1),
-         dict(pipeline=1, variant=1)]
-PIPE_IDS = ["fused_lat", "fused_thr", "fused_pk", "two_pass", "two_pass_thr"]
+PIPES = [dict(pipeline=0, variant=4), dict(pipeline=0, variant=2), dict(pipeline=0, variant=1), dict(pipeline=0, variant=3),
+         dict(pipeline=1), dict(pipeline=1, variant=1)]
+PIPE_IDS = ["fused_pipe", "fused_lat", "fused_thr", "fused_pk", "two_pass", "two_pass_thr"]
 MATH = [dict(fast_math=0), dict(fast_math=1)]
 
 
@@ -199,6 +199,12 @@ def test_latency_variant_shapes(K, N, B, consumers):
     assert info["block_threads"] == 256 and info["blocks_per_controller"] == K // (32 * consumers)
     m.close()
     run_case(wl, f"lat K{K} N{N} B{B}", variant=2)
+    # the pipelined kernel (three warps per rollout): always 32 samples per 256-thread block
+    m = Pz.make_ctx(wl, variant=4)
+    info = m.info()
+    assert info["block_threads"] == 256 and info["blocks_per_controller"] == K // 32
+    m.close()
+    run_case(wl, f"pipe K{K} N{N} B{B}", variant=4)
 
 
 # ---- ragged / degenerate / maximum sizes ----------------------------------------------------------
@@ -208,9 +214,9 @@ def test_latency_variant_shapes(K, N, B, consumers):
 @pytest.mark.parametrize("pipe", PIPES, ids=PIPE_IDS)
 def test_sizes_and_block_shapes(K, N, tpb, pipe):
     wl = W.stress_gate(K=K, N=N)
-    if pipe.get("variant") == 3 and K % (2 * tpb) != 0:
+    if pipe.get("variant") == 3 and (K % (2 * tpb) != 0 or tpb > 128):
         from paper_2509_14726_b200 import binding as Bd
-        with pytest.raises(Bd.MppiError) as e:                 # two samples per thread: 2*tpb must divide K
+        with pytest.raises(Bd.MppiError) as e:                 # two samples per thread: tpb <= 128, 2*tpb divides K
             Pz.make_ctx(wl, block_threads=tpb, **pipe)
         assert e.value.status == -2
         return
