@@ -12,7 +12,9 @@
 //   warp 1 (Q)  attitude chain:  the four RK4 stage quaternions      -> ring Q (16 floats / sample)
 //   warp 2 (P)  translation: r(q_i) sums, p, v update, position part of the objective
 //
-// W runs ahead of Q, Q ahead of P, each by up to kPipeDepth steps.  Every warp accumulates the terms
+// The rings are handed over in CHUNKS of kPipeChunk steps (one mbarrier wait + one arrive per chunk and
+// side: a per-step handshake costs more than the arithmetic of a step -- measured), W runs ahead of Q
+// and Q ahead of P by up to kPipeDepth chunks.  Every warp accumulates the terms
 // of the objective that depend on its part of the state; they are added at the end.  The state
 // trajectory is bit-identical to rk4_step (same operations in the same order per component).
 // Block = 256 threads = 32 samples; grid = (K / 32, B).
@@ -21,9 +23,10 @@
 
 namespace mppi {
 
-constexpr int kPipeDepth = 8;      // ring slots (steps in flight between two stages of the pipeline)
+constexpr int kPipeChunk = 5;      // steps per ring slot = steps per thrust mbarrier = noise warps
+constexpr int kPipeDepth = 4;      // ring slots (chunks in flight between two stages of the pipeline)
 constexpr int kPipeThreads = 256;
-constexpr int kPipeNoiseWarps = 5;
+constexpr int kPipeNoiseWarps = kPipeChunk;
 
 // ---- mbarrier helpers (CTA scope, shared memory) ------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -49,12 +52,13 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
 // float4 units of dynamic shared memory after the nominal + track + 16 float4 of reduction scratch
 __host__ __device__ inline size_t pipe_extra_f4(int N, int nb)
 {
-    return (size_t)N * 33                         // s_T   [N][33] thrusts
-           + (size_t)kPipeDepth * 3 * 32          // ring W
-           + (size_t)kPipeDepth * 4 * 32          // ring Q
-           + 24 + 8                               // s_J [3][32], s_e [32]
-           + (size_t)(3 * nb + 3) / 4             // combine scratch
-           + (size_t)(N + 4 * kPipeDepth + 1) / 2;   // mbarriers (8 B each)
+    const int nchunks = (N + kPipeChunk - 1) / kPipeChunk;
+    return (size_t)N * 33                                   // s_T   [N][33] thrusts
+           + (size_t)kPipeDepth * kPipeChunk * 3 * 32       // ring W
+           + (size_t)kPipeDepth * kPipeChunk * 4 * 32       // ring Q
+           + 24 + 8                                         // s_J [3][32], s_e [32]
+           + (size_t)(3 * nb + 3) / 4                       // combine scratch
+           + (size_t)(nchunks + 4 * kPipeDepth + 1) / 2;    // mbarriers (8 B each)
 }
 
 // quaternion rate times two: G(q, w) = q (x) (0, w)    (the 1/2 is folded into the step constants)
@@ -70,27 +74,29 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
     extern __shared__ float4 smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int b = blockIdx.y, N = P.N;
-    constexpr int RS = 33, D = kPipeDepth;
+    constexpr int RS = 33, D = kPipeDepth, C = kPipeChunk;
     const int kbase = blockIdx.x * 32;
+    const int nchunks = (N + C - 1) / C;
 
     float4* s_unom = smem;
     float4* s_trk = smem + N;
     float* s_red = reinterpret_cast<float*>(s_trk + track_f4(P, OBJ));   // 64 floats
     float4* s_T = reinterpret_cast<float4*>(s_red + 64);                 // [N][RS]
-    float4* s_w = s_T + (size_t)N * RS;                                  // [D][3][32]
-    float4* s_q = s_w + D * 3 * 32;                                      // [D][4][32]
-    float* s_J = reinterpret_cast<float*>(s_q + D * 4 * 32);             // [3][32]
+    float4* s_w = s_T + (size_t)N * RS;                                  // [D][C][3][32]
+    float4* s_q = s_w + D * C * 3 * 32;                                  // [D][C][4][32]
+    float* s_J = reinterpret_cast<float*>(s_q + D * C * 4 * 32);         // [3][32]
     float* s_e = s_J + 96;                                               // [32]
     float* s_pair = s_e + 32;                                            // 3 nb floats
     uint64_t* bar_T = reinterpret_cast<uint64_t*>(reinterpret_cast<float4*>(s_pair) + (3 * P.blocks_per_ctrl + 3) / 4);
-    uint64_t* bar_wf = bar_T + N;          // ring W full / empty, ring Q full / empty
+    uint64_t* bar_wf = bar_T + nchunks;    // ring W full / empty, ring Q full / empty
     uint64_t* bar_we = bar_wf + D;
     uint64_t* bar_qf = bar_we + D;
     uint64_t* bar_qe = bar_qf + D;
 
     const int start = A.start[b];
     stage_inputs<OBJ>(P, A, b, start, s_unom, s_trk);
-    for (int i = tid; i < N + 4 * D; i += kPipeThreads) mbar_init(bar_T + i, 32);
+    for (int i = tid; i < nchunks + 4 * D; i += kPipeThreads)
+        mbar_init(bar_T + i, i < nchunks ? 32 * min(C, N - i * C) : 32);
     const State x0 = load_state(A.x0 + 13 * b);
     __syncthreads();
     const int i0 = OBJ == OBJ_CONTOUR ? contour_start_index(P, s_trk, start, x0, s_red) : 0;
@@ -101,7 +107,7 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
             const float4 un = s_unom[t];
             const float4 T = sample_thrust<MATH>(P, A.rk, (uint32_t)(kbase + lane), (uint32_t)t, A.iter, (uint32_t)b, un);
             s_T[t * RS + lane] = T;
-            mbar_arrive(bar_T + t);
+            mbar_arrive(bar_T + t / C);
             if (STORE_DU)
                 A.du[((size_t)b * N + t) * P.K + kbase + lane] = make_float4(T.x - un.x, T.y - un.y, T.z - un.z, T.w - un.w);
         }
@@ -109,44 +115,47 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
         // ---- W: body rates.  omega' = J^-1 (tau - omega x J omega), PAPER.md:65-70 ----
         float ox = x0.ox, oy = x0.oy, oz = x0.oz;
         float acc = 0.0f;      // gate: sum |omega_{t+1}|^2; contour / track: this warp's cost terms
-        for (int t = 0; t < N; ++t) {
-            const int s = t & (D - 1);
-            mbar_wait(bar_T + t, 0);
-            const float4 T = s_T[t * RS + lane];
-            if (OBJ == OBJ_TRACK) {
-                const float4 c = s_trk[4 * t + 2], d = s_trk[4 * t + 3];
-                const float wx = ox - c.z, wy = oy - c.w, wz = oz - d.x;
-                const float a0 = T.x - P.hover, a1 = T.y - P.hover, a2 = T.z - P.hover, a3 = T.w - P.hover;
-                acc = fmaf(P.Qw, wx * wx + wy * wy + wz * wz, acc);
-                acc = fmaf(P.R, a0 * a0 + a1 * a1 + a2 * a2 + a3 * a3, acc);
+        for (int c = 0; c < nchunks; ++c) {
+            const int s = c & (D - 1), cnt = min(C, N - c * C);
+            mbar_wait(bar_T + c, 0);                           // the chunk's thrusts are drawn
+            mbar_wait(bar_we + s, ((c / D) & 1) ^ 1);          // Q has drained this slot
+            for (int j = 0; j < cnt; ++j) {
+                const int t = c * C + j;
+                const float4 T = s_T[t * RS + lane];
+                if (OBJ == OBJ_TRACK) {
+                    const float4 r2 = s_trk[4 * t + 2], r3 = s_trk[4 * t + 3];
+                    const float wx = ox - r2.z, wy = oy - r2.w, wz = oz - r3.x;
+                    const float a0 = T.x - P.hover, a1 = T.y - P.hover, a2 = T.z - P.hover, a3 = T.w - P.hover;
+                    acc = fmaf(P.Qw, wx * wx + wy * wy + wz * wz, acc);
+                    acc = fmaf(P.R, a0 * a0 + a1 * a1 + a2 * a2 + a3 * a3, acc);
+                }
+                const float s01 = T.x + T.y, s23 = T.z + T.w;
+                const float ax = P.ltx * (s01 - s23);
+                const float ay = P.lty * ((T.y + T.z) - (T.x + T.w));
+                const float az = P.ltz * ((T.x + T.z) - (T.y + T.w));
+                float kx = fmaf(P.gyx, oy * oz, ax), ky = fmaf(P.gyy, oz * ox, ay), kz = fmaf(P.gyz, ox * oy, az);
+                float nx = fmaf(P.h6, kx, ox), ny = fmaf(P.h6, ky, oy), nz = fmaf(P.h6, kz, oz);
+                const float o2x = fmaf(P.h2, kx, ox), o2y = fmaf(P.h2, ky, oy), o2z = fmaf(P.h2, kz, oz);
+                kx = fmaf(P.gyx, o2y * o2z, ax); ky = fmaf(P.gyy, o2z * o2x, ay); kz = fmaf(P.gyz, o2x * o2y, az);
+                nx = fmaf(P.h3, kx, nx); ny = fmaf(P.h3, ky, ny); nz = fmaf(P.h3, kz, nz);
+                const float o3x = fmaf(P.h2, kx, ox), o3y = fmaf(P.h2, ky, oy), o3z = fmaf(P.h2, kz, oz);
+                kx = fmaf(P.gyx, o3y * o3z, ax); ky = fmaf(P.gyy, o3z * o3x, ay); kz = fmaf(P.gyz, o3x * o3y, az);
+                nx = fmaf(P.h3, kx, nx); ny = fmaf(P.h3, ky, ny); nz = fmaf(P.h3, kz, nz);
+                const float o4x = fmaf(P.dt, kx, ox), o4y = fmaf(P.dt, ky, oy), o4z = fmaf(P.dt, kz, oz);
+                float4* w = s_w + (s * C + j) * 96 + lane;
+                w[0] = make_float4(ox, oy, oz, o2x);
+                w[32] = make_float4(o2y, o2z, o3x, o3y);
+                w[64] = make_float4(o3z, o4x, o4y, o4z);
+                kx = fmaf(P.gyx, o4y * o4z, ax); ky = fmaf(P.gyy, o4z * o4x, ay); kz = fmaf(P.gyz, o4x * o4y, az);
+                ox = fmaf(P.h6, kx, nx); oy = fmaf(P.h6, ky, ny); oz = fmaf(P.h6, kz, nz);
+                if (OBJ == OBJ_GATE) acc = fmaf(oz, oz, fmaf(oy, oy, fmaf(ox, ox, acc)));
+                if (OBJ == OBJ_CONTOUR) acc = fmaf(P.w_omega, ox * ox + oy * oy + oz * oz, acc);
             }
-            const float s01 = T.x + T.y, s23 = T.z + T.w;
-            const float ax = P.ltx * (s01 - s23);
-            const float ay = P.lty * ((T.y + T.z) - (T.x + T.w));
-            const float az = P.ltz * ((T.x + T.z) - (T.y + T.w));
-            float kx = fmaf(P.gyx, oy * oz, ax), ky = fmaf(P.gyy, oz * ox, ay), kz = fmaf(P.gyz, ox * oy, az);
-            float nx = fmaf(P.h6, kx, ox), ny = fmaf(P.h6, ky, oy), nz = fmaf(P.h6, kz, oz);
-            const float o2x = fmaf(P.h2, kx, ox), o2y = fmaf(P.h2, ky, oy), o2z = fmaf(P.h2, kz, oz);
-            kx = fmaf(P.gyx, o2y * o2z, ax); ky = fmaf(P.gyy, o2z * o2x, ay); kz = fmaf(P.gyz, o2x * o2y, az);
-            nx = fmaf(P.h3, kx, nx); ny = fmaf(P.h3, ky, ny); nz = fmaf(P.h3, kz, nz);
-            const float o3x = fmaf(P.h2, kx, ox), o3y = fmaf(P.h2, ky, oy), o3z = fmaf(P.h2, kz, oz);
-            kx = fmaf(P.gyx, o3y * o3z, ax); ky = fmaf(P.gyy, o3z * o3x, ay); kz = fmaf(P.gyz, o3x * o3y, az);
-            nx = fmaf(P.h3, kx, nx); ny = fmaf(P.h3, ky, ny); nz = fmaf(P.h3, kz, nz);
-            const float o4x = fmaf(P.dt, kx, ox), o4y = fmaf(P.dt, ky, oy), o4z = fmaf(P.dt, kz, oz);
-            mbar_wait(bar_we + s, ((t / D) & 1) ^ 1);
-            float4* w = s_w + s * 96 + lane;
-            w[0] = make_float4(ox, oy, oz, o2x);
-            w[32] = make_float4(o2y, o2z, o3x, o3y);
-            w[64] = make_float4(o3z, o4x, o4y, o4z);
             mbar_arrive(bar_wf + s);
-            kx = fmaf(P.gyx, o4y * o4z, ax); ky = fmaf(P.gyy, o4z * o4x, ay); kz = fmaf(P.gyz, o4x * o4y, az);
-            ox = fmaf(P.h6, kx, nx); oy = fmaf(P.h6, ky, ny); oz = fmaf(P.h6, kz, nz);
-            if (OBJ == OBJ_GATE) acc = fmaf(oz, oz, fmaf(oy, oy, fmaf(ox, ox, acc)));
-            if (OBJ == OBJ_CONTOUR) acc = fmaf(P.w_omega, ox * ox + oy * oy + oz * oz, acc);
         }
         if (OBJ == OBJ_TRACK) {
-            const float4 c = s_trk[4 * N + 2], d = s_trk[4 * N + 3];
-            const float wx = ox - c.z, wy = oy - c.w, wz = oz - d.x;
+            const float4 r2 = s_trk[4 * N + 2], r3 = s_trk[4 * N + 3];
+            const float wx = ox - r2.z, wy = oy - r2.w, wz = oz - r3.x;
             acc = fmaf(P.Qw, wx * wx + wy * wy + wz * wz, acc);
         }
         s_J[lane] = acc;
@@ -161,34 +170,36 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
             const float e0 = fmaf(-sg, a.w, qw), e1 = fmaf(-sg, r.x, qx), e2 = fmaf(-sg, r.y, qy), e3 = fmaf(-sg, r.z, qz);
             acc = fmaf(P.Qq, e0 * e0 + e1 * e1 + e2 * e2 + e3 * e3, acc);
         };
-        for (int t = 0; t < N; ++t) {
-            const int s = t & (D - 1);
-            if (OBJ == OBJ_TRACK) quat_term(s_trk + 4 * t);
-            mbar_wait(bar_wf + s, (t / D) & 1);
-            const float4* w = s_w + s * 96 + lane;
-            const float4 f0 = w[0], f1 = w[32], f2 = w[64];
+        for (int c = 0; c < nchunks; ++c) {
+            const int s = c & (D - 1), cnt = min(C, N - c * C);
+            mbar_wait(bar_wf + s, (c / D) & 1);                // W has filled this slot
+            mbar_wait(bar_qe + s, ((c / D) & 1) ^ 1);          // P has drained the slot written below
+            for (int j = 0; j < cnt; ++j) {
+                if (OBJ == OBJ_TRACK) quat_term(s_trk + 4 * (c * C + j));
+                const float4* w = s_w + (s * C + j) * 96 + lane;
+                const float4 f0 = w[0], f1 = w[32], f2 = w[64];
+                float gw, gx, gy, gz;
+                MPPI_G(qw, qx, qy, qz, f0.x, f0.y, f0.z, gw, gx, gy, gz)
+                float nw = fmaf(P.h12, gw, qw), nx = fmaf(P.h12, gx, qx), ny = fmaf(P.h12, gy, qy), nz = fmaf(P.h12, gz, qz);
+                const float q2w = fmaf(P.h4, gw, qw), q2x = fmaf(P.h4, gx, qx), q2y = fmaf(P.h4, gy, qy), q2z = fmaf(P.h4, gz, qz);
+                MPPI_G(q2w, q2x, q2y, q2z, f0.w, f1.x, f1.y, gw, gx, gy, gz)
+                nw = fmaf(P.h6, gw, nw); nx = fmaf(P.h6, gx, nx); ny = fmaf(P.h6, gy, ny); nz = fmaf(P.h6, gz, nz);
+                const float q3w = fmaf(P.h4, gw, qw), q3x = fmaf(P.h4, gx, qx), q3y = fmaf(P.h4, gy, qy), q3z = fmaf(P.h4, gz, qz);
+                MPPI_G(q3w, q3x, q3y, q3z, f1.z, f1.w, f2.x, gw, gx, gy, gz)
+                nw = fmaf(P.h6, gw, nw); nx = fmaf(P.h6, gx, nx); ny = fmaf(P.h6, gy, ny); nz = fmaf(P.h6, gz, nz);
+                const float q4w = fmaf(P.h2, gw, qw), q4x = fmaf(P.h2, gx, qx), q4y = fmaf(P.h2, gy, qy), q4z = fmaf(P.h2, gz, qz);
+                float4* o = s_q + (s * C + j) * 128 + lane;
+                o[0] = make_float4(qw, qx, qy, qz);
+                o[32] = make_float4(q2w, q2x, q2y, q2z);
+                o[64] = make_float4(q3w, q3x, q3y, q3z);
+                o[96] = make_float4(q4w, q4x, q4y, q4z);
+                MPPI_G(q4w, q4x, q4y, q4z, f2.y, f2.z, f2.w, gw, gx, gy, gz)
+                nw = fmaf(P.h12, gw, nw); nx = fmaf(P.h12, gx, nx); ny = fmaf(P.h12, gy, ny); nz = fmaf(P.h12, gz, nz);
+                const float inv = rsqrtf(fmaf(nz, nz, fmaf(ny, ny, fmaf(nx, nx, nw * nw))));
+                qw = nw * inv; qx = nx * inv; qy = ny * inv; qz = nz * inv;
+            }
             mbar_arrive(bar_we + s);
-            float gw, gx, gy, gz;
-            MPPI_G(qw, qx, qy, qz, f0.x, f0.y, f0.z, gw, gx, gy, gz)
-            float nw = fmaf(P.h12, gw, qw), nx = fmaf(P.h12, gx, qx), ny = fmaf(P.h12, gy, qy), nz = fmaf(P.h12, gz, qz);
-            const float q2w = fmaf(P.h4, gw, qw), q2x = fmaf(P.h4, gx, qx), q2y = fmaf(P.h4, gy, qy), q2z = fmaf(P.h4, gz, qz);
-            MPPI_G(q2w, q2x, q2y, q2z, f0.w, f1.x, f1.y, gw, gx, gy, gz)
-            nw = fmaf(P.h6, gw, nw); nx = fmaf(P.h6, gx, nx); ny = fmaf(P.h6, gy, ny); nz = fmaf(P.h6, gz, nz);
-            const float q3w = fmaf(P.h4, gw, qw), q3x = fmaf(P.h4, gx, qx), q3y = fmaf(P.h4, gy, qy), q3z = fmaf(P.h4, gz, qz);
-            MPPI_G(q3w, q3x, q3y, q3z, f1.z, f1.w, f2.x, gw, gx, gy, gz)
-            nw = fmaf(P.h6, gw, nw); nx = fmaf(P.h6, gx, nx); ny = fmaf(P.h6, gy, ny); nz = fmaf(P.h6, gz, nz);
-            const float q4w = fmaf(P.h2, gw, qw), q4x = fmaf(P.h2, gx, qx), q4y = fmaf(P.h2, gy, qy), q4z = fmaf(P.h2, gz, qz);
-            mbar_wait(bar_qe + s, ((t / D) & 1) ^ 1);
-            float4* o = s_q + s * 128 + lane;
-            o[0] = make_float4(qw, qx, qy, qz);
-            o[32] = make_float4(q2w, q2x, q2y, q2z);
-            o[64] = make_float4(q3w, q3x, q3y, q3z);
-            o[96] = make_float4(q4w, q4x, q4y, q4z);
             mbar_arrive(bar_qf + s);
-            MPPI_G(q4w, q4x, q4y, q4z, f2.y, f2.z, f2.w, gw, gx, gy, gz)
-            nw = fmaf(P.h12, gw, nw); nx = fmaf(P.h12, gx, nx); ny = fmaf(P.h12, gy, ny); nz = fmaf(P.h12, gz, nz);
-            const float inv = rsqrtf(fmaf(nz, nz, fmaf(ny, ny, fmaf(nx, nx, nw * nw))));
-            qw = nw * inv; qx = nx * inv; qy = ny * inv; qz = nz * inv;
         }
         if (OBJ == OBJ_TRACK) quat_term(s_trk + 4 * N);
         s_J[32 + lane] = acc;
@@ -202,37 +213,39 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
         if (OBJ == OBJ_GATE) gc.init<MATH>(P, s_trk, start, x);
         if (OBJ == OBJ_CONTOUR) cc.init(s_trk, i0, x);
         auto pv_term = [&](const float4* row) {
-            const float4 a = row[0], r = row[1], c = row[2];
+            const float4 a = row[0], r = row[1], r2 = row[2];
             const float ex = x.px - a.x, ey = x.py - a.y, ez = x.pz - a.z;
-            const float ux = x.vx - r.w, uy = x.vy - c.x, uz = x.vz - c.y;
+            const float ux = x.vx - r.w, uy = x.vy - r2.x, uz = x.vz - r2.y;
             J = fmaf(P.Qp, ex * ex + ey * ey + ez * ez, J);
             J = fmaf(P.Qv, ux * ux + uy * uy + uz * uz, J);
         };
-        for (int t = 0; t < N; ++t) {
-            const int s = t & (D - 1);
-            mbar_wait(bar_T + t, 0);
-            const float4 T = s_T[t * RS + lane];
-            if (OBJ == OBJ_TRACK) pv_term(s_trk + 4 * t);
-            const float c = ((T.x + T.y) + (T.z + T.w)) * P.inv_mass;
-            const float cz0 = c - P.g, kp = c * P.hh3, kv = c * P.h3;
-            mbar_wait(bar_qf + s, (t / D) & 1);
-            const float4* o = s_q + s * 128 + lane;
-            const float4 q1 = o[0], q2 = o[32], q3 = o[64], q4 = o[96];
-            mbar_arrive(bar_qe + s);
+        for (int c = 0; c < nchunks; ++c) {
+            const int s = c & (D - 1), cnt = min(C, N - c * C);
+            mbar_wait(bar_qf + s, (c / D) & 1);                // Q has filled this slot (its thrusts are older)
+            for (int j = 0; j < cnt; ++j) {
+                const int t = c * C + j;
+                const float4 T = s_T[t * RS + lane];
+                const float4* o = s_q + (s * C + j) * 128 + lane;
+                const float4 q1 = o[0], q2 = o[32], q3 = o[64], q4 = o[96];
+                if (OBJ == OBJ_TRACK) pv_term(s_trk + 4 * t);
+                const float cm = ((T.x + T.y) + (T.z + T.w)) * P.inv_mass;
+                const float cz0 = cm - P.g, kp = cm * P.hh3, kv = cm * P.h3;
 #define MPPI_R(Q, RX, RY, RZ)                                                              \
     const float RX = fmaf(Q.x, Q.z, Q.y * Q.w), RY = fmaf(-Q.x, Q.y, Q.z * Q.w), RZ = fmaf(Q.z, Q.z, Q.y * Q.y);
-            MPPI_R(q1, r1x, r1y, r1z) MPPI_R(q2, r2x, r2y, r2z) MPPI_R(q3, r3x, r3y, r3z) MPPI_R(q4, r4x, r4y, r4z)
+                MPPI_R(q1, r1x, r1y, r1z) MPPI_R(q2, r2x, r2y, r2z) MPPI_R(q3, r3x, r3y, r3z) MPPI_R(q4, r4x, r4y, r4z)
 #undef MPPI_R
-            const float mx = r2x + r3x, my = r2y + r3y, mz = r2z + r3z;
-            const float Ax = r1x + mx, Ay = r1y + my, Az = r1z + mz;
-            x.px = fmaf(kp, Ax, fmaf(P.dt, x.vx, x.px));
-            x.py = fmaf(kp, Ay, fmaf(P.dt, x.vy, x.py));
-            x.pz = fmaf(-kp, Az, fmaf(P.hh2, cz0, fmaf(P.dt, x.vz, x.pz)));
-            x.vx = fmaf(kv, (Ax + mx) + r4x, x.vx);
-            x.vy = fmaf(kv, (Ay + my) + r4y, x.vy);
-            x.vz = fmaf(-kv, (Az + mz) + r4z, fmaf(P.dt, cz0, x.vz));
-            if (OBJ == OBJ_GATE) gc.step<MATH>(P, s_trk, x);
-            if (OBJ == OBJ_CONTOUR) J += cc.step(P, s_trk, x);
+                const float mx = r2x + r3x, my = r2y + r3y, mz = r2z + r3z;
+                const float Ax = r1x + mx, Ay = r1y + my, Az = r1z + mz;
+                x.px = fmaf(kp, Ax, fmaf(P.dt, x.vx, x.px));
+                x.py = fmaf(kp, Ay, fmaf(P.dt, x.vy, x.py));
+                x.pz = fmaf(-kp, Az, fmaf(P.hh2, cz0, fmaf(P.dt, x.vz, x.pz)));
+                x.vx = fmaf(kv, (Ax + mx) + r4x, x.vx);
+                x.vy = fmaf(kv, (Ay + my) + r4y, x.vy);
+                x.vz = fmaf(-kv, (Az + mz) + r4z, fmaf(P.dt, cz0, x.vz));
+                if (OBJ == OBJ_GATE) gc.step<MATH>(P, s_trk, x);
+                if (OBJ == OBJ_CONTOUR) J += cc.step(P, s_trk, x);
+            }
+            mbar_arrive(bar_qe + s);
         }
         if (OBJ == OBJ_GATE) J = gc.finish<MATH>(P, s_trk, x);
         if (OBJ == OBJ_TRACK) pv_term(s_trk + 4 * N);
@@ -241,18 +254,19 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
     __syncthreads();
 
     // ---- the three parts of the cost meet; warp 0 owns the block's 32 samples from here on ----
-    float J = __int_as_float(0x7f800000);
+    float m = 0.0f, Zb = 0.0f;
     if (warp == 0) {
         const float jw = s_J[lane], jq = s_J[32 + lane], jp = s_J[64 + lane];
+        float J;
         if (OBJ == OBJ_GATE) J = fmaf(P.w_omega, jw, jp);          // = GateCost::finish with W's sum |omega|^2
         else if (OBJ == OBJ_TRACK) J = (jp + jq) + jw;
         else J = jp + jw;
         A.cost[(size_t)b * P.K + kbase + lane] = J;
+        m = warp_min(J);
+        const float e = exp_weight<MATH>((m - J) * P.inv_lambda);
+        Zb = warp_sum(e);
+        s_e[lane] = e;
     }
-    const float m = block_min(J, s_red);
-    const float e = warp == 0 ? exp_weight<MATH>((m - J) * P.inv_lambda) : 0.0f;
-    const float Zb = block_sum(e, s_red);
-    if (warp == 0) s_e[lane] = e;
     __syncthreads();
 
     // ---- block partial S[t][i] = sum_l e_l (T_l[t][i] - u_nom[t][i]) from the thrusts in shared memory ----
