@@ -176,9 +176,13 @@ MPPI_API int mppi_optimize(mppi_ctx* ctx, const float* d_x0, const int32_t* d_st
                   uint64_t seed, uint32_t iter0, int n_iters, float* d_cost, float* d_weights,
                   void* cuda_stream);
 
-/* Same as mppi_step with HOST buffers: copies x0, start, u_nom to the device, runs the
- * iteration, copies u_new (and cost / weights when non-NULL) back and synchronises the stream.
- * This is the end-to-end call a host-side control loop makes every cycle. */
+/* Same as mppi_step with HOST buffers; returns when the outputs are in the caller's buffers.
+ * This is the end-to-end call a host-side control loop makes every cycle.  Fused pipeline: the
+ * inputs go down as ONE packed copy from pinned staging memory, the kernel writes u_new (and cost /
+ * weights when non-NULL) into mapped host memory itself and raises a sequence number the calling
+ * thread polls -- no copy back and no stream synchronisation (a failed stream is still reported:
+ * the poll checks cudaStreamQuery every few thousand spins).  Two-pass pipeline, or no mapped
+ * memory: explicit copies both ways and cudaStreamSynchronize. */
 MPPI_API int mppi_step_host(mppi_ctx* ctx, const float* h_x0, const int32_t* h_start, const float* h_u_nom,
                    uint64_t seed, uint32_t iter, float* h_u_new, float* h_cost, float* h_weights,
                    void* cuda_stream);

@@ -238,6 +238,28 @@ class Mppi:
                                     _stream_ptr(stream)))
         return u_new, cost, weights
 
+    def step_host_fn(self, x0, start, u_nom, u_new, cost=None, weights=None, stream=None):
+        """Pre-marshalled mppi_step_host: checks the (numpy, C-contiguous) host buffers once and
+        returns f(seed, it) that only passes the stored pointers through -- for control loops that
+        call every cycle with the same buffers.  The arrays must stay alive and in place."""
+        B, N, K = self.B, self.N, self.K
+
+        def chk(a, shape, dtype):
+            if not (isinstance(a, np.ndarray) and a.dtype == dtype and a.flags["C_CONTIGUOUS"]
+                    and a.size == int(np.prod(shape))):
+                raise ValueError(f"need a C-contiguous {np.dtype(dtype).name} array with {int(np.prod(shape))} elements")
+            return C.c_void_p(a.ctypes.data)
+        px0, pst, pu = chk(x0, (B, 13), np.float32), chk(start, (B,), np.int32), chk(u_nom, (B, N, 4), np.float32)
+        pun = chk(u_new, (B, N, 4), np.float32)
+        pc = chk(cost, (B, K), np.float32) if cost is not None else None
+        pw = chk(weights, (B, K), np.float32) if weights is not None else None
+        ps = _stream_ptr(stream)
+        h, fn, ck, u64, u32 = self._h, lib.mppi_step_host, self._ck, C.c_uint64, C.c_uint32
+
+        def call(seed, it):
+            ck(fn(h, px0, pst, pu, u64(seed), u32(it), pun, pc, pw, ps))
+        return call
+
     def sim_step(self, x, start, u_new, u_nom_next=None, stream=None):
         import torch
         B, N = self.B, self.N

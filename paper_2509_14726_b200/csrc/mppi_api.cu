@@ -1,5 +1,7 @@
 // mppi_api.cu -- host side of libmppi: the C ABI declared in include/mppi.h.
 // Parameter validation, track packing, scratch allocation, stream launches and CUDA-graph replay.
+#include <atomic>
+#include <chrono>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -35,6 +37,12 @@ struct mppi_ctx {
     // device staging for mppi_step_host
     float* d_hx0 = nullptr; int* d_hstart = nullptr; float* d_hu = nullptr; float* d_hcost = nullptr;
     float* d_hw = nullptr;
+    // mapped pinned host staging of mppi_step_host: the inputs go down in ONE packed copy (reading them
+    // from host memory inside the kernel costs thousands of small bus reads -- measured slower), the
+    // kernel writes its outputs straight into host memory and raises a flag the host polls
+    unsigned char* h_pin = nullptr; unsigned char* d_pin = nullptr; unsigned char* d_in = nullptr;
+    size_t pin_x0 = 0, pin_start = 0, pin_u = 0, pin_unew = 0, pin_cost = 0, pin_w = 0, pin_flag = 0, pin_bytes = 0;
+    unsigned host_seq = 0;
     int64_t scratch_bytes = 0;
     int64_t launches = 0;
     GraphSlot g_step, g_opt;
@@ -180,6 +188,8 @@ extern "C" int mppi_destroy(mppi_ctx* c)
     free_graph(c->g_step); free_graph(c->g_opt);
     cudaFree(c->d_gates); cudaFree(c->d_ref); cudaFree(c->d_path); cudaFree(c->d_du);
     cudaFree(c->d_partials); cudaFree(c->d_counters);
+    if (c->h_pin) cudaFreeHost(c->h_pin);
+    cudaFree(c->d_in);
     cudaFree(c->d_hx0); cudaFree(c->d_hstart); cudaFree(c->d_hu); cudaFree(c->d_hcost); cudaFree(c->d_hw);
     delete c;
     return MPPI_OK;
@@ -254,8 +264,8 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     if (cfg.store_du) CKC(dev_alloc(c, &c->d_du, (size_t)p->B * p->N * p->K));
     if (cfg.fused) {
         CKC(dev_alloc(c, &c->d_partials, (size_t)p->B * d.blocks_per_ctrl * (4 * p->N + 4)));
-        CKC(dev_alloc(c, &c->d_counters, (size_t)p->B));
-        CKC(cudaMemset(c->d_counters, 0, (size_t)p->B * sizeof(unsigned)));
+        CKC(dev_alloc(c, &c->d_counters, (size_t)p->B + 1));
+        CKC(cudaMemset(c->d_counters, 0, ((size_t)p->B + 1) * sizeof(unsigned)));
     }
     CKC(dev_alloc(c, &c->d_hx0, (size_t)p->B * 13));
     CKC(dev_alloc(c, &c->d_hstart, (size_t)p->B));
@@ -263,6 +273,31 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     CKC(dev_alloc(c, &c->d_hcost, BK));
     CKC(dev_alloc(c, &c->d_hw, BK));
 #undef CKC
+    if (cfg.fused) {
+        // layout of the mapped staging block, every part 256-byte aligned
+        auto up = [](size_t v) { return (v + 255) & ~(size_t)255; };
+        size_t o = 0;
+        c->pin_x0 = o; o = up(o + (size_t)p->B * 13 * sizeof(float));
+        c->pin_start = o; o = up(o + (size_t)p->B * sizeof(int32_t));
+        c->pin_u = o; o = up(o + BN4 * sizeof(float));
+        c->pin_unew = o; o = up(o + BN4 * sizeof(float));
+        c->pin_cost = o; o = up(o + BK * sizeof(float));
+        c->pin_w = o; o = up(o + BK * sizeof(float));
+        c->pin_flag = o; o = up(o + sizeof(unsigned));
+        c->pin_bytes = o;
+        void* hp = nullptr; void* dp = nullptr;
+        if (cudaHostAlloc(&hp, o, cudaHostAllocMapped) == cudaSuccess &&
+            cudaHostGetDevicePointer(&dp, hp, 0) == cudaSuccess) {
+            c->h_pin = (unsigned char*)hp; c->d_pin = (unsigned char*)dp;
+            std::memset(hp, 0, o);
+            if (dev_alloc(c, &c->d_in, c->pin_unew) != cudaSuccess) {
+                cudaGetLastError(); cudaFreeHost(hp); c->h_pin = nullptr; c->d_in = nullptr;
+            }
+        } else {
+            if (hp) cudaFreeHost(hp);
+            cudaGetLastError();          // mapping unavailable: mppi_step_host uses explicit copies
+        }
+    }
     *out = c;
     return MPPI_OK;
 }
@@ -402,6 +437,7 @@ static StepArgs make_args(mppi_ctx* c, const float* x0, const int32_t* start, co
     StepArgs a;
     a.x0 = x0; a.start = start; a.u_nom = u_nom; a.u_new = u_new; a.cost = cost; a.weights = w;
     a.du = c->d_du; a.partials = c->d_partials; a.counters = c->d_counters;
+    a.done_flag = nullptr; a.done_value = 0;
     a.seed_lo = (uint32_t)(seed & 0xffffffffu); a.seed_hi = (uint32_t)(seed >> 32); a.iter = iter;
     for (uint32_t r = 0; r < 10; ++r) {          // Philox key schedule (Weyl sequence), hoisted out of the kernel
         a.rk[2 * r] = a.seed_lo + r * 0x9E3779B9u;
@@ -522,6 +558,46 @@ extern "C" int mppi_step_host(mppi_ctx* c, const float* h_x0, const int32_t* h_s
     if (!h_x0 || !h_start || !h_u_nom || !h_u_new) return fail(c, MPPI_E_NULL, "mppi_step_host: NULL host pointer");
     cudaStream_t s = (cudaStream_t)stream;
     const size_t B = c->prm.B, N = c->prm.N, K = c->prm.K;
+    if (c->h_pin) {
+        // inputs: packed in pinned memory, one copy down.  outputs: u_new (and cost / weights when asked
+        // for) are written into mapped host memory by the kernel itself, whose last block raises a
+        // sequence number this thread polls -- no copy back, no stream synchronisation
+        int rc = prepare(c);
+        if (rc) return rc;
+        unsigned char* hp = c->h_pin; unsigned char* dp = c->d_pin;
+        std::memcpy(hp + c->pin_x0, h_x0, B * 13 * sizeof(float));
+        std::memcpy(hp + c->pin_start, h_start, B * sizeof(int32_t));
+        std::memcpy(hp + c->pin_u, h_u_nom, B * N * 4 * sizeof(float));
+        CK(c, cudaMemcpyAsync(c->d_in, hp, c->pin_u + B * N * 4 * sizeof(float), cudaMemcpyHostToDevice, s));
+        const unsigned char* di = c->d_in;
+        StepArgs a = make_args(c, (const float*)(di + c->pin_x0), (const int32_t*)(di + c->pin_start),
+                               (const float*)(di + c->pin_u), seed, iter, (float*)(dp + c->pin_unew),
+                               h_cost ? (float*)(dp + c->pin_cost) : c->d_hcost,
+                               h_weights ? (float*)(dp + c->pin_w) : c->d_hw);
+        volatile unsigned* flag = (volatile unsigned*)(hp + c->pin_flag);
+        const unsigned seq = ++c->host_seq ? c->host_seq : ++c->host_seq;     // never 0
+        a.done_flag = (unsigned*)(dp + c->pin_flag); a.done_value = seq;
+        rc = enqueue_iteration(c, a, s);
+        if (rc) return rc;
+        const auto t0 = std::chrono::steady_clock::now();
+        unsigned spins = 0;
+        while (*flag != seq) {
+            if ((++spins & 0x3fff) == 0) {
+                // every so often: has the stream failed, or is this taking implausibly long?
+                const cudaError_t q = cudaStreamQuery(s);
+                if (q != cudaSuccess && q != cudaErrorNotReady) return cuda_fail(c, q, "mppi_step_host: kernel");
+                if (std::chrono::steady_clock::now() - t0 > std::chrono::seconds(10)) {
+                    CK(c, cudaStreamSynchronize(s));
+                    if (*flag != seq) return fail(c, MPPI_E_CUDA, "mppi_step_host: completion flag never arrived");
+                }
+            }
+        }
+        std::atomic_thread_fence(std::memory_order_acquire);
+        std::memcpy(h_u_new, hp + c->pin_unew, B * N * 4 * sizeof(float));
+        if (h_cost) std::memcpy(h_cost, hp + c->pin_cost, B * K * sizeof(float));
+        if (h_weights) std::memcpy(h_weights, hp + c->pin_w, B * K * sizeof(float));
+        return MPPI_OK;
+    }
     CK(c, cudaMemcpyAsync(c->d_hx0, h_x0, B * 13 * sizeof(float), cudaMemcpyHostToDevice, s));
     CK(c, cudaMemcpyAsync(c->d_hstart, h_start, B * sizeof(int32_t), cudaMemcpyHostToDevice, s));
     CK(c, cudaMemcpyAsync(c->d_hu, h_u_nom, B * N * 4 * sizeof(float), cudaMemcpyHostToDevice, s));

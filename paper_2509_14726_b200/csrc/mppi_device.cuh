@@ -37,7 +37,9 @@ struct StepArgs {
     float* weights;        // [B][K]
     float4* du;            // [B][N][K] float4 or nullptr
     float* partials;       // [B][blocks_per_ctrl][4N+4]  (fused pipeline)
-    unsigned int* counters;// [B]                         (fused pipeline)
+    unsigned int* counters;// [B + 1]: last-block tickets per controller, finished controllers (fused pipeline)
+    unsigned int* done_flag;   // mapped host word, or nullptr: set to done_value once every output of the
+    unsigned int done_value;   // call is visible to the host (mppi_step_host polls it instead of a stream sync)
     uint32_t seed_lo, seed_hi, iter;
     uint32_t rk[20];       // Philox round keys: rk[2r] = seed_lo + r W0, rk[2r+1] = seed_hi + r W1
 };

@@ -242,6 +242,21 @@ __device__ __forceinline__ void publish_and_combine(const DevParams& P, const St
                             exp_weight<MATH>((c.z - beta) * nil) * invZ, exp_weight<MATH>((c.w - beta) * nil) * invZ);
     }
     if (tid == 0) A.counters[b] = 0u;          // ready for the next launch
+    if (A.done_flag) {
+        // host-polled completion: every output store of this block is made visible system-wide, then
+        // the block that finishes the last controller raises the flag in mapped host memory
+        __threadfence_system();
+        __syncthreads();
+        if (tid == 0) {
+            bool all = true;
+            if (P.B > 1) {
+                all = atomicAdd(&A.counters[P.B], 1u) == (unsigned)(P.B - 1);
+                if (all) A.counters[P.B] = 0u;
+                __threadfence_system();
+            }
+            if (all) *reinterpret_cast<volatile unsigned*>(A.done_flag) = A.done_value;
+        }
+    }
 }
 
 }  // namespace mppi

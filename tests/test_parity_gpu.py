@@ -289,7 +289,14 @@ def test_determinism_and_host_entry_point():
         un, co, we = m.step_host(wl.x0, wl.start, wl.u_nom, 9, 1)
         np.testing.assert_array_equal(un, a["u_new"]); np.testing.assert_array_equal(co, a["cost"])
         np.testing.assert_array_equal(we, a["weights"])
-        assert m.launch_count() == (5 if opts["pipeline"] == 0 else 10)
+        # the pre-marshalled form of the same call, with and without the optional outputs
+        un2, co2 = np.empty_like(un), np.empty_like(co)
+        m.step_host_fn(wl.x0, wl.start, wl.u_nom, un2, cost=co2)(9, 1)
+        np.testing.assert_array_equal(un2, un); np.testing.assert_array_equal(co2, co)
+        un3 = np.empty_like(un)
+        m.step_host_fn(wl.x0, wl.start, wl.u_nom, un3)(9, 1)
+        np.testing.assert_array_equal(un3, un)
+        assert m.launch_count() == (7 if opts["pipeline"] == 0 else 14)
         m.close()
 
 
