@@ -308,6 +308,22 @@ def run_ours(args):
             m4.step(x4, s4, u4, 0, j[0], u_new=un4, cost=c4, weights=w4); j[0] += 1
         ms4 = time_steps(step4, flush, 30, 5)
         units4 = P4["K"] * P4["N"] * P4["B"]
+
+        # configs[4] as stated: the closed loop -- MPPI iteration, plant step, gate advance and shift of
+        # the nominal every control step, 500 steps, per-step latency by CUDA events (no L2 flush: the
+        # loop's own working set is what a controller sees)
+        n_loop = wl4.iters
+        x4.copy_(torch.from_numpy(wl4.x0).to(dev)); s4.copy_(torch.from_numpy(wl4.start).to(dev))
+        u4.copy_(torch.from_numpy(wl4.u_nom).to(dev))
+        ev = _events(n_loop + 1)
+        ev[0].record()
+        for i in range(n_loop):
+            m4.step(x4, s4, u4, wl4.seed, i, u_new=un4, cost=c4, weights=w4)
+            m4.sim_step(x4, s4, un4, u_nom_next=u4)
+            ev[i + 1].record()
+        torch.cuda.synchronize()
+        loop_ms = np.array([ev[i].elapsed_time(ev[i + 1]) for i in range(n_loop)])[5:]
+        gates_passed = int(s4.max().item())
         flops = FLOPS_PER_SAMPLE_STEP[0]
         sm = info["sm_count"]
         peak_tf = sm * FP32_LANES_PER_SM * 2 * (clocks["sm_max_mhz"] or clock_attr_mhz) * 1e6 / 1e12
@@ -327,6 +343,7 @@ def run_ours(args):
                        "l2": "flushed between timed iterations (256 MiB write outside the events)",
                        "pipeline": "fused" if args.pipeline == 0 else "two_pass", "fast_math": args.fast_math,
                        "cuda_graph": bool(args.graph), "block_threads": info["block_threads"],
+                       "kernel": "rollout_pipe_kernel" if info["rollout_warps_per_block"] == 3 and info["block_threads"] == 256 else "rollout",
                        "grid_blocks": info["grid_blocks"], "replicas": world},
             "clocks": clocks,
             "latency_us": {"p50": float(np.median(ms) * 1e3), "p99": float(np.percentile(ms, 99) * 1e3),
@@ -337,7 +354,7 @@ def run_ours(args):
                     "timer": "host perf_counter around mppi_step_host: one packed H2D copy from pinned memory, the kernel, u_new written by the kernel into mapped host memory, completion flag polled by the host"},
             "gpu_launches": int(launches),
             "roofline": {"bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
-                         "traffic": None, "kernel": "rollout_kernel<gate>" + (" (fused update)" if args.pipeline == 0 else ""),
+                         "traffic": None, "kernel": "the iteration's single kernel (pipelined rollout + cost + fused softmax update)" if args.pipeline == 0 else "rollout kernel of the two-pass pipeline",
                          "flops_per_sample_step": flops, "units_per_launch": units,
                          "peak_how": f"{sm} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 x clocks.max.sm (B200_PROFILING.md)",
                          "peak_measured_ffma_tflops": fma_tflops, "frac_of_measured_ffma": ach / fma_tflops,
@@ -346,7 +363,12 @@ def run_ours(args):
             "batched": {"workload": wl4.name, "K": P4["K"], "N": P4["N"], "B": P4["B"],
                         "value": units4 / (float(ms4.mean()) * 1e-3), "unit": UNIT, "ms_per_step": float(ms4.mean()),
                         "roofline": {"bound": "alu", "achieved": ach4, "peak": peak_tf, "unit": "TFLOP/s",
-                                     "frac": ach4 / peak_tf, "frac_of_measured_ffma": ach4 / fma_tflops}},
+                                     "frac": ach4 / peak_tf, "frac_of_measured_ffma": ach4 / fma_tflops},
+                        "closed_loop": {"control_steps": n_loop, "value": units4 / (float(loop_ms.mean()) * 1e-3),
+                                        "unit": UNIT, "latency_us_p50": float(np.median(loop_ms) * 1e3),
+                                        "latency_us_p99": float(np.percentile(loop_ms, 99) * 1e3),
+                                        "max_gate_index_reached": gates_passed,
+                                        "what": "mppi_step + mppi_sim_step per control step, 64 drones, CUDA events"}},
             "cpu_baseline": {"value": cpu_rate, "unit": UNIT, "cores": cpu_threads, "kind": "oracle",
                              "sample": f"{cpu_n} full iterations of {wl.name} ({cpu_s_iter * 1e3:.1f} ms each), float64, OpenMP over samples"},
         }
