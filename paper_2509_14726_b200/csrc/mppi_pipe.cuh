@@ -49,6 +49,20 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
         "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
 
+// two barriers at once: both phase checks are in flight together (a satisfied check costs ~100 cycles)
+__device__ __forceinline__ void mbar_wait2(uint64_t* bar_a, uint32_t par_a, uint64_t* bar_b, uint32_t par_b)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred pa, pb;\n"
+        "WAIT2_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 pa, [%0], %1;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 pb, [%2], %3;\n"
+        "and.pred pa, pa, pb;\n"
+        "@!pa bra WAIT2_%=;\n"
+        "}\n" ::"r"(smem_u32(bar_a)), "r"(par_a), "r"(smem_u32(bar_b)), "r"(par_b) : "memory");
+}
+
 // float4 units of dynamic shared memory after the nominal + track + 16 float4 of reduction scratch
 __host__ __device__ inline size_t pipe_extra_f4(int N, int nb)
 {
@@ -117,8 +131,8 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
         float acc = 0.0f;      // gate: sum |omega_{t+1}|^2; contour / track: this warp's cost terms
         for (int c = 0; c < nchunks; ++c) {
             const int s = c & (D - 1), cnt = min(C, N - c * C);
-            mbar_wait(bar_T + c, 0);                           // the chunk's thrusts are drawn
-            mbar_wait(bar_we + s, ((c / D) & 1) ^ 1);          // Q has drained this slot
+            // the chunk's thrusts are drawn; Q has drained this slot
+            mbar_wait2(bar_T + c, 0, bar_we + s, ((c / D) & 1) ^ 1);
             for (int j = 0; j < cnt; ++j) {
                 const int t = c * C + j;
                 const float4 T = s_T[t * RS + lane];
@@ -172,8 +186,8 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
         };
         for (int c = 0; c < nchunks; ++c) {
             const int s = c & (D - 1), cnt = min(C, N - c * C);
-            mbar_wait(bar_wf + s, (c / D) & 1);                // W has filled this slot
-            mbar_wait(bar_qe + s, ((c / D) & 1) ^ 1);          // P has drained the slot written below
+            // W has filled this slot; P has drained the slot written below
+            mbar_wait2(bar_wf + s, (c / D) & 1, bar_qe + s, ((c / D) & 1) ^ 1);
             for (int j = 0; j < cnt; ++j) {
                 if (OBJ == OBJ_TRACK) quat_term(s_trk + 4 * (c * C + j));
                 const float4* w = s_w + (s * C + j) * 96 + lane;
@@ -195,7 +209,8 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
                 o[96] = make_float4(q4w, q4x, q4y, q4z);
                 MPPI_G(q4w, q4x, q4y, q4z, f2.y, f2.z, f2.w, gw, gx, gy, gz)
                 nw = fmaf(P.h12, gw, nw); nx = fmaf(P.h12, gx, nx); ny = fmaf(P.h12, gy, ny); nz = fmaf(P.h12, gz, nz);
-                const float inv = rsqrtf(fmaf(nz, nz, fmaf(ny, ny, fmaf(nx, nx, nw * nw))));
+                // |n|^2 is within rounding of 1: the plain MUFU.RSQ (no denormal fix-up) returns rsqrtf's value
+                const float inv = mufu_rsq(fmaf(nz, nz, fmaf(ny, ny, fmaf(nx, nx, nw * nw))));
                 qw = nw * inv; qx = nx * inv; qy = ny * inv; qz = nz * inv;
             }
             mbar_arrive(bar_we + s);
