@@ -36,6 +36,7 @@ UNIT = "sample-steps/s"
 FLOPS_PER_SAMPLE_STEP = {0: 417.0, 1: 449.0, 2: 685.0}
 FP32_LANES_PER_SM = 128
 L2_FLUSH_BYTES = 256 << 20
+NCU_DRAM_BYTES_PER_LAUNCH = 56320     # rollout_pipe_kernel<gate>, cfg1: 56.3 KB read + 0 B written (profiles/README_r01b.md)
 
 
 def dist_env():
@@ -332,7 +333,7 @@ def run_ours(args):
 
         # ---- cpu_baseline: the oracle on this host's cores, bounded sample
         from oracle import oracle as O   # noqa: F401  (cpu_baseline leg only)
-        cpu_rate, cpu_s_iter, cpu_n, cpu_threads = time_oracle(wl, args.cpu_budget, 400)
+        cpu_rate, cpu_s_iter, cpu_n, cpu_threads = time_oracle(wl, args.cpu_budget, 5000)
 
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -354,7 +355,9 @@ def run_ours(args):
                     "timer": "host perf_counter around mppi_step_host: one packed H2D copy from pinned memory, the kernel, u_new written by the kernel into mapped host memory, completion flag polled by the host"},
             "gpu_launches": int(launches),
             "roofline": {"bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
-                         "traffic": None, "kernel": "the iteration's single kernel (pipelined rollout + cost + fused softmax update)" if args.pipeline == 0 else "rollout kernel of the two-pass pipeline",
+                         # dram__bytes_read.sum + dram__bytes_write.sum of this kernel, per launch, from the
+                         # ncu --set full capture summarised in profiles/README_r01b.md (not measured live)
+                         "traffic": NCU_DRAM_BYTES_PER_LAUNCH if args.pipeline == 0 else None, "kernel": "the iteration's single kernel (pipelined rollout + cost + fused softmax update)" if args.pipeline == 0 else "rollout kernel of the two-pass pipeline",
                          "flops_per_sample_step": flops, "units_per_launch": units,
                          "peak_how": f"{sm} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 x clocks.max.sm (B200_PROFILING.md)",
                          "peak_measured_ffma_tflops": fma_tflops, "frac_of_measured_ffma": ach / fma_tflops,
