@@ -34,6 +34,7 @@
 #define ORC_OBJ_GATE 0
 #define ORC_OBJ_TRACK 1
 #define ORC_OBJ_CONTOUR 2
+#define ORC_OBJ_GATE_PAPER 3   /* the paper's own J_gate, eq.(6),(7) + temporal check */
 
 typedef struct {
     int32_t K, N, B, objective;
@@ -46,6 +47,7 @@ typedef struct {
     double q_contour, q_lag, mu_progress;
     int32_t window;
     int32_t pad_;
+    double q_near, r_near;   /* eq.(7): weight and threshold radius [R-24] */
 } orc_params;
 
 typedef struct {
@@ -57,6 +59,8 @@ typedef struct {
                             unit in-plane axis h(3), half-width along h, half-height along v=h x n */
     const double* ref;   /* [M][13]: p(3), q wxyz(4), v(3), omega(3) */
     const double* pts;   /* [P][3]  */
+    const int32_t* prev_front; /* [B][N+1] or NULL: ORC_OBJ_GATE_PAPER, state k of the previous control
+                            iteration was in front of the start gate (Fig. 2) [R-25] */
 } orc_track;
 
 /* ------------------------------------------------------------------------------------------
@@ -236,6 +240,91 @@ double orc_gate_step(const orc_params* P, const orc_track* trk, const double p_p
  * Q_K = Q; quaternion error |q - s q_ref|^2, s = sign(q . q_ref) (double cover);
  * R on (T - hover) per BASELINE.json configs[2].
  * ---------------------------------------------------------------------------------------- */
+/* ------------------------------------------------------------------------------------------
+ * The paper's own gate-progress objective, one step (eq.(6),(7) PAPER.md:105-129), readings
+ * [R-23]..[R-25] of DESIGN.md:
+ *   progress   |p_{t+1} - c|^2 - |p_t - c|^2, squared distances, against the gate targeted at the
+ *              start of the step                                                 (eq.(6))
+ *   near term  + Q_near |p_t - c|^2 when |p_t - c| < r_near (pre-step state p_k)  (eq.(7))
+ *   switching  a front->back crossing of the target plane inside the opening is REGISTERED (bonus,
+ *              target <- next gate from the next step on) only if the target is not the horizon's
+ *              start gate, or the corresponding state of the previous control iteration was in
+ *              front of the gate: front_ok != 0 (Fig. 2).  An unregistered pass
+ *              changes nothing; a crossing outside the opening adds the miss penalty, as in
+ *              orc_gate_step.
+ *   body rates + w_omega |omega_{t+1}|^2
+ * margin additionally tracks | |p_t - c| - r_near | (the near term is discontinuous there).
+ * ---------------------------------------------------------------------------------------- */
+double orc_gate_paper_step(const orc_params* P, const orc_track* trk, const double p_prev[3],
+                           const double p[3], const double omega[3], int32_t* gate, int32_t gate0,
+                           int32_t front_ok, double* margin, int32_t* ncross)
+{
+    const double* gt = trk->gates + 11 * (*gate);
+    const double* c = gt; const double* n = gt + 3; const double* h = gt + 6;
+    const double a_h = gt[9], a_v = gt[10];
+    const double v[3] = { h[1] * n[2] - h[2] * n[1], h[2] * n[0] - h[0] * n[2],
+                          h[0] * n[1] - h[1] * n[0] };           /* v = h x n */
+    double r_prev[3], r[3];
+    for (int i = 0; i < 3; ++i) { r_prev[i] = p_prev[i] - c[i]; r[i] = p[i] - c[i]; }
+    const double d2_prev = dot3(r_prev, r_prev), d2 = dot3(r, r);
+
+    double J = d2 - d2_prev;                                     /* eq.(6) */
+    const double d_prev = sqrt(d2_prev);
+    if (d_prev < P->r_near) J += P->q_near * d2_prev;            /* eq.(7) */
+    if (margin && fabs(d_prev - P->r_near) < *margin) *margin = fabs(d_prev - P->r_near);
+
+    const double s_prev = dot3(n, r_prev), s = dot3(n, r);
+    if (margin) {
+        if (fabs(s_prev) < *margin) *margin = fabs(s_prev);
+        if (fabs(s) < *margin) *margin = fabs(s);
+    }
+    if (s_prev < 0.0 && s >= 0.0) {
+        const double alpha = s_prev / (s_prev - s);
+        double rx[3];
+        for (int i = 0; i < 3; ++i) rx[i] = r_prev[i] + alpha * (r[i] - r_prev[i]);
+        const double y = dot3(h, rx), z = dot3(v, rx);
+        if (margin) {
+            if (fabs(fabs(y) - a_h) < *margin) *margin = fabs(fabs(y) - a_h);
+            if (fabs(fabs(z) - a_v) < *margin) *margin = fabs(fabs(z) - a_v);
+        }
+        if (fabs(y) <= a_h && fabs(z) <= a_v) {
+            if (*gate != gate0 || front_ok) {                    /* temporally consistent pass */
+                J -= P->gate_pass_bonus;
+                *gate = (*gate + 1) % trk->G;
+                if (ncross) *ncross += 1;
+            }
+        } else {
+            J += P->gate_miss_penalty;
+        }
+    }
+    J += P->w_omega * dot3(omega, omega);
+    return J;
+}
+
+/* "In front of the gate" flags of a nominal rollout [R-26]: front[k] = 1 iff n.(p_k - c) < 0 for the
+ * start gate, k = 0..N, states of the noise-free rollout of u (clamped) from x0.  margin (may be
+ * NULL) receives min_k |n.(p_k - c)|. */
+void orc_front_flags(const orc_params* P, const orc_track* trk, const double x0[13], int32_t start,
+                     const double* u /*[N][4]*/, int32_t* front /*[N+1]*/, double* margin)
+{
+    int32_t g = start % trk->G; if (g < 0) g += trk->G;
+    const double* c = trk->gates + 11 * g; const double* n = c + 3;
+    double x[13], xn[13], mg = INFINITY;
+    memcpy(x, x0, sizeof x);
+    for (int k = 0; k <= P->N; ++k) {
+        const double r[3] = { x[0] - c[0], x[1] - c[1], x[2] - c[2] };
+        const double s = dot3(n, r);
+        front[k] = s < 0.0 ? 1 : 0;
+        if (fabs(s) < mg) mg = fabs(s);
+        if (k == P->N) break;
+        double T[4];
+        for (int i = 0; i < 4; ++i) T[i] = fmin(fmax(u[4 * k + i], P->T_min), P->T_max);
+        orc_rk4_step(P, x, T, P->dt, xn);
+        memcpy(x, xn, sizeof x);
+    }
+    if (margin) *margin = mg;
+}
+
 double orc_track_state_term(const orc_params* P, const double x[13], const double xr[13])
 {
     double ep = 0, eq = 0, ev = 0, ew = 0;
@@ -359,6 +448,8 @@ double orc_rollout_cost(const orc_params* P, const orc_track* trk, const orc_pat
     double x[13];
     memcpy(x, x0, sizeof x);
     int32_t aux = start;
+    if (P->objective == ORC_OBJ_GATE_PAPER) { aux = start % trk->G; if (aux < 0) aux += trk->G; }
+    const int32_t gate0 = aux;
     double J = 0.0, theta_prev = 0.0;
     double marg = INFINITY; int32_t nc = 0;
 
@@ -387,7 +478,10 @@ double orc_rollout_cost(const orc_params* P, const orc_track* trk, const orc_pat
 
         if (P->objective == ORC_OBJ_GATE)
             J += orc_gate_step(P, trk, x, xn, xn + 10, &aux, &marg, &nc);
-        else if (P->objective == ORC_OBJ_CONTOUR)
+        else if (P->objective == ORC_OBJ_GATE_PAPER) {
+            const int32_t front_ok = trk->prev_front ? trk->prev_front[(size_t)b * (P->N + 1) + t + 1] : 1;
+            J += orc_gate_paper_step(P, trk, x, xn, xn + 10, &aux, gate0, front_ok, &marg, &nc);
+        } else if (P->objective == ORC_OBJ_CONTOUR)
             J += orc_contour_step(P, trk, pa->s, pa->tan, pa->L, xn, xn + 10, &aux, &theta_prev);
         memcpy(x, xn, sizeof x);
     }
@@ -489,7 +583,7 @@ int orc_sim_step(const orc_params* P, const orc_track* trk, double* x, int32_t* 
         const double* ub = u_new + (size_t)b * N * 4;
         double xn[13];
         orc_rk4_step(P, xb, ub, P->dt, xn);
-        if (P->objective == ORC_OBJ_GATE) {
+        if (P->objective == ORC_OBJ_GATE || P->objective == ORC_OBJ_GATE_PAPER) {
             int32_t gate = start[b];
             (void)orc_gate_step(P, trk, xb, xn, xn + 10, &gate, NULL, NULL);
             start[b] = gate;

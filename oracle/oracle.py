@@ -18,7 +18,7 @@ _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "mppi_oracle.c"
 _LIB = _HERE / "libmppi_oracle.so"
 
-OBJ_GATE, OBJ_TRACK, OBJ_CONTOUR = 0, 1, 2
+OBJ_GATE, OBJ_TRACK, OBJ_CONTOUR, OBJ_GATE_PAPER = 0, 1, 2, 3
 
 
 def build(force: bool = False) -> Path:
@@ -41,13 +41,14 @@ class _Params(C.Structure):
                 ("gate_miss_penalty", C.c_double), ("gate_pass_bonus", C.c_double),
                 ("Qp", C.c_double), ("Qv", C.c_double), ("Qq", C.c_double), ("Qw", C.c_double),
                 ("R", C.c_double), ("q_contour", C.c_double), ("q_lag", C.c_double),
-                ("mu_progress", C.c_double), ("window", C.c_int32), ("pad_", C.c_int32)]
+                ("mu_progress", C.c_double), ("window", C.c_int32), ("pad_", C.c_int32),
+                ("q_near", C.c_double), ("r_near", C.c_double)]
 
 
 class _Track(C.Structure):
     _fields_ = [("G", C.c_int32), ("M", C.c_int32), ("P", C.c_int32), ("closed", C.c_int32),
                 ("gates", C.POINTER(C.c_double)), ("ref", C.POINTER(C.c_double)),
-                ("pts", C.POINTER(C.c_double))]
+                ("pts", C.POINTER(C.c_double)), ("prev_front", C.POINTER(C.c_int32))]
 
 
 _PARAM_KEYS = [f for f, _ in _Params._fields_ if f not in ("pad_",)]
@@ -76,6 +77,11 @@ def lib():
         L.orc_gate_step.argtypes = [C.POINTER(_Params), C.POINTER(_Track), _dp, _dp, _dp, _ip, _dp,
                                     _ip]
         L.orc_gate_step.restype = C.c_double
+        L.orc_gate_paper_step.argtypes = [C.POINTER(_Params), C.POINTER(_Track), _dp, _dp, _dp, _ip,
+                                          C.c_int32, C.c_int32, _dp, _ip]
+        L.orc_gate_paper_step.restype = C.c_double
+        L.orc_front_flags.argtypes = [C.POINTER(_Params), C.POINTER(_Track), _dp, C.c_int32, _dp, _ip, _dp]
+        L.orc_front_flags.restype = None
         L.orc_track_state_term.argtypes = [C.POINTER(_Params), _dp, _dp]
         L.orc_track_state_term.restype = C.c_double
         L.orc_track_stage.argtypes = [C.POINTER(_Params), _dp, _dp, _dp]
@@ -123,6 +129,9 @@ def make_params(p: dict) -> _Params:
         src["lambda_"] = src.pop("lambda")
     for k in _PARAM_KEYS:
         if k not in src:
+            if k in ("q_near", "r_near"):           # only the paper's J_gate (objective 3) uses them
+                src[k] = 0.0
+                continue
             raise KeyError(f"oracle params: missing '{k}'")
         v = src[k]
         setattr(s, k, int(v) if k in ("K", "N", "B", "objective", "window") else float(v))
@@ -132,7 +141,7 @@ def make_params(p: dict) -> _Params:
 class Track:
     """Holds float64 copies of the track arrays and the C view of them."""
 
-    def __init__(self, gates=None, ref=None, path=None, closed=True):
+    def __init__(self, gates=None, ref=None, path=None, closed=True, prev_front=None):
         self.gates = _f64(gates, (-1, 11)) if gates is not None else None
         self.ref = _f64(ref, (-1, 13)) if ref is not None else None
         self.path = _f64(path, (-1, 3)) if path is not None else None
@@ -145,6 +154,9 @@ class Track:
         self.c.gates = _d(self.gates) if self.gates is not None else null
         self.c.ref = _d(self.ref) if self.ref is not None else null
         self.c.pts = _d(self.path) if self.path is not None else null
+        self.prev_front = (np.ascontiguousarray(np.asarray(prev_front, dtype=np.int32))
+                           if prev_front is not None else None)
+        self.c.prev_front = _i(self.prev_front) if self.prev_front is not None else C.cast(None, _ip)
 
 
 # ---- thin wrappers -----------------------------------------------------------------------
@@ -188,6 +200,24 @@ def gate_step(params, track: Track, p_prev, p, omega, gate):
     J = lib().orc_gate_step(C.byref(P), C.byref(track.c), _d(_f64(p_prev, (3,))), _d(_f64(p, (3,))),
                             _d(_f64(omega, (3,))), C.byref(g), C.byref(m), C.byref(n))
     return J, g.value, m.value, n.value
+
+
+def gate_paper_step(params, track: Track, p_prev, p, omega, gate, gate0, front_ok):
+    """The paper's J_gate, one step -> (step cost, new gate index, margin, registered passes)."""
+    P = make_params(params)
+    g = C.c_int32(int(gate)); m = C.c_double(np.inf); n = C.c_int32(0)
+    J = lib().orc_gate_paper_step(C.byref(P), C.byref(track.c), _d(_f64(p_prev, (3,))), _d(_f64(p, (3,))),
+                                  _d(_f64(omega, (3,))), C.byref(g), int(gate0), int(front_ok),
+                                  C.byref(m), C.byref(n))
+    return J, g.value, m.value, n.value
+
+
+def front_flags(params, track: Track, x0, start, u):
+    """[R-26] -> (front[N+1] int32, margin) of the noise-free rollout of u from x0."""
+    P = make_params(params)
+    u = _f64(u, (P.N, 4)); f = np.zeros(P.N + 1, np.int32); m = C.c_double(np.inf)
+    lib().orc_front_flags(C.byref(P), C.byref(track.c), _d(_f64(x0, (13,))), int(start), _d(u), _i(f), C.byref(m))
+    return f, m.value
 
 
 def track_state_term(params, x, xr):

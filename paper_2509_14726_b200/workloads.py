@@ -16,7 +16,7 @@ from dataclasses import dataclass, field
 
 import numpy as np
 
-OBJ_GATE, OBJ_TRACK, OBJ_CONTOUR = 0, 1, 2
+OBJ_GATE, OBJ_TRACK, OBJ_CONTOUR, OBJ_GATE_PAPER = 0, 1, 2, 3
 
 
 def _f32(v):
@@ -29,7 +29,7 @@ def base_params(**over) -> dict:
              dt=0.02, sigma=1.0, mass=0.85, Jx=1e-3, Jy=1e-3, Jz=1.7e-3, arm=0.15, c_tau=0.016,
              g=9.81, T_min=0.0, T_max=7.0, w_omega=0.01, gate_miss_penalty=10.0,
              gate_pass_bonus=5.0, Qp=100.0, Qv=1.0, Qq=10.0, Qw=0.1, R=0.01, q_contour=200.0,
-             q_lag=50.0, mu_progress=2.0, window=16)
+             q_lag=50.0, mu_progress=2.0, window=16, q_near=0.0, r_near=0.0)
     p["lambda"] = 1.0
     p.update(over)
     for k, v in p.items():
@@ -53,6 +53,7 @@ class Workload:
     gates: np.ndarray | None = None     # [G,11] f32
     ref: np.ndarray | None = None       # [M,13] f32
     path: np.ndarray | None = None      # [P,3] f32
+    prev_front: np.ndarray | None = None  # [B,N+1] i32, objective 3 only (None = all in front)
     closed: bool = True
     seed: int = 0
     iters: int = 1                      # optimiser iterations (cfg1) or control steps (cfg4)
@@ -234,5 +235,26 @@ def stress_gate(K=1024, N=30) -> Workload:
                     np.zeros(1, np.int32), _hover_nominal(p, 1, N), gates=gates, seed=3, iters=1)
 
 
-ALL = {"cfg0": cfg0, "cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg4": cfg4,
+def gate_paper(K=4096, N=50) -> Workload:
+    """The paper's own J_gate (eq.(6),(7) + temporal check) on the
+    configs[1] track: squared-distance progress, Q_near = 2 inside r_near = 1.5 m (the paper gives
+    neither value), no pass bonus / miss penalty, all states of the previous iteration in front."""
+    wl = cfg1(K=K, N=N, iters=1)
+    p = dict(wl.params, objective=OBJ_GATE_PAPER, gate_pass_bonus=0.0, gate_miss_penalty=0.0,
+             q_near=_f32(2.0), r_near=_f32(1.5))
+    return Workload(f"gate_paper_K{K}_N{N}", p, wl.x0, wl.start, wl.u_nom, gates=wl.gates, seed=wl.seed)
+
+
+def stress_gate_paper(K=1024, N=30, flag_seed=5) -> Workload:
+    """stress_gate under the paper's J_gate with random previous-iteration flags, so that registered and
+    unregistered passes, misses and the near term all occur at scale."""
+    wl = stress_gate(K=K, N=N)
+    p = dict(wl.params, objective=OBJ_GATE_PAPER, q_near=_f32(2.0), r_near=_f32(1.5))
+    rng = np.random.default_rng(flag_seed)
+    front = (rng.uniform(size=(1, N + 1)) < 0.6).astype(np.int32)
+    return Workload("stress_gate_paper", p, wl.x0, wl.start, wl.u_nom, gates=wl.gates, seed=wl.seed,
+                    prev_front=front)
+
+
+ALL = {"gate_paper": gate_paper, "stress_gate_paper": stress_gate_paper, "cfg0": cfg0, "cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg4": cfg4,
        "stress_gate": stress_gate}

@@ -126,6 +126,28 @@ def rollout_cost(P, trk, x0, start, u_nom, seed, it, k, b):
                     J -= P["gate_pass_bonus"]; aux = (aux + 1) % len(gates)
                 else:
                     J += P["gate_miss_penalty"]
+    elif P["objective"] == 3:
+        # the paper's own J_gate: eq.(6),(7) PAPER.md:105-129 + the temporal check of Fig. 2
+        gates = trk["gates"]
+        front = trk.get("prev_front")
+        aux = start % len(gates)
+        g0 = aux
+        for t in range(N):
+            g = gates[aux]
+            c, n, h, aw, ah = g[0:3], g[3:6], g[6:9], g[9], g[10]
+            a, bpt = xs[t][0:3], xs[t + 1][0:3]
+            J += np.sum((bpt - c) ** 2) - np.sum((a - c) ** 2)
+            if np.linalg.norm(a - c) < P["r_near"]:
+                J += P["q_near"] * np.sum((a - c) ** 2)
+            J += P["w_omega"] * np.sum(xs[t + 1][10:13] ** 2)
+            sa, sb = n @ (a - c), n @ (bpt - c)
+            if sa < 0 <= sb:
+                hit = a + (bpt - a) * (sa / (sa - sb)) - c
+                if abs(h @ hit) <= aw and abs(np.cross(h, n) @ hit) <= ah:
+                    if aux != g0 or front is None or front[b][t + 1]:
+                        J -= P["gate_pass_bonus"]; aux = (aux + 1) % len(gates)
+                else:
+                    J += P["gate_miss_penalty"]
     elif P["objective"] == 1:
         ref = trk["ref"]
         Q = np.diag([P["Qp"]] * 3 + [P["Qv"]] * 3 + [P["Qw"]] * 3)
