@@ -52,7 +52,10 @@ typedef struct mppi_ctx mppi_ctx; /* opaque, owned by the library */
 typedef enum {
     MPPI_OBJ_GATE = 0,    /* J_gate,    eq.(6) PAPER.md:105-112 (BASELINE.json configs[0,1,4]) */
     MPPI_OBJ_TRACK = 1,   /* J_track,   eq.(8) PAPER.md:139-147 (configs[2])                   */
-    MPPI_OBJ_CONTOUR = 2  /* J_contour, eq.(9) PAPER.md:149-161 (configs[3])                   */
+    MPPI_OBJ_CONTOUR = 2, /* J_contour, eq.(9) PAPER.md:149-161 (configs[3])                   */
+    MPPI_OBJ_GATE_PAPER = 3 /* the paper's own J_gate: eq.(6),(7) PAPER.md:105-129 with squared distances,
+                             the Q_near term and the temporal gate-switching check of Fig. 2
+                             (PAPER.md:114-122); tracks are gates; see mppi_set_prev_front          */
 } mppi_objective;
 
 typedef enum {
@@ -122,6 +125,9 @@ typedef struct {
     int32_t store_noise; /* 1: also keep dU of the last step for mppi_debug_noise (always kept
                             in the TWO_PASS pipeline)                                            */
     int32_t variant;   /* mppi_variant: which rollout kernel the fused pipeline launches          */
+    float q_near, r_near; /* MPPI_OBJ_GATE_PAPER, eq.(7): + q_near |p_k - c|^2 on every pre-step state
+                          within r_near metres of its target gate centre; both >= 0 (the paper
+                          prints neither value)                                                  */
 } mppi_params;
 
 #define MPPI_MAX_N 256
@@ -194,6 +200,22 @@ MPPI_API int mppi_step_host(mppi_ctx* ctx, const float* h_x0, const int32_t* h_s
  * d_u_new. */
 MPPI_API int mppi_sim_step(mppi_ctx* ctx, float* d_x, int32_t* d_start, const float* d_u_new,
                   float* d_u_nom_next, void* cuda_stream);
+
+/* MPPI_OBJ_GATE_PAPER: flags of the previous control iteration for the temporal gate-switching check
+ * (Fig. 2).  d_prev_front [B][N+1] int32 device, caller-owned, read by every
+ * later mppi_step until replaced: entry [b][k] != 0 says that state k of the previous iteration's
+ * horizon was in front of the controller's start gate.  A geometric pass of the START gate at state
+ * k registers (bonus, target switch) only if that entry is set; passes of later gates of the horizon
+ * register on geometry alone.  NULL (the initial setting) = all set = purely geometric.  How the
+ * indices of two iterations correspond (same index, or shifted by the control steps elapsed) is the
+ * caller's choice: shift the array accordingly. */
+MPPI_API int mppi_set_prev_front(mppi_ctx* ctx, const int32_t* d_prev_front);
+
+/* The flags mppi_set_prev_front takes, computed for a nominal sequence: rolls d_u [B][N][4] out from
+ * d_x0 [B][13] without noise (thrusts clamped) and writes d_front_out [B][N+1] int32:
+ * [b][k] = 1 iff n.(p_k - c) < 0 for the gate d_start[b] (wrapped mod G).  Needs mppi_set_gates. */
+MPPI_API int mppi_front_flags(mppi_ctx* ctx, const float* d_x0, const int32_t* d_start, const float* d_u,
+                     int32_t* d_front_out, void* cuda_stream);
 
 /* Device pointer to dU [B][N][K][4] of the last step (parity debugging); NULL unless the
  * context keeps it (TWO_PASS pipeline or store_noise). */

@@ -14,13 +14,13 @@ import numpy as np
 _HERE = Path(__file__).resolve().parent
 LIB_PATH = _HERE / "libmppi.so"
 
-OBJ_GATE, OBJ_TRACK, OBJ_CONTOUR = 0, 1, 2
+OBJ_GATE, OBJ_TRACK, OBJ_CONTOUR, OBJ_GATE_PAPER = 0, 1, 2, 3
 PIPE_FUSED, PIPE_TWO_PASS = 0, 1
 VARIANT_AUTO, VARIANT_THROUGHPUT, VARIANT_LATENCY, VARIANT_PACKED, VARIANT_PIPELINED = 0, 1, 2, 3, 4
 
 EXPORTS = ["mppi_default_params", "mppi_create", "mppi_destroy", "mppi_set_gates",
            "mppi_set_reference", "mppi_set_path", "mppi_step", "mppi_optimize", "mppi_step_host",
-           "mppi_sim_step", "mppi_debug_noise", "mppi_get_info", "mppi_launch_count",
+           "mppi_sim_step", "mppi_set_prev_front", "mppi_front_flags", "mppi_debug_noise", "mppi_get_info", "mppi_launch_count",
            "mppi_error_string", "mppi_last_error", "mppi_measure_fma_peak", "mppi_measure_copy_bw"]
 
 
@@ -36,7 +36,8 @@ class MppiParams(C.Structure):
                 ("R", C.c_float), ("q_contour", C.c_float), ("q_lag", C.c_float),
                 ("mu_progress", C.c_float), ("window", C.c_int32), ("pipeline", C.c_int32),
                 ("use_graph", C.c_int32), ("block_threads", C.c_int32), ("fast_math", C.c_int32),
-                ("store_noise", C.c_int32), ("variant", C.c_int32)]
+                ("store_noise", C.c_int32), ("variant", C.c_int32), ("q_near", C.c_float),
+                ("r_near", C.c_float)]
 
 
 class MppiInfo(C.Structure):
@@ -65,6 +66,8 @@ def _load():
     L.mppi_optimize.argtypes = [vp, fp, ip, fp, C.c_uint64, C.c_uint32, C.c_int, fp, fp, vp]
     L.mppi_step_host.argtypes = [vp, fp, ip, fp, C.c_uint64, C.c_uint32, fp, fp, fp, vp]
     L.mppi_sim_step.argtypes = [vp, fp, ip, fp, fp, vp]
+    L.mppi_set_prev_front.argtypes = [vp, ip]
+    L.mppi_front_flags.argtypes = [vp, fp, ip, fp, ip, vp]
     L.mppi_debug_noise.argtypes = [vp]
     L.mppi_debug_noise.restype = C.c_void_p
     L.mppi_get_info.argtypes = [vp, C.POINTER(MppiInfo)]
@@ -178,6 +181,9 @@ class Mppi:
         """Convenience: feed whichever of gates / ref / path a workloads.Workload carries."""
         if wl.gates is not None:
             self.set_gates(wl.gates)
+        if getattr(wl, "prev_front", None) is not None:
+            import torch
+            self.set_prev_front(torch.from_numpy(np.ascontiguousarray(wl.prev_front, dtype=np.int32)).cuda())
         if wl.ref is not None:
             self.set_reference(wl.ref)
         if wl.path is not None:
@@ -270,6 +276,26 @@ class Mppi:
                                    self._dev(u_nom_next, (B, N, 4), torch.float32),
                                    _stream_ptr(stream)))
         return x, start, u_nom_next
+
+    def set_prev_front(self, prev_front):
+        """prev_front: CUDA int32 tensor [B, N+1] (kept alive by this object), or None."""
+        import torch
+        if prev_front is None:
+            self._prev_front = None
+            self._ck(lib.mppi_set_prev_front(self._h, None))
+            return
+        self._prev_front = prev_front
+        self._ck(lib.mppi_set_prev_front(self._h, self._dev(prev_front, (self.B, self.N + 1), torch.int32)))
+
+    def front_flags(self, x0, start, u, out=None, stream=None):
+        import torch
+        B, N = self.B, self.N
+        out = torch.empty((B, N + 1), dtype=torch.int32, device=x0.device) if out is None else out
+        self._ck(lib.mppi_front_flags(self._h, self._dev(x0, (B, 13), torch.float32),
+                                      self._dev(start, (B,), torch.int32),
+                                      self._dev(u, (B, N, 4), torch.float32),
+                                      self._dev(out, (B, N + 1), torch.int32), _stream_ptr(stream)))
+        return out
 
     def debug_noise(self):
         """dU [B,N,K,4] of the last step as a torch tensor copy, or None if the context keeps none."""

@@ -34,6 +34,7 @@ struct mppi_ctx {
     float4* d_du = nullptr;
     float* d_partials = nullptr;
     unsigned* d_counters = nullptr;
+    const int* d_prev_front = nullptr;     // caller-owned (mppi_set_prev_front)
     // device staging for mppi_step_host
     float* d_hx0 = nullptr; int* d_hstart = nullptr; float* d_hu = nullptr; float* d_hcost = nullptr;
     float* d_hw = nullptr;
@@ -99,6 +100,7 @@ extern "C" int mppi_default_params(mppi_params* p)
     p->window = 16;
     p->pipeline = MPPI_PIPE_FUSED; p->use_graph = 0; p->block_threads = 0; p->fast_math = 0;
     p->store_noise = 0; p->variant = MPPI_VARIANT_AUTO;
+    p->q_near = 0.0f; p->r_near = 0.0f;
     return MPPI_OK;
 }
 
@@ -111,7 +113,9 @@ static int validate(const mppi_params* p)
     BAD(p->K <= 0 || p->K % 32 != 0, "K must be a positive multiple of 32");
     BAD(p->N <= 0 || p->N > MPPI_MAX_N, "N must be in 1..MPPI_MAX_N");
     BAD(p->B <= 0 || p->B > 65535, "B must be in 1..65535");
-    BAD(p->objective < 0 || p->objective > 2, "objective must be 0, 1 or 2");
+    BAD(p->objective < 0 || p->objective > 3, "objective must be 0..3");
+    BAD(!(std::isfinite(p->q_near) && p->q_near >= 0.0f) || !(std::isfinite(p->r_near) && p->r_near >= 0.0f),
+        "q_near and r_near must be >= 0");
     BAD(!finite_pos(p->dt), "dt must be > 0");
     BAD(!finite_pos(p->lambda), "lambda must be > 0");
     BAD(!(std::isfinite(p->sigma) && p->sigma >= 0.0f), "sigma must be >= 0");
@@ -239,6 +243,7 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     d.gyy = (float)(((double)p->Jz - p->Jx) / p->Jy);
     d.gyz = (float)(((double)p->Jx - p->Jy) / p->Jz);
     d.w_omega = p->w_omega; d.miss = p->gate_miss_penalty; d.bonus = p->gate_pass_bonus;
+    d.q_near = p->q_near; d.r_near2 = (float)((double)p->r_near * (double)p->r_near);
     d.Qp = p->Qp; d.Qv = p->Qv; d.Qq = p->Qq; d.Qw = p->Qw; d.R = p->R;
     d.q_c = p->q_contour; d.q_l = p->q_lag; d.mu = p->mu_progress;
 
@@ -412,7 +417,7 @@ extern "C" int mppi_set_path(mppi_ctx* c, const float* pts, int P, int closed)
 static int prepare(mppi_ctx* c)
 {
     const int obj = c->prm.objective;
-    if ((obj == MPPI_OBJ_GATE && !c->have_gates) || (obj == MPPI_OBJ_TRACK && !c->have_ref) ||
+    if (((obj == MPPI_OBJ_GATE || obj == MPPI_OBJ_GATE_PAPER) && !c->have_gates) || (obj == MPPI_OBJ_TRACK && !c->have_ref) ||
         (obj == MPPI_OBJ_CONTOUR && !c->have_path))
         return fail(c, MPPI_E_NO_TRACK, "mppi_set_gates / mppi_set_reference / mppi_set_path not called for this objective");
     const size_t need = rollout_smem_bytes(c->dp, c->cfg);
@@ -437,7 +442,7 @@ static StepArgs make_args(mppi_ctx* c, const float* x0, const int32_t* start, co
     StepArgs a;
     a.x0 = x0; a.start = start; a.u_nom = u_nom; a.u_new = u_new; a.cost = cost; a.weights = w;
     a.du = c->d_du; a.partials = c->d_partials; a.counters = c->d_counters;
-    a.done_flag = nullptr; a.done_value = 0;
+    a.prev_front = c->d_prev_front; a.done_flag = nullptr; a.done_value = 0;
     a.seed_lo = (uint32_t)(seed & 0xffffffffu); a.seed_hi = (uint32_t)(seed >> 32); a.iter = iter;
     for (uint32_t r = 0; r < 10; ++r) {          // Philox key schedule (Weyl sequence), hoisted out of the kernel
         a.rk[2 * r] = a.seed_lo + r * 0x9E3779B9u;
@@ -621,6 +626,26 @@ extern "C" int mppi_sim_step(mppi_ctx* c, float* d_x, int32_t* d_start, const fl
     int rc = prepare(c);
     if (rc) return rc;
     CK(c, launch_sim(c->dp, c->prm.objective, d_x, d_start, d_u_new, d_u_nom_next, (cudaStream_t)stream));
+    c->launches += 1;
+    return MPPI_OK;
+}
+
+extern "C" int mppi_set_prev_front(mppi_ctx* c, const int32_t* d_prev_front)
+{
+    if (!c) return MPPI_E_NULL;
+    if (c->prm.objective != MPPI_OBJ_GATE_PAPER)
+        return fail(c, MPPI_E_PARAM, "mppi_set_prev_front: the objective is not MPPI_OBJ_GATE_PAPER");
+    c->d_prev_front = d_prev_front;
+    return MPPI_OK;
+}
+
+extern "C" int mppi_front_flags(mppi_ctx* c, const float* d_x0, const int32_t* d_start, const float* d_u,
+                                int32_t* d_front_out, void* stream)
+{
+    if (!c) return MPPI_E_NULL;
+    if (!d_x0 || !d_start || !d_u || !d_front_out) return fail(c, MPPI_E_NULL, "mppi_front_flags: NULL device pointer");
+    if (!c->have_gates) return fail(c, MPPI_E_NO_TRACK, "mppi_front_flags: mppi_set_gates not called");
+    CK(c, launch_front(c->dp, d_x0, d_start, d_u, d_front_out, (cudaStream_t)stream));
     c->launches += 1;
     return MPPI_OK;
 }

@@ -5,7 +5,7 @@
 
 namespace mppi {
 
-enum { OBJ_GATE = 0, OBJ_TRACK = 1, OBJ_CONTOUR = 2 };
+enum { OBJ_GATE = 0, OBJ_TRACK = 1, OBJ_CONTOUR = 2, OBJ_GATE_PAPER = 3 };
 
 // ---- gate progress: eq.(6) PAPER.md:105-110 with un-squared distances [D-2], in-horizon target
 // switching PAPER.md:112, geometric pass test [R-9],[R-10]; constants BASELINE.json configs[0].
@@ -78,6 +78,76 @@ struct GateCost {
         const float4 c = s_gates[4 * gate];
         const float d = norm3<MATH>(x.px - c.x, x.py - c.y, x.pz - c.z);
         return fmaf(P.w_omega, w2, J + (d - d0));
+    }
+};
+
+// ---- the paper's own gate progress: eq.(6),(7) PAPER.md:105-129 with SQUARED distances [R-23], the
+// conditional near-gate term Q_near |p_k - c|^2 for |p_k - c| < r_near on the pre-step state [R-24],
+// and the temporal gate-switching check of Fig. 2 [R-25]: a geometric pass of the
+// horizon's START gate at state index t+1 registers only if the caller's previous-iteration flag
+// front[t+1] is set; later gates of the horizon switch on geometry alone.  As in GateCost the
+// progress sum telescopes per constant-target segment (here without any square root).
+// s_front: N+1 ints in shared memory (all ones when the caller gave no flags).
+struct GatePaperCost {
+    int gate, gate0;
+    float d2_0;               // |p - c|^2 where the current segment began
+    float d2_prev;            // |p_t - c|^2 of the pre-step state against the current target
+    float s_prev;             // n . (p_t - c)
+    float ppx, ppy, ppz;      // p_t
+    float J;                  // bonuses / penalties / near terms / finished segments
+    float w2;                 // sum_t |omega_t|^2
+
+    __device__ __forceinline__ void retarget(const float4* s_gates, float px, float py, float pz)
+    {
+        const float4 c = s_gates[4 * gate], n = s_gates[4 * gate + 1];
+        const float rx = px - c.x, ry = py - c.y, rz = pz - c.z;
+        d2_0 = fmaf(rz, rz, fmaf(ry, ry, rx * rx));
+        d2_prev = d2_0;
+        s_prev = fmaf(n.z, rz, fmaf(n.y, ry, n.x * rx));
+    }
+    __device__ __forceinline__ void init(const DevParams& P, const float4* s_gates, int start, const State& x)
+    {
+        gate = wrap_index(start, P.G);
+        gate0 = gate;
+        J = 0.0f; w2 = 0.0f;
+        ppx = x.px; ppy = x.py; ppz = x.pz;
+        retarget(s_gates, x.px, x.py, x.pz);
+    }
+    // post-step state x_{t+1} of step t
+    __device__ __forceinline__ void step(const DevParams& P, const float4* s_gates, const int* s_front,
+                                         const State& x, int t)
+    {
+        if (d2_prev < P.r_near2) J = fmaf(P.q_near, d2_prev, J);          // eq.(7), pre-step state
+        const float4 c = s_gates[4 * gate], n = s_gates[4 * gate + 1];
+        const float ax = x.px - c.x, ay = x.py - c.y, az = x.pz - c.z;
+        const float d2 = fmaf(az, az, fmaf(ay, ay, ax * ax));
+        const float s = fmaf(n.z, az, fmaf(n.y, ay, n.x * ax));
+        bool switched = false;
+        if (s_prev < 0.0f && s >= 0.0f) {                 // front -> back through the plane
+            const float4 h = s_gates[4 * gate + 2], v = s_gates[4 * gate + 3];
+            const float alpha = s_prev / (s_prev - s);
+            const float rx = ppx - c.x, ry = ppy - c.y, rz = ppz - c.z;
+            const float hx = fmaf(alpha, ax - rx, rx), hy = fmaf(alpha, ay - ry, ry), hz = fmaf(alpha, az - rz, rz);
+            const float y = fmaf(h.z, hz, fmaf(h.y, hy, h.x * hx));
+            const float z = fmaf(v.z, hz, fmaf(v.y, hy, v.x * hx));
+            if (fabsf(y) <= c.w && fabsf(z) <= n.w) {
+                if (gate != gate0 || s_front[t + 1] != 0) {           // temporally consistent pass
+                    J += (d2 - d2_0) - P.bonus;                       // close the segment
+                    gate = (gate + 1 == P.G) ? 0 : gate + 1;
+                    retarget(s_gates, x.px, x.py, x.pz);              // new target from the next step on
+                    switched = true;
+                }
+            } else {
+                J += P.miss;                                          // miss: target unchanged
+            }
+        }
+        if (!switched) { s_prev = s; d2_prev = d2; }
+        ppx = x.px; ppy = x.py; ppz = x.pz;
+        w2 = fmaf(x.oz, x.oz, fmaf(x.oy, x.oy, fmaf(x.ox, x.ox, w2)));
+    }
+    __device__ __forceinline__ float finish(const DevParams& P) const
+    {
+        return fmaf(P.w_omega, w2, J + (d2_prev - d2_0));
     }
 };
 

@@ -20,6 +20,7 @@ struct DevParams {
     float ltx, lty, ltz;               // (arm/sqrt2)/Jx, (arm/sqrt2)/Jy, c_tau/Jz
     float gyx, gyy, gyz;               // (Jy-Jz)/Jx, (Jz-Jx)/Jy, (Jx-Jy)/Jz   (omega x J omega)
     float w_omega, miss, bonus;        // gate objective constants (BASELINE.json configs[0])
+    float q_near, r_near2;             // eq.(7): weight, threshold radius squared [R-24]
     float Qp, Qv, Qq, Qw, R;           // eq.(8)
     float q_c, q_l, mu, path_L, inv_path_L; // eq.(9) + closed path length
     const float4* gates;               // [G][4]: (c, a_h) (n, a_v) (h, 0) (v = h x n, 0)
@@ -38,6 +39,7 @@ struct StepArgs {
     float4* du;            // [B][N][K] float4 or nullptr
     float* partials;       // [B][blocks_per_ctrl][4N+4]  (fused pipeline)
     unsigned int* counters;// [B + 1]: last-block tickets per controller, finished controllers (fused pipeline)
+    const int* prev_front; // [B][N+1] or nullptr: previous-iteration "in front" flags (paper's J_gate, Fig. 2)
     unsigned int* done_flag;   // mapped host word, or nullptr: set to done_value once every output of the
     unsigned int done_value;   // call is visible to the host (mppi_step_host polls it instead of a stream sync)
     uint32_t seed_lo, seed_hi, iter;

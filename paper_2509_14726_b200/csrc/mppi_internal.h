@@ -29,6 +29,9 @@ cudaError_t launch_reduce(const DevParams& P, const StepArgs& A, cudaStream_t s)
 cudaError_t launch_sim(const DevParams& P, int objective, float* x, int* start, const float* u_new,
                        float* u_nom_next, cudaStream_t s);
 
+cudaError_t launch_front(const DevParams& P, const float* x0, const int* start, const float* u, int* front,
+                         cudaStream_t s);
+
 constexpr int kReduceThreads = 256;
 
 }  // namespace mppi

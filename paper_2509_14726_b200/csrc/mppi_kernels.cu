@@ -45,8 +45,11 @@ __device__ __forceinline__ void rollout_cost2(const DevParams& P, const StepArgs
     const int N = P.N;
     Ja = 0.0f; Jb = 0.0f;
     GateCost ga, gb;
+    GatePaperCost pa, pb;
     ContourCost ca, cb;
+    const int* s_front = reinterpret_cast<const int*>(s_trk + 4 * P.G);      // OBJ_GATE_PAPER only
     if (OBJ == OBJ_GATE) { ga.init<MATH>(P, s_trk, start, lane_state<0>(x)); gb = ga; }
+    if (OBJ == OBJ_GATE_PAPER) { pa.init(P, s_trk, start, lane_state<0>(x)); pb = pa; }
     if (OBJ == OBJ_CONTOUR) { ca.init(s_trk, contour_i0, lane_state<0>(x)); cb = ca; }
     for (int t = 0; t < N; ++t) {
         const float4 un = s_unom[t];
@@ -65,6 +68,10 @@ __device__ __forceinline__ void rollout_cost2(const DevParams& P, const StepArgs
             ga.step<MATH>(P, s_trk, lane_state<0>(x));
             gb.step<MATH>(P, s_trk, lane_state<1>(x));
         }
+        if (OBJ == OBJ_GATE_PAPER) {
+            pa.step(P, s_trk, s_front, lane_state<0>(x), t);
+            pb.step(P, s_trk, s_front, lane_state<1>(x), t);
+        }
         if (OBJ == OBJ_CONTOUR) {
             Ja += ca.step(P, s_trk, lane_state<0>(x));
             Jb += cb.step(P, s_trk, lane_state<1>(x));
@@ -74,6 +81,7 @@ __device__ __forceinline__ void rollout_cost2(const DevParams& P, const StepArgs
         Ja = ga.finish<MATH>(P, s_trk, lane_state<0>(x));
         Jb = gb.finish<MATH>(P, s_trk, lane_state<1>(x));
     }
+    if (OBJ == OBJ_GATE_PAPER) { Ja = pa.finish(P); Jb = pb.finish(P); }
     if (OBJ == OBJ_TRACK) {
         Ja += track_state_term(P, s_trk + 4 * N, lane_state<0>(x));
         Jb += track_state_term(P, s_trk + 4 * N, lane_state<1>(x));
@@ -423,6 +431,33 @@ __global__ void sim_kernel(const DevParams P, float* __restrict__ xs, int* __res
 }
 
 // ---------------------------------------------------------------------------------------------
+// "In front of the gate" flags of the noise-free rollout of a nominal sequence [R-26]: what the
+// temporal gate-switching check of the paper's J_gate (Fig. 2) compares the next
+// control iteration against.  front[b][k] = 1 iff n.(p_k - c) < 0 for the start gate, k = 0..N.
+// One thread per controller.
+// ---------------------------------------------------------------------------------------------
+__global__ void front_flags_kernel(const DevParams P, const float* __restrict__ x0, const int* __restrict__ start,
+                                   const float* __restrict__ u, int* __restrict__ front)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= P.B) return;
+    State x = load_state(x0 + 13 * b);
+    const int g = wrap_index(start[b], P.G);
+    const float4 c = P.gates[4 * g], n = P.gates[4 * g + 1];
+    const float4* ub = reinterpret_cast<const float4*>(u) + (size_t)b * P.N;
+    int* fb = front + (size_t)b * (P.N + 1);
+    for (int k = 0; k <= P.N; ++k) {
+        const float s = fmaf(n.z, x.pz - c.z, fmaf(n.y, x.py - c.y, n.x * (x.px - c.x)));
+        fb[k] = s < 0.0f ? 1 : 0;
+        if (k == P.N) break;
+        float4 T = ub[k];
+        T.x = fminf(fmaxf(T.x, P.T_min), P.T_max); T.y = fminf(fmaxf(T.y, P.T_min), P.T_max);
+        T.z = fminf(fmaxf(T.z, P.T_min), P.T_max); T.w = fminf(fmaxf(T.w, P.T_min), P.T_max);
+        rk4_step(P, x, T);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // host-side dispatch
 // ---------------------------------------------------------------------------------------------
 typedef void (*RolloutFn)(const DevParams, const StepArgs);
@@ -446,6 +481,7 @@ static RolloutFn pick(const LaunchCfg& c)
 {
     switch (c.objective) {
         case OBJ_GATE: return pick1<OBJ_GATE>(c);
+        case OBJ_GATE_PAPER: return pick1<OBJ_GATE_PAPER>(c);
         case OBJ_TRACK: return pick1<OBJ_TRACK>(c);
         default: return pick1<OBJ_CONTOUR>(c);
     }
@@ -463,6 +499,7 @@ static LatFn pick_lat(const LaunchCfg& c)
 {
     switch (c.objective) {
         case OBJ_GATE: return pick_lat1<OBJ_GATE>(c);
+        case OBJ_GATE_PAPER: return pick_lat1<OBJ_GATE_PAPER>(c);
         case OBJ_TRACK: return pick_lat1<OBJ_TRACK>(c);
         default: return pick_lat1<OBJ_CONTOUR>(c);
     }
@@ -479,6 +516,7 @@ static PipeFn pick_pipe(const LaunchCfg& c)
 {
     switch (c.objective) {
         case OBJ_GATE: return pick_pipe1<OBJ_GATE>(c);
+        case OBJ_GATE_PAPER: return pick_pipe1<OBJ_GATE_PAPER>(c);
         case OBJ_TRACK: return pick_pipe1<OBJ_TRACK>(c);
         default: return pick_pipe1<OBJ_CONTOUR>(c);
     }
@@ -511,9 +549,17 @@ cudaError_t launch_sim(const DevParams& P, int objective, float* x, int* start, 
                        float* u_nom_next, cudaStream_t s)
 {
     const int threads = 64;
-    if (objective == OBJ_GATE) sim_kernel<OBJ_GATE><<<P.B, threads, 0, s>>>(P, x, start, u_new, u_nom_next);
+    if (objective == OBJ_GATE || objective == OBJ_GATE_PAPER)       // the plant's gate advance is geometric
+        sim_kernel<OBJ_GATE><<<P.B, threads, 0, s>>>(P, x, start, u_new, u_nom_next);
     else if (objective == OBJ_TRACK) sim_kernel<OBJ_TRACK><<<P.B, threads, 0, s>>>(P, x, start, u_new, u_nom_next);
     else sim_kernel<OBJ_CONTOUR><<<P.B, threads, 0, s>>>(P, x, start, u_new, u_nom_next);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_front(const DevParams& P, const float* x0, const int* start, const float* u, int* front,
+                         cudaStream_t s)
+{
+    front_flags_kernel<<<(P.B + 63) / 64, 64, 0, s>>>(P, x0, start, u, front);
     return cudaGetLastError();
 }
 

@@ -162,7 +162,7 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
                 w[64] = make_float4(o3z, o4x, o4y, o4z);
                 kx = fmaf(P.gyx, o4y * o4z, ax); ky = fmaf(P.gyy, o4z * o4x, ay); kz = fmaf(P.gyz, o4x * o4y, az);
                 ox = fmaf(P.h6, kx, nx); oy = fmaf(P.h6, ky, ny); oz = fmaf(P.h6, kz, nz);
-                if (OBJ == OBJ_GATE) acc = fmaf(oz, oz, fmaf(oy, oy, fmaf(ox, ox, acc)));
+                if (OBJ == OBJ_GATE || OBJ == OBJ_GATE_PAPER) acc = fmaf(oz, oz, fmaf(oy, oy, fmaf(ox, ox, acc)));
                 if (OBJ == OBJ_CONTOUR) acc = fmaf(P.w_omega, ox * ox + oy * oy + oz * oz, acc);
             }
             mbar_arrive(bar_wf + s);
@@ -224,8 +224,11 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
         x.ox = x.oy = x.oz = 0.0f;          // the body-rate terms are W's
         float J = 0.0f;
         GateCost gc;
+        GatePaperCost gp;
         ContourCost cc;
+        const int* s_front = reinterpret_cast<const int*>(s_trk + 4 * P.G);      // OBJ_GATE_PAPER only
         if (OBJ == OBJ_GATE) gc.init<MATH>(P, s_trk, start, x);
+        if (OBJ == OBJ_GATE_PAPER) gp.init(P, s_trk, start, x);
         if (OBJ == OBJ_CONTOUR) cc.init(s_trk, i0, x);
         auto pv_term = [&](const float4* row) {
             const float4 a = row[0], r = row[1], r2 = row[2];
@@ -258,11 +261,13 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
                 x.vy = fmaf(kv, (Ay + my) + r4y, x.vy);
                 x.vz = fmaf(-kv, (Az + mz) + r4z, fmaf(P.dt, cz0, x.vz));
                 if (OBJ == OBJ_GATE) gc.step<MATH>(P, s_trk, x);
+                if (OBJ == OBJ_GATE_PAPER) gp.step(P, s_trk, s_front, x, t);
                 if (OBJ == OBJ_CONTOUR) J += cc.step(P, s_trk, x);
             }
             mbar_arrive(bar_qe + s);
         }
         if (OBJ == OBJ_GATE) J = gc.finish<MATH>(P, s_trk, x);
+        if (OBJ == OBJ_GATE_PAPER) J = gp.finish(P);
         if (OBJ == OBJ_TRACK) pv_term(s_trk + 4 * N);
         s_J[64 + lane] = J;
     }
@@ -273,7 +278,7 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
     if (warp == 0) {
         const float jw = s_J[lane], jq = s_J[32 + lane], jp = s_J[64 + lane];
         float J;
-        if (OBJ == OBJ_GATE) J = fmaf(P.w_omega, jw, jp);          // = GateCost::finish with W's sum |omega|^2
+        if (OBJ == OBJ_GATE || OBJ == OBJ_GATE_PAPER) J = fmaf(P.w_omega, jw, jp);   // = finish() with W's sum |omega|^2
         else if (OBJ == OBJ_TRACK) J = (jp + jq) + jw;
         else J = jp + jw;
         A.cost[(size_t)b * P.K + kbase + lane] = J;

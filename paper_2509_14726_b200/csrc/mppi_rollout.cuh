@@ -53,7 +53,9 @@ __device__ __forceinline__ float block_sum(float v, float* s_red)
 
 __host__ __device__ inline int track_f4(const DevParams& P, int objective)
 {
-    return objective == OBJ_GATE ? 4 * P.G : objective == OBJ_TRACK ? 4 * (P.N + 1) : 2 * P.P;
+    return objective == OBJ_GATE ? 4 * P.G
+         : objective == OBJ_GATE_PAPER ? 4 * P.G + (P.N + 4) / 4      // gates + N+1 previous-iteration flags
+         : objective == OBJ_TRACK ? 4 * (P.N + 1) : 2 * P.P;
 }
 
 // Stage the nominal sequence of controller b and the objective's track data in shared memory.
@@ -66,6 +68,10 @@ __device__ __forceinline__ void stage_inputs(const DevParams& P, const StepArgs&
     for (int t = tid; t < N; t += blockDim.x) s_unom[t] = un[t];
     if (OBJ == OBJ_GATE) {
         for (int i = tid; i < 4 * P.G; i += blockDim.x) s_trk[i] = P.gates[i];
+    } else if (OBJ == OBJ_GATE_PAPER) {
+        for (int i = tid; i < 4 * P.G; i += blockDim.x) s_trk[i] = P.gates[i];
+        int* s_front = reinterpret_cast<int*>(s_trk + 4 * P.G);
+        for (int i = tid; i <= N; i += blockDim.x) s_front[i] = A.prev_front ? A.prev_front[(size_t)b * (N + 1) + i] : 1;
     } else if (OBJ == OBJ_TRACK) {
         const int t0 = min(max(start, 0), P.M - 1 - N);
         for (int i = tid; i < 4 * (N + 1); i += blockDim.x) s_trk[i] = P.ref[4 * t0 + i];
@@ -121,17 +127,22 @@ __device__ __forceinline__ float rollout_cost(const DevParams& P, const float4* 
     const int N = P.N;
     float J = 0.0f;
     GateCost gc;
+    GatePaperCost gp;
     ContourCost cc;
+    const int* s_front = reinterpret_cast<const int*>(s_trk + 4 * P.G);      // OBJ_GATE_PAPER only
     if (OBJ == OBJ_GATE) gc.init<MATH>(P, s_trk, start, x);
+    if (OBJ == OBJ_GATE_PAPER) gp.init(P, s_trk, start, x);
     if (OBJ == OBJ_CONTOUR) cc.init(s_trk, contour_i0, x);
     for (int t = 0; t < N; ++t) {
         const float4 T = thrust(t);
         if (OBJ == OBJ_TRACK) J += track_stage(P, s_trk + 4 * t, x, T);
         rk4_step(P, x, T);
         if (OBJ == OBJ_GATE) gc.step<MATH>(P, s_trk, x);
+        if (OBJ == OBJ_GATE_PAPER) gp.step(P, s_trk, s_front, x, t);
         if (OBJ == OBJ_CONTOUR) J += cc.step(P, s_trk, x);
     }
     if (OBJ == OBJ_GATE) J = gc.finish<MATH>(P, s_trk, x);
+    if (OBJ == OBJ_GATE_PAPER) J = gp.finish(P);
     if (OBJ == OBJ_TRACK) J += track_state_term(P, s_trk + 4 * N, x);
     return J;
 }

@@ -20,7 +20,8 @@ REPORT: list[str] = []          # "reported separately" lines, printed at the en
 
 def oracle_track(wl):
     from oracle import oracle as O
-    return O.Track(gates=wl.gates, ref=wl.ref, path=wl.path, closed=wl.closed)
+    return O.Track(gates=wl.gates, ref=wl.ref, path=wl.path, closed=wl.closed,
+                   prev_front=getattr(wl, "prev_front", None))
 
 
 def make_ctx(wl, **opts):

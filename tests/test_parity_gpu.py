@@ -338,3 +338,75 @@ def test_error_paths_on_device():
         m.set_path(np.zeros((10, 3), np.float32))                         # P < 2 window + 1
     assert e.value.status == -4
     m.close()
+
+
+# ---- the paper's own J_gate (eq.(6),(7) + temporal check), objective 3 ----------
+
+@pytest.mark.parametrize("pipe", PIPES, ids=PIPE_IDS)
+@pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
+def test_gate_paper_objective(pipe, math):
+    # configs[1] geometry, squared progress + Q_near term, no flags (all in front)
+    g, o, st = run_case(W.gate_paper(), f"gate_paper[{pipe},{math}]", **pipe, **math)
+    # the near term is active for a good share of the samples: their costs differ from pure progress
+    wl = W.gate_paper(); wl.params["q_near"] = 0.0
+    o0 = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, wl.seed, 0)
+    assert (np.abs(o0["cost"] - o["cost"]) > 1e-3).mean() > 0.1
+
+
+@pytest.mark.parametrize("pipe", PIPES, ids=PIPE_IDS)
+def test_gate_paper_temporal_check_at_scale(pipe):
+    # crossing-heavy case with random previous-iteration flags: registered passes, ignored passes and
+    # misses all occur; the GPU must take every one of those decisions like the oracle
+    wl = W.stress_gate_paper(K=4096, N=30)
+    g, o, st = run_case(wl, f"stress_paper[{pipe}]", **pipe)
+    wl_all = W.stress_gate_paper(K=4096, N=30); wl_all.prev_front = None
+    o_all = Pz.oracle_step(wl_all, wl.x0, wl.start, wl.u_nom, wl.seed, 0)
+    reg, geo = o["ncross"][0] > 0, o_all["ncross"][0] > 0
+    assert reg.mean() > 0.1 and (geo & ~reg).mean() > 0.1
+    # and the flags really change the GPU result
+    m = Pz.make_ctx(wl_all, **pipe)
+    x0, start, u = Pz.to_dev(wl_all)
+    g_all = Pz.gpu_step(m, x0, start, u, wl.seed, 0)
+    m.close()
+    assert (np.abs(g_all["cost"] - g["cost"]) > 1.0).mean() > 0.1
+
+
+def test_front_flags_and_closed_loop_feed():
+    # the flags of the new nominal feed the next control iteration (shifted by the one control step
+    # that elapsed); every iteration is compared with the oracle, teacher-forced [R-17]
+    import torch
+    from oracle import oracle as O
+    B, K, N = 4, 1024, 30
+    wl = W.stress_gate_paper(K=K, N=N)
+    p = dict(wl.params, B=B)
+    rng = np.random.default_rng(2)
+    x0 = np.repeat(wl.x0, B, 0); x0[:, 0:3] += rng.uniform(-0.2, 0.2, (B, 3)).astype(np.float32)
+    from paper_2509_14726_b200 import binding as Bd
+    m = Bd.Mppi(p); m.set_gates(wl.gates)
+    x = torch.from_numpy(x0).cuda(); start = torch.zeros(B, dtype=torch.int32, device="cuda")
+    u = torch.from_numpy(np.repeat(wl.u_nom, B, 0)).cuda()
+    front = None
+    seen_zero = False
+    for step in range(6):
+        x_in, s_in, u_in = x.cpu().numpy(), start.cpu().numpy(), u.cpu().numpy()
+        m.set_prev_front(front)
+        u_new, cost, w = m.step(x, start, u, 7, step)
+        torch.cuda.synchronize()
+        trk = O.Track(gates=wl.gates, prev_front=None if front is None else front.cpu().numpy())
+        o = O.step(p, trk, x_in, s_in, u_in, 7, step)
+        o["u_nom"] = u_in.astype(np.float64)
+        gdict = dict(u_new=u_new.cpu().numpy(), cost=cost.cpu().numpy(), weights=w.cpu().numpy())
+        Pz.compare(f"paper loop step{step}", gdict, o, p["lambda"], True)
+        # flags of the new nominal from the current state, against the oracle's
+        f = m.front_flags(x, start, u_new); torch.cuda.synchronize()
+        fg = f.cpu().numpy()
+        for b in range(B):
+            fo, mg = O.front_flags(p, trk, x_in[b], int(s_in[b]), gdict["u_new"][b])
+            assert mg < 1e-5 or np.array_equal(fg[b], fo), (step, b)
+            assert fg[b, 0] == (1 if fo[0] else 0)
+        seen_zero |= bool((fg == 0).any())
+        # plant step, shift of the nominal and of the flags by one control step (last repeated)
+        m.sim_step(x, start, u_new, u_nom_next=u)
+        front = torch.cat([f[:, 1:], f[:, -1:]], dim=1).contiguous()
+    assert seen_zero                        # the nominal really crosses the gate plane within the horizon
+    m.close()
