@@ -11,10 +11,12 @@
  *                                                                  (eq.(2))
  *   3. each scored under one objective: gate progress with gate-plane crossing and target
  *      switching (eq.(6)), full-state tracking (eq.(8)) or
- *      contouring against an arc-length path (eq.(9))
+ *      contouring against an arc-length path (eq.(9)); or the paper's own gate
+ *      objective with squared progress, Q_near term and temporal switching check (eq.(6),(7),
+ *      Fig. 2)
  *   4. weights w_k = softmax(-J_k / lambda) and U*_new = sum_k w_k U^k
  *                                                     (eq.(4),(5))
- * The exact readings of every point the paper leaves open are listed in DESIGN.md (R-1..R-22).
+ * The exact readings of every point the paper leaves open are listed in DESIGN.md (R-1..R-26).
  *
  * Conventions
  *   - Notation follows BASELINE.json: K samples, N horizon steps, B controllers (the paper
@@ -194,7 +196,7 @@ MPPI_API int mppi_step_host(mppi_ctx* ctx, const float* h_x0, const int32_t* h_s
                    void* cuda_stream);
 
 /* Closed-loop glue of BASELINE.json configs[4] (receding horizon): the plant
- * (the same RK4 model) applies u_new[b][0] to d_x in place; d_start advances (gate: on a valid
+ * (the same RK4 model) applies u_new[b][0] to d_x in place; d_start advances (gate objectives: on a valid
  * pass of the plant segment through the current gate; tracking: +1 row; contouring: windowed
  * nearest vertex); d_u_nom_next[b][t] = d_u_new[b][min(t+1, N-1)].  d_u_nom_next may equal
  * d_u_new. */
