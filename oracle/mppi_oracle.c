@@ -48,6 +48,12 @@ typedef struct {
     int32_t window;
     int32_t pad_;
     double q_near, r_near;   /* eq.(7): weight and threshold radius [R-24] */
+    /* the paper's own input model, PAPER.md:72 and Table I */
+    int32_t input_model;     /* 0: rotor thrusts are the inputs (configs); 1: u = dT/dt, thrusts are states */
+    int32_t pad2_;
+    double rate_max;         /* |u_i| <= rate_max, N/s (Table I "Delta T_s [-10,10]") [R-28]            */
+    double drag_x, drag_y, drag_z; /* D = diag(.) of eq.(2), body frame, 1/s [R-30]                       */
+    double w_limit, omega_max;     /* "external cost" on the body-rate range [R-31]         */
 } orc_params;
 
 typedef struct {
@@ -144,6 +150,19 @@ void orc_fdyn(const orc_params* P, const double x[13], const double T[4], double
     xd[7] = (S / P->mass) * r13;
     xd[8] = (S / P->mass) * r23;
     xd[9] = (S / P->mass) * r33 - P->g;
+    if (P->drag_x != 0.0 || P->drag_y != 0.0 || P->drag_z != 0.0) {
+        /* - R D R^T v, D = diag(drag) in the body frame (eq.(2)) [R-30]: full R(q) */
+        const double R[3][3] = {
+            { 1.0 - 2.0 * (qy * qy + qz * qz), 2.0 * (qx * qy - qw * qz), r13 },
+            { 2.0 * (qx * qy + qw * qz), 1.0 - 2.0 * (qx * qx + qz * qz), r23 },
+            { 2.0 * (qx * qz - qw * qy), 2.0 * (qy * qz + qw * qx), r33 } };
+        const double d[3] = { P->drag_x, P->drag_y, P->drag_z };
+        const double v[3] = { vx, vy, vz };
+        for (int j = 0; j < 3; ++j) {                      /* body axis j = column j of R */
+            const double vb = R[0][j] * v[0] + R[1][j] * v[1] + R[2][j] * v[2];   /* (R^T v)_j */
+            for (int i = 0; i < 3; ++i) xd[7 + i] -= R[i][j] * d[j] * vb;
+        }
+    }
 
     /* omega_dot = J^-1 (tau - omega x J omega) */
     const double lever = P->arm / sqrt(2.0);
@@ -177,6 +196,43 @@ void orc_rk4_step(const orc_params* P, const double x[13], const double T[4], do
         xn[i] = x[i] + (dt / 6.0) * (k1[i] + 2.0 * k2[i] + 2.0 * k3[i] + k4[i]);
     const double nq = sqrt(xn[3] * xn[3] + xn[4] * xn[4] + xn[5] * xn[5] + xn[6] * xn[6]);
     for (int i = 3; i < 7; ++i) xn[i] /= nq;
+}
+
+/* The paper's own input model ("Following the approach in [4], we define the control
+ * input u as the derivative of the single rotor thrust"): state x = [p, q, v, omega, T(4)] (17),
+ * T' = u held over the step [R-27].  Classical RK4 on the 17-vector (the stage thrusts are
+ * T, T + dt/2 u, T + dt/2 u, T + dt u, unclamped), quaternion renormalised, then the thrust STATES
+ * are projected onto [T_min, T_max] (Table I "T_s [0,10]"; the paper's soft external cost for the
+ * range has no printed form) [R-29]. */
+void orc_rk4_rate_step(const orc_params* P, const double x[17], const double u[4], double dt,
+                       double xn[17])
+{
+    double k[4][17], xs[17];
+    memcpy(xs, x, sizeof xs);
+    for (int st = 0; st < 4; ++st) {
+        orc_fdyn(P, xs, xs + 13, k[st]);
+        for (int i = 0; i < 4; ++i) k[st][13 + i] = u[i];
+        if (st == 3) break;
+        const double c = st == 2 ? dt : 0.5 * dt;
+        for (int i = 0; i < 17; ++i) xs[i] = x[i] + c * k[st][i];
+    }
+    for (int i = 0; i < 17; ++i)
+        xn[i] = x[i] + (dt / 6.0) * (k[0][i] + 2.0 * k[1][i] + 2.0 * k[2][i] + k[3][i]);
+    const double nq = sqrt(xn[3] * xn[3] + xn[4] * xn[4] + xn[5] * xn[5] + xn[6] * xn[6]);
+    for (int i = 3; i < 7; ++i) xn[i] /= nq;
+    for (int i = 13; i < 17; ++i) xn[i] = fmin(fmax(xn[i], P->T_min), P->T_max);
+}
+
+/* "External cost" for the body-rate range of Table I [R-31]:
+ * w_limit sum_i max(0, |omega_i| - omega_max)^2 on a state's body rates. */
+double orc_rate_limit_cost(const orc_params* P, const double omega[3])
+{
+    double J = 0.0;
+    for (int i = 0; i < 3; ++i) {
+        const double e = fabs(omega[i]) - P->omega_max;
+        if (e > 0.0) J += e * e;
+    }
+    return P->w_limit * J;
 }
 
 /* ------------------------------------------------------------------------------------------
@@ -445,8 +501,9 @@ double orc_rollout_cost(const orc_params* P, const orc_track* trk, const orc_pat
                         double* du /*[N][4]*/, double* margin, int32_t* ncross, int32_t* aux_end,
                         double* x_end /*[13] or NULL*/)
 {
-    double x[13];
-    memcpy(x, x0, sizeof x);
+    const int rate = P->input_model == 1;            /* x0 then has 17 entries: ..., T(4) */
+    double x[17];
+    memcpy(x, x0, sizeof(double) * (rate ? 17 : 13));
     int32_t aux = start;
     if (P->objective == ORC_OBJ_GATE_PAPER) { aux = start % trk->G; if (aux < 0) aux += trk->G; }
     const int32_t gate0 = aux;
@@ -464,17 +521,27 @@ double orc_rollout_cost(const orc_params* P, const orc_track* trk, const orc_pat
     for (int t = 0; t < P->N; ++t) {
         double z[4], T[4];
         orc_normals(seed, k, (uint32_t)t, iter, b, z);                   /* eq.(3) */
+        const double lo = rate ? -P->rate_max : P->T_min, hi = rate ? P->rate_max : P->T_max;
         for (int i = 0; i < 4; ++i) {
             double Ti = u_nom[4 * t + i] + P->sigma * z[i];
-            Ti = fmin(fmax(Ti, P->T_min), P->T_max);                       /* hard clamp [D-5] */
+            Ti = fmin(fmax(Ti, lo), hi);          /* hard clamp [D-5]; thrust rates: [R-28] */
             T[i] = Ti;
             du[4 * t + i] = Ti - u_nom[4 * t + i];                         /* [R-8] */
         }
-        if (P->objective == ORC_OBJ_TRACK)
-            J += orc_track_stage(P, x, T, trk->ref + 13 * (start + t));    /* eq.(8) stage */
+        if (P->objective == ORC_OBJ_TRACK) {
+            if (rate) {                           /* eq.(8): ||u_k||^2_R on the inputs = the rates [R-32] */
+                double eu = 0.0;
+                for (int i = 0; i < 4; ++i) eu += T[i] * T[i];
+                J += orc_track_state_term(P, x, trk->ref + 13 * (start + t)) + P->R * eu;
+            } else {
+                J += orc_track_stage(P, x, T, trk->ref + 13 * (start + t));    /* eq.(8) stage */
+            }
+        }
 
-        double xn[13];
-        orc_rk4_step(P, x, T, P->dt, xn);                                  /* Alg.1 l.7-9 */
+        double xn[17];
+        if (rate) orc_rk4_rate_step(P, x, T, P->dt, xn);                   /* [R-27],[R-29] */
+        else orc_rk4_step(P, x, T, P->dt, xn);                             /* Alg.1 l.7-9 */
+        if (rate) J += orc_rate_limit_cost(P, xn + 10);                    /* [R-31] */
 
         if (P->objective == ORC_OBJ_GATE)
             J += orc_gate_step(P, trk, x, xn, xn + 10, &aux, &marg, &nc);
@@ -483,7 +550,7 @@ double orc_rollout_cost(const orc_params* P, const orc_track* trk, const orc_pat
             J += orc_gate_paper_step(P, trk, x, xn, xn + 10, &aux, gate0, front_ok, &marg, &nc);
         } else if (P->objective == ORC_OBJ_CONTOUR)
             J += orc_contour_step(P, trk, pa->s, pa->tan, pa->L, xn, xn + 10, &aux, &theta_prev);
-        memcpy(x, xn, sizeof x);
+        memcpy(x, xn, sizeof(double) * (rate ? 17 : 13));
     }
     if (P->objective == ORC_OBJ_TRACK)
         J += orc_track_state_term(P, x, trk->ref + 13 * (start + P->N));   /* eq.(8) terminal */
@@ -491,7 +558,7 @@ double orc_rollout_cost(const orc_params* P, const orc_track* trk, const orc_pat
     if (margin) *margin = marg;
     if (ncross) *ncross = nc;
     if (aux_end) *aux_end = aux;
-    if (x_end) memcpy(x_end, x, sizeof x);
+    if (x_end) memcpy(x_end, x, sizeof(double) * (rate ? 17 : 13));
     return J;
 }
 
@@ -550,7 +617,7 @@ int orc_step(const orc_params* P, const orc_track* trk, const double* x0 /*[B][1
         for (int k = 0; k < K; ++k) {
             double mg; int32_t nc, ae;
             cost[(size_t)b * K + k] =
-                orc_rollout_cost(P, trk, &pa, x0 + 13 * b, start[b], un, seed, iter, (uint32_t)k,
+                orc_rollout_cost(P, trk, &pa, x0 + (P->input_model == 1 ? 17 : 13) * b, start[b], un, seed, iter, (uint32_t)k,
                                  (uint32_t)b, du + (size_t)k * N * 4, &mg, &nc, &ae, NULL);
             if (margin) margin[(size_t)b * K + k] = mg;
             if (ncross) ncross[(size_t)b * K + k] = nc;

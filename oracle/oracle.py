@@ -42,7 +42,10 @@ class _Params(C.Structure):
                 ("Qp", C.c_double), ("Qv", C.c_double), ("Qq", C.c_double), ("Qw", C.c_double),
                 ("R", C.c_double), ("q_contour", C.c_double), ("q_lag", C.c_double),
                 ("mu_progress", C.c_double), ("window", C.c_int32), ("pad_", C.c_int32),
-                ("q_near", C.c_double), ("r_near", C.c_double)]
+                ("q_near", C.c_double), ("r_near", C.c_double),
+                ("input_model", C.c_int32), ("pad2_", C.c_int32), ("rate_max", C.c_double),
+                ("drag_x", C.c_double), ("drag_y", C.c_double), ("drag_z", C.c_double),
+                ("w_limit", C.c_double), ("omega_max", C.c_double)]
 
 
 class _Track(C.Structure):
@@ -51,7 +54,9 @@ class _Track(C.Structure):
                 ("pts", C.POINTER(C.c_double)), ("prev_front", C.POINTER(C.c_int32))]
 
 
-_PARAM_KEYS = [f for f, _ in _Params._fields_ if f not in ("pad_",)]
+_PARAM_KEYS = [f for f, _ in _Params._fields_ if f not in ("pad_", "pad2_")]
+_OPTIONAL = {"q_near": 0.0, "r_near": 0.0, "input_model": 0, "rate_max": 0.0, "drag_x": 0.0, "drag_y": 0.0,
+             "drag_z": 0.0, "w_limit": 0.0, "omega_max": 0.0}
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int32)
 _up = C.POINTER(C.c_uint32)
@@ -74,6 +79,10 @@ def lib():
         L.orc_fdyn.restype = None
         L.orc_rk4_step.argtypes = [C.POINTER(_Params), _dp, _dp, C.c_double, _dp]
         L.orc_rk4_step.restype = None
+        L.orc_rk4_rate_step.argtypes = [C.POINTER(_Params), _dp, _dp, C.c_double, _dp]
+        L.orc_rk4_rate_step.restype = None
+        L.orc_rate_limit_cost.argtypes = [C.POINTER(_Params), _dp]
+        L.orc_rate_limit_cost.restype = C.c_double
         L.orc_gate_step.argtypes = [C.POINTER(_Params), C.POINTER(_Track), _dp, _dp, _dp, _ip, _dp,
                                     _ip]
         L.orc_gate_step.restype = C.c_double
@@ -129,12 +138,12 @@ def make_params(p: dict) -> _Params:
         src["lambda_"] = src.pop("lambda")
     for k in _PARAM_KEYS:
         if k not in src:
-            if k in ("q_near", "r_near"):           # only the paper's J_gate (objective 3) uses them
-                src[k] = 0.0
-                continue
-            raise KeyError(f"oracle params: missing '{k}'")
+            if k in _OPTIONAL:                      # the paper-variant extensions (objective 3, NEXT-2)
+                src[k] = _OPTIONAL[k]
+            else:
+                raise KeyError(f"oracle params: missing '{k}'")
         v = src[k]
-        setattr(s, k, int(v) if k in ("K", "N", "B", "objective", "window") else float(v))
+        setattr(s, k, int(v) if k in ("K", "N", "B", "objective", "window", "input_model") else float(v))
     return s
 
 
@@ -191,6 +200,19 @@ def rk4_step(params, x, T, dt=None):
     x = _f64(x, (13,)); T = _f64(T, (4,)); out = np.zeros(13)
     lib().orc_rk4_step(C.byref(P), _d(x), _d(T), float(P.dt if dt is None else dt), _d(out))
     return out
+
+
+def rk4_rate_step(params, x, u, dt=None):
+    """One RK4 step of the 17-state thrust-rate model [R-27],[R-29]."""
+    P = make_params(params)
+    x = _f64(x, (17,)); u = _f64(u, (4,)); out = np.zeros(17)
+    lib().orc_rk4_rate_step(C.byref(P), _d(x), _d(u), float(P.dt if dt is None else dt), _d(out))
+    return out
+
+
+def rate_limit_cost(params, omega):
+    P = make_params(params)
+    return lib().orc_rate_limit_cost(C.byref(P), _d(_f64(omega, (3,))))
 
 
 def gate_step(params, track: Track, p_prev, p, omega, gate):
@@ -270,7 +292,7 @@ def step(params, track: Track, x0, start, u_nom, seed, it, want_du=False, want_d
     du [B,K,N,4] | None, margin [B,K], ncross [B,K], aux_end [B,K])."""
     P = make_params(params)
     B, K, N = P.B, P.K, P.N
-    x0 = _f64(x0, (B, 13)); u_nom = _f64(u_nom, (B, N, 4))
+    x0 = _f64(x0, (B, 17 if P.input_model == 1 else 13)); u_nom = _f64(u_nom, (B, N, 4))
     start = np.ascontiguousarray(np.asarray(start, dtype=np.int32).reshape(B))
     u_new = np.zeros((B, N, 4)); cost = np.zeros((B, K)); w = np.zeros((B, K))
     du = np.zeros((B, K, N, 4)) if want_du else None

@@ -29,11 +29,12 @@ def base_params(**over) -> dict:
              dt=0.02, sigma=1.0, mass=0.85, Jx=1e-3, Jy=1e-3, Jz=1.7e-3, arm=0.15, c_tau=0.016,
              g=9.81, T_min=0.0, T_max=7.0, w_omega=0.01, gate_miss_penalty=10.0,
              gate_pass_bonus=5.0, Qp=100.0, Qv=1.0, Qq=10.0, Qw=0.1, R=0.01, q_contour=200.0,
-             q_lag=50.0, mu_progress=2.0, window=16, q_near=0.0, r_near=0.0)
+             q_lag=50.0, mu_progress=2.0, window=16, q_near=0.0, r_near=0.0,
+             input_model=0, rate_max=0.0, drag_x=0.0, drag_y=0.0, drag_z=0.0, w_limit=0.0, omega_max=0.0)
     p["lambda"] = 1.0
     p.update(over)
     for k, v in p.items():
-        if k not in ("K", "N", "B", "objective", "window"):
+        if k not in ("K", "N", "B", "objective", "window", "input_model"):
             p[k] = _f32(v)
     return p
 
@@ -256,5 +257,35 @@ def stress_gate_paper(K=1024, N=30, flag_seed=5) -> Workload:
                     prev_front=front)
 
 
-ALL = {"gate_paper": gate_paper, "stress_gate_paper": stress_gate_paper, "cfg0": cfg0, "cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg4": cfg4,
+def _rate_model(wl: Workload, name: str, **over) -> Workload:
+    """The same scene under the paper's own input model (PAPER.md:72, Table I PAPER.md:216-221;
+    SURVEY.md NEXT-2): u = thrust RATES with the four rotor thrusts as extra states (x0 gets T = hover),
+    rates clamped to +-10 N/s, thrusts to [0, 10] N, sigma 5 N/s, rotor drag D = diag(0.25, 0.25, 0.1) 1/s
+    and a soft body-rate limit at 10 rad/s (the paper prints no drag value and no penalty form)."""
+    p = dict(wl.params, input_model=1, rate_max=_f32(10.0), T_max=_f32(10.0), sigma=_f32(5.0),
+             drag_x=_f32(0.25), drag_y=_f32(0.25), drag_z=_f32(0.1), w_limit=_f32(1.0), omega_max=_f32(10.0))
+    p.update(over)
+    B = wl.x0.shape[0]
+    x0 = np.concatenate([wl.x0, np.full((B, 4), hover_thrust(p), np.float32)], axis=1)
+    return Workload(name, p, x0.astype(np.float32), wl.start, np.zeros_like(wl.u_nom), gates=wl.gates,
+                    ref=wl.ref, path=wl.path, closed=wl.closed, seed=wl.seed, prev_front=wl.prev_front)
+
+
+def rate_gate_paper(K=4096, N=50) -> Workload:
+    """NEXT-2 + NEXT-1 together: the paper's model and the paper's J_gate on the configs[1] track."""
+    return _rate_model(gate_paper(K=K, N=N), f"rate_gate_paper_K{K}_N{N}")
+
+
+def rate_track(K=4096, N=50) -> Workload:
+    """NEXT-2 under the tracking objective: eq.(8)'s input term acts on the rates."""
+    return _rate_model(cfg2(K=K, N=N), f"rate_track_K{K}_N{N}")
+
+
+def rate_stress(K=1024, N=30) -> Workload:
+    """Crossing-heavy gate case (objective 0) under the rate model, faster noise so that thrusts saturate."""
+    return _rate_model(stress_gate(K=K, N=N), "rate_stress_gate", sigma=_f32(40.0), rate_max=_f32(60.0))
+
+
+ALL = {"rate_gate_paper": rate_gate_paper, "rate_track": rate_track, "rate_stress": rate_stress,
+       "gate_paper": gate_paper, "stress_gate_paper": stress_gate_paper, "cfg0": cfg0, "cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg4": cfg4,
        "stress_gate": stress_gate}

@@ -61,6 +61,9 @@ def fdyn(P, x, T):
     vdot = np.array([0, 0, -P["g"]]) + rot(q) @ np.array([0, 0, np.sum(T)]) / P["mass"]
     qdot = 0.5 * lam(q) @ np.concatenate([[0.0], om])
     omdot = np.linalg.solve(J, tau - np.cross(om, J @ om))
+    if any(P.get(k, 0.0) for k in ("drag_x", "drag_y", "drag_z")):
+        Dm = np.diag([P["drag_x"], P["drag_y"], P["drag_z"]])          # eq.(2): - R D R^T v
+        vdot = vdot - rot(q) @ Dm @ rot(q).T @ v
     return np.concatenate([v, qdot, vdot, omdot])
 
 
@@ -70,6 +73,17 @@ def rk4(P, x, T):
     k3 = fdyn(P, x + h / 2 * k2, T); k4 = fdyn(P, x + h * k3, T)
     xn = x + h / 6 * (k1 + 2 * k2 + 2 * k3 + k4)
     xn[3:7] /= np.linalg.norm(xn[3:7])
+    return xn
+
+
+def rk4_rate(P, x, u):
+    """17-state thrust-rate model: z = [x13, T4], z' = [f_dyn(x13, T), u]."""
+    h = P["dt"]
+    f = lambda z: np.concatenate([fdyn(P, z[:13], z[13:]), u])
+    k1 = f(x); k2 = f(x + h / 2 * k1); k3 = f(x + h / 2 * k2); k4 = f(x + h * k3)
+    xn = x + h / 6 * (k1 + 2 * k2 + 2 * k3 + k4)
+    xn[3:7] /= np.linalg.norm(xn[3:7])
+    xn[13:] = np.clip(xn[13:], P["T_min"], P["T_max"])
     return xn
 
 
@@ -103,13 +117,18 @@ def rollout_cost(P, trk, x0, start, u_nom, seed, it, k, b):
     hover = P["mass"] * P["g"] / 4
     xs = [np.array(x0, dtype=float)]
     Ts = []
+    rate = P.get("input_model", 0) == 1
+    lo, hi = (-P["rate_max"], P["rate_max"]) if rate else (P["T_min"], P["T_max"])
     for t in range(N):
-        T = np.clip(u_nom[t] + P["sigma"] * normals(seed, k, t, it, b), P["T_min"], P["T_max"])
+        T = np.clip(u_nom[t] + P["sigma"] * normals(seed, k, t, it, b), lo, hi)
         Ts.append(T)
-        xs.append(rk4(P, xs[-1], T))
+        xs.append(rk4_rate(P, xs[-1], T) if rate else rk4(P, xs[-1], T))
     Ts = np.array(Ts)
     du = Ts - u_nom
     J = 0.0
+    if rate:                                   # soft body-rate limit on every post-step state
+        for t in range(1, N + 1):
+            J += P["w_limit"] * np.sum(np.maximum(np.abs(xs[t][10:13]) - P["omega_max"], 0.0) ** 2)
     aux = start
     if P["objective"] == 0:
         gates = trk["gates"]
@@ -157,7 +176,7 @@ def rollout_cost(P, trk, x0, start, u_nom, seed, it, k, b):
             qerr = x[3:7] @ x[3:7] + r[3:7] @ r[3:7] - 2 * abs(x[3:7] @ r[3:7])
             J += e @ Q @ e + P["Qq"] * qerr
             if t < N:
-                J += P["R"] * np.sum((Ts[t] - hover) ** 2)
+                J += P["R"] * np.sum((Ts[t] - (0.0 if rate else hover)) ** 2)
     else:
         pts, closed, W = trk["path"], trk["closed"], P["window"]
         s, tan, L = path_tables(pts, closed)
