@@ -130,6 +130,19 @@ typedef struct {
     float q_near, r_near; /* MPPI_OBJ_GATE_PAPER, eq.(7): + q_near |p_k - c|^2 on every pre-step state
                           within r_near metres of its target gate centre; both >= 0 (the paper
                           prints neither value)                                                  */
+    int32_t input_model; /* 0: the inputs are the four rotor thrusts, x has 13 entries (configs).
+                          1: the paper's own model: the inputs are the thrust RATES
+                          dT/dt in N/s and the rotor thrusts are states: every x / x0 row has 17
+                          entries (p, q, v, omega, T(4)); u_nom / u_new hold rates; sigma is in N/s.
+                          Rates are clamped to [-rate_max, rate_max], the thrust states are
+                          projected onto [T_min, T_max] after every step, eq.(8)'s input term
+                          R |u|^2 acts on the rates.  Runs on the scalar throughput kernel
+                          (variant AUTO or THROUGHPUT); mppi_sim_step / mppi_front_flags: not yet  */
+    float rate_max;      /* N/s, > 0 when input_model = 1 (Table I: 10)            */
+    float drag_x, drag_y, drag_z; /* D = diag(.) of eq.(2)'s rotor drag - R D R^T v, body frame, 1/s,
+                          >= 0; input_model = 1 only (the paper prints no value)                  */
+    float w_limit, omega_max; /* input_model = 1: soft body-rate limit ("external cost"):
+                          + w_limit sum_i max(0, |omega_i| - omega_max)^2 on every post-step state */
 } mppi_params;
 
 #define MPPI_MAX_N 256

@@ -37,7 +37,9 @@ class MppiParams(C.Structure):
                 ("mu_progress", C.c_float), ("window", C.c_int32), ("pipeline", C.c_int32),
                 ("use_graph", C.c_int32), ("block_threads", C.c_int32), ("fast_math", C.c_int32),
                 ("store_noise", C.c_int32), ("variant", C.c_int32), ("q_near", C.c_float),
-                ("r_near", C.c_float)]
+                ("r_near", C.c_float), ("input_model", C.c_int32), ("rate_max", C.c_float),
+                ("drag_x", C.c_float), ("drag_y", C.c_float), ("drag_z", C.c_float),
+                ("w_limit", C.c_float), ("omega_max", C.c_float)]
 
 
 class MppiInfo(C.Structure):
@@ -147,6 +149,7 @@ class Mppi:
             raise MppiError(rc, lib.mppi_last_error(None).decode())
         self._h = h
         self.K, self.N, self.B = self.params.K, self.params.N, self.params.B
+        self.xdim = 17 if self.params.input_model == 1 else 13
 
     # -- lifetime
     def close(self):
@@ -205,7 +208,7 @@ class Mppi:
         u_new = torch.empty((B, N, 4), dtype=torch.float32, device=dev) if u_new is None else u_new
         cost = torch.empty((B, K), dtype=torch.float32, device=dev) if cost is None else cost
         weights = torch.empty((B, K), dtype=torch.float32, device=dev) if weights is None else weights
-        self._ck(lib.mppi_step(self._h, self._dev(x0, (B, 13), torch.float32),
+        self._ck(lib.mppi_step(self._h, self._dev(x0, (B, self.xdim), torch.float32),
                                self._dev(start, (B,), torch.int32),
                                self._dev(u_nom, (B, N, 4), torch.float32), C.c_uint64(int(seed)),
                                C.c_uint32(int(it)), self._dev(u_new, (B, N, 4), torch.float32),
@@ -219,7 +222,7 @@ class Mppi:
         dev = x0.device
         cost = torch.empty((B, K), dtype=torch.float32, device=dev) if cost is None else cost
         weights = torch.empty((B, K), dtype=torch.float32, device=dev) if weights is None else weights
-        self._ck(lib.mppi_optimize(self._h, self._dev(x0, (B, 13), torch.float32),
+        self._ck(lib.mppi_optimize(self._h, self._dev(x0, (B, self.xdim), torch.float32),
                                    self._dev(start, (B,), torch.int32),
                                    self._dev(u, (B, N, 4), torch.float32), C.c_uint64(int(seed)),
                                    C.c_uint32(int(it0)), int(n_iters),
@@ -231,7 +234,7 @@ class Mppi:
                   want_cost=True, stream=None):
         """Host buffers in, host buffers out (numpy, or pinned torch CPU tensors via .numpy())."""
         B, N, K = self.B, self.N, self.K
-        x0 = _host_f32(x0, (B, 13)); u_nom = _host_f32(u_nom, (B, N, 4))
+        x0 = _host_f32(x0, (B, self.xdim)); u_nom = _host_f32(u_nom, (B, N, 4))
         start = np.ascontiguousarray(np.asarray(start, dtype=np.int32)).reshape(B)
         u_new = np.empty((B, N, 4), np.float32) if u_new is None else u_new
         if want_cost:
@@ -255,7 +258,7 @@ class Mppi:
                     and a.size == int(np.prod(shape))):
                 raise ValueError(f"need a C-contiguous {np.dtype(dtype).name} array with {int(np.prod(shape))} elements")
             return C.c_void_p(a.ctypes.data)
-        px0, pst, pu = chk(x0, (B, 13), np.float32), chk(start, (B,), np.int32), chk(u_nom, (B, N, 4), np.float32)
+        px0, pst, pu = chk(x0, (B, self.xdim), np.float32), chk(start, (B,), np.int32), chk(u_nom, (B, N, 4), np.float32)
         pun = chk(u_new, (B, N, 4), np.float32)
         pc = chk(cost, (B, K), np.float32) if cost is not None else None
         pw = chk(weights, (B, K), np.float32) if weights is not None else None
@@ -291,7 +294,7 @@ class Mppi:
         import torch
         B, N = self.B, self.N
         out = torch.empty((B, N + 1), dtype=torch.int32, device=x0.device) if out is None else out
-        self._ck(lib.mppi_front_flags(self._h, self._dev(x0, (B, 13), torch.float32),
+        self._ck(lib.mppi_front_flags(self._h, self._dev(x0, (B, self.xdim), torch.float32),
                                       self._dev(start, (B,), torch.int32),
                                       self._dev(u, (B, N, 4), torch.float32),
                                       self._dev(out, (B, N + 1), torch.int32), _stream_ptr(stream)))

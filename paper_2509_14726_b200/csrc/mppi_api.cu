@@ -44,6 +44,7 @@ struct mppi_ctx {
     unsigned char* h_pin = nullptr; unsigned char* d_pin = nullptr; unsigned char* d_in = nullptr;
     size_t pin_x0 = 0, pin_start = 0, pin_u = 0, pin_unew = 0, pin_cost = 0, pin_w = 0, pin_flag = 0, pin_bytes = 0;
     unsigned host_seq = 0;
+    int xdim = 13;         // floats per state row: 13, or 17 under the thrust-rate input model
     int64_t scratch_bytes = 0;
     int64_t launches = 0;
     GraphSlot g_step, g_opt;
@@ -101,6 +102,8 @@ extern "C" int mppi_default_params(mppi_params* p)
     p->pipeline = MPPI_PIPE_FUSED; p->use_graph = 0; p->block_threads = 0; p->fast_math = 0;
     p->store_noise = 0; p->variant = MPPI_VARIANT_AUTO;
     p->q_near = 0.0f; p->r_near = 0.0f;
+    p->input_model = 0; p->rate_max = 0.0f; p->drag_x = p->drag_y = p->drag_z = 0.0f;
+    p->w_limit = 0.0f; p->omega_max = 0.0f;
     return MPPI_OK;
 }
 
@@ -135,6 +138,18 @@ static int validate(const mppi_params* p)
         "the packed variant needs K % 64 == 0, block_threads <= 128 and 2*block_threads dividing K");
     BAD((p->variant == MPPI_VARIANT_LATENCY || p->variant == MPPI_VARIANT_PIPELINED) && p->pipeline != MPPI_PIPE_FUSED,
         "the latency variants need the fused pipeline");
+    BAD(p->input_model != 0 && p->input_model != 1, "input_model must be 0 or 1");
+    auto nonneg = [](float v) { return std::isfinite(v) && v >= 0.0f; };
+    BAD(!nonneg(p->drag_x) || !nonneg(p->drag_y) || !nonneg(p->drag_z) || !nonneg(p->w_limit) || !nonneg(p->omega_max) ||
+            !nonneg(p->rate_max), "drag, w_limit, omega_max, rate_max must be >= 0");
+    if (p->input_model == 0) {
+        BAD(p->drag_x != 0.0f || p->drag_y != 0.0f || p->drag_z != 0.0f || p->w_limit != 0.0f,
+            "rotor drag and the body-rate limit cost need input_model = 1");
+    } else {
+        BAD(!(p->rate_max > 0.0f), "rate_max must be > 0 when input_model = 1");
+        BAD(p->variant != MPPI_VARIANT_AUTO && p->variant != MPPI_VARIANT_THROUGHPUT,
+            "input_model = 1 runs on the scalar throughput kernel: variant must be AUTO or THROUGHPUT");
+    }
 #undef BAD
     return MPPI_OK;
 }
@@ -148,6 +163,11 @@ static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, i
     *lat_consumers = 0;
     *packed = 0;
     *pipe = 0;
+    if (p->input_model == 1) {                     // thrust-rate model: its own scalar kernel (mppi_rate.cu)
+        if (p->block_threads) { *block_threads = p->block_threads; return; }
+        for (int tpb : {128, 64, 32})
+            if (p->K % tpb == 0) { *block_threads = tpb; return; }
+    }
     const bool lat_ok = p->pipeline == MPPI_PIPE_FUSED && p->block_threads == 0;
     if (lat_ok && (p->variant == MPPI_VARIANT_PIPELINED || (p->variant == MPPI_VARIANT_AUTO && warps <= 4 * (int64_t)sm_count))) {
         *pipe = 1; *block_threads = 256;
@@ -244,6 +264,9 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     d.gyz = (float)(((double)p->Jx - p->Jy) / p->Jz);
     d.w_omega = p->w_omega; d.miss = p->gate_miss_penalty; d.bonus = p->gate_pass_bonus;
     d.q_near = p->q_near; d.r_near2 = (float)((double)p->r_near * (double)p->r_near);
+    d.input_model = p->input_model; d.rate_max = p->rate_max;
+    d.drag_x = p->drag_x; d.drag_y = p->drag_y; d.drag_z = p->drag_z;
+    d.w_limit = p->w_limit; d.omega_max = p->omega_max;
     d.Qp = p->Qp; d.Qv = p->Qv; d.Qq = p->Qq; d.Qw = p->Qw; d.R = p->R;
     d.q_c = p->q_contour; d.q_l = p->q_lag; d.mu = p->mu_progress;
 
@@ -252,6 +275,8 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     cfg.fused = p->pipeline == MPPI_PIPE_FUSED;
     cfg.store_du = (!cfg.fused || p->store_noise) ? 1 : 0;
     pick_shape(p, c->sm_count, &cfg.block_threads, &cfg.lat_consumers, &cfg.packed, &cfg.pipe);
+    cfg.rate = p->input_model == 1;
+    c->xdim = cfg.rate ? 17 : 13;
     d.blocks_per_ctrl = cfg.pipe ? p->K / 32 : cfg.lat_consumers ? p->K / (32 * cfg.lat_consumers)
                                           : p->K / (cfg.block_threads * (cfg.packed ? 2 : 1));
     cfg.smem_bytes = 0;   // fixed once the track is known
@@ -272,7 +297,7 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
         CKC(dev_alloc(c, &c->d_counters, (size_t)p->B + 1));
         CKC(cudaMemset(c->d_counters, 0, ((size_t)p->B + 1) * sizeof(unsigned)));
     }
-    CKC(dev_alloc(c, &c->d_hx0, (size_t)p->B * 13));
+    CKC(dev_alloc(c, &c->d_hx0, (size_t)p->B * c->xdim));
     CKC(dev_alloc(c, &c->d_hstart, (size_t)p->B));
     CKC(dev_alloc(c, &c->d_hu, BN4));
     CKC(dev_alloc(c, &c->d_hcost, BK));
@@ -282,7 +307,7 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
         // layout of the mapped staging block, every part 256-byte aligned
         auto up = [](size_t v) { return (v + 255) & ~(size_t)255; };
         size_t o = 0;
-        c->pin_x0 = o; o = up(o + (size_t)p->B * 13 * sizeof(float));
+        c->pin_x0 = o; o = up(o + (size_t)p->B * c->xdim * sizeof(float));
         c->pin_start = o; o = up(o + (size_t)p->B * sizeof(int32_t));
         c->pin_u = o; o = up(o + BN4 * sizeof(float));
         c->pin_unew = o; o = up(o + BN4 * sizeof(float));
@@ -570,7 +595,7 @@ extern "C" int mppi_step_host(mppi_ctx* c, const float* h_x0, const int32_t* h_s
         int rc = prepare(c);
         if (rc) return rc;
         unsigned char* hp = c->h_pin; unsigned char* dp = c->d_pin;
-        std::memcpy(hp + c->pin_x0, h_x0, B * 13 * sizeof(float));
+        std::memcpy(hp + c->pin_x0, h_x0, B * c->xdim * sizeof(float));
         std::memcpy(hp + c->pin_start, h_start, B * sizeof(int32_t));
         std::memcpy(hp + c->pin_u, h_u_nom, B * N * 4 * sizeof(float));
         CK(c, cudaMemcpyAsync(c->d_in, hp, c->pin_u + B * N * 4 * sizeof(float), cudaMemcpyHostToDevice, s));
@@ -603,7 +628,7 @@ extern "C" int mppi_step_host(mppi_ctx* c, const float* h_x0, const int32_t* h_s
         if (h_weights) std::memcpy(h_weights, hp + c->pin_w, B * K * sizeof(float));
         return MPPI_OK;
     }
-    CK(c, cudaMemcpyAsync(c->d_hx0, h_x0, B * 13 * sizeof(float), cudaMemcpyHostToDevice, s));
+    CK(c, cudaMemcpyAsync(c->d_hx0, h_x0, B * c->xdim * sizeof(float), cudaMemcpyHostToDevice, s));
     CK(c, cudaMemcpyAsync(c->d_hstart, h_start, B * sizeof(int32_t), cudaMemcpyHostToDevice, s));
     CK(c, cudaMemcpyAsync(c->d_hu, h_u_nom, B * N * 4 * sizeof(float), cudaMemcpyHostToDevice, s));
     int rc = mppi_step(c, c->d_hx0, c->d_hstart, c->d_hu, seed, iter, c->d_hu, c->d_hcost, c->d_hw, stream);
@@ -620,6 +645,7 @@ extern "C" int mppi_sim_step(mppi_ctx* c, float* d_x, int32_t* d_start, const fl
 {
     if (!c) return MPPI_E_NULL;
     if (!d_x || !d_start || !d_u_new || !d_u_nom_next) return fail(c, MPPI_E_NULL, "mppi_sim_step: NULL device pointer");
+    if (c->prm.input_model == 1) return fail(c, MPPI_E_PARAM, "mppi_sim_step: not available under input_model = 1 yet");
     const size_t ub = (size_t)c->prm.B * c->prm.N * 4 * sizeof(float);
     if (d_u_nom_next != d_u_new && overlaps(d_u_nom_next, ub, d_u_new, ub))
         return fail(c, MPPI_E_RANGE, "d_u_nom_next partially overlaps d_u_new");
@@ -645,6 +671,7 @@ extern "C" int mppi_front_flags(mppi_ctx* c, const float* d_x0, const int32_t* d
     if (!c) return MPPI_E_NULL;
     if (!d_x0 || !d_start || !d_u || !d_front_out) return fail(c, MPPI_E_NULL, "mppi_front_flags: NULL device pointer");
     if (!c->have_gates) return fail(c, MPPI_E_NO_TRACK, "mppi_front_flags: mppi_set_gates not called");
+    if (c->prm.input_model == 1) return fail(c, MPPI_E_PARAM, "mppi_front_flags: not available under input_model = 1 yet");
     CK(c, launch_front(c->dp, d_x0, d_start, d_u, d_front_out, (cudaStream_t)stream));
     c->launches += 1;
     return MPPI_OK;

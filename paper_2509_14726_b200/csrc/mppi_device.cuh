@@ -21,6 +21,9 @@ struct DevParams {
     float gyx, gyy, gyz;               // (Jy-Jz)/Jx, (Jz-Jx)/Jy, (Jx-Jy)/Jz   (omega x J omega)
     float w_omega, miss, bonus;        // gate objective constants (BASELINE.json configs[0])
     float q_near, r_near2;             // eq.(7): weight, threshold radius squared [R-24]
+    // the paper's own input model (Table I) [R-27]..[R-32]: u = dT/dt, thrusts are states
+    int input_model;
+    float rate_max, drag_x, drag_y, drag_z, w_limit, omega_max;
     float Qp, Qv, Qq, Qw, R;           // eq.(8)
     float q_c, q_l, mu, path_L, inv_path_L; // eq.(9) + closed path length
     const float4* gates;               // [G][4]: (c, a_h) (n, a_v) (h, 0) (v = h x n, 0)
@@ -112,18 +115,25 @@ __device__ __forceinline__ void perturb_pair(uint32_t ra, uint32_t rb, float sig
 // Perturbed, clamped rotor thrusts of one (sample, step) [R-8]: T = clamp(u_nom + sigma z).
 // The perturbation actually applied is dU = T - u_nom (formed by the callers that need it).
 template <int MATH>
-__device__ __forceinline__ float4 sample_thrust(const DevParams& P, const uint32_t (&rk)[20], uint32_t k,
-                                                uint32_t t, uint32_t iter, uint32_t b, const float4 un)
+__device__ __forceinline__ float4 sample_input(const DevParams& P, const uint32_t (&rk)[20], uint32_t k,
+                                               uint32_t t, uint32_t iter, uint32_t b, const float4 un,
+                                               const float lo, const float hi)
 {
     const uint4 r = philox4x32_10(k, t, iter, b, rk);
     float4 T;
     perturb_pair<MATH>(r.x, r.y, P.sigma, un.x, un.y, T.x, T.y);
     perturb_pair<MATH>(r.z, r.w, P.sigma, un.z, un.w, T.z, T.w);
-    T.x = fminf(fmaxf(T.x, P.T_min), P.T_max);
-    T.y = fminf(fmaxf(T.y, P.T_min), P.T_max);
-    T.z = fminf(fmaxf(T.z, P.T_min), P.T_max);
-    T.w = fminf(fmaxf(T.w, P.T_min), P.T_max);
+    T.x = fminf(fmaxf(T.x, lo), hi);
+    T.y = fminf(fmaxf(T.y, lo), hi);
+    T.z = fminf(fmaxf(T.z, lo), hi);
+    T.w = fminf(fmaxf(T.w, lo), hi);
     return T;
+}
+template <int MATH>
+__device__ __forceinline__ float4 sample_thrust(const DevParams& P, const uint32_t (&rk)[20], uint32_t k,
+                                                uint32_t t, uint32_t iter, uint32_t b, const float4 un)
+{
+    return sample_input<MATH>(P, rk, k, t, iter, b, un, P.T_min, P.T_max);
 }
 
 // ---- quadrotor state and dynamics, eq.(2) PAPER.md:65-72 -------------------------------------

@@ -12,6 +12,7 @@ struct LaunchCfg {
     int block_threads;  // rollout block size
     int packed;         // 1: rollout2_kernel, two samples per thread in fp32x2 registers
     int pipe;           // 1: rollout_pipe_kernel, one rollout pipelined over three warps (32 samples per block)
+    int rate;           // 1: rollout_rate_kernel (thrust-rate input model, mppi_rate.cu)
     int lat_consumers;  // 0: throughput kernel; 1, 2 or 4: latency kernel with that many rollout warps per block
     size_t smem_bytes;  // dynamic shared memory of the rollout kernel
 };
@@ -28,6 +29,10 @@ cudaError_t launch_rollout(const DevParams& P, const StepArgs& A, const LaunchCf
 cudaError_t launch_reduce(const DevParams& P, const StepArgs& A, cudaStream_t s);
 cudaError_t launch_sim(const DevParams& P, int objective, float* x, int* start, const float* u_new,
                        float* u_nom_next, cudaStream_t s);
+
+// mppi_rate.cu: the thrust-rate input model
+const void* rate_kernel_ptr(const LaunchCfg& c);
+cudaError_t launch_rate(const DevParams& P, const StepArgs& A, const LaunchCfg& c, cudaStream_t s);
 
 cudaError_t launch_front(const DevParams& P, const float* x0, const int* start, const float* u, int* front,
                          cudaStream_t s);

@@ -204,42 +204,8 @@ __global__ void rollout_kernel(const DevParams P, const StepArgs A)
 
     if (!FUSED) return;
 
-    // ---- block-local softmax partial (online-softmax form of eq.(4),(5)) ----
-    // m = min_k J, e_k = exp(-(J_k - m)/lambda), Z = sum e_k, S[t] = sum_k e_k dU_k[t].
-    // dU is not stored anywhere: for the samples with e_k > 0 it is re-derived from the
-    // counter-based stream, the warp's lanes spread over the horizon steps.
-    const float m = block_min(J, s_red);
-    const float e = exp_weight<MATH>((m - J) * P.inv_lambda);
-    const float Zb = block_sum(e, s_red);
-    {
-        const unsigned contrib = __ballot_sync(kFull, e > 0.0f);
-        const uint32_t kbase = (uint32_t)(blockIdx.x * blockDim.x + warp * 32);
-        for (int t0 = 0; t0 < N; t0 += 32) {
-            const int t = t0 + lane;
-            const float4 un = t < N ? s_unom[t] : make_float4(0.f, 0.f, 0.f, 0.f);
-            float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-            unsigned mm = contrib;
-            while (mm) {
-                const int l = __ffs(mm) - 1;
-                mm &= mm - 1;
-                const float el = __shfl_sync(kFull, e, l);
-                const float4 T = sample_thrust<MATH>(P, A.rk, kbase + l, (uint32_t)t, A.iter, (uint32_t)b, un);
-                acc.x = fmaf(el, T.x - un.x, acc.x); acc.y = fmaf(el, T.y - un.y, acc.y);
-                acc.z = fmaf(el, T.z - un.z, acc.z); acc.w = fmaf(el, T.w - un.w, acc.w);
-            }
-            if (t < N) s_acc[warp * N + t] = acc;
-        }
-    }
-    __syncthreads();
-    const int nw = blockDim.x >> 5;
-    float* part = A.partials + ((size_t)b * P.blocks_per_ctrl + blockIdx.x) * (4 * N + 4);
-    for (int j = tid; j < 4 * N; j += blockDim.x) {
-        float s = 0.0f;
-        for (int w = 0; w < nw; ++w) s += reinterpret_cast<const float*>(s_acc)[w * 4 * N + j];
-        part[j] = s;
-    }
-    if (tid == 0) { part[4 * N] = m; part[4 * N + 1] = Zb; }
-    publish_and_combine<MATH>(P, A, b, P.blocks_per_ctrl, s_unom, s_red, s_pair);
+    // block-local softmax partial + last-block combine (mppi_rollout.cuh)
+    block_partial_and_combine<MATH>(P, A, b, blockIdx.x, J, P.T_min, P.T_max, s_unom, s_red, s_acc, s_pair);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -524,6 +490,7 @@ static PipeFn pick_pipe(const LaunchCfg& c)
 
 const void* rollout_kernel_ptr(const LaunchCfg& c)
 {
+    if (c.rate) return rate_kernel_ptr(c);
     if (c.pipe) return reinterpret_cast<const void*>(pick_pipe(c));
     return c.lat_consumers > 0 ? reinterpret_cast<const void*>(pick_lat(c)) : reinterpret_cast<const void*>(pick(c));
 }
@@ -533,6 +500,7 @@ const void* sim_kernel_ptr() { return reinterpret_cast<const void*>(sim_kernel<O
 cudaError_t launch_rollout(const DevParams& P, const StepArgs& A, const LaunchCfg& c, cudaStream_t s)
 {
     const dim3 grid(P.blocks_per_ctrl, P.B), block(c.block_threads);
+    if (c.rate) return launch_rate(P, A, c, s);
     if (c.pipe) pick_pipe(c)<<<grid, block, c.smem_bytes, s>>>(P, A);
     else if (c.lat_consumers > 0) pick_lat(c)<<<grid, block, c.smem_bytes, s>>>(P, A, c.lat_consumers);
     else pick(c)<<<grid, block, c.smem_bytes, s>>>(P, A);

@@ -147,6 +147,54 @@ __device__ __forceinline__ float rollout_cost(const DevParams& P, const float4* 
     return J;
 }
 
+// Fused softmax update, first half, for kernels with one sample per thread: the block's online-softmax
+// partial  m = min_k J, e_k = exp(-(J_k - m)/lambda), Z = sum e_k, S[t] = sum_k e_k dU_k[t]  (eq.(4),(5)).
+// dU is not stored anywhere: for the samples with e_k > 0 it is re-derived from the counter-based
+// stream (inputs clamped to [lo, hi] as in the rollout), the warp's lanes spread over the horizon
+// steps.  Then publish_and_combine.  All threads of the block must call this.
+template <int MATH>
+__device__ __forceinline__ void publish_and_combine(const DevParams& P, const StepArgs& A, int b, int nb,
+                                                    const float4* s_unom, float* s_red, float* s_pair);
+template <int MATH>
+__device__ __forceinline__ void block_partial_and_combine(const DevParams& P, const StepArgs& A, const int b,
+                                                          const int chunk, const float J, const float lo, const float hi,
+                                                          const float4* s_unom, float* s_red, float4* s_acc, float* s_pair)
+{
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, N = P.N;
+    const float m = block_min(J, s_red);
+    const float e = exp_weight<MATH>((m - J) * P.inv_lambda);
+    const float Zb = block_sum(e, s_red);
+    {
+        const unsigned contrib = __ballot_sync(kFull, e > 0.0f);
+        const uint32_t kbase = (uint32_t)(chunk * blockDim.x + warp * 32);
+        for (int t0 = 0; t0 < N; t0 += 32) {
+            const int t = t0 + lane;
+            const float4 un = t < N ? s_unom[t] : make_float4(0.f, 0.f, 0.f, 0.f);
+            float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+            unsigned mm = contrib;
+            while (mm) {
+                const int l = __ffs(mm) - 1;
+                mm &= mm - 1;
+                const float el = __shfl_sync(kFull, e, l);
+                const float4 T = sample_input<MATH>(P, A.rk, kbase + l, (uint32_t)t, A.iter, (uint32_t)b, un, lo, hi);
+                acc.x = fmaf(el, T.x - un.x, acc.x); acc.y = fmaf(el, T.y - un.y, acc.y);
+                acc.z = fmaf(el, T.z - un.z, acc.z); acc.w = fmaf(el, T.w - un.w, acc.w);
+            }
+            if (t < N) s_acc[warp * N + t] = acc;
+        }
+    }
+    __syncthreads();
+    const int nw = blockDim.x >> 5;
+    float* part = A.partials + ((size_t)b * P.blocks_per_ctrl + chunk) * (4 * N + 4);
+    for (int j = tid; j < 4 * N; j += blockDim.x) {
+        float s = 0.0f;
+        for (int w = 0; w < nw; ++w) s += reinterpret_cast<const float*>(s_acc)[w * 4 * N + j];
+        part[j] = s;
+    }
+    if (tid == 0) { part[4 * N] = m; part[4 * N + 1] = Zb; }
+    publish_and_combine<MATH>(P, A, b, P.blocks_per_ctrl, s_unom, s_red, s_pair);
+}
+
 // Fused softmax update, second half ("last block done").  Every block of controller b has written
 // its partial  part = { S[4N] = sum_k e_k dU_k, m = min_k J_k, Z = sum_k e_k }  with
 // e_k = exp(-(J_k - m)/lambda)  (online-softmax form of eq.(4),(5)).  The block that

@@ -410,3 +410,62 @@ def test_front_flags_and_closed_loop_feed():
         front = torch.cat([f[:, 1:], f[:, -1:]], dim=1).contiguous()
     assert seen_zero                        # the nominal really crosses the gate plane within the horizon
     m.close()
+
+
+# ---- the paper's own input model (thrust rates, thrust states, drag, rate limit) ----
+
+RATE_PIPES = [dict(pipeline=0), dict(pipeline=0, variant=1, block_threads=64), dict(pipeline=1)]
+
+
+@pytest.mark.parametrize("pipe", RATE_PIPES, ids=["fused", "fused_tpb64", "two_pass"])
+@pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
+@pytest.mark.parametrize("name", ["rate_gate_paper", "rate_track"])
+def test_rate_model_objectives(name, pipe, math):
+    wl = W.ALL[name]()
+    g, o, st = run_case(wl, f"{name}[{pipe},{math}]", **pipe, **math)
+    # drag and the rate limit are really in play: switching them off changes the costs
+    wl0 = W.ALL[name](); wl0.params.update(drag_x=0.0, drag_y=0.0, drag_z=0.0, w_limit=0.0)
+    o0 = Pz.oracle_step(wl0, wl0.x0, wl0.start, wl0.u_nom, wl0.seed, 0)
+    assert (np.abs(o0["cost"] - o["cost"]) > 1e-3 * np.abs(o["cost"])).mean() > 0.5
+
+
+@pytest.mark.parametrize("pipe", RATE_PIPES, ids=["fused", "fused_tpb64", "two_pass"])
+def test_rate_model_saturation_and_crossings(pipe):
+    wl = W.rate_stress(K=4096, N=30)
+    g, o, st = run_case(wl, f"rate_stress[{pipe}]", **pipe)
+    nc = o["ncross"]
+    assert (nc > 0).mean() > 0.1 and (nc == 0).mean() > 0.1
+    assert (np.abs(o["du"]) == wl.params["rate_max"]).mean() > 0.05          # rate clamp acts at scale
+
+
+def test_rate_model_contouring_batch_and_warm_start():
+    # contouring under the rate model, B = 3, three warm-started iterations (teacher-forced)
+    import torch
+    wl = W._rate_model(W.cfg3(K=512, N=30), "rate_contour")
+    B = 3
+    wl.params = dict(wl.params, B=B)
+    wl.x0 = np.repeat(wl.x0, B, 0); wl.x0[1, 0:3] += np.float32([0.1, -0.1, 0.05]); wl.x0[2, 13:17] += np.float32(0.3)
+    wl.start = np.repeat(wl.start, B, 0); wl.u_nom = np.repeat(wl.u_nom, B, 0)
+    m = Pz.make_ctx(wl)
+    x0, start, u = Pz.to_dev(wl)
+    for it in range(3):
+        u_in = u.cpu().numpy()
+        g = Pz.gpu_step(m, x0, start, u, wl.seed, it, u_new=u)
+        o = Pz.oracle_step(wl, wl.x0, wl.start, u_in, wl.seed, it, want_du=True)
+        o["u_nom"] = u_in.astype(np.float64)
+        Pz.compare(f"rate_contour it{it}", g, o, wl.params["lambda"], False)
+    un, co, we = m.step_host(wl.x0, wl.start, u_in, wl.seed, 2)
+    np.testing.assert_array_equal(co, g["cost"])
+    m.close()
+
+
+def test_rate_model_rejects_what_it_does_not_support():
+    from paper_2509_14726_b200 import binding as Bd
+    wl = W.rate_gate_paper(K=64, N=8)
+    for bad in (dict(variant=2), dict(variant=3), dict(variant=4), dict(rate_max=0.0)):
+        with pytest.raises(Bd.MppiError) as e:
+            Bd.Mppi(wl.params, **bad)
+        assert e.value.status == -2
+    with pytest.raises(Bd.MppiError) as e:
+        Bd.Mppi(W.cfg0().params, drag_x=0.1)                    # drag needs the rate model
+    assert e.value.status == -2
