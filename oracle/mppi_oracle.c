@@ -19,6 +19,9 @@
  * invariant; closed-form free fall; yaw / roll / pitch torque closed forms; torque-free
  * precession; quaternion norm; hand-built gate cases; softmax invariants; a K=1,N=1 step by
  * hand; the survey's worked example (tests/golden/); an independently written numpy evaluator.
+ * The paper's own J_gate (objective 3) and input model (input_model = 1) have their own pins in
+ * tests/test_oracle_gate_paper.py and tests/test_oracle_rate_model.py (hand-built segments, free-fall
+ * flags, thrust-ramp / torque / drag closed forms, the numpy evaluator's own branches).
  * "parity unpinned": the numbers of the five BASELINE.json configs themselves -- the paper
  * prints no hot-path values -- and the uniform->normal mapping beyond its moments (it is a
  * definition, [R-2],[R-3]).
