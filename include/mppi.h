@@ -137,7 +137,7 @@ typedef struct {
                           Rates are clamped to [-rate_max, rate_max], the thrust states are
                           projected onto [T_min, T_max] after every step, eq.(8)'s input term
                           R |u|^2 acts on the rates.  Runs on the scalar throughput kernel
-                          (variant AUTO or THROUGHPUT); mppi_sim_step / mppi_front_flags: not yet  */
+                          (variant AUTO or THROUGHPUT); mppi_sim_step advances the 17-entry rows  */
     float rate_max;      /* N/s, > 0 when input_model = 1 (Table I: 10)            */
     float drag_x, drag_y, drag_z; /* D = diag(.) of eq.(2)'s rotor drag - R D R^T v, body frame, 1/s,
                           >= 0; input_model = 1 only (the paper prints no value)                  */

@@ -368,8 +368,9 @@ void orc_front_flags(const orc_params* P, const orc_track* trk, const double x0[
 {
     int32_t g = start % trk->G; if (g < 0) g += trk->G;
     const double* c = trk->gates + 11 * g; const double* n = c + 3;
-    double x[13], xn[13], mg = INFINITY;
-    memcpy(x, x0, sizeof x);
+    const int rate = P->input_model == 1;                    /* x0 then has 17 entries, u are rates */
+    double x[17], xn[17], mg = INFINITY;
+    memcpy(x, x0, sizeof(double) * (rate ? 17 : 13));
     for (int k = 0; k <= P->N; ++k) {
         const double r[3] = { x[0] - c[0], x[1] - c[1], x[2] - c[2] };
         const double s = dot3(n, r);
@@ -377,9 +378,11 @@ void orc_front_flags(const orc_params* P, const orc_track* trk, const double x0[
         if (fabs(s) < mg) mg = fabs(s);
         if (k == P->N) break;
         double T[4];
-        for (int i = 0; i < 4; ++i) T[i] = fmin(fmax(u[4 * k + i], P->T_min), P->T_max);
-        orc_rk4_step(P, x, T, P->dt, xn);
-        memcpy(x, xn, sizeof x);
+        const double lo = rate ? -P->rate_max : P->T_min, hi = rate ? P->rate_max : P->T_max;
+        for (int i = 0; i < 4; ++i) T[i] = fmin(fmax(u[4 * k + i], lo), hi);
+        if (rate) orc_rk4_rate_step(P, x, T, P->dt, xn);
+        else orc_rk4_step(P, x, T, P->dt, xn);
+        memcpy(x, xn, sizeof(double) * (rate ? 17 : 13));
     }
     if (margin) *margin = mg;
 }
@@ -649,10 +652,12 @@ int orc_sim_step(const orc_params* P, const orc_track* trk, double* x, int32_t* 
     if (!P || !trk || !x || !start || !u_new || !u_nom_next) return -1;
     const int N = P->N;
     for (int b = 0; b < P->B; ++b) {
-        double* xb = x + 13 * b;
+        const int rate = P->input_model == 1, xdim = rate ? 17 : 13;   /* [R-27]: rows of 17 */
+        double* xb = x + xdim * b;
         const double* ub = u_new + (size_t)b * N * 4;
-        double xn[13];
-        orc_rk4_step(P, xb, ub, P->dt, xn);
+        double xn[17];
+        if (rate) orc_rk4_rate_step(P, xb, ub, P->dt, xn);
+        else orc_rk4_step(P, xb, ub, P->dt, xn);
         if (P->objective == ORC_OBJ_GATE || P->objective == ORC_OBJ_GATE_PAPER) {
             int32_t gate = start[b];
             (void)orc_gate_step(P, trk, xb, xn, xn + 10, &gate, NULL, NULL);
@@ -664,7 +669,7 @@ int orc_sim_step(const orc_params* P, const orc_track* trk, double* x, int32_t* 
         } else {
             start[b] = orc_path_nearest(trk->pts, trk->P, trk->closed, xn, start[b], P->window);
         }
-        memcpy(xb, xn, sizeof xn);
+        memcpy(xb, xn, sizeof(double) * xdim);
         double* nn = u_nom_next + (size_t)b * N * 4;
         for (int t = 0; t < N; ++t) {
             const int src = (t + 1 < N) ? t + 1 : N - 1;

@@ -238,7 +238,7 @@ def front_flags(params, track: Track, x0, start, u):
     """[R-26] -> (front[N+1] int32, margin) of the noise-free rollout of u from x0."""
     P = make_params(params)
     u = _f64(u, (P.N, 4)); f = np.zeros(P.N + 1, np.int32); m = C.c_double(np.inf)
-    lib().orc_front_flags(C.byref(P), C.byref(track.c), _d(_f64(x0, (13,))), int(start), _d(u), _i(f), C.byref(m))
+    lib().orc_front_flags(C.byref(P), C.byref(track.c), _d(_f64(x0, (17 if P.input_model == 1 else 13,))), int(start), _d(u), _i(f), C.byref(m))
     return f, m.value
 
 
@@ -314,7 +314,7 @@ def sim_step(params, track: Track, x, start, u_new):
     """Closed-loop glue: -> (x_next [B,13], start_next [B], u_nom_next [B,N,4])."""
     P = make_params(params)
     B, N = P.B, P.N
-    x = _f64(x, (B, 13)).copy(); u_new = _f64(u_new, (B, N, 4))
+    x = _f64(x, (B, 17 if P.input_model == 1 else 13)).copy(); u_new = _f64(u_new, (B, N, 4))
     start = np.ascontiguousarray(np.asarray(start, dtype=np.int32).reshape(B)).copy()
     nxt = np.zeros((B, N, 4))
     rc = lib().orc_sim_step(C.byref(P), C.byref(track.c), _d(x), _i(start), _d(u_new), _d(nxt))

@@ -273,7 +273,7 @@ class Mppi:
         import torch
         B, N = self.B, self.N
         u_nom_next = torch.empty_like(u_new) if u_nom_next is None else u_nom_next
-        self._ck(lib.mppi_sim_step(self._h, self._dev(x, (B, 13), torch.float32),
+        self._ck(lib.mppi_sim_step(self._h, self._dev(x, (B, self.xdim), torch.float32),
                                    self._dev(start, (B,), torch.int32),
                                    self._dev(u_new, (B, N, 4), torch.float32),
                                    self._dev(u_nom_next, (B, N, 4), torch.float32),

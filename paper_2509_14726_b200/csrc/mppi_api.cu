@@ -645,7 +645,6 @@ extern "C" int mppi_sim_step(mppi_ctx* c, float* d_x, int32_t* d_start, const fl
 {
     if (!c) return MPPI_E_NULL;
     if (!d_x || !d_start || !d_u_new || !d_u_nom_next) return fail(c, MPPI_E_NULL, "mppi_sim_step: NULL device pointer");
-    if (c->prm.input_model == 1) return fail(c, MPPI_E_PARAM, "mppi_sim_step: not available under input_model = 1 yet");
     const size_t ub = (size_t)c->prm.B * c->prm.N * 4 * sizeof(float);
     if (d_u_nom_next != d_u_new && overlaps(d_u_nom_next, ub, d_u_new, ub))
         return fail(c, MPPI_E_RANGE, "d_u_nom_next partially overlaps d_u_new");
@@ -671,7 +670,6 @@ extern "C" int mppi_front_flags(mppi_ctx* c, const float* d_x0, const int32_t* d
     if (!c) return MPPI_E_NULL;
     if (!d_x0 || !d_start || !d_u || !d_front_out) return fail(c, MPPI_E_NULL, "mppi_front_flags: NULL device pointer");
     if (!c->have_gates) return fail(c, MPPI_E_NO_TRACK, "mppi_front_flags: mppi_set_gates not called");
-    if (c->prm.input_model == 1) return fail(c, MPPI_E_PARAM, "mppi_front_flags: not available under input_model = 1 yet");
     CK(c, launch_front(c->dp, d_x0, d_start, d_u, d_front_out, (cudaStream_t)stream));
     c->launches += 1;
     return MPPI_OK;

@@ -12,6 +12,7 @@
 #include "mppi_rollout.cuh"
 #include "mppi_packed.cuh"
 #include "mppi_pipe.cuh"
+#include "mppi_rate.cuh"
 
 namespace mppi {
 
@@ -350,19 +351,32 @@ __global__ void sim_kernel(const DevParams P, float* __restrict__ xs, int* __res
     const int b = blockIdx.x;
     const int N = P.N;
     if (threadIdx.x == 0) {
-        State x = load_state(xs + 13 * b);
-        const float4 T = reinterpret_cast<const float4*>(u_new)[(size_t)b * N];
+        const int xdim = P.input_model == 1 ? 17 : 13;
+        float* xb = xs + xdim * b;
+        State x = load_state(xb);
+        const float4 T = reinterpret_cast<const float4*>(u_new)[(size_t)b * N];   // thrusts, or thrust rates
+        float4 Ts = make_float4(0.f, 0.f, 0.f, 0.f);                               // thrust states (rate model)
+        if (P.input_model == 1) Ts = make_float4(xb[13], xb[14], xb[15], xb[16]);
+        auto plant = [&]() {
+            if (P.input_model == 1) {
+                const float4 u = make_float4(fminf(fmaxf(T.x, -P.rate_max), P.rate_max), fminf(fmaxf(T.y, -P.rate_max), P.rate_max),
+                                             fminf(fmaxf(T.z, -P.rate_max), P.rate_max), fminf(fmaxf(T.w, -P.rate_max), P.rate_max));
+                rk4_rate_step(P, x, Ts, u);
+            } else {
+                rk4_step(P, x, T);
+            }
+        };
         if (OBJ == OBJ_GATE) {
             GateCost gc;
             gc.init<0>(P, P.gates, start[b], x);
-            rk4_step(P, x, T);
+            plant();
             gc.step<0>(P, P.gates, x);
             start[b] = gc.gate;
         } else if (OBJ == OBJ_TRACK) {
-            rk4_step(P, x, T);
+            plant();
             start[b] = min(start[b] + 1, P.M - 1 - N);
         } else {
-            rk4_step(P, x, T);
+            plant();
             const int s0 = start[b];
             int i0;
             if (s0 < 0) {
@@ -379,7 +393,8 @@ __global__ void sim_kernel(const DevParams P, float* __restrict__ xs, int* __res
             }
             start[b] = i0;
         }
-        float* o = xs + 13 * b;
+        float* o = xb;
+        if (P.input_model == 1) { o[13] = Ts.x; o[14] = Ts.y; o[15] = Ts.z; o[16] = Ts.w; }
         o[0] = x.px; o[1] = x.py; o[2] = x.pz; o[3] = x.qw; o[4] = x.qx; o[5] = x.qy; o[6] = x.qz;
         o[7] = x.vx; o[8] = x.vy; o[9] = x.vz; o[10] = x.ox; o[11] = x.oy; o[12] = x.oz;
     }
@@ -407,7 +422,10 @@ __global__ void front_flags_kernel(const DevParams P, const float* __restrict__ 
 {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= P.B) return;
-    State x = load_state(x0 + 13 * b);
+    const float* xb = x0 + (P.input_model == 1 ? 17 : 13) * b;
+    State x = load_state(xb);
+    float4 Ts = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (P.input_model == 1) Ts = make_float4(xb[13], xb[14], xb[15], xb[16]);
     const int g = wrap_index(start[b], P.G);
     const float4 c = P.gates[4 * g], n = P.gates[4 * g + 1];
     const float4* ub = reinterpret_cast<const float4*>(u) + (size_t)b * P.N;
@@ -417,9 +435,11 @@ __global__ void front_flags_kernel(const DevParams P, const float* __restrict__ 
         fb[k] = s < 0.0f ? 1 : 0;
         if (k == P.N) break;
         float4 T = ub[k];
-        T.x = fminf(fmaxf(T.x, P.T_min), P.T_max); T.y = fminf(fmaxf(T.y, P.T_min), P.T_max);
-        T.z = fminf(fmaxf(T.z, P.T_min), P.T_max); T.w = fminf(fmaxf(T.w, P.T_min), P.T_max);
-        rk4_step(P, x, T);
+        const float lo = P.input_model == 1 ? -P.rate_max : P.T_min, hi = P.input_model == 1 ? P.rate_max : P.T_max;
+        T.x = fminf(fmaxf(T.x, lo), hi); T.y = fminf(fmaxf(T.y, lo), hi);
+        T.z = fminf(fmaxf(T.z, lo), hi); T.w = fminf(fmaxf(T.w, lo), hi);
+        if (P.input_model == 1) rk4_rate_step(P, x, Ts, T);
+        else rk4_step(P, x, T);
     }
 }
 

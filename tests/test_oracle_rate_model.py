@@ -138,3 +138,22 @@ def test_stress_case_saturates_thrusts_and_crosses_gates():
     r = O.step(wl.params, O.Track(gates=wl.gates), wl.x0, wl.start, wl.u_nom, wl.seed, 0, want_du=True)
     assert (r["ncross"][0] > 0).sum() >= 20 and (r["ncross"][0] == 0).sum() >= 20
     assert (np.abs(r["du"]) == wl.params["rate_max"]).mean() > 0.05      # rate clamp acts at scale
+
+
+def test_plant_step_and_front_flags_under_the_rate_model():
+    # plant: one rate-model RK4 step with u_new[0], thrust states advance, nominal shifts [R-14]
+    wl = W.rate_gate_paper(K=8, N=6)
+    p = wl.params
+    trk = O.Track(gates=wl.gates)
+    u = np.linspace(-3, 3, 24).reshape(1, 6, 4)
+    x1, s1, un = O.sim_step(p, trk, wl.x0, wl.start, u)
+    np.testing.assert_allclose(x1[0], O.rk4_rate_step(p, wl.x0[0], u[0, 0]), atol=1e-15)
+    np.testing.assert_allclose(x1[0, 13:], wl.x0[0, 13:].astype(np.float64) + p["dt"] * u[0, 0], atol=1e-15)
+    np.testing.assert_array_equal(un[0, :-1], u[0, 1:]); np.testing.assert_array_equal(un[0, -1], u[0, -1])
+    # flags: free fall under the rate model (T = 0, u = 0) against the closed form, as in the thrust model
+    pf = dict(W.base_params(N=40, objective=W.OBJ_GATE_PAPER), input_model=1, rate_max=10.0, T_max=10.0)
+    g = np.array([[0, 0, 1.0, 0, 0, -1, 1, 0, 0, 5, 5]], dtype=np.float64)
+    x0 = np.zeros(17); x0[2] = 2.0; x0[3] = 1.0
+    f, _ = O.front_flags(pf, O.Track(gates=g), x0, 0, np.zeros((40, 4)))
+    k = np.arange(41)
+    np.testing.assert_array_equal(f, (k * pf["dt"] < np.sqrt(2 * 1.0 / pf["g"])).astype(np.int32))

@@ -469,3 +469,42 @@ def test_rate_model_rejects_what_it_does_not_support():
     with pytest.raises(Bd.MppiError) as e:
         Bd.Mppi(W.cfg0().params, drag_x=0.1)                    # drag needs the rate model
     assert e.value.status == -2
+
+
+def test_rate_model_closed_loop_with_flags():
+    # the paper's model + the paper's J_gate in a closed loop: plant step on the 17-entry rows, flags of
+    # the new nominal fed to the next control step; every step teacher-forced against the oracle [R-17]
+    import torch
+    from oracle import oracle as O
+    from paper_2509_14726_b200 import binding as Bd
+    B, K, N = 4, 1024, 30
+    wl = W.rate_gate_paper(K=K, N=N)
+    p = dict(wl.params, B=B)
+    rng = np.random.default_rng(4)
+    x0 = np.repeat(wl.x0, B, 0); x0[:, 0:3] += rng.uniform(-0.2, 0.2, (B, 3)).astype(np.float32)
+    m = Bd.Mppi(p); m.set_gates(wl.gates)
+    x = torch.from_numpy(x0).cuda(); start = torch.zeros(B, dtype=torch.int32, device="cuda")
+    u = torch.from_numpy(np.repeat(wl.u_nom, B, 0)).cuda()
+    front = None
+    for step in range(5):
+        x_in, s_in, u_in = x.cpu().numpy(), start.cpu().numpy(), u.cpu().numpy()
+        m.set_prev_front(front)
+        u_new, cost, w = m.step(x, start, u, 3, step)
+        torch.cuda.synchronize()
+        trk = O.Track(gates=wl.gates, prev_front=None if front is None else front.cpu().numpy())
+        o = O.step(p, trk, x_in, s_in, u_in, 3, step)
+        o["u_nom"] = u_in.astype(np.float64)
+        g = dict(u_new=u_new.cpu().numpy(), cost=cost.cpu().numpy(), weights=w.cpu().numpy())
+        Pz.compare(f"rate loop step{step}", g, o, p["lambda"], True)
+        f = m.front_flags(x, start, u_new); torch.cuda.synchronize()
+        for b in range(B):
+            fo, mg = O.front_flags(p, trk, x_in[b], int(s_in[b]), g["u_new"][b])
+            assert mg < 1e-5 or np.array_equal(f.cpu().numpy()[b], fo), (step, b)
+        xo, so, uo = O.sim_step(p, trk, x_in, s_in, g["u_new"])
+        m.sim_step(x, start, u_new, u_nom_next=u); torch.cuda.synchronize()
+        np.testing.assert_allclose(x.cpu().numpy(), xo, rtol=3e-6, atol=2e-5)
+        np.testing.assert_array_equal(u.cpu().numpy(), uo.astype(np.float32))
+        np.testing.assert_array_equal(start.cpu().numpy(), so)
+        front = torch.cat([f[:, 1:], f[:, -1:]], dim=1).contiguous()
+    assert not np.array_equal(x.cpu().numpy()[:, 13:], x0[:, 13:])      # the thrust states moved
+    m.close()
