@@ -288,6 +288,29 @@ def rate_stress(K=1024, N=30) -> Workload:
     return _rate_model(stress_gate(K=K, N=N), "rate_stress_gate", sigma=_f32(12.0), rate_max=_f32(20.0))
 
 
+def lap(kind="gate", B=8, K=4096, N=50, steps=1500) -> Workload:
+    """Closed-loop lap experiment (shaped like Table II) on the 4-gate
+    circle of configs[0] / its spline path / the Lissajous reference, B jittered drones.  The noise and
+    temperature are the ones a controller can actually fly with -- sigma 0.5 N, lambda 0.02, w_omega
+    0.001: under configs[4]'s sigma 1.5 / lambda 0.5 the closed loop does not stay in the air (measured)."""
+    rng = np.random.default_rng(7)
+    tune = dict(sigma=_f32(0.5), w_omega=_f32(0.001))
+    if kind in ("gate", "gate_paper"):
+        wl = cfg4(K=K, N=N, B=B, steps=steps)
+        p = dict(wl.params, **tune)
+        if kind == "gate_paper":
+            p.update(objective=OBJ_GATE_PAPER, gate_pass_bonus=0.0, gate_miss_penalty=0.0, q_near=_f32(0.5), r_near=_f32(1.5))
+        p["lambda"] = _f32(0.5 if kind == "gate_paper" else 0.02)      # squared distances: larger cost scale
+        return Workload(f"lap_{kind}_B{B}", p, wl.x0, wl.start, wl.u_nom, gates=wl.gates, seed=0, iters=steps)
+    base = cfg2(K=K, N=N, extra_rows=steps + 1) if kind == "track" else cfg3(K=K, N=N)
+    p = dict(base.params, B=B, **tune)
+    p["lambda"] = _f32(0.02 if kind == "contour" else 0.5)
+    x0 = np.repeat(base.x0, B, 0)
+    x0[:, 0:3] += rng.uniform(-0.2, 0.2, (B, 3)).astype(np.float32)
+    return Workload(f"lap_{kind}_B{B}", p, x0.astype(np.float32), np.repeat(base.start, B, 0),
+                    np.repeat(base.u_nom, B, 0), ref=base.ref, path=base.path, closed=base.closed, seed=0, iters=steps)
+
+
 ALL = {"rate_gate_paper": rate_gate_paper, "rate_track": rate_track, "rate_stress": rate_stress,
        "gate_paper": gate_paper, "stress_gate_paper": stress_gate_paper, "cfg0": cfg0, "cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg4": cfg4,
        "stress_gate": stress_gate}

@@ -508,3 +508,40 @@ def test_rate_model_closed_loop_with_flags():
         front = torch.cat([f[:, 1:], f[:, -1:]], dim=1).contiguous()
     assert not np.array_equal(x.cpu().numpy()[:, 13:], x0[:, 13:])      # the thrust states moved
     m.close()
+
+
+# ---- closed-loop lap experiment (paper_2509_14726_b200/closed_loop.py) ---------------
+
+@pytest.mark.parametrize("kind,iters", [("gate", 1), ("gate_paper", 2)])
+def test_lap_experiment_gate_objectives(kind, iters):
+    from paper_2509_14726_b200 import closed_loop as CL
+    wl = W.lap(kind, B=4, K=2048, steps=700)
+    m = Pz.make_ctx(wl)
+    log = CL.fly(m, wl, 700, iters_per_step=iters, prev_front_feedback=(kind == "gate_paper"))
+    m.close()
+    assert np.isfinite(log.x).all()
+    mt = CL.lap_metrics(log, wl.gates, laps=1)
+    G = wl.gates.shape[0]
+    for b, q in enumerate(mt):
+        assert q["flight_time_s"] is not None and q["flight_time_s"] < 14.0, (b, q)     # a lap of 31 m
+        assert q["wp_dist_max"] <= np.hypot(0.75, 0.75) + 1e-6                         # inside the opening
+        assert 2.0 < q["speed_mean"] < 15.0
+        # the device's own gate counter (float32 plant test) agrees with the float64 host replay
+        assert int(log.start[-1, b]) == q["passes"] % G
+
+
+def test_lap_experiment_tracking_and_contouring():
+    from paper_2509_14726_b200 import closed_loop as CL
+    wl = W.lap("track", B=4, K=2048, steps=400)
+    m = Pz.make_ctx(wl)
+    log = CL.fly(m, wl, 400)
+    m.close()
+    assert (CL.tracking_rmse(log, wl.ref) < 0.6).all()
+    np.testing.assert_array_equal(log.start[-1], 400)          # the reference clock advanced one row per step
+    wl = W.lap("contour", B=4, K=2048, steps=400)
+    m = Pz.make_ctx(wl)
+    log = CL.fly(m, wl, 400)
+    m.close()
+    assert (CL.contour_rms(log, wl.path) < 0.3).all()
+    travelled = np.linalg.norm(np.diff(log.x[:, :, 0:3].astype(np.float64), axis=0), axis=-1).sum(0)
+    assert (travelled > 15.0).all()                            # it really flies along the path
