@@ -37,6 +37,7 @@
 #define ORC_OBJ_GATE 0
 #define ORC_OBJ_TRACK 1
 #define ORC_OBJ_CONTOUR 2
+#define ORC_OBJ_CONTOUR_PAPER 4 /* the paper's own J_contour: theta, v_theta states, Delta v_theta sampled, eq.(9) */
 #define ORC_OBJ_GATE_PAPER 3   /* the paper's own J_gate, eq.(6),(7) + temporal check */
 
 typedef struct {
@@ -57,6 +58,11 @@ typedef struct {
     double rate_max;         /* |u_i| <= rate_max, N/s (Table I "Delta T_s [-10,10]") [R-28]            */
     double drag_x, drag_y, drag_z; /* D = diag(.) of eq.(2), body frame, 1/s [R-30]                       */
     double w_limit, omega_max;     /* "external cost" on the body-rate range [R-31]         */
+    /* the paper's own contouring formulation, eq.(9), Table I */
+    double sigma_v;          /* std of the sampled progress acceleration Delta v_theta, m/s^2 [R-35]     */
+    double dv_max;           /* |Delta v_theta| <= dv_max (Table I "[-20,20]")                           */
+    double v_theta_max;      /* 0 <= v_theta <= v_theta_max (eq.(9); Table I "[0,10]")                   */
+    double r_dv;             /* weight of |Delta v_theta|^2                                              */
 } orc_params;
 
 typedef struct {
@@ -68,6 +74,10 @@ typedef struct {
                             unit in-plane axis h(3), half-width along h, half-height along v=h x n */
     const double* ref;   /* [M][13]: p(3), q wxyz(4), v(3), omega(3) */
     const double* pts;   /* [P][3]  */
+    /* ORC_OBJ_CONTOUR_PAPER: the fifth column of the nominal and of the update [R-35] */
+    const double* v_nom;  /* [B][N]  nominal progress accelerations                     (in)          */
+    double* v_new;        /* [B][N]  updated ones, eq.(5) applied to the fifth input     (out)         */
+    double* dv_out;       /* [B][K][N] or NULL: the clamped perturbations actually applied (out)       */
     const int32_t* prev_front; /* [B][N+1] or NULL: ORC_OBJ_GATE_PAPER, state k of the previous control
                             iteration was in front of the start gate (Fig. 2) [R-25] */
 } orc_track;
@@ -496,20 +506,86 @@ double orc_contour_step(const orc_params* P, const orc_track* trk, const double*
 }
 
 /* ------------------------------------------------------------------------------------------
+ * The paper's own contouring formulation, eq.(9): the progress
+ * theta and its speed v_theta are STATES, the progress acceleration Delta v_theta is a fifth sampled
+ * input next to the four thrust rates Delta T (so it needs input_model = 1), and the path is looked
+ * up BY theta instead of searched.  Readings [R-33]..[R-37] of DESIGN.md.
+ * ---------------------------------------------------------------------------------------- */
+/* P(theta) and the unit tangent at theta [R-36]: theta wrapped into [0, L) on a closed path (clamped
+ * to [0, s_last] on an open one); segment i with s_i <= theta < s_{i+1} (the closing segment runs from
+ * the last point to the first, s_P = L); linear interpolation of the points, normalised linear
+ * interpolation of the vertex tangents of [R-22]. */
+void orc_path_eval(const double* pts, const double* s, const double* tan, int32_t Pn, int32_t closed,
+                   double L, double theta, double pos[3], double tg[3])
+{
+    double th = theta;
+    if (closed) { th = fmod(th, L); if (th < 0.0) th += L; }
+    else { if (th < 0.0) th = 0.0; if (th > s[Pn - 1]) th = s[Pn - 1]; }
+    int i = 0;
+    const int last = closed ? Pn - 1 : Pn - 2;
+    while (i < last && s[i + 1] <= th) ++i;
+    const int j = (i + 1) % Pn;
+    const double s1 = (i + 1 < Pn) ? s[i + 1] : L;
+    double lam = (th - s[i]) / (s1 - s[i]);
+    if (lam > 1.0) lam = 1.0;
+    double t[3];
+    for (int a = 0; a < 3; ++a) {
+        pos[a] = (1.0 - lam) * pts[3 * i + a] + lam * pts[3 * j + a];
+        t[a] = (1.0 - lam) * tan[3 * i + a] + lam * tan[3 * j + a];
+    }
+    const double nt = sqrt(dot3(t, t));
+    for (int a = 0; a < 3; ++a) tg[a] = t[a] / nt;
+}
+
+/* the fifth standard normal of a (sample, step): first Box-Muller output of Philox4x32-10 at counter
+ * (k, t + 2^31, iter, b), same key -- a block the four rotor normals never use [R-35] */
+double orc_normal5(uint64_t seed, uint32_t k, uint32_t t, uint32_t iter, uint32_t b)
+{
+    double z[4];
+    orc_normals(seed, k, t + 0x80000000u, iter, b, z);
+    return z[0];
+}
+
+/* stage cost of eq.(9) at a pre-step state [R-37] */
+double orc_contour_paper_stage(const orc_params* P, const orc_track* trk, const double* s, const double* tan,
+                               double L, const double x[19], const double dT[4], double dv)
+{
+    double pos[3], tg[3];
+    orc_path_eval(trk->pts, s, tan, trk->P, trk->closed, L, x[17], pos, tg);
+    const double e[3] = { x[0] - pos[0], x[1] - pos[1], x[2] - pos[2] };
+    const double e_l = dot3(e, tg);
+    double e_c2 = dot3(e, e) - e_l * e_l;
+    if (e_c2 < 0.0) e_c2 = 0.0;
+    double r = 0.0;
+    for (int i = 0; i < 4; ++i) r += dT[i] * dT[i];
+    return P->q_lag * e_l * e_l + P->q_contour * e_c2 + P->w_omega * dot3(x + 10, x + 10)
+         + P->r_dv * dv * dv + P->R * r - P->mu_progress * x[18];
+}
+
+/* progress states over one step with the acceleration held [R-34] */
+void orc_progress_step(const orc_params* P, double theta, double v, double dv, double* theta_n, double* v_n)
+{
+    *theta_n = theta + P->dt * v + 0.5 * P->dt * P->dt * dv;
+    *v_n = fmin(fmax(v + P->dt * dv, 0.0), P->v_theta_max);
+}
+
+/* ------------------------------------------------------------------------------------------
  * One sample: Alg. 1 lines 6-13.  Writes du[N][4] (the clamped
  * perturbation actually rolled out [R-8]) and returns the trajectory cost J.
  * ---------------------------------------------------------------------------------------- */
 typedef struct { const double* s; const double* tan; double L; } orc_path_aux;
 
 double orc_rollout_cost(const orc_params* P, const orc_track* trk, const orc_path_aux* pa,
-                        const double x0[13], int32_t start, const double* u_nom /*[N][4]*/,
+                        const double* x0 /*[13 | 17 | 19]*/, int32_t start, const double* u_nom /*[N][4]*/,
                         uint64_t seed, uint32_t iter, uint32_t k, uint32_t b,
                         double* du /*[N][4]*/, double* margin, int32_t* ncross, int32_t* aux_end,
                         double* x_end /*[13] or NULL*/)
 {
     const int rate = P->input_model == 1;            /* x0 then has 17 entries: ..., T(4) */
-    double x[17];
-    memcpy(x, x0, sizeof(double) * (rate ? 17 : 13));
+    const int cpaper = P->objective == ORC_OBJ_CONTOUR_PAPER;   /* ... and theta, v_theta: 19 [R-33] */
+    const int xdim = cpaper ? 19 : (rate ? 17 : 13);
+    double x[19];
+    memcpy(x, x0, sizeof(double) * xdim);
     int32_t aux = start;
     if (P->objective == ORC_OBJ_GATE_PAPER) { aux = start % trk->G; if (aux < 0) aux += trk->G; }
     const int32_t gate0 = aux;
@@ -544,7 +620,16 @@ double orc_rollout_cost(const orc_params* P, const orc_track* trk, const orc_pat
             }
         }
 
-        double xn[17];
+        double dv = 0.0;
+        if (cpaper) {                             /* fifth sampled input + stage cost of eq.(9) [R-35],[R-37] */
+            const double vn = trk->v_nom[(size_t)b * P->N + t];
+            dv = fmin(fmax(vn + P->sigma_v * orc_normal5(seed, k, (uint32_t)t, iter, b), -P->dv_max), P->dv_max);
+            if (trk->dv_out) trk->dv_out[((size_t)b * P->K + k) * P->N + t] = dv - vn;
+            J += orc_contour_paper_stage(P, trk, pa->s, pa->tan, pa->L, x, T, dv);
+        }
+
+        double xn[19];
+        if (cpaper) orc_progress_step(P, x[17], x[18], dv, &xn[17], &xn[18]);   /* [R-34] */
         if (rate) orc_rk4_rate_step(P, x, T, P->dt, xn);                   /* [R-27],[R-29] */
         else orc_rk4_step(P, x, T, P->dt, xn);                             /* Alg.1 l.7-9 */
         if (rate) J += orc_rate_limit_cost(P, xn + 10);                    /* [R-31] */
@@ -556,7 +641,7 @@ double orc_rollout_cost(const orc_params* P, const orc_track* trk, const orc_pat
             J += orc_gate_paper_step(P, trk, x, xn, xn + 10, &aux, gate0, front_ok, &marg, &nc);
         } else if (P->objective == ORC_OBJ_CONTOUR)
             J += orc_contour_step(P, trk, pa->s, pa->tan, pa->L, xn, xn + 10, &aux, &theta_prev);
-        memcpy(x, xn, sizeof(double) * (rate ? 17 : 13));
+        memcpy(x, xn, sizeof(double) * xdim);
     }
     if (P->objective == ORC_OBJ_TRACK)
         J += orc_track_state_term(P, x, trk->ref + 13 * (start + P->N));   /* eq.(8) terminal */
@@ -564,7 +649,7 @@ double orc_rollout_cost(const orc_params* P, const orc_track* trk, const orc_pat
     if (margin) *margin = marg;
     if (ncross) *ncross = nc;
     if (aux_end) *aux_end = aux;
-    if (x_end) memcpy(x_end, x, sizeof(double) * (rate ? 17 : 13));
+    if (x_end) memcpy(x_end, x, sizeof(double) * xdim);
     return J;
 }
 
@@ -604,7 +689,8 @@ int orc_step(const orc_params* P, const orc_track* trk, const double* x0 /*[B][1
     const int K = P->K, N = P->N, B = P->B;
     orc_path_aux pa = { NULL, NULL, 0.0 };
     double* s = NULL; double* tan = NULL;
-    if (P->objective == ORC_OBJ_CONTOUR) {
+    if (P->objective == ORC_OBJ_CONTOUR_PAPER && (P->input_model != 1 || !trk->v_nom || !trk->v_new)) return -1;
+    if (P->objective == ORC_OBJ_CONTOUR || P->objective == ORC_OBJ_CONTOUR_PAPER) {
         s = (double*)malloc(sizeof(double) * trk->P);
         tan = (double*)malloc(sizeof(double) * 3 * trk->P);
         if (!s || !tan) { free(s); free(tan); return -1; }
@@ -616,6 +702,14 @@ int orc_step(const orc_params* P, const orc_track* trk, const double* x0 /*[B][1
         du_local = (double*)malloc(sizeof(double) * (size_t)K * N * 4);
         if (!du_local) { free(s); free(tan); return -1; }
     }
+    orc_track trk5 = *trk;                       /* the fifth column needs its perturbations for eq.(5) */
+    double* dv_local = NULL;
+    if (P->objective == ORC_OBJ_CONTOUR_PAPER && !trk->dv_out) {
+        dv_local = (double*)malloc(sizeof(double) * (size_t)B * K * N);
+        if (!dv_local) { free(du_local); free(s); free(tan); return -1; }
+        trk5.dv_out = dv_local;
+    }
+    trk = &trk5;
     for (int b = 0; b < B; ++b) {
         double* du = du_out ? du_out + (size_t)b * K * N * 4 : du_local;
         const double* un = u_nom + (size_t)b * N * 4;
@@ -623,7 +717,7 @@ int orc_step(const orc_params* P, const orc_track* trk, const double* x0 /*[B][1
         for (int k = 0; k < K; ++k) {
             double mg; int32_t nc, ae;
             cost[(size_t)b * K + k] =
-                orc_rollout_cost(P, trk, &pa, x0 + (P->input_model == 1 ? 17 : 13) * b, start[b], un, seed, iter, (uint32_t)k,
+                orc_rollout_cost(P, trk, &pa, x0 + (P->objective == ORC_OBJ_CONTOUR_PAPER ? 19 : P->input_model == 1 ? 17 : 13) * b, start[b], un, seed, iter, (uint32_t)k,
                                  (uint32_t)b, du + (size_t)k * N * 4, &mg, &nc, &ae, NULL);
             if (margin) margin[(size_t)b * K + k] = mg;
             if (ncross) ncross[(size_t)b * K + k] = nc;
@@ -631,8 +725,15 @@ int orc_step(const orc_params* P, const orc_track* trk, const double* x0 /*[B][1
         }
         orc_weights_update(K, N, P->lambda, cost + (size_t)b * K, du, un,
                            weights + (size_t)b * K, u_new + (size_t)b * N * 4);
+        if (P->objective == ORC_OBJ_CONTOUR_PAPER)            /* eq.(5) for the fifth input */
+            for (int t = 0; t < N; ++t) {
+                double acc = 0.0;
+                for (int k = 0; k < K; ++k)
+                    acc += weights[(size_t)b * K + k] * trk->dv_out[((size_t)b * K + k) * N + t];
+                trk->v_new[(size_t)b * N + t] = trk->v_nom[(size_t)b * N + t] + acc;
+            }
     }
-    free(du_local); free(s); free(tan);
+    free(du_local); free(dv_local); free(s); free(tan);
     return 0;
 }
 

@@ -18,7 +18,7 @@ _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "mppi_oracle.c"
 _LIB = _HERE / "libmppi_oracle.so"
 
-OBJ_GATE, OBJ_TRACK, OBJ_CONTOUR, OBJ_GATE_PAPER = 0, 1, 2, 3
+OBJ_GATE, OBJ_TRACK, OBJ_CONTOUR, OBJ_GATE_PAPER, OBJ_CONTOUR_PAPER = 0, 1, 2, 3, 4
 
 
 def build(force: bool = False) -> Path:
@@ -45,18 +45,22 @@ class _Params(C.Structure):
                 ("q_near", C.c_double), ("r_near", C.c_double),
                 ("input_model", C.c_int32), ("pad2_", C.c_int32), ("rate_max", C.c_double),
                 ("drag_x", C.c_double), ("drag_y", C.c_double), ("drag_z", C.c_double),
-                ("w_limit", C.c_double), ("omega_max", C.c_double)]
+                ("w_limit", C.c_double), ("omega_max", C.c_double),
+                ("sigma_v", C.c_double), ("dv_max", C.c_double), ("v_theta_max", C.c_double), ("r_dv", C.c_double)]
 
 
 class _Track(C.Structure):
     _fields_ = [("G", C.c_int32), ("M", C.c_int32), ("P", C.c_int32), ("closed", C.c_int32),
                 ("gates", C.POINTER(C.c_double)), ("ref", C.POINTER(C.c_double)),
-                ("pts", C.POINTER(C.c_double)), ("prev_front", C.POINTER(C.c_int32))]
+                ("pts", C.POINTER(C.c_double)), ("v_nom", C.POINTER(C.c_double)),
+                ("v_new", C.POINTER(C.c_double)), ("dv_out", C.POINTER(C.c_double)),
+                ("prev_front", C.POINTER(C.c_int32))]
 
 
 _PARAM_KEYS = [f for f, _ in _Params._fields_ if f not in ("pad_", "pad2_")]
 _OPTIONAL = {"q_near": 0.0, "r_near": 0.0, "input_model": 0, "rate_max": 0.0, "drag_x": 0.0, "drag_y": 0.0,
-             "drag_z": 0.0, "w_limit": 0.0, "omega_max": 0.0}
+             "drag_z": 0.0, "w_limit": 0.0, "omega_max": 0.0, "sigma_v": 0.0, "dv_max": 0.0, "v_theta_max": 0.0,
+             "r_dv": 0.0}
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int32)
 _up = C.POINTER(C.c_uint32)
@@ -79,6 +83,12 @@ def lib():
         L.orc_fdyn.restype = None
         L.orc_rk4_step.argtypes = [C.POINTER(_Params), _dp, _dp, C.c_double, _dp]
         L.orc_rk4_step.restype = None
+        L.orc_path_eval.argtypes = [_dp, _dp, _dp, C.c_int32, C.c_int32, C.c_double, C.c_double, _dp, _dp]
+        L.orc_path_eval.restype = None
+        L.orc_normal5.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32]
+        L.orc_normal5.restype = C.c_double
+        L.orc_progress_step.argtypes = [C.POINTER(_Params), C.c_double, C.c_double, C.c_double, _dp, _dp]
+        L.orc_progress_step.restype = None
         L.orc_rk4_rate_step.argtypes = [C.POINTER(_Params), _dp, _dp, C.c_double, _dp]
         L.orc_rk4_rate_step.restype = None
         L.orc_rate_limit_cost.argtypes = [C.POINTER(_Params), _dp]
@@ -202,6 +212,27 @@ def rk4_step(params, x, T, dt=None):
     return out
 
 
+def path_eval(pts, closed, theta):
+    """[R-36] -> (P(theta), unit tangent at theta, path length L) for a caller-supplied path."""
+    pts = _f64(pts, (-1, 3)); n = pts.shape[0]
+    s = np.zeros(n); tan = np.zeros((n, 3))
+    L = lib().orc_path_prepare(_d(pts), n, 1 if closed else 0, _d(s), _d(tan))
+    pos = np.zeros(3); tg = np.zeros(3)
+    lib().orc_path_eval(_d(pts), _d(s), _d(tan), n, 1 if closed else 0, L, float(theta), _d(pos), _d(tg))
+    return pos, tg, L
+
+
+def normal5(seed, k, t, it, b):
+    return lib().orc_normal5(int(seed), int(k), int(t), int(it), int(b))
+
+
+def progress_step(params, theta, v, dv):
+    P = make_params(params)
+    a = np.zeros(1); b = np.zeros(1)
+    lib().orc_progress_step(C.byref(P), float(theta), float(v), float(dv), _d(a), _d(b))
+    return float(a[0]), float(b[0])
+
+
 def rk4_rate_step(params, x, u, dt=None):
     """One RK4 step of the 17-state thrust-rate model [R-27],[R-29]."""
     P = make_params(params)
@@ -287,12 +318,19 @@ def weights_update(lam, cost, du, u_nom):
     return w, un
 
 
-def step(params, track: Track, x0, start, u_nom, seed, it, want_du=False, want_diag=True):
+def step(params, track: Track, x0, start, u_nom, seed, it, want_du=False, want_diag=True, v_nom=None):
     """One MPPI iteration.  Returns dict(u_new [B,N,4], cost [B,K], weights [B,K],
-    du [B,K,N,4] | None, margin [B,K], ncross [B,K], aux_end [B,K])."""
+    du [B,K,N,4] | None, margin [B,K], ncross [B,K], aux_end [B,K]); under OBJ_CONTOUR_PAPER (v_nom
+    [B,N] required) also v_new [B,N] and dv [B,K,N] | None."""
     P = make_params(params)
     B, K, N = P.B, P.K, P.N
-    x0 = _f64(x0, (B, 17 if P.input_model == 1 else 13)); u_nom = _f64(u_nom, (B, N, 4))
+    xdim = 19 if P.objective == OBJ_CONTOUR_PAPER else (17 if P.input_model == 1 else 13)
+    x0 = _f64(x0, (B, xdim)); u_nom = _f64(u_nom, (B, N, 4))
+    v_new = dv = None
+    if P.objective == OBJ_CONTOUR_PAPER:
+        v_nom = _f64(v_nom, (B, N)); v_new = np.zeros((B, N)); dv = np.zeros((B, K, N)) if want_du else None
+        track.c.v_nom = _d(v_nom); track.c.v_new = _d(v_new)
+        track.c.dv_out = _d(dv) if dv is not None else C.cast(None, _dp)
     start = np.ascontiguousarray(np.asarray(start, dtype=np.int32).reshape(B))
     u_new = np.zeros((B, N, 4)); cost = np.zeros((B, K)); w = np.zeros((B, K))
     du = np.zeros((B, K, N, 4)) if want_du else None
@@ -307,7 +345,7 @@ def step(params, track: Track, x0, start, u_nom, seed, it, want_du=False, want_d
     if rc != 0:
         raise RuntimeError(f"orc_step failed ({rc})")
     return dict(u_new=u_new, cost=cost, weights=w, du=du, margin=margin, ncross=ncross,
-                aux_end=aux_end)
+                aux_end=aux_end, v_new=v_new, dv=dv)
 
 
 def sim_step(params, track: Track, x, start, u_new):

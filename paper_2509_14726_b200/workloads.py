@@ -16,7 +16,7 @@ from dataclasses import dataclass, field
 
 import numpy as np
 
-OBJ_GATE, OBJ_TRACK, OBJ_CONTOUR, OBJ_GATE_PAPER = 0, 1, 2, 3
+OBJ_GATE, OBJ_TRACK, OBJ_CONTOUR, OBJ_GATE_PAPER, OBJ_CONTOUR_PAPER = 0, 1, 2, 3, 4
 
 
 def _f32(v):
@@ -30,7 +30,8 @@ def base_params(**over) -> dict:
              g=9.81, T_min=0.0, T_max=7.0, w_omega=0.01, gate_miss_penalty=10.0,
              gate_pass_bonus=5.0, Qp=100.0, Qv=1.0, Qq=10.0, Qw=0.1, R=0.01, q_contour=200.0,
              q_lag=50.0, mu_progress=2.0, window=16, q_near=0.0, r_near=0.0,
-             input_model=0, rate_max=0.0, drag_x=0.0, drag_y=0.0, drag_z=0.0, w_limit=0.0, omega_max=0.0)
+             input_model=0, rate_max=0.0, drag_x=0.0, drag_y=0.0, drag_z=0.0, w_limit=0.0, omega_max=0.0,
+             sigma_v=0.0, dv_max=0.0, v_theta_max=0.0, r_dv=0.0)
     p["lambda"] = 1.0
     p.update(over)
     for k, v in p.items():
@@ -55,6 +56,7 @@ class Workload:
     ref: np.ndarray | None = None       # [M,13] f32
     path: np.ndarray | None = None      # [P,3] f32
     prev_front: np.ndarray | None = None  # [B,N+1] i32, objective 3 only (None = all in front)
+    v_nom: np.ndarray | None = None     # [B,N] f32, objective 4 only: nominal progress accelerations
     closed: bool = True
     seed: int = 0
     iters: int = 1                      # optimiser iterations (cfg1) or control steps (cfg4)
@@ -288,6 +290,23 @@ def rate_stress(K=1024, N=30) -> Workload:
     return _rate_model(stress_gate(K=K, N=N), "rate_stress_gate", sigma=_f32(12.0), rate_max=_f32(20.0))
 
 
+def contour_paper(K=4096, N=50) -> Workload:
+    """The paper's own contouring formulation (eq.(9)) on configs[3]'s
+    spline path under the paper's input model: states + (theta, v_theta), sampled inputs = four thrust
+    rates + the progress acceleration (sigma_v 5 m/s^2, range +-20, v_theta in [0, 10]: Table I), weights
+    q_c 200, q_l 50, mu 2 (configs[3]), r_dv 0.01, R 0.01 on the rates.  theta_0 = arc length of the path
+    vertex nearest to p_0, v_theta,0 = 2 m/s."""
+    wl = _rate_model(cfg3(K=K, N=N), f"contour_paper_K{K}_N{N}", objective=OBJ_CONTOUR_PAPER, sigma_v=_f32(5.0),
+                     dv_max=_f32(20.0), v_theta_max=_f32(10.0), r_dv=_f32(0.01))
+    pts = wl.path.astype(np.float64)
+    s = np.concatenate([[0.0], np.cumsum(np.linalg.norm(np.diff(pts, axis=0), axis=1))])
+    i = int(np.argmin(np.sum((pts - wl.x0[0, 0:3].astype(np.float64)) ** 2, axis=1)))
+    x0 = np.concatenate([wl.x0, np.array([[s[i], 2.0]], np.float32)], axis=1).astype(np.float32)
+    wl.x0 = x0
+    wl.v_nom = np.zeros((1, N), np.float32)
+    return wl
+
+
 def lap(kind="gate", B=8, K=4096, N=50, steps=1500) -> Workload:
     """Closed-loop lap experiment (shaped like Table II) on the 4-gate
     circle of configs[0] / its spline path / the Lissajous reference, B jittered drones.  The noise and
@@ -311,6 +330,6 @@ def lap(kind="gate", B=8, K=4096, N=50, steps=1500) -> Workload:
                     np.repeat(base.u_nom, B, 0), ref=base.ref, path=base.path, closed=base.closed, seed=0, iters=steps)
 
 
-ALL = {"rate_gate_paper": rate_gate_paper, "rate_track": rate_track, "rate_stress": rate_stress,
+ALL = {"contour_paper": contour_paper, "rate_gate_paper": rate_gate_paper, "rate_track": rate_track, "rate_stress": rate_stress,
        "gate_paper": gate_paper, "stress_gate_paper": stress_gate_paper, "cfg0": cfg0, "cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg4": cfg4,
        "stress_gate": stress_gate}

@@ -111,6 +111,53 @@ def nearest(pts, closed, p, centre, W):
     return int(idx[int(np.argmin(d2))])
 
 
+def path_eval(pts, closed, theta):
+    """P(theta) and unit tangent by linear interpolation over the (closed) polyline, written with
+    searchsorted on an explicitly extended table -- a different route from the oracle's scan."""
+    s, tan, L = path_tables(pts, closed)
+    if closed:
+        th = theta % L
+        se = np.concatenate([s, [L]]); pe = np.vstack([pts, pts[:1]]); te = np.vstack([tan, tan[:1]])
+    else:
+        th = min(max(theta, 0.0), s[-1]); se, pe, te = s, pts, tan
+    i = int(np.searchsorted(se, th, side="right")) - 1
+    i = min(max(i, 0), len(se) - 2)
+    lam = (th - se[i]) / (se[i + 1] - se[i])
+    t = (1 - lam) * te[i] + lam * te[i + 1]
+    return (1 - lam) * pe[i] + lam * pe[i + 1], t / np.linalg.norm(t)
+
+
+def rollout_cost5(P, trk, x0, u_nom, v_nom, seed, it, k, b):
+    """Objective 4 (the paper's eq.(9)): -> (J, du[N,4], dv[N])"""
+    N, h = P["N"], P["dt"]
+    x = np.array(x0, dtype=float)
+    J = 0.0; du = np.zeros((N, 4)); dvs = np.zeros(N)
+    for t in range(N):
+        u = np.clip(u_nom[t] + P["sigma"] * normals(seed, k, t, it, b), -P["rate_max"], P["rate_max"])
+        z5 = normals(seed, k, t + 2 ** 31, it, b)[0]
+        dv = float(np.clip(v_nom[t] + P["sigma_v"] * z5, -P["dv_max"], P["dv_max"]))
+        du[t] = u - u_nom[t]; dvs[t] = dv - v_nom[t]
+        pos, tg = path_eval(trk["path"], trk["closed"], x[17])
+        e = x[0:3] - pos
+        el = e @ tg
+        J += (P["q_lag"] * el ** 2 + P["q_contour"] * max(e @ e - el ** 2, 0.0) + P["w_omega"] * np.sum(x[10:13] ** 2)
+              + P["r_dv"] * dv ** 2 + P["R"] * np.sum(u ** 2) - P["mu_progress"] * x[18])
+        xn = np.empty(19)
+        xn[:17] = rk4_rate(P, x[:17], u)
+        xn[17] = x[17] + h * x[18] + 0.5 * h * h * dv
+        xn[18] = min(max(x[18] + h * dv, 0.0), P["v_theta_max"])
+        J += P["w_limit"] * np.sum(np.maximum(np.abs(xn[10:13]) - P["omega_max"], 0.0) ** 2)
+        x = xn
+    return J, du, dvs
+
+
+def mppi_step5(P, trk, x0, u_nom, v_nom, seed, it, b=0):
+    res = [rollout_cost5(P, trk, x0, u_nom, v_nom, seed, it, k, b) for k in range(P["K"])]
+    J = np.array([r[0] for r in res]); du = np.array([r[1] for r in res]); dv = np.array([r[2] for r in res])
+    w = softmax(-J / P["lambda"])
+    return J, w, u_nom + np.einsum("k,ktn->tn", w, du), v_nom + w @ dv, du, dv
+
+
 def rollout_cost(P, trk, x0, start, u_nom, seed, it, k, b):
     """-> (J, du[N,4], final aux)"""
     N = P["N"]
