@@ -55,9 +55,14 @@ typedef enum {
     MPPI_OBJ_GATE = 0,    /* J_gate,    eq.(6) PAPER.md:105-112 (BASELINE.json configs[0,1,4]) */
     MPPI_OBJ_TRACK = 1,   /* J_track,   eq.(8) PAPER.md:139-147 (configs[2])                   */
     MPPI_OBJ_CONTOUR = 2, /* J_contour, eq.(9) PAPER.md:149-161 (configs[3])                   */
-    MPPI_OBJ_GATE_PAPER = 3 /* the paper's own J_gate: eq.(6),(7) PAPER.md:105-129 with squared distances,
+    MPPI_OBJ_GATE_PAPER = 3, /* the paper's own J_gate: eq.(6),(7) PAPER.md:105-129 with squared distances,
                              the Q_near term and the temporal gate-switching check of Fig. 2
                              (PAPER.md:114-122); tracks are gates; see mppi_set_prev_front          */
+    MPPI_OBJ_CONTOUR_PAPER = 4 /* the paper's own J_contour, eq.(9): the progress theta and
+                             its speed v_theta are STATES (every x / x0 row has 19 entries: ..., T(4),
+                             theta, v_theta), the progress acceleration is a FIFTH sampled input next to
+                             the four thrust rates (so input_model must be 1), the path is looked up by
+                             theta; fused pipeline only; see mppi_set_progress                      */
 } mppi_objective;
 
 typedef enum {
@@ -141,6 +146,10 @@ typedef struct {
     float rate_max;      /* N/s, > 0 when input_model = 1 (Table I: 10)            */
     float drag_x, drag_y, drag_z; /* D = diag(.) of eq.(2)'s rotor drag - R D R^T v, body frame, 1/s,
                           >= 0; input_model = 1 only (the paper prints no value)                  */
+    float sigma_v;       /* MPPI_OBJ_CONTOUR_PAPER: std of the sampled progress acceleration, m/s^2, >= 0    */
+    float dv_max;        /* its range [-dv_max, dv_max], > 0 (Table I: 20)                  */
+    float v_theta_max;   /* 0 <= v_theta <= v_theta_max, > 0 (eq.(9); Table I: 10)                       */
+    float r_dv;          /* weight of |Delta v_theta|^2 in eq.(9), >= 0                                  */
     float w_limit, omega_max; /* input_model = 1: soft body-rate limit ("external cost"):
                           + w_limit sum_i max(0, |omega_i| - omega_max)^2 on every post-step state */
 } mppi_params;
@@ -231,6 +240,14 @@ MPPI_API int mppi_set_prev_front(mppi_ctx* ctx, const int32_t* d_prev_front);
  * [b][k] = 1 iff n.(p_k - c) < 0 for the gate d_start[b] (wrapped mod G).  Needs mppi_set_gates. */
 MPPI_API int mppi_front_flags(mppi_ctx* ctx, const float* d_x0, const int32_t* d_start, const float* d_u,
                      int32_t* d_front_out, void* cuda_stream);
+
+/* MPPI_OBJ_CONTOUR_PAPER: the fifth column of the nominal and of the update.  d_v_nom [B][N] device, in:
+ * nominal progress accelerations; d_v_new [B][N] device, out: v_nom + sum_k w_k dv_k (eq.(5)); the two
+ * may be the same buffer (in-place warm start).  Caller-owned, used by every later mppi_step (which
+ * enqueues a second small kernel for this column) until replaced.  Required before the first step.
+ * mppi_optimize needs the in-place form; mppi_step_host and mppi_sim_step return MPPI_E_PARAM under
+ * this objective. */
+MPPI_API int mppi_set_progress(mppi_ctx* ctx, const float* d_v_nom, float* d_v_new);
 
 /* Device pointer to dU [B][N][K][4] of the last step (parity debugging); NULL unless the
  * context keeps it (TWO_PASS pipeline or store_noise). */

@@ -14,13 +14,13 @@ import numpy as np
 _HERE = Path(__file__).resolve().parent
 LIB_PATH = _HERE / "libmppi.so"
 
-OBJ_GATE, OBJ_TRACK, OBJ_CONTOUR, OBJ_GATE_PAPER = 0, 1, 2, 3
+OBJ_GATE, OBJ_TRACK, OBJ_CONTOUR, OBJ_GATE_PAPER, OBJ_CONTOUR_PAPER = 0, 1, 2, 3, 4
 PIPE_FUSED, PIPE_TWO_PASS = 0, 1
 VARIANT_AUTO, VARIANT_THROUGHPUT, VARIANT_LATENCY, VARIANT_PACKED, VARIANT_PIPELINED = 0, 1, 2, 3, 4
 
 EXPORTS = ["mppi_default_params", "mppi_create", "mppi_destroy", "mppi_set_gates",
            "mppi_set_reference", "mppi_set_path", "mppi_step", "mppi_optimize", "mppi_step_host",
-           "mppi_sim_step", "mppi_set_prev_front", "mppi_front_flags", "mppi_debug_noise", "mppi_get_info", "mppi_launch_count",
+           "mppi_sim_step", "mppi_set_prev_front", "mppi_front_flags", "mppi_set_progress", "mppi_debug_noise", "mppi_get_info", "mppi_launch_count",
            "mppi_error_string", "mppi_last_error", "mppi_measure_fma_peak", "mppi_measure_copy_bw"]
 
 
@@ -39,6 +39,7 @@ class MppiParams(C.Structure):
                 ("store_noise", C.c_int32), ("variant", C.c_int32), ("q_near", C.c_float),
                 ("r_near", C.c_float), ("input_model", C.c_int32), ("rate_max", C.c_float),
                 ("drag_x", C.c_float), ("drag_y", C.c_float), ("drag_z", C.c_float),
+                ("sigma_v", C.c_float), ("dv_max", C.c_float), ("v_theta_max", C.c_float), ("r_dv", C.c_float),
                 ("w_limit", C.c_float), ("omega_max", C.c_float)]
 
 
@@ -68,6 +69,7 @@ def _load():
     L.mppi_optimize.argtypes = [vp, fp, ip, fp, C.c_uint64, C.c_uint32, C.c_int, fp, fp, vp]
     L.mppi_step_host.argtypes = [vp, fp, ip, fp, C.c_uint64, C.c_uint32, fp, fp, fp, vp]
     L.mppi_sim_step.argtypes = [vp, fp, ip, fp, fp, vp]
+    L.mppi_set_progress.argtypes = [vp, fp, fp]
     L.mppi_set_prev_front.argtypes = [vp, ip]
     L.mppi_front_flags.argtypes = [vp, fp, ip, fp, ip, vp]
     L.mppi_debug_noise.argtypes = [vp]
@@ -149,7 +151,8 @@ class Mppi:
             raise MppiError(rc, lib.mppi_last_error(None).decode())
         self._h = h
         self.K, self.N, self.B = self.params.K, self.params.N, self.params.B
-        self.xdim = 17 if self.params.input_model == 1 else 13
+        self._v = None
+        self.xdim = 19 if self.params.objective == OBJ_CONTOUR_PAPER else 17 if self.params.input_model == 1 else 13
 
     # -- lifetime
     def close(self):
@@ -191,6 +194,10 @@ class Mppi:
             self.set_reference(wl.ref)
         if wl.path is not None:
             self.set_path(wl.path, wl.closed)
+        if getattr(wl, "v_nom", None) is not None and self.params.objective == OBJ_CONTOUR_PAPER:
+            import torch
+            v = torch.from_numpy(np.ascontiguousarray(wl.v_nom, dtype=np.float32)).cuda()
+            self.set_progress(v, torch.empty_like(v))
 
     # -- device calls
     @staticmethod
@@ -279,6 +286,14 @@ class Mppi:
                                    self._dev(u_nom_next, (B, N, 4), torch.float32),
                                    _stream_ptr(stream)))
         return x, start, u_nom_next
+
+    def set_progress(self, v_nom, v_new=None):
+        """Objective 4: v_nom / v_new CUDA float32 tensors [B, N] (kept alive here); v_new=None = in place."""
+        import torch
+        v_new = v_nom if v_new is None else v_new
+        self._v = (v_nom, v_new)
+        self._ck(lib.mppi_set_progress(self._h, self._dev(v_nom, (self.B, self.N), torch.float32),
+                                       self._dev(v_new, (self.B, self.N), torch.float32)))
 
     def set_prev_front(self, prev_front):
         """prev_front: CUDA int32 tensor [B, N+1] (kept alive by this object), or None."""

@@ -35,6 +35,7 @@ struct mppi_ctx {
     float* d_partials = nullptr;
     unsigned* d_counters = nullptr;
     const int* d_prev_front = nullptr;     // caller-owned (mppi_set_prev_front)
+    const float* d_v_nom = nullptr; float* d_v_new = nullptr;   // caller-owned (mppi_set_progress)
     // device staging for mppi_step_host
     float* d_hx0 = nullptr; int* d_hstart = nullptr; float* d_hu = nullptr; float* d_hcost = nullptr;
     float* d_hw = nullptr;
@@ -104,6 +105,7 @@ extern "C" int mppi_default_params(mppi_params* p)
     p->q_near = 0.0f; p->r_near = 0.0f;
     p->input_model = 0; p->rate_max = 0.0f; p->drag_x = p->drag_y = p->drag_z = 0.0f;
     p->w_limit = 0.0f; p->omega_max = 0.0f;
+    p->sigma_v = 0.0f; p->dv_max = 0.0f; p->v_theta_max = 0.0f; p->r_dv = 0.0f;
     return MPPI_OK;
 }
 
@@ -116,7 +118,13 @@ static int validate(const mppi_params* p)
     BAD(p->K <= 0 || p->K % 32 != 0, "K must be a positive multiple of 32");
     BAD(p->N <= 0 || p->N > MPPI_MAX_N, "N must be in 1..MPPI_MAX_N");
     BAD(p->B <= 0 || p->B > 65535, "B must be in 1..65535");
-    BAD(p->objective < 0 || p->objective > 3, "objective must be 0..3");
+    BAD(p->objective < 0 || p->objective > 4, "objective must be 0..4");
+    if (p->objective == MPPI_OBJ_CONTOUR_PAPER) {
+        BAD(p->input_model != 1, "MPPI_OBJ_CONTOUR_PAPER needs input_model = 1 (its inputs are thrust rates)");
+        BAD(p->pipeline != MPPI_PIPE_FUSED || p->use_graph, "MPPI_OBJ_CONTOUR_PAPER: fused pipeline, no graph replay");
+        BAD(!(std::isfinite(p->sigma_v) && p->sigma_v >= 0.0f) || !(p->dv_max > 0.0f) || !(p->v_theta_max > 0.0f) ||
+                !(std::isfinite(p->r_dv) && p->r_dv >= 0.0f), "need sigma_v >= 0, dv_max > 0, v_theta_max > 0, r_dv >= 0");
+    }
     BAD(!(std::isfinite(p->q_near) && p->q_near >= 0.0f) || !(std::isfinite(p->r_near) && p->r_near >= 0.0f),
         "q_near and r_near must be >= 0");
     BAD(!finite_pos(p->dt), "dt must be > 0");
@@ -267,6 +275,7 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     d.input_model = p->input_model; d.rate_max = p->rate_max;
     d.drag_x = p->drag_x; d.drag_y = p->drag_y; d.drag_z = p->drag_z;
     d.w_limit = p->w_limit; d.omega_max = p->omega_max;
+    d.sigma_v = p->sigma_v; d.dv_max = p->dv_max; d.v_theta_max = p->v_theta_max; d.r_dv = p->r_dv;
     d.Qp = p->Qp; d.Qv = p->Qv; d.Qq = p->Qq; d.Qw = p->Qw; d.R = p->R;
     d.q_c = p->q_contour; d.q_l = p->q_lag; d.mu = p->mu_progress;
 
@@ -276,7 +285,7 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     cfg.store_du = (!cfg.fused || p->store_noise) ? 1 : 0;
     pick_shape(p, c->sm_count, &cfg.block_threads, &cfg.lat_consumers, &cfg.packed, &cfg.pipe);
     cfg.rate = p->input_model == 1;
-    c->xdim = cfg.rate ? 17 : 13;
+    c->xdim = p->objective == MPPI_OBJ_CONTOUR_PAPER ? 19 : cfg.rate ? 17 : 13;
     d.blocks_per_ctrl = cfg.pipe ? p->K / 32 : cfg.lat_consumers ? p->K / (32 * cfg.lat_consumers)
                                           : p->K / (cfg.block_threads * (cfg.packed ? 2 : 1));
     cfg.smem_bytes = 0;   // fixed once the track is known
@@ -443,8 +452,10 @@ static int prepare(mppi_ctx* c)
 {
     const int obj = c->prm.objective;
     if (((obj == MPPI_OBJ_GATE || obj == MPPI_OBJ_GATE_PAPER) && !c->have_gates) || (obj == MPPI_OBJ_TRACK && !c->have_ref) ||
-        (obj == MPPI_OBJ_CONTOUR && !c->have_path))
+        ((obj == MPPI_OBJ_CONTOUR || obj == MPPI_OBJ_CONTOUR_PAPER) && !c->have_path))
         return fail(c, MPPI_E_NO_TRACK, "mppi_set_gates / mppi_set_reference / mppi_set_path not called for this objective");
+    if (obj == MPPI_OBJ_CONTOUR_PAPER && (!c->d_v_nom || !c->d_v_new))
+        return fail(c, MPPI_E_NO_TRACK, "mppi_set_progress not called (MPPI_OBJ_CONTOUR_PAPER)");
     const size_t need = rollout_smem_bytes(c->dp, c->cfg);
     if (need != c->cfg.smem_bytes) {
         if (need > 227 * 1024) return fail(c, MPPI_E_PARAM, "track + horizon do not fit in shared memory");
@@ -467,7 +478,8 @@ static StepArgs make_args(mppi_ctx* c, const float* x0, const int32_t* start, co
     StepArgs a;
     a.x0 = x0; a.start = start; a.u_nom = u_nom; a.u_new = u_new; a.cost = cost; a.weights = w;
     a.du = c->d_du; a.partials = c->d_partials; a.counters = c->d_counters;
-    a.prev_front = c->d_prev_front; a.done_flag = nullptr; a.done_value = 0;
+    a.prev_front = c->d_prev_front; a.v_nom = c->d_v_nom; a.v_new = c->d_v_new;
+    a.done_flag = nullptr; a.done_value = 0;
     a.seed_lo = (uint32_t)(seed & 0xffffffffu); a.seed_hi = (uint32_t)(seed >> 32); a.iter = iter;
     for (uint32_t r = 0; r < 10; ++r) {          // Philox key schedule (Weyl sequence), hoisted out of the kernel
         a.rk[2 * r] = a.seed_lo + r * 0x9E3779B9u;
@@ -479,7 +491,7 @@ static StepArgs make_args(mppi_ctx* c, const float* x0, const int32_t* start, co
 static int enqueue_iteration(mppi_ctx* c, const StepArgs& a, cudaStream_t s)
 {
     CK(c, launch_rollout(c->dp, a, c->cfg, s));
-    c->launches += 1;
+    c->launches += c->prm.objective == MPPI_OBJ_CONTOUR_PAPER ? 2 : 1;
     if (!c->cfg.fused) {
         CK(c, launch_reduce(c->dp, a, s));
         c->launches += 1;
@@ -567,6 +579,8 @@ extern "C" int mppi_optimize(mppi_ctx* c, const float* d_x0, const int32_t* d_st
     if (!d_x0 || !d_start || !d_u || !d_cost || !d_weights)
         return fail(c, MPPI_E_NULL, "mppi_optimize: NULL device pointer");
     if (n_iters < 1 || n_iters > 1024) return fail(c, MPPI_E_RANGE, "n_iters must be in 1..1024");
+    if (c->prm.objective == MPPI_OBJ_CONTOUR_PAPER && c->d_v_nom != c->d_v_new)
+        return fail(c, MPPI_E_RANGE, "mppi_optimize under MPPI_OBJ_CONTOUR_PAPER needs mppi_set_progress(v, v) (in place)");
     int rc = prepare(c);
     if (rc) return rc;
     std::vector<StepArgs> args;
@@ -586,6 +600,8 @@ extern "C" int mppi_step_host(mppi_ctx* c, const float* h_x0, const int32_t* h_s
 {
     if (!c) return MPPI_E_NULL;
     if (!h_x0 || !h_start || !h_u_nom || !h_u_new) return fail(c, MPPI_E_NULL, "mppi_step_host: NULL host pointer");
+    if (c->prm.objective == MPPI_OBJ_CONTOUR_PAPER)
+        return fail(c, MPPI_E_PARAM, "mppi_step_host: not available for MPPI_OBJ_CONTOUR_PAPER (its progress column lives on the device)");
     cudaStream_t s = (cudaStream_t)stream;
     const size_t B = c->prm.B, N = c->prm.N, K = c->prm.K;
     if (c->h_pin) {
@@ -645,6 +661,8 @@ extern "C" int mppi_sim_step(mppi_ctx* c, float* d_x, int32_t* d_start, const fl
 {
     if (!c) return MPPI_E_NULL;
     if (!d_x || !d_start || !d_u_new || !d_u_nom_next) return fail(c, MPPI_E_NULL, "mppi_sim_step: NULL device pointer");
+    if (c->prm.objective == MPPI_OBJ_CONTOUR_PAPER)
+        return fail(c, MPPI_E_PARAM, "mppi_sim_step: not available for MPPI_OBJ_CONTOUR_PAPER yet (the progress states have no plant)");
     const size_t ub = (size_t)c->prm.B * c->prm.N * 4 * sizeof(float);
     if (d_u_nom_next != d_u_new && overlaps(d_u_nom_next, ub, d_u_new, ub))
         return fail(c, MPPI_E_RANGE, "d_u_nom_next partially overlaps d_u_new");
@@ -652,6 +670,16 @@ extern "C" int mppi_sim_step(mppi_ctx* c, float* d_x, int32_t* d_start, const fl
     if (rc) return rc;
     CK(c, launch_sim(c->dp, c->prm.objective, d_x, d_start, d_u_new, d_u_nom_next, (cudaStream_t)stream));
     c->launches += 1;
+    return MPPI_OK;
+}
+
+extern "C" int mppi_set_progress(mppi_ctx* c, const float* d_v_nom, float* d_v_new)
+{
+    if (!c) return MPPI_E_NULL;
+    if (c->prm.objective != MPPI_OBJ_CONTOUR_PAPER)
+        return fail(c, MPPI_E_PARAM, "mppi_set_progress: the objective is not MPPI_OBJ_CONTOUR_PAPER");
+    if (!d_v_nom || !d_v_new) return fail(c, MPPI_E_NULL, "mppi_set_progress: NULL device pointer");
+    c->d_v_nom = d_v_nom; c->d_v_new = d_v_new;
     return MPPI_OK;
 }
 
@@ -699,7 +727,7 @@ extern "C" int mppi_get_info(mppi_ctx* c, mppi_info* o)
     o->local_bytes_per_thread = (int32_t)fa.localSizeBytes;
     o->max_blocks_per_sm = nb;
     o->sm_count = c->sm_count;
-    o->kernels_per_step = c->cfg.fused ? 1 : 2;
+    o->kernels_per_step = (c->cfg.fused ? 1 : 2) + (c->prm.objective == MPPI_OBJ_CONTOUR_PAPER ? 1 : 0);
     o->samples_per_thread = c->cfg.packed ? 2 : 1;
     o->rollout_warps_per_block = c->cfg.pipe ? 3 : c->cfg.lat_consumers ? c->cfg.lat_consumers : c->cfg.block_threads / 32;
     o->l2_bytes = c->l2_bytes;

@@ -5,7 +5,7 @@
 
 namespace mppi {
 
-enum { OBJ_GATE = 0, OBJ_TRACK = 1, OBJ_CONTOUR = 2, OBJ_GATE_PAPER = 3 };
+enum { OBJ_GATE = 0, OBJ_TRACK = 1, OBJ_CONTOUR = 2, OBJ_GATE_PAPER = 3, OBJ_CONTOUR_PAPER = 4 };
 
 // ---- gate progress: eq.(6) PAPER.md:105-110 with un-squared distances [D-2], in-horizon target
 // switching PAPER.md:112, geometric pass test [R-9],[R-10]; constants BASELINE.json configs[0].

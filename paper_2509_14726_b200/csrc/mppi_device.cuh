@@ -24,6 +24,7 @@ struct DevParams {
     // the paper's own input model (Table I) [R-27]..[R-32]: u = dT/dt, thrusts are states
     int input_model;
     float rate_max, drag_x, drag_y, drag_z, w_limit, omega_max;
+    float sigma_v, dv_max, v_theta_max, r_dv;   // the paper's own contouring, eq.(9) [R-33]..[R-37]
     float Qp, Qv, Qq, Qw, R;           // eq.(8)
     float q_c, q_l, mu, path_L, inv_path_L; // eq.(9) + closed path length
     const float4* gates;               // [G][4]: (c, a_h) (n, a_v) (h, 0) (v = h x n, 0)
@@ -42,6 +43,8 @@ struct StepArgs {
     float4* du;            // [B][N][K] float4 or nullptr
     float* partials;       // [B][blocks_per_ctrl][4N+4]  (fused pipeline)
     unsigned int* counters;// [B + 1]: last-block tickets per controller, finished controllers (fused pipeline)
+    const float* v_nom;    // [B][N] nominal progress accelerations (OBJ_CONTOUR_PAPER), or nullptr
+    float* v_new;          // [B][N] updated ones
     const int* prev_front; // [B][N+1] or nullptr: previous-iteration "in front" flags (paper's J_gate, Fig. 2)
     unsigned int* done_flag;   // mapped host word, or nullptr: set to done_value once every output of the
     unsigned int done_value;   // call is visible to the host (mppi_step_host polls it instead of a stream sync)

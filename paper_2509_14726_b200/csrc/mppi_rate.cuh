@@ -94,4 +94,61 @@ __device__ __forceinline__ float rate_limit_cost(const DevParams& P, const State
     return P.w_limit * fmaf(ez, ez, fmaf(ey, ey, ex * ex));
 }
 
+// ---- the paper's own contouring formulation, eq.(9) PAPER.md:149-161 ----------------
+// P(theta) and the unit tangent at theta from the path in shared memory ((P_i, s_i), (t_i, 0)) [R-36]:
+// theta wrapped into [0, L) on a closed path (clamped on an open one); the segment is found from the
+// uniform-spacing guess theta P / L and corrected by stepping (the arc lengths are cumulative chord
+// lengths, only nearly uniform); linear interpolation of the points, normalised linear interpolation
+// of the vertex tangents.
+__device__ __forceinline__ void path_eval(const DevParams& P, const float4* s_path, const float theta,
+                                          float& px, float& py, float& pz, float& tx, float& ty, float& tz)
+{
+    const int n = P.P;
+    float th = theta;
+    if (P.closed) { th = fmaf(-P.path_L, floorf(th * P.inv_path_L), th); if (th >= P.path_L) th = 0.0f; if (th < 0.0f) th = 0.0f; }
+    else th = fminf(fmaxf(th, 0.0f), s_path[2 * (n - 1)].w);
+    const int last = P.closed ? n - 1 : n - 2;
+    int i = min(max((int)(th * P.inv_path_L * (float)n), 0), last);
+    while (i > 0 && s_path[2 * i].w > th) --i;
+    while (i < last && s_path[2 * (i + 1)].w <= th) ++i;
+    const int j = (i + 1 == n) ? 0 : i + 1;
+    const float4 a = s_path[2 * i], b = s_path[2 * j], ta = s_path[2 * i + 1], tb = s_path[2 * j + 1];
+    const float s1 = (i + 1 < n) ? b.w : P.path_L;
+    const float lam = fminf((th - a.w) / (s1 - a.w), 1.0f), mu = 1.0f - lam;
+    px = fmaf(lam, b.x, mu * a.x); py = fmaf(lam, b.y, mu * a.y); pz = fmaf(lam, b.z, mu * a.z);
+    const float ux = fmaf(lam, tb.x, mu * ta.x), uy = fmaf(lam, tb.y, mu * ta.y), uz = fmaf(lam, tb.z, mu * ta.z);
+    const float inv = rsqrtf(fmaf(uz, uz, fmaf(uy, uy, ux * ux)));
+    tx = ux * inv; ty = uy * inv; tz = uz * inv;
+}
+
+// the fifth sampled input [R-35]: dv = clamp(v_nom + sigma_v z5, -dv_max, dv_max), z5 = first Box-Muller
+// output of the Philox block at counter (k, t + 2^31, iter, b)
+template <int MATH>
+__device__ __forceinline__ float sample_progress_accel(const DevParams& P, const uint32_t (&rk)[20], uint32_t k,
+                                                       uint32_t t, uint32_t iter, uint32_t b, const float vn)
+{
+    const uint4 r = philox4x32_10(k, t + 0x80000000u, iter, b, rk);
+    float a, unused;
+    perturb_pair<MATH>(r.x, r.y, P.sigma_v, vn, 0.0f, a, unused);
+    return fminf(fmaxf(a, -P.dv_max), P.dv_max);
+}
+
+// stage cost of eq.(9) at a pre-step state [R-37]
+__device__ __forceinline__ float contour_paper_stage(const DevParams& P, const float4* s_path, const State& x,
+                                                     const float theta, const float v_theta, const float4 dT,
+                                                     const float dv)
+{
+    float px, py, pz, tx, ty, tz;
+    path_eval(P, s_path, theta, px, py, pz, tx, ty, tz);
+    const float ex = x.px - px, ey = x.py - py, ez = x.pz - pz;
+    const float e_l = fmaf(ez, tz, fmaf(ey, ty, ex * tx));
+    const float e_c2 = fmaxf(fmaf(ez, ez, fmaf(ey, ey, ex * ex)) - e_l * e_l, 0.0f);
+    float J = P.q_l * e_l * e_l;
+    J = fmaf(P.q_c, e_c2, J);
+    J = fmaf(P.w_omega, fmaf(x.oz, x.oz, fmaf(x.oy, x.oy, x.ox * x.ox)), J);
+    J = fmaf(P.r_dv, dv * dv, J);
+    J = fmaf(P.R, fmaf(dT.w, dT.w, fmaf(dT.z, dT.z, fmaf(dT.y, dT.y, dT.x * dT.x))), J);
+    return fmaf(-P.mu, v_theta, J);
+}
+
 }  // namespace mppi

@@ -55,7 +55,7 @@ __host__ __device__ inline int track_f4(const DevParams& P, int objective)
 {
     return objective == OBJ_GATE ? 4 * P.G
          : objective == OBJ_GATE_PAPER ? 4 * P.G + (P.N + 4) / 4      // gates + N+1 previous-iteration flags
-         : objective == OBJ_TRACK ? 4 * (P.N + 1) : 2 * P.P;
+         : objective == OBJ_TRACK ? 4 * (P.N + 1) : 2 * P.P;          // both contouring forms stage the path
 }
 
 // Stage the nominal sequence of controller b and the objective's track data in shared memory.

@@ -41,21 +41,27 @@ def gpu_step(m, x0, start, u_nom, seed, it, **kw):
     import torch
     u_new, cost, w = m.step(x0, start, u_nom, seed, it, **kw)
     torch.cuda.synchronize()
-    return dict(u_new=u_new.cpu().numpy(), cost=cost.cpu().numpy(), weights=w.cpu().numpy())
+    r = dict(u_new=u_new.cpu().numpy(), cost=cost.cpu().numpy(), weights=w.cpu().numpy())
+    if getattr(m, "_v", None) is not None:
+        r["v_new"] = m._v[1].cpu().numpy()
+    return r
 
 
-def oracle_step(wl, x0, start, u_nom, seed, it, want_du=False, params=None):
+def oracle_step(wl, x0, start, u_nom, seed, it, want_du=False, params=None, v_nom=None):
     from oracle import oracle as O
     return O.step(params or wl.params, oracle_track(wl), np.asarray(x0, np.float64),
-                  np.asarray(start, np.int32), np.asarray(u_nom, np.float64), seed, it, want_du=want_du)
+                  np.asarray(start, np.int32), np.asarray(u_nom, np.float64), seed, it, want_du=want_du,
+                  v_nom=None if v_nom is None else np.asarray(v_nom, np.float64))
 
 
-def compare(tag, g, o, lam, gate_objective):
-    """Asserts parity of one iteration; returns a small stats dict."""
+def compare(tag, g, o, lam, gate_objective, cost_floor=1.0):
+    """Asserts parity of one iteration; returns a small stats dict.  cost_floor: the smallest magnitude
+    the cost error is measured against (1 by [R-20]; objective 4 passes the size of the progress reward
+    its positive terms cancel against [R-38])."""
     Jg, Jo = g["cost"].astype(np.float64), o["cost"]
     assert np.isfinite(Jg).all(), f"{tag}: non-finite GPU cost"
     flagged = (o["margin"] < MARGIN) if gate_objective else np.zeros_like(Jo, dtype=bool)
-    err = np.abs(Jg - Jo) / np.maximum(np.abs(Jo), 1.0)
+    err = np.abs(Jg - Jo) / np.maximum(np.abs(Jo), cost_floor)
     ok = err <= COST_RTOL
     n_flag = int(flagged.sum())
     assert ok[~flagged].all(), (f"{tag}: {int((~ok & ~flagged).sum())} costs out of tolerance, worst rel "

@@ -63,7 +63,7 @@ def test_default_params_are_config0(B):
 
 
 @pytest.mark.parametrize("field,value", [("K", 0), ("K", 100), ("N", 0), ("N", 257), ("B", 0),
-                                         ("objective", 4), ("q_near", -1.0), ("r_near", float("nan")), ("dt", 0.0), ("lambda_", 0.0), ("lambda_", -1.0),
+                                         ("objective", 5), ("objective", 4), ("q_near", -1.0), ("r_near", float("nan")), ("dt", 0.0), ("lambda_", 0.0), ("lambda_", -1.0),
                                          ("sigma", -0.1), ("mass", 0.0), ("Jz", -1.0), ("T_min", 8.0),
                                          ("window", 0), ("window", 65), ("pipeline", 2),
                                          ("block_threads", 48), ("block_threads", 512), ("dt", float("nan"))])

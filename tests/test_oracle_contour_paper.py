@@ -74,9 +74,14 @@ def test_clamps_of_the_fifth_input_enter_the_update():
     assert r["weights"][0, k] == r["weights"][0].max()
 
 
-@pytest.mark.parametrize("kw", [dict(K=6, N=12), dict(K=4, N=40)])
-def test_brute_force_definition(kw):
+@pytest.mark.parametrize("kw,closed", [(dict(K=6, N=12), True), (dict(K=4, N=40), True), (dict(K=5, N=30), False)])
+def test_brute_force_definition(kw, closed):
     wl = W.contour_paper(**kw)
+    wl.v_nom = np.random.default_rng(3).uniform(-4, 4, wl.v_nom.shape).astype(np.float32)
+    if not closed:                       # open form, theta_0 just before the end at the upper speed limit
+        wl.closed = 0
+        L = float(np.linalg.norm(np.diff(wl.path.astype(np.float64), axis=0), axis=1).sum())
+        wl.x0[0, 17:19] = np.float32([L - 0.2, 10.0]); wl.x0[0, 0:3] = wl.path[-3]
     r = O.step(wl.params, O.Track(path=wl.path, closed=wl.closed), wl.x0, wl.start, wl.u_nom, 11, 3,
                want_du=True, v_nom=wl.v_nom)
     J, w, un, vn, du, dv = D.mppi_step5(wl.params, dict(path=wl.path.astype(np.float64), closed=wl.closed),

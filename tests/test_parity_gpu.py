@@ -510,6 +510,117 @@ def test_rate_model_closed_loop_with_flags():
     m.close()
 
 
+# ---- the paper's own contouring formulation (objective 4; readings R-33..R-37) --------
+
+V_ATOL = 1e-4        # m/s^2 on the fifth column of the update: north_star's u_new bound carried over
+
+
+def _cp_check(tag, wl, g, o):
+    # [R-38] eq.(9) sums a reward -mu v_theta against positive error terms: J can cancel to ~0 while both
+    # parts are ~ mu v_theta_max N; the fp32 error scales with the parts, so that is the floor of the bound
+    floor = max(1.0, float(wl.params["mu_progress"]) * float(wl.params["v_theta_max"]) * wl.params["N"])
+    st = Pz.compare(tag, g, o, wl.params["lambda"], False, cost_floor=floor)
+    verr = float(np.abs(g["v_new"].astype(np.float64) - o["v_new"]).max())
+    Pz.STATS.append(f"{tag}: v_new {verr:.2e}")
+    if verr > V_ATOL:
+        # as for u_new in parity.compare: allowed only where fp32 cannot resolve the weights (a "reported
+        # separately" line exists for this tag); the column must then be the exact update of the GPU's weights
+        assert any(r.startswith(tag + ": near-tied") for r in Pz.REPORT), f"{tag}: v_new err {verr:.3e}"
+        v_self = o["v_nom"] + np.einsum("bk,bkt->bt", g["weights"].astype(np.float64), o["dv"])
+        assert np.abs(g["v_new"] - v_self).max() <= V_ATOL, f"{tag}: v_new inconsistent with its weights"
+    return st
+
+
+@pytest.mark.parametrize("pipe", [dict(), dict(variant=1, block_threads=64), dict(variant=1, block_threads=256)],
+                         ids=["fused", "fused_tpb64", "fused_tpb256"])
+@pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
+@pytest.mark.parametrize("regime", [dict(), {"sigma": np.float32(2.0), "lambda": np.float32(1000.0)}], ids=["argmin", "mixing"])
+def test_contour_paper_full_size(pipe, math, regime):
+    # "argmin": the workload as it stands -- like the paper's lambda = 0.01 (Table I) the softmax picks one
+    # sample (ESS 1); "mixing": a temperature at the scale of the cost spread, so that the weights and
+    # both updates average over tens of samples
+    wl = W.contour_paper()
+    wl.params.update(regime)
+    rng = np.random.default_rng(5)
+    wl.v_nom = rng.uniform(-3, 3, wl.v_nom.shape).astype(np.float32)       # a non-trivial nominal fifth column
+    m = Pz.make_ctx(wl, **pipe, **math)
+    x0, start, u = Pz.to_dev(wl)
+    g = Pz.gpu_step(m, x0, start, u, wl.seed, 0)
+    o = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, wl.seed, 0, want_du=True, v_nom=wl.v_nom)
+    o["u_nom"] = wl.u_nom.astype(np.float64); o["v_nom"] = wl.v_nom.astype(np.float64)
+    st = _cp_check(f"contour_paper[{pipe},{math},{sorted(regime)}]", wl, g, o)
+    assert (st["ess"] > 10) == bool(regime)
+    assert (np.abs(o["dv"] + wl.v_nom[:, None, :] ) == wl.params["dv_max"]).any()      # the fifth input's clamp acts
+    assert np.abs(o["v_new"] - wl.v_nom).max() > 0.05                                  # and the update moves it
+    m.close()
+
+
+def test_contour_paper_batch_warm_start_open_path_and_speed_limits():
+    # B = 3 on the OPEN form of the path, theta_0 near both ends and v_theta,0 at both limits, four
+    # warm-started iterations in place (u and v); teacher-forced against the oracle [R-17]
+    import torch
+    wl = W.contour_paper(K=1024, N=40)
+    B = 3
+    wl.closed = 0
+    wl.params = dict(wl.params, B=B, sigma=np.float32(2.0))
+    wl.params["lambda"] = np.float32(300.0)                      # mixing regime: ESS 15..70 over the four iterations
+    L = float(np.linalg.norm(np.diff(wl.path.astype(np.float64), axis=0), axis=1).sum())
+    wl.x0 = np.repeat(wl.x0, B, 0)
+    wl.x0[1, 17:19] = np.float32([L - 0.3, 10.0]); wl.x0[1, 0:3] = wl.path[-2]
+    wl.x0[2, 17:19] = np.float32([0.05, 0.0]); wl.x0[2, 0:3] = wl.path[0] + np.float32([0.1, 0.0, -0.1])
+    wl.start = np.repeat(wl.start, B, 0); wl.u_nom = np.repeat(wl.u_nom, B, 0)
+    wl.v_nom = np.repeat(wl.v_nom, B, 0)
+    m = Pz.make_ctx(wl)
+    x0, start, u = Pz.to_dev(wl)
+    v = torch.from_numpy(wl.v_nom.copy()).cuda()
+    m.set_progress(v)                                            # in place
+    for it in range(4):
+        u_in, v_in = u.cpu().numpy(), v.cpu().numpy()
+        g = Pz.gpu_step(m, x0, start, u, wl.seed, it, u_new=u)
+        o = Pz.oracle_step(wl, wl.x0, wl.start, u_in, wl.seed, it, want_du=True, v_nom=v_in)
+        o["u_nom"] = u_in.astype(np.float64); o["v_nom"] = v_in.astype(np.float64)
+        assert _cp_check(f"contour_paper open it{it}", wl, g, o)["ess"] > 10
+    assert np.abs(v.cpu().numpy()).max() > 0.1
+    # mppi_optimize runs the same four iterations in one call
+    u2 = torch.from_numpy(wl.u_nom.copy()).cuda(); v2 = torch.from_numpy(wl.v_nom.copy()).cuda()
+    m.set_progress(v2)
+    m.optimize(x0, start, u2, wl.seed, 0, 4); torch.cuda.synchronize()
+    np.testing.assert_array_equal(u2.cpu().numpy(), u.cpu().numpy())
+    np.testing.assert_array_equal(v2.cpu().numpy(), v.cpu().numpy())
+    assert m.info()["kernels_per_step"] == 2
+    m.close()
+
+
+def test_contour_paper_rejects_what_it_does_not_support():
+    import torch
+    from paper_2509_14726_b200 import binding as Bd
+    wl = W.contour_paper(K=64, N=8)
+    for bad in (dict(input_model=0, drag_x=0.0, drag_y=0.0, drag_z=0.0, w_limit=0.0), dict(pipeline=1), dict(use_graph=1),
+                dict(dv_max=0.0), dict(v_theta_max=0.0), dict(sigma_v=-1.0), dict(r_dv=-1.0)):
+        with pytest.raises(Bd.MppiError) as e:
+            Bd.Mppi(wl.params, **bad)
+        assert e.value.status == -2, bad
+    m = Bd.Mppi(wl.params); m.set_path(wl.path, wl.closed)
+    x0, start, u = Pz.to_dev(wl)
+    with pytest.raises(Bd.MppiError) as e:
+        m.step(x0, start, u, 1, 0)                              # mppi_set_progress not called
+    assert e.value.status == -3
+    v = torch.zeros((1, 8), device="cuda")
+    m.set_progress(v, torch.empty_like(v))
+    with pytest.raises(Bd.MppiError) as e:
+        m.optimize(x0, start, u, 1, 0, 2)                       # needs the in-place form
+    assert e.value.status == -5
+    with pytest.raises(Bd.MppiError) as e:
+        m.step_host(wl.x0, wl.start, wl.u_nom, 1, 0)
+    assert e.value.status == -2
+    m.close()
+    m = Bd.Mppi(W.cfg3().params)
+    with pytest.raises(Bd.MppiError) as e:
+        m.set_progress(torch.zeros((1, 50), device="cuda"))    # another objective
+    assert e.value.status == -2
+    m.close()
+
+
 # ---- closed-loop lap experiment (paper_2509_14726_b200/closed_loop.py) ---------------
 
 @pytest.mark.parametrize("kind,iters", [("gate", 1), ("gate_paper", 2)])
