@@ -12,6 +12,9 @@ outside the events).  Rank 0 prints ONE JSON line.  Multi-GPU: the path does not
 (north_star: one GPU, no collectives) -> N independent replicas, value = N * units / max time.
 
 --impl reference times the float64 CPU oracle (oracle/) as it stands on the host cores.
+--survey (one GPU) times one iteration of EVERY workload of workloads.py -- the five configs, the
+paper's own J_gate, input model and contouring -- for one controller and for 64, and prints a table
+(not the JSON line; DESIGN.md section 7 quotes it).
 """
 from __future__ import annotations
 
@@ -385,6 +388,48 @@ def run_ours(args):
     return 0
 
 
+def run_survey(args):
+    """One iteration of every workload, alone and x64: device time per iteration (CUDA events, L2 flushed
+    between iterations), sample-steps/s, the kernel that ran.  Prints a markdown table."""
+    import torch
+    from paper_2509_14726_b200 import binding as Bd
+    from paper_2509_14726_b200 import workloads as W
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --survey: no CUDA device")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    flush_buf = torch.empty(L2_FLUSH_BYTES // 4, dtype=torch.float32, device=dev)
+    names = ["cfg0", "cfg1", "cfg2", "cfg3", "gate_paper", "rate_gate_paper", "rate_track", "contour_paper"]
+    print("| workload | objective | input model | K | N | B | kernel | launches / iteration | us / iteration | sample-steps/s |")
+    print("|---|---|---|---|---|---|---|---|---|---|")
+    for name in names:
+        for B in (1, 64):
+            wl = W.ALL[name]()
+            if B > 1:
+                wl = W.replicate(wl, B, 0.3)
+            P = wl.params
+            m = Bd.Mppi(P, fast_math=args.fast_math)
+            m.set_track(wl)
+            x0 = torch.from_numpy(wl.x0).to(dev); start = torch.from_numpy(wl.start).to(dev)
+            u = torch.from_numpy(wl.u_nom).to(dev); un = torch.empty_like(u)
+            cost = torch.empty((P["B"], P["K"]), device=dev); w = torch.empty_like(cost)
+            it = [0]
+
+            def step():
+                m.step(x0, start, u, wl.seed, it[0], u_new=un, cost=cost, weights=w); it[0] += 1
+            ms = time_steps(step, lambda: flush_buf.fill_(float(it[0] & 7)), 40 if B > 1 else 200, 5)
+            info = m.info()
+            k = ("rate-model scalar" if P.get("input_model", 0) == 1 else
+                 "pipelined" if info["rollout_warps_per_block"] == 3 and info["block_threads"] == 256 else
+                 "packed fp32x2" if info["samples_per_thread"] == 2 else "scalar")
+            units = P["K"] * P["N"] * P["B"]
+            print(f"| {name} | {P['objective']} | {P.get('input_model', 0)} | {P['K']} | {P['N']} | {P['B']} | {k} "
+                  f"({info['block_threads']} thr x {info['grid_blocks']} blocks, {info['regs_per_thread']} regs) | "
+                  f"{info['kernels_per_step']} | {float(np.median(ms)) * 1e3:.1f} | {units / (float(ms.mean()) * 1e-3):.3g} |", flush=True)
+            m.close()
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -395,7 +440,10 @@ def main(argv=None):
     ap.add_argument("--fast-math", dest="fast_math", type=int, default=1)
     ap.add_argument("--graph", type=int, default=0)
     ap.add_argument("--cpu-budget", dest="cpu_budget", type=float, default=10.0)
+    ap.add_argument("--survey", action="store_true", help="time one iteration of every workload (table, one GPU)")
     args = ap.parse_args(argv)
+    if args.survey:
+        return run_survey(args)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)

@@ -243,8 +243,8 @@ MPPI_API int mppi_front_flags(mppi_ctx* ctx, const float* d_x0, const int32_t* d
 
 /* MPPI_OBJ_CONTOUR_PAPER: the fifth column of the nominal and of the update.  d_v_nom [B][N] device, in:
  * nominal progress accelerations; d_v_new [B][N] device, out: v_nom + sum_k w_k dv_k (eq.(5)); the two
- * may be the same buffer (in-place warm start).  Caller-owned, used by every later mppi_step (which
- * enqueues a second small kernel for this column) until replaced.  Required before the first step.
+ * may be the same buffer (in-place warm start).  Caller-owned, used by every later mppi_step (the fused
+ * update writes this column in the same launch) until replaced.  Required before the first step.
  * mppi_optimize needs the in-place form; mppi_step_host and mppi_sim_step return MPPI_E_PARAM under
  * this objective. */
 MPPI_API int mppi_set_progress(mppi_ctx* ctx, const float* d_v_nom, float* d_v_new);

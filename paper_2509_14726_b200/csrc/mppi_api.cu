@@ -288,6 +288,7 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     c->xdim = p->objective == MPPI_OBJ_CONTOUR_PAPER ? 19 : cfg.rate ? 17 : 13;
     d.blocks_per_ctrl = cfg.pipe ? p->K / 32 : cfg.lat_consumers ? p->K / (32 * cfg.lat_consumers)
                                           : p->K / (cfg.block_threads * (cfg.packed ? 2 : 1));
+    d.part_stride = 4 * p->N + 4 + (p->objective == MPPI_OBJ_CONTOUR_PAPER ? ((p->N + 3) & ~3) : 0);
     cfg.smem_bytes = 0;   // fixed once the track is known
 
     const size_t BN4 = (size_t)p->B * p->N * 4, BK = (size_t)p->B * p->K;
@@ -302,7 +303,7 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     } while (0)
     if (cfg.store_du) CKC(dev_alloc(c, &c->d_du, (size_t)p->B * p->N * p->K));
     if (cfg.fused) {
-        CKC(dev_alloc(c, &c->d_partials, (size_t)p->B * d.blocks_per_ctrl * (4 * p->N + 4)));
+        CKC(dev_alloc(c, &c->d_partials, (size_t)p->B * d.blocks_per_ctrl * d.part_stride));
         CKC(dev_alloc(c, &c->d_counters, (size_t)p->B + 1));
         CKC(cudaMemset(c->d_counters, 0, ((size_t)p->B + 1) * sizeof(unsigned)));
     }
@@ -491,7 +492,7 @@ static StepArgs make_args(mppi_ctx* c, const float* x0, const int32_t* start, co
 static int enqueue_iteration(mppi_ctx* c, const StepArgs& a, cudaStream_t s)
 {
     CK(c, launch_rollout(c->dp, a, c->cfg, s));
-    c->launches += c->prm.objective == MPPI_OBJ_CONTOUR_PAPER ? 2 : 1;
+    c->launches += 1;
     if (!c->cfg.fused) {
         CK(c, launch_reduce(c->dp, a, s));
         c->launches += 1;
@@ -727,7 +728,7 @@ extern "C" int mppi_get_info(mppi_ctx* c, mppi_info* o)
     o->local_bytes_per_thread = (int32_t)fa.localSizeBytes;
     o->max_blocks_per_sm = nb;
     o->sm_count = c->sm_count;
-    o->kernels_per_step = (c->cfg.fused ? 1 : 2) + (c->prm.objective == MPPI_OBJ_CONTOUR_PAPER ? 1 : 0);
+    o->kernels_per_step = c->cfg.fused ? 1 : 2;
     o->samples_per_thread = c->cfg.packed ? 2 : 1;
     o->rollout_warps_per_block = c->cfg.pipe ? 3 : c->cfg.lat_consumers ? c->cfg.lat_consumers : c->cfg.block_threads / 32;
     o->l2_bytes = c->l2_bytes;

@@ -14,6 +14,7 @@ struct DevParams {
     int K, N, B;
     int G, M, P, closed, window;      // gates, reference rows, path points
     int blocks_per_ctrl;               // rollout blocks per controller = K / blockDim.x
+    int part_stride;                   // floats per partial: 4N + 4 (+ N rounded up to 4 under OBJ_CONTOUR_PAPER)
     float dt, inv_lambda, sigma, T_min, T_max;
     float h2, h3, h4, h6, h12, hh2, hh3;   // dt/2, dt/3, dt/4, dt/6, dt/12, dt^2/2, dt^2/3
     float inv_mass, g, hover;
@@ -41,7 +42,7 @@ struct StepArgs {
     float* cost;           // [B][K]
     float* weights;        // [B][K]
     float4* du;            // [B][N][K] float4 or nullptr
-    float* partials;       // [B][blocks_per_ctrl][4N+4]  (fused pipeline)
+    float* partials;       // [B][blocks_per_ctrl][part_stride]: S[4N], m, Z, -, - [, S5[N]]  (fused pipeline)
     unsigned int* counters;// [B + 1]: last-block tickets per controller, finished controllers (fused pipeline)
     const float* v_nom;    // [B][N] nominal progress accelerations (OBJ_CONTOUR_PAPER), or nullptr
     float* v_new;          // [B][N] updated ones

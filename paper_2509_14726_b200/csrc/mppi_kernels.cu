@@ -31,6 +31,8 @@ size_t rollout_smem_bytes(const DevParams& P, const LaunchCfg& c)
         return f4 * sizeof(float4);
     }
     if (c.fused) f4 += (size_t)(c.block_threads / 32) * P.N + (3 * P.blocks_per_ctrl + 3) / 4;
+    if (c.objective == OBJ_CONTOUR_PAPER)      // fifth column: its nominal + one accumulator row per warp
+        f4 += ((size_t)(c.block_threads / 32 + 1) * P.N + 3) / 4;
     return f4 * sizeof(float4);
 }
 
@@ -149,7 +151,7 @@ __global__ void __launch_bounds__(MPPI_PK_THREADS, MPPI_PK_MINB) rollout2_kernel
     }
     __syncthreads();
     const int nw = blockDim.x >> 5;
-    float* part = A.partials + ((size_t)b * P.blocks_per_ctrl + blockIdx.x) * (4 * N + 4);
+    float* part = A.partials + ((size_t)b * P.blocks_per_ctrl + blockIdx.x) * P.part_stride;
     for (int j = tid; j < 4 * N; j += blockDim.x) {
         float s = 0.0f;
         for (int w = 0; w < nw; ++w) s += reinterpret_cast<const float*>(s_acc)[w * 4 * N + j];
@@ -275,7 +277,7 @@ __global__ void __launch_bounds__(kLatThreads) rollout_lat_kernel(const DevParam
     __syncthreads();
 
     // ---- phase 3: S[t][i] = sum_l e_l (T_l[t][i] - u_nom[t][i]) from shared memory ----
-    float* part = A.partials + ((size_t)b * P.blocks_per_ctrl + blockIdx.x) * (4 * N + 4);
+    float* part = A.partials + ((size_t)b * P.blocks_per_ctrl + blockIdx.x) * P.part_stride;
     for (int j = tid; j < 4 * N; j += kLatThreads) {
         const int t = j >> 2, i = j & 3;
         const float un = reinterpret_cast<const float*>(s_unom)[j];

@@ -290,7 +290,7 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
     __syncthreads();
 
     // ---- block partial S[t][i] = sum_l e_l (T_l[t][i] - u_nom[t][i]) from the thrusts in shared memory ----
-    float* part = A.partials + ((size_t)b * P.blocks_per_ctrl + blockIdx.x) * (4 * N + 4);
+    float* part = A.partials + ((size_t)b * P.blocks_per_ctrl + blockIdx.x) * P.part_stride;
     for (int j = tid; j < 4 * N; j += kPipeThreads) {
         const int t = j >> 2, i = j & 3;
         const float un = reinterpret_cast<const float*>(s_unom)[j];

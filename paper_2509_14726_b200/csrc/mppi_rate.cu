@@ -26,9 +26,14 @@ __global__ void __launch_bounds__(256, 3) rollout_rate_kernel(const DevParams P,
     float* s_red = reinterpret_cast<float*>(s_trk + track_f4(P, OBJ));   // 64 floats
     float4* s_acc = reinterpret_cast<float4*>(s_red + 64);
     float* s_pair = reinterpret_cast<float*>(s_acc + (blockDim.x >> 5) * N);
+    // OBJ_CONTOUR_PAPER: nominal of the fifth input [N] + one accumulator row per warp, after the pair area
+    float* s_vnom = s_pair + 4 * ((3 * P.blocks_per_ctrl + 3) / 4);
+    float* s_acc5 = s_vnom + N;
 
     const int start = A.start[b];
     stage_inputs<OBJ>(P, A, b, start, s_unom, s_trk);
+    if (OBJ == OBJ_CONTOUR_PAPER)
+        for (int t = tid; t < N; t += blockDim.x) s_vnom[t] = A.v_nom[(size_t)b * N + t];
     __syncthreads();
 
     const float* xb = A.x0 + (OBJ == OBJ_CONTOUR_PAPER ? 19 : 17) * b;   // p, q, v, omega, T(4) [, theta, v_theta]
@@ -56,7 +61,7 @@ __global__ void __launch_bounds__(256, 3) rollout_rate_kernel(const DevParams P,
             J += fmaf(P.R, u.x * u.x + u.y * u.y + u.z * u.z + u.w * u.w, track_state_term(P, s_trk + 4 * t, x));
         if (OBJ == OBJ_CONTOUR_PAPER) {            // fifth sampled input, stage cost, progress states [R-34]..[R-37]
             const float dv = sample_progress_accel<MATH>(P, A.rk, (uint32_t)k, (uint32_t)t, A.iter, (uint32_t)b,
-                                                         A.v_nom[(size_t)b * N + t]);
+                                                         s_vnom[t]);
             J += contour_paper_stage(P, s_trk, x, theta, v_theta, u, dv);
             theta = fmaf(P.hh2, dv, fmaf(P.dt, v_theta, theta));
             v_theta = fminf(fmaxf(fmaf(P.dt, dv, v_theta), 0.0f), P.v_theta_max);
@@ -73,35 +78,10 @@ __global__ void __launch_bounds__(256, 3) rollout_rate_kernel(const DevParams P,
     A.cost[(size_t)b * P.K + k] = J;
 
     if (!FUSED) return;
-    block_partial_and_combine<MATH>(P, A, b, blockIdx.x, J, lo, hi, s_unom, s_red, s_acc, s_pair);
-}
-
-// eq.(5) for the fifth input (OBJ_CONTOUR_PAPER): v_new[b][t] = v_nom[b][t] + sum_k w_k dv_k[t], from the weights
-// the fused update has just written.  dv is re-derived from the counter-based stream for the samples
-// with a non-zero weight only (thread t owns step t and walks the samples in order: deterministic).
-// grid = B, block = 256.
-template <int MATH>
-__global__ void __launch_bounds__(256) progress_update_kernel(const DevParams P, const StepArgs A)
-{
-    __shared__ float s_w[1024];
-    const int b = blockIdx.x, tid = threadIdx.x, N = P.N, K = P.K;
-    for (int t0 = 0; t0 < N; t0 += blockDim.x) {
-        const int t = t0 + tid;
-        const float vn = t < N ? A.v_nom[(size_t)b * N + t] : 0.0f;
-        float acc = 0.0f;
-        for (int k0 = 0; k0 < K; k0 += 1024) {
-            __syncthreads();
-            for (int i = tid; i < 1024 && k0 + i < K; i += blockDim.x) s_w[i] = A.weights[(size_t)b * K + k0 + i];
-            __syncthreads();
-            if (t < N)
-                for (int i = 0; i < 1024 && k0 + i < K; ++i) {
-                    const float w = s_w[i];                        // block-uniform
-                    if (w != 0.0f)
-                        acc = fmaf(w, sample_progress_accel<MATH>(P, A.rk, (uint32_t)(k0 + i), (uint32_t)t, A.iter, (uint32_t)b, vn) - vn, acc);
-                }
-        }
-        if (t < N) A.v_new[(size_t)b * N + t] = vn + acc;
-    }
+    if (OBJ == OBJ_CONTOUR_PAPER)
+        block_partial_and_combine<MATH>(P, A, b, blockIdx.x, J, lo, hi, s_unom, s_red, s_acc, s_pair, s_vnom, s_acc5);
+    else
+        block_partial_and_combine<MATH>(P, A, b, blockIdx.x, J, lo, hi, s_unom, s_red, s_acc, s_pair);
 }
 
 // ---- host-side dispatch ------------------------------------------------------------------------------
@@ -134,10 +114,6 @@ const void* rate_kernel_ptr(const LaunchCfg& c) { return reinterpret_cast<const 
 cudaError_t launch_rate(const DevParams& P, const StepArgs& A, const LaunchCfg& c, cudaStream_t s)
 {
     pick_rate(c)<<<dim3(P.blocks_per_ctrl, P.B), c.block_threads, c.smem_bytes, s>>>(P, A);
-    if (c.objective == OBJ_CONTOUR_PAPER) {        // second launch: the fifth column of the update
-        if (c.fast_math) progress_update_kernel<1><<<P.B, 256, 0, s>>>(P, A);
-        else progress_update_kernel<0><<<P.B, 256, 0, s>>>(P, A);
-    }
     return cudaGetLastError();
 }
 

@@ -154,11 +154,18 @@ __device__ __forceinline__ float rollout_cost(const DevParams& P, const float4* 
 // steps.  Then publish_and_combine.  All threads of the block must call this.
 template <int MATH>
 __device__ __forceinline__ void publish_and_combine(const DevParams& P, const StepArgs& A, int b, int nb,
-                                                    const float4* s_unom, float* s_red, float* s_pair);
+                                                    const float4* s_unom, float* s_red, float* s_pair,
+                                                    const float* s_vnom = nullptr);
+template <int MATH>
+__device__ __forceinline__ float sample_progress_accel(const DevParams& P, const uint32_t (&rk)[20], uint32_t k,
+                                                       uint32_t t, uint32_t iter, uint32_t b, const float vn);
+// s_vnom / s_acc5 (OBJ_CONTOUR_PAPER only, else nullptr): the nominal of the fifth sampled input [N] and one
+// accumulator row per warp [warps][N]; the block's partial then carries S5[N] after its (m, Z) header.
 template <int MATH>
 __device__ __forceinline__ void block_partial_and_combine(const DevParams& P, const StepArgs& A, const int b,
                                                           const int chunk, const float J, const float lo, const float hi,
-                                                          const float4* s_unom, float* s_red, float4* s_acc, float* s_pair)
+                                                          const float4* s_unom, float* s_red, float4* s_acc, float* s_pair,
+                                                          const float* s_vnom = nullptr, float* s_acc5 = nullptr)
 {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, N = P.N;
     const float m = block_min(J, s_red);
@@ -170,7 +177,9 @@ __device__ __forceinline__ void block_partial_and_combine(const DevParams& P, co
         for (int t0 = 0; t0 < N; t0 += 32) {
             const int t = t0 + lane;
             const float4 un = t < N ? s_unom[t] : make_float4(0.f, 0.f, 0.f, 0.f);
+            const float vn = (s_vnom && t < N) ? s_vnom[t] : 0.0f;
             float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+            float acc5 = 0.0f;
             unsigned mm = contrib;
             while (mm) {
                 const int l = __ffs(mm) - 1;
@@ -179,20 +188,28 @@ __device__ __forceinline__ void block_partial_and_combine(const DevParams& P, co
                 const float4 T = sample_input<MATH>(P, A.rk, kbase + l, (uint32_t)t, A.iter, (uint32_t)b, un, lo, hi);
                 acc.x = fmaf(el, T.x - un.x, acc.x); acc.y = fmaf(el, T.y - un.y, acc.y);
                 acc.z = fmaf(el, T.z - un.z, acc.z); acc.w = fmaf(el, T.w - un.w, acc.w);
+                if (s_vnom)
+                    acc5 = fmaf(el, sample_progress_accel<MATH>(P, A.rk, kbase + l, (uint32_t)t, A.iter, (uint32_t)b, vn) - vn, acc5);
             }
-            if (t < N) s_acc[warp * N + t] = acc;
+            if (t < N) { s_acc[warp * N + t] = acc; if (s_vnom) s_acc5[warp * N + t] = acc5; }
         }
     }
     __syncthreads();
     const int nw = blockDim.x >> 5;
-    float* part = A.partials + ((size_t)b * P.blocks_per_ctrl + chunk) * (4 * N + 4);
+    float* part = A.partials + ((size_t)b * P.blocks_per_ctrl + chunk) * P.part_stride;
     for (int j = tid; j < 4 * N; j += blockDim.x) {
         float s = 0.0f;
         for (int w = 0; w < nw; ++w) s += reinterpret_cast<const float*>(s_acc)[w * 4 * N + j];
         part[j] = s;
     }
+    if (s_vnom)
+        for (int t = tid; t < N; t += blockDim.x) {
+            float s = 0.0f;
+            for (int w = 0; w < nw; ++w) s += s_acc5[w * N + t];
+            part[4 * N + 4 + t] = s;
+        }
     if (tid == 0) { part[4 * N] = m; part[4 * N + 1] = Zb; }
-    publish_and_combine<MATH>(P, A, b, P.blocks_per_ctrl, s_unom, s_red, s_pair);
+    publish_and_combine<MATH>(P, A, b, P.blocks_per_ctrl, s_unom, s_red, s_pair, s_vnom);
 }
 
 // Fused softmax update, second half ("last block done").  Every block of controller b has written
@@ -216,9 +233,10 @@ __device__ __forceinline__ unsigned ticket_acq_rel(unsigned* ctr)
 
 template <int MATH>
 __device__ __forceinline__ void publish_and_combine(const DevParams& P, const StepArgs& A, int b, int nb,
-                                                    const float4* s_unom, float* s_red, float* s_pair)
+                                                    const float4* s_unom, float* s_red, float* s_pair,
+                                                    const float* s_vnom)
 {
-    const int tid = threadIdx.x, lane = tid & 31, N = P.N, stride = 4 * N + 4, nthr = blockDim.x;
+    const int tid = threadIdx.x, lane = tid & 31, N = P.N, stride = P.part_stride, nthr = blockDim.x;
     int* s_flag = reinterpret_cast<int*>(s_red) + 48;
     int* s_cnt = s_flag + 1;
     __syncthreads();                               // the block's partial is written (CTA-scope order) ...
@@ -267,8 +285,10 @@ __device__ __forceinline__ void publish_and_combine(const DevParams& P, const St
     }
     __syncthreads();
     const int cnt = *s_cnt;
-    // round trip 3: S rows of the contributing partials
-    for (int j = tid; j < 4 * N; j += nthr) {
+    // round trip 3: S rows of the contributing partials (columns 4N.. = the fifth input, kept after the header)
+    const int ncol = s_vnom ? 5 * N : 4 * N;
+    for (int jj = tid; jj < ncol; jj += nthr) {
+        const int j = jj < 4 * N ? jj : jj + 4;
         float acc = 0.0f;
         int i = 0;
         for (; i + 4 <= cnt; i += 4) {
@@ -282,7 +302,8 @@ __device__ __forceinline__ void publish_and_combine(const DevParams& P, const St
             const int q = s_list[i];
             acc = fmaf(__ldcg(pb + (size_t)q * stride + j), s_scale[q], acc);
         }
-        A.u_new[(size_t)b * 4 * N + j] = fmaf(acc, invZ, reinterpret_cast<const float*>(s_unom)[j]);
+        if (jj < 4 * N) A.u_new[(size_t)b * 4 * N + j] = fmaf(acc, invZ, reinterpret_cast<const float*>(s_unom)[j]);
+        else A.v_new[(size_t)b * N + jj - 4 * N] = fmaf(acc, invZ, s_vnom[jj - 4 * N]);
     }
     float4* w4 = reinterpret_cast<float4*>(A.weights + (size_t)b * P.K);
     const float nil = -P.inv_lambda;

@@ -330,6 +330,18 @@ def lap(kind="gate", B=8, K=4096, N=50, steps=1500) -> Workload:
                     np.repeat(base.u_nom, B, 0), ref=base.ref, path=base.path, closed=base.closed, seed=0, iters=steps)
 
 
+def replicate(wl: Workload, B: int, jitter: float = 0.0) -> Workload:
+    """The same single-controller workload for B controllers (positions jittered by +-jitter m, seeded)."""
+    rng = np.random.default_rng(11)
+    rep = lambda a: None if a is None else np.repeat(a[:1], B, 0).copy()
+    x0 = rep(wl.x0)
+    if jitter:
+        x0[:, 0:3] += rng.uniform(-jitter, jitter, (B, 3)).astype(np.float32)
+    return Workload(f"{wl.name}_x{B}", dict(wl.params, B=B), x0, rep(wl.start), rep(wl.u_nom), gates=wl.gates, ref=wl.ref,
+                    path=wl.path, prev_front=rep(wl.prev_front), v_nom=rep(wl.v_nom), closed=wl.closed, seed=wl.seed,
+                    iters=wl.iters)
+
+
 ALL = {"contour_paper": contour_paper, "rate_gate_paper": rate_gate_paper, "rate_track": rate_track, "rate_stress": rate_stress,
        "gate_paper": gate_paper, "stress_gate_paper": stress_gate_paper, "cfg0": cfg0, "cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg4": cfg4,
        "stress_gate": stress_gate}
