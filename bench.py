@@ -402,8 +402,8 @@ def run_survey(args):
     names = ["cfg0", "cfg1", "cfg2", "cfg3", "gate_paper", "rate_gate_paper", "rate_track", "contour_paper"]
     print("| workload | objective | input model | K | N | B | kernel | launches / iteration | us / iteration | sample-steps/s |")
     print("|---|---|---|---|---|---|---|---|---|---|")
-    for name in names:
-        for B in (1, 64):
+    for name in ([args.only] if args.only else names):
+        for B in ((args.batch,) if args.batch else (1, 64)):
             wl = W.ALL[name]()
             if B > 1:
                 wl = W.replicate(wl, B, 0.3)
@@ -441,6 +441,8 @@ def main(argv=None):
     ap.add_argument("--graph", type=int, default=0)
     ap.add_argument("--cpu-budget", dest="cpu_budget", type=float, default=10.0)
     ap.add_argument("--survey", action="store_true", help="time one iteration of every workload (table, one GPU)")
+    ap.add_argument("--only", default=None, help="--survey: this workload only (a key of workloads.ALL)")
+    ap.add_argument("--batch", type=int, default=0, help="--survey: this number of controllers only")
     args = ap.parse_args(argv)
     if args.survey:
         return run_survey(args)
