@@ -780,6 +780,34 @@ int orc_sim_step(const orc_params* P, const orc_track* trk, double* x, int32_t* 
     return 0;
 }
 
+/* Closed-loop glue under ORC_OBJ_CONTOUR_PAPER [R-39]: rows of 19.  The drone part of the state takes one
+ * rate-model RK4 step with u_new[b][0] (as orc_sim_step); the progress states are the controller's own
+ * (virtual) states and advance by [R-34] with the optimised v_new[b][0]; both nominals shift by one step
+ * with the last entry repeated [R-14].  start is not used by this objective (the path is looked up by
+ * theta) and is left alone.  x [B][19] is updated in place. */
+int orc_sim_step_progress(const orc_params* P, double* x, const double* u_new, double* u_nom_next,
+                          const double* v_new, double* v_nom_next)
+{
+    if (!P || !x || !u_new || !u_nom_next || !v_new || !v_nom_next) return -1;
+    if (P->objective != ORC_OBJ_CONTOUR_PAPER || P->input_model != 1) return -2;
+    const int N = P->N;
+    for (int b = 0; b < P->B; ++b) {
+        double* xb = x + 19 * b;
+        const double* ub = u_new + (size_t)b * N * 4;
+        const double* vb = v_new + (size_t)b * N;
+        double xn[19];
+        orc_rk4_rate_step(P, xb, ub, P->dt, xn);
+        orc_progress_step(P, xb[17], xb[18], vb[0], &xn[17], &xn[18]);
+        memcpy(xb, xn, sizeof(xn));
+        for (int t = 0; t < N; ++t) {
+            const int src = (t + 1 < N) ? t + 1 : N - 1;
+            for (int i = 0; i < 4; ++i) u_nom_next[((size_t)b * N + t) * 4 + i] = ub[4 * src + i];
+        }
+        for (int t = 0; t < N; ++t) v_nom_next[(size_t)b * N + t] = vb[(t + 1 < N) ? t + 1 : N - 1];
+    }
+    return 0;
+}
+
 /* Threads the sample loop will use (reported by bench.py's cpu_baseline). */
 int orc_num_threads(void)
 {

@@ -119,6 +119,8 @@ def lib():
         L.orc_step.restype = C.c_int
         L.orc_sim_step.argtypes = [C.POINTER(_Params), C.POINTER(_Track), _dp, _ip, _dp, _dp]
         L.orc_sim_step.restype = C.c_int
+        L.orc_sim_step_progress.argtypes = [C.POINTER(_Params), _dp, _dp, _dp, _dp, _dp]
+        L.orc_sim_step_progress.restype = C.c_int
         L.orc_num_threads.argtypes = []
         L.orc_num_threads.restype = C.c_int
     return _lib
@@ -359,6 +361,18 @@ def sim_step(params, track: Track, x, start, u_new):
     if rc != 0:
         raise RuntimeError(f"orc_sim_step failed ({rc})")
     return x, start, nxt
+
+
+def sim_step_progress(params, x, u_new, v_new):
+    """Closed-loop glue under OBJ_CONTOUR_PAPER [R-39]: -> (x_next [B,19], u_nom_next [B,N,4], v_nom_next [B,N])."""
+    P = make_params(params)
+    B, N = P.B, P.N
+    x = _f64(x, (B, 19)).copy(); u_new = _f64(u_new, (B, N, 4)); v_new = _f64(v_new, (B, N))
+    nu = np.zeros((B, N, 4)); nv = np.zeros((B, N))
+    rc = lib().orc_sim_step_progress(C.byref(P), _d(x), _d(u_new), _d(nu), _d(v_new), _d(nv))
+    if rc != 0:
+        raise RuntimeError(f"orc_sim_step_progress failed ({rc})")
+    return x, nu, nv
 
 
 def num_threads() -> int:

@@ -92,3 +92,27 @@ def test_brute_force_definition(kw, closed):
     np.testing.assert_allclose(r["dv"][0], dv, rtol=0, atol=1e-13)
     np.testing.assert_allclose(r["u_new"][0], un, rtol=0, atol=1e-12)
     np.testing.assert_allclose(r["v_new"][0], vn, rtol=0, atol=1e-12)
+
+
+def test_plant_step_advances_the_progress_states_and_shifts_both_nominals():
+    # [R-39] drone part = one rate-model RK4 step with u_new[0]; theta, v_theta by the closed form of a held
+    # acceleration v_new[0]; both nominals shift by one with the last entry repeated
+    wl = W.contour_paper(K=8, N=6)
+    p = wl.params
+    x0 = wl.x0.astype(np.float64); x0[0, 17:19] = (3.0, 9.9)
+    u = np.linspace(-3, 3, 24).reshape(1, 6, 4)
+    v = np.array([[7.0, -1.0, 2.0, 0.5, -4.0, 6.0]])
+    x1, un, vn = O.sim_step_progress(p, x0, u, v)
+    h = float(p["dt"])
+    np.testing.assert_allclose(x1[0, :17], O.rk4_rate_step(p, x0[0, :17], u[0, 0]), atol=1e-15)
+    assert x1[0, 17] == pytest.approx(3.0 + h * 9.9 + 0.5 * h * h * 7.0, abs=1e-15)
+    assert x1[0, 18] == pytest.approx(min(9.9 + h * 7.0, float(p["v_theta_max"])), abs=1e-15) and x1[0, 18] == p["v_theta_max"]
+    np.testing.assert_array_equal(un[0, :-1], u[0, 1:]); np.testing.assert_array_equal(un[0, -1], u[0, -1])
+    np.testing.assert_array_equal(vn[0], [-1.0, 2.0, 0.5, -4.0, 6.0, 6.0])
+    # hover + zero progress acceleration: the drone stays, theta advances uniformly
+    x = wl.x0.astype(np.float64); x[0, 7:13] = 0.0; x[0, 17:19] = (1.0, 2.0)
+    p0 = dict(p, drag_x=0.0, drag_y=0.0, drag_z=0.0)
+    for _ in range(10):
+        x, _, _ = O.sim_step_progress(p0, x, np.zeros((1, 6, 4)), np.zeros((1, 6)))
+    np.testing.assert_allclose(x[0, :3], wl.x0[0, :3], atol=1e-7)
+    assert x[0, 17] == pytest.approx(1.0 + 10 * h * 2.0, abs=1e-13) and x[0, 18] == 2.0
