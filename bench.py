@@ -421,7 +421,8 @@ def run_survey(args):
             info = m.info()
             k = ("rate-model scalar" if P.get("input_model", 0) == 1 else
                  "pipelined" if info["rollout_warps_per_block"] == 3 and info["block_threads"] == 256 else
-                 "packed fp32x2" if info["samples_per_thread"] == 2 else "scalar")
+                 "packed fp32x2" if info["samples_per_thread"] == 2 else
+                 "latency" if info["block_threads"] == 256 and info["rollout_warps_per_block"] < 8 else "scalar")
             units = P["K"] * P["N"] * P["B"]
             print(f"| {name} | {P['objective']} | {P.get('input_model', 0)} | {P['K']} | {P['N']} | {P['B']} | {k} "
                   f"({info['block_threads']} thr x {info['grid_blocks']} blocks, {info['regs_per_thread']} regs) | "

@@ -246,8 +246,18 @@ MPPI_API int mppi_front_flags(mppi_ctx* ctx, const float* d_x0, const int32_t* d
  * may be the same buffer (in-place warm start).  Caller-owned, used by every later mppi_step (the fused
  * update writes this column in the same launch) until replaced.  Required before the first step.
  * mppi_optimize needs the in-place form; mppi_step_host and mppi_sim_step return MPPI_E_PARAM under
- * this objective. */
+ * this objective (the plant step is mppi_sim_step_progress). */
 MPPI_API int mppi_set_progress(mppi_ctx* ctx, const float* d_v_nom, float* d_v_new);
+
+/* Closed-loop glue under MPPI_OBJ_CONTOUR_PAPER (reading R-39 of DESIGN.md; the counterpart of
+ * mppi_sim_step for rows of 19): d_x [B][19] device, in/out: the drone part takes one rate-model RK4 step
+ * with d_u_new[b][0] (clamped to the rate range), theta and v_theta advance with d_v_new[b][0] held over
+ * the step (theta += dt v_theta + dt^2/2 dv; v_theta clamped to [0, v_theta_max]); d_u_nom_next [B][N][4]
+ * and d_v_nom_next [B][N] receive the nominals shifted by one step, last entry repeated.  Each output
+ * may be the same buffer as its input (partial overlap: MPPI_E_RANGE).  The start indices are not used
+ * by this objective.  One kernel launch on `stream`. */
+MPPI_API int mppi_sim_step_progress(mppi_ctx* ctx, float* d_x, const float* d_u_new, float* d_u_nom_next,
+                                    const float* d_v_new, float* d_v_nom_next, void* stream);
 
 /* Device pointer to dU [B][N][K][4] of the last step (parity debugging); NULL unless the
  * context keeps it (TWO_PASS pipeline or store_noise). */

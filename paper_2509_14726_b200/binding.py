@@ -20,7 +20,7 @@ VARIANT_AUTO, VARIANT_THROUGHPUT, VARIANT_LATENCY, VARIANT_PACKED, VARIANT_PIPEL
 
 EXPORTS = ["mppi_default_params", "mppi_create", "mppi_destroy", "mppi_set_gates",
            "mppi_set_reference", "mppi_set_path", "mppi_step", "mppi_optimize", "mppi_step_host",
-           "mppi_sim_step", "mppi_set_prev_front", "mppi_front_flags", "mppi_set_progress", "mppi_debug_noise", "mppi_get_info", "mppi_launch_count",
+           "mppi_sim_step", "mppi_set_prev_front", "mppi_front_flags", "mppi_set_progress", "mppi_sim_step_progress", "mppi_debug_noise", "mppi_get_info", "mppi_launch_count",
            "mppi_error_string", "mppi_last_error", "mppi_measure_fma_peak", "mppi_measure_copy_bw"]
 
 
@@ -70,6 +70,7 @@ def _load():
     L.mppi_step_host.argtypes = [vp, fp, ip, fp, C.c_uint64, C.c_uint32, fp, fp, fp, vp]
     L.mppi_sim_step.argtypes = [vp, fp, ip, fp, fp, vp]
     L.mppi_set_progress.argtypes = [vp, fp, fp]
+    L.mppi_sim_step_progress.argtypes = [vp, fp, fp, fp, fp, fp, vp]
     L.mppi_set_prev_front.argtypes = [vp, ip]
     L.mppi_front_flags.argtypes = [vp, fp, ip, fp, ip, vp]
     L.mppi_debug_noise.argtypes = [vp]
@@ -294,6 +295,19 @@ class Mppi:
         self._v = (v_nom, v_new)
         self._ck(lib.mppi_set_progress(self._h, self._dev(v_nom, (self.B, self.N), torch.float32),
                                        self._dev(v_new, (self.B, self.N), torch.float32)))
+
+    def sim_step_progress(self, x, u_new, v_new, u_nom_next=None, v_nom_next=None, stream=None):
+        """Objective 4: plant step on rows of 19 + shift of both nominals (in place when the outputs are None)."""
+        import torch
+        B, N = self.B, self.N
+        u_nom_next = u_new if u_nom_next is None else u_nom_next
+        v_nom_next = v_new if v_nom_next is None else v_nom_next
+        self._ck(lib.mppi_sim_step_progress(self._h, self._dev(x, (B, 19), torch.float32),
+                                            self._dev(u_new, (B, N, 4), torch.float32),
+                                            self._dev(u_nom_next, (B, N, 4), torch.float32),
+                                            self._dev(v_new, (B, N), torch.float32),
+                                            self._dev(v_nom_next, (B, N), torch.float32), _stream_ptr(stream)))
+        return x, u_nom_next, v_nom_next
 
     def set_prev_front(self, prev_front):
         """prev_front: CUDA int32 tensor [B, N+1] (kept alive by this object), or None."""

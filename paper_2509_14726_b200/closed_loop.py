@@ -20,6 +20,7 @@ import numpy as np
 @dataclass
 class FlightLog:
     x: np.ndarray          # [steps + 1, B, xdim] float32: plant state before every control step + the last
+                           # (xdim 13; 17 under the rate model; 19 under objective 4: ..., theta, v_theta)
     start: np.ndarray      # [steps + 1, B] int32: the controller's start index (target gate / row / path index)
     dt: float
 
@@ -42,8 +43,17 @@ def fly(m, wl, steps: int, iters_per_step: int = 1, seed=None, prev_front_feedba
     log_x = torch.empty((steps + 1, B, x.shape[1]), device=dev)
     log_s = torch.empty((steps + 1, B), dtype=torch.int32, device=dev)
     front = None
+    progress = m.params.objective == 4        # the paper's contouring: rows of 19, fifth column v [B,N]
+    if progress:
+        v = torch.from_numpy(np.ascontiguousarray(wl.v_nom)).to(dev)
+        m.set_progress(v)                     # in place
     for i in range(steps):
         log_x[i].copy_(x); log_s[i].copy_(start)
+        if progress:
+            for j in range(iters_per_step):
+                m.step(x, start, u, seed, i * iters_per_step + j, u_new=u, cost=cost, weights=w)
+            m.sim_step_progress(x, u, v)
+            continue
         if prev_front_feedback:
             m.set_prev_front(front)
         for j in range(iters_per_step):
@@ -111,6 +121,30 @@ def tracking_rmse(log: FlightLog, ref: np.ndarray, first_row: int = 0) -> np.nda
     r = np.asarray(ref, np.float64)[first_row: first_row + T, 0:3]
     e = log.x[: len(r), :, 0:3].astype(np.float64) - r[:, None, :]
     return np.sqrt((e ** 2).sum(-1).mean(0))
+
+
+def progress_metrics(log: FlightLog, path: np.ndarray) -> list[dict]:
+    """Objective 4 (rows of 19): per drone the progress made (theta_end - theta_0, in laps of the closed path
+    too), the time of every completed lap of theta, the largest distance between the drone and P(theta)
+    (how well the virtual progress state and the vehicle stay together) and speed statistics."""
+    P = np.asarray(path, np.float64)
+    seg = np.linalg.norm(np.diff(np.vstack([P, P[:1]]), axis=0), axis=1)
+    s = np.concatenate([[0.0], np.cumsum(seg)])                # s[P] = L
+    L = float(s[-1])
+    Pc = np.vstack([P, P[:1]])
+    res = []
+    for b in range(log.x.shape[1]):
+        th = log.x[:, b, 17].astype(np.float64)
+        p = log.x[:, b, 0:3].astype(np.float64)
+        tw = np.mod(th, L)
+        on = np.stack([np.interp(tw, s, Pc[:, a]) for a in range(3)], axis=1)
+        adv = th - th[0]
+        lap_t = [float(np.argmax(adv >= k * L) * log.dt) for k in range(1, int(adv[-1] // L) + 1)]
+        speed = np.linalg.norm(log.x[:, b, 7:10].astype(np.float64), axis=1)
+        res.append(dict(progress_m=float(adv[-1]), laps=float(adv[-1] / L), lap_times_s=lap_t,
+                        dist_to_progress_point_max=float(np.linalg.norm(p - on, axis=1).max()),
+                        speed_mean=float(speed.mean()), speed_max=float(speed.max())))
+    return res
 
 
 def contour_rms(log: FlightLog, path: np.ndarray) -> np.ndarray:

@@ -177,11 +177,16 @@ static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, i
             if (p->K % tpb == 0) { *block_threads = tpb; return; }
     }
     const bool lat_ok = p->pipeline == MPPI_PIPE_FUSED && p->block_threads == 0;
-    if (lat_ok && (p->variant == MPPI_VARIANT_PIPELINED || (p->variant == MPPI_VARIANT_AUTO && warps <= 4 * (int64_t)sm_count))) {
+    // the windowed nearest-vertex search of objective 2 is ~2/3 of a step and cannot be split over the
+    // pipeline's roles (it would all sit in the translation warp: 112 us at configs[3]); the latency
+    // kernel spreads whole rollouts over the consumer warps instead (68 us, measured)
+    const bool few = p->variant == MPPI_VARIANT_AUTO && warps <= 4 * (int64_t)sm_count;
+    const bool search = p->objective == MPPI_OBJ_CONTOUR;
+    if (lat_ok && (p->variant == MPPI_VARIANT_PIPELINED || (few && !search))) {
         *pipe = 1; *block_threads = 256;
         return;
     }
-    if (lat_ok && p->variant == MPPI_VARIANT_LATENCY) {
+    if (lat_ok && (p->variant == MPPI_VARIANT_LATENCY || (few && search))) {
         int best = 0;
         for (int c : {1, 2, 4})
             if (p->K % (32 * c) == 0) {
@@ -663,13 +668,30 @@ extern "C" int mppi_sim_step(mppi_ctx* c, float* d_x, int32_t* d_start, const fl
     if (!c) return MPPI_E_NULL;
     if (!d_x || !d_start || !d_u_new || !d_u_nom_next) return fail(c, MPPI_E_NULL, "mppi_sim_step: NULL device pointer");
     if (c->prm.objective == MPPI_OBJ_CONTOUR_PAPER)
-        return fail(c, MPPI_E_PARAM, "mppi_sim_step: not available for MPPI_OBJ_CONTOUR_PAPER yet (the progress states have no plant)");
+        return fail(c, MPPI_E_PARAM, "mppi_sim_step: MPPI_OBJ_CONTOUR_PAPER has rows of 19 and a fifth column: use mppi_sim_step_progress");
     const size_t ub = (size_t)c->prm.B * c->prm.N * 4 * sizeof(float);
     if (d_u_nom_next != d_u_new && overlaps(d_u_nom_next, ub, d_u_new, ub))
         return fail(c, MPPI_E_RANGE, "d_u_nom_next partially overlaps d_u_new");
     int rc = prepare(c);
     if (rc) return rc;
     CK(c, launch_sim(c->dp, c->prm.objective, d_x, d_start, d_u_new, d_u_nom_next, (cudaStream_t)stream));
+    c->launches += 1;
+    return MPPI_OK;
+}
+
+extern "C" int mppi_sim_step_progress(mppi_ctx* c, float* d_x, const float* d_u_new, float* d_u_nom_next,
+                                      const float* d_v_new, float* d_v_nom_next, void* stream)
+{
+    if (!c) return MPPI_E_NULL;
+    if (c->prm.objective != MPPI_OBJ_CONTOUR_PAPER)
+        return fail(c, MPPI_E_PARAM, "mppi_sim_step_progress: the objective is not MPPI_OBJ_CONTOUR_PAPER");
+    if (!d_x || !d_u_new || !d_u_nom_next || !d_v_new || !d_v_nom_next)
+        return fail(c, MPPI_E_NULL, "mppi_sim_step_progress: NULL device pointer");
+    const size_t ub = (size_t)c->prm.B * c->prm.N * 4 * sizeof(float), vb = ub / 4;
+    if ((d_u_nom_next != d_u_new && overlaps(d_u_nom_next, ub, d_u_new, ub)) ||
+        (d_v_nom_next != d_v_new && overlaps(d_v_nom_next, vb, d_v_new, vb)))
+        return fail(c, MPPI_E_RANGE, "an output partially overlaps its input");
+    CK(c, launch_sim_progress(c->dp, d_x, d_u_new, d_u_nom_next, d_v_new, d_v_nom_next, (cudaStream_t)stream));
     c->launches += 1;
     return MPPI_OK;
 }

@@ -413,6 +413,48 @@ __global__ void sim_kernel(const DevParams P, float* __restrict__ xs, int* __res
     }
 }
 
+// Plant step under OBJ_CONTOUR_PAPER [R-39]: rows of 19.  The drone takes one rate-model RK4 step with
+// u_new[b][0]; the progress states advance by [R-34] with v_new[b][0]; both nominals shift by one step.
+// One block per controller; the shifts keep their source in a register so that the outputs may alias
+// the inputs.
+__global__ void sim_progress_kernel(const DevParams P, float* __restrict__ xs, const float* u_new, float* u_nom_next,
+                                    const float* v_new, float* v_nom_next)
+{
+    const int b = blockIdx.x;
+    const int N = P.N;
+    if (threadIdx.x == 0) {
+        float* xb = xs + 19 * b;
+        State x = load_state(xb);
+        float4 Ts = make_float4(xb[13], xb[14], xb[15], xb[16]);
+        const float theta = xb[17], v_theta = xb[18];
+        const float4 T = reinterpret_cast<const float4*>(u_new)[(size_t)b * N];
+        const float4 u = make_float4(fminf(fmaxf(T.x, -P.rate_max), P.rate_max), fminf(fmaxf(T.y, -P.rate_max), P.rate_max),
+                                     fminf(fmaxf(T.z, -P.rate_max), P.rate_max), fminf(fmaxf(T.w, -P.rate_max), P.rate_max));
+        const float dv = fminf(fmaxf(v_new[(size_t)b * N], -P.dv_max), P.dv_max);
+        rk4_rate_step(P, x, Ts, u);
+        float* o = xb;
+        o[0] = x.px; o[1] = x.py; o[2] = x.pz; o[3] = x.qw; o[4] = x.qx; o[5] = x.qy; o[6] = x.qz;
+        o[7] = x.vx; o[8] = x.vy; o[9] = x.vz; o[10] = x.ox; o[11] = x.oy; o[12] = x.oz;
+        o[13] = Ts.x; o[14] = Ts.y; o[15] = Ts.z; o[16] = Ts.w;
+        o[17] = fmaf(P.hh2, dv, fmaf(P.dt, v_theta, theta));
+        o[18] = fminf(fmaxf(fmaf(P.dt, dv, v_theta), 0.0f), P.v_theta_max);
+    }
+    const float4* src = reinterpret_cast<const float4*>(u_new) + (size_t)b * N;
+    float4* dst = reinterpret_cast<float4*>(u_nom_next) + (size_t)b * N;
+    const float* vsrc = v_new + (size_t)b * N;
+    float* vdst = v_nom_next + (size_t)b * N;
+    __syncthreads();                       // thread 0 has read u_new[0], v_new[0]
+    for (int t0 = 0; t0 < N; t0 += blockDim.x) {
+        const int t = t0 + threadIdx.x;
+        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+        float w = 0.0f;
+        if (t < N) { v = src[min(t + 1, N - 1)]; w = vsrc[min(t + 1, N - 1)]; }
+        __syncthreads();
+        if (t < N) { dst[t] = v; vdst[t] = w; }
+        __syncthreads();
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 // "In front of the gate" flags of the noise-free rollout of a nominal sequence [R-26]: what the
 // temporal gate-switching check of the paper's J_gate (Fig. 2) compares the next
@@ -543,6 +585,13 @@ cudaError_t launch_sim(const DevParams& P, int objective, float* x, int* start, 
         sim_kernel<OBJ_GATE><<<P.B, threads, 0, s>>>(P, x, start, u_new, u_nom_next);
     else if (objective == OBJ_TRACK) sim_kernel<OBJ_TRACK><<<P.B, threads, 0, s>>>(P, x, start, u_new, u_nom_next);
     else sim_kernel<OBJ_CONTOUR><<<P.B, threads, 0, s>>>(P, x, start, u_new, u_nom_next);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_sim_progress(const DevParams& P, float* x, const float* u_new, float* u_nom_next,
+                                const float* v_new, float* v_nom_next, cudaStream_t s)
+{
+    sim_progress_kernel<<<P.B, 64, 0, s>>>(P, x, u_new, u_nom_next, v_new, v_nom_next);
     return cudaGetLastError();
 }
 

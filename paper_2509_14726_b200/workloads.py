@@ -321,6 +321,16 @@ def lap(kind="gate", B=8, K=4096, N=50, steps=1500) -> Workload:
             p.update(objective=OBJ_GATE_PAPER, gate_pass_bonus=0.0, gate_miss_penalty=0.0, q_near=_f32(0.5), r_near=_f32(1.5))
         p["lambda"] = _f32(0.5 if kind == "gate_paper" else 0.02)      # squared distances: larger cost scale
         return Workload(f"lap_{kind}_B{B}", p, wl.x0, wl.start, wl.u_nom, gates=wl.gates, seed=0, iters=steps)
+    if kind == "contour_paper":
+        # the paper's own contouring under the paper's model; tuned like the other lap workloads so that it flies
+        base = contour_paper(K=K, N=N)
+        p = dict(base.params, B=B, sigma=_f32(3.0), sigma_v=_f32(3.0), w_omega=_f32(0.001), q_contour=_f32(200.0),
+                 q_lag=_f32(100.0), mu_progress=_f32(10.0))
+        p["lambda"] = _f32(1.0)
+        x0 = np.repeat(base.x0, B, 0)
+        x0[:, 0:3] += rng.uniform(-0.2, 0.2, (B, 3)).astype(np.float32)
+        return Workload(f"lap_{kind}_B{B}", p, x0.astype(np.float32), np.repeat(base.start, B, 0), np.repeat(base.u_nom, B, 0),
+                        path=base.path, closed=base.closed, v_nom=np.repeat(base.v_nom, B, 0), seed=0, iters=steps)
     base = cfg2(K=K, N=N, extra_rows=steps + 1) if kind == "track" else cfg3(K=K, N=N)
     p = dict(base.params, B=B, **tune)
     p["lambda"] = _f32(0.02 if kind == "contour" else 0.5)

@@ -656,3 +656,51 @@ def test_lap_experiment_tracking_and_contouring():
     assert (CL.contour_rms(log, wl.path) < 0.3).all()
     travelled = np.linalg.norm(np.diff(log.x[:, :, 0:3].astype(np.float64), axis=0), axis=-1).sum(0)
     assert (travelled > 15.0).all()                            # it really flies along the path
+
+
+def test_contour_paper_closed_loop_teacher_forced():
+    # the paper's contouring in a closed loop: iteration (u and v updated in place), plant step on rows of 19,
+    # shift of both nominals; every step compared with the oracle from the GPU's own inputs [R-17]
+    import torch
+    from oracle import oracle as O
+    B, K, N = 3, 1024, 30
+    wl = W.lap("contour_paper", B=B, K=K, N=N)
+    p = wl.params
+    m = Pz.make_ctx(wl)
+    x, start, u = Pz.to_dev(wl)
+    v = torch.from_numpy(wl.v_nom.copy()).cuda()
+    m.set_progress(v)
+    for step in range(5):
+        x_in, u_in, v_in = x.cpu().numpy(), u.cpu().numpy(), v.cpu().numpy()
+        g = Pz.gpu_step(m, x, start, u, 5, step, u_new=u)
+        o = O.step(p, O.Track(path=wl.path, closed=wl.closed), x_in, wl.start, u_in, 5, step, want_du=True, v_nom=v_in)
+        o["u_nom"] = u_in.astype(np.float64); o["v_nom"] = v_in.astype(np.float64)
+        _cp_check(f"contour_paper loop step{step}", wl, g, o)
+        xo, uo, vo = O.sim_step_progress(p, x_in, g["u_new"], g["v_new"])
+        m.sim_step_progress(x, u, v); torch.cuda.synchronize()
+        np.testing.assert_allclose(x.cpu().numpy(), xo, rtol=3e-6, atol=2e-5)
+        np.testing.assert_array_equal(u.cpu().numpy(), uo.astype(np.float32))
+        np.testing.assert_array_equal(v.cpu().numpy(), vo.astype(np.float32))
+    assert (x.cpu().numpy()[:, 17] > wl.x0[:, 17] + 0.1).all()            # theta moved on
+    # out-of-place form gives the same plant step
+    x2 = torch.from_numpy(x_in).cuda(); u2 = torch.from_numpy(g["u_new"]).cuda(); v2 = torch.from_numpy(g["v_new"]).cuda()
+    un = torch.empty_like(u2); vn = torch.empty_like(v2)
+    m.sim_step_progress(x2, u2, v2, u_nom_next=un, v_nom_next=vn); torch.cuda.synchronize()
+    np.testing.assert_array_equal(x2.cpu().numpy(), x.cpu().numpy())
+    np.testing.assert_array_equal(un.cpu().numpy(), u.cpu().numpy()); np.testing.assert_array_equal(vn.cpu().numpy(), v.cpu().numpy())
+    m.close()
+
+
+def test_lap_experiment_contour_paper():
+    from paper_2509_14726_b200 import closed_loop as CL
+    wl = W.lap("contour_paper", B=4, K=2048, steps=500)
+    m = Pz.make_ctx(wl)
+    log = CL.fly(m, wl, 500)
+    m.close()
+    assert np.isfinite(log.x).all()
+    for b, q in enumerate(CL.progress_metrics(log, wl.path)):
+        assert q["laps"] > 1.5 and len(q["lap_times_s"]) >= 1 and q["lap_times_s"][0] < 8.0, (b, q)   # 31 m per lap
+        assert q["dist_to_progress_point_max"] < 1.5, (b, q)       # the vehicle stays with its progress state
+        assert 3.0 < q["speed_mean"] < 12.0
+    assert (CL.contour_rms(log, wl.path) < 0.4).all()
+    assert log.x[:, :, 2].min() > 0.5                              # and in the air (the path is at z = 1.5 m)
