@@ -64,3 +64,44 @@ def test_lap_workloads_are_well_formed():
         assert wl.x0.shape == (3, 13) and wl.u_nom.shape == (3, 10, 4) and wl.params["B"] == 3
         if kind == "track":
             assert wl.ref.shape[0] >= 20 + 10 + 1
+
+
+def test_progress_metrics_on_a_square_path():
+    # rows of 19 (objective 4): the vehicle runs 0.3 m beside a 4 x 4 m square path at 4 m/s while its
+    # progress state theta advances at exactly that speed: laps, lap times and the distance between the
+    # vehicle and P(theta) have closed forms
+    path = np.array([[0, 0, 1], [4, 0, 1], [4, 4, 1], [0, 4, 1]], np.float32)      # closed, L = 16
+    dt, steps, v = 0.02, 500, 4.0
+    t = np.arange(steps + 1) * dt
+    th = 1.0 + v * t                                        # theta_0 = 1 m
+    s = np.mod(th, 16.0)
+    on = np.stack([np.select([s < 4, s < 8, s < 12], [s, 4 + 0 * s, 12 - s], 0 * s),
+                   np.select([s < 4, s < 8, s < 12], [0 * s, s - 4, 4 + 0 * s], 16 - s), np.ones_like(s)], 1)
+    x = np.zeros((steps + 1, 2, 19), np.float32)
+    x[:, 0, 0:3] = on + [0, 0, 0.3]                         # drone 0: 0.3 m above P(theta)
+    x[:, 1, 0:3] = on                                       # drone 1: exactly on it ...
+    x[:, :, 7] = v; x[:, :, 17] = th[:, None]
+    x[:, 1, 17] = 1.0 + 0.5 * v * t                         # ... but its theta runs at half the speed
+    log = CL.FlightLog(x, np.zeros((steps + 1, 2), np.int32), dt)
+    m0, m1 = CL.progress_metrics(log, path)
+    assert m0["progress_m"] == pytest.approx(v * steps * dt, abs=1e-4) and m0["laps"] == pytest.approx(40.0 / 16.0, abs=1e-5)
+    np.testing.assert_allclose(m0["lap_times_s"], [4.0, 8.0], atol=dt)
+    assert m0["dist_to_progress_point_max"] == pytest.approx(0.3, abs=1e-5)
+    assert m0["speed_mean"] == pytest.approx(v)
+    assert m1["laps"] == pytest.approx(20.0 / 16.0, abs=1e-5) and len(m1["lap_times_s"]) == 1
+    assert m1["dist_to_progress_point_max"] > 3.9          # the vehicle ran away from its progress point
+    # contour_rms sees the same flights: 0.3 m beside the path / on it
+    np.testing.assert_allclose(CL.contour_rms(log, path), [0.3, 0.0], atol=1e-5)
+
+
+def test_replicate_keeps_every_array_consistent():
+    for name in ("cfg1", "gate_paper", "contour_paper"):
+        base = W.ALL[name](K=64, N=8)
+        wl = W.replicate(base, 5, jitter=0.2)
+        assert wl.params["B"] == 5 and wl.x0.shape == (5, base.x0.shape[1]) and wl.u_nom.shape == (5, 8, 4)
+        assert np.abs(wl.x0[:, 0:3] - base.x0[0, 0:3]).max() <= 0.2 + 1e-6 and np.ptp(wl.x0[:, 0]) > 0
+        np.testing.assert_array_equal(wl.x0[:, 3:], np.repeat(base.x0[:, 3:], 5, 0))
+        assert (wl.v_nom is None) == (base.v_nom is None) and (wl.prev_front is None) == (base.prev_front is None)
+        if wl.v_nom is not None:
+            assert wl.v_nom.shape == (5, 8)
+        assert base.params["B"] == 1                                  # the original is untouched
