@@ -94,7 +94,10 @@ typedef enum {
     MPPI_VARIANT_PIPELINED = 4,  /* latency kernel, 256-thread blocks of 32 samples: five warps draw the noise,
                                     three warps on three SM sub-partitions carry the body-rate, attitude and
                                     translation chains of the same rollouts, pipelined over the horizon steps
-                                    through shared-memory rings (mbarriers); fused pipeline only           */
+                                    through shared-memory rings (mbarriers); fused pipeline only.  Under
+                                    input_model = 1: 320-thread blocks, five chains (thrust states + body
+                                    rates, attitude, two warps for the drag matrices of the RK4 stages,
+                                    velocity / position); N <= 100, objectives gate / gate_paper / track   */
     MPPI_VARIANT_PACKED = 3      /* throughput kernel with TWO samples per thread held in packed fp32x2
                                     registers (sm_100a FFMA2); needs K % 64 == 0; costs are bit-identical
                                     to MPPI_VARIANT_THROUGHPUT                                             */
@@ -141,8 +144,9 @@ typedef struct {
                           entries (p, q, v, omega, T(4)); u_nom / u_new hold rates; sigma is in N/s.
                           Rates are clamped to [-rate_max, rate_max], the thrust states are
                           projected onto [T_min, T_max] after every step, eq.(8)'s input term
-                          R |u|^2 acts on the rates.  Runs on the scalar throughput kernel
-                          (variant AUTO or THROUGHPUT); mppi_sim_step advances the 17-entry rows  */
+                          R |u|^2 acts on the rates.  Kernels: scalar throughput (THROUGHPUT) and
+                          pipelined latency (PIPELINED); AUTO picks the latter when B*K/32 warps
+                          fit one per SM; mppi_sim_step advances the 17-entry rows                */
     float rate_max;      /* N/s, > 0 when input_model = 1 (Table I: 10)            */
     float drag_x, drag_y, drag_z; /* D = diag(.) of eq.(2)'s rotor drag - R D R^T v, body frame, 1/s,
                           >= 0; input_model = 1 only (the paper prints no value)                  */

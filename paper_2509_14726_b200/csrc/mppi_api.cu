@@ -155,8 +155,12 @@ static int validate(const mppi_params* p)
             "rotor drag and the body-rate limit cost need input_model = 1");
     } else {
         BAD(!(p->rate_max > 0.0f), "rate_max must be > 0 when input_model = 1");
-        BAD(p->variant != MPPI_VARIANT_AUTO && p->variant != MPPI_VARIANT_THROUGHPUT,
-            "input_model = 1 runs on the scalar throughput kernel: variant must be AUTO or THROUGHPUT");
+        BAD(p->variant != MPPI_VARIANT_AUTO && p->variant != MPPI_VARIANT_THROUGHPUT && p->variant != MPPI_VARIANT_PIPELINED,
+            "input_model = 1 has a scalar throughput kernel and a pipelined latency kernel: variant must be AUTO, THROUGHPUT or PIPELINED");
+        BAD(p->variant == MPPI_VARIANT_PIPELINED &&
+                (p->pipeline != MPPI_PIPE_FUSED || p->block_threads != 0 || p->N > 100 || p->K % 32 != 0 ||
+                 (p->objective != MPPI_OBJ_GATE && p->objective != MPPI_OBJ_GATE_PAPER && p->objective != MPPI_OBJ_TRACK)),
+            "input_model = 1, PIPELINED: fused pipeline, block_threads 0, N <= 100, K % 32 == 0, objective gate / gate_paper / track");
     }
 #undef BAD
     return MPPI_OK;
@@ -171,7 +175,14 @@ static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, i
     *lat_consumers = 0;
     *packed = 0;
     *pipe = 0;
-    if (p->input_model == 1) {                     // thrust-rate model: its own scalar kernel (mppi_rate.cu)
+    if (p->input_model == 1) {                     // thrust-rate model: its own kernels (mppi_rate.cu)
+        // few rollouts: the pipelined latency kernel (mppi_pipe_rate.cuh; its rings need N <= 100)
+        const bool can = p->pipeline == MPPI_PIPE_FUSED && p->block_threads == 0 && p->N <= 100 && p->K % 32 == 0 &&
+                         (p->objective == MPPI_OBJ_GATE || p->objective == MPPI_OBJ_GATE_PAPER || p->objective == MPPI_OBJ_TRACK);
+        if (can && (p->variant == MPPI_VARIANT_PIPELINED || (p->variant == MPPI_VARIANT_AUTO && warps <= (int64_t)sm_count))) {
+            *pipe = 1; *block_threads = 320;
+            return;
+        }
         if (p->block_threads) { *block_threads = p->block_threads; return; }
         for (int tpb : {128, 64, 32})
             if (p->K % tpb == 0) { *block_threads = tpb; return; }
@@ -752,7 +763,7 @@ extern "C" int mppi_get_info(mppi_ctx* c, mppi_info* o)
     o->sm_count = c->sm_count;
     o->kernels_per_step = c->cfg.fused ? 1 : 2;
     o->samples_per_thread = c->cfg.packed ? 2 : 1;
-    o->rollout_warps_per_block = c->cfg.pipe ? 3 : c->cfg.lat_consumers ? c->cfg.lat_consumers : c->cfg.block_threads / 32;
+    o->rollout_warps_per_block = c->cfg.pipe ? (c->cfg.rate ? 5 : 3) : c->cfg.lat_consumers ? c->cfg.lat_consumers : c->cfg.block_threads / 32;
     o->l2_bytes = c->l2_bytes;
     o->scratch_bytes = c->scratch_bytes;
     return MPPI_OK;

@@ -8,6 +8,7 @@
 #include "mppi_internal.h"
 #include "mppi_rollout.cuh"
 #include "mppi_rate.cuh"
+#include "mppi_pipe_rate.cuh"
 
 namespace mppi {
 
@@ -109,11 +110,29 @@ static RateFn pick_rate(const LaunchCfg& c)
     }
 }
 
-const void* rate_kernel_ptr(const LaunchCfg& c) { return reinterpret_cast<const void*>(pick_rate(c)); }
+template <int OBJ>
+static RateFn pick_pipe_rate1(const LaunchCfg& c)
+{
+    if (c.fast_math) return c.store_du ? rollout_pipe_rate_kernel<OBJ, 1, true> : rollout_pipe_rate_kernel<OBJ, 1, false>;
+    return c.store_du ? rollout_pipe_rate_kernel<OBJ, 0, true> : rollout_pipe_rate_kernel<OBJ, 0, false>;
+}
+static RateFn pick_pipe_rate(const LaunchCfg& c)
+{
+    switch (c.objective) {
+        case OBJ_GATE: return pick_pipe_rate1<OBJ_GATE>(c);
+        case OBJ_GATE_PAPER: return pick_pipe_rate1<OBJ_GATE_PAPER>(c);
+        default: return pick_pipe_rate1<OBJ_TRACK>(c);
+    }
+}
+
+const void* rate_kernel_ptr(const LaunchCfg& c)
+{
+    return reinterpret_cast<const void*>(c.pipe ? pick_pipe_rate(c) : pick_rate(c));
+}
 
 cudaError_t launch_rate(const DevParams& P, const StepArgs& A, const LaunchCfg& c, cudaStream_t s)
 {
-    pick_rate(c)<<<dim3(P.blocks_per_ctrl, P.B), c.block_threads, c.smem_bytes, s>>>(P, A);
+    (c.pipe ? pick_pipe_rate(c) : pick_rate(c))<<<dim3(P.blocks_per_ctrl, P.B), c.block_threads, c.smem_bytes, s>>>(P, A);
     return cudaGetLastError();
 }
 

@@ -414,10 +414,13 @@ def test_front_flags_and_closed_loop_feed():
 
 # ---- the paper's own input model (thrust rates, thrust states, drag, rate limit) ----
 
-RATE_PIPES = [dict(pipeline=0), dict(pipeline=0, variant=1, block_threads=64), dict(pipeline=1)]
+RATE_PIPES = [dict(pipeline=0, variant=4), dict(pipeline=0, variant=1), dict(pipeline=0, variant=1, block_threads=64), dict(pipeline=1)]
 
 
-@pytest.mark.parametrize("pipe", RATE_PIPES, ids=["fused", "fused_tpb64", "two_pass"])
+RATE_IDS = ["fused_pipe", "fused", "fused_tpb64", "two_pass"]
+
+
+@pytest.mark.parametrize("pipe", RATE_PIPES, ids=RATE_IDS)
 @pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
 @pytest.mark.parametrize("name", ["rate_gate_paper", "rate_track"])
 def test_rate_model_objectives(name, pipe, math):
@@ -429,13 +432,41 @@ def test_rate_model_objectives(name, pipe, math):
     assert (np.abs(o0["cost"] - o["cost"]) > 1e-3 * np.abs(o["cost"])).mean() > 0.5
 
 
-@pytest.mark.parametrize("pipe", RATE_PIPES, ids=["fused", "fused_tpb64", "two_pass"])
+@pytest.mark.parametrize("pipe", RATE_PIPES, ids=RATE_IDS)
 def test_rate_model_saturation_and_crossings(pipe):
     wl = W.rate_stress(K=4096, N=30)
     g, o, st = run_case(wl, f"rate_stress[{pipe}]", **pipe)
     nc = o["ncross"]
     assert (nc > 0).mean() > 0.1 and (nc == 0).mean() > 0.1
     assert (np.abs(o["du"]) == wl.params["rate_max"]).mean() > 0.05          # rate clamp acts at scale
+
+
+@pytest.mark.parametrize("K,N,B", [(32, 1, 1), (64, 7, 3), (96, 23, 2), (256, 100, 1), (2048, 50, 2)])
+@pytest.mark.parametrize("name", ["rate_gate_paper", "rate_track", "rate_stress"])
+def test_rate_model_pipelined_kernel_sizes(name, K, N, B):
+    # the pipelined latency kernel of the rate model: ragged last chunk (N % 5 != 0), a single step, the
+    # longest horizon its rings take, several controllers; against the oracle and against the scalar kernel
+    if name == "rate_stress":
+        N = min(N, 30)    # its sigma = 12 N/s is tuned for 30 steps: longer horizons leave the fp32 range
+    wl = W.replicate(W.ALL[name](K=K, N=N), B, 0.2)
+    if N >= 100:          # two seconds of sigma = 5 N/s rate noise tumble past the stability limit of explicit RK4
+        wl.params["sigma"] = np.float32(1.0)
+    if wl.prev_front is not None:
+        wl.prev_front = np.random.default_rng(2).integers(0, 2, (B, N + 1)).astype(np.int32)
+    m = Pz.make_ctx(wl, variant=4)
+    assert m.info()["block_threads"] == 320 and m.info()["rollout_warps_per_block"] == 5
+    x0, start, u = Pz.to_dev(wl)
+    g = Pz.gpu_step(m, x0, start, u, 9, 2)
+    o = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, 9, 2, want_du=True)
+    o["u_nom"] = wl.u_nom.astype(np.float64)
+    Pz.compare(f"{name} pipe K{K} N{N} B{B}", g, o, wl.params["lambda"], wl.params["objective"] == 0)
+    m2 = Pz.make_ctx(wl, variant=1)
+    g2 = Pz.gpu_step(m2, x0, start, u, 9, 2)
+    np.testing.assert_allclose(g["cost"], g2["cost"], rtol=2e-4, atol=2e-4)
+    g_again = Pz.gpu_step(m, x0, start, u, 9, 2)                  # run-to-run determinism
+    for k in ("cost", "weights", "u_new"):
+        np.testing.assert_array_equal(g[k], g_again[k])
+    m.close(); m2.close()
 
 
 def test_rate_model_contouring_batch_and_warm_start():
@@ -462,7 +493,8 @@ def test_rate_model_contouring_batch_and_warm_start():
 def test_rate_model_rejects_what_it_does_not_support():
     from paper_2509_14726_b200 import binding as Bd
     wl = W.rate_gate_paper(K=64, N=8)
-    for bad in (dict(variant=2), dict(variant=3), dict(variant=4), dict(rate_max=0.0)):
+    for bad in (dict(variant=2), dict(variant=3), dict(variant=4, pipeline=1), dict(variant=4, block_threads=64),
+                dict(variant=4, N=101), dict(rate_max=0.0)):
         with pytest.raises(Bd.MppiError) as e:
             Bd.Mppi(wl.params, **bad)
         assert e.value.status == -2
