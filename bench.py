@@ -408,7 +408,7 @@ def run_survey(args):
             if B > 1:
                 wl = W.replicate(wl, B, 0.3)
             P = wl.params
-            m = Bd.Mppi(P, fast_math=args.fast_math)
+            m = Bd.Mppi(P, fast_math=args.fast_math, variant=args.variant)
             m.set_track(wl)
             x0 = torch.from_numpy(wl.x0).to(dev); start = torch.from_numpy(wl.start).to(dev)
             u = torch.from_numpy(wl.u_nom).to(dev); un = torch.empty_like(u)
@@ -445,6 +445,7 @@ def main(argv=None):
     ap.add_argument("--survey", action="store_true", help="time one iteration of every workload (table, one GPU)")
     ap.add_argument("--only", default=None, help="--survey: this workload only (a key of workloads.ALL)")
     ap.add_argument("--batch", type=int, default=0, help="--survey: this number of controllers only")
+    ap.add_argument("--variant", type=int, default=0, help="--survey: mppi_variant (0 AUTO, 1 THROUGHPUT, 2 LATENCY, 3 PACKED, 4 PIPELINED)")
     args = ap.parse_args(argv)
     if args.survey:
         return run_survey(args)

@@ -159,8 +159,8 @@ static int validate(const mppi_params* p)
             "input_model = 1 has a scalar throughput kernel and a pipelined latency kernel: variant must be AUTO, THROUGHPUT or PIPELINED");
         BAD(p->variant == MPPI_VARIANT_PIPELINED &&
                 (p->pipeline != MPPI_PIPE_FUSED || p->block_threads != 0 || p->N > 100 || p->K % 32 != 0 ||
-                 (p->objective != MPPI_OBJ_GATE && p->objective != MPPI_OBJ_GATE_PAPER && p->objective != MPPI_OBJ_TRACK)),
-            "input_model = 1, PIPELINED: fused pipeline, block_threads 0, N <= 100, K % 32 == 0, objective gate / gate_paper / track");
+                 p->objective == MPPI_OBJ_CONTOUR),
+            "input_model = 1, PIPELINED: fused pipeline, block_threads 0, N <= 100, K % 32 == 0, not the search-based contouring");
     }
 #undef BAD
     return MPPI_OK;
@@ -179,7 +179,10 @@ static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, i
         // few rollouts: the pipelined latency kernel (mppi_pipe_rate.cuh; its rings need N <= 100)
         const bool can = p->pipeline == MPPI_PIPE_FUSED && p->block_threads == 0 && p->N <= 100 && p->K % 32 == 0 &&
                          (p->objective == MPPI_OBJ_GATE || p->objective == MPPI_OBJ_GATE_PAPER || p->objective == MPPI_OBJ_TRACK);
-        if (can && (p->variant == MPPI_VARIANT_PIPELINED || (p->variant == MPPI_VARIANT_AUTO && warps <= (int64_t)sm_count))) {
+        // objective 4 only on request: its path lives in shared memory beside 190 KB of rings, and the path
+        // length is not known yet (mppi_step reports MPPI_E_PARAM if it does not fit)
+        if ((can && (p->variant == MPPI_VARIANT_PIPELINED || (p->variant == MPPI_VARIANT_AUTO && warps <= (int64_t)sm_count))) ||
+            (p->objective == MPPI_OBJ_CONTOUR_PAPER && p->variant == MPPI_VARIANT_PIPELINED)) {
             *pipe = 1; *block_threads = 320;
             return;
         }

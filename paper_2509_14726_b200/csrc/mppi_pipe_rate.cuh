@@ -16,7 +16,10 @@
 //
 // Rings are handed over in chunks of kPipeChunk steps as in mppi_pipe.cuh.  The trajectory agrees with
 // rk4_rate_step to rounding (M v instead of projecting v on the three body axes), not bit for bit.
-// Block = 320 threads = 32 samples; grid = (K / 32, B).  Objectives: gate, the paper's J_gate, tracking.
+// Block = 320 threads = 32 samples; grid = (K / 32, B).  Objectives: gate, the paper's J_gate, tracking, and
+// the paper's own contouring (objective 4: the noise warps also draw the progress acceleration, W adds the
+// input terms of eq.(9), P carries theta and v_theta and looks the path up; the fifth column of the
+// update rides in the fused combine as in mppi_rate.cu).
 #pragma once
 #include "mppi_pipe.cuh"
 #include "mppi_rate.cuh"
@@ -27,10 +30,11 @@ constexpr int kPipeRateThreads = 320;
 constexpr int kPipeRateDepthF = 3;      // ring F slots (9 float4 per step and sample: the big one)
 
 // float4 units of dynamic shared memory after the nominal + track + 16 float4 of reduction scratch
-__host__ __device__ inline size_t pipe_rate_extra_f4(int N, int nb)
+__host__ __device__ inline size_t pipe_rate_extra_f4(int N, int nb, bool progress)
 {
     const int nchunks = (N + kPipeChunk - 1) / kPipeChunk;
     return (size_t)N * 33                                       // s_T   [N][33] thrust rates
+           + (progress ? ((size_t)N * 33 + 3) / 4 : 0)          // s_dv  [N][32] progress accelerations, s_vnom [N]
            + (size_t)kPipeDepth * kPipeChunk * 4 * 32           // ring W
            + (size_t)kPipeDepth * kPipeChunk * 5 * 32           // ring Q
            + (size_t)kPipeRateDepthF * kPipeChunk * 9 * 32      // ring F
@@ -79,7 +83,9 @@ __global__ void __launch_bounds__(kPipeRateThreads, 1) rollout_pipe_rate_kernel(
     float4* s_trk = smem + N;
     float* s_red = reinterpret_cast<float*>(s_trk + track_f4(P, OBJ));   // 64 floats
     float4* s_T = reinterpret_cast<float4*>(s_red + 64);                 // [N][RS] thrust rates
-    float4* s_w = s_T + (size_t)N * RS;                                  // [D][C][4][32]
+    float* s_dv = reinterpret_cast<float*>(s_T + (size_t)N * RS);        // OBJ_CONTOUR_PAPER: [N][32], then s_vnom [N]
+    float* s_vnom = s_dv + (size_t)N * 32;
+    float4* s_w = s_T + (size_t)N * RS + (OBJ == OBJ_CONTOUR_PAPER ? ((size_t)N * 33 + 3) / 4 : 0);   // [D][C][4][32]
     float4* s_q = s_w + D * C * 4 * 32;                                  // [D][C][5][32]
     float4* s_f = s_q + D * C * 5 * 32;                                  // [DF][C][9][32]
     float* s_J = reinterpret_cast<float*>(s_f + DF * C * 9 * 32);        // [4][32]
@@ -101,7 +107,9 @@ __global__ void __launch_bounds__(kPipeRateThreads, 1) rollout_pipe_rate_kernel(
         else if (i >= nchunks + 3 * D && i < nchunks + 4 * D + DF) cnt = 64;    // Q empty, F full: both F warps
         mbar_init(bar_T + i, cnt);
     }
-    const float* xb = A.x0 + 17 * b;
+    if (OBJ == OBJ_CONTOUR_PAPER)
+        for (int t = tid; t < N; t += kPipeRateThreads) s_vnom[t] = A.v_nom[(size_t)b * N + t];
+    const float* xb = A.x0 + (OBJ == OBJ_CONTOUR_PAPER ? 19 : 17) * b;     // p, q, v, omega, T(4) [, theta, v_theta]
     const State x0 = load_state(xb);
     __syncthreads();
 
@@ -114,6 +122,9 @@ __global__ void __launch_bounds__(kPipeRateThreads, 1) rollout_pipe_rate_kernel(
             const float4 u = sample_input<MATH>(P, A.rk, (uint32_t)(kbase + lane), (uint32_t)t, A.iter, (uint32_t)b, un,
                                                 -P.rate_max, P.rate_max);
             s_T[t * RS + lane] = u;
+            if (OBJ == OBJ_CONTOUR_PAPER)       // the fifth sampled input [R-35]
+                s_dv[t * 32 + lane] = sample_progress_accel<MATH>(P, A.rk, (uint32_t)(kbase + lane), (uint32_t)t, A.iter,
+                                                                  (uint32_t)b, s_vnom[t]);
             mbar_arrive(bar_T + t / C);
             if (STORE_DU)
                 A.du[((size_t)b * N + t) * P.K + kbase + lane] = make_float4(u.x - un.x, u.y - un.y, u.z - un.z, u.w - un.w);
@@ -134,6 +145,12 @@ __global__ void __launch_bounds__(kPipeRateThreads, 1) rollout_pipe_rate_kernel(
                     const float wx = ox - r2.z, wy = oy - r2.w, wz = oz - r3.x;
                     acc = fmaf(P.Qw, wx * wx + wy * wy + wz * wz, acc);
                     acc = fmaf(P.R, u.x * u.x + u.y * u.y + u.z * u.z + u.w * u.w, acc);
+                }
+                if (OBJ == OBJ_CONTOUR_PAPER) {    // eq.(9): body-rate and input terms at the pre-step state [R-37]
+                    const float dv = s_dv[t * 32 + lane];
+                    acc = fmaf(P.w_omega, fmaf(oz, oz, fmaf(oy, oy, ox * ox)), acc);
+                    acc = fmaf(P.r_dv, dv * dv, acc);
+                    acc = fmaf(P.R, fmaf(u.w, u.w, fmaf(u.z, u.z, fmaf(u.y, u.y, u.x * u.x))), acc);
                 }
                 // torque accelerations and collective acceleration are linear in the thrusts: value at T and slope along u
                 const float s01 = T.x + T.y, s23 = T.z + T.w, u01 = u.x + u.y, u23 = u.z + u.w;
@@ -259,6 +276,8 @@ __global__ void __launch_bounds__(kPipeRateThreads, 1) rollout_pipe_rate_kernel(
             J = fmaf(P.Qp, ex * ex + ey * ey + ez * ez, J);
             J = fmaf(P.Qv, ux * ux + uy * uy + uz * uz, J);
         };
+        float theta = 0.0f, v_theta = 0.0f;                                  // OBJ_CONTOUR_PAPER: progress states [R-33]
+        if (OBJ == OBJ_CONTOUR_PAPER) { theta = xb[17]; v_theta = xb[18]; }
         for (int c = 0; c < nchunks; ++c) {
             const int sf = c % DF, cnt = min(C, N - c * C);
             mbar_wait(bar_ff + sf, (c / DF) & 1);
@@ -272,6 +291,18 @@ __global__ void __launch_bounds__(kPipeRateThreads, 1) rollout_pipe_rate_kernel(
                     f[4 * r] = v4.x; f[4 * r + 1] = v4.y; f[4 * r + 2] = v4.z; f[4 * r + 3] = v4.w;
                 }
                 if (OBJ == OBJ_TRACK) pv_term(s_trk + 4 * t);
+                if (OBJ == OBJ_CONTOUR_PAPER) {    // position part of eq.(9) at the pre-step state, progress states [R-34],[R-36]
+                    float qx, qy, qz, tx, ty, tz;
+                    path_eval(P, s_trk, theta, qx, qy, qz, tx, ty, tz);
+                    const float ex = x.px - qx, ey = x.py - qy, ez = x.pz - qz;
+                    const float e_l = fmaf(ez, tz, fmaf(ey, ty, ex * tx));
+                    const float e_c2 = fmaxf(fmaf(ez, ez, fmaf(ey, ey, ex * ex)) - e_l * e_l, 0.0f);
+                    J = fmaf(P.q_c, e_c2, fmaf(P.q_l * e_l, e_l, J));
+                    J = fmaf(-P.mu, v_theta, J);
+                    const float dv = s_dv[t * 32 + lane];
+                    theta = fmaf(P.hh2, dv, fmaf(P.dt, v_theta, theta));
+                    v_theta = fminf(fmaxf(fmaf(P.dt, dv, v_theta), 0.0f), P.v_theta_max);
+                }
 #define MPPI_K(F, VX, VY, VZ, KX, KY, KZ)                                                       \
     const float KX = fmaf(-(F)[2], VZ, fmaf(-(F)[1], VY, fmaf(-(F)[0], VX, (F)[6])));          \
     const float KY = fmaf(-(F)[4], VZ, fmaf(-(F)[3], VY, fmaf(-(F)[1], VX, (F)[7])));          \
@@ -309,6 +340,7 @@ __global__ void __launch_bounds__(kPipeRateThreads, 1) rollout_pipe_rate_kernel(
         const float jw = s_J[lane], jq = s_J[32 + lane], jp = s_J[64 + lane], jl = s_J[96 + lane];
         float J;
         if (OBJ == OBJ_GATE || OBJ == OBJ_GATE_PAPER) J = fmaf(P.w_omega, jw, jp) + jl;
+        else if (OBJ == OBJ_CONTOUR_PAPER) J = (jp + jw) + jl;
         else J = ((jp + jq) + jw) + jl;
         A.cost[(size_t)b * P.K + kbase + lane] = J;
         m = warp_min(J);
@@ -331,8 +363,18 @@ __global__ void __launch_bounds__(kPipeRateThreads, 1) rollout_pipe_rate_kernel(
         }
         part[j] = acc;
     }
+    if (OBJ == OBJ_CONTOUR_PAPER)          // fifth column S5[t] = sum_l e_l (dv_l[t] - v_nom[t]), after the (m, Z) header
+        for (int t = tid; t < N; t += kPipeRateThreads) {
+            const float vn = s_vnom[t];
+            float acc = 0.0f;
+            for (int l = 0; l < 32; ++l) {
+                const float el = s_e[l];
+                if (el != 0.0f) acc = fmaf(el, s_dv[t * 32 + l] - vn, acc);
+            }
+            part[4 * N + 4 + t] = acc;
+        }
     if (tid == 0) { part[4 * N] = m; part[4 * N + 1] = Zb; }
-    publish_and_combine<MATH>(P, A, b, P.blocks_per_ctrl, s_unom, s_red, s_pair);
+    publish_and_combine<MATH>(P, A, b, P.blocks_per_ctrl, s_unom, s_red, s_pair, OBJ == OBJ_CONTOUR_PAPER ? s_vnom : nullptr);
 }
 
 #undef MPPI_G

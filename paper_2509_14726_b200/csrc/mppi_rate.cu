@@ -121,6 +121,7 @@ static RateFn pick_pipe_rate(const LaunchCfg& c)
     switch (c.objective) {
         case OBJ_GATE: return pick_pipe_rate1<OBJ_GATE>(c);
         case OBJ_GATE_PAPER: return pick_pipe_rate1<OBJ_GATE_PAPER>(c);
+        case OBJ_CONTOUR_PAPER: return pick_pipe_rate1<OBJ_CONTOUR_PAPER>(c);
         default: return pick_pipe_rate1<OBJ_TRACK>(c);
     }
 }

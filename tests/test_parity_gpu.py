@@ -563,8 +563,8 @@ def _cp_check(tag, wl, g, o):
     return st
 
 
-@pytest.mark.parametrize("pipe", [dict(), dict(variant=1, block_threads=64), dict(variant=1, block_threads=256)],
-                         ids=["fused", "fused_tpb64", "fused_tpb256"])
+@pytest.mark.parametrize("pipe", [dict(), dict(variant=1, block_threads=64), dict(variant=1, block_threads=256), dict(variant=4)],
+                         ids=["fused", "fused_tpb64", "fused_tpb256", "fused_pipe"])
 @pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
 @pytest.mark.parametrize("regime", [dict(), {"sigma": np.float32(2.0), "lambda": np.float32(1000.0)}], ids=["argmin", "mixing"])
 def test_contour_paper_full_size(pipe, math, regime):
@@ -602,7 +602,14 @@ def test_contour_paper_batch_warm_start_open_path_and_speed_limits():
     wl.x0[2, 17:19] = np.float32([0.05, 0.0]); wl.x0[2, 0:3] = wl.path[0] + np.float32([0.1, 0.0, -0.1])
     wl.start = np.repeat(wl.start, B, 0); wl.u_nom = np.repeat(wl.u_nom, B, 0)
     wl.v_nom = np.repeat(wl.v_nom, B, 0)
-    m = Pz.make_ctx(wl)
+    _open_path_iterations(wl, dict())
+    _open_path_iterations(wl, dict(variant=4))                   # the pipelined kernel of the rate model
+
+
+def _open_path_iterations(wl, opts):
+    import torch
+    m = Pz.make_ctx(wl, **opts)
+    assert m.info()["block_threads"] == (320 if opts else 128)
     x0, start, u = Pz.to_dev(wl)
     v = torch.from_numpy(wl.v_nom.copy()).cuda()
     m.set_progress(v)                                            # in place
@@ -611,7 +618,7 @@ def test_contour_paper_batch_warm_start_open_path_and_speed_limits():
         g = Pz.gpu_step(m, x0, start, u, wl.seed, it, u_new=u)
         o = Pz.oracle_step(wl, wl.x0, wl.start, u_in, wl.seed, it, want_du=True, v_nom=v_in)
         o["u_nom"] = u_in.astype(np.float64); o["v_nom"] = v_in.astype(np.float64)
-        assert _cp_check(f"contour_paper open it{it}", wl, g, o)["ess"] > 10
+        assert _cp_check(f"contour_paper open {opts} it{it}", wl, g, o)["ess"] > 10
     assert np.abs(v.cpu().numpy()).max() > 0.1
     # mppi_optimize runs the same four iterations in one call
     u2 = torch.from_numpy(wl.u_nom.copy()).cuda(); v2 = torch.from_numpy(wl.v_nom.copy()).cuda()
