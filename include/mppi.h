@@ -98,8 +98,9 @@ typedef enum {
                                     input_model = 1: 320-thread blocks, five chains (thrust states + body
                                     rates, attitude, two warps for the drag matrices of the RK4 stages,
                                     velocity / position); N <= 100, every objective but the search-based
-                                    contouring; MPPI_OBJ_CONTOUR_PAPER only on request (the path must fit
-                                    in shared memory beside the rings, else mppi_step -> MPPI_E_PARAM)      */
+                                    contouring; under MPPI_OBJ_CONTOUR_PAPER the path must fit in shared memory
+                                    beside the rings (else mppi_step -> MPPI_E_PARAM; AUTO then stays on the
+                                    throughput kernel)                                                      */
     MPPI_VARIANT_PACKED = 3      /* throughput kernel with TWO samples per thread held in packed fp32x2
                                     registers (sm_100a FFMA2); needs K % 64 == 0; costs are bit-identical
                                     to MPPI_VARIANT_THROUGHPUT                                             */

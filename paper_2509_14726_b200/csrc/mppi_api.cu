@@ -27,6 +27,7 @@ struct mppi_ctx {
     DevParams dp;
     LaunchCfg cfg;
     int device = 0, sm_count = 0, l2_bytes = 0;
+    int lazy_pipe = 0, scalar_tpb = 0;     // objective 4 under AUTO: pipelined kernel iff the path fits (decided in prepare)
     bool have_gates = false, have_ref = false, have_path = false;
     float4* d_gates = nullptr;
     float4* d_ref = nullptr;
@@ -309,6 +310,13 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
                                           : p->K / (cfg.block_threads * (cfg.packed ? 2 : 1));
     d.part_stride = 4 * p->N + 4 + (p->objective == MPPI_OBJ_CONTOUR_PAPER ? ((p->N + 3) & ~3) : 0);
     cfg.smem_bytes = 0;   // fixed once the track is known
+    // objective 4, lone controller, AUTO: the pipelined kernel is the faster one (34.9 vs 57.4 us) but its path
+    // must fit in shared memory beside the rings, and the path is not known yet: keep the scalar shape, size
+    // the partials for either, and let prepare() switch once mppi_set_path has been called
+    c->scalar_tpb = cfg.block_threads;
+    c->lazy_pipe = p->objective == MPPI_OBJ_CONTOUR_PAPER && p->variant == MPPI_VARIANT_AUTO && !cfg.pipe && cfg.fused &&
+                   p->block_threads == 0 && p->N <= 100 && p->K % 32 == 0 && (int64_t)p->B * p->K / 32 <= c->sm_count;
+    const int max_blocks = c->lazy_pipe ? p->K / 32 : d.blocks_per_ctrl;
 
     const size_t BN4 = (size_t)p->B * p->N * 4, BK = (size_t)p->B * p->K;
 #define CKC(call)                                                        \
@@ -322,7 +330,7 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     } while (0)
     if (cfg.store_du) CKC(dev_alloc(c, &c->d_du, (size_t)p->B * p->N * p->K));
     if (cfg.fused) {
-        CKC(dev_alloc(c, &c->d_partials, (size_t)p->B * d.blocks_per_ctrl * d.part_stride));
+        CKC(dev_alloc(c, &c->d_partials, (size_t)p->B * max_blocks * d.part_stride));
         CKC(dev_alloc(c, &c->d_counters, (size_t)p->B + 1));
         CKC(cudaMemset(c->d_counters, 0, ((size_t)p->B + 1) * sizeof(unsigned)));
     }
@@ -476,6 +484,17 @@ static int prepare(mppi_ctx* c)
         return fail(c, MPPI_E_NO_TRACK, "mppi_set_gates / mppi_set_reference / mppi_set_path not called for this objective");
     if (obj == MPPI_OBJ_CONTOUR_PAPER && (!c->d_v_nom || !c->d_v_new))
         return fail(c, MPPI_E_NO_TRACK, "mppi_set_progress not called (MPPI_OBJ_CONTOUR_PAPER)");
+    if (c->lazy_pipe) {
+        LaunchCfg pc = c->cfg; pc.pipe = 1; pc.block_threads = 320;
+        DevParams pd = c->dp; pd.blocks_per_ctrl = c->prm.K / 32;
+        const bool fits = rollout_smem_bytes(pd, pc) <= 227 * 1024;
+        if (fits != (c->cfg.pipe == 1)) {
+            c->cfg.pipe = fits ? 1 : 0;
+            c->cfg.block_threads = fits ? 320 : c->scalar_tpb;
+            c->dp.blocks_per_ctrl = fits ? c->prm.K / 32 : c->prm.K / c->scalar_tpb;
+            c->cfg.smem_bytes = 0;
+        }
+    }
     const size_t need = rollout_smem_bytes(c->dp, c->cfg);
     if (need != c->cfg.smem_bytes) {
         if (need > 227 * 1024) return fail(c, MPPI_E_PARAM, "track + horizon do not fit in shared memory");

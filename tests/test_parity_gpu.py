@@ -563,8 +563,8 @@ def _cp_check(tag, wl, g, o):
     return st
 
 
-@pytest.mark.parametrize("pipe", [dict(), dict(variant=1, block_threads=64), dict(variant=1, block_threads=256), dict(variant=4)],
-                         ids=["fused", "fused_tpb64", "fused_tpb256", "fused_pipe"])
+@pytest.mark.parametrize("pipe", [dict(variant=1), dict(variant=1, block_threads=64), dict(variant=1, block_threads=256), dict(variant=4), dict()],
+                         ids=["fused", "fused_tpb64", "fused_tpb256", "fused_pipe", "auto"])
 @pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
 @pytest.mark.parametrize("regime", [dict(), {"sigma": np.float32(2.0), "lambda": np.float32(1000.0)}], ids=["argmin", "mixing"])
 def test_contour_paper_full_size(pipe, math, regime):
@@ -602,14 +602,13 @@ def test_contour_paper_batch_warm_start_open_path_and_speed_limits():
     wl.x0[2, 17:19] = np.float32([0.05, 0.0]); wl.x0[2, 0:3] = wl.path[0] + np.float32([0.1, 0.0, -0.1])
     wl.start = np.repeat(wl.start, B, 0); wl.u_nom = np.repeat(wl.u_nom, B, 0)
     wl.v_nom = np.repeat(wl.v_nom, B, 0)
-    _open_path_iterations(wl, dict())
-    _open_path_iterations(wl, dict(variant=4))                   # the pipelined kernel of the rate model
+    _open_path_iterations(wl, dict(variant=1), 128)              # scalar kernel of the rate model
+    _open_path_iterations(wl, dict(), 320)                       # AUTO: 96 warps, the path fits -> the pipelined kernel
 
 
-def _open_path_iterations(wl, opts):
+def _open_path_iterations(wl, opts, threads):
     import torch
     m = Pz.make_ctx(wl, **opts)
-    assert m.info()["block_threads"] == (320 if opts else 128)
     x0, start, u = Pz.to_dev(wl)
     v = torch.from_numpy(wl.v_nom.copy()).cuda()
     m.set_progress(v)                                            # in place
@@ -627,6 +626,31 @@ def _open_path_iterations(wl, opts):
     np.testing.assert_array_equal(u2.cpu().numpy(), u.cpu().numpy())
     np.testing.assert_array_equal(v2.cpu().numpy(), v.cpu().numpy())
     assert m.info()["kernels_per_step"] == 1                     # the fifth column rides in the fused update
+    assert m.info()["block_threads"] == threads
+    m.close()
+
+
+def test_contour_paper_auto_falls_back_when_the_path_does_not_fit():
+    # AUTO takes the pipelined kernel for a lone controller only if the path fits in shared memory beside its rings:
+    # 500 points do, 1800 do not (-> scalar kernel); an explicit PIPELINED request then fails with MPPI_E_PARAM
+    from paper_2509_14726_b200 import binding as Bd
+    wl = W.contour_paper(K=256, N=20)
+    long_path = W.spline_path(W.circle_gates()[:, 0:3], 1800)
+    for path, threads in ((wl.path, 320), (long_path, 128)):
+        wl.path = path
+        m = Pz.make_ctx(wl)
+        x0, start, u = Pz.to_dev(wl)
+        g = Pz.gpu_step(m, x0, start, u, 4, 1)
+        assert m.info()["block_threads"] == threads
+        o = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, 4, 1, want_du=True, v_nom=wl.v_nom)
+        o["u_nom"] = wl.u_nom.astype(np.float64); o["v_nom"] = wl.v_nom.astype(np.float64)
+        _cp_check(f"contour_paper auto P{len(path)}", wl, g, o)
+        m.close()
+    m = Pz.make_ctx(wl, variant=4)
+    x0, start, u = Pz.to_dev(wl)
+    with pytest.raises(Bd.MppiError) as e:
+        m.step(x0, start, u, 4, 1)
+    assert e.value.status == -2
     m.close()
 
 
