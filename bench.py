@@ -399,7 +399,8 @@ def run_survey(args):
     dev = torch.device("cuda", 0)
     torch.cuda.set_device(dev)
     flush_buf = torch.empty(L2_FLUSH_BYTES // 4, dtype=torch.float32, device=dev)
-    names = ["cfg0", "cfg1", "cfg2", "cfg3", "gate_paper", "rate_gate_paper", "rate_track", "contour_paper"]
+    names = ["cfg0", "cfg1", "cfg2", "cfg3", "gate_paper", "rate_gate_paper", "rate_track", "contour_paper",
+             "table1_gate", "table1_contour"]
     print("| workload | objective | input model | K | N | B | kernel | launches / iteration | us / iteration | sample-steps/s |")
     print("|---|---|---|---|---|---|---|---|---|---|")
     for name in ([args.only] if args.only else names):

@@ -340,6 +340,18 @@ def lap(kind="gate", B=8, K=4096, N=50, steps=1500) -> Workload:
                     np.repeat(base.u_nom, B, 0), ref=base.ref, path=base.path, closed=base.closed, seed=0, iters=steps)
 
 
+def table1(kind="gate") -> Workload:
+    """The sizes of the paper's own Table I: M = 8192 samples, horizon K = 20 steps of
+    dt = 0.03 s, lambda = 0.01, thrust-rate inputs in [-10, 10] N/s, thrusts in [0, 10] N, body rates limited
+    to 10 rad/s, (contouring) progress acceleration in [-20, 20], v_theta in [0, 10] -- on the synthetic circle
+    track / its spline path, under the paper's J_gate ("gate") or the paper's contouring ("contour")."""
+    wl = rate_gate_paper(K=8192, N=20) if kind == "gate" else contour_paper(K=8192, N=20)
+    wl.params.update(dt=_f32(0.03))
+    wl.params["lambda"] = _f32(0.01)
+    wl.name = f"table1_{kind}_M8192_K20"
+    return wl
+
+
 def replicate(wl: Workload, B: int, jitter: float = 0.0) -> Workload:
     """The same single-controller workload for B controllers (positions jittered by +-jitter m, seeded)."""
     rng = np.random.default_rng(11)
@@ -352,6 +364,6 @@ def replicate(wl: Workload, B: int, jitter: float = 0.0) -> Workload:
                     iters=wl.iters)
 
 
-ALL = {"contour_paper": contour_paper, "rate_gate_paper": rate_gate_paper, "rate_track": rate_track, "rate_stress": rate_stress,
+ALL = {"table1_gate": lambda: table1("gate"), "table1_contour": lambda: table1("contour"), "contour_paper": contour_paper, "rate_gate_paper": rate_gate_paper, "rate_track": rate_track, "rate_stress": rate_stress,
        "gate_paper": gate_paper, "stress_gate_paper": stress_gate_paper, "cfg0": cfg0, "cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg4": cfg4,
        "stress_gate": stress_gate}

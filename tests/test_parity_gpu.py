@@ -630,6 +630,31 @@ def _open_path_iterations(wl, opts, threads):
     m.close()
 
 
+def test_table1_sizes():
+    # the sizes of the paper's own Table I (M = 8192, K = 20, dt = 0.03, lambda = 0.01) under the paper's J_gate
+    # and the paper's contouring, thrust-rate model
+    # [R-38] the squared progress of eq.(6) is a difference of squared distances to the target: costs near 0
+    # carry the fp32 error of parts of size |p_0 - c|^2, which is therefore the floor of the relative bound
+    wl = W.table1("gate")
+    m = Pz.make_ctx(wl)
+    x0, start, u = Pz.to_dev(wl)
+    g = Pz.gpu_step(m, x0, start, u, wl.seed, 0)
+    o = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, wl.seed, 0, want_du=True)
+    o["u_nom"] = wl.u_nom.astype(np.float64)
+    d2 = float(np.sum((wl.x0[0, 0:3].astype(np.float64) - wl.gates[int(wl.start[0]), 0:3]) ** 2))
+    assert d2 > 1.0
+    Pz.compare("table1_gate", g, o, wl.params["lambda"], False, cost_floor=d2)
+    m.close()
+    wl = W.table1("contour")
+    m = Pz.make_ctx(wl)
+    x0, start, u = Pz.to_dev(wl)
+    g = Pz.gpu_step(m, x0, start, u, wl.seed, 0)
+    o = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, wl.seed, 0, want_du=True, v_nom=wl.v_nom)
+    o["u_nom"] = wl.u_nom.astype(np.float64); o["v_nom"] = wl.v_nom.astype(np.float64)
+    _cp_check("table1_contour", wl, g, o)
+    m.close()
+
+
 def test_contour_paper_auto_falls_back_when_the_path_does_not_fit():
     # AUTO takes the pipelined kernel for a lone controller only if the path fits in shared memory beside its rings:
     # 500 points do, 1800 do not (-> scalar kernel); an explicit PIPELINED request then fails with MPPI_E_PARAM
