@@ -27,7 +27,7 @@ struct mppi_ctx {
     DevParams dp;
     LaunchCfg cfg;
     int device = 0, sm_count = 0, l2_bytes = 0;
-    int lazy_pipe = 0, scalar_tpb = 0;     // objective 4 under AUTO: pipelined kernel iff the path fits (decided in prepare)
+    int lazy_pipe = 0, scalar_tpb = 0;     // input_model = 1: pipelined kernel iff it fits in shared memory (decided in prepare)
     bool have_gates = false, have_ref = false, have_path = false;
     float4* d_gates = nullptr;
     float4* d_ref = nullptr;
@@ -170,6 +170,16 @@ static int validate(const mppi_params* p)
 // Launch shape.  Latency variant: C rollout warps per 256-thread block, the smallest C in {1,2,4}
 // that brings the grid down to one block per SM (so every rollout warp owns a scheduler).
 // Throughput variant: 256-thread blocks when the grid still covers the chip several times, else 128.
+// input_model = 1: may the pipelined latency kernel (mppi_pipe_rate.cuh) run this configuration at all?
+static bool rate_pipe_candidate(const mppi_params* p, int sm_count)
+{
+    if (p->input_model != 1 || p->pipeline != MPPI_PIPE_FUSED || p->block_threads != 0 || p->N > 100 || p->K % 32 != 0 ||
+        p->objective == MPPI_OBJ_CONTOUR || p->use_graph)
+        return false;
+    if (p->variant == MPPI_VARIANT_PIPELINED) return true;
+    return p->variant == MPPI_VARIANT_AUTO && (int64_t)p->B * p->K / 32 <= 2 * (int64_t)sm_count;
+}
+
 static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, int* lat_consumers, int* packed, int* pipe)
 {
     const int64_t warps = (int64_t)p->B * p->K / 32;
@@ -177,16 +187,8 @@ static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, i
     *packed = 0;
     *pipe = 0;
     if (p->input_model == 1) {                     // thrust-rate model: its own kernels (mppi_rate.cu)
-        // few rollouts: the pipelined latency kernel (mppi_pipe_rate.cuh; its rings need N <= 100)
-        const bool can = p->pipeline == MPPI_PIPE_FUSED && p->block_threads == 0 && p->N <= 100 && p->K % 32 == 0 &&
-                         (p->objective == MPPI_OBJ_GATE || p->objective == MPPI_OBJ_GATE_PAPER || p->objective == MPPI_OBJ_TRACK);
-        // objective 4 only on request: its path lives in shared memory beside 190 KB of rings, and the path
-        // length is not known yet (mppi_step reports MPPI_E_PARAM if it does not fit)
-        if ((can && (p->variant == MPPI_VARIANT_PIPELINED || (p->variant == MPPI_VARIANT_AUTO && warps <= (int64_t)sm_count))) ||
-            (p->objective == MPPI_OBJ_CONTOUR_PAPER && p->variant == MPPI_VARIANT_PIPELINED)) {
-            *pipe = 1; *block_threads = 320;
-            return;
-        }
+        // the scalar shape; whether the pipelined latency kernel takes over is decided in prepare(), once the
+        // track (and with it the shared-memory footprint) is known -- see rate_pipe_candidate
         if (p->block_threads) { *block_threads = p->block_threads; return; }
         for (int tpb : {128, 64, 32})
             if (p->K % tpb == 0) { *block_threads = tpb; return; }
@@ -310,12 +312,12 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
                                           : p->K / (cfg.block_threads * (cfg.packed ? 2 : 1));
     d.part_stride = 4 * p->N + 4 + (p->objective == MPPI_OBJ_CONTOUR_PAPER ? ((p->N + 3) & ~3) : 0);
     cfg.smem_bytes = 0;   // fixed once the track is known
-    // objective 4, lone controller, AUTO: the pipelined kernel is the faster one (34.9 vs 57.4 us) but its path
-    // must fit in shared memory beside the rings, and the path is not known yet: keep the scalar shape, size
-    // the partials for either, and let prepare() switch once mppi_set_path has been called
+    // input_model = 1: the pipelined latency kernel is the faster one for few rollouts, but its rings share the
+    // shared memory with the track, which is not known yet: keep the scalar shape, size the partials for
+    // either, and let prepare() switch once the track has been set
     c->scalar_tpb = cfg.block_threads;
-    c->lazy_pipe = p->objective == MPPI_OBJ_CONTOUR_PAPER && p->variant == MPPI_VARIANT_AUTO && !cfg.pipe && cfg.fused &&
-                   p->block_threads == 0 && p->N <= 100 && p->K % 32 == 0 && (int64_t)p->B * p->K / 32 <= c->sm_count;
+    c->lazy_pipe = rate_pipe_candidate(p, c->sm_count) ? 1 : 0;
+    d.pipe_d = 4; d.pipe_df = 3;
     const int max_blocks = c->lazy_pipe ? p->K / 32 : d.blocks_per_ctrl;
 
     const size_t BN4 = (size_t)p->B * p->N * 4, BK = (size_t)p->B * p->K;
@@ -485,13 +487,27 @@ static int prepare(mppi_ctx* c)
     if (obj == MPPI_OBJ_CONTOUR_PAPER && (!c->d_v_nom || !c->d_v_new))
         return fail(c, MPPI_E_NO_TRACK, "mppi_set_progress not called (MPPI_OBJ_CONTOUR_PAPER)");
     if (c->lazy_pipe) {
+        // deep rings (4, 3) with at most one block per SM, or shallow rings (2, 2) and two blocks per SM for
+        // grids up to twice the SM count; an explicit PIPELINED request takes whichever fits
+        const bool force = c->prm.variant == MPPI_VARIANT_PIPELINED;
+        const int64_t grid = (int64_t)c->prm.B * c->prm.K / 32;
         LaunchCfg pc = c->cfg; pc.pipe = 1; pc.block_threads = 320;
         DevParams pd = c->dp; pd.blocks_per_ctrl = c->prm.K / 32;
-        const bool fits = rollout_smem_bytes(pd, pc) <= 227 * 1024;
-        if (fits != (c->cfg.pipe == 1)) {
-            c->cfg.pipe = fits ? 1 : 0;
-            c->cfg.block_threads = fits ? 320 : c->scalar_tpb;
-            c->dp.blocks_per_ctrl = fits ? c->prm.K / 32 : c->prm.K / c->scalar_tpb;
+        int use_d = 0, use_df = 0;
+        pd.pipe_d = 4; pd.pipe_df = 3;
+        const bool deep = rollout_smem_bytes(pd, pc) <= 227 * 1024;
+        pd.pipe_d = 2; pd.pipe_df = 2;
+        const bool shallow2 = 2 * (rollout_smem_bytes(pd, pc) + 1024) <= 228 * 1024;
+        if (deep && (grid <= c->sm_count || (force && !shallow2))) { use_d = 4; use_df = 3; }
+        else if (shallow2 && (grid <= 2 * (int64_t)c->sm_count || force)) { use_d = 2; use_df = 2; }
+        else if (deep && force) { use_d = 4; use_df = 3; }
+        if (force && !use_d) return fail(c, MPPI_E_PARAM, "PIPELINED: track + horizon do not fit in shared memory beside the rings");
+        const bool on = use_d != 0;
+        if (on != (c->cfg.pipe == 1) || (on && (c->dp.pipe_d != use_d || c->dp.pipe_df != use_df))) {
+            c->cfg.pipe = on ? 1 : 0;
+            c->cfg.block_threads = on ? 320 : c->scalar_tpb;
+            c->dp.blocks_per_ctrl = on ? c->prm.K / 32 : c->prm.K / c->scalar_tpb;
+            if (on) { c->dp.pipe_d = use_d; c->dp.pipe_df = use_df; }
             c->cfg.smem_bytes = 0;
         }
     }

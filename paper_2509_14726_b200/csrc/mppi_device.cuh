@@ -14,6 +14,7 @@ struct DevParams {
     int K, N, B;
     int G, M, P, closed, window;      // gates, reference rows, path points
     int blocks_per_ctrl;               // rollout blocks per controller = K / blockDim.x
+    int pipe_d, pipe_df;               // rollout_pipe_rate_kernel: ring depths in chunks (W / Q rings, F ring)
     int part_stride;                   // floats per partial: 4N + 4 (+ N rounded up to 4 under OBJ_CONTOUR_PAPER)
     float dt, inv_lambda, sigma, T_min, T_max;
     float h2, h3, h4, h6, h12, hh2, hh3;   // dt/2, dt/3, dt/4, dt/6, dt/12, dt^2/2, dt^2/3

@@ -26,7 +26,7 @@ namespace mppi {
 size_t rollout_smem_bytes(const DevParams& P, const LaunchCfg& c)
 {
     size_t f4 = (size_t)P.N + track_f4(P, c.objective) + 16;
-    if (c.pipe) return (f4 + (c.rate ? pipe_rate_extra_f4(P.N, P.blocks_per_ctrl, c.objective == OBJ_CONTOUR_PAPER) : pipe_extra_f4(P.N, P.blocks_per_ctrl))) * sizeof(float4);
+    if (c.pipe) return (f4 + (c.rate ? pipe_rate_extra_f4(P.N, P.blocks_per_ctrl, c.objective == OBJ_CONTOUR_PAPER, P.pipe_d, P.pipe_df) : pipe_extra_f4(P.N, P.blocks_per_ctrl))) * sizeof(float4);
     if (c.lat_consumers > 0) {
         f4 += (size_t)P.N * (32 * c.lat_consumers + 1) + 32 + (3 * P.blocks_per_ctrl + 3) / 4;
         return f4 * sizeof(float4);

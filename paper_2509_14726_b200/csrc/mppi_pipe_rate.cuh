@@ -27,20 +27,22 @@
 namespace mppi {
 
 constexpr int kPipeRateThreads = 320;
-constexpr int kPipeRateDepthF = 3;      // ring F slots (9 float4 per step and sample: the big one)
+// ring depths (chunks in flight) are launch parameters: (4, 3) when the grid is at most one block per SM
+// (190 KB at N = 50), (2, 2) so that two blocks share an SM when the grid is up to twice the SM count
+// (short horizons: the paper's Table I sizes, M = 8192, K = 20)
 
 // float4 units of dynamic shared memory after the nominal + track + 16 float4 of reduction scratch
-__host__ __device__ inline size_t pipe_rate_extra_f4(int N, int nb, bool progress)
+__host__ __device__ inline size_t pipe_rate_extra_f4(int N, int nb, bool progress, int d, int df)
 {
     const int nchunks = (N + kPipeChunk - 1) / kPipeChunk;
     return (size_t)N * 33                                       // s_T   [N][33] thrust rates
            + (progress ? ((size_t)N * 33 + 3) / 4 : 0)          // s_dv  [N][32] progress accelerations, s_vnom [N]
-           + (size_t)kPipeDepth * kPipeChunk * 4 * 32           // ring W
-           + (size_t)kPipeDepth * kPipeChunk * 5 * 32           // ring Q
-           + (size_t)kPipeRateDepthF * kPipeChunk * 9 * 32      // ring F
+           + (size_t)d * kPipeChunk * 4 * 32                    // ring W
+           + (size_t)d * kPipeChunk * 5 * 32                    // ring Q
+           + (size_t)df * kPipeChunk * 9 * 32                   // ring F
            + 32 + 8                                             // s_J [4][32], s_e [32]
            + (size_t)(3 * nb + 3) / 4                           // combine scratch
-           + (size_t)(nchunks + 4 * kPipeDepth + 2 * kPipeRateDepthF + 1) / 2;    // mbarriers (8 B each)
+           + (size_t)(nchunks + 4 * d + 2 * df + 1) / 2;        // mbarriers (8 B each)
 }
 
 #define MPPI_G(QW, QX, QY, QZ, OX, OY, OZ, GW, GX, GY, GZ)                 \
@@ -70,12 +72,13 @@ __device__ __forceinline__ void stage_force(const DevParams& P, const float4 q /
 }
 
 template <int OBJ, int MATH, bool STORE_DU>
-__global__ void __launch_bounds__(kPipeRateThreads, 1) rollout_pipe_rate_kernel(const DevParams P, const StepArgs A)
+__global__ void __launch_bounds__(kPipeRateThreads, 2) rollout_pipe_rate_kernel(const DevParams P, const StepArgs A)
 {
     extern __shared__ float4 smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int b = blockIdx.y, N = P.N;
-    constexpr int RS = 33, D = kPipeDepth, DF = kPipeRateDepthF, C = kPipeChunk;
+    constexpr int RS = 33, C = kPipeChunk;
+    const int D = P.pipe_d, DF = P.pipe_df;            // D is a power of two
     const int kbase = blockIdx.x * 32;
     const int nchunks = (N + C - 1) / C;
 

@@ -454,9 +454,9 @@ def test_rate_model_pipelined_kernel_sizes(name, K, N, B):
     if wl.prev_front is not None:
         wl.prev_front = np.random.default_rng(2).integers(0, 2, (B, N + 1)).astype(np.int32)
     m = Pz.make_ctx(wl, variant=4)
-    assert m.info()["block_threads"] == 320 and m.info()["rollout_warps_per_block"] == 5
     x0, start, u = Pz.to_dev(wl)
     g = Pz.gpu_step(m, x0, start, u, 9, 2)
+    assert m.info()["block_threads"] == 320 and m.info()["rollout_warps_per_block"] == 5     # chosen at the first step
     o = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, 9, 2, want_du=True)
     o["u_nom"] = wl.u_nom.astype(np.float64)
     Pz.compare(f"{name} pipe K{K} N{N} B{B}", g, o, wl.params["lambda"], wl.params["objective"] == 0)
@@ -628,6 +628,24 @@ def _open_path_iterations(wl, opts, threads):
     assert m.info()["kernels_per_step"] == 1                     # the fifth column rides in the fused update
     assert m.info()["block_threads"] == threads
     m.close()
+
+
+def test_rate_model_auto_kernel_choice():
+    # input_model = 1 under AUTO: pipelined kernel with deep rings up to one block per SM, with shallow rings (two
+    # blocks per SM) up to twice the SM count when they fit, else the scalar kernel -- decided at the first step
+    sm = Pz.make_ctx(W.cfg0()).info()["sm_count"]
+    for K, N, B, threads in ((4096, 50, 1, 320), (8192, 20, 1, 320), (8192, 50, 1, 128), (4096, 50, 3, 128)):
+        wl = W.replicate(W.rate_gate_paper(K=K, N=N), B, 0.2)
+        m = Pz.make_ctx(wl)
+        x0, start, u = Pz.to_dev(wl)
+        g = Pz.gpu_step(m, x0, start, u, 2, 0)
+        assert m.info()["block_threads"] == threads, (K, N, B, m.info())
+        if threads == 320:
+            assert m.info()["grid_blocks"] <= (1 if N == 50 else 2) * sm
+        o = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, 2, 0, want_du=True)
+        o["u_nom"] = wl.u_nom.astype(np.float64)
+        Pz.compare(f"rate auto K{K} N{N} B{B}", g, o, wl.params["lambda"], False)
+        m.close()
 
 
 def test_table1_sizes():
