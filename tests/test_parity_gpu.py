@@ -630,6 +630,24 @@ def _open_path_iterations(wl, opts, threads):
     m.close()
 
 
+def test_rate_model_stored_noise_matches_the_oracle():
+    # store_noise = 1: the clamped rate perturbations dU the kernels rolled out, pipelined and scalar kernel
+    wl = W.rate_gate_paper(K=256, N=23)
+    o = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, 5, 7, want_du=True)
+    du_o = np.transpose(o["du"], (0, 2, 1, 3))
+    outs = {}
+    for name, opts in dict(pipe=dict(variant=4, store_noise=1), thr=dict(variant=1, store_noise=1)).items():
+        m = Pz.make_ctx(wl, **opts)
+        x0, start, u = Pz.to_dev(wl)
+        outs[name] = Pz.gpu_step(m, x0, start, u, 5, 7)
+        du = m.debug_noise().cpu().numpy()                      # [B,N,K,4]
+        np.testing.assert_allclose(du, du_o, rtol=0, atol=1e-5)
+        outs[name]["du"] = du
+        m.close()
+    np.testing.assert_array_equal(outs["pipe"]["du"], outs["thr"]["du"])
+    assert (np.abs(wl.u_nom[:, :, None, :] + outs["pipe"]["du"]) == wl.params["rate_max"]).any()     # the rate clamp acts
+
+
 def test_rate_model_auto_kernel_choice():
     # input_model = 1 under AUTO: pipelined kernel with deep rings up to one block per SM, with shallow rings (two
     # blocks per SM) up to twice the SM count when they fit, else the scalar kernel -- decided at the first step
