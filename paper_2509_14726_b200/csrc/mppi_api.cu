@@ -311,6 +311,7 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     d.blocks_per_ctrl = cfg.pipe ? p->K / 32 : cfg.lat_consumers ? p->K / (32 * cfg.lat_consumers)
                                           : p->K / (cfg.block_threads * (cfg.packed ? 2 : 1));
     d.part_stride = 4 * p->N + 4 + (p->objective == MPPI_OBJ_CONTOUR_PAPER ? ((p->N + 3) & ~3) : 0);
+    cfg.pipe_shallow = 0;
     cfg.smem_bytes = 0;   // fixed once the track is known
     // input_model = 1: the pipelined latency kernel is the faster one for few rollouts, but its rings share the
     // shared memory with the track, which is not known yet: keep the scalar shape, size the partials for
@@ -465,8 +466,9 @@ extern "C" int mppi_set_path(mppi_ctx* c, const float* pts, int P, int closed)
         for (int a = 0; a < 3; ++a) t[a] = (double)pts[3 * ip + a] - pts[3 * im + a];
         const double nt = std::sqrt(t[0] * t[0] + t[1] * t[1] + t[2] * t[2]);
         if (!(nt > 0.0)) return fail(c, MPPI_E_TRACK, "degenerate path tangent");
-        v[2 * i] = make_float4(pts[3 * i], pts[3 * i + 1], pts[3 * i + 2], (float)s[i]);
-        v[2 * i + 1] = make_float4((float)(t[0] / nt), (float)(t[1] / nt), (float)(t[2] / nt), 0.0f);
+        // all points first, then all tangents: the nearest-vertex search reads points only, at a 16-byte stride
+        v[i] = make_float4(pts[3 * i], pts[3 * i + 1], pts[3 * i + 2], (float)s[i]);
+        v[(size_t)P + i] = make_float4((float)(t[0] / nt), (float)(t[1] / nt), (float)(t[2] / nt), 0.0f);
     }
     int rc = upload_f4(c, &c->d_path, v);
     if (rc) return rc;
@@ -507,7 +509,7 @@ static int prepare(mppi_ctx* c)
             c->cfg.pipe = on ? 1 : 0;
             c->cfg.block_threads = on ? 320 : c->scalar_tpb;
             c->dp.blocks_per_ctrl = on ? c->prm.K / 32 : c->prm.K / c->scalar_tpb;
-            if (on) { c->dp.pipe_d = use_d; c->dp.pipe_df = use_df; }
+            if (on) { c->dp.pipe_d = use_d; c->dp.pipe_df = use_df; c->cfg.pipe_shallow = use_d == 2; }
             c->cfg.smem_bytes = 0;
         }
     }

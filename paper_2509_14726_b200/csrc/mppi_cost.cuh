@@ -179,7 +179,7 @@ __device__ __forceinline__ float track_stage(const DevParams& P, const float4* r
 }
 
 // ---- contouring: eq.(9) PAPER.md:149-161 in the projection variant of configs[3] [D-6] ---------
-// s_path holds all P points: (P_i, s_i), (t_i, 0).
+// s_path holds all P points (P_i, s_i), then all P tangents (t_i, 0).
 struct ContourCost {
     int idx;
     float theta_prev;
@@ -193,7 +193,7 @@ struct ContourCost {
         if (P.closed) {
             int i = wrap_index(centre - P.window, P.P);
             for (int o = -P.window; o <= P.window; ++o) {
-                const float4 q = s_path[2 * i];
+                const float4 q = s_path[i];
                 const float dx = px - q.x, dy = py - q.y, dz = pz - q.z;
                 const float d2 = dx * dx + dy * dy + dz * dz;
                 if (d2 < best) { best = d2; ibest = i; }
@@ -202,7 +202,7 @@ struct ContourCost {
         } else {
             const int lo = max(centre - P.window, 0), hi = min(centre + P.window, P.P - 1);
             for (int i = lo; i <= hi; ++i) {
-                const float4 q = s_path[2 * i];
+                const float4 q = s_path[i];
                 const float dx = px - q.x, dy = py - q.y, dz = pz - q.z;
                 const float d2 = dx * dx + dy * dy + dz * dz;
                 if (d2 < best) { best = d2; ibest = i; }
@@ -211,27 +211,27 @@ struct ContourCost {
         return ibest;
     }
     // lag error e_l, contour error squared e_c^2, progress theta = s_i + e_l
-    __device__ __forceinline__ static void project(const float4* s_path, int i, float px, float py,
+    __device__ __forceinline__ static void project(const DevParams& P, const float4* s_path, int i, float px, float py,
                                                    float pz, float& e_l, float& e_c2, float& theta)
     {
-        const float4 q = s_path[2 * i], t = s_path[2 * i + 1];
+        const float4 q = s_path[i], t = s_path[P.P + i];
         const float dx = px - q.x, dy = py - q.y, dz = pz - q.z;
         e_l = dx * t.x + dy * t.y + dz * t.z;
         e_c2 = fmaxf((dx * dx + dy * dy + dz * dz) - e_l * e_l, 0.0f);
         theta = q.w + e_l;
     }
     // i0 is the block-wide initial index (global or windowed search done by the caller)
-    __device__ __forceinline__ void init(const float4* s_path, int i0, const State& x)
+    __device__ __forceinline__ void init(const DevParams& P, const float4* s_path, int i0, const State& x)
     {
         float e_l, e_c2;
         idx = i0;
-        project(s_path, i0, x.px, x.py, x.pz, e_l, e_c2, theta_prev);
+        project(P, s_path, i0, x.px, x.py, x.pz, e_l, e_c2, theta_prev);
     }
     __device__ __forceinline__ float step(const DevParams& P, const float4* s_path, const State& x)
     {
         idx = nearest(P, s_path, idx, x.px, x.py, x.pz);
         float e_l, e_c2, theta;
-        project(s_path, idx, x.px, x.py, x.pz, e_l, e_c2, theta);
+        project(P, s_path, idx, x.px, x.py, x.pz, e_l, e_c2, theta);
         float d = theta - theta_prev;
         if (P.closed) d -= P.path_L * ceilf((d - 0.5f * P.path_L) * P.inv_path_L);  // (-L/2, L/2]
         theta_prev = theta;

@@ -31,7 +31,7 @@ struct DevParams {
     float q_c, q_l, mu, path_L, inv_path_L; // eq.(9) + closed path length
     const float4* gates;               // [G][4]: (c, a_h) (n, a_v) (h, 0) (v = h x n, 0)
     const float4* ref;                 // [M][4]: (p, qw) (qx qy qz, vx) (vy vz, wx wy) (wz,0,0,0)
-    const float4* path;                // [P][2]: (P_i, s_i) (t_i, 0)
+    const float4* path;                // [2][P]: all (P_i, s_i), then all (t_i, 0)
 };
 
 // ---- per-call arguments ---------------------------------------------------------------------

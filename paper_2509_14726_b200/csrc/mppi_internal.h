@@ -13,6 +13,7 @@ struct LaunchCfg {
     int packed;         // 1: rollout2_kernel, two samples per thread in fp32x2 registers
     int pipe;           // 1: rollout_pipe_kernel, one rollout pipelined over three warps (32 samples per block)
     int rate;           // 1: rollout_rate_kernel (thrust-rate input model, mppi_rate.cu)
+    int pipe_shallow;   // rollout_pipe_rate_kernel: 1 = rings (2, 2) chunks deep (two blocks per SM), 0 = (4, 3)
     int lat_consumers;  // 0: throughput kernel; 1, 2 or 4: latency kernel with that many rollout warps per block
     size_t smem_bytes;  // dynamic shared memory of the rollout kernel
 };

@@ -54,7 +54,7 @@ __device__ __forceinline__ void rollout_cost2(const DevParams& P, const StepArgs
     const int* s_front = reinterpret_cast<const int*>(s_trk + 4 * P.G);      // OBJ_GATE_PAPER only
     if (OBJ == OBJ_GATE) { ga.init<MATH>(P, s_trk, start, lane_state<0>(x)); gb = ga; }
     if (OBJ == OBJ_GATE_PAPER) { pa.init(P, s_trk, start, lane_state<0>(x)); pb = pa; }
-    if (OBJ == OBJ_CONTOUR) { ca.init(s_trk, contour_i0, lane_state<0>(x)); cb = ca; }
+    if (OBJ == OBJ_CONTOUR) { ca.init(P, s_trk, contour_i0, lane_state<0>(x)); cb = ca; }
     for (int t = 0; t < N; ++t) {
         const float4 un = s_unom[t];
         const float4 Ta = sample_thrust<MATH>(P, A.rk, k0, (uint32_t)t, A.iter, b, un);
@@ -386,7 +386,7 @@ __global__ void sim_kernel(const DevParams P, float* __restrict__ xs, int* __res
                 float best = __int_as_float(0x7f800000);
                 i0 = 0;
                 for (int i = 0; i < P.P; ++i) {
-                    const float4 q = P.path[2 * i];
+                    const float4 q = P.path[i];
                     const float dx = x.px - q.x, dy = x.py - q.y, dz = x.pz - q.z;
                     const float d2 = dx * dx + dy * dy + dz * dz;
                     if (d2 < best) { best = d2; i0 = i; }

@@ -229,7 +229,7 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
         const int* s_front = reinterpret_cast<const int*>(s_trk + 4 * P.G);      // OBJ_GATE_PAPER only
         if (OBJ == OBJ_GATE) gc.init<MATH>(P, s_trk, start, x);
         if (OBJ == OBJ_GATE_PAPER) gp.init(P, s_trk, start, x);
-        if (OBJ == OBJ_CONTOUR) cc.init(s_trk, i0, x);
+        if (OBJ == OBJ_CONTOUR) cc.init(P, s_trk, i0, x);
         auto pv_term = [&](const float4* row) {
             const float4 a = row[0], r = row[1], r2 = row[2];
             const float ex = x.px - a.x, ey = x.py - a.y, ez = x.pz - a.z;

@@ -71,14 +71,14 @@ __device__ __forceinline__ void stage_force(const DevParams& P, const float4 q /
     f[6] = c * c2x; f[7] = c * c2y; f[8] = fmaf(c, c2z, -P.g);
 }
 
-template <int OBJ, int MATH, bool STORE_DU>
-__global__ void __launch_bounds__(kPipeRateThreads, 2) rollout_pipe_rate_kernel(const DevParams P, const StepArgs A)
+template <int OBJ, int MATH, bool STORE_DU, bool SHALLOW>
+__global__ void __launch_bounds__(kPipeRateThreads, SHALLOW ? 2 : 1) rollout_pipe_rate_kernel(const DevParams P, const StepArgs A)
 {
     extern __shared__ float4 smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int b = blockIdx.y, N = P.N;
     constexpr int RS = 33, C = kPipeChunk;
-    const int D = P.pipe_d, DF = P.pipe_df;            // D is a power of two
+    constexpr int D = SHALLOW ? 2 : 4, DF = SHALLOW ? 2 : 3;      // = P.pipe_d, P.pipe_df (the host sizes the rings with those)
     const int kbase = blockIdx.x * 32;
     const int nchunks = (N + C - 1) / C;
 
@@ -137,9 +137,9 @@ __global__ void __launch_bounds__(kPipeRateThreads, 2) rollout_pipe_rate_kernel(
         float ox = x0.ox, oy = x0.oy, oz = x0.oz;
         float4 T = make_float4(xb[13], xb[14], xb[15], xb[16]);
         float acc = 0.0f, lim = 0.0f;
-        for (int c = 0; c < nchunks; ++c) {
-            const int s = c & (D - 1), cnt = min(C, N - c * C);
-            mbar_wait2(bar_T + c, 0, bar_we + s, ((c / D) & 1) ^ 1);
+        for (int c = 0, s = 0, ph = 0; c < nchunks; ++c, ph ^= (s + 1 == D), s = (s + 1 == D) ? 0 : s + 1) {
+            const int cnt = min(C, N - c * C);       // s = c % D, ph = (c / D) & 1, kept as running counters
+            mbar_wait2(bar_T + c, 0, bar_we + s, ph ^ 1);
             for (int j = 0; j < cnt; ++j) {
                 const int t = c * C + j;
                 const float4 u = s_T[t * RS + lane];
@@ -208,9 +208,9 @@ __global__ void __launch_bounds__(kPipeRateThreads, 2) rollout_pipe_rate_kernel(
             const float e0 = fmaf(-sg, a.w, qw), e1 = fmaf(-sg, r.x, qx), e2 = fmaf(-sg, r.y, qy), e3 = fmaf(-sg, r.z, qz);
             acc = fmaf(P.Qq, e0 * e0 + e1 * e1 + e2 * e2 + e3 * e3, acc);
         };
-        for (int c = 0; c < nchunks; ++c) {
-            const int s = c & (D - 1), cnt = min(C, N - c * C);
-            mbar_wait2(bar_wf + s, (c / D) & 1, bar_qe + s, ((c / D) & 1) ^ 1);
+        for (int c = 0, s = 0, ph = 0; c < nchunks; ++c, ph ^= (s + 1 == D), s = (s + 1 == D) ? 0 : s + 1) {
+            const int cnt = min(C, N - c * C);
+            mbar_wait2(bar_wf + s, ph, bar_qe + s, ph ^ 1);
             for (int j = 0; j < cnt; ++j) {
                 if (OBJ == OBJ_TRACK) quat_term(s_trk + 4 * (c * C + j));
                 const float4* w = s_w + (s * C + j) * 128 + lane;
@@ -244,9 +244,10 @@ __global__ void __launch_bounds__(kPipeRateThreads, 2) rollout_pipe_rate_kernel(
     } else if (warp == 3 || warp == 7) {
         // ---- F: drag matrix and thrust acceleration of the four stages; warp 3 even steps, warp 7 odd ----
         const int par = warp == 3 ? 0 : 1;
-        for (int c = 0; c < nchunks; ++c) {
-            const int s = c & (D - 1), sf = c % DF, cnt = min(C, N - c * C);
-            mbar_wait2(bar_qf + s, (c / D) & 1, bar_fe + sf, ((c / DF) & 1) ^ 1);
+        for (int c = 0, s = 0, ph = 0, sf = 0, phf = 0; c < nchunks;
+             ++c, ph ^= (s + 1 == D), s = (s + 1 == D) ? 0 : s + 1, phf ^= (sf + 1 == DF), sf = (sf + 1 == DF) ? 0 : sf + 1) {
+            const int cnt = min(C, N - c * C);
+            mbar_wait2(bar_qf + s, ph, bar_fe + sf, phf ^ 1);
             for (int j = (c * C + par) & 1 ? 1 : 0; j < cnt; j += 2) {
                 const float4* o = s_q + (s * C + j) * 160 + lane;
                 const float4 cc = o[128];
@@ -281,9 +282,9 @@ __global__ void __launch_bounds__(kPipeRateThreads, 2) rollout_pipe_rate_kernel(
         };
         float theta = 0.0f, v_theta = 0.0f;                                  // OBJ_CONTOUR_PAPER: progress states [R-33]
         if (OBJ == OBJ_CONTOUR_PAPER) { theta = xb[17]; v_theta = xb[18]; }
-        for (int c = 0; c < nchunks; ++c) {
-            const int sf = c % DF, cnt = min(C, N - c * C);
-            mbar_wait(bar_ff + sf, (c / DF) & 1);
+        for (int c = 0, sf = 0, phf = 0; c < nchunks; ++c, phf ^= (sf + 1 == DF), sf = (sf + 1 == DF) ? 0 : sf + 1) {
+            const int cnt = min(C, N - c * C);
+            mbar_wait(bar_ff + sf, phf);
             for (int j = 0; j < cnt; ++j) {
                 const int t = c * C + j;
                 const float4* g = s_f + (sf * C + j) * 288 + lane;

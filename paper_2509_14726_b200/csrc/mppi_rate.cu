@@ -52,7 +52,7 @@ __global__ void __launch_bounds__(256, 3) rollout_rate_kernel(const DevParams P,
     const int* s_front = reinterpret_cast<const int*>(s_trk + 4 * P.G);  // OBJ_GATE_PAPER only
     if (OBJ == OBJ_GATE) gc.init<MATH>(P, s_trk, start, x);
     if (OBJ == OBJ_GATE_PAPER) gp.init(P, s_trk, start, x);
-    if (OBJ == OBJ_CONTOUR) cc.init(s_trk, i0, x);
+    if (OBJ == OBJ_CONTOUR) cc.init(P, s_trk, i0, x);
     float4* du_out = STORE_DU ? A.du + (size_t)b * N * P.K + k : nullptr;
     for (int t = 0; t < N; ++t) {
         const float4 un = s_unom[t];
@@ -110,11 +110,16 @@ static RateFn pick_rate(const LaunchCfg& c)
     }
 }
 
+template <int OBJ, bool SHALLOW>
+static RateFn pick_pipe_rate2(const LaunchCfg& c)
+{
+    if (c.fast_math) return c.store_du ? rollout_pipe_rate_kernel<OBJ, 1, true, SHALLOW> : rollout_pipe_rate_kernel<OBJ, 1, false, SHALLOW>;
+    return c.store_du ? rollout_pipe_rate_kernel<OBJ, 0, true, SHALLOW> : rollout_pipe_rate_kernel<OBJ, 0, false, SHALLOW>;
+}
 template <int OBJ>
 static RateFn pick_pipe_rate1(const LaunchCfg& c)
 {
-    if (c.fast_math) return c.store_du ? rollout_pipe_rate_kernel<OBJ, 1, true> : rollout_pipe_rate_kernel<OBJ, 1, false>;
-    return c.store_du ? rollout_pipe_rate_kernel<OBJ, 0, true> : rollout_pipe_rate_kernel<OBJ, 0, false>;
+    return c.pipe_shallow ? pick_pipe_rate2<OBJ, true>(c) : pick_pipe_rate2<OBJ, false>(c);
 }
 static RateFn pick_pipe_rate(const LaunchCfg& c)
 {

@@ -95,7 +95,7 @@ __device__ __forceinline__ float rate_limit_cost(const DevParams& P, const State
 }
 
 // ---- the paper's own contouring formulation, eq.(9) PAPER.md:149-161 ----------------
-// P(theta) and the unit tangent at theta from the path in shared memory ((P_i, s_i), (t_i, 0)) [R-36]:
+// P(theta) and the unit tangent at theta from the path in shared memory (points (P_i, s_i), then tangents) [R-36]:
 // theta wrapped into [0, L) on a closed path (clamped on an open one); the segment is found from the
 // uniform-spacing guess theta P / L and corrected by stepping (the arc lengths are cumulative chord
 // lengths, only nearly uniform); linear interpolation of the points, normalised linear interpolation
@@ -106,13 +106,13 @@ __device__ __forceinline__ void path_eval(const DevParams& P, const float4* s_pa
     const int n = P.P;
     float th = theta;
     if (P.closed) { th = fmaf(-P.path_L, floorf(th * P.inv_path_L), th); if (th >= P.path_L) th = 0.0f; if (th < 0.0f) th = 0.0f; }
-    else th = fminf(fmaxf(th, 0.0f), s_path[2 * (n - 1)].w);
+    else th = fminf(fmaxf(th, 0.0f), s_path[n - 1].w);
     const int last = P.closed ? n - 1 : n - 2;
     int i = min(max((int)(th * P.inv_path_L * (float)n), 0), last);
-    while (i > 0 && s_path[2 * i].w > th) --i;
-    while (i < last && s_path[2 * (i + 1)].w <= th) ++i;
+    while (i > 0 && s_path[i].w > th) --i;
+    while (i < last && s_path[i + 1].w <= th) ++i;
     const int j = (i + 1 == n) ? 0 : i + 1;
-    const float4 a = s_path[2 * i], b = s_path[2 * j], ta = s_path[2 * i + 1], tb = s_path[2 * j + 1];
+    const float4 a = s_path[i], b = s_path[j], ta = s_path[n + i], tb = s_path[n + j];
     const float s1 = (i + 1 < n) ? b.w : P.path_L;
     const float lam = fminf((th - a.w) / (s1 - a.w), 1.0f), mu = 1.0f - lam;
     px = fmaf(lam, b.x, mu * a.x); py = fmaf(lam, b.y, mu * a.y); pz = fmaf(lam, b.z, mu * a.z);

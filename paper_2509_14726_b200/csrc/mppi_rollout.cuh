@@ -94,7 +94,7 @@ __device__ __forceinline__ int contour_start_index(const DevParams& P, const flo
     float best = __int_as_float(0x7f800000);
     int ib = 0x7fffffff;
     for (int i = tid; i < P.P; i += blockDim.x) {
-        const float4 q = s_path[2 * i];
+        const float4 q = s_path[i];
         const float dx = x.px - q.x, dy = x.py - q.y, dz = x.pz - q.z;
         const float d2 = dx * dx + dy * dy + dz * dz;
         if (d2 < best) { best = d2; ib = i; }
@@ -132,7 +132,7 @@ __device__ __forceinline__ float rollout_cost(const DevParams& P, const float4* 
     const int* s_front = reinterpret_cast<const int*>(s_trk + 4 * P.G);      // OBJ_GATE_PAPER only
     if (OBJ == OBJ_GATE) gc.init<MATH>(P, s_trk, start, x);
     if (OBJ == OBJ_GATE_PAPER) gp.init(P, s_trk, start, x);
-    if (OBJ == OBJ_CONTOUR) cc.init(s_trk, contour_i0, x);
+    if (OBJ == OBJ_CONTOUR) cc.init(P, s_trk, contour_i0, x);
     for (int t = 0; t < N; ++t) {
         const float4 T = thrust(t);
         if (OBJ == OBJ_TRACK) J += track_stage(P, s_trk + 4 * t, x, T);
