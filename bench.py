@@ -421,6 +421,7 @@ def run_survey(args):
             ms = time_steps(step, lambda: flush_buf.fill_(float(it[0] & 7)), 40 if B > 1 else 200, 5)
             info = m.info()
             k = ("rate-model pipelined" if P.get("input_model", 0) == 1 and info["block_threads"] == 320 else
+                 "rate-model packed fp32x2" if P.get("input_model", 0) == 1 and info["samples_per_thread"] == 2 else
                  "rate-model scalar" if P.get("input_model", 0) == 1 else
                  "pipelined" if info["rollout_warps_per_block"] == 3 and info["block_threads"] == 256 else
                  "packed fp32x2" if info["samples_per_thread"] == 2 else

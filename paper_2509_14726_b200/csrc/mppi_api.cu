@@ -27,7 +27,7 @@ struct mppi_ctx {
     DevParams dp;
     LaunchCfg cfg;
     int device = 0, sm_count = 0, l2_bytes = 0;
-    int lazy_pipe = 0, scalar_tpb = 0;     // input_model = 1: pipelined kernel iff it fits in shared memory (decided in prepare)
+    int lazy_pipe = 0, scalar_tpb = 0, scalar_packed = 0;     // input_model = 1: pipelined kernel iff it fits in shared memory (decided in prepare)
     bool have_gates = false, have_ref = false, have_path = false;
     float4* d_gates = nullptr;
     float4* d_ref = nullptr;
@@ -156,8 +156,12 @@ static int validate(const mppi_params* p)
             "rotor drag and the body-rate limit cost need input_model = 1");
     } else {
         BAD(!(p->rate_max > 0.0f), "rate_max must be > 0 when input_model = 1");
-        BAD(p->variant != MPPI_VARIANT_AUTO && p->variant != MPPI_VARIANT_THROUGHPUT && p->variant != MPPI_VARIANT_PIPELINED,
-            "input_model = 1 has a scalar throughput kernel and a pipelined latency kernel: variant must be AUTO, THROUGHPUT or PIPELINED");
+        BAD(p->variant != MPPI_VARIANT_AUTO && p->variant != MPPI_VARIANT_THROUGHPUT && p->variant != MPPI_VARIANT_PIPELINED &&
+                p->variant != MPPI_VARIANT_PACKED,
+            "input_model = 1 has scalar and packed throughput kernels and a pipelined latency kernel: variant must not be LATENCY");
+        BAD(p->variant == MPPI_VARIANT_PACKED &&
+                (p->K % 64 != 0 || (p->objective != MPPI_OBJ_GATE && p->objective != MPPI_OBJ_GATE_PAPER && p->objective != MPPI_OBJ_TRACK)),
+            "input_model = 1, PACKED: K % 64 == 0, objective gate / gate_paper / track");
         BAD(p->variant == MPPI_VARIANT_PIPELINED &&
                 (p->pipeline != MPPI_PIPE_FUSED || p->block_threads != 0 || p->N > 100 || p->K % 32 != 0 ||
                  p->objective == MPPI_OBJ_CONTOUR),
@@ -189,6 +193,17 @@ static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, i
     if (p->input_model == 1) {                     // thrust-rate model: its own kernels (mppi_rate.cu)
         // the scalar shape; whether the pipelined latency kernel takes over is decided in prepare(), once the
         // track (and with it the shared-memory footprint) is known -- see rate_pipe_candidate
+        const bool pk_obj = p->objective == MPPI_OBJ_GATE || p->objective == MPPI_OBJ_GATE_PAPER || p->objective == MPPI_OBJ_TRACK;
+        // packed fp32x2 throughput kernel (rollout_rate2_kernel): when the grid covers the chip
+        if (pk_obj && p->K % 64 == 0 && (p->variant == MPPI_VARIANT_PACKED ||
+                                         (p->variant == MPPI_VARIANT_AUTO && warps >= 8 * (int64_t)sm_count))) {
+            if (!p->block_threads || (p->block_threads <= 128 && p->K % (2 * p->block_threads) == 0)) {
+                *packed = 1;
+                if (p->block_threads) { *block_threads = p->block_threads; return; }
+                for (int tpb : {128, 64, 32})
+                    if (p->K % (2 * tpb) == 0) { *block_threads = tpb; return; }
+            }
+        }
         if (p->block_threads) { *block_threads = p->block_threads; return; }
         for (int tpb : {128, 64, 32})
             if (p->K % tpb == 0) { *block_threads = tpb; return; }
@@ -316,7 +331,7 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     // input_model = 1: the pipelined latency kernel is the faster one for few rollouts, but its rings share the
     // shared memory with the track, which is not known yet: keep the scalar shape, size the partials for
     // either, and let prepare() switch once the track has been set
-    c->scalar_tpb = cfg.block_threads;
+    c->scalar_tpb = cfg.block_threads; c->scalar_packed = cfg.packed;
     c->lazy_pipe = rate_pipe_candidate(p, c->sm_count) ? 1 : 0;
     d.pipe_d = 4; d.pipe_df = 3;
     const int max_blocks = c->lazy_pipe ? p->K / 32 : d.blocks_per_ctrl;
@@ -508,7 +523,8 @@ static int prepare(mppi_ctx* c)
         if (on != (c->cfg.pipe == 1) || (on && (c->dp.pipe_d != use_d || c->dp.pipe_df != use_df))) {
             c->cfg.pipe = on ? 1 : 0;
             c->cfg.block_threads = on ? 320 : c->scalar_tpb;
-            c->dp.blocks_per_ctrl = on ? c->prm.K / 32 : c->prm.K / c->scalar_tpb;
+            c->cfg.packed = on ? 0 : c->scalar_packed;
+            c->dp.blocks_per_ctrl = on ? c->prm.K / 32 : c->prm.K / (c->scalar_tpb * (c->scalar_packed ? 2 : 1));
             if (on) { c->dp.pipe_d = use_d; c->dp.pipe_df = use_df; c->cfg.pipe_shallow = use_d == 2; }
             c->cfg.smem_bytes = 0;
         }

@@ -85,6 +85,110 @@ __global__ void __launch_bounds__(256, 3) rollout_rate_kernel(const DevParams P,
         block_partial_and_combine<MATH>(P, A, b, blockIdx.x, J, lo, hi, s_unom, s_red, s_acc, s_pair);
 }
 
+// ---------------------------------------------------------------------------------------------
+// packed throughput variant of the rate model: two samples per thread in fp32x2 registers
+// (mppi_rate.cuh: fdyn_general2 / rk4_rate_step2).  grid = (K / (2 blockDim.x), B); thread j of the grid
+// row owns samples 2j and 2j+1.  Objectives: gate, the paper's J_gate, tracking.
+// ---------------------------------------------------------------------------------------------
+template <int OBJ, int MATH, bool STORE_DU, bool FUSED>
+__global__ void __launch_bounds__(128, 3) rollout_rate2_kernel(const DevParams P, const StepArgs A)
+{
+    extern __shared__ float4 smem[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int b = blockIdx.y;
+    const int k0 = 2 * (blockIdx.x * blockDim.x + tid);
+    const int N = P.N;
+
+    float4* s_unom = smem;
+    float4* s_trk = smem + N;
+    float* s_red = reinterpret_cast<float*>(s_trk + track_f4(P, OBJ));   // 64 floats
+    float4* s_acc = reinterpret_cast<float4*>(s_red + 64);
+    float* s_pair = reinterpret_cast<float*>(s_acc + (blockDim.x >> 5) * N);
+
+    const int start = A.start[b];
+    stage_inputs<OBJ>(P, A, b, start, s_unom, s_trk);
+    __syncthreads();
+
+    const float* xb = A.x0 + 17 * b;
+    const State x0 = load_state(xb);
+    State2 x = splat_state(x0);
+    float2 T[4] = { bc2(xb[13]), bc2(xb[14]), bc2(xb[15]), bc2(xb[16]) };
+    const float lo = -P.rate_max, hi = P.rate_max;
+
+    float Ja = 0.0f, Jb = 0.0f;
+    GateCost ga, gb;
+    GatePaperCost pa, pb;
+    const int* s_front = reinterpret_cast<const int*>(s_trk + 4 * P.G);  // OBJ_GATE_PAPER only
+    if (OBJ == OBJ_GATE) { ga.init<MATH>(P, s_trk, start, x0); gb = ga; }
+    if (OBJ == OBJ_GATE_PAPER) { pa.init(P, s_trk, start, x0); pb = pa; }
+    float4* du_out = STORE_DU ? A.du + (size_t)b * N * P.K + k0 : nullptr;
+    for (int t = 0; t < N; ++t) {
+        const float4 un = s_unom[t];
+        const float4 ua = sample_input<MATH>(P, A.rk, (uint32_t)k0, (uint32_t)t, A.iter, (uint32_t)b, un, lo, hi);
+        const float4 ub = sample_input<MATH>(P, A.rk, (uint32_t)k0 + 1u, (uint32_t)t, A.iter, (uint32_t)b, un, lo, hi);
+        if (STORE_DU) {
+            du_out[(size_t)t * P.K] = make_float4(ua.x - un.x, ua.y - un.y, ua.z - un.z, ua.w - un.w);
+            du_out[(size_t)t * P.K + 1] = make_float4(ub.x - un.x, ub.y - un.y, ub.z - un.z, ub.w - un.w);
+        }
+        if (OBJ == OBJ_TRACK) {
+            Ja += fmaf(P.R, ua.x * ua.x + ua.y * ua.y + ua.z * ua.z + ua.w * ua.w, track_state_term(P, s_trk + 4 * t, lane_state<0>(x)));
+            Jb += fmaf(P.R, ub.x * ub.x + ub.y * ub.y + ub.z * ub.z + ub.w * ub.w, track_state_term(P, s_trk + 4 * t, lane_state<1>(x)));
+        }
+        rk4_rate_step2(P, x, T, ua, ub);
+        const State xa = lane_state<0>(x), xc = lane_state<1>(x);
+        Ja += rate_limit_cost(P, xa);
+        Jb += rate_limit_cost(P, xc);
+        if (OBJ == OBJ_GATE) { ga.step<MATH>(P, s_trk, xa); gb.step<MATH>(P, s_trk, xc); }
+        if (OBJ == OBJ_GATE_PAPER) { pa.step(P, s_trk, s_front, xa, t); pb.step(P, s_trk, s_front, xc, t); }
+    }
+    if (OBJ == OBJ_GATE) { Ja += ga.finish<MATH>(P, s_trk, lane_state<0>(x)); Jb += gb.finish<MATH>(P, s_trk, lane_state<1>(x)); }
+    if (OBJ == OBJ_GATE_PAPER) { Ja += pa.finish(P); Jb += pb.finish(P); }
+    if (OBJ == OBJ_TRACK) {
+        Ja += track_state_term(P, s_trk + 4 * N, lane_state<0>(x));
+        Jb += track_state_term(P, s_trk + 4 * N, lane_state<1>(x));
+    }
+    *reinterpret_cast<float2*>(A.cost + (size_t)b * P.K + k0) = make_float2(Ja, Jb);
+
+    if (!FUSED) return;
+
+    // ---- block-local softmax partial over the block's 2 blockDim.x samples (as rollout2_kernel) ----
+    const float m = block_min(fminf(Ja, Jb), s_red);
+    const float ea = exp_weight<MATH>((m - Ja) * P.inv_lambda), eb = exp_weight<MATH>((m - Jb) * P.inv_lambda);
+    const float Zb = block_sum(ea + eb, s_red);
+    {
+        const unsigned ca = __ballot_sync(kFull, ea > 0.0f), cb = __ballot_sync(kFull, eb > 0.0f);
+        const uint32_t kbase = (uint32_t)(2 * (blockIdx.x * blockDim.x + warp * 32));
+        for (int t0 = 0; t0 < N; t0 += 32) {
+            const int t = t0 + lane;
+            const float4 un = t < N ? s_unom[t] : make_float4(0.f, 0.f, 0.f, 0.f);
+            float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                unsigned mm = h ? cb : ca;
+                while (mm) {
+                    const int l = __ffs(mm) - 1;
+                    mm &= mm - 1;
+                    const float el = __shfl_sync(kFull, h ? eb : ea, l);
+                    const float4 u = sample_input<MATH>(P, A.rk, kbase + 2u * l + h, (uint32_t)t, A.iter, (uint32_t)b, un, lo, hi);
+                    acc.x = fmaf(el, u.x - un.x, acc.x); acc.y = fmaf(el, u.y - un.y, acc.y);
+                    acc.z = fmaf(el, u.z - un.z, acc.z); acc.w = fmaf(el, u.w - un.w, acc.w);
+                }
+            }
+            if (t < N) s_acc[warp * N + t] = acc;
+        }
+    }
+    __syncthreads();
+    const int nw = blockDim.x >> 5;
+    float* part = A.partials + ((size_t)b * P.blocks_per_ctrl + blockIdx.x) * P.part_stride;
+    for (int j = tid; j < 4 * N; j += blockDim.x) {
+        float s = 0.0f;
+        for (int w = 0; w < nw; ++w) s += reinterpret_cast<const float*>(s_acc)[w * 4 * N + j];
+        part[j] = s;
+    }
+    if (tid == 0) { part[4 * N] = m; part[4 * N + 1] = Zb; }
+    publish_and_combine<MATH>(P, A, b, P.blocks_per_ctrl, s_unom, s_red, s_pair);
+}
+
 // ---- host-side dispatch ------------------------------------------------------------------------------
 typedef void (*RateFn)(const DevParams, const StepArgs);
 
@@ -131,14 +235,33 @@ static RateFn pick_pipe_rate(const LaunchCfg& c)
     }
 }
 
-const void* rate_kernel_ptr(const LaunchCfg& c)
+template <int OBJ, int MATH>
+static RateFn pick_rate2p2(const LaunchCfg& c)
 {
-    return reinterpret_cast<const void*>(c.pipe ? pick_pipe_rate(c) : pick_rate(c));
+    if (c.fused) return c.store_du ? rollout_rate2_kernel<OBJ, MATH, true, true> : rollout_rate2_kernel<OBJ, MATH, false, true>;
+    return rollout_rate2_kernel<OBJ, MATH, true, false>;
 }
+template <int OBJ>
+static RateFn pick_rate2p1(const LaunchCfg& c)
+{
+    return c.fast_math ? pick_rate2p2<OBJ, 1>(c) : pick_rate2p2<OBJ, 0>(c);
+}
+static RateFn pick_rate_packed(const LaunchCfg& c)
+{
+    switch (c.objective) {
+        case OBJ_GATE: return pick_rate2p1<OBJ_GATE>(c);
+        case OBJ_GATE_PAPER: return pick_rate2p1<OBJ_GATE_PAPER>(c);
+        default: return pick_rate2p1<OBJ_TRACK>(c);
+    }
+}
+
+static RateFn pick_any(const LaunchCfg& c) { return c.pipe ? pick_pipe_rate(c) : c.packed ? pick_rate_packed(c) : pick_rate(c); }
+
+const void* rate_kernel_ptr(const LaunchCfg& c) { return reinterpret_cast<const void*>(pick_any(c)); }
 
 cudaError_t launch_rate(const DevParams& P, const StepArgs& A, const LaunchCfg& c, cudaStream_t s)
 {
-    (c.pipe ? pick_pipe_rate(c) : pick_rate(c))<<<dim3(P.blocks_per_ctrl, P.B), c.block_threads, c.smem_bytes, s>>>(P, A);
+    pick_any(c)<<<dim3(P.blocks_per_ctrl, P.B), c.block_threads, c.smem_bytes, s>>>(P, A);
     return cudaGetLastError();
 }
 

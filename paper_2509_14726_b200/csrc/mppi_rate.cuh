@@ -3,6 +3,7 @@
 // Used by the rollout kernel (mppi_rate.cu) and by the plant / nominal-rollout kernels (mppi_kernels.cu).
 #pragma once
 #include "mppi_device.cuh"
+#include "mppi_packed.cuh"
 
 namespace mppi {
 
@@ -149,6 +150,92 @@ __device__ __forceinline__ float contour_paper_stage(const DevParams& P, const f
     J = fmaf(P.r_dv, dv * dv, J);
     J = fmaf(P.R, fmaf(dT.w, dT.w, fmaf(dT.z, dT.z, fmaf(dT.y, dT.y, dT.x * dT.x))), J);
     return fmaf(-P.mu, v_theta, J);
+}
+
+// ---- two samples per thread in packed fp32x2 registers (see mppi_packed.cuh): the same model ------------
+struct Deriv2 { float2 qw, qx, qy, qz, vx, vy, vz, ox, oy, oz; };
+
+// f_dyn of eq.(2) with drag for two samples; T0..T3: rotor thrusts (halves = the two samples)
+__device__ __forceinline__ Deriv2 fdyn_general2(const DevParams& P, const float2 qw, const float2 qx, const float2 qy,
+                                                const float2 qz, const float2 vx, const float2 vy, const float2 vz,
+                                                const float2 ox, const float2 oy, const float2 oz, const float2 T0,
+                                                const float2 T1, const float2 T2, const float2 T3)
+{
+    Deriv2 d;
+    const float2 hf = bc2(0.5f), two = bc2(2.0f), one = bc2(1.0f), m2 = bc2(-2.0f);
+    d.qw = mul2(hf, fma2(neg2(qz), oz, fma2(neg2(qy), oy, mul2(neg2(qx), ox))));
+    d.qx = mul2(hf, fma2(neg2(qz), oy, fma2(qy, oz, mul2(qw, ox))));
+    d.qy = mul2(hf, fma2(neg2(qx), oz, fma2(qz, ox, mul2(qw, oy))));
+    d.qz = mul2(hf, fma2(neg2(qy), ox, fma2(qx, oy, mul2(qw, oz))));
+    const float2 s01 = add2(T0, T1), s23 = add2(T2, T3);
+    d.ox = fma2(P.gyx, mul2(oy, oz), mul2(bc2(P.ltx), sub2(s01, s23)));
+    d.oy = fma2(P.gyy, mul2(oz, ox), mul2(bc2(P.lty), sub2(add2(T1, T2), add2(T0, T3))));
+    d.oz = fma2(P.gyz, mul2(ox, oy), mul2(bc2(P.ltz), sub2(add2(T0, T2), add2(T1, T3))));
+    const float2 c0x = fma2(m2, fma2(qy, qy, mul2(qz, qz)), one), c0y = mul2(two, fma2(qx, qy, mul2(qw, qz))),
+                 c0z = mul2(two, fma2(qx, qz, mul2(neg2(qw), qy)));
+    const float2 c1x = mul2(two, fma2(qx, qy, mul2(neg2(qw), qz))), c1y = fma2(m2, fma2(qx, qx, mul2(qz, qz)), one),
+                 c1z = mul2(two, fma2(qy, qz, mul2(qw, qx)));
+    const float2 c2x = mul2(two, fma2(qx, qz, mul2(qw, qy))), c2y = mul2(two, fma2(qy, qz, mul2(neg2(qw), qx))),
+                 c2z = fma2(m2, fma2(qx, qx, mul2(qy, qy)), one);
+    const float2 c = mul2(add2(s01, s23), bc2(P.inv_mass));
+    const float2 b0 = mul2(bc2(P.drag_x), fma2(c0z, vz, fma2(c0y, vy, mul2(c0x, vx))));
+    const float2 b1 = mul2(bc2(P.drag_y), fma2(c1z, vz, fma2(c1y, vy, mul2(c1x, vx))));
+    const float2 b2 = mul2(bc2(P.drag_z), fma2(c2z, vz, fma2(c2y, vy, mul2(c2x, vx))));
+    d.vx = fma2(c, c2x, neg2(fma2(c2x, b2, fma2(c1x, b1, mul2(c0x, b0)))));
+    d.vy = fma2(c, c2y, neg2(fma2(c2y, b2, fma2(c1y, b1, mul2(c0y, b0)))));
+    d.vz = sub2(fma2(c, c2z, neg2(fma2(c2z, b2, fma2(c1z, b1, mul2(c0z, b0))))), bc2(P.g));
+    return d;
+}
+
+__device__ __forceinline__ float2 clamp2(const float2 v, const float lo, const float hi)
+{
+    return make_float2(fminf(fmaxf(v.x, lo), hi), fminf(fmaxf(v.y, lo), hi));
+}
+
+// rk4_rate_step for two samples: x, T (4 rotor thrust pairs) <- one step with the rates ua / ub held
+__device__ __forceinline__ void rk4_rate_step2(const DevParams& P, State2& x, float2 (&T)[4], const float4 ua, const float4 ub)
+{
+    const float2 h = bc2(P.dt), hh = bc2(P.h2), h6 = bc2(P.h6), two = bc2(2.0f);
+    const float2 u0 = make_float2(ua.x, ub.x), u1 = make_float2(ua.y, ub.y), u2 = make_float2(ua.z, ub.z), u3 = make_float2(ua.w, ub.w);
+    const float2 Tm0 = fma2(hh, u0, T[0]), Tm1 = fma2(hh, u1, T[1]), Tm2 = fma2(hh, u2, T[2]), Tm3 = fma2(hh, u3, T[3]);
+    const float2 Te0 = fma2(h, u0, T[0]), Te1 = fma2(h, u1, T[1]), Te2 = fma2(h, u2, T[2]), Te3 = fma2(h, u3, T[3]);
+    Deriv2 k = fdyn_general2(P, x.qw, x.qx, x.qy, x.qz, x.vx, x.vy, x.vz, x.ox, x.oy, x.oz, T[0], T[1], T[2], T[3]);
+    float2 apx = x.vx, apy = x.vy, apz = x.vz;
+    Deriv2 a = k;
+#define MPPI_STAGE2(HS)                                                                              \
+    vx = fma2(HS, k.vx, x.vx); vy = fma2(HS, k.vy, x.vy); vz = fma2(HS, k.vz, x.vz);               \
+    qw = fma2(HS, k.qw, x.qw); qx = fma2(HS, k.qx, x.qx); qy = fma2(HS, k.qy, x.qy); qz = fma2(HS, k.qz, x.qz); \
+    ox = fma2(HS, k.ox, x.ox); oy = fma2(HS, k.oy, x.oy); oz = fma2(HS, k.oz, x.oz);
+#define MPPI_ACC2(W)                                                                                 \
+    a.qw = fma2(W, k.qw, a.qw); a.qx = fma2(W, k.qx, a.qx); a.qy = fma2(W, k.qy, a.qy); a.qz = fma2(W, k.qz, a.qz); \
+    a.vx = fma2(W, k.vx, a.vx); a.vy = fma2(W, k.vy, a.vy); a.vz = fma2(W, k.vz, a.vz);             \
+    a.ox = fma2(W, k.ox, a.ox); a.oy = fma2(W, k.oy, a.oy); a.oz = fma2(W, k.oz, a.oz);
+    float2 vx, vy, vz, qw, qx, qy, qz, ox, oy, oz;
+    MPPI_STAGE2(hh)
+    apx = fma2(two, vx, apx); apy = fma2(two, vy, apy); apz = fma2(two, vz, apz);
+    k = fdyn_general2(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Tm0, Tm1, Tm2, Tm3);
+    MPPI_ACC2(two)
+    MPPI_STAGE2(hh)
+    apx = fma2(two, vx, apx); apy = fma2(two, vy, apy); apz = fma2(two, vz, apz);
+    k = fdyn_general2(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Tm0, Tm1, Tm2, Tm3);
+    MPPI_ACC2(two)
+    MPPI_STAGE2(h)
+    apx = add2(apx, vx); apy = add2(apy, vy); apz = add2(apz, vz);
+    k = fdyn_general2(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Te0, Te1, Te2, Te3);
+    a.qw = add2(a.qw, k.qw); a.qx = add2(a.qx, k.qx); a.qy = add2(a.qy, k.qy); a.qz = add2(a.qz, k.qz);
+    a.vx = add2(a.vx, k.vx); a.vy = add2(a.vy, k.vy); a.vz = add2(a.vz, k.vz);
+    a.ox = add2(a.ox, k.ox); a.oy = add2(a.oy, k.oy); a.oz = add2(a.oz, k.oz);
+#undef MPPI_STAGE2
+#undef MPPI_ACC2
+    x.px = fma2(h6, apx, x.px); x.py = fma2(h6, apy, x.py); x.pz = fma2(h6, apz, x.pz);
+    x.vx = fma2(h6, a.vx, x.vx); x.vy = fma2(h6, a.vy, x.vy); x.vz = fma2(h6, a.vz, x.vz);
+    x.ox = fma2(h6, a.ox, x.ox); x.oy = fma2(h6, a.oy, x.oy); x.oz = fma2(h6, a.oz, x.oz);
+    const float2 nw = fma2(h6, a.qw, x.qw), nx = fma2(h6, a.qx, x.qx), ny = fma2(h6, a.qy, x.qy), nz = fma2(h6, a.qz, x.qz);
+    const float2 n2 = fma2(nz, nz, fma2(ny, ny, fma2(nx, nx, mul2(nw, nw))));
+    const float2 inv = make_float2(rsqrtf(n2.x), rsqrtf(n2.y));
+    x.qw = mul2(nw, inv); x.qx = mul2(nx, inv); x.qy = mul2(ny, inv); x.qz = mul2(nz, inv);
+    T[0] = clamp2(Te0, P.T_min, P.T_max); T[1] = clamp2(Te1, P.T_min, P.T_max);
+    T[2] = clamp2(Te2, P.T_min, P.T_max); T[3] = clamp2(Te3, P.T_min, P.T_max);
 }
 
 }  // namespace mppi

@@ -414,10 +414,11 @@ def test_front_flags_and_closed_loop_feed():
 
 # ---- the paper's own input model (thrust rates, thrust states, drag, rate limit) ----
 
-RATE_PIPES = [dict(pipeline=0, variant=4), dict(pipeline=0, variant=1), dict(pipeline=0, variant=1, block_threads=64), dict(pipeline=1)]
+RATE_PIPES = [dict(pipeline=0, variant=4), dict(pipeline=0, variant=1), dict(pipeline=0, variant=1, block_threads=64), dict(pipeline=1),
+              dict(pipeline=0, variant=3), dict(pipeline=1, variant=3, block_threads=64)]
 
 
-RATE_IDS = ["fused_pipe", "fused", "fused_tpb64", "two_pass"]
+RATE_IDS = ["fused_pipe", "fused", "fused_tpb64", "two_pass", "fused_pk", "two_pass_pk64"]
 
 
 @pytest.mark.parametrize("pipe", RATE_PIPES, ids=RATE_IDS)
@@ -493,7 +494,7 @@ def test_rate_model_contouring_batch_and_warm_start():
 def test_rate_model_rejects_what_it_does_not_support():
     from paper_2509_14726_b200 import binding as Bd
     wl = W.rate_gate_paper(K=64, N=8)
-    for bad in (dict(variant=2), dict(variant=3), dict(variant=4, pipeline=1), dict(variant=4, block_threads=64),
+    for bad in (dict(variant=2), dict(variant=3, K=96), dict(variant=3, block_threads=256), dict(variant=4, pipeline=1), dict(variant=4, block_threads=64),
                 dict(variant=4, N=101), dict(rate_max=0.0)):
         with pytest.raises(Bd.MppiError) as e:
             Bd.Mppi(wl.params, **bad)
