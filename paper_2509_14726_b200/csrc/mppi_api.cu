@@ -299,6 +299,8 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
         d.h12 = (float)(h / 12); d.hh2 = (float)(h * h / 2); d.hh3 = (float)(h * h / 3);
     }
     d.dt = p->dt; d.inv_lambda = (float)(1.0 / (double)p->lambda); d.sigma = p->sigma;
+    d.bm_k = (float)(-2.0 * 0.6931471805599453 * (double)p->sigma * (double)p->sigma);
+    d.bm_kv = (float)(-2.0 * 0.6931471805599453 * (double)p->sigma_v * (double)p->sigma_v);
     d.T_min = p->T_min; d.T_max = p->T_max;
     d.inv_mass = (float)(1.0 / (double)p->mass); d.g = p->g;
     d.hover = (float)((double)p->mass * (double)p->g / 4.0);

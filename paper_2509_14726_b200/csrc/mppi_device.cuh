@@ -17,6 +17,7 @@ struct DevParams {
     int pipe_d, pipe_df;               // rollout_pipe_rate_kernel: ring depths in chunks (W / Q rings, F ring)
     int part_stride;                   // floats per partial: 4N + 4 (+ N rounded up to 4 under OBJ_CONTOUR_PAPER)
     float dt, inv_lambda, sigma, T_min, T_max;
+    float bm_k, bm_kv;                 // -2 ln2 sigma^2, -2 ln2 sigma_v^2: Box-Muller radius constants of the fast path
     float h2, h3, h4, h6, h12, hh2, hh3;   // dt/2, dt/3, dt/4, dt/6, dt/12, dt^2/2, dt^2/3
     float inv_mass, g, hover;
     float ltx, lty, ltz;               // (arm/sqrt2)/Jx, (arm/sqrt2)/Jy, c_tau/Jz
@@ -94,9 +95,9 @@ __device__ __forceinline__ float mufu_ex2(float x) { float y; asm("ex2.approx.ft
 // z0 = rad cos(2 pi u2), z1 = rad sin(2 pi u2), rad = sqrt(-2 ln u1).
 // MATH = 0: IEEE-accurate library functions, in the oracle's operation order.
 // MATH = 1: MUFU lg2 / rsq / sin / cos.  The angle is taken as 2 pi (u2 - 1/2) in [-pi, pi), where the
-// MUFU error bound holds, and the sign flip cos(x - pi) = -cos x is folded into the radius.
+// MUFU error bound holds, and the sign flip cos(x - pi) = -cos x is folded into the final fma.
 template <int MATH>
-__device__ __forceinline__ void perturb_pair(uint32_t ra, uint32_t rb, float sigma, float una, float unb,
+__device__ __forceinline__ void perturb_pair(uint32_t ra, uint32_t rb, float sigma, float bm_k, float una, float unb,
                                              float& a, float& b)
 {
     if (MATH == 0) {
@@ -107,13 +108,17 @@ __device__ __forceinline__ void perturb_pair(uint32_t ra, uint32_t rb, float sig
         a = fmaf(sigma, rad * c, una);
         b = fmaf(sigma, rad * s, unb);
     } else {
-        const float u1 = u01(ra);
-        const float t = -1.3862943611198906f * mufu_lg2(u1);          // -2 ln u1 > 0
-        const float nrad = (t * -sigma) * mufu_rsq(t);                // -sigma sqrt(t)
-        const float w = __uint_as_float(0x3f800000u | (rb >> 9)) - 1.5f;   // u2 - 1/2 - 2^-24, exact
-        const float ang = fmaf(w, 6.283185307179586f, 3.7450704e-7f);      // 2 pi (u2 - 1/2) in [-pi, pi)
-        a = fmaf(nrad, mufu_cos(ang), una);
-        b = fmaf(nrad, mufu_sin(ang), unb);
+        // rad = sigma sqrt(-2 ln u1) = sqrt(bm_k lg2 u1), bm_k = -2 ln2 sigma^2 from the host: one multiply
+        // and MUFU.SQRT.
+        const float rad = mufu_sqrt(mufu_lg2(u01(ra)) * bm_k);
+        // ang = 2 pi (u2 - 1/2) = 2 pi m2 - 3 pi + 2 pi 2^-24 with m2 = 1 + (rb >> 9) 2^-23 in [1, 2): ONE fma
+        // straight from the mantissa trick.  The additive constant is the float next to
+        // -3 pi + 2 pi 2^-24 - 1.5 (fl(2 pi) - 2 pi), which centres the error of fl(2 pi) m2 on m2 = 1.5:
+        // |angle error| <= 3.4e-7 rad, below the MUFU.SIN / MUFU.COS error itself.
+        const float m2 = __uint_as_float(0x3f800000u | (rb >> 9));
+        const float ang = fmaf(m2, 6.283185307179586f, -9.42477798461914f);
+        a = fmaf(-rad, mufu_cos(ang), una);
+        b = fmaf(-rad, mufu_sin(ang), unb);
     }
 }
 
@@ -126,8 +131,8 @@ __device__ __forceinline__ float4 sample_input(const DevParams& P, const uint32_
 {
     const uint4 r = philox4x32_10(k, t, iter, b, rk);
     float4 T;
-    perturb_pair<MATH>(r.x, r.y, P.sigma, un.x, un.y, T.x, T.y);
-    perturb_pair<MATH>(r.z, r.w, P.sigma, un.z, un.w, T.z, T.w);
+    perturb_pair<MATH>(r.x, r.y, P.sigma, P.bm_k, un.x, un.y, T.x, T.y);
+    perturb_pair<MATH>(r.z, r.w, P.sigma, P.bm_k, un.z, un.w, T.z, T.w);
     T.x = fminf(fmaxf(T.x, lo), hi);
     T.y = fminf(fmaxf(T.y, lo), hi);
     T.z = fminf(fmaxf(T.z, lo), hi);
@@ -164,8 +169,9 @@ __device__ __forceinline__ void rk4_step(const DevParams& P, State& x, const flo
     const float s01 = T.x + T.y, s23 = T.z + T.w;
     const float c = (s01 + s23) * P.inv_mass;                  // S / m
     const float ax = P.ltx * (s01 - s23);                      // tau_x / Jx
-    const float ay = P.lty * ((T.y + T.z) - (T.x + T.w));      // tau_y / Jy
-    const float az = P.ltz * ((T.x + T.z) - (T.y + T.w));      // tau_z / Jz
+    const float d10 = T.y - T.x, d23 = T.z - T.w;
+    const float ay = P.lty * (d10 + d23);                      // tau_y / Jy  ((T1 + T2) - (T0 + T3))
+    const float az = P.ltz * (d23 - d10);                      // tau_z / Jz  ((T0 + T2) - (T1 + T3))
     const float cz0 = c - P.g;
     const float kp = c * P.hh3, kv = c * P.h3;                 // h^2/6 c2, h/6 c2
 

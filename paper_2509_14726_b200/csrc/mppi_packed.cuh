@@ -60,8 +60,9 @@ __device__ __forceinline__ void rk4_step2(const DevParams& P, State2& x, const f
     const float2 s01 = add2(T0, T1), s23 = add2(T2, T3);
     const float2 c = mul2(add2(s01, s23), bc2(P.inv_mass));                    // S / m
     const float2 ax = mul2(bc2(P.ltx), sub2(s01, s23));                        // tau_x / Jx
-    const float2 ay = mul2(bc2(P.lty), sub2(add2(T1, T2), add2(T0, T3)));      // tau_y / Jy
-    const float2 az = mul2(bc2(P.ltz), sub2(add2(T0, T2), add2(T1, T3)));      // tau_z / Jz
+    const float2 d10 = sub2(T1, T0), d23 = sub2(T2, T3);
+    const float2 ay = mul2(bc2(P.lty), add2(d10, d23));                        // tau_y / Jy
+    const float2 az = mul2(bc2(P.ltz), sub2(d23, d10));                        // tau_z / Jz
     const float2 cz0 = sub2(c, bc2(P.g));
     const float2 kp = mul2(c, bc2(P.hh3)), kv = mul2(c, bc2(P.h3));
 

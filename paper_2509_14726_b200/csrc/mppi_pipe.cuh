@@ -145,8 +145,9 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
                 }
                 const float s01 = T.x + T.y, s23 = T.z + T.w;
                 const float ax = P.ltx * (s01 - s23);
-                const float ay = P.lty * ((T.y + T.z) - (T.x + T.w));
-                const float az = P.ltz * ((T.x + T.z) - (T.y + T.w));
+                const float d10 = T.y - T.x, d23 = T.z - T.w;
+                const float ay = P.lty * (d10 + d23);
+                const float az = P.ltz * (d23 - d10);
                 float kx = fmaf(P.gyx, oy * oz, ax), ky = fmaf(P.gyy, oz * ox, ay), kz = fmaf(P.gyz, ox * oy, az);
                 float nx = fmaf(P.h6, kx, ox), ny = fmaf(P.h6, ky, oy), nz = fmaf(P.h6, kz, oz);
                 const float o2x = fmaf(P.h2, kx, ox), o2y = fmaf(P.h2, ky, oy), o2z = fmaf(P.h2, kz, oz);

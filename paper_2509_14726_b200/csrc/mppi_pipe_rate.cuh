@@ -158,8 +158,9 @@ __global__ void __launch_bounds__(kPipeRateThreads, SHALLOW ? 2 : 1) rollout_pip
                 // torque accelerations and collective acceleration are linear in the thrusts: value at T and slope along u
                 const float s01 = T.x + T.y, s23 = T.z + T.w, u01 = u.x + u.y, u23 = u.z + u.w;
                 const float ax = P.ltx * (s01 - s23), bx = P.ltx * (u01 - u23);
-                const float ay = P.lty * ((T.y + T.z) - (T.x + T.w)), by = P.lty * ((u.y + u.z) - (u.x + u.w));
-                const float az = P.ltz * ((T.x + T.z) - (T.y + T.w)), bz = P.ltz * ((u.x + u.z) - (u.y + u.w));
+                const float d10 = T.y - T.x, d23 = T.z - T.w, e10 = u.y - u.x, e23 = u.z - u.w;
+                const float ay = P.lty * (d10 + d23), by = P.lty * (e10 + e23);
+                const float az = P.ltz * (d23 - d10), bz = P.ltz * (e23 - e10);
                 const float c0 = (s01 + s23) * P.inv_mass, cu = (u01 + u23) * P.inv_mass;
                 const float amx = fmaf(P.h2, bx, ax), amy = fmaf(P.h2, by, ay), amz = fmaf(P.h2, bz, az);
                 const float aex = fmaf(P.dt, bx, ax), aey = fmaf(P.dt, by, ay), aez = fmaf(P.dt, bz, az);

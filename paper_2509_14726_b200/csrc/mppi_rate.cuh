@@ -22,8 +22,9 @@ __device__ __forceinline__ Deriv fdyn_general(const DevParams& P, const float qw
     d.qz = 0.5f * fmaf(-qy, ox, fmaf(qx, oy, qw * oz));
     const float s01 = T.x + T.y, s23 = T.z + T.w;
     d.ox = fmaf(P.gyx, oy * oz, P.ltx * (s01 - s23));                  // PAPER.md:70, J^-1 folded in
-    d.oy = fmaf(P.gyy, oz * ox, P.lty * ((T.y + T.z) - (T.x + T.w)));
-    d.oz = fmaf(P.gyz, ox * oy, P.ltz * ((T.x + T.z) - (T.y + T.w)));
+    const float d10 = T.y - T.x, d23 = T.z - T.w;                      // (T1 + T2) - (T0 + T3) = d10 + d23, (T0 + T2) - (T1 + T3) = d23 - d10
+    d.oy = fmaf(P.gyy, oz * ox, P.lty * (d10 + d23));
+    d.oz = fmaf(P.gyz, ox * oy, P.ltz * (d23 - d10));
     // columns of R(q): the body axes in the world frame
     const float c0x = 1.0f - 2.0f * (qy * qy + qz * qz), c0y = 2.0f * (qx * qy + qw * qz), c0z = 2.0f * (qx * qz - qw * qy);
     const float c1x = 2.0f * (qx * qy - qw * qz), c1y = 1.0f - 2.0f * (qx * qx + qz * qz), c1z = 2.0f * (qy * qz + qw * qx);
@@ -130,7 +131,7 @@ __device__ __forceinline__ float sample_progress_accel(const DevParams& P, const
 {
     const uint4 r = philox4x32_10(k, t + 0x80000000u, iter, b, rk);
     float a, unused;
-    perturb_pair<MATH>(r.x, r.y, P.sigma_v, vn, 0.0f, a, unused);
+    perturb_pair<MATH>(r.x, r.y, P.sigma_v, P.bm_kv, vn, 0.0f, a, unused);
     return fminf(fmaxf(a, -P.dv_max), P.dv_max);
 }
 
@@ -169,8 +170,9 @@ __device__ __forceinline__ Deriv2 fdyn_general2(const DevParams& P, const float2
     d.qz = mul2(hf, fma2(neg2(qy), ox, fma2(qx, oy, mul2(qw, oz))));
     const float2 s01 = add2(T0, T1), s23 = add2(T2, T3);
     d.ox = fma2(P.gyx, mul2(oy, oz), mul2(bc2(P.ltx), sub2(s01, s23)));
-    d.oy = fma2(P.gyy, mul2(oz, ox), mul2(bc2(P.lty), sub2(add2(T1, T2), add2(T0, T3))));
-    d.oz = fma2(P.gyz, mul2(ox, oy), mul2(bc2(P.ltz), sub2(add2(T0, T2), add2(T1, T3))));
+    const float2 d10 = sub2(T1, T0), d23 = sub2(T2, T3);
+    d.oy = fma2(P.gyy, mul2(oz, ox), mul2(bc2(P.lty), add2(d10, d23)));
+    d.oz = fma2(P.gyz, mul2(ox, oy), mul2(bc2(P.ltz), sub2(d23, d10)));
     const float2 c0x = fma2(m2, fma2(qy, qy, mul2(qz, qz)), one), c0y = mul2(two, fma2(qx, qy, mul2(qw, qz))),
                  c0z = mul2(two, fma2(qx, qz, mul2(neg2(qw), qy)));
     const float2 c1x = mul2(two, fma2(qx, qy, mul2(neg2(qw), qz))), c1y = fma2(m2, fma2(qx, qx, mul2(qz, qz)), one),
