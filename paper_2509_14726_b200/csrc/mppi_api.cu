@@ -419,7 +419,8 @@ extern "C" int mppi_set_gates(mppi_ctx* c, const float* g, int G)
         const double vx = h[1] * n[2] - h[2] * n[1], vy = h[2] * n[0] - h[0] * n[2], vz = h[0] * n[1] - h[1] * n[0];
         v[4 * i + 0] = make_float4(r[0], r[1], r[2], r[9]);
         v[4 * i + 1] = make_float4(r[3], r[4], r[5], r[10]);
-        v[4 * i + 2] = make_float4(r[6], r[7], r[8], 0.0f);
+        const double nc = n[0] * (double)r[0] + n[1] * (double)r[1] + n[2] * (double)r[2];   // plane offset n . c
+        v[4 * i + 2] = make_float4(r[6], r[7], r[8], (float)nc);
         v[4 * i + 3] = make_float4((float)vx, (float)vy, (float)vz, 0.0f);
     }
     int rc = upload_f4(c, &c->d_gates, v);

@@ -30,7 +30,7 @@ struct DevParams {
     float sigma_v, dv_max, v_theta_max, r_dv;   // the paper's own contouring, eq.(9) [R-33]..[R-37]
     float Qp, Qv, Qq, Qw, R;           // eq.(8)
     float q_c, q_l, mu, path_L, inv_path_L; // eq.(9) + closed path length
-    const float4* gates;               // [G][4]: (c, a_h) (n, a_v) (h, 0) (v = h x n, 0)
+    const float4* gates;               // [G][4]: (c, a_h) (n, a_v) (h, n.c) (v = h x n, 0)
     const float4* ref;                 // [M][4]: (p, qw) (qx qy qz, vx) (vy vz, wx wy) (wz,0,0,0)
     const float4* path;                // [2][P]: all (P_i, s_i), then all (t_i, 0)
 };
