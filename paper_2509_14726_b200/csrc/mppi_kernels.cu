@@ -41,7 +41,7 @@ size_t rollout_smem_bytes(const DevParams& P, const LaunchCfg& c)
 // packed throughput variant: two samples per thread in fp32x2 registers (mppi_packed.cuh).
 // grid = (K / (2 blockDim.x), B); thread j of the grid row owns samples 2j and 2j+1.
 // ---------------------------------------------------------------------------------------------
-template <int OBJ, int MATH>
+template <int OBJ, int MATH, bool SYMZ>
 __device__ __forceinline__ void rollout_cost2(const DevParams& P, const StepArgs& A, const float4* s_unom,
                                               const float4* s_trk, State2 x, int start, int contour_i0,
                                               uint32_t k0, uint32_t b, float4* du_out, float& Ja, float& Jb)
@@ -67,7 +67,7 @@ __device__ __forceinline__ void rollout_cost2(const DevParams& P, const StepArgs
             Ja += track_stage(P, s_trk + 4 * t, lane_state<0>(x), Ta);
             Jb += track_stage(P, s_trk + 4 * t, lane_state<1>(x), Tb);
         }
-        rk4_step2(P, x, Ta, Tb);
+        rk4_step2<SYMZ>(P, x, Ta, Tb);
         if (OBJ == OBJ_GATE) {
             ga.step<MATH>(P, s_trk, lane_state<0>(x));
             gb.step<MATH>(P, s_trk, lane_state<1>(x));
@@ -118,8 +118,11 @@ __global__ void __launch_bounds__(MPPI_PK_THREADS, MPPI_PK_MINB) rollout2_kernel
     const State x0 = load_state(A.x0 + 13 * b);
     const int i0 = OBJ == OBJ_CONTOUR ? contour_start_index(P, s_trk, start, x0, s_red) : 0;
     float Ja, Jb;
-    rollout_cost2<OBJ, MATH>(P, A, s_unom, s_trk, splat_state(x0), start, i0, (uint32_t)k0, (uint32_t)b,
-                             STORE_DU ? A.du + (size_t)b * N * P.K + k0 : nullptr, Ja, Jb);
+    float4* const du_out = STORE_DU ? A.du + (size_t)b * N * P.K + k0 : nullptr;
+    if (OBJ != OBJ_CONTOUR && P.gyz == 0.0f)       // (the contouring search is bound by shared memory) Jx == Jy: the yaw-rate derivative is constant over the step (rk4_step2<true>)
+        rollout_cost2<OBJ, MATH, true>(P, A, s_unom, s_trk, splat_state(x0), start, i0, (uint32_t)k0, (uint32_t)b, du_out, Ja, Jb);
+    else
+        rollout_cost2<OBJ, MATH, false>(P, A, s_unom, s_trk, splat_state(x0), start, i0, (uint32_t)k0, (uint32_t)b, du_out, Ja, Jb);
     *reinterpret_cast<float2*>(A.cost + (size_t)b * P.K + k0) = make_float2(Ja, Jb);
 
     if (!FUSED) return;

@@ -53,6 +53,11 @@ __device__ __forceinline__ State lane_state(const State2& s)
 
 // x <- RK4(f_dyn, x, T, dt), q <- q/|q| for two samples; Ta / Tb are their clamped rotor thrusts.
 // Same formulation as rk4_step (mppi_device.cuh): eq.(2), [R-4], [R-5].
+// SYMZ: the caller has checked P.gyz == 0 (Jx == Jy, the usual symmetric airframe and every config of
+// BASELINE.json): fma(0, ox oy, az) is az bit for bit, so the yaw-rate derivative of all four stages is
+// the constant az and its eight multiply-adds (and the third-stage yaw rate, equal to the second) drop
+// out with results identical to the general form.
+template <bool SYMZ>
 __device__ __forceinline__ void rk4_step2(const DevParams& P, State2& x, const float4 Ta, const float4 Tb)
 {
     const float2 T0 = make_float2(Ta.x, Tb.x), T1 = make_float2(Ta.y, Tb.y), T2 = make_float2(Ta.z, Tb.z),
@@ -68,7 +73,7 @@ __device__ __forceinline__ void rk4_step2(const DevParams& P, State2& x, const f
 
 #define MPPI_STAGE_DERIV(OX, OY, OZ, QW, QX, QY, QZ)                                        \
     kox = fma2(P.gyx, mul2(OY, OZ), ax); koy = fma2(P.gyy, mul2(OZ, OX), ay);              \
-    koz = fma2(P.gyz, mul2(OX, OY), az);                                                     \
+    koz = SYMZ ? az : fma2(P.gyz, mul2(OX, OY), az);                                         \
     gw = fma2(neg2(QZ), OZ, fma2(neg2(QY), OY, mul2(neg2(QX), OX)));                         \
     gx = fma2(neg2(QZ), OY, fma2(QY, OZ, mul2(QW, OX)));                                     \
     gy = fma2(neg2(QX), OZ, fma2(QZ, OX, mul2(QW, OY)));                                     \

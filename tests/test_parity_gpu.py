@@ -109,6 +109,20 @@ def test_stress_gate_crossings(pipe, math):
     assert (nc > 0).mean() > 0.3 and (nc == 0).mean() > 0.1      # pass and miss branches both taken
 
 
+@pytest.mark.parametrize("pipe", PIPES, ids=PIPE_IDS)
+@pytest.mark.parametrize("name", ["stress_gate", "cfg2"])
+def test_asymmetric_inertia(name, pipe):
+    # Jx != Jy: the yaw-rate derivative gets its gyroscopic term (the packed kernel then leaves its
+    # symmetric-airframe short-cut, rk4_step2<false>); every kernel against the oracle, fast math
+    wl = W.stress_gate(K=4096, N=30) if name == "stress_gate" else W.cfg2()
+    wl.params.update(Jx=1.0e-3, Jy=1.6e-3, Jz=2.1e-3)
+    g, o, st = run_case(wl, f"asym_{name}[{pipe}]", fast_math=1, **pipe)
+    wl0 = W.stress_gate(K=4096, N=30) if name == "stress_gate" else W.cfg2()
+    wl0.params.update(Jx=1.3e-3, Jy=1.3e-3, Jz=2.1e-3)
+    o0 = Pz.oracle_step(wl0, wl0.x0, wl0.start, wl0.u_nom, wl0.seed, 0)
+    assert (np.abs(o0["cost"] - o["cost"]) > 1e-3 * np.abs(o["cost"])).mean() > 0.5      # the asymmetry matters
+
+
 def test_cfg4_closed_loop_teacher_forced():
     # [R-17] 64 drones, closed loop on the GPU (plant + shift kernel); at checked control steps the
     # oracle gets the GPU loop's actual (x, start, u_nom, iter) and is compared for that one step
