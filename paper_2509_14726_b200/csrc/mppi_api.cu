@@ -313,6 +313,8 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     d.q_near = p->q_near; d.r_near2 = (float)((double)p->r_near * (double)p->r_near);
     d.input_model = p->input_model; d.rate_max = p->rate_max;
     d.drag_x = p->drag_x; d.drag_y = p->drag_y; d.drag_z = p->drag_z;
+    d.drag4_x = 4.0f * p->drag_x; d.drag4_y = 4.0f * p->drag_y; d.drag4_z = 4.0f * p->drag_z;
+    d.inv_mass2 = 2.0f * d.inv_mass;                       // exact rescalings (fdyn_general, mppi_rate.cuh)
     d.w_limit = p->w_limit; d.omega_max = p->omega_max;
     d.sigma_v = p->sigma_v; d.dv_max = p->dv_max; d.v_theta_max = p->v_theta_max; d.r_dv = p->r_dv;
     d.Qp = p->Qp; d.Qv = p->Qv; d.Qq = p->Qq; d.Qw = p->Qw; d.R = p->R;

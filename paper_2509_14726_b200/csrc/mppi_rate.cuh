@@ -7,36 +7,39 @@
 
 namespace mppi {
 
-struct Deriv { float qw, qx, qy, qz, vx, vy, vz, ox, oy, oz; };     // p' = v needs no slot
+struct Deriv { float qw, qx, qy, qz, vx, vy, vz, ox, oy, oz; };     // q slots: 2 q'; p' = v needs no slot
 
 // f_dyn of eq.(2) for the attitude, velocity and body-rate parts at stage state (q, v, o) with rotor
-// thrusts T.  q' carries its 1/2 here (general form).
+// thrusts T.  Powers of two are kept out of the inner arithmetic (exact rescalings, folded into host
+// constants and step sizes): the q slots hold G = 2 q' = q (x) (0, omega); R(q) is formed as its half
+// E = R / 2 (diagonal 1/2 - (a^2 + b^2) in two FFMAs, off-diagonals without their factor 2), so
+// - R D R^T v = - E (4 D) E^T v with drag4 = 4 D and the thrust term is (2 S / m) e2 with inv_mass2 = 2 / m.
 __device__ __forceinline__ Deriv fdyn_general(const DevParams& P, const float qw, const float qx, const float qy,
                                               const float qz, const float vx, const float vy, const float vz,
                                               const float ox, const float oy, const float oz, const float4 T)
 {
     Deriv d;
-    d.qw = 0.5f * fmaf(-qz, oz, fmaf(-qy, oy, -qx * ox));
-    d.qx = 0.5f * fmaf(-qz, oy, fmaf(qy, oz, qw * ox));
-    d.qy = 0.5f * fmaf(-qx, oz, fmaf(qz, ox, qw * oy));
-    d.qz = 0.5f * fmaf(-qy, ox, fmaf(qx, oy, qw * oz));
+    d.qw = fmaf(-qz, oz, fmaf(-qy, oy, -qx * ox));
+    d.qx = fmaf(-qz, oy, fmaf(qy, oz, qw * ox));
+    d.qy = fmaf(-qx, oz, fmaf(qz, ox, qw * oy));
+    d.qz = fmaf(-qy, ox, fmaf(qx, oy, qw * oz));
     const float s01 = T.x + T.y, s23 = T.z + T.w;
     d.ox = fmaf(P.gyx, oy * oz, P.ltx * (s01 - s23));                  // PAPER.md:70, J^-1 folded in
     const float d10 = T.y - T.x, d23 = T.z - T.w;                      // (T1 + T2) - (T0 + T3) = d10 + d23, (T0 + T2) - (T1 + T3) = d23 - d10
     d.oy = fmaf(P.gyy, oz * ox, P.lty * (d10 + d23));
     d.oz = fmaf(P.gyz, ox * oy, P.ltz * (d23 - d10));
-    // columns of R(q): the body axes in the world frame
-    const float c0x = 1.0f - 2.0f * (qy * qy + qz * qz), c0y = 2.0f * (qx * qy + qw * qz), c0z = 2.0f * (qx * qz - qw * qy);
-    const float c1x = 2.0f * (qx * qy - qw * qz), c1y = 1.0f - 2.0f * (qx * qx + qz * qz), c1z = 2.0f * (qy * qz + qw * qx);
-    const float c2x = 2.0f * (qx * qz + qw * qy), c2y = 2.0f * (qy * qz - qw * qx), c2z = 1.0f - 2.0f * (qx * qx + qy * qy);
-    const float c = (s01 + s23) * P.inv_mass;
+    // half columns of R(q): the body axes in the world frame, times 1/2
+    const float e0x = fmaf(-qz, qz, fmaf(-qy, qy, 0.5f)), e0y = fmaf(qx, qy, qw * qz), e0z = fmaf(qx, qz, -qw * qy);
+    const float e1x = fmaf(qx, qy, -qw * qz), e1y = fmaf(-qz, qz, fmaf(-qx, qx, 0.5f)), e1z = fmaf(qy, qz, qw * qx);
+    const float e2x = fmaf(qx, qz, qw * qy), e2y = fmaf(qy, qz, -qw * qx), e2z = fmaf(-qy, qy, fmaf(-qx, qx, 0.5f));
+    const float c = (s01 + s23) * P.inv_mass2;                         // 2 S / m
     // - R D R^T v: project v on each body axis, scale by that axis' coefficient [R-30]
-    const float b0 = P.drag_x * fmaf(c0z, vz, fmaf(c0y, vy, c0x * vx));
-    const float b1 = P.drag_y * fmaf(c1z, vz, fmaf(c1y, vy, c1x * vx));
-    const float b2 = P.drag_z * fmaf(c2z, vz, fmaf(c2y, vy, c2x * vx));
-    d.vx = fmaf(c, c2x, -fmaf(c2x, b2, fmaf(c1x, b1, c0x * b0)));
-    d.vy = fmaf(c, c2y, -fmaf(c2y, b2, fmaf(c1y, b1, c0y * b0)));
-    d.vz = fmaf(c, c2z, -fmaf(c2z, b2, fmaf(c1z, b1, c0z * b0))) - P.g;
+    const float b0 = P.drag4_x * fmaf(e0z, vz, fmaf(e0y, vy, e0x * vx));
+    const float b1 = P.drag4_y * fmaf(e1z, vz, fmaf(e1y, vy, e1x * vx));
+    const float b2 = P.drag4_z * fmaf(e2z, vz, fmaf(e2y, vy, e2x * vx));
+    d.vx = fmaf(c, e2x, -fmaf(e2x, b2, fmaf(e1x, b1, e0x * b0)));
+    d.vy = fmaf(c, e2y, -fmaf(e2y, b2, fmaf(e1y, b1, e0y * b0)));
+    d.vz = fmaf(c, e2z, -fmaf(e2z, b2, fmaf(e1z, b1, e0z * b0))) - P.g;
     return d;
 }
 
@@ -44,7 +47,7 @@ __device__ __forceinline__ Deriv fdyn_general(const DevParams& P, const float qw
 // thrust states projected onto [T_min, T_max] afterwards [R-27],[R-29].
 __device__ __forceinline__ void rk4_rate_step(const DevParams& P, State& x, float4& T, const float4 u)
 {
-    const float h = P.dt, hh = P.h2;
+    const float h = P.dt, hh = P.h2, hq = P.h4;                       // hq: the q slots of Deriv hold 2 q'
     const float4 Tm = make_float4(fmaf(hh, u.x, T.x), fmaf(hh, u.y, T.y), fmaf(hh, u.z, T.z), fmaf(hh, u.w, T.w));
     const float4 Te = make_float4(fmaf(h, u.x, T.x), fmaf(h, u.y, T.y), fmaf(h, u.z, T.z), fmaf(h, u.w, T.w));
     // stage 1
@@ -52,7 +55,7 @@ __device__ __forceinline__ void rk4_rate_step(const DevParams& P, State& x, floa
     float apx = x.vx, apy = x.vy, apz = x.vz;                         // sums of p' = v over the stages
     Deriv a = k;
     float vx = fmaf(hh, k.vx, x.vx), vy = fmaf(hh, k.vy, x.vy), vz = fmaf(hh, k.vz, x.vz);
-    float qw = fmaf(hh, k.qw, x.qw), qx = fmaf(hh, k.qx, x.qx), qy = fmaf(hh, k.qy, x.qy), qz = fmaf(hh, k.qz, x.qz);
+    float qw = fmaf(hq, k.qw, x.qw), qx = fmaf(hq, k.qx, x.qx), qy = fmaf(hq, k.qy, x.qy), qz = fmaf(hq, k.qz, x.qz);
     float ox = fmaf(hh, k.ox, x.ox), oy = fmaf(hh, k.oy, x.oy), oz = fmaf(hh, k.oz, x.oz);
 #define MPPI_ACC(W)                                                                                    \
     a.qw = fmaf(W, k.qw, a.qw); a.qx = fmaf(W, k.qx, a.qx); a.qy = fmaf(W, k.qy, a.qy); a.qz = fmaf(W, k.qz, a.qz); \
@@ -63,14 +66,14 @@ __device__ __forceinline__ void rk4_rate_step(const DevParams& P, State& x, floa
     k = fdyn_general(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Tm);
     MPPI_ACC(2.0f)
     vx = fmaf(hh, k.vx, x.vx); vy = fmaf(hh, k.vy, x.vy); vz = fmaf(hh, k.vz, x.vz);
-    qw = fmaf(hh, k.qw, x.qw); qx = fmaf(hh, k.qx, x.qx); qy = fmaf(hh, k.qy, x.qy); qz = fmaf(hh, k.qz, x.qz);
+    qw = fmaf(hq, k.qw, x.qw); qx = fmaf(hq, k.qx, x.qx); qy = fmaf(hq, k.qy, x.qy); qz = fmaf(hq, k.qz, x.qz);
     ox = fmaf(hh, k.ox, x.ox); oy = fmaf(hh, k.oy, x.oy); oz = fmaf(hh, k.oz, x.oz);
     // stage 3
     apx = fmaf(2.0f, vx, apx); apy = fmaf(2.0f, vy, apy); apz = fmaf(2.0f, vz, apz);
     k = fdyn_general(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Tm);
     MPPI_ACC(2.0f)
     vx = fmaf(h, k.vx, x.vx); vy = fmaf(h, k.vy, x.vy); vz = fmaf(h, k.vz, x.vz);
-    qw = fmaf(h, k.qw, x.qw); qx = fmaf(h, k.qx, x.qx); qy = fmaf(h, k.qy, x.qy); qz = fmaf(h, k.qz, x.qz);
+    qw = fmaf(hh, k.qw, x.qw); qx = fmaf(hh, k.qx, x.qx); qy = fmaf(hh, k.qy, x.qy); qz = fmaf(hh, k.qz, x.qz);
     ox = fmaf(h, k.ox, x.ox); oy = fmaf(h, k.oy, x.oy); oz = fmaf(h, k.oz, x.oz);
     // stage 4 (state x + h k3, thrusts T + h u)
     apx += vx; apy += vy; apz += vz;
@@ -81,7 +84,8 @@ __device__ __forceinline__ void rk4_rate_step(const DevParams& P, State& x, floa
     x.px = fmaf(h6, apx, x.px); x.py = fmaf(h6, apy, x.py); x.pz = fmaf(h6, apz, x.pz);
     x.vx = fmaf(h6, a.vx, x.vx); x.vy = fmaf(h6, a.vy, x.vy); x.vz = fmaf(h6, a.vz, x.vz);
     x.ox = fmaf(h6, a.ox, x.ox); x.oy = fmaf(h6, a.oy, x.oy); x.oz = fmaf(h6, a.oz, x.oz);
-    const float nw = fmaf(h6, a.qw, x.qw), nx = fmaf(h6, a.qx, x.qx), ny = fmaf(h6, a.qy, x.qy), nz = fmaf(h6, a.qz, x.qz);
+    const float h12 = P.h12;
+    const float nw = fmaf(h12, a.qw, x.qw), nx = fmaf(h12, a.qx, x.qx), ny = fmaf(h12, a.qy, x.qy), nz = fmaf(h12, a.qz, x.qz);
     const float inv = rsqrtf(fmaf(nz, nz, fmaf(ny, ny, fmaf(nx, nx, nw * nw))));
     x.qw = nw * inv; x.qx = nx * inv; x.qy = ny * inv; x.qz = nz * inv;
     T.x = fminf(fmaxf(Te.x, P.T_min), P.T_max); T.y = fminf(fmaxf(Te.y, P.T_min), P.T_max);
@@ -162,30 +166,30 @@ __device__ __forceinline__ Deriv2 fdyn_general2(const DevParams& P, const float2
                                                 const float2 ox, const float2 oy, const float2 oz, const float2 T0,
                                                 const float2 T1, const float2 T2, const float2 T3)
 {
-    Deriv2 d;
-    const float2 hf = bc2(0.5f), two = bc2(2.0f), one = bc2(1.0f), m2 = bc2(-2.0f);
-    d.qw = mul2(hf, fma2(neg2(qz), oz, fma2(neg2(qy), oy, mul2(neg2(qx), ox))));
-    d.qx = mul2(hf, fma2(neg2(qz), oy, fma2(qy, oz, mul2(qw, ox))));
-    d.qy = mul2(hf, fma2(neg2(qx), oz, fma2(qz, ox, mul2(qw, oy))));
-    d.qz = mul2(hf, fma2(neg2(qy), ox, fma2(qx, oy, mul2(qw, oz))));
+    Deriv2 d;                                  // same operations, same order as fdyn_general on each half
+    const float2 hf = bc2(0.5f);
+    d.qw = fma2(neg2(qz), oz, fma2(neg2(qy), oy, mul2(neg2(qx), ox)));
+    d.qx = fma2(neg2(qz), oy, fma2(qy, oz, mul2(qw, ox)));
+    d.qy = fma2(neg2(qx), oz, fma2(qz, ox, mul2(qw, oy)));
+    d.qz = fma2(neg2(qy), ox, fma2(qx, oy, mul2(qw, oz)));
     const float2 s01 = add2(T0, T1), s23 = add2(T2, T3);
     d.ox = fma2(P.gyx, mul2(oy, oz), mul2(bc2(P.ltx), sub2(s01, s23)));
     const float2 d10 = sub2(T1, T0), d23 = sub2(T2, T3);
     d.oy = fma2(P.gyy, mul2(oz, ox), mul2(bc2(P.lty), add2(d10, d23)));
     d.oz = fma2(P.gyz, mul2(ox, oy), mul2(bc2(P.ltz), sub2(d23, d10)));
-    const float2 c0x = fma2(m2, fma2(qy, qy, mul2(qz, qz)), one), c0y = mul2(two, fma2(qx, qy, mul2(qw, qz))),
-                 c0z = mul2(two, fma2(qx, qz, mul2(neg2(qw), qy)));
-    const float2 c1x = mul2(two, fma2(qx, qy, mul2(neg2(qw), qz))), c1y = fma2(m2, fma2(qx, qx, mul2(qz, qz)), one),
-                 c1z = mul2(two, fma2(qy, qz, mul2(qw, qx)));
-    const float2 c2x = mul2(two, fma2(qx, qz, mul2(qw, qy))), c2y = mul2(two, fma2(qy, qz, mul2(neg2(qw), qx))),
-                 c2z = fma2(m2, fma2(qx, qx, mul2(qy, qy)), one);
-    const float2 c = mul2(add2(s01, s23), bc2(P.inv_mass));
-    const float2 b0 = mul2(bc2(P.drag_x), fma2(c0z, vz, fma2(c0y, vy, mul2(c0x, vx))));
-    const float2 b1 = mul2(bc2(P.drag_y), fma2(c1z, vz, fma2(c1y, vy, mul2(c1x, vx))));
-    const float2 b2 = mul2(bc2(P.drag_z), fma2(c2z, vz, fma2(c2y, vy, mul2(c2x, vx))));
-    d.vx = fma2(c, c2x, neg2(fma2(c2x, b2, fma2(c1x, b1, mul2(c0x, b0)))));
-    d.vy = fma2(c, c2y, neg2(fma2(c2y, b2, fma2(c1y, b1, mul2(c0y, b0)))));
-    d.vz = sub2(fma2(c, c2z, neg2(fma2(c2z, b2, fma2(c1z, b1, mul2(c0z, b0))))), bc2(P.g));
+    const float2 e0x = fma2(neg2(qz), qz, fma2(neg2(qy), qy, hf)), e0y = fma2(qx, qy, mul2(qw, qz)),
+                 e0z = fma2(qx, qz, mul2(neg2(qw), qy));
+    const float2 e1x = fma2(qx, qy, mul2(neg2(qw), qz)), e1y = fma2(neg2(qz), qz, fma2(neg2(qx), qx, hf)),
+                 e1z = fma2(qy, qz, mul2(qw, qx));
+    const float2 e2x = fma2(qx, qz, mul2(qw, qy)), e2y = fma2(qy, qz, mul2(neg2(qw), qx)),
+                 e2z = fma2(neg2(qy), qy, fma2(neg2(qx), qx, hf));
+    const float2 c = mul2(add2(s01, s23), bc2(P.inv_mass2));
+    const float2 b0 = mul2(bc2(P.drag4_x), fma2(e0z, vz, fma2(e0y, vy, mul2(e0x, vx))));
+    const float2 b1 = mul2(bc2(P.drag4_y), fma2(e1z, vz, fma2(e1y, vy, mul2(e1x, vx))));
+    const float2 b2 = mul2(bc2(P.drag4_z), fma2(e2z, vz, fma2(e2y, vy, mul2(e2x, vx))));
+    d.vx = fma2(c, e2x, neg2(fma2(e2x, b2, fma2(e1x, b1, mul2(e0x, b0)))));
+    d.vy = fma2(c, e2y, neg2(fma2(e2y, b2, fma2(e1y, b1, mul2(e0y, b0)))));
+    d.vz = sub2(fma2(c, e2z, neg2(fma2(e2z, b2, fma2(e1z, b1, mul2(e0z, b0))))), bc2(P.g));
     return d;
 }
 
@@ -197,31 +201,31 @@ __device__ __forceinline__ float2 clamp2(const float2 v, const float lo, const f
 // rk4_rate_step for two samples: x, T (4 rotor thrust pairs) <- one step with the rates ua / ub held
 __device__ __forceinline__ void rk4_rate_step2(const DevParams& P, State2& x, float2 (&T)[4], const float4 ua, const float4 ub)
 {
-    const float2 h = bc2(P.dt), hh = bc2(P.h2), h6 = bc2(P.h6), two = bc2(2.0f);
+    const float2 h = bc2(P.dt), hh = bc2(P.h2), hq = bc2(P.h4), h6 = bc2(P.h6), h12 = bc2(P.h12), two = bc2(2.0f);
     const float2 u0 = make_float2(ua.x, ub.x), u1 = make_float2(ua.y, ub.y), u2 = make_float2(ua.z, ub.z), u3 = make_float2(ua.w, ub.w);
     const float2 Tm0 = fma2(hh, u0, T[0]), Tm1 = fma2(hh, u1, T[1]), Tm2 = fma2(hh, u2, T[2]), Tm3 = fma2(hh, u3, T[3]);
     const float2 Te0 = fma2(h, u0, T[0]), Te1 = fma2(h, u1, T[1]), Te2 = fma2(h, u2, T[2]), Te3 = fma2(h, u3, T[3]);
     Deriv2 k = fdyn_general2(P, x.qw, x.qx, x.qy, x.qz, x.vx, x.vy, x.vz, x.ox, x.oy, x.oz, T[0], T[1], T[2], T[3]);
     float2 apx = x.vx, apy = x.vy, apz = x.vz;
     Deriv2 a = k;
-#define MPPI_STAGE2(HS)                                                                              \
+#define MPPI_STAGE2(HS, HQ)                                                                          \
     vx = fma2(HS, k.vx, x.vx); vy = fma2(HS, k.vy, x.vy); vz = fma2(HS, k.vz, x.vz);               \
-    qw = fma2(HS, k.qw, x.qw); qx = fma2(HS, k.qx, x.qx); qy = fma2(HS, k.qy, x.qy); qz = fma2(HS, k.qz, x.qz); \
+    qw = fma2(HQ, k.qw, x.qw); qx = fma2(HQ, k.qx, x.qx); qy = fma2(HQ, k.qy, x.qy); qz = fma2(HQ, k.qz, x.qz); \
     ox = fma2(HS, k.ox, x.ox); oy = fma2(HS, k.oy, x.oy); oz = fma2(HS, k.oz, x.oz);
 #define MPPI_ACC2(W)                                                                                 \
     a.qw = fma2(W, k.qw, a.qw); a.qx = fma2(W, k.qx, a.qx); a.qy = fma2(W, k.qy, a.qy); a.qz = fma2(W, k.qz, a.qz); \
     a.vx = fma2(W, k.vx, a.vx); a.vy = fma2(W, k.vy, a.vy); a.vz = fma2(W, k.vz, a.vz);             \
     a.ox = fma2(W, k.ox, a.ox); a.oy = fma2(W, k.oy, a.oy); a.oz = fma2(W, k.oz, a.oz);
     float2 vx, vy, vz, qw, qx, qy, qz, ox, oy, oz;
-    MPPI_STAGE2(hh)
+    MPPI_STAGE2(hh, hq)
     apx = fma2(two, vx, apx); apy = fma2(two, vy, apy); apz = fma2(two, vz, apz);
     k = fdyn_general2(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Tm0, Tm1, Tm2, Tm3);
     MPPI_ACC2(two)
-    MPPI_STAGE2(hh)
+    MPPI_STAGE2(hh, hq)
     apx = fma2(two, vx, apx); apy = fma2(two, vy, apy); apz = fma2(two, vz, apz);
     k = fdyn_general2(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Tm0, Tm1, Tm2, Tm3);
     MPPI_ACC2(two)
-    MPPI_STAGE2(h)
+    MPPI_STAGE2(h, hh)
     apx = add2(apx, vx); apy = add2(apy, vy); apz = add2(apz, vz);
     k = fdyn_general2(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Te0, Te1, Te2, Te3);
     a.qw = add2(a.qw, k.qw); a.qx = add2(a.qx, k.qx); a.qy = add2(a.qy, k.qy); a.qz = add2(a.qz, k.qz);
@@ -232,7 +236,7 @@ __device__ __forceinline__ void rk4_rate_step2(const DevParams& P, State2& x, fl
     x.px = fma2(h6, apx, x.px); x.py = fma2(h6, apy, x.py); x.pz = fma2(h6, apz, x.pz);
     x.vx = fma2(h6, a.vx, x.vx); x.vy = fma2(h6, a.vy, x.vy); x.vz = fma2(h6, a.vz, x.vz);
     x.ox = fma2(h6, a.ox, x.ox); x.oy = fma2(h6, a.oy, x.oy); x.oz = fma2(h6, a.oz, x.oz);
-    const float2 nw = fma2(h6, a.qw, x.qw), nx = fma2(h6, a.qx, x.qx), ny = fma2(h6, a.qy, x.qy), nz = fma2(h6, a.qz, x.qz);
+    const float2 nw = fma2(h12, a.qw, x.qw), nx = fma2(h12, a.qx, x.qx), ny = fma2(h12, a.qy, x.qy), nz = fma2(h12, a.qz, x.qz);
     const float2 n2 = fma2(nz, nz, fma2(ny, ny, fma2(nx, nx, mul2(nw, nw))));
     const float2 inv = make_float2(rsqrtf(n2.x), rsqrtf(n2.y));
     x.qw = mul2(nw, inv); x.qx = mul2(nx, inv); x.qy = mul2(ny, inv); x.qz = mul2(nz, inv);
