@@ -39,7 +39,7 @@ UNIT = "sample-steps/s"
 FLOPS_PER_SAMPLE_STEP = {0: 417.0, 1: 449.0, 2: 685.0}
 FP32_LANES_PER_SM = 128
 L2_FLUSH_BYTES = 256 << 20
-NCU_DRAM_BYTES_PER_LAUNCH = 56320     # rollout_pipe_kernel<gate>, cfg1: 56.3 KB read + 0 B written (profiles/README_r01b.md)
+NCU_DRAM_BYTES_PER_LAUNCH = 53248     # rollout_pipe_kernel<gate>, cfg1: 53.2 KB read + 0 B written (profiles/README_r01e.md)
 
 
 def dist_env():
@@ -359,7 +359,7 @@ def run_ours(args):
             "gpu_launches": int(launches),
             "roofline": {"bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
                          # dram__bytes_read.sum + dram__bytes_write.sum of this kernel, per launch, from the
-                         # ncu --set full capture summarised in profiles/README_r01b.md (not measured live)
+                         # ncu --set full capture summarised in profiles/README_r01e.md (not measured live)
                          "traffic": NCU_DRAM_BYTES_PER_LAUNCH if args.pipeline == 0 else None, "kernel": "the iteration's single kernel (pipelined rollout + cost + fused softmax update)" if args.pipeline == 0 else "rollout kernel of the two-pass pipeline",
                          "flops_per_sample_step": flops, "units_per_launch": units,
                          "peak_how": f"{sm} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 x clocks.max.sm (B200_PROFILING.md)",
