@@ -314,6 +314,7 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     d.input_model = p->input_model; d.rate_max = p->rate_max;
     d.drag_x = p->drag_x; d.drag_y = p->drag_y; d.drag_z = p->drag_z;
     d.drag4_x = 4.0f * p->drag_x; d.drag4_y = 4.0f * p->drag_y; d.drag4_z = 4.0f * p->drag_z;
+    d.drag_dd4 = (float)(4.0 * ((double)p->drag_z - (double)p->drag_x));
     d.inv_mass2 = 2.0f * d.inv_mass;                       // exact rescalings (fdyn_general, mppi_rate.cuh)
     d.w_limit = p->w_limit; d.omega_max = p->omega_max;
     d.sigma_v = p->sigma_v; d.dv_max = p->dv_max; d.v_theta_max = p->v_theta_max; d.r_dv = p->r_dv;

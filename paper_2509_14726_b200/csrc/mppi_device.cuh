@@ -27,6 +27,7 @@ struct DevParams {
     // the paper's own input model (Table I) [R-27]..[R-32]: u = dT/dt, thrusts are states
     int input_model;
     float rate_max, drag_x, drag_y, drag_z, w_limit, omega_max;
+    float drag_dd4;                    // 4 (drag_z - drag_x): axisymmetric form of the drag (drag_x == drag_y)
     float drag4_x, drag4_y, drag4_z, inv_mass2;   // 4 D and 2 / m: fdyn_general works with R / 2 (mppi_rate.cuh)
     float sigma_v, dv_max, v_theta_max, r_dv;   // the paper's own contouring, eq.(9) [R-33]..[R-37]
     float Qp, Qv, Qq, Qw, R;           // eq.(8)

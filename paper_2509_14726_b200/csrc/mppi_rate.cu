@@ -5,6 +5,7 @@
 // Readings R-27..R-32 of DESIGN.md.  First correct path: one sample per thread, the 17-dim state in
 // registers, a general 4-stage RK4 (the drag makes v' depend on v, so the triangular short-cuts of
 // rk4_step do not apply), the same objectives and the same fused softmax update as rollout_kernel.
+#include <type_traits>
 #include "mppi_internal.h"
 #include "mppi_rollout.cuh"
 #include "mppi_rate.cuh"
@@ -54,6 +55,8 @@ __global__ void __launch_bounds__(256, 3) rollout_rate_kernel(const DevParams P,
     if (OBJ == OBJ_GATE_PAPER) gp.init(P, s_trk, start, x);
     if (OBJ == OBJ_CONTOUR) cc.init(P, s_trk, i0, x);
     float4* du_out = STORE_DU ? A.du + (size_t)b * N * P.K + k : nullptr;
+    // the horizon loop, instantiated for the axisymmetric drag form (drag_x == drag_y) and the general one
+    auto horizon = [&](auto axi) {
     for (int t = 0; t < N; ++t) {
         const float4 un = s_unom[t];
         const float4 u = sample_input<MATH>(P, A.rk, (uint32_t)k, (uint32_t)t, A.iter, (uint32_t)b, un, lo, hi);
@@ -67,12 +70,14 @@ __global__ void __launch_bounds__(256, 3) rollout_rate_kernel(const DevParams P,
             theta = fmaf(P.hh2, dv, fmaf(P.dt, v_theta, theta));
             v_theta = fminf(fmaxf(fmaf(P.dt, dv, v_theta), 0.0f), P.v_theta_max);
         }
-        rk4_rate_step(P, x, T, u);
+        rk4_rate_step<decltype(axi)::value>(P, x, T, u);
         J += rate_limit_cost(P, x);
-        if (OBJ == OBJ_GATE) gc.step<MATH>(P, s_trk, x);
+        if (OBJ == OBJ_GATE) gc.template step<MATH>(P, s_trk, x);
         if (OBJ == OBJ_GATE_PAPER) gp.step(P, s_trk, s_front, x, t);
         if (OBJ == OBJ_CONTOUR) J += cc.step(P, s_trk, x);
     }
+    };
+    if (P.drag_x == P.drag_y) horizon(std::true_type{}); else horizon(std::false_type{});
     if (OBJ == OBJ_GATE) J += gc.finish<MATH>(P, s_trk, x);
     if (OBJ == OBJ_GATE_PAPER) J += gp.finish(P);
     if (OBJ == OBJ_TRACK) J += track_state_term(P, s_trk + 4 * N, x);
@@ -122,6 +127,7 @@ __global__ void __launch_bounds__(128, 3) rollout_rate2_kernel(const DevParams P
     if (OBJ == OBJ_GATE) { ga.init<MATH>(P, s_trk, start, x0); gb = ga; }
     if (OBJ == OBJ_GATE_PAPER) { pa.init(P, s_trk, start, x0); pb = pa; }
     float4* du_out = STORE_DU ? A.du + (size_t)b * N * P.K + k0 : nullptr;
+    auto horizon = [&](auto axi) {         // as in rollout_rate_kernel: axisymmetric drag form / general form
     for (int t = 0; t < N; ++t) {
         const float4 un = s_unom[t];
         const float4 ua = sample_input<MATH>(P, A.rk, (uint32_t)k0, (uint32_t)t, A.iter, (uint32_t)b, un, lo, hi);
@@ -134,13 +140,15 @@ __global__ void __launch_bounds__(128, 3) rollout_rate2_kernel(const DevParams P
             Ja += fmaf(P.R, ua.x * ua.x + ua.y * ua.y + ua.z * ua.z + ua.w * ua.w, track_state_term(P, s_trk + 4 * t, lane_state<0>(x)));
             Jb += fmaf(P.R, ub.x * ub.x + ub.y * ub.y + ub.z * ub.z + ub.w * ub.w, track_state_term(P, s_trk + 4 * t, lane_state<1>(x)));
         }
-        rk4_rate_step2(P, x, T, ua, ub);
+        rk4_rate_step2<decltype(axi)::value>(P, x, T, ua, ub);
         const State xa = lane_state<0>(x), xc = lane_state<1>(x);
         Ja += rate_limit_cost(P, xa);
         Jb += rate_limit_cost(P, xc);
-        if (OBJ == OBJ_GATE) { ga.step<MATH>(P, s_trk, xa); gb.step<MATH>(P, s_trk, xc); }
+        if (OBJ == OBJ_GATE) { ga.template step<MATH>(P, s_trk, xa); gb.template step<MATH>(P, s_trk, xc); }
         if (OBJ == OBJ_GATE_PAPER) { pa.step(P, s_trk, s_front, xa, t); pb.step(P, s_trk, s_front, xc, t); }
     }
+    };
+    if (P.drag_x == P.drag_y) horizon(std::true_type{}); else horizon(std::false_type{});
     if (OBJ == OBJ_GATE) { Ja += ga.finish<MATH>(P, s_trk, lane_state<0>(x)); Jb += gb.finish<MATH>(P, s_trk, lane_state<1>(x)); }
     if (OBJ == OBJ_GATE_PAPER) { Ja += pa.finish(P); Jb += pb.finish(P); }
     if (OBJ == OBJ_TRACK) {

@@ -14,6 +14,15 @@ struct Deriv { float qw, qx, qy, qz, vx, vy, vz, ox, oy, oz; };     // q slots: 
 // constants and step sizes): the q slots hold G = 2 q' = q (x) (0, omega); R(q) is formed as its half
 // E = R / 2 (diagonal 1/2 - (a^2 + b^2) in two FFMAs, off-diagonals without their factor 2), so
 // - R D R^T v = - E (4 D) E^T v with drag4 = 4 D and the thrust term is (2 S / m) e2 with inv_mass2 = 2 / m.
+// AXI != 0: the caller has checked drag_x == drag_y (rotor drag of an axisymmetric airframe, as in every
+// workload here): R D R^T = d_x R R^T + (d_z - d_x) r3 r3^T, so only the thrust axis r3 = 2 e2 is formed.
+// R(q) is the usual polynomial, evaluated at the UN-normalised stage quaternions of RK4 (that is the vector
+// field the oracle integrates): with n = |q|^2, u = (qx, qy, qz) it satisfies R R^T v = v + 4 (1 - n)
+// [(u . v) u - |u|^2 v] exactly, so
+//   v' = [2 S / m - 4 (d_z - d_x) (e2 . v)] e2 + (k |u|^2 - d_x) v - k (u . v) u - g z,   k = 4 d_x (1 - n).
+// AXI = 1: stage 1, where q is the step's normalised state (n = 1 to rounding, k dropped): 16 operations;
+// AXI = 2: inner stages with the k terms: 29 operations; general form: 43.
+template <int AXI = 0>
 __device__ __forceinline__ Deriv fdyn_general(const DevParams& P, const float qw, const float qx, const float qy,
                                               const float qz, const float vx, const float vy, const float vz,
                                               const float ox, const float oy, const float oz, const float4 T)
@@ -28,11 +37,28 @@ __device__ __forceinline__ Deriv fdyn_general(const DevParams& P, const float qw
     const float d10 = T.y - T.x, d23 = T.z - T.w;                      // (T1 + T2) - (T0 + T3) = d10 + d23, (T0 + T2) - (T1 + T3) = d23 - d10
     d.oy = fmaf(P.gyy, oz * ox, P.lty * (d10 + d23));
     d.oz = fmaf(P.gyz, ox * oy, P.ltz * (d23 - d10));
+    const float c = (s01 + s23) * P.inv_mass2;                         // 2 S / m
+    if (AXI) {
+        const float e2x = fmaf(qx, qz, qw * qy), e2y = fmaf(qy, qz, -qw * qx), e2z = fmaf(-qy, qy, fmaf(-qx, qx, 0.5f));
+        const float w = fmaf(-P.drag_dd4, fmaf(e2z, vz, fmaf(e2y, vy, e2x * vx)), c);
+        if (AXI == 1) {
+            d.vx = fmaf(w, e2x, -P.drag_x * vx);
+            d.vy = fmaf(w, e2y, -P.drag_x * vy);
+            d.vz = fmaf(w, e2z, fmaf(-P.drag_x, vz, -P.g));
+        } else {
+            const float uu = fmaf(qz, qz, fmaf(qy, qy, qx * qx));
+            const float k = fmaf(-P.drag4_x, fmaf(qw, qw, uu), P.drag4_x);
+            const float cu = -k * fmaf(qz, vz, fmaf(qy, vy, qx * vx)), cv = fmaf(k, uu, -P.drag_x);
+            d.vx = fmaf(w, e2x, fmaf(cv, vx, cu * qx));
+            d.vy = fmaf(w, e2y, fmaf(cv, vy, cu * qy));
+            d.vz = fmaf(w, e2z, fmaf(cv, vz, fmaf(cu, qz, -P.g)));
+        }
+        return d;
+    }
     // half columns of R(q): the body axes in the world frame, times 1/2
     const float e0x = fmaf(-qz, qz, fmaf(-qy, qy, 0.5f)), e0y = fmaf(qx, qy, qw * qz), e0z = fmaf(qx, qz, -qw * qy);
     const float e1x = fmaf(qx, qy, -qw * qz), e1y = fmaf(-qz, qz, fmaf(-qx, qx, 0.5f)), e1z = fmaf(qy, qz, qw * qx);
     const float e2x = fmaf(qx, qz, qw * qy), e2y = fmaf(qy, qz, -qw * qx), e2z = fmaf(-qy, qy, fmaf(-qx, qx, 0.5f));
-    const float c = (s01 + s23) * P.inv_mass2;                         // 2 S / m
     // - R D R^T v: project v on each body axis, scale by that axis' coefficient [R-30]
     const float b0 = P.drag4_x * fmaf(e0z, vz, fmaf(e0y, vy, e0x * vx));
     const float b1 = P.drag4_y * fmaf(e1z, vz, fmaf(e1y, vy, e1x * vx));
@@ -45,13 +71,14 @@ __device__ __forceinline__ Deriv fdyn_general(const DevParams& P, const float qw
 
 // x <- RK4 on the 17-vector [p, q, v, omega, T] with T' = u held over the step; q renormalised; the
 // thrust states projected onto [T_min, T_max] afterwards [R-27],[R-29].
+template <bool AXI = false>      // AXI: drag_x == drag_y (see fdyn_general)
 __device__ __forceinline__ void rk4_rate_step(const DevParams& P, State& x, float4& T, const float4 u)
 {
     const float h = P.dt, hh = P.h2, hq = P.h4;                       // hq: the q slots of Deriv hold 2 q'
     const float4 Tm = make_float4(fmaf(hh, u.x, T.x), fmaf(hh, u.y, T.y), fmaf(hh, u.z, T.z), fmaf(hh, u.w, T.w));
     const float4 Te = make_float4(fmaf(h, u.x, T.x), fmaf(h, u.y, T.y), fmaf(h, u.z, T.z), fmaf(h, u.w, T.w));
     // stage 1
-    Deriv k = fdyn_general(P, x.qw, x.qx, x.qy, x.qz, x.vx, x.vy, x.vz, x.ox, x.oy, x.oz, T);
+    Deriv k = fdyn_general<(AXI ? 1 : 0)>(P, x.qw, x.qx, x.qy, x.qz, x.vx, x.vy, x.vz, x.ox, x.oy, x.oz, T);
     float apx = x.vx, apy = x.vy, apz = x.vz;                         // sums of p' = v over the stages
     Deriv a = k;
     float vx = fmaf(hh, k.vx, x.vx), vy = fmaf(hh, k.vy, x.vy), vz = fmaf(hh, k.vz, x.vz);
@@ -63,21 +90,21 @@ __device__ __forceinline__ void rk4_rate_step(const DevParams& P, State& x, floa
     a.ox = fmaf(W, k.ox, a.ox); a.oy = fmaf(W, k.oy, a.oy); a.oz = fmaf(W, k.oz, a.oz);
     // stage 2 (state x + h/2 k1, thrusts T + h/2 u)
     apx = fmaf(2.0f, vx, apx); apy = fmaf(2.0f, vy, apy); apz = fmaf(2.0f, vz, apz);
-    k = fdyn_general(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Tm);
+    k = fdyn_general<(AXI ? 2 : 0)>(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Tm);
     MPPI_ACC(2.0f)
     vx = fmaf(hh, k.vx, x.vx); vy = fmaf(hh, k.vy, x.vy); vz = fmaf(hh, k.vz, x.vz);
     qw = fmaf(hq, k.qw, x.qw); qx = fmaf(hq, k.qx, x.qx); qy = fmaf(hq, k.qy, x.qy); qz = fmaf(hq, k.qz, x.qz);
     ox = fmaf(hh, k.ox, x.ox); oy = fmaf(hh, k.oy, x.oy); oz = fmaf(hh, k.oz, x.oz);
     // stage 3
     apx = fmaf(2.0f, vx, apx); apy = fmaf(2.0f, vy, apy); apz = fmaf(2.0f, vz, apz);
-    k = fdyn_general(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Tm);
+    k = fdyn_general<(AXI ? 2 : 0)>(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Tm);
     MPPI_ACC(2.0f)
     vx = fmaf(h, k.vx, x.vx); vy = fmaf(h, k.vy, x.vy); vz = fmaf(h, k.vz, x.vz);
     qw = fmaf(hh, k.qw, x.qw); qx = fmaf(hh, k.qx, x.qx); qy = fmaf(hh, k.qy, x.qy); qz = fmaf(hh, k.qz, x.qz);
     ox = fmaf(h, k.ox, x.ox); oy = fmaf(h, k.oy, x.oy); oz = fmaf(h, k.oz, x.oz);
     // stage 4 (state x + h k3, thrusts T + h u)
     apx += vx; apy += vy; apz += vz;
-    k = fdyn_general(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Te);
+    k = fdyn_general<(AXI ? 2 : 0)>(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Te);
     MPPI_ACC(1.0f)
 #undef MPPI_ACC
     const float h6 = P.h6;
@@ -161,6 +188,7 @@ __device__ __forceinline__ float contour_paper_stage(const DevParams& P, const f
 struct Deriv2 { float2 qw, qx, qy, qz, vx, vy, vz, ox, oy, oz; };
 
 // f_dyn of eq.(2) with drag for two samples; T0..T3: rotor thrusts (halves = the two samples)
+template <int AXI = 0>
 __device__ __forceinline__ Deriv2 fdyn_general2(const DevParams& P, const float2 qw, const float2 qx, const float2 qy,
                                                 const float2 qz, const float2 vx, const float2 vy, const float2 vz,
                                                 const float2 ox, const float2 oy, const float2 oz, const float2 T0,
@@ -177,13 +205,32 @@ __device__ __forceinline__ Deriv2 fdyn_general2(const DevParams& P, const float2
     const float2 d10 = sub2(T1, T0), d23 = sub2(T2, T3);
     d.oy = fma2(P.gyy, mul2(oz, ox), mul2(bc2(P.lty), add2(d10, d23)));
     d.oz = fma2(P.gyz, mul2(ox, oy), mul2(bc2(P.ltz), sub2(d23, d10)));
+    const float2 c = mul2(add2(s01, s23), bc2(P.inv_mass2));
+    if (AXI) {
+        const float2 e2x = fma2(qx, qz, mul2(qw, qy)), e2y = fma2(qy, qz, mul2(neg2(qw), qx)),
+                     e2z = fma2(neg2(qy), qy, fma2(neg2(qx), qx, hf));
+        const float2 w = fma2(bc2(-P.drag_dd4), fma2(e2z, vz, fma2(e2y, vy, mul2(e2x, vx))), c);
+        const float2 ndx = bc2(-P.drag_x);
+        if (AXI == 1) {
+            d.vx = fma2(w, e2x, mul2(ndx, vx));
+            d.vy = fma2(w, e2y, mul2(ndx, vy));
+            d.vz = fma2(w, e2z, fma2(ndx, vz, bc2(-P.g)));
+        } else {
+            const float2 uu = fma2(qz, qz, fma2(qy, qy, mul2(qx, qx)));
+            const float2 k = fma2(bc2(-P.drag4_x), fma2(qw, qw, uu), bc2(P.drag4_x));
+            const float2 cu = mul2(neg2(k), fma2(qz, vz, fma2(qy, vy, mul2(qx, vx)))), cv = fma2(k, uu, ndx);
+            d.vx = fma2(w, e2x, fma2(cv, vx, mul2(cu, qx)));
+            d.vy = fma2(w, e2y, fma2(cv, vy, mul2(cu, qy)));
+            d.vz = fma2(w, e2z, fma2(cv, vz, fma2(cu, qz, bc2(-P.g))));
+        }
+        return d;
+    }
     const float2 e0x = fma2(neg2(qz), qz, fma2(neg2(qy), qy, hf)), e0y = fma2(qx, qy, mul2(qw, qz)),
                  e0z = fma2(qx, qz, mul2(neg2(qw), qy));
     const float2 e1x = fma2(qx, qy, mul2(neg2(qw), qz)), e1y = fma2(neg2(qz), qz, fma2(neg2(qx), qx, hf)),
                  e1z = fma2(qy, qz, mul2(qw, qx));
     const float2 e2x = fma2(qx, qz, mul2(qw, qy)), e2y = fma2(qy, qz, mul2(neg2(qw), qx)),
                  e2z = fma2(neg2(qy), qy, fma2(neg2(qx), qx, hf));
-    const float2 c = mul2(add2(s01, s23), bc2(P.inv_mass2));
     const float2 b0 = mul2(bc2(P.drag4_x), fma2(e0z, vz, fma2(e0y, vy, mul2(e0x, vx))));
     const float2 b1 = mul2(bc2(P.drag4_y), fma2(e1z, vz, fma2(e1y, vy, mul2(e1x, vx))));
     const float2 b2 = mul2(bc2(P.drag4_z), fma2(e2z, vz, fma2(e2y, vy, mul2(e2x, vx))));
@@ -199,13 +246,14 @@ __device__ __forceinline__ float2 clamp2(const float2 v, const float lo, const f
 }
 
 // rk4_rate_step for two samples: x, T (4 rotor thrust pairs) <- one step with the rates ua / ub held
+template <bool AXI = false>
 __device__ __forceinline__ void rk4_rate_step2(const DevParams& P, State2& x, float2 (&T)[4], const float4 ua, const float4 ub)
 {
     const float2 h = bc2(P.dt), hh = bc2(P.h2), hq = bc2(P.h4), h6 = bc2(P.h6), h12 = bc2(P.h12), two = bc2(2.0f);
     const float2 u0 = make_float2(ua.x, ub.x), u1 = make_float2(ua.y, ub.y), u2 = make_float2(ua.z, ub.z), u3 = make_float2(ua.w, ub.w);
     const float2 Tm0 = fma2(hh, u0, T[0]), Tm1 = fma2(hh, u1, T[1]), Tm2 = fma2(hh, u2, T[2]), Tm3 = fma2(hh, u3, T[3]);
     const float2 Te0 = fma2(h, u0, T[0]), Te1 = fma2(h, u1, T[1]), Te2 = fma2(h, u2, T[2]), Te3 = fma2(h, u3, T[3]);
-    Deriv2 k = fdyn_general2(P, x.qw, x.qx, x.qy, x.qz, x.vx, x.vy, x.vz, x.ox, x.oy, x.oz, T[0], T[1], T[2], T[3]);
+    Deriv2 k = fdyn_general2<(AXI ? 1 : 0)>(P, x.qw, x.qx, x.qy, x.qz, x.vx, x.vy, x.vz, x.ox, x.oy, x.oz, T[0], T[1], T[2], T[3]);
     float2 apx = x.vx, apy = x.vy, apz = x.vz;
     Deriv2 a = k;
 #define MPPI_STAGE2(HS, HQ)                                                                          \
@@ -219,15 +267,15 @@ __device__ __forceinline__ void rk4_rate_step2(const DevParams& P, State2& x, fl
     float2 vx, vy, vz, qw, qx, qy, qz, ox, oy, oz;
     MPPI_STAGE2(hh, hq)
     apx = fma2(two, vx, apx); apy = fma2(two, vy, apy); apz = fma2(two, vz, apz);
-    k = fdyn_general2(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Tm0, Tm1, Tm2, Tm3);
+    k = fdyn_general2<(AXI ? 2 : 0)>(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Tm0, Tm1, Tm2, Tm3);
     MPPI_ACC2(two)
     MPPI_STAGE2(hh, hq)
     apx = fma2(two, vx, apx); apy = fma2(two, vy, apy); apz = fma2(two, vz, apz);
-    k = fdyn_general2(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Tm0, Tm1, Tm2, Tm3);
+    k = fdyn_general2<(AXI ? 2 : 0)>(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Tm0, Tm1, Tm2, Tm3);
     MPPI_ACC2(two)
     MPPI_STAGE2(h, hh)
     apx = add2(apx, vx); apy = add2(apy, vy); apz = add2(apz, vz);
-    k = fdyn_general2(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Te0, Te1, Te2, Te3);
+    k = fdyn_general2<(AXI ? 2 : 0)>(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Te0, Te1, Te2, Te3);
     a.qw = add2(a.qw, k.qw); a.qx = add2(a.qx, k.qx); a.qy = add2(a.qy, k.qy); a.qz = add2(a.qz, k.qz);
     a.vx = add2(a.vx, k.vx); a.vy = add2(a.vy, k.vy); a.vz = add2(a.vz, k.vz);
     a.ox = add2(a.ox, k.ox); a.oy = add2(a.oy, k.oy); a.oz = add2(a.oz, k.oz);

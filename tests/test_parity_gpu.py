@@ -448,6 +448,20 @@ def test_rate_model_objectives(name, pipe, math):
 
 
 @pytest.mark.parametrize("pipe", RATE_PIPES, ids=RATE_IDS)
+@pytest.mark.parametrize("name", ["rate_gate_paper", "rate_track"])
+def test_rate_model_anisotropic_drag(name, pipe):
+    # drag_x != drag_y: the scalar and packed kernels leave the axisymmetric short-cut of f_dyn
+    # (fdyn_general<false>: all three body axes projected); Jx != Jy on top
+    wl = W.ALL[name]()
+    wl.params.update(drag_x=np.float32(0.8), drag_y=np.float32(0.05), drag_z=np.float32(0.1), Jx=1.0e-3, Jy=1.5e-3)
+    g, o, st = run_case(wl, f"aniso_{name}[{pipe}]", fast_math=1, **pipe)
+    wl0 = W.ALL[name]()
+    wl0.params.update(drag_x=np.float32(0.425), drag_y=np.float32(0.425), drag_z=np.float32(0.1), Jx=1.0e-3, Jy=1.5e-3)
+    o0 = Pz.oracle_step(wl0, wl0.x0, wl0.start, wl0.u_nom, wl0.seed, 0)
+    assert (np.abs(o0["cost"] - o["cost"]) > 2e-4 * np.abs(o["cost"])).mean() > 0.2       # the anisotropy matters
+
+
+@pytest.mark.parametrize("pipe", RATE_PIPES, ids=RATE_IDS)
 def test_rate_model_saturation_and_crossings(pipe):
     wl = W.rate_stress(K=4096, N=30)
     g, o, st = run_case(wl, f"rate_stress[{pipe}]", **pipe)
