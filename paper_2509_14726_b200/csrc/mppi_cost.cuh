@@ -217,6 +217,62 @@ struct ContourCost {
         }
         return ibest;
     }
+    // The same search on the padded copy of the points that stage_inputs<OBJ_CONTOUR> appends to the path in
+    // shared memory: ext[j] = point (j - W), wrapped on a closed path, a far sentinel (distance inf, never
+    // the minimum) beyond the ends of an open one, ext = s_path + 2 P.  The window of `centre` is then the
+    // contiguous run ext[centre .. centre + 2W]: no wrap test per candidate, and with the window known at
+    // compile time (WFIX = 16, the default) every load has an immediate offset and is independent of the
+    // others.  Four runs of the window are scanned independently and merged in scan order -- a later
+    // run wins only when strictly smaller -- which keeps [R-12]'s first minimiser with a four times
+    // shorter dependency chain.  Distances are formed exactly as in nearest().
+    template <int LO, int HI>
+    __device__ __forceinline__ static void scan_run(const float4* w, float px, float py, float pz, float& best, int& ob)
+    {
+#pragma unroll
+        for (int o = LO; o < HI; ++o) {
+            const float4 q = w[o];
+            const float dx = px - q.x, dy = py - q.y, dz = pz - q.z;
+            const float d2 = dx * dx + dy * dy + dz * dz;
+            if (d2 < best) { best = d2; ob = o; }
+        }
+    }
+    template <int WFIX>
+    __device__ __forceinline__ static int nearest_ext(const DevParams& P, const float4* s_path, int centre,
+                                                      float px, float py, float pz)
+    {
+        const int W = WFIX > 0 ? WFIX : P.window;
+        const float4* w = s_path + 2 * P.P + centre;
+        const float inf = __int_as_float(0x7f800000);
+        float best = inf;
+        int ob = W;
+        if (WFIX > 0) {
+            constexpr int n = 2 * WFIX + 1, g = (n + 3) / 4;
+            float b1 = inf, b2 = inf, b3 = inf;
+            int o1 = g, o2 = 2 * g, o3 = 3 * g;
+            scan_run<0, g>(w, px, py, pz, best, ob);
+            scan_run<g, 2 * g>(w, px, py, pz, b1, o1);
+            scan_run<2 * g, 3 * g>(w, px, py, pz, b2, o2);
+            scan_run<3 * g, n>(w, px, py, pz, b3, o3);
+            if (b1 < best) { best = b1; ob = o1; }
+            if (b2 < best) { best = b2; ob = o2; }
+            if (b3 < best) { best = b3; ob = o3; }
+        } else {
+            for (int o = 0; o <= 2 * W; ++o) {
+                const float4 q = w[o];
+                const float dx = px - q.x, dy = py - q.y, dz = pz - q.z;
+                const float d2 = dx * dx + dy * dy + dz * dz;
+                if (d2 < best) { best = d2; ob = o; }
+            }
+        }
+        int i = centre + ob - W;
+        if (P.closed) { if (i < 0) i += P.P; else if (i >= P.P) i -= P.P; }
+        return i;
+    }
+    __device__ __forceinline__ static int nearest_smem(const DevParams& P, const float4* s_path, int centre,
+                                                       float px, float py, float pz)
+    {
+        return P.window == 16 ? nearest_ext<16>(P, s_path, centre, px, py, pz) : nearest_ext<0>(P, s_path, centre, px, py, pz);
+    }
     // lag error e_l, contour error squared e_c^2, progress theta = s_i + e_l
     __device__ __forceinline__ static void project(const DevParams& P, const float4* s_path, int i, float px, float py,
                                                    float pz, float& e_l, float& e_c2, float& theta)
@@ -236,7 +292,7 @@ struct ContourCost {
     }
     __device__ __forceinline__ float step(const DevParams& P, const float4* s_path, const State& x)
     {
-        idx = nearest(P, s_path, idx, x.px, x.py, x.pz);
+        idx = nearest_smem(P, s_path, idx, x.px, x.py, x.pz);
         float e_l, e_c2, theta;
         project(P, s_path, idx, x.px, x.py, x.pz, e_l, e_c2, theta);
         float d = theta - theta_prev;

@@ -55,7 +55,9 @@ __host__ __device__ inline int track_f4(const DevParams& P, int objective)
 {
     return objective == OBJ_GATE ? 4 * P.G
          : objective == OBJ_GATE_PAPER ? 4 * P.G + (P.N + 4) / 4      // gates + N+1 previous-iteration flags
-         : objective == OBJ_TRACK ? 4 * (P.N + 1) : 2 * P.P;          // both contouring forms stage the path
+         : objective == OBJ_TRACK ? 4 * (P.N + 1)
+         : objective == OBJ_CONTOUR ? 3 * P.P + 2 * P.window            // path + padded copy of the points (nearest_ext)
+         : 2 * P.P;                                                    // the paper's contouring: the path
 }
 
 // Stage the nominal sequence of controller b and the objective's track data in shared memory.
@@ -77,6 +79,14 @@ __device__ __forceinline__ void stage_inputs(const DevParams& P, const StepArgs&
         for (int i = tid; i < 4 * (N + 1); i += blockDim.x) s_trk[i] = P.ref[4 * t0 + i];
     } else {
         for (int i = tid; i < 2 * P.P; i += blockDim.x) s_trk[i] = P.path[i];
+        if (OBJ == OBJ_CONTOUR) {      // padded copy of the points for the windowed search (ContourCost::nearest_ext)
+            float4* ext = s_trk + 2 * P.P;
+            for (int j = tid; j < P.P + 2 * P.window; j += blockDim.x) {
+                int i = j - P.window;
+                if (P.closed) i = i < 0 ? i + P.P : (i >= P.P ? i - P.P : i);
+                ext[j] = (i >= 0 && i < P.P) ? P.path[i] : make_float4(1e30f, 1e30f, 1e30f, 0.0f);
+            }
+        }
     }
 }
 
@@ -88,7 +98,7 @@ __device__ __forceinline__ int contour_start_index(const DevParams& P, const flo
 {
     if (start >= 0) {
         const int centre = P.closed ? wrap_index(start, P.P) : min(max(start, 0), P.P - 1);
-        return ContourCost::nearest(P, s_path, centre, x.px, x.py, x.pz);
+        return ContourCost::nearest_smem(P, s_path, centre, x.px, x.py, x.pz);
     }
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     float best = __int_as_float(0x7f800000);
