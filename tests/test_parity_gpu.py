@@ -286,6 +286,21 @@ def test_contour_hint_and_open_path():
     run_case(wl, "contour open near start")
 
 
+@pytest.mark.parametrize("pipe", [dict(pipeline=0, variant=2), dict(pipeline=0, variant=3), dict(pipeline=0, variant=1),
+                                  dict(pipeline=1)], ids=["fused_lat", "fused_pk", "fused_thr", "two_pass"])
+@pytest.mark.parametrize("window,closed,near_end", [(5, True, True), (40, True, False), (7, False, True), (16, False, True)])
+def test_contour_window_sizes(window, closed, near_end, pipe):
+    # the search runs on the padded copy of the points: windows other than the unrolled default (16),
+    # wrap-around of a closed path and the clipped window at both ends of an open one
+    wl = W.cfg3(K=1024, N=30)
+    wl.params["window"] = window
+    wl.closed = closed
+    if near_end:                      # start next to the seam / the end: the window reaches past index P - 1
+        wl.x0[0, 0:3] = wl.path[-2] + np.float32([0.03, -0.02, 0.01])
+        wl.start[:] = wl.path.shape[0] - 3
+    run_case(wl, f"contour W{window} closed{closed} [{pipe}]", fast_math=1, **pipe)
+
+
 def test_determinism_and_host_entry_point():
     import torch
     wl = W.stress_gate(K=1024, N=30)
