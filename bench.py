@@ -409,7 +409,7 @@ def run_survey(args):
             if B > 1:
                 wl = W.replicate(wl, B, 0.3)
             P = wl.params
-            m = Bd.Mppi(P, fast_math=args.fast_math, variant=args.variant)
+            m = Bd.Mppi(P, fast_math=args.fast_math, variant=args.variant, pipeline=args.pipeline)
             m.set_track(wl)
             x0 = torch.from_numpy(wl.x0).to(dev); start = torch.from_numpy(wl.start).to(dev)
             u = torch.from_numpy(wl.u_nom).to(dev); un = torch.empty_like(u)
