@@ -225,6 +225,7 @@ struct ContourCost {
     // others.  Four runs of the window are scanned independently and merged in scan order -- a later
     // run wins only when strictly smaller -- which keeps [R-12]'s first minimiser with a four times
     // shorter dependency chain.  Distances are formed exactly as in nearest().
+    static constexpr int kExtPad = 7;     // extra entries before and after the padded copy (nearest_rot)
     template <int LO, int HI>
     __device__ __forceinline__ static void scan_run(const float4* w, float px, float py, float pz, float& best, int& ob)
     {
@@ -241,7 +242,7 @@ struct ContourCost {
                                                       float px, float py, float pz)
     {
         const int W = WFIX > 0 ? WFIX : P.window;
-        const float4* w = s_path + 2 * P.P + centre;
+        const float4* w = s_path + 2 * P.P + kExtPad + centre;
         const float inf = __int_as_float(0x7f800000);
         float best = inf;
         int ob = W;
@@ -268,6 +269,35 @@ struct ContourCost {
         if (P.closed) { if (i < 0) i += P.P; else if (i >= P.P) i -= P.P; }
         return i;
     }
+    // Bank-conflict-free form for the throughput kernels (window 16): a 128-bit shared load is served per
+    // quarter-warp, 8 lanes x 16 B over the 32 banks, and is conflict-free when the 8 vertex indices are
+    // distinct mod 8.  Each lane therefore starts its scan at the last entry at or before its window whose
+    // index is congruent to its lane number mod 8 (r <= 7 entries early) and walks 40 entries instead of
+    // 33; entry o belongs to the window iff r <= o <= r + 32, which only the first and the last seven
+    // need to test.  Scan order, strict comparison and distances are those of nearest(): same minimiser.
+    __device__ __forceinline__ static int nearest_rot(const DevParams& P, const float4* s_path, int centre,
+                                                      float px, float py, float pz)
+    {
+        constexpr int W = 16, n = 2 * W + 1;
+        const int ws = centre + kExtPad;                         // window start in the padded copy
+        const int r = (ws - (int)(threadIdx.x & 7)) & 7;
+        const float4* w = s_path + 2 * P.P + (ws - r);
+        const float inf = __int_as_float(0x7f800000);
+        float best = inf;
+        int ob = W + r;
+#pragma unroll
+        for (int o = 0; o < n + kExtPad; ++o) {
+            const float4 q = w[o];
+            const float dx = px - q.x, dy = py - q.y, dz = pz - q.z;
+            float d2 = dx * dx + dy * dy + dz * dz;
+            if (o < kExtPad) d2 = o >= r ? d2 : inf;
+            if (o >= n) d2 = o <= r + 2 * W ? d2 : inf;
+            if (d2 < best) { best = d2; ob = o; }
+        }
+        int i = centre + (ob - r) - W;
+        if (P.closed) { if (i < 0) i += P.P; else if (i >= P.P) i -= P.P; }
+        return i;
+    }
     __device__ __forceinline__ static int nearest_smem(const DevParams& P, const float4* s_path, int centre,
                                                        float px, float py, float pz)
     {
@@ -290,9 +320,11 @@ struct ContourCost {
         idx = i0;
         project(P, s_path, i0, x.px, x.py, x.pz, e_l, e_c2, theta_prev);
     }
+    template <bool ROT = false>
     __device__ __forceinline__ float step(const DevParams& P, const float4* s_path, const State& x)
     {
-        idx = nearest_smem(P, s_path, idx, x.px, x.py, x.pz);
+        idx = (ROT && P.window == 16) ? nearest_rot(P, s_path, idx, x.px, x.py, x.pz)
+                                      : nearest_smem(P, s_path, idx, x.px, x.py, x.pz);
         float e_l, e_c2, theta;
         project(P, s_path, idx, x.px, x.py, x.pz, e_l, e_c2, theta);
         float d = theta - theta_prev;

@@ -77,8 +77,8 @@ __device__ __forceinline__ void rollout_cost2(const DevParams& P, const StepArgs
             pb.step(P, s_trk, s_front, lane_state<1>(x), t);
         }
         if (OBJ == OBJ_CONTOUR) {
-            Ja += ca.step(P, s_trk, lane_state<0>(x));
-            Jb += cb.step(P, s_trk, lane_state<1>(x));
+            Ja += ca.template step<true>(P, s_trk, lane_state<0>(x));     // conflict-free scan (nearest_rot)
+            Jb += cb.template step<true>(P, s_trk, lane_state<1>(x));
         }
     }
     if (OBJ == OBJ_GATE) {

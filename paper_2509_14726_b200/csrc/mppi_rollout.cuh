@@ -56,7 +56,7 @@ __host__ __device__ inline int track_f4(const DevParams& P, int objective)
     return objective == OBJ_GATE ? 4 * P.G
          : objective == OBJ_GATE_PAPER ? 4 * P.G + (P.N + 4) / 4      // gates + N+1 previous-iteration flags
          : objective == OBJ_TRACK ? 4 * (P.N + 1)
-         : objective == OBJ_CONTOUR ? 3 * P.P + 2 * P.window            // path + padded copy of the points (nearest_ext)
+         : objective == OBJ_CONTOUR ? 3 * P.P + 2 * P.window + 14       // path + padded copy of the points (nearest_ext; 2 kExtPad)
          : 2 * P.P;                                                    // the paper's contouring: the path
 }
 
@@ -81,8 +81,8 @@ __device__ __forceinline__ void stage_inputs(const DevParams& P, const StepArgs&
         for (int i = tid; i < 2 * P.P; i += blockDim.x) s_trk[i] = P.path[i];
         if (OBJ == OBJ_CONTOUR) {      // padded copy of the points for the windowed search (ContourCost::nearest_ext)
             float4* ext = s_trk + 2 * P.P;
-            for (int j = tid; j < P.P + 2 * P.window; j += blockDim.x) {
-                int i = j - P.window;
+            for (int j = tid; j < P.P + 2 * P.window + 14; j += blockDim.x) {
+                int i = j - P.window - 7;                        // ContourCost::kExtPad entries in front and behind
                 if (P.closed) i = i < 0 ? i + P.P : (i >= P.P ? i - P.P : i);
                 ext[j] = (i >= 0 && i < P.P) ? P.path[i] : make_float4(1e30f, 1e30f, 1e30f, 0.0f);
             }
