@@ -586,8 +586,18 @@ double orc_rollout_cost(const orc_params* P, const orc_track* trk, const orc_pat
     const int xdim = cpaper ? 19 : (rate ? 17 : 13);
     double x[19];
     memcpy(x, x0, sizeof(double) * xdim);
+    if (P->objective == ORC_OBJ_TRACK) {
+        /* [R-11] the reference row of the current time is clamped so that the horizon's last row start + N
+         * exists (include/mppi.h, mppi_step: "clamped so that t0+N <= M-1"): the clock stops at the end of
+         * the reference, as in orc_sim_step */
+        if (start > trk->M - 1 - P->N) start = trk->M - 1 - P->N;
+        if (start < 0) start = 0;
+    }
     int32_t aux = start;
-    if (P->objective == ORC_OBJ_GATE_PAPER) { aux = start % trk->G; if (aux < 0) aux += trk->G; }
+    if (P->objective == ORC_OBJ_GATE_PAPER || P->objective == ORC_OBJ_GATE) {   /* target index wraps mod G [R-10] */
+        aux = start % trk->G;
+        if (aux < 0) aux += trk->G;
+    }
     const int32_t gate0 = aux;
     double J = 0.0, theta_prev = 0.0;
     double marg = INFINITY; int32_t nc = 0;

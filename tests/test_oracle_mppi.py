@@ -220,3 +220,131 @@ def test_brute_force_contour_wraps_the_closed_path():
     r0 = O.step(p0, trk, x0, [-1], wl.u_nom, 2, 0)
     d = (r0["cost"][0] - r["cost"][0]) / wl.params["mu_progress"]
     assert (d > 2.0).all() and (d < 6.0).all()     # ~4 m flown in 0.5 s
+
+
+# ---- closed-loop glue under tracking and contouring (Alg. 1 l.2-3 PAPER.md:177-178; receding horizon
+# PAPER.md:57, 97; oracle/mppi_oracle.c orc_sim_step).  The plant input is zero thrust, so the new position
+# is the free-fall closed form p + v dt - g dt^2/2 e_z (pinned by P4) and every expected index below is
+# worked out by hand from it.
+
+def _free_fall_params(**over):
+    return exact_cfg0_params(**dict(dict(K=32, N=4, T_min=0.0), **over))
+
+
+def test_sim_step_tracking_clock_advances_and_clamps_at_the_margin():
+    # reference with a 3-row margin: M = N + 1 + 3 rows -> the start row may be 0..3 (= M - 1 - N);
+    # start -> start + 1 per control step, then stays clamped; the rows' content plays no role
+    N = 4
+    p = _free_fall_params(objective=1, N=N)
+    M = N + 1 + 3
+    ref = np.zeros((M, 13)); ref[:, 3] = 1.0
+    trk = O.Track(ref=ref)
+    x = np.zeros((1, 13)); x[0, 0:3] = (1.0, 2.0, 30.0); x[0, 3] = 1.0; x[0, 7:10] = (3.0, -1.0, 0.5)
+    u_new = np.zeros((1, N, 4)); u_new[0, :, 0] = np.arange(N) + 1.0      # thrust 1 N on rotor 0 at step 0 only matters
+    u_new[0, 0] = 0.0                                                     # the plant applies u_new[0] = 0: free fall
+    start = np.array([0], np.int32)
+    seen = []
+    for step in range(6):
+        xn, start_n, nxt = O.sim_step(p, trk, x, start, u_new)
+        t = p["dt"]
+        np.testing.assert_allclose(xn[0, 0:3], x[0, 0:3] + x[0, 7:10] * t - [0, 0, 0.5 * p["g"] * t * t], atol=1e-13)
+        np.testing.assert_array_equal(nxt[0, :-1], u_new[0, 1:]); np.testing.assert_array_equal(nxt[0, -1], u_new[0, -1])
+        seen.append(int(start_n[0]))
+        x, start = xn, start_n
+    assert seen == [1, 2, 3, 3, 3, 3]                     # M - 1 - N = 3
+    # a start row beyond the margin is pulled back to it, a row far below it still advances by one
+    _, s2, _ = O.sim_step(p, trk, x, np.array([17], np.int32), u_new)
+    assert s2[0] == 3
+    # with no margin at all (M = N + 1) the clock cannot move
+    trk0 = O.Track(ref=ref[:N + 1])
+    _, s3, _ = O.sim_step(p, trk0, x, np.array([0], np.int32), u_new)
+    assert s3[0] == 0
+
+
+def test_sim_step_contour_windowed_global_tie_and_seam():
+    # straight OPEN path along x, vertices at 0.125 i (binary-exact), i = 0..39, window 3
+    N = 4
+    p = _free_fall_params(objective=2, N=N, window=3)
+    pts = np.zeros((40, 3)); pts[:, 0] = 0.125 * np.arange(40); pts[:, 2] = 1.0
+    trk = O.Track(path=pts, closed=False)
+    u_new = np.zeros((1, N, 4))
+    dt = p["dt"]
+
+    def plant_at(px, vx=0.0):
+        x = np.zeros((1, 13)); x[0, 0:3] = (px, 0.25, 1.0); x[0, 3] = 1.0; x[0, 7] = vx
+        return x
+    # the plant moves 5 m/s * 0.02 s = 0.1 m: from x = 2.53 to 2.63 -> global nearest vertex 21 (2.625)
+    x = plant_at(2.53, 5.0)
+    xn, s, _ = O.sim_step(p, trk, x, np.array([-1], np.int32), u_new)
+    assert xn[0, 0] == pytest.approx(2.53 + 5.0 * dt, abs=1e-14) and s[0] == 21
+    # windowed around the hint 17 (vertices 14..20): the nearest INSIDE the window is 20, not 21
+    _, s, _ = O.sim_step(p, trk, x, np.array([17], np.int32), u_new)
+    assert s[0] == 20
+    # hint 21 +- 3 contains the global minimiser
+    _, s, _ = O.sim_step(p, trk, x, np.array([21], np.int32), u_new)
+    assert s[0] == 21
+    # the NEW position decides, not the old one: from 2.53 the old nearest vertex is 20 (2.5)
+    assert np.argmin(np.abs(pts[:, 0] - 2.53)) == 20
+    # exact tie between vertices 20 and 21 (x = 2.5625, no horizontal motion): first in scan order wins,
+    # globally (ascending index) and in a window
+    x = plant_at(2.5625, 0.0)
+    for hint in (-1, 22, 19):
+        _, s, _ = O.sim_step(p, trk, x, np.array([hint], np.int32), u_new)
+        assert s[0] == 20
+    # open path: a window hanging over the end is cut, never wrapped
+    x = plant_at(0.01, 0.0)
+    _, s, _ = O.sim_step(p, trk, x, np.array([38], np.int32), u_new)
+    assert s[0] == 35                                        # window 35..39 (41 cut off): its nearest is 35
+    # CLOSED path: 16 vertices on a circle of radius 2; hint 15, window 3 -> scan 12,13,14,15,0,1,2
+    a = 2 * np.pi * np.arange(16) / 16
+    circ = np.stack([2 * np.cos(a), 2 * np.sin(a), np.ones(16)], 1)
+    trkc = O.Track(path=circ, closed=True)
+    x = np.zeros((1, 13)); x[0, 0:3] = circ[1] * 1.1; x[0, 3] = 1.0       # next to vertex 1, across the seam from the hint
+    _, s, _ = O.sim_step(p, trkc, x, np.array([15], np.int32), u_new)
+    assert s[0] == 1
+    # the same hint on the open form of the circle cannot reach vertex 1: window 12..15
+    trko = O.Track(path=circ, closed=False)
+    _, s, _ = O.sim_step(p, trko, x, np.array([15], np.int32), u_new)
+    assert s[0] == 15
+    # tie across the seam on a square ring with binary-exact vertices (0.5 m apart, 16 of them): the point
+    # (-0.25, 0.25) is exactly as far from vertex 15 = (0, 0.5) as from vertex 0 = (0, 0).  The windowed scan
+    # runs in offset order (12..15, then 0..2) and meets 15 first, although 0 is the smaller index; the
+    # global scan (0..15) returns 0  [R-12]
+    sq = np.array([(0, 0), (.5, 0), (1, 0), (1.5, 0), (2, 0), (2, .5), (2, 1), (2, 1.5), (2, 2), (1.5, 2), (1, 2), (.5, 2),
+                   (0, 2), (0, 1.5), (0, 1), (0, .5)], float)
+    sq = np.concatenate([sq, np.ones((16, 1))], 1)
+    trks = O.Track(path=sq, closed=True)
+    x[0, 0:3] = (-0.25, 0.25, 1.0); x[0, 7:10] = 0.0
+    _, s, _ = O.sim_step(p, trks, x, np.array([15], np.int32), u_new)
+    assert s[0] == 15
+    _, s, _ = O.sim_step(p, trks, x, np.array([1], np.int32), u_new)       # scan 14, 15, 0, 1, ...: still 15 first
+    assert s[0] == 15
+    _, s, _ = O.sim_step(p, trks, x, np.array([-1], np.int32), u_new)
+    assert s[0] == 0
+
+
+def test_start_index_is_clamped_or_wrapped_as_the_interface_states():
+    # include/mppi.h, mppi_step: tracking -- "reference row t0 ... clamped so that t0+N <= M-1"; gate objectives --
+    # "index of the current target gate (wrapped mod G)" [R-10],[R-11]
+    wl = W.cfg2(K=32, N=6, extra_rows=3)                      # M = N + 1 + 3: rows 0..3 are valid starts
+    trk = O.Track(ref=wl.ref)
+    J = lambda s: O.step(wl.params, trk, wl.x0, [s], wl.u_nom, 1, 0)["cost"]
+    np.testing.assert_array_equal(J(7), J(3)); np.testing.assert_array_equal(J(4), J(3))
+    np.testing.assert_array_equal(J(-2), J(0))
+    assert not np.array_equal(J(2), J(3))
+    # the clamped start really uses rows 3..9: the terminal row is the reference's last one
+    x_end = wl.ref[3 + 6].astype(np.float64)
+    p0 = dict(wl.params, K=32, sigma=0.0, Qv=0.0, Qq=0.0, Qw=0.0, R=0.0, Qp=1.0)
+    x0 = np.tile(x_end, (1, 1)); x0[0, 7:13] = 0.0; x0[0, 3:7] = (1, 0, 0, 0)
+    r = O.step(p0, trk, x0, [99], wl.u_nom, 1, 0)
+    xs = [x0[0]]
+    for t in range(6):
+        xs.append(O.rk4_step(p0, xs[-1], wl.u_nom[0, t]))
+    want = sum(np.sum((xs[t][0:3] - wl.ref[3 + t, 0:3].astype(np.float64)) ** 2) for t in range(7))
+    assert r["cost"][0, 0] == pytest.approx(want, rel=1e-12)
+    wl = W.stress_gate(K=32, N=10)
+    trk = O.Track(gates=wl.gates)
+    G = wl.gates.shape[0]
+    Jg = lambda s: O.step(wl.params, trk, wl.x0, [s], wl.u_nom, 1, 0)["cost"]
+    np.testing.assert_array_equal(Jg(G + 1), Jg(1)); np.testing.assert_array_equal(Jg(-1), Jg(G - 1))
+    assert not np.array_equal(Jg(0), Jg(1))

@@ -124,19 +124,24 @@ def test_asymmetric_inertia(name, pipe):
 
 
 def test_cfg4_closed_loop_teacher_forced():
-    # [R-17] 64 drones, closed loop on the GPU (plant + shift kernel); at checked control steps the
-    # oracle gets the GPU loop's actual (x, start, u_nom, iter) and is compared for that one step
+    # [R-17] configs[4] as stated: 64 drones, 500 control steps, closed loop on the GPU (plant + shift kernel) --
+    # the loop bench.py times.  At control step 0, every 50th and the last one the oracle gets the GPU loop's
+    # actual (x, start, u_nom, iter) and is compared for that one step (iteration AND plant step).
+    # With configs[4]'s sigma = 1.5 N, lambda = 0.5 the drones pass one gate and then lose height (DESIGN.md
+    # section 10, "Finding"): the late checks compare rollouts from states far below the track.
     import torch
     from oracle import oracle as O
-    wl = W.cfg4(steps=120)
+    wl = W.cfg4()
+    assert wl.iters == 500
     m = Pz.make_ctx(wl)
     x, start, u = Pz.to_dev(wl)
     trk = Pz.oracle_track(wl)
-    checked = 0
+    checked, passes = 0, np.zeros(wl.params["B"], np.int64)
     for step in range(wl.iters):
-        check = step in (0, 1, 2) or step % 40 == 0 or step == wl.iters - 1
+        check = step % 50 == 0 or step == wl.iters - 1
         if check:
             x_in, s_in, u_in = x.cpu().numpy(), start.cpu().numpy(), u.cpu().numpy()
+        s_before = start.clone()
         u_new, cost, w = m.step(x, start, u, wl.seed, step)
         if check:
             torch.cuda.synchronize()
@@ -145,6 +150,7 @@ def test_cfg4_closed_loop_teacher_forced():
             Pz.compare(f"cfg4 step{step}", g, o, wl.params["lambda"], True)
             xo, so, uo = O.sim_step(wl.params, trk, x_in, s_in, g["u_new"])
         m.sim_step(x, start, u_new, u_nom_next=u)
+        passes += (start != s_before).cpu().numpy()
         if check:
             torch.cuda.synchronize()
             np.testing.assert_allclose(x.cpu().numpy(), xo, rtol=3e-6, atol=2e-5)
@@ -152,8 +158,80 @@ def test_cfg4_closed_loop_teacher_forced():
             # the plant's gate decision may differ only if the plant sat within the margin
             assert (start.cpu().numpy() == so).mean() >= 0.98
             checked += 1
-    assert checked >= 6
-    assert int(start.max()) >= 1            # the loop really flies through gates
+    assert checked == 11
+    assert passes.max() >= 1            # the loop really flies through gates
+    Pz.STATS.append(f"cfg4 closed loop, 500 control steps: gate passes per drone min {passes.min()} / median "
+                    f"{int(np.median(passes))} / max {passes.max()}; final height min {float(x[:, 2].min()):.1f} m")
+    m.close()
+
+
+def _sim_step_case(kind, rate):
+    """B drones whose start indices / positions exercise every branch of mppi_sim_step under tracking and
+    search-contouring (include/mppi.h: mppi_sim_step; Alg. 1 l.2-3 PAPER.md:177-178)."""
+    K, N = 256, 20
+    if kind == "track":
+        base = W.cfg2(K=K, N=N, extra_rows=3)                 # M = N + 1 + 3: the start row clamps at 3
+        B = 4
+        wl = W.replicate(base, B, 0.2)
+        wl.start = np.array([0, 1, 3, 7], np.int32)           # advances, advances, stays clamped, pulled back
+    else:
+        base = W.cfg3(K=K, N=N)
+        pts = base.path.astype(np.float64)
+        P = len(pts)
+        spec = [(P - 3, P - 3, 8.0), (P - 3, -1, 8.0), (100, 100, 5.0), (100, 80, 5.0), (100, -1, 0.0), (250, 255, 3.0)]
+        B = len(spec)
+        wl = W.replicate(base, B, 0.0)
+        for b, (at, hint, speed) in enumerate(spec):          # next to vertex `at`, flying along the path
+            tan = pts[(at + 1) % P] - pts[(at - 1) % P]; tan /= np.linalg.norm(tan)
+            wl.x0[b, 0:3] = (pts[at] + np.array([0.05, -0.03, 0.04])).astype(np.float32)
+            wl.x0[b, 7:10] = (speed * tan).astype(np.float32)
+            wl.start[b] = hint
+    if rate:
+        wl = W._rate_model(wl, wl.name + "_rate")
+    return wl
+
+
+@pytest.mark.parametrize("rate", [0, 1], ids=["thrusts", "rate_model"])
+@pytest.mark.parametrize("kind", ["track", "contour"])
+def test_sim_step_tracking_and_contouring_match_the_oracle(kind, rate):
+    # the closed-loop glue under objectives 1 and 2, both input models: every control step of a short loop is
+    # compared with orc_sim_step from the GPU loop's own inputs [R-17] -- plant state, start index (tracking:
+    # +1 clamped at M - 1 - N; contouring: windowed / global nearest vertex incl. the seam), shifted nominal
+    import torch
+    from oracle import oracle as O
+    wl = _sim_step_case(kind, rate)
+    p = wl.params
+    m = Pz.make_ctx(wl)
+    x, start, u = Pz.to_dev(wl)
+    trk = Pz.oracle_track(wl)
+    pts = None if wl.path is None else wl.path.astype(np.float64)
+    seen = []
+    for step in range(6):
+        x_in, s_in, u_in = x.cpu().numpy(), start.cpu().numpy(), u.cpu().numpy()
+        g = Pz.gpu_step(m, x, start, u, wl.seed, step)
+        o = Pz.oracle_step(wl, x_in, s_in, u_in, wl.seed, step, want_du=True)
+        Pz.compare(f"sim {kind} rate{rate} step{step}", g, o, p["lambda"], False)
+        xo, so, uo = O.sim_step(p, trk, x_in, s_in, g["u_new"])
+        m.sim_step(x, start, torch.from_numpy(g["u_new"]).cuda(), u_nom_next=u); torch.cuda.synchronize()
+        np.testing.assert_allclose(x.cpu().numpy(), xo, rtol=3e-6, atol=2e-5)
+        np.testing.assert_array_equal(u.cpu().numpy(), uo.astype(np.float32))
+        sg = start.cpu().numpy()
+        if kind == "track":
+            np.testing.assert_array_equal(sg, so)
+        else:
+            for b in np.nonzero(sg != so)[0]:             # only an fp32-unresolvable tie may pick the other vertex
+                da, db = (np.sum((xo[b, 0:3] - pts[i]) ** 2) for i in (sg[b], so[b]))
+                assert abs(da - db) <= 1e-5 * max(da, db), (step, b, sg[b], so[b])
+        seen.append(sg.copy())
+    seen = np.array(seen)
+    if kind == "track":
+        np.testing.assert_array_equal(seen[:, 0], [1, 2, 3, 3, 3, 3])
+        np.testing.assert_array_equal(seen[-1], [3, 3, 3, 3])
+    else:
+        P = len(pts)
+        assert seen[-1, 0] < 50 and seen[-1, 1] < 50          # crossed the seam (started at P - 3)
+        assert seen[0, 3] <= 96                               # hint 80: the window 64..96 does not reach vertex ~100
+        assert abs(int(seen[0, 4]) - 100) <= 1                # global search finds it
     m.close()
 
 
@@ -422,7 +500,7 @@ def test_front_flags_and_closed_loop_feed():
         u_new, cost, w = m.step(x, start, u, 7, step)
         torch.cuda.synchronize()
         trk = O.Track(gates=wl.gates, prev_front=None if front is None else front.cpu().numpy())
-        o = O.step(p, trk, x_in, s_in, u_in, 7, step)
+        o = O.step(p, trk, x_in, s_in, u_in, 7, step, want_du=True)
         o["u_nom"] = u_in.astype(np.float64)
         gdict = dict(u_new=u_new.cpu().numpy(), cost=cost.cpu().numpy(), weights=w.cpu().numpy())
         Pz.compare(f"paper loop step{step}", gdict, o, p["lambda"], True)
@@ -568,7 +646,7 @@ def test_rate_model_closed_loop_with_flags():
         u_new, cost, w = m.step(x, start, u, 3, step)
         torch.cuda.synchronize()
         trk = O.Track(gates=wl.gates, prev_front=None if front is None else front.cpu().numpy())
-        o = O.step(p, trk, x_in, s_in, u_in, 3, step)
+        o = O.step(p, trk, x_in, s_in, u_in, 3, step, want_du=True)
         o["u_nom"] = u_in.astype(np.float64)
         g = dict(u_new=u_new.cpu().numpy(), cost=cost.cpu().numpy(), weights=w.cpu().numpy())
         Pz.compare(f"rate loop step{step}", g, o, p["lambda"], True)
@@ -713,16 +791,18 @@ def test_rate_model_auto_kernel_choice():
 def test_table1_sizes():
     # the sizes of the paper's own Table I (M = 8192, K = 20, dt = 0.03, lambda = 0.01) under the paper's J_gate
     # and the paper's contouring, thrust-rate model
-    # [R-38] the squared progress of eq.(6) is a difference of squared distances to the target: costs near 0
-    # carry the fp32 error of parts of size |p_0 - c|^2, which is therefore the floor of the relative bound
     wl = W.table1("gate")
     m = Pz.make_ctx(wl)
     x0, start, u = Pz.to_dev(wl)
     g = Pz.gpu_step(m, x0, start, u, wl.seed, 0)
     o = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, wl.seed, 0, want_du=True)
     o["u_nom"] = wl.u_nom.astype(np.float64)
+    # Measured (profiles/README_r02a.md): the squared progress alone is within 9.3e-6 (absolute) of the oracle on all
+    # 8192 samples; the sample that misses [R-20] (J = 1.14 = -6.38 progress + 3.95 body rates + 3.57 rate-limit
+    # cost, error 1.9e-4) owes its error to the soft body-rate limit (|omega| - omega_max)^2 of [R-31] next to the
+    # limit, which amplifies the fp32 error of omega.  Until the thrust differences are carried as states, the bound
+    # is taken against the parts the cost is the sum of.
     d2 = float(np.sum((wl.x0[0, 0:3].astype(np.float64) - wl.gates[int(wl.start[0]), 0:3]) ** 2))
-    assert d2 > 1.0
     Pz.compare("table1_gate", g, o, wl.params["lambda"], False, cost_floor=d2)
     m.close()
     wl = W.table1("contour")
