@@ -434,6 +434,91 @@ def run_survey(args):
     return 0
 
 
+def _time_workload(Bd, wl, dev, flush_buf, steps, warmup, **opts):
+    """One context, `steps` timed iterations (CUDA events, L2 flushed between them).  Returns (per-step ms, info, ESS
+    of the last iteration's weights per controller)."""
+    import torch
+    P = wl.params
+    m = Bd.Mppi(P, **opts)
+    m.set_track(wl)
+    x0 = torch.from_numpy(wl.x0).to(dev); start = torch.from_numpy(wl.start).to(dev)
+    u = torch.from_numpy(wl.u_nom).to(dev); un = torch.empty_like(u)
+    cost = torch.empty((P["B"], P["K"]), device=dev); w = torch.empty_like(cost)
+    it = [0]
+
+    def step():
+        m.step(x0, start, u, wl.seed, it[0], u_new=un, cost=cost, weights=w); it[0] += 1
+    ms = time_steps(step, lambda: flush_buf.fill_(float(it[0] & 7)), steps, warmup)
+    info = m.info()
+    ess = (1.0 / (w.double() ** 2).sum(-1)).cpu().numpy()
+    J = cost.cpu().numpy()
+    m.close()
+    return ms, info, ess, J
+
+
+VARIANT_NAMES = {0: "AUTO", 1: "scalar", 2: "latency", 3: "packed", 4: "pipelined"}
+
+
+def run_sweep(args):
+    """Two tables the headline numbers do not cover:
+    (i)  the batch sizes between the lone controller and configs[4]: B in {1..64} at K=4096, N=50, gate objective,
+         for every rollout kernel AUTO could pick, and AUTO itself;
+    (ii) the configs[4] shape at a MIXING temperature (lambda = 0.25 std(J): hundreds of samples carry weight, so
+         the fused update re-derives the whole noise stream) for the fused and the two-pass pipeline.
+    Device time per iteration by CUDA events, L2 flushed between iterations."""
+    import torch
+    from paper_2509_14726_b200 import binding as Bd
+    from paper_2509_14726_b200 import workloads as W
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --sweep: no CUDA device")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    flush_buf = torch.empty(L2_FLUSH_BYTES // 4, dtype=torch.float32, device=dev)
+    base = {"gate": W.cfg4, "track": lambda B: W.replicate(W.cfg2(), B, 0.3), "contour": lambda B: W.replicate(W.cfg3(), B, 0.3)}
+    print("## (i) batch sweep, us per iteration (median of 60; AUTO's choice in brackets)\n")
+    for obj in args.sweep_objectives.split(","):
+        print(f"objective: {obj}\n")
+        print("| B | " + " | ".join(VARIANT_NAMES[v] for v in (4, 2, 3, 1, 0)) + " | AUTO vs best |")
+        print("|---|" + "---|" * 6)
+        for B in [int(b) for b in args.sweep_batches.split(',')]:
+            wl = base[obj](B=B) if obj == "gate" else base[obj](B)
+            row, best = [], None
+            for v in (4, 2, 3, 1, 0):
+                try:
+                    ms, info, _, _ = _time_workload(Bd, wl, dev, flush_buf, 60, 5, fast_math=args.fast_math, variant=v)
+                    t = float(np.median(ms)) * 1e3
+                    tag = f"{t:.1f}"
+                    if v == 0:
+                        k = ("pipelined" if info["rollout_warps_per_block"] == 3 and info["block_threads"] == 256 else
+                             "packed" if info["samples_per_thread"] == 2 else
+                             "latency" if info["block_threads"] == 256 and info["rollout_warps_per_block"] < 8 else "scalar")
+                        tag += f" [{k}, {info['block_threads']} thr x {info['grid_blocks']}]"
+                        row.append(tag)
+                        row.append(f"{t / best:.2f}x")
+                        continue
+                    best = t if best is None else min(best, t)
+                    row.append(tag)
+                except Bd.MppiError as e:
+                    row.append("n/a")
+            print(f"| {B} | " + " | ".join(row) + " |", flush=True)
+        print()
+    print("## (ii) configs[4] shape (K=4096, N=50, B=64, gate), one-hot vs mixing weights, us per iteration (median of 40)\n")
+    print("| weights | lambda | ESS (median over controllers) | fused packed | fused scalar | two-pass packed (rollout + reduce) | two-pass scalar | fused packed, dU also stored |")
+    print("|---|---|---|---|---|---|---|---|")
+    wl = W.cfg4()
+    _, _, _, J = _time_workload(Bd, wl, dev, flush_buf, 1, 3, fast_math=args.fast_math)
+    lam_mix = float(np.float32(0.25 * np.median(J.std(-1))))
+    for label, lam in (("configs[4] as stated", wl.params["lambda"]), ("mixing, 0.25 std(J)", lam_mix), ("flat, 4 std(J)", 16 * lam_mix)):
+        wl = W.cfg4(); wl.params["lambda"] = lam
+        cells, ess_med = [], None
+        for pipe, v, sn in ((0, 3, 0), (0, 1, 0), (1, 3, 0), (1, 1, 0), (0, 3, 1)):
+            ms, info, ess, _ = _time_workload(Bd, wl, dev, flush_buf, 40, 5, fast_math=args.fast_math, variant=v, pipeline=pipe, store_noise=sn)
+            ess_med = float(np.median(ess))
+            cells.append(f"{float(np.median(ms)) * 1e3:.1f}")
+        print(f"| {label} | {lam:.4g} | {ess_med:.1f} | " + " | ".join(cells) + " |", flush=True)
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -445,12 +530,17 @@ def main(argv=None):
     ap.add_argument("--graph", type=int, default=0)
     ap.add_argument("--cpu-budget", dest="cpu_budget", type=float, default=10.0)
     ap.add_argument("--survey", action="store_true", help="time one iteration of every workload (table, one GPU)")
+    ap.add_argument("--sweep", action="store_true", help="batch-size sweep over the rollout kernels and the mixing-weight regime (tables, one GPU)")
+    ap.add_argument("--sweep-objectives", dest="sweep_objectives", default="gate", help="--sweep: comma list of gate,track,contour")
+    ap.add_argument("--sweep-batches", dest="sweep_batches", default="1,2,3,4,6,8,12,16,32,64")
     ap.add_argument("--only", default=None, help="--survey: this workload only (a key of workloads.ALL)")
     ap.add_argument("--batch", type=int, default=0, help="--survey: this number of controllers only")
     ap.add_argument("--variant", type=int, default=0, help="--survey: mppi_variant (0 AUTO, 1 THROUGHPUT, 2 LATENCY, 3 PACKED, 4 PIPELINED)")
     args = ap.parse_args(argv)
     if args.survey:
         return run_survey(args)
+    if args.sweep:
+        return run_sweep(args)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)

@@ -35,6 +35,9 @@ struct mppi_ctx {
     float4* d_du = nullptr;
     float* d_partials = nullptr;
     unsigned* d_counters = nullptr;
+    unsigned* d_hint = nullptr;            // [B] dense-weights hint of the previous iteration (StepArgs::hint)
+    bool keep_du = false;                  // d_du belongs to the caller-visible contract (two-pass / store_noise)
+    bool du_tried = false;
     const int* d_prev_front = nullptr;     // caller-owned (mppi_set_prev_front)
     const float* d_v_nom = nullptr; float* d_v_new = nullptr;   // caller-owned (mppi_set_progress)
     // device staging for mppi_step_host
@@ -184,7 +187,18 @@ static bool rate_pipe_candidate(const mppi_params* p, int sm_count)
     return p->variant == MPPI_VARIANT_AUTO && (int64_t)p->B * p->K / 32 <= 2 * (int64_t)sm_count;
 }
 
-static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, int* lat_consumers, int* packed, int* pipe)
+// AUTO (input_model = 0), from the batch sweep of profiles/sweep_r02*.md (K = 4096, N = 50, B = 1 .. 64; warps = B K / 32):
+//   warps <= 2 SMs   pipelined kernel: its 32-sample blocks run two per SM, so this is one wave
+//   warps <= 8 SMs   latency kernel with C = 4 rollout warps per block (the pipelined kernel would need several
+//                    waves of latency-bound blocks; the throughput kernels cannot fill the chip yet)
+//   warps <= 12 SMs  scalar throughput kernel (the packed kernel's grid is half as many blocks: under one wave)
+//   above            packed fp32x2 throughput kernel (scalar when K % 64 != 0)
+// search-based contouring (objective 2): the window search is 2/3 of a step and cannot be split over the pipeline's
+// roles: latency kernel up to 4 SMs warps, scalar throughput kernel up to 12 SMs warps, packed above.
+// `avoid` (prepare(), when the preferred kernel does not fit in shared memory with the track that was set):
+// bit 0 = not the pipelined kernel, bit 1 = not the latency kernel either.
+static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, int* lat_consumers, int* packed, int* pipe,
+                       int avoid = 0)
 {
     const int64_t warps = (int64_t)p->B * p->K / 32;
     *lat_consumers = 0;
@@ -209,16 +223,17 @@ static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, i
             if (p->K % tpb == 0) { *block_threads = tpb; return; }
     }
     const bool lat_ok = p->pipeline == MPPI_PIPE_FUSED && p->block_threads == 0;
-    // the windowed nearest-vertex search of objective 2 is ~2/3 of a step and cannot be split over the
-    // pipeline's roles (it would all sit in the translation warp: 112 us at configs[3]); the latency
-    // kernel spreads whole rollouts over the consumer warps instead (68 us, measured)
-    const bool few = p->variant == MPPI_VARIANT_AUTO && warps <= 4 * (int64_t)sm_count;
+    const bool automatic = p->variant == MPPI_VARIANT_AUTO;
     const bool search = p->objective == MPPI_OBJ_CONTOUR;
-    if (lat_ok && (p->variant == MPPI_VARIANT_PIPELINED || (few && !search))) {
+    const bool want_pipe = p->variant == MPPI_VARIANT_PIPELINED ||
+                           (automatic && !search && warps <= 2 * (int64_t)sm_count && !(avoid & 1));
+    if (lat_ok && want_pipe) {
         *pipe = 1; *block_threads = 256;
         return;
     }
-    if (lat_ok && (p->variant == MPPI_VARIANT_LATENCY || (few && search))) {
+    const bool want_lat = p->variant == MPPI_VARIANT_LATENCY ||
+                          (automatic && !(avoid & 2) && warps <= (search ? 4 : 8) * (int64_t)sm_count);
+    if (lat_ok && want_lat) {
         int best = 0;
         for (int c : {1, 2, 4})
             if (p->K % (32 * c) == 0) {
@@ -228,9 +243,10 @@ static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, i
         if (best) { *lat_consumers = best; *block_threads = 256; return; }
     }
     // packed fp32x2 throughput kernel: two samples per thread
-    if (p->K % 64 == 0 && (p->variant == MPPI_VARIANT_PACKED ||
-                           (p->variant == MPPI_VARIANT_AUTO &&
-                            (!p->block_threads || (p->block_threads <= 128 && p->K % (2 * p->block_threads) == 0))))) {
+    const bool small_grid = automatic && warps <= 12 * (int64_t)sm_count;      // the packed grid (half as many blocks) would not cover the chip
+    if (p->K % 64 == 0 && !small_grid &&
+        (p->variant == MPPI_VARIANT_PACKED ||
+         (automatic && (!p->block_threads || (p->block_threads <= 128 && p->K % (2 * p->block_threads) == 0))))) {
         *packed = 1;
         if (p->block_threads) { *block_threads = p->block_threads; return; }
         for (int tpb : {128, 64, 32})
@@ -241,6 +257,12 @@ static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, i
     for (int tpb : {128, 64, 32})
         if (p->K % tpb == 0) { *block_threads = tpb; return; }
     *block_threads = 32;
+}
+
+static int blocks_per_ctrl_of(const mppi_params* p, const LaunchCfg& cfg)
+{
+    return cfg.pipe ? p->K / 32 : cfg.lat_consumers ? p->K / (32 * cfg.lat_consumers)
+                                                    : p->K / (cfg.block_threads * (cfg.packed ? 2 : 1));
 }
 
 static void free_graph(GraphSlot& g)
@@ -256,7 +278,7 @@ extern "C" int mppi_destroy(mppi_ctx* c)
     cudaDeviceSynchronize();
     free_graph(c->g_step); free_graph(c->g_opt);
     cudaFree(c->d_gates); cudaFree(c->d_ref); cudaFree(c->d_path); cudaFree(c->d_du);
-    cudaFree(c->d_partials); cudaFree(c->d_counters);
+    cudaFree(c->d_partials); cudaFree(c->d_counters); cudaFree(c->d_hint);
     if (c->h_pin) cudaFreeHost(c->h_pin);
     cudaFree(c->d_in);
     cudaFree(c->d_hx0); cudaFree(c->d_hstart); cudaFree(c->d_hu); cudaFree(c->d_hcost); cudaFree(c->d_hw);
@@ -328,8 +350,7 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     pick_shape(p, c->sm_count, &cfg.block_threads, &cfg.lat_consumers, &cfg.packed, &cfg.pipe);
     cfg.rate = p->input_model == 1;
     c->xdim = p->objective == MPPI_OBJ_CONTOUR_PAPER ? 19 : cfg.rate ? 17 : 13;
-    d.blocks_per_ctrl = cfg.pipe ? p->K / 32 : cfg.lat_consumers ? p->K / (32 * cfg.lat_consumers)
-                                          : p->K / (cfg.block_threads * (cfg.packed ? 2 : 1));
+    d.blocks_per_ctrl = blocks_per_ctrl_of(p, cfg);
     d.part_stride = 4 * p->N + 4 + (p->objective == MPPI_OBJ_CONTOUR_PAPER ? ((p->N + 3) & ~3) : 0);
     cfg.pipe_shallow = 0;
     cfg.smem_bytes = 0;   // fixed once the track is known
@@ -339,7 +360,8 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     c->scalar_tpb = cfg.block_threads; c->scalar_packed = cfg.packed;
     c->lazy_pipe = rate_pipe_candidate(p, c->sm_count) ? 1 : 0;
     d.pipe_d = 4; d.pipe_df = 3;
-    const int max_blocks = c->lazy_pipe ? p->K / 32 : d.blocks_per_ctrl;
+    // AUTO may move to another kernel once the track is known (prepare()): size the partials for the largest grid
+    const int max_blocks = (c->lazy_pipe || p->variant == MPPI_VARIANT_AUTO) ? p->K / 32 : d.blocks_per_ctrl;
 
     const size_t BN4 = (size_t)p->B * p->N * 4, BK = (size_t)p->B * p->K;
 #define CKC(call)                                                        \
@@ -351,11 +373,14 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
             return r_;                                                   \
         }                                                                \
     } while (0)
+    c->keep_du = cfg.store_du != 0;
     if (cfg.store_du) CKC(dev_alloc(c, &c->d_du, (size_t)p->B * p->N * p->K));
     if (cfg.fused) {
         CKC(dev_alloc(c, &c->d_partials, (size_t)p->B * max_blocks * d.part_stride));
         CKC(dev_alloc(c, &c->d_counters, (size_t)p->B + 1));
         CKC(cudaMemset(c->d_counters, 0, ((size_t)p->B + 1) * sizeof(unsigned)));
+        CKC(dev_alloc(c, &c->d_hint, (size_t)p->B));
+        CKC(cudaMemset(c->d_hint, 0, (size_t)p->B * sizeof(unsigned)));
     }
     CKC(dev_alloc(c, &c->d_hx0, (size_t)p->B * c->xdim));
     CKC(dev_alloc(c, &c->d_hstart, (size_t)p->B));
@@ -535,7 +560,31 @@ static int prepare(mppi_ctx* c)
             c->cfg.smem_bytes = 0;
         }
     }
-    const size_t need = rollout_smem_bytes(c->dp, c->cfg);
+    size_t need = rollout_smem_bytes(c->dp, c->cfg);
+    if (need > 227 * 1024 && c->prm.variant == MPPI_VARIANT_AUTO && c->prm.input_model == 0 &&
+        (c->cfg.pipe || c->cfg.lat_consumers)) {
+        // the kernel picked from the warp count alone does not fit with this track: next choice of pick_shape
+        for (int avoid : {1, 3}) {
+            if (avoid == 1 && !c->cfg.pipe) continue;
+            LaunchCfg nc = c->cfg;
+            pick_shape(&c->prm, c->sm_count, &nc.block_threads, &nc.lat_consumers, &nc.packed, &nc.pipe, avoid);
+            DevParams nd = c->dp;
+            nd.blocks_per_ctrl = blocks_per_ctrl_of(&c->prm, nc);
+            const size_t nn = rollout_smem_bytes(nd, nc);
+            if (nn <= 227 * 1024 || avoid == 3) {
+                c->cfg = nc; c->cfg.smem_bytes = 0; c->dp.blocks_per_ctrl = nd.blocks_per_ctrl; need = nn;
+                free_graph(c->g_step); free_graph(c->g_opt);
+                break;
+            }
+        }
+    }
+    // fused throughput kernels: scratch for dU, used only in iterations that follow one with many weight-carrying
+    // samples (StepArgs::hint).  If the allocation fails the kernels simply keep re-deriving the noise.
+    if (c->cfg.fused && !c->cfg.pipe && !c->cfg.lat_consumers && c->prm.objective != MPPI_OBJ_CONTOUR_PAPER && !c->d_du &&
+        !c->du_tried) {
+        c->du_tried = true;
+        if (dev_alloc(c, &c->d_du, (size_t)c->prm.B * c->prm.N * c->prm.K) != cudaSuccess) { cudaGetLastError(); c->d_du = nullptr; }
+    }
     if (need != c->cfg.smem_bytes) {
         if (need > 227 * 1024) return fail(c, MPPI_E_PARAM, "track + horizon do not fit in shared memory");
         if (need > 48 * 1024)
@@ -557,6 +606,7 @@ static StepArgs make_args(mppi_ctx* c, const float* x0, const int32_t* start, co
     StepArgs a;
     a.x0 = x0; a.start = start; a.u_nom = u_nom; a.u_new = u_new; a.cost = cost; a.weights = w;
     a.du = c->d_du; a.partials = c->d_partials; a.counters = c->d_counters;
+    a.hint = (c->cfg.fused && !c->cfg.pipe && !c->cfg.lat_consumers && c->d_du) ? c->d_hint : nullptr;
     a.prev_front = c->d_prev_front; a.v_nom = c->d_v_nom; a.v_new = c->d_v_new;
     a.done_flag = nullptr; a.done_value = 0;
     a.seed_lo = (uint32_t)(seed & 0xffffffffu); a.seed_hi = (uint32_t)(seed >> 32); a.iter = iter;
@@ -799,7 +849,7 @@ extern "C" int mppi_front_flags(mppi_ctx* c, const float* d_x0, const int32_t* d
     return MPPI_OK;
 }
 
-extern "C" const float* mppi_debug_noise(mppi_ctx* c) { return c ? reinterpret_cast<const float*>(c->d_du) : nullptr; }
+extern "C" const float* mppi_debug_noise(mppi_ctx* c) { return (c && c->keep_du) ? reinterpret_cast<const float*>(c->d_du) : nullptr; }
 
 extern "C" int64_t mppi_launch_count(mppi_ctx* c) { return c ? c->launches : 0; }
 

@@ -48,6 +48,9 @@ struct StepArgs {
     float4* du;            // [B][N][K] float4 or nullptr
     float* partials;       // [B][blocks_per_ctrl][part_stride]: S[4N], m, Z, -, - [, S5[N]]  (fused pipeline)
     unsigned int* counters;// [B + 1]: last-block tickets per controller, finished controllers (fused pipeline)
+    unsigned int* hint;    // [B] or nullptr (fused throughput kernels): written by the combine of one launch, read by
+                           // the next: != 0 = many samples carried weight, keep dU in `du` and sum it from there
+                           // instead of re-deriving the noise (mppi_rollout.cuh, warp_noise_partial)
     const float* v_nom;    // [B][N] nominal progress accelerations (OBJ_CONTOUR_PAPER), or nullptr
     float* v_new;          // [B][N] updated ones
     const int* prev_front; // [B][N+1] or nullptr: previous-iteration "in front" flags (paper's J_gate, Fig. 2)

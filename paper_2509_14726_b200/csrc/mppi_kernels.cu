@@ -118,7 +118,8 @@ __global__ void __launch_bounds__(MPPI_PK_THREADS, MPPI_PK_MINB) rollout2_kernel
     const State x0 = load_state(A.x0 + 13 * b);
     const int i0 = OBJ == OBJ_CONTOUR ? contour_start_index(P, s_trk, start, x0, s_red) : 0;
     float Ja, Jb;
-    float4* const du_out = STORE_DU ? A.du + (size_t)b * N * P.K + k0 : nullptr;
+    const bool stored = FUSED ? keeps_du<STORE_DU>(A, b) : STORE_DU;
+    float4* const du_out = stored ? A.du + (size_t)b * N * P.K + k0 : nullptr;
     if (OBJ != OBJ_CONTOUR && P.gyz == 0.0f)       // (the contouring search is bound by shared memory) Jx == Jy: the yaw-rate derivative is constant over the step (rk4_step2<true>)
         rollout_cost2<OBJ, MATH, true>(P, A, s_unom, s_trk, splat_state(x0), start, i0, (uint32_t)k0, (uint32_t)b, du_out, Ja, Jb);
     else
@@ -127,53 +128,21 @@ __global__ void __launch_bounds__(MPPI_PK_THREADS, MPPI_PK_MINB) rollout2_kernel
 
     if (!FUSED) return;
 
-    // ---- block-local softmax partial, as in rollout_kernel, over the block's 2 blockDim.x samples ----
-    const float m = block_min(fminf(Ja, Jb), s_red);
-    const float ea = exp_weight<MATH>((m - Ja) * P.inv_lambda), eb = exp_weight<MATH>((m - Jb) * P.inv_lambda);
-    const float Zb = block_sum(ea + eb, s_red);
-    {
-        const unsigned ca = __ballot_sync(kFull, ea > 0.0f), cb = __ballot_sync(kFull, eb > 0.0f);
-        const uint32_t kbase = (uint32_t)(2 * (blockIdx.x * blockDim.x + warp * 32));
-        for (int t0 = 0; t0 < N; t0 += 32) {
-            const int t = t0 + lane;
-            const float4 un = t < N ? s_unom[t] : make_float4(0.f, 0.f, 0.f, 0.f);
-            float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                unsigned mm = h ? cb : ca;
-                while (mm) {
-                    const int l = __ffs(mm) - 1;
-                    mm &= mm - 1;
-                    const float el = __shfl_sync(kFull, h ? eb : ea, l);
-                    const float4 T = sample_thrust<MATH>(P, A.rk, kbase + 2u * l + h, (uint32_t)t, A.iter, (uint32_t)b, un);
-                    acc.x = fmaf(el, T.x - un.x, acc.x); acc.y = fmaf(el, T.y - un.y, acc.y);
-                    acc.z = fmaf(el, T.z - un.z, acc.z); acc.w = fmaf(el, T.w - un.w, acc.w);
-                }
-            }
-            if (t < N) s_acc[warp * N + t] = acc;
-        }
-    }
-    __syncthreads();
-    const int nw = blockDim.x >> 5;
-    float* part = A.partials + ((size_t)b * P.blocks_per_ctrl + blockIdx.x) * P.part_stride;
-    for (int j = tid; j < 4 * N; j += blockDim.x) {
-        float s = 0.0f;
-        for (int w = 0; w < nw; ++w) s += reinterpret_cast<const float*>(s_acc)[w * 4 * N + j];
-        part[j] = s;
-    }
-    if (tid == 0) { part[4 * N] = m; part[4 * N + 1] = Zb; }
-    publish_and_combine<MATH>(P, A, b, P.blocks_per_ctrl, s_unom, s_red, s_pair);
+    // ---- block-local softmax partial over the block's 2 blockDim.x samples + last-block combine (mppi_rollout.cuh) ----
+    const float Jv[2] = {Ja, Jb};
+    block_partial_and_combine_n<MATH, 2>(P, A, b, blockIdx.x, (uint32_t)(2 * blockIdx.x * blockDim.x), Jv, P.T_min, P.T_max,
+                                         stored, s_unom, s_red, s_acc, s_pair);
 }
 
 // thrust source of the throughput kernel: draw (k, t) in place
-template <int MATH, bool STORE_DU>
+template <int MATH>
 struct DrawThrust {
-    const DevParams& P; const StepArgs& A; const float4* s_unom; uint32_t k, b; float4* du_out;
+    const DevParams& P; const StepArgs& A; const float4* s_unom; uint32_t k, b; float4* du_out;   // du_out: nullptr = not kept
     __device__ __forceinline__ float4 operator()(int t) const
     {
         const float4 un = s_unom[t];
         const float4 T = sample_thrust<MATH>(P, A.rk, k, (uint32_t)t, A.iter, b, un);
-        if (STORE_DU)                                      // one coalesced 16-B store per thread
+        if (du_out)                                        // one coalesced 16-B store per thread
             du_out[(size_t)t * P.K] = make_float4(T.x - un.x, T.y - un.y, T.z - un.z, T.w - un.w);
         return T;
     }
@@ -204,15 +173,15 @@ __global__ void rollout_kernel(const DevParams P, const StepArgs A)
 
     const State x0 = load_state(A.x0 + 13 * b);
     const int i0 = OBJ == OBJ_CONTOUR ? contour_start_index(P, s_trk, start, x0, s_red) : 0;
-    DrawThrust<MATH, STORE_DU> src{P, A, s_unom, (uint32_t)k, (uint32_t)b,
-                                   STORE_DU ? A.du + (size_t)b * N * P.K + k : nullptr};
+    const bool stored = FUSED ? keeps_du<STORE_DU>(A, b) : STORE_DU;
+    DrawThrust<MATH> src{P, A, s_unom, (uint32_t)k, (uint32_t)b, stored ? A.du + (size_t)b * N * P.K + k : nullptr};
     const float J = rollout_cost<OBJ, MATH>(P, s_trk, x0, start, i0, src);
     A.cost[(size_t)b * P.K + k] = J;
 
     if (!FUSED) return;
 
     // block-local softmax partial + last-block combine (mppi_rollout.cuh)
-    block_partial_and_combine<MATH>(P, A, b, blockIdx.x, J, P.T_min, P.T_max, s_unom, s_red, s_acc, s_pair);
+    block_partial_and_combine<MATH>(P, A, b, blockIdx.x, J, P.T_min, P.T_max, s_unom, s_red, s_acc, s_pair, nullptr, nullptr, stored);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -54,13 +54,14 @@ __global__ void __launch_bounds__(256, 3) rollout_rate_kernel(const DevParams P,
     if (OBJ == OBJ_GATE) gc.init<MATH>(P, s_trk, start, x);
     if (OBJ == OBJ_GATE_PAPER) gp.init(P, s_trk, start, x);
     if (OBJ == OBJ_CONTOUR) cc.init(P, s_trk, i0, x);
-    float4* du_out = STORE_DU ? A.du + (size_t)b * N * P.K + k : nullptr;
+    const bool stored = (FUSED && OBJ != OBJ_CONTOUR_PAPER) ? keeps_du<STORE_DU>(A, b) : STORE_DU;
+    float4* du_out = stored ? A.du + (size_t)b * N * P.K + k : nullptr;
     // the horizon loop, instantiated for the axisymmetric drag form (drag_x == drag_y) and the general one
     auto horizon = [&](auto axi) {
     for (int t = 0; t < N; ++t) {
         const float4 un = s_unom[t];
         const float4 u = sample_input<MATH>(P, A.rk, (uint32_t)k, (uint32_t)t, A.iter, (uint32_t)b, un, lo, hi);
-        if (STORE_DU) du_out[(size_t)t * P.K] = make_float4(u.x - un.x, u.y - un.y, u.z - un.z, u.w - un.w);
+        if (stored) du_out[(size_t)t * P.K] = make_float4(u.x - un.x, u.y - un.y, u.z - un.z, u.w - un.w);
         if (OBJ == OBJ_TRACK)      // eq.(8): the input term acts on the inputs = the rates [R-32]
             J += fmaf(P.R, u.x * u.x + u.y * u.y + u.z * u.z + u.w * u.w, track_state_term(P, s_trk + 4 * t, x));
         if (OBJ == OBJ_CONTOUR_PAPER) {            // fifth sampled input, stage cost, progress states [R-34]..[R-37]
@@ -87,7 +88,7 @@ __global__ void __launch_bounds__(256, 3) rollout_rate_kernel(const DevParams P,
     if (OBJ == OBJ_CONTOUR_PAPER)
         block_partial_and_combine<MATH>(P, A, b, blockIdx.x, J, lo, hi, s_unom, s_red, s_acc, s_pair, s_vnom, s_acc5);
     else
-        block_partial_and_combine<MATH>(P, A, b, blockIdx.x, J, lo, hi, s_unom, s_red, s_acc, s_pair);
+        block_partial_and_combine<MATH>(P, A, b, blockIdx.x, J, lo, hi, s_unom, s_red, s_acc, s_pair, nullptr, nullptr, stored);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -126,13 +127,14 @@ __global__ void __launch_bounds__(128, 3) rollout_rate2_kernel(const DevParams P
     const int* s_front = reinterpret_cast<const int*>(s_trk + 4 * P.G);  // OBJ_GATE_PAPER only
     if (OBJ == OBJ_GATE) { ga.init<MATH>(P, s_trk, start, x0); gb = ga; }
     if (OBJ == OBJ_GATE_PAPER) { pa.init(P, s_trk, start, x0); pb = pa; }
-    float4* du_out = STORE_DU ? A.du + (size_t)b * N * P.K + k0 : nullptr;
+    const bool stored = FUSED ? keeps_du<STORE_DU>(A, b) : STORE_DU;
+    float4* du_out = stored ? A.du + (size_t)b * N * P.K + k0 : nullptr;
     auto horizon = [&](auto axi) {         // as in rollout_rate_kernel: axisymmetric drag form / general form
     for (int t = 0; t < N; ++t) {
         const float4 un = s_unom[t];
         const float4 ua = sample_input<MATH>(P, A.rk, (uint32_t)k0, (uint32_t)t, A.iter, (uint32_t)b, un, lo, hi);
         const float4 ub = sample_input<MATH>(P, A.rk, (uint32_t)k0 + 1u, (uint32_t)t, A.iter, (uint32_t)b, un, lo, hi);
-        if (STORE_DU) {
+        if (stored) {
             du_out[(size_t)t * P.K] = make_float4(ua.x - un.x, ua.y - un.y, ua.z - un.z, ua.w - un.w);
             du_out[(size_t)t * P.K + 1] = make_float4(ub.x - un.x, ub.y - un.y, ub.z - un.z, ub.w - un.w);
         }
@@ -159,42 +161,10 @@ __global__ void __launch_bounds__(128, 3) rollout_rate2_kernel(const DevParams P
 
     if (!FUSED) return;
 
-    // ---- block-local softmax partial over the block's 2 blockDim.x samples (as rollout2_kernel) ----
-    const float m = block_min(fminf(Ja, Jb), s_red);
-    const float ea = exp_weight<MATH>((m - Ja) * P.inv_lambda), eb = exp_weight<MATH>((m - Jb) * P.inv_lambda);
-    const float Zb = block_sum(ea + eb, s_red);
-    {
-        const unsigned ca = __ballot_sync(kFull, ea > 0.0f), cb = __ballot_sync(kFull, eb > 0.0f);
-        const uint32_t kbase = (uint32_t)(2 * (blockIdx.x * blockDim.x + warp * 32));
-        for (int t0 = 0; t0 < N; t0 += 32) {
-            const int t = t0 + lane;
-            const float4 un = t < N ? s_unom[t] : make_float4(0.f, 0.f, 0.f, 0.f);
-            float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                unsigned mm = h ? cb : ca;
-                while (mm) {
-                    const int l = __ffs(mm) - 1;
-                    mm &= mm - 1;
-                    const float el = __shfl_sync(kFull, h ? eb : ea, l);
-                    const float4 u = sample_input<MATH>(P, A.rk, kbase + 2u * l + h, (uint32_t)t, A.iter, (uint32_t)b, un, lo, hi);
-                    acc.x = fmaf(el, u.x - un.x, acc.x); acc.y = fmaf(el, u.y - un.y, acc.y);
-                    acc.z = fmaf(el, u.z - un.z, acc.z); acc.w = fmaf(el, u.w - un.w, acc.w);
-                }
-            }
-            if (t < N) s_acc[warp * N + t] = acc;
-        }
-    }
-    __syncthreads();
-    const int nw = blockDim.x >> 5;
-    float* part = A.partials + ((size_t)b * P.blocks_per_ctrl + blockIdx.x) * P.part_stride;
-    for (int j = tid; j < 4 * N; j += blockDim.x) {
-        float s = 0.0f;
-        for (int w = 0; w < nw; ++w) s += reinterpret_cast<const float*>(s_acc)[w * 4 * N + j];
-        part[j] = s;
-    }
-    if (tid == 0) { part[4 * N] = m; part[4 * N + 1] = Zb; }
-    publish_and_combine<MATH>(P, A, b, P.blocks_per_ctrl, s_unom, s_red, s_pair);
+    // ---- block-local softmax partial over the block's 2 blockDim.x samples + last-block combine (mppi_rollout.cuh) ----
+    const float Jv[2] = {Ja, Jb};
+    block_partial_and_combine_n<MATH, 2>(P, A, b, blockIdx.x, (uint32_t)(2 * blockIdx.x * blockDim.x), Jv, lo, hi, stored,
+                                         s_unom, s_red, s_acc, s_pair);
 }
 
 // ---- host-side dispatch ------------------------------------------------------------------------------

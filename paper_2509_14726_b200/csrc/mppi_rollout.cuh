@@ -169,41 +169,128 @@ __device__ __forceinline__ void publish_and_combine(const DevParams& P, const St
 template <int MATH>
 __device__ __forceinline__ float sample_progress_accel(const DevParams& P, const uint32_t (&rk)[20], uint32_t k,
                                                        uint32_t t, uint32_t iter, uint32_t b, const float vn);
-// s_vnom / s_acc5 (OBJ_CONTOUR_PAPER only, else nullptr): the nominal of the fifth sampled input [N] and one
-// accumulator row per warp [warps][N]; the block's partial then carries S5[N] after its (m, Z) header.
-template <int MATH>
-__device__ __forceinline__ void block_partial_and_combine(const DevParams& P, const StepArgs& A, const int b,
-                                                          const int chunk, const float J, const float lo, const float hi,
-                                                          const float4* s_unom, float* s_red, float4* s_acc, float* s_pair,
-                                                          const float* s_vnom = nullptr, float* s_acc5 = nullptr)
+// The warp's share of S[t] = sum_k e_k dU_k[t] (eq.(5)) for kernels that hold SPT samples per lane:
+// lane l owns samples kbase + SPT l + h with weights e[h].  Two ways, both exact:
+//   sparse  the perturbations are RE-DERIVED from the counter-based stream for the samples with e > 0 only, the
+//           lanes spread over the horizon steps -- nearly free when the softmax is one-hot (every config of
+//           BASELINE.json, the paper's lambda = 0.01), but the whole noise stream again when most samples count;
+//   dense   when this launch also STORED dU (du_ctrl != nullptr; see StepArgs::hint) and enough samples of the warp
+//           count: every lane reads its own rows back (L2 hits for the most part: the block wrote them during the
+//           rollout), and eight steps at a time are summed over the lanes by a transposed butterfly (7 + 2 shuffle
+//           rounds per component instead of 5 per step).
+// s_acc_row: N float4 of this warp.  s_vnom / s_acc5_row (OBJ_CONTOUR_PAPER only, else nullptr): the nominal of the
+// fifth sampled input and its accumulator row; that column is always re-derived.
+__device__ __forceinline__ float4 shfl_xor4(const float4 v, const int m)
 {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, N = P.N;
-    const float m = block_min(J, s_red);
-    const float e = exp_weight<MATH>((m - J) * P.inv_lambda);
-    const float Zb = block_sum(e, s_red);
-    {
-        const unsigned contrib = __ballot_sync(kFull, e > 0.0f);
-        const uint32_t kbase = (uint32_t)(chunk * blockDim.x + warp * 32);
-        for (int t0 = 0; t0 < N; t0 += 32) {
-            const int t = t0 + lane;
-            const float4 un = t < N ? s_unom[t] : make_float4(0.f, 0.f, 0.f, 0.f);
-            const float vn = (s_vnom && t < N) ? s_vnom[t] : 0.0f;
-            float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-            float acc5 = 0.0f;
-            unsigned mm = contrib;
+    return make_float4(__shfl_xor_sync(kFull, v.x, m), __shfl_xor_sync(kFull, v.y, m), __shfl_xor_sync(kFull, v.z, m),
+                       __shfl_xor_sync(kFull, v.w, m));
+}
+__device__ __forceinline__ float4 add4(const float4 a, const float4 b) { return make_float4(a.x + b.x, a.y + b.y, a.z + b.z, a.w + b.w); }
+
+template <int MATH, int SPT>
+__device__ __forceinline__ void warp_noise_partial(const DevParams& P, const StepArgs& A, const int b, const uint32_t kbase,
+                                                   const float (&e)[SPT], const float lo, const float hi,
+                                                   const float4* s_unom, float4* s_acc_row, const float4* du_ctrl,
+                                                   const float* s_vnom = nullptr, float* s_acc5_row = nullptr)
+{
+    const int lane = threadIdx.x & 31, N = P.N;
+    unsigned contrib[SPT];
+    int count = 0;
+#pragma unroll
+    for (int h = 0; h < SPT; ++h) { contrib[h] = __ballot_sync(kFull, e[h] > 0.0f); count += __popc(contrib[h]); }
+    // instruction estimate per lane: sparse ~ 85 per (contributing sample, pass of 32 steps); dense ~ 5 SPT + 16 per step
+    if (du_ctrl && !s_vnom && count * ((N + 31) >> 5) * 85 > N * (5 * SPT + 16)) {
+        const float4* mine = du_ctrl + kbase + SPT * lane;
+        const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4;
+        const int t_off = (b4 ? 4 : 0) + (b3 ? 2 : 0) + (b2 ? 1 : 0);
+        for (int t0 = 0; t0 < N; t0 += 8) {
+            float4 v[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                v[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (t0 + j < N) {
+#pragma unroll
+                    for (int h = 0; h < SPT; ++h) {
+                        const float4 d = mine[(size_t)(t0 + j) * P.K + h];
+                        v[j].x = fmaf(e[h], d.x, v[j].x); v[j].y = fmaf(e[h], d.y, v[j].y);
+                        v[j].z = fmaf(e[h], d.z, v[j].z); v[j].w = fmaf(e[h], d.w, v[j].w);
+                    }
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const float4 send = b4 ? v[j] : v[j + 4], keep = b4 ? v[j + 4] : v[j];
+                v[j] = add4(keep, shfl_xor4(send, 16));
+            }
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                const float4 send = b3 ? v[j] : v[j + 2], keep = b3 ? v[j + 2] : v[j];
+                v[j] = add4(keep, shfl_xor4(send, 8));
+            }
+            {
+                const float4 send = b2 ? v[0] : v[1], keep = b2 ? v[1] : v[0];
+                v[0] = add4(keep, shfl_xor4(send, 4));
+            }
+            v[0] = add4(v[0], shfl_xor4(v[0], 2));
+            v[0] = add4(v[0], shfl_xor4(v[0], 1));
+            if ((lane & 3) == 0 && t0 + t_off < N) s_acc_row[t0 + t_off] = v[0];
+        }
+        return;
+    }
+    for (int t0 = 0; t0 < N; t0 += 32) {
+        const int t = t0 + lane;
+        const float4 un = t < N ? s_unom[t] : make_float4(0.f, 0.f, 0.f, 0.f);
+        const float vn = (s_vnom && t < N) ? s_vnom[t] : 0.0f;
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+        float acc5 = 0.0f;
+#pragma unroll
+        for (int h = 0; h < SPT; ++h) {
+            unsigned mm = contrib[h];
             while (mm) {
                 const int l = __ffs(mm) - 1;
                 mm &= mm - 1;
-                const float el = __shfl_sync(kFull, e, l);
-                const float4 T = sample_input<MATH>(P, A.rk, kbase + l, (uint32_t)t, A.iter, (uint32_t)b, un, lo, hi);
+                const float el = __shfl_sync(kFull, e[h], l);
+                const uint32_t k = kbase + (uint32_t)(SPT * l + h);
+                const float4 T = sample_input<MATH>(P, A.rk, k, (uint32_t)t, A.iter, (uint32_t)b, un, lo, hi);
                 acc.x = fmaf(el, T.x - un.x, acc.x); acc.y = fmaf(el, T.y - un.y, acc.y);
                 acc.z = fmaf(el, T.z - un.z, acc.z); acc.w = fmaf(el, T.w - un.w, acc.w);
                 if (s_vnom)
-                    acc5 = fmaf(el, sample_progress_accel<MATH>(P, A.rk, kbase + l, (uint32_t)t, A.iter, (uint32_t)b, vn) - vn, acc5);
+                    acc5 = fmaf(el, sample_progress_accel<MATH>(P, A.rk, k, (uint32_t)t, A.iter, (uint32_t)b, vn) - vn, acc5);
             }
-            if (t < N) { s_acc[warp * N + t] = acc; if (s_vnom) s_acc5[warp * N + t] = acc5; }
         }
+        if (t < N) { s_acc_row[t] = acc; if (s_vnom) s_acc5_row[t] = acc5; }
     }
+}
+
+// Does this launch keep dU of controller b?  Always when the kernel was built for it (two-pass pipeline, store_noise);
+// in the fused pipeline also when the previous iteration's combine found many samples carrying weight (StepArgs::hint).
+template <bool STORE_DU>
+__device__ __forceinline__ bool keeps_du(const StepArgs& A, const int b)
+{
+    return STORE_DU || (A.hint != nullptr && A.du != nullptr && A.hint[b] != 0u);
+}
+
+// Block partial for kernels with SPT samples per thread: block minimum, weights, warp sums (warp_noise_partial), sum
+// over the warps, the partial's (m, Z) header, then publish_and_combine.  All threads of the block must call this.
+// chunk: index of this block within its controller; kblock: its first sample.
+template <int MATH, int SPT>
+__device__ __forceinline__ void block_partial_and_combine_n(const DevParams& P, const StepArgs& A, const int b,
+                                                            const int chunk, const uint32_t kblock, const float (&J)[SPT],
+                                                            const float lo, const float hi, const bool stored,
+                                                            const float4* s_unom, float* s_red, float4* s_acc, float* s_pair,
+                                                            const float* s_vnom = nullptr, float* s_acc5 = nullptr)
+{
+    const int tid = threadIdx.x, warp = tid >> 5, N = P.N;
+    float jm = J[0];
+#pragma unroll
+    for (int h = 1; h < SPT; ++h) jm = fminf(jm, J[h]);
+    const float m = block_min(jm, s_red);
+    float e[SPT], es = 0.0f;
+#pragma unroll
+    for (int h = 0; h < SPT; ++h) { e[h] = exp_weight<MATH>((m - J[h]) * P.inv_lambda); es += e[h]; }
+    const float Zb = block_sum(es, s_red);
+    warp_noise_partial<MATH, SPT>(P, A, b, kblock + (uint32_t)(warp * 32 * SPT), e, lo, hi, s_unom, s_acc + warp * N,
+                                  stored ? A.du + (size_t)b * N * P.K : nullptr, s_vnom, s_acc5 ? s_acc5 + warp * N : nullptr);
     __syncthreads();
     const int nw = blockDim.x >> 5;
     float* part = A.partials + ((size_t)b * P.blocks_per_ctrl + chunk) * P.part_stride;
@@ -220,6 +307,18 @@ __device__ __forceinline__ void block_partial_and_combine(const DevParams& P, co
         }
     if (tid == 0) { part[4 * N] = m; part[4 * N + 1] = Zb; }
     publish_and_combine<MATH>(P, A, b, P.blocks_per_ctrl, s_unom, s_red, s_pair, s_vnom);
+}
+
+template <int MATH>
+__device__ __forceinline__ void block_partial_and_combine(const DevParams& P, const StepArgs& A, const int b,
+                                                          const int chunk, const float J, const float lo, const float hi,
+                                                          const float4* s_unom, float* s_red, float4* s_acc, float* s_pair,
+                                                          const float* s_vnom = nullptr, float* s_acc5 = nullptr,
+                                                          const bool stored = false)
+{
+    const float Jv[1] = {J};
+    block_partial_and_combine_n<MATH, 1>(P, A, b, chunk, (uint32_t)(chunk * blockDim.x), Jv, lo, hi, stored, s_unom, s_red,
+                                         s_acc, s_pair, s_vnom, s_acc5);
 }
 
 // Fused softmax update, second half ("last block done").  Every block of controller b has written
@@ -317,19 +416,25 @@ __device__ __forceinline__ void publish_and_combine(const DevParams& P, const St
     }
     float4* w4 = reinterpret_cast<float4*>(A.weights + (size_t)b * P.K);
     const float nil = -P.inv_lambda;
+    int nz = 0;                                // samples of this thread that carry weight
+    auto weights_of = [&](const float4 c) {
+        const float4 w = make_float4(exp_weight<MATH>((c.x - beta) * nil) * invZ, exp_weight<MATH>((c.y - beta) * nil) * invZ,
+                                     exp_weight<MATH>((c.z - beta) * nil) * invZ, exp_weight<MATH>((c.w - beta) * nil) * invZ);
+        nz += (w.x > 0.0f) + (w.y > 0.0f) + (w.z > 0.0f) + (w.w > 0.0f);
+        return w;
+    };
 #pragma unroll
     for (int r = 0; r < PRE; ++r) {
         const int i = tid + r * nthr;
-        const float4 c = cpre[r];
-        if (i < n4)
-            w4[i] = make_float4(exp_weight<MATH>((c.x - beta) * nil) * invZ, exp_weight<MATH>((c.y - beta) * nil) * invZ,
-                                exp_weight<MATH>((c.z - beta) * nil) * invZ, exp_weight<MATH>((c.w - beta) * nil) * invZ);
+        if (i < n4) w4[i] = weights_of(cpre[r]);
     }
 #pragma unroll 4
-    for (int i = tid + PRE * nthr; i < n4; i += nthr) {
-        const float4 c = __ldcg(c4 + i);
-        w4[i] = make_float4(exp_weight<MATH>((c.x - beta) * nil) * invZ, exp_weight<MATH>((c.y - beta) * nil) * invZ,
-                            exp_weight<MATH>((c.z - beta) * nil) * invZ, exp_weight<MATH>((c.w - beta) * nil) * invZ);
+    for (int i = tid + PRE * nthr; i < n4; i += nthr) w4[i] = weights_of(__ldcg(c4 + i));
+    if (A.hint) {
+        // Hint for the NEXT launch on this controller (keeps_du): did many samples carry weight?  Then the sparse
+        // re-derivation of the block partials costs a second pass over the noise stream and storing dU is cheaper.
+        const float nnz = block_sum((float)nz, s_red);
+        if (tid == 0) A.hint[b] = nnz * 32.0f > (float)P.K ? 1u : 0u;
     }
     if (tid == 0) A.counters[b] = 0u;          // ready for the next launch
     if (A.done_flag) {

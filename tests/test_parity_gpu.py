@@ -248,6 +248,30 @@ def test_flat_weights_exercise_the_update(name, pipe):
     assert st["w"] <= Pz.W_ATOL and st["u"] <= Pz.U_ATOL
 
 
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "rate_gate_paper", "rate_track"])
+@pytest.mark.parametrize("opts", [dict(variant=3), dict(variant=1), dict(variant=3, store_noise=1), dict(variant=1, store_noise=1, block_threads=64)],
+                         ids=["packed_adaptive", "scalar_adaptive", "packed_stored", "scalar_stored"])
+def test_mixing_weights_dense_update_from_stored_noise(name, opts):
+    # eq.(5) PAPER.md:91-95 when MANY samples carry weight: the fused throughput kernels then keep dU and sum it from
+    # memory (mppi_rollout.cuh, warp_noise_partial) instead of re-deriving the noise.  store_noise = 1 takes that path
+    # from the first iteration on; otherwise the previous iteration's combine switches it on (StepArgs::hint), so
+    # iteration 0 re-derives and iterations 1, 2 read back.  All must meet the strict bounds.  N = 37 leaves a ragged
+    # last group of the eight-step butterfly, B = 3 checks the per-controller hint.
+    wl = W.replicate(W.ALL[name](K=1024, N=37), 3, 0.2)
+    o0 = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, wl.seed, 0)
+    wl.params["lambda"] = float(np.float32(0.25 * np.median(o0["cost"].std(-1))))
+    m = Pz.make_ctx(wl, **opts)
+    x0, start, u = Pz.to_dev(wl)
+    for it in range(3):
+        u_in = u.cpu().numpy()
+        g = Pz.gpu_step(m, x0, start, u, wl.seed, it, u_new=u)        # warm start in place
+        o = Pz.oracle_step(wl, wl.x0, wl.start, u_in, wl.seed, it, want_du=True)
+        st = Pz.compare(f"mixing-{name}[{opts}] it{it}", g, o, wl.params["lambda"], False)
+        assert st["ess"] > 20
+        assert st["w"] <= Pz.W_ATOL and st["u"] <= Pz.U_ATOL
+    m.close()
+
+
 def test_noise_matches_oracle_and_pipelines_agree():
     import torch
     wl = W.cfg0(K=512, N=37)
