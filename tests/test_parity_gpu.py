@@ -431,6 +431,40 @@ def test_determinism_and_host_entry_point():
         m.close()
 
 
+@pytest.mark.parametrize("case", ["contour_max_path_max_horizon", "track_max_horizon_many_samples", "gate_max_horizon"])
+def test_auto_falls_back_when_the_latency_kernels_do_not_fit(case):
+    # AUTO picks the pipelined / latency kernel from the warp count alone, before the track is known; at the limits of
+    # include/mppi.h (MPPI_MAX_N = 256, MPPI_MAX_PATH = 2048) their rings / thrust tables do not fit in 227 KB of
+    # shared memory beside the track.  The first step must then move to a kernel that fits instead of failing.
+    if case == "contour_max_path_max_horizon":
+        wl = W.cfg3(K=4096, N=256)
+        a = 2 * np.pi * np.arange(2048) / 2048
+        wl.path = np.stack([5 * np.cos(a), 5 * np.sin(a), 1.5 + 0.2 * np.sin(3 * a)], 1).astype(np.float32)
+    elif case == "track_max_horizon_many_samples":
+        wl = W.cfg2(K=16384, N=256)
+    else:
+        wl = W.cfg1(K=2048, N=256)
+    wl.params["sigma"] = float(np.float32(0.3))
+    wl.params["dt"] = float(np.float32(0.005))             # 256 steps = 1.28 s of horizon (at 0.02 s the fp32 error of 5 s of free flight is the test)
+    m = Pz.make_ctx(wl)
+    x0, start, u = Pz.to_dev(wl)
+    g = Pz.gpu_step(m, x0, start, u, wl.seed, 0)
+    info = m.info()
+    assert info["dynamic_smem_bytes"] <= 227 * 1024
+    o = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, wl.seed, 0, want_du=True)
+    Pz.compare(f"auto fallback {case} ({info['block_threads']} thr x {info['grid_blocks']})", g, o, wl.params["lambda"],
+               wl.params["objective"] == 0)
+    m.close()
+    # an explicit request for a kernel that does not fit still fails cleanly
+    if case != "gate_max_horizon":
+        from paper_2509_14726_b200 import binding as Bd
+        m = Pz.make_ctx(wl, variant=2 if case.startswith("contour") else 4)
+        with pytest.raises(Bd.MppiError) as e:
+            m.step(x0, start, u, wl.seed, 0)
+        assert e.value.status == -2
+        m.close()
+
+
 def test_seed_high_word_reaches_the_key():
     wl = W.cfg0(K=64, N=5)
     wl.seed = (0xDEADBEEF << 32) | 0x12345678
