@@ -34,6 +34,7 @@ struct mppi_ctx {
     float4* d_path = nullptr;
     float4* d_du = nullptr;
     float* d_partials = nullptr;
+    float2* d_headers = nullptr;
     unsigned* d_counters = nullptr;
     unsigned* d_hint = nullptr;            // [B] dense-weights hint of the previous iteration (StepArgs::hint)
     bool keep_du = false;                  // d_du belongs to the caller-visible contract (two-pass / store_noise)
@@ -278,7 +279,7 @@ extern "C" int mppi_destroy(mppi_ctx* c)
     cudaDeviceSynchronize();
     free_graph(c->g_step); free_graph(c->g_opt);
     cudaFree(c->d_gates); cudaFree(c->d_ref); cudaFree(c->d_path); cudaFree(c->d_du);
-    cudaFree(c->d_partials); cudaFree(c->d_counters); cudaFree(c->d_hint);
+    cudaFree(c->d_partials); cudaFree(c->d_headers); cudaFree(c->d_counters); cudaFree(c->d_hint);
     if (c->h_pin) cudaFreeHost(c->h_pin);
     cudaFree(c->d_in);
     cudaFree(c->d_hx0); cudaFree(c->d_hstart); cudaFree(c->d_hu); cudaFree(c->d_hcost); cudaFree(c->d_hw);
@@ -351,7 +352,8 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     cfg.rate = p->input_model == 1;
     c->xdim = p->objective == MPPI_OBJ_CONTOUR_PAPER ? 19 : cfg.rate ? 17 : 13;
     d.blocks_per_ctrl = blocks_per_ctrl_of(p, cfg);
-    d.part_stride = 4 * p->N + 4 + (p->objective == MPPI_OBJ_CONTOUR_PAPER ? ((p->N + 3) & ~3) : 0);
+    // floats per partial, a multiple of 8: every 32-byte sector of a partial is then written completely
+    d.part_stride = (4 * p->N + 4 + (p->objective == MPPI_OBJ_CONTOUR_PAPER ? p->N : 0) + 7) & ~7;
     cfg.pipe_shallow = 0;
     cfg.smem_bytes = 0;   // fixed once the track is known
     // input_model = 1: the pipelined latency kernel is the faster one for few rollouts, but its rings share the
@@ -377,6 +379,7 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     if (cfg.store_du) CKC(dev_alloc(c, &c->d_du, (size_t)p->B * p->N * p->K));
     if (cfg.fused) {
         CKC(dev_alloc(c, &c->d_partials, (size_t)p->B * max_blocks * d.part_stride));
+        CKC(dev_alloc(c, &c->d_headers, (size_t)p->B * max_blocks));
         CKC(dev_alloc(c, &c->d_counters, (size_t)p->B + 1));
         CKC(cudaMemset(c->d_counters, 0, ((size_t)p->B + 1) * sizeof(unsigned)));
         CKC(dev_alloc(c, &c->d_hint, (size_t)p->B));
@@ -605,10 +608,17 @@ static StepArgs make_args(mppi_ctx* c, const float* x0, const int32_t* start, co
 {
     StepArgs a;
     a.x0 = x0; a.start = start; a.u_nom = u_nom; a.u_new = u_new; a.cost = cost; a.weights = w;
-    a.du = c->d_du; a.partials = c->d_partials; a.counters = c->d_counters;
+    a.du = c->d_du; a.partials = c->d_partials; a.headers = c->d_headers; a.counters = c->d_counters;
     a.hint = (c->cfg.fused && !c->cfg.pipe && !c->cfg.lat_consumers && c->d_du) ? c->d_hint : nullptr;
     a.prev_front = c->d_prev_front; a.v_nom = c->d_v_nom; a.v_new = c->d_v_new;
     a.done_flag = nullptr; a.done_value = 0;
+#ifdef MPPI_TIMELINE
+    {
+        static unsigned long long* tl = nullptr;      // profiling builds only: one buffer, read back by the probe script
+        if (!tl) { cudaMalloc(&tl, 16 * 65536 * sizeof(unsigned long long)); cudaMemset(tl, 0, 16 * 65536 * sizeof(unsigned long long)); }
+        a.timeline = tl;
+    }
+#endif
     a.seed_lo = (uint32_t)(seed & 0xffffffffu); a.seed_hi = (uint32_t)(seed >> 32); a.iter = iter;
     for (uint32_t r = 0; r < 10; ++r) {          // Philox key schedule (Weyl sequence), hoisted out of the kernel
         a.rk[2 * r] = a.seed_lo + r * 0x9E3779B9u;
@@ -852,6 +862,15 @@ extern "C" int mppi_front_flags(mppi_ctx* c, const float* d_x0, const int32_t* d
 extern "C" const float* mppi_debug_noise(mppi_ctx* c) { return (c && c->keep_du) ? reinterpret_cast<const float*>(c->d_du) : nullptr; }
 
 extern "C" int64_t mppi_launch_count(mppi_ctx* c) { return c ? c->launches : 0; }
+
+#ifdef MPPI_TIMELINE
+extern "C" MPPI_API int mppi_timeline_read(mppi_ctx* c, unsigned long long* host_out, int blocks)
+{
+    StepArgs a = make_args(c, nullptr, nullptr, nullptr, 0, 0, nullptr, nullptr, nullptr);
+    cudaDeviceSynchronize();
+    return cudaMemcpy(host_out, a.timeline, (size_t)blocks * 16 * sizeof(unsigned long long), cudaMemcpyDeviceToHost) == cudaSuccess ? 0 : -6;
+}
+#endif
 
 extern "C" int mppi_get_info(mppi_ctx* c, mppi_info* o)
 {

@@ -15,7 +15,7 @@ struct DevParams {
     int G, M, P, closed, window;      // gates, reference rows, path points
     int blocks_per_ctrl;               // rollout blocks per controller = K / blockDim.x
     int pipe_d, pipe_df;               // rollout_pipe_rate_kernel: ring depths in chunks (W / Q rings, F ring)
-    int part_stride;                   // floats per partial: 4N + 4 (+ N rounded up to 4 under OBJ_CONTOUR_PAPER)
+    int part_stride;                   // floats per partial: 4N + 4 (+ N under OBJ_CONTOUR_PAPER), rounded up to a multiple of 8
     float dt, inv_lambda, sigma, T_min, T_max;
     float bm_k, bm_kv;                 // -2 ln2 sigma^2, -2 ln2 sigma_v^2: Box-Muller radius constants of the fast path
     float h2, h3, h4, h6, h12, hh2, hh3;   // dt/2, dt/3, dt/4, dt/6, dt/12, dt^2/2, dt^2/3
@@ -46,7 +46,8 @@ struct StepArgs {
     float* cost;           // [B][K]
     float* weights;        // [B][K]
     float4* du;            // [B][N][K] float4 or nullptr
-    float* partials;       // [B][blocks_per_ctrl][part_stride]: S[4N], m, Z, -, - [, S5[N]]  (fused pipeline)
+    float* partials;       // [B][blocks_per_ctrl][part_stride]: S[4N], 4 spare, [S5[N]]  (fused pipeline)
+    float2* headers;       // [B][blocks_per_ctrl]: (m, Z) of every partial, contiguous per controller
     unsigned int* counters;// [B + 1]: last-block tickets per controller, finished controllers (fused pipeline)
     unsigned int* hint;    // [B] or nullptr (fused throughput kernels): written by the combine of one launch, read by
                            // the next: != 0 = many samples carried weight, keep dU in `du` and sum it from there
@@ -56,9 +57,25 @@ struct StepArgs {
     const int* prev_front; // [B][N+1] or nullptr: previous-iteration "in front" flags (paper's J_gate, Fig. 2)
     unsigned int* done_flag;   // mapped host word, or nullptr: set to done_value once every output of the
     unsigned int done_value;   // call is visible to the host (mppi_step_host polls it instead of a stream sync)
+#ifdef MPPI_TIMELINE
+    unsigned long long* timeline;   // profiling builds only (-DMPPI_TIMELINE): [blocks][16] %globaltimer stamps
+#endif
     uint32_t seed_lo, seed_hi, iter;
     uint32_t rk[20];       // Philox round keys: rk[2r] = seed_lo + r W0, rk[2r+1] = seed_hi + r W1
 };
+
+// Profiling aid, compiled only with -DMPPI_TIMELINE (never in the library that ships): thread `who` of the block
+// stamps %globaltimer into slot i of its block's row.
+#ifdef MPPI_TIMELINE
+#if MPPI_TIMELINE == 2      // SM-local cycle counter (deltas within one block only)
+#define MPPI_STAMP(A, i) do { (A).timeline[(size_t)(blockIdx.y * gridDim.x + blockIdx.x) * 16 + (i)] = (unsigned long long)clock64(); } while (0)
+#else
+#define MPPI_STAMP(A, i) do { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); \
+    (A).timeline[(size_t)(blockIdx.y * gridDim.x + blockIdx.x) * 16 + (i)] = t_; } while (0)
+#endif
+#else
+#define MPPI_STAMP(A, i) do { } while (0)
+#endif
 
 // ---- Philox4x32-10, counter-based (Salmon et al., SC'11) [R-1] -----------------------------
 // eq.(3) PAPER.md:78-82 asks for independent Gaussian perturbations; north_star fixes the

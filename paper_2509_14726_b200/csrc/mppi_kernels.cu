@@ -203,7 +203,7 @@ struct SmemThrust {
 constexpr int kLatThreads = 256;
 
 template <int OBJ, int MATH, bool STORE_DU>
-__global__ void __launch_bounds__(kLatThreads) rollout_lat_kernel(const DevParams P, const StepArgs A, const int C)
+__global__ void __launch_bounds__(kLatThreads, 2) rollout_lat_kernel(const DevParams P, const StepArgs A, const int C)
 {
     extern __shared__ float4 smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -262,8 +262,8 @@ __global__ void __launch_bounds__(kLatThreads) rollout_lat_kernel(const DevParam
         }
         part[j] = acc;
     }
-    if (tid == 0) { part[4 * N] = m; part[4 * N + 1] = Zb; }
-    publish_and_combine<MATH>(P, A, b, P.blocks_per_ctrl, s_unom, s_red, s_pair);
+    if (tid == 0) write_partial_header(P, A, b, blockIdx.x, m, Zb);
+    publish_and_combine<MATH, 4>(P, A, b, P.blocks_per_ctrl, s_unom, s_red, s_pair, reinterpret_cast<float*>(s_T));
 }
 
 // ---------------------------------------------------------------------------------------------

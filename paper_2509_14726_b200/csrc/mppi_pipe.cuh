@@ -99,14 +99,14 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
     float4* s_w = s_T + (size_t)N * RS;                                  // [D][C][3][32]
     float4* s_q = s_w + D * C * 3 * 32;                                  // [D][C][4][32]
     float* s_J = reinterpret_cast<float*>(s_q + D * C * 4 * 32);         // [3][32]
-    float* s_e = s_J + 96;                                               // [32]
-    float* s_pair = s_e + 32;                                            // 3 nb floats
+    float* s_pair = s_J + 128;                                           // 3 nb floats (32 floats after s_J are spare)
     uint64_t* bar_T = reinterpret_cast<uint64_t*>(reinterpret_cast<float4*>(s_pair) + (3 * P.blocks_per_ctrl + 3) / 4);
     uint64_t* bar_wf = bar_T + nchunks;    // ring W full / empty, ring Q full / empty
     uint64_t* bar_we = bar_wf + D;
     uint64_t* bar_qf = bar_we + D;
     uint64_t* bar_qe = bar_qf + D;
 
+    if (tid == 0) MPPI_STAMP(A, 0);
     const int start = A.start[b];
     stage_inputs<OBJ>(P, A, b, start, s_unom, s_trk);
     for (int i = tid; i < nchunks + 4 * D; i += kPipeThreads)
@@ -114,6 +114,7 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
     const State x0 = load_state(A.x0 + 13 * b);
     __syncthreads();
     const int i0 = OBJ == OBJ_CONTOUR ? contour_start_index(P, s_trk, start, x0, s_red) : 0;
+    if (tid == 0) MPPI_STAMP(A, 1);
 
     if (warp >= 3) {
         // ---- noise producers: step t is drawn by warp 3 + t % 5, one sample per lane (eq.(3)) ----
@@ -122,6 +123,8 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
             const float4 T = sample_thrust<MATH>(P, A.rk, (uint32_t)(kbase + lane), (uint32_t)t, A.iter, (uint32_t)b, un);
             s_T[t * RS + lane] = T;
             mbar_arrive(bar_T + t / C);
+            if (lane == 0 && t == 0) MPPI_STAMP(A, 2);
+            if (lane == 0 && t == N - 1) MPPI_STAMP(A, 3);
             if (STORE_DU)
                 A.du[((size_t)b * N + t) * P.K + kbase + lane] = make_float4(T.x - un.x, T.y - un.y, T.z - un.z, T.w - un.w);
         }
@@ -174,6 +177,7 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
             acc = fmaf(P.Qw, wx * wx + wy * wy + wz * wz, acc);
         }
         s_J[lane] = acc;
+        if (lane == 0) MPPI_STAMP(A, 4);
     } else if (warp == 1) {
         // ---- Q: attitude.  q' = 1/2 q (x) (0, omega), renormalised once per step [R-5] ----
         float qw = x0.qw, qx = x0.qx, qy = x0.qy, qz = x0.qz;
@@ -219,6 +223,7 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
         }
         if (OBJ == OBJ_TRACK) quat_term(s_trk + 4 * N);
         s_J[32 + lane] = acc;
+        if (lane == 0) MPPI_STAMP(A, 5);
     } else {
         // ---- P: translation and the position part of the objective ----
         State x = x0;
@@ -271,40 +276,46 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
         if (OBJ == OBJ_GATE_PAPER) J = gp.finish(P);
         if (OBJ == OBJ_TRACK) pv_term(s_trk + 4 * N);
         s_J[64 + lane] = J;
+        if (lane == 0) MPPI_STAMP(A, 6);
     }
     __syncthreads();
 
-    // ---- the three parts of the cost meet; warp 0 owns the block's 32 samples from here on ----
-    float m = 0.0f, Zb = 0.0f;
-    if (warp == 0) {
-        const float jw = s_J[lane], jq = s_J[32 + lane], jp = s_J[64 + lane];
-        float J;
-        if (OBJ == OBJ_GATE || OBJ == OBJ_GATE_PAPER) J = fmaf(P.w_omega, jw, jp);   // = finish() with W's sum |omega|^2
-        else if (OBJ == OBJ_TRACK) J = (jp + jq) + jw;
-        else J = jp + jw;
-        A.cost[(size_t)b * P.K + kbase + lane] = J;
-        m = warp_min(J);
-        const float e = exp_weight<MATH>((m - J) * P.inv_lambda);
-        Zb = warp_sum(e);
-        s_e[lane] = e;
-    }
-    __syncthreads();
+    // ---- the three parts of the cost meet.  Every warp forms the 32 costs, their minimum and the weights e_l on its
+    // own (three shared-memory reads and two shuffle reductions, the same values in every warp): no second barrier
+    // and no round trip through shared memory before the partial ----
+    const float jw = s_J[lane], jq = s_J[32 + lane], jp = s_J[64 + lane];
+    float J;
+    if (OBJ == OBJ_GATE || OBJ == OBJ_GATE_PAPER) J = fmaf(P.w_omega, jw, jp);   // = finish() with W's sum |omega|^2
+    else if (OBJ == OBJ_TRACK) J = (jp + jq) + jw;
+    else J = jp + jw;
+    if (warp == 0) A.cost[(size_t)b * P.K + kbase + lane] = J;
+    const float m = warp_min(J);
+    const float e = exp_weight<MATH>((m - J) * P.inv_lambda);
+    const float Zb = warp_sum(e);
+    const unsigned contrib = __ballot_sync(kFull, e != 0.0f);
 
-    // ---- block partial S[t][i] = sum_l e_l (T_l[t][i] - u_nom[t][i]) from the thrusts in shared memory ----
+    // ---- block partial S[t][i] = sum_l e_l (T_l[t][i] - u_nom[t][i]) from the thrusts in shared memory: thread j
+    // owns column j; only the samples with a non-zero weight are visited, in ascending order (e_l by shuffle) ----
     float* part = A.partials + ((size_t)b * P.blocks_per_ctrl + blockIdx.x) * P.part_stride;
-    for (int j = tid; j < 4 * N; j += kPipeThreads) {
+    for (int j0 = warp * 32; j0 < 4 * N; j0 += kPipeThreads) {
+        const int j = j0 + lane;
+        const bool live = j < 4 * N;
         const int t = j >> 2, i = j & 3;
-        const float un = reinterpret_cast<const float*>(s_unom)[j];
-        const float* row = reinterpret_cast<const float*>(s_T + t * RS) + i;
+        const float un = live ? reinterpret_cast<const float*>(s_unom)[j] : 0.0f;
+        const float* row = reinterpret_cast<const float*>(s_T + (live ? t : 0) * RS) + i;
         float acc = 0.0f;
-        for (int l = 0; l < 32; ++l) {
-            const float el = s_e[l];                      // block-uniform
-            if (el != 0.0f) acc = fmaf(el, row[4 * l] - un, acc);
+        unsigned mm = contrib;
+        while (mm) {
+            const int l = __ffs(mm) - 1;
+            mm &= mm - 1;
+            acc = fmaf(__shfl_sync(kFull, e, l), row[4 * l] - un, acc);
         }
-        part[j] = acc;
+        if (live) part[j] = acc;
     }
-    if (tid == 0) { part[4 * N] = m; part[4 * N + 1] = Zb; }
-    publish_and_combine<MATH>(P, A, b, P.blocks_per_ctrl, s_unom, s_red, s_pair);
+    if (tid == 0) write_partial_header(P, A, b, blockIdx.x, m, Zb);
+    if (tid == 0) MPPI_STAMP(A, 7);
+    publish_and_combine<MATH, 4>(P, A, b, P.blocks_per_ctrl, s_unom, s_red, s_pair, reinterpret_cast<float*>(s_T));
+    if (tid == 0) MPPI_STAMP(A, 12);
 }
 
 #undef MPPI_G

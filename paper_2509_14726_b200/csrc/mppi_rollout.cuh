@@ -157,14 +157,22 @@ __device__ __forceinline__ float rollout_cost(const DevParams& P, const float4* 
     return J;
 }
 
+// header of a partial: (m, Z) of block `chunk` of controller b, in an array of its own (8 bytes per partial, contiguous
+// per controller) so that the combining block reads all headers of a controller in nb / 16 cache lines.
+__device__ __forceinline__ void write_partial_header(const DevParams& P, const StepArgs& A, const int b, const int chunk,
+                                                     const float m, const float Zb)
+{
+    A.headers[(size_t)b * P.blocks_per_ctrl + chunk] = make_float2(m, Zb);
+}
+
 // Fused softmax update, first half, for kernels with one sample per thread: the block's online-softmax
 // partial  m = min_k J, e_k = exp(-(J_k - m)/lambda), Z = sum e_k, S[t] = sum_k e_k dU_k[t]  (eq.(4),(5)).
 // dU is not stored anywhere: for the samples with e_k > 0 it is re-derived from the counter-based
 // stream (inputs clamped to [lo, hi] as in the rollout), the warp's lanes spread over the horizon
 // steps.  Then publish_and_combine.  All threads of the block must call this.
-template <int MATH>
+template <int MATH, int ROWS = 2>
 __device__ __forceinline__ void publish_and_combine(const DevParams& P, const StepArgs& A, int b, int nb,
-                                                    const float4* s_unom, float* s_red, float* s_pair,
+                                                    const float4* s_unom, float* s_red, float* s_pair, float* s_work,
                                                     const float* s_vnom = nullptr);
 template <int MATH>
 __device__ __forceinline__ float sample_progress_accel(const DevParams& P, const uint32_t (&rk)[20], uint32_t k,
@@ -305,8 +313,8 @@ __device__ __forceinline__ void block_partial_and_combine_n(const DevParams& P, 
             for (int w = 0; w < nw; ++w) s += s_acc5[w * N + t];
             part[4 * N + 4 + t] = s;
         }
-    if (tid == 0) { part[4 * N] = m; part[4 * N + 1] = Zb; }
-    publish_and_combine<MATH>(P, A, b, P.blocks_per_ctrl, s_unom, s_red, s_pair, s_vnom);
+    if (tid == 0) write_partial_header(P, A, b, chunk, m, Zb);
+    publish_and_combine<MATH>(P, A, b, P.blocks_per_ctrl, s_unom, s_red, s_pair, reinterpret_cast<float*>(s_acc), s_vnom);
 }
 
 template <int MATH>
@@ -328,10 +336,14 @@ __device__ __forceinline__ void block_partial_and_combine(const DevParams& P, co
 //   u_new = u_nom + sum_q S_q exp(-(m_q - beta)/lambda) / Z_tot,   w_k = exp(-(J_k - beta)/lambda) / Z_tot.
 // Partials whose rescale factor underflows to 0 contribute exactly 0 and are not read.
 //
-// This runs after the last rollout of the controller has finished, so it is on the critical path of
-// the iteration latency: the chain is kept to three L2 round trips -- ticket; (m, Z) pairs together
-// with the first costs; the S rows of the few partials that still count -- and the contributing
-// partials are compacted (deterministically, by index) so that nobody scans nb scale factors.
+// This runs after the last rollout of the controller has finished, so it is on the critical path of the
+// iteration latency.  Measured with clock64 stamps (profiles/README_r02c.md): round 1's form -- block-wide min,
+// sum and compaction, seven __syncthreads -- took 7600 cycles in the block that runs it (5400 with a warm
+// instruction cache), of which only ~1500 are the two L2 round trips it needs.  For up to kCombineFast x 32
+// partials every WARP therefore derives beta, Z and the list of contributing partials on its own, from registers
+// and shuffles (all warps compute the same values in the same order, so the result does not depend on the warp),
+// and goes straight on to its columns of u_new and its share of the weights: ticket; (m, Z) pairs together with
+// the first costs; S rows of the partials that count -- and no block barrier after the ticket.
 // s_pair: 3 nb floats of shared memory.  All threads of the block must call this.
 __device__ __forceinline__ unsigned ticket_acq_rel(unsigned* ctr)
 {
@@ -340,24 +352,29 @@ __device__ __forceinline__ unsigned ticket_acq_rel(unsigned* ctr)
     return old;
 }
 
-template <int MATH>
+constexpr int kCombineFast = 8;        // (m, Z) pairs a lane keeps in registers: per-warp combine for nb <= 256
+
+template <int MATH, int ROWS>
 __device__ __forceinline__ void publish_and_combine(const DevParams& P, const StepArgs& A, int b, int nb,
-                                                    const float4* s_unom, float* s_red, float* s_pair,
+                                                    const float4* s_unom, float* s_red, float* s_pair, float* s_work,
                                                     const float* s_vnom)
 {
-    const int tid = threadIdx.x, lane = tid & 31, N = P.N, stride = P.part_stride, nthr = blockDim.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, N = P.N, stride = P.part_stride, nthr = blockDim.x;
+    const int nw = nthr >> 5;
     int* s_flag = reinterpret_cast<int*>(s_red) + 48;
     int* s_cnt = s_flag + 1;
     __syncthreads();                               // the block's partial is written (CTA-scope order) ...
     if (tid == 0) *s_flag = (ticket_acq_rel(&A.counters[b]) == (unsigned)(nb - 1));   // ... and released here
+    if (tid == 0) MPPI_STAMP(A, 8);
     __syncthreads();
     if (!*s_flag) return;
+    if (tid == 0) MPPI_STAMP(A, 13);
 
     const float* pb = A.partials + (size_t)b * nb * stride;
+    const float2* hb = A.headers + (size_t)b * nb;
     float* s_scale = s_pair;
-    float* s_z = s_pair + nb;
     int* s_list = reinterpret_cast<int*>(s_pair + 2 * nb);
-    // round trip 2: the (m, Z) pairs and this thread's first costs, all in flight together
+    // this thread's first costs (for the weights) go out together with the (m, Z) pairs
     const float4* c4 = reinterpret_cast<const float4*>(A.cost + (size_t)b * P.K);
     const int n4 = P.K >> 2;
     constexpr int PRE = 4;
@@ -365,55 +382,133 @@ __device__ __forceinline__ void publish_and_combine(const DevParams& P, const St
 #pragma unroll
     for (int r = 0; r < PRE; ++r)
         cpre[r] = tid + r * nthr < n4 ? __ldcg(c4 + tid + r * nthr) : make_float4(0.f, 0.f, 0.f, 0.f);
-    float bm = __int_as_float(0x7f800000);
-    for (int j = tid; j < nb; j += nthr) {
-        const float2 mz = __ldcg(reinterpret_cast<const float2*>(pb + (size_t)j * stride + 4 * N));
-        s_scale[j] = mz.x; s_z[j] = mz.y;
-        bm = fminf(bm, mz.x);
-    }
-    const float beta = block_min(bm, s_red);
-    float zz = 0.0f;
-    for (int j = tid; j < nb; j += nthr) {
-        const float sc = exp_weight<MATH>((beta - s_scale[j]) * P.inv_lambda);
-        s_scale[j] = sc;
-        zz = fmaf(s_z[j], sc, zz);
-    }
-    const float Z = block_sum(zz, s_red);      // its barriers also order the s_scale writes
-    const float invZ = 1.0f / Z;
-    // deterministic compaction of the partials with a non-zero scale (warp 0, ascending index)
-    if (tid < 32) {
-        int cnt = 0;
-        for (int j0 = 0; j0 < nb; j0 += 32) {
-            const int j = j0 + lane;
-            const bool on = j < nb && s_scale[j] != 0.0f;
-            const unsigned msk = __ballot_sync(kFull, on);
-            if (on) s_list[cnt + __popc(msk & ((1u << lane) - 1u))] = j;
-            cnt += __popc(msk);
+    const float inf = __int_as_float(0x7f800000);
+    float beta, invZ;
+    int cnt;
+    if (nb <= 32 * kCombineFast) {
+        // ---- per warp: registers and shuffles, no block barrier.  The headers are contiguous (8 bytes per partial),
+        // so a warp reads all of them in nb / 16 cache lines ----
+        float mq[kCombineFast], zq[kCombineFast];
+        float bm = inf;
+#pragma unroll
+        for (int r = 0; r < kCombineFast; ++r) {
+            const int j = lane + 32 * r;
+            mq[r] = inf; zq[r] = 0.0f;
+            if (j < nb) {
+                const float2 mz = __ldcg(hb + j);
+                mq[r] = mz.x; zq[r] = mz.y;
+            }
         }
-        if (lane == 0) *s_cnt = cnt;
-    }
-    __syncthreads();
-    const int cnt = *s_cnt;
-    // round trip 3: S rows of the contributing partials (columns 4N.. = the fifth input, kept after the header)
-    const int ncol = s_vnom ? 5 * N : 4 * N;
-    for (int jj = tid; jj < ncol; jj += nthr) {
-        const int j = jj < 4 * N ? jj : jj + 4;
-        float acc = 0.0f;
-        int i = 0;
-        for (; i + 4 <= cnt; i += 4) {
-            const int q0 = s_list[i], q1 = s_list[i + 1], q2 = s_list[i + 2], q3 = s_list[i + 3];
-            const float v0 = __ldcg(pb + (size_t)q0 * stride + j), v1 = __ldcg(pb + (size_t)q1 * stride + j),
-                        v2 = __ldcg(pb + (size_t)q2 * stride + j), v3 = __ldcg(pb + (size_t)q3 * stride + j);
-            acc = fmaf(v0, s_scale[q0], acc); acc = fmaf(v1, s_scale[q1], acc);
-            acc = fmaf(v2, s_scale[q2], acc); acc = fmaf(v3, s_scale[q3], acc);
+#pragma unroll
+        for (int r = 0; r < kCombineFast; ++r) bm = fminf(bm, mq[r]);
+        if (tid == 0) MPPI_STAMP(A, 9);
+        beta = warp_min(bm);
+        if (tid == 0) MPPI_STAMP(A, 14);
+        float zz = 0.0f;
+        cnt = 0;
+#pragma unroll
+        for (int r = 0; r < kCombineFast; ++r) {
+            if (32 * r < nb) {                         // uniform
+                const float sc = lane + 32 * r < nb ? exp_weight<MATH>((beta - mq[r]) * P.inv_lambda) : 0.0f;
+                zz = fmaf(zq[r], sc, zz);
+                const bool on = sc != 0.0f;
+                const unsigned msk = __ballot_sync(kFull, on);
+                if (on) {                              // ascending partial index: deterministic order of the sums
+                    const int at = cnt + __popc(msk & ((1u << lane) - 1u));
+                    s_list[at] = lane + 32 * r; s_scale[at] = sc;
+                }
+                cnt += __popc(msk);
+            }
         }
-        for (; i < cnt; ++i) {
-            const int q = s_list[i];
-            acc = fmaf(__ldcg(pb + (size_t)q * stride + j), s_scale[q], acc);
+        if (tid == 0) MPPI_STAMP(A, 15);
+        invZ = 1.0f / warp_sum(zz);                    // fixed butterfly order: identical in every warp
+        __syncwarp();                                  // this warp's (identical) copy of the list is visible to its lanes
+    } else {
+        // ---- general form: block-wide reductions through shared memory ----
+        float* s_z = s_pair + nb;
+        float bm = inf;
+        for (int j = tid; j < nb; j += nthr) {
+            const float2 mz = __ldcg(hb + j);
+            s_scale[j] = mz.x; s_z[j] = mz.y;
+            bm = fminf(bm, mz.x);
         }
-        if (jj < 4 * N) A.u_new[(size_t)b * 4 * N + j] = fmaf(acc, invZ, reinterpret_cast<const float*>(s_unom)[j]);
-        else A.v_new[(size_t)b * N + jj - 4 * N] = fmaf(acc, invZ, s_vnom[jj - 4 * N]);
+        beta = block_min(bm, s_red);
+        float zz = 0.0f;
+        for (int j = tid; j < nb; j += nthr) {
+            const float sc = exp_weight<MATH>((beta - s_scale[j]) * P.inv_lambda);
+            zz = fmaf(s_z[j], sc, zz);
+            s_scale[j] = sc;
+        }
+        invZ = 1.0f / block_sum(zz, s_red);      // its barriers also order the s_scale writes
+        // deterministic compaction of the partials with a non-zero scale (warp 0, ascending index): (index, scale)
+        // pairs; the compacted scales go to s_z, which nobody reads any more
+        if (tid < 32) {
+            int c = 0;
+            for (int j0 = 0; j0 < nb; j0 += 32) {
+                const int j = j0 + lane;
+                const float sc = j < nb ? s_scale[j] : 0.0f;
+                const bool on = sc != 0.0f;
+                const unsigned msk = __ballot_sync(kFull, on);
+                if (on) { const int at = c + __popc(msk & ((1u << lane) - 1u)); s_list[at] = j; s_z[at] = sc; }
+                c += __popc(msk);
+            }
+            if (lane == 0) *s_cnt = c;
+        }
+        __syncthreads();
+        cnt = *s_cnt;
+        s_scale = s_z;
     }
+    if (tid == 0) MPPI_STAMP(A, 10);
+#ifdef MPPI_TIMELINE
+    if (tid == 0) A.timeline[(size_t)(blockIdx.y * gridDim.x + blockIdx.x) * 16 + 3] = (unsigned long long)cnt;
+#endif
+    // ---- S rows of the contributing partials.  Warp w takes the partials list[w], list[w + nw], ...; its lanes take
+    // the columns lane, lane + 32, ... -- every load of the block is in flight at once (one L2 round trip whatever the
+    // number of contributing partials; thread-per-column with four loads per round took cnt / 4 round trips).  The
+    // warps' sums meet in s_work [nw][group columns] and are added in warp order: deterministic.
+    // Column groups: the 4N thrust columns, then (fifth input) the N columns kept after the header.
+    const float* unf = reinterpret_cast<const float*>(s_unom);
+    for (int grp = 0; grp < (s_vnom ? 2 : 1); ++grp) {
+        const int gcol = grp ? N : 4 * N, goff = grp ? 4 * N + 4 : 0;
+        constexpr int CMAX = 8;                        // columns per lane and sweep: 256 columns per sweep
+        for (int c0 = 0; c0 < gcol; c0 += 32 * CMAX) {
+            float acc[CMAX];
+#pragma unroll
+            for (int c = 0; c < CMAX; ++c) acc[c] = 0.0f;
+            // batches of kRows partials per warp: all their loads are issued before the first use (ROWS: 4 in the
+            // latency kernels, where the iteration time is this chain; 2 where the register budget is the rollout's)
+            constexpr int kRows = ROWS;
+            for (int i0 = warp; i0 < cnt; i0 += kRows * nw) {
+                float v[kRows][CMAX], sc[kRows];
+#pragma unroll
+                for (int r = 0; r < kRows; ++r) {
+                    const int i = i0 + r * nw;
+                    const bool on = i < cnt;
+                    sc[r] = on ? s_scale[i] : 0.0f;
+                    const float* row = pb + (size_t)(on ? s_list[i] : 0) * stride + goff + c0 + lane;
+#pragma unroll
+                    for (int c = 0; c < CMAX; ++c)
+                        v[r][c] = (on && c0 + 32 * c + lane < gcol) ? __ldcg(row + 32 * c) : 0.0f;
+                }
+#pragma unroll
+                for (int r = 0; r < kRows; ++r)
+#pragma unroll
+                    for (int c = 0; c < CMAX; ++c) acc[c] = fmaf(v[r][c], sc[r], acc[c]);
+            }
+#pragma unroll
+            for (int c = 0; c < CMAX; ++c)
+                if (c0 + 32 * c + lane < gcol) s_work[warp * gcol + c0 + 32 * c + lane] = acc[c];
+        }
+        __syncthreads();
+        for (int j = tid; j < gcol; j += nthr) {
+            float s = 0.0f;
+            for (int w = 0; w < nw; ++w) s += s_work[w * gcol + j];
+            if (grp == 0) A.u_new[(size_t)b * 4 * N + j] = fmaf(s, invZ, unf[j]);
+            else A.v_new[(size_t)b * N + j] = fmaf(s, invZ, s_vnom[j]);
+        }
+        if (s_vnom) __syncthreads();                   // s_work is reused by the next group
+    }
+    if (tid == 0) MPPI_STAMP(A, 11);
     float4* w4 = reinterpret_cast<float4*>(A.weights + (size_t)b * P.K);
     const float nil = -P.inv_lambda;
     int nz = 0;                                // samples of this thread that carry weight
