@@ -39,6 +39,10 @@ UNIT = "sample-steps/s"
 FLOPS_PER_SAMPLE_STEP = {0: 417.0, 1: 449.0, 2: 685.0}
 FP32_LANES_PER_SM = 128
 L2_FLUSH_BYTES = 256 << 20
+# Issue slots of the scalar gate loop per warp-step (32 sample-steps), by instruction class (
+# cuobjdump -sass of rollout_kernel<OBJ_GATE, fast math>): 154 FFMA (53 with three register operands, 101 with a
+# constant operand), 67 FMUL, 44 FADD, 20 Philox half-rounds (IMAD.WIDE + LOP3), 11 MUFU, 8 FMNMX, 7 LDS.128.
+GATE_LOOP_MIX = {"ffma_rrr": 53, "ffma_const": 101, "fmul": 67, "fadd": 44, "philox_half_round": 20, "mufu": 11, "fmnmx": 8, "lds": 7}
 NCU_DRAM_BYTES_PER_LAUNCH = 53248     # rollout_pipe_kernel<gate>, cfg1: 53.2 KB read + 0 B written (profiles/README_r01e.md)
 
 
@@ -117,6 +121,26 @@ class ClockSampler(threading.Thread):
 # the reference arm / cpu_baseline: the oracle as it stands, on the host cores
 # ---------------------------------------------------------------------------------------------
 
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.lower().startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def set_oracle_threads(n: int | None):
+    """OpenMP team size of the oracle's sample loop (None = all online cores).  The oracle itself is not touched:
+    this calls omp_set_num_threads of the OpenMP runtime it is linked against."""
+    import ctypes
+    from oracle import oracle as O
+    O.lib()                                     # make sure libgomp is loaded
+    gomp = ctypes.CDLL("libgomp.so.1")
+    gomp.omp_set_num_threads(int(n or os.cpu_count() or 1))
+
+
 def time_oracle(wl, budget_s: float, max_iters: int, sample_K: int | None = None):
     """Runs full oracle iterations of `wl` (optionally on the first sample_K samples) until the
     budget or max_iters is reached.  Returns (sample-steps/s, seconds per iteration, iterations, threads)."""
@@ -170,7 +194,8 @@ def run_reference(args):
             "data": "synthetic",
             "config": {"workload": wl.name, "K": wl.params["K"], "N": wl.params["N"], "B": 1,
                        "objective": "gate", "sample_K": sample_K},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
+                             "cpu": cpu_model()},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -297,6 +322,18 @@ def run_ours(args):
         t_all = time.perf_counter() - t_all
         h2d = hx0.numel() * 4 + hstart.numel() * 4 + hu.numel() * 4
         d2h = hout.numel() * 4
+        # the same call returning everything north_star lists (u_new, per-sample costs, weights): 32 KB more through
+        # mapped host memory
+        hcost = np.empty((P["B"], P["K"]), np.float32); hw = np.empty_like(hcost)
+        host_call_all = m.step_host_fn(hx0.numpy(), hstart.numpy(), hu.numpy(), hout.numpy(), cost=hcost, weights=hw)
+        for i in range(max(args.warmup, 3)):
+            host_call_all(wl.seed, i)
+        lat_all = np.empty(n_e2e)
+        for i in range(n_e2e):
+            t0 = time.perf_counter()
+            host_call_all(wl.seed, i)
+            lat_all[i] = time.perf_counter() - t0
+        d2h_all = d2h + hcost.nbytes + hw.nbytes
 
         # ---- the batched configuration (configs[4] shape): where the FP32 roofline is reachable
         wl4 = W.cfg4()
@@ -327,16 +364,55 @@ def run_ours(args):
             ev[i + 1].record()
         torch.cuda.synchronize()
         loop_ms = np.array([ev[i].elapsed_time(ev[i + 1]) for i in range(n_loop)])[5:]
-        gates_passed = int(s4.max().item())
+        final_height_min = float(x4[:, 2].min().item())
+        # untimed replay of the same loop (same seeds: bit-identical) that counts the gate passes of every drone
+        x4.copy_(torch.from_numpy(wl4.x0).to(dev)); s4.copy_(torch.from_numpy(wl4.start).to(dev))
+        u4.copy_(torch.from_numpy(wl4.u_nom).to(dev))
+        passes = torch.zeros(P4["B"], dtype=torch.int64, device=dev)
+        for i in range(n_loop):
+            before = s4.clone()
+            m4.step(x4, s4, u4, wl4.seed, i, u_new=un4, cost=c4, weights=w4)
+            m4.sim_step(x4, s4, un4, u_nom_next=u4)
+            passes += (s4 != before)
+        passes = passes.cpu().numpy()
         flops = FLOPS_PER_SAMPLE_STEP[0]
         sm = info["sm_count"]
         peak_tf = sm * FP32_LANES_PER_SM * 2 * (clocks["sm_max_mhz"] or clock_attr_mhz) * 1e6 / 1e12
         ach = units * flops / (float(ms.mean()) * 1e-3) / 1e12
         ach4 = units4 * flops / (float(ms4.mean()) * 1e-3) / 1e12
 
-        # ---- cpu_baseline: the oracle on this host's cores, bounded sample
+        # ---- the instruction mix's own ceiling: issue rates measured on this device x the
+        # instruction counts of the scalar gate loop per 32 sample-steps (cuobjdump -sass of rollout_kernel<gate, fast>)
+        rates = Bd.measure_issue_rates()
+        mix = GATE_LOOP_MIX
+        pipes32 = {   # clocks per warp-step (32 sample-steps) each resource of a sub-partition is busy
+            "fma_pipe": (mix["ffma_rrr"] * rates["ffma_rrr"] + mix["ffma_const"] * rates["ffma_const"] + mix["fmul"] * rates["fmul"]
+                         + mix["fadd"] * rates["fadd"] + mix["philox_half_round"] * rates["philox_half_round"]),
+            "alu_pipe": mix["philox_half_round"] * 1.0 + mix["fmnmx"] * rates["fmnmx"],
+            "mufu_pipe": mix["mufu"] * rates["mufu"],
+            "issue_slots": float(sum(v * (2 if k == "philox_half_round" else 1) for k, v in mix.items())),
+        }
+        clocks32 = max(pipes32.values())
+        ideal32 = 32 * flops / (2 * FP32_LANES_PER_SM / 4)          # 64 flops per clock and sub-partition
+        launch_floor_us = Bd.measure_launch_floor(400)
+
+        # ---- cpu_baseline: the oracle as it stands on this host's cores, bounded samples:
+        # all online cores and ONE thread on the metric's config, and 5 control steps x 64 drones of configs[4]
         from oracle import oracle as O   # noqa: F401  (cpu_baseline leg only)
+        set_oracle_threads(None)
         cpu_rate, cpu_s_iter, cpu_n, cpu_threads = time_oracle(wl, args.cpu_budget, 5000)
+        set_oracle_threads(1)
+        cpu1_rate, cpu1_s_iter, cpu1_n, _ = time_oracle(wl, min(args.cpu_budget, 5.0), 5000)
+        set_oracle_threads(None)
+        wl4c = W.cfg4(steps=5)
+        trk4 = O.Track(gates=wl4c.gates)
+        xo, so, uo = wl4c.x0.astype(np.float64), wl4c.start.copy(), wl4c.u_nom.astype(np.float64)
+        O.step(wl4c.params, trk4, xo, so, uo, wl4c.seed, 0, want_diag=False)                   # warm
+        t0 = time.perf_counter()
+        for i in range(5):
+            r4 = O.step(wl4c.params, trk4, xo, so, uo, wl4c.seed, i, want_diag=False)
+            xo, so, uo = O.sim_step(wl4c.params, trk4, xo, so, r4["u_new"])
+        cpu4_s = (time.perf_counter() - t0) / 5
 
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -355,7 +431,10 @@ def run_ours(args):
             "e2e": {"value": units * n_e2e / t_all, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                     "d2h_bytes_per_step": int(d2h), "latency_us_p50": float(np.median(lat) * 1e6),
                     "latency_us_p99": float(np.percentile(lat, 99) * 1e6),
-                    "timer": "host perf_counter around mppi_step_host: one packed H2D copy from pinned memory, the kernel, u_new written by the kernel into mapped host memory, completion flag polled by the host"},
+                    "timer": "host perf_counter around mppi_step_host returning u_new only (cost / weights pointers NULL): one packed H2D copy from pinned memory, the kernel, u_new written by the kernel into mapped host memory, completion flag polled by the host",
+                    "with_cost_and_weights": {"value": units * n_e2e / float(lat_all.sum()), "unit": UNIT, "d2h_bytes_per_step": int(d2h_all),
+                                              "latency_us_p50": float(np.median(lat_all) * 1e6), "latency_us_p99": float(np.percentile(lat_all, 99) * 1e6),
+                                              "timer": "the same call returning u_new, the K costs and the K weights (what north_star's mppi_step returns), all written by the kernel into mapped host memory"}},
             "gpu_launches": int(launches),
             "roofline": {"bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
                          # dram__bytes_read.sum + dram__bytes_write.sum of this kernel, per launch, from the
@@ -365,18 +444,31 @@ def run_ours(args):
                          "peak_how": f"{sm} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 x clocks.max.sm (B200_PROFILING.md)",
                          "peak_measured_ffma_tflops": fma_tflops, "frac_of_measured_ffma": ach / fma_tflops,
                          "regs_per_thread": info["regs_per_thread"], "spill_bytes": info["local_bytes_per_thread"],
+                         "traffic_source": "profiles/README_r02c.md (ncu --set full capture of this kernel, dram__bytes_read.sum + dram__bytes_write.sum per launch; not measured in this run)" if args.pipeline == 0 else None,
                          "note": "K=4096 is 128 warps on 148 SMs: latency-bound by construction; see 'batched'"},
             "batched": {"workload": wl4.name, "K": P4["K"], "N": P4["N"], "B": P4["B"],
                         "value": units4 / (float(ms4.mean()) * 1e-3), "unit": UNIT, "ms_per_step": float(ms4.mean()),
                         "roofline": {"bound": "alu", "achieved": ach4, "peak": peak_tf, "unit": "TFLOP/s",
-                                     "frac": ach4 / peak_tf, "frac_of_measured_ffma": ach4 / fma_tflops},
+                                     "frac": ach4 / peak_tf, "frac_of_measured_ffma": ach4 / fma_tflops,
+                                     "mix_ceiling": {"issue_cycles_per_warp_instr": rates, "gate_loop_instr_per_32_sample_steps": GATE_LOOP_MIX,
+                                                     "busy_clocks_per_32_sample_steps": pipes32, "clocks_per_32_sample_steps": clocks32,
+                                                     "clocks_at_fp32_peak": ideal32, "frac_of_peak": ideal32 / clocks32,
+                                                     "how": "per resource of a sub-partition: sum over the loop's instruction classes of count x cycles per warp-instruction measured by mppi_measure_issue_rates (FFMA / FMUL / FADD and the 32x32->64 multiply of a Philox half-round occupy the FMA pipe, LOP3 / FMNMX the ALU pipe, MUFU its own; one issue slot per instruction); the busiest resource bounds the loop, and 32 x flops_per_sample_step / 64 flops per clock is the time at the FP32 peak -- their ratio is the fraction of the peak this instruction mix can reach however it is scheduled"}},
                         "closed_loop": {"control_steps": n_loop, "value": units4 / (float(loop_ms.mean()) * 1e-3),
                                         "unit": UNIT, "latency_us_p50": float(np.median(loop_ms) * 1e3),
                                         "latency_us_p99": float(np.percentile(loop_ms, 99) * 1e3),
-                                        "max_gate_index_reached": gates_passed,
+                                        "gate_passes_per_drone": {"min": int(passes.min()), "median": float(np.median(passes)), "max": int(passes.max())},
+                                        "final_height_min_m": final_height_min,
+                                        "note": "configs[4] as stated (sigma 1.5 N, lambda 0.5): the drones pass at most one gate and then lose height, so most timed control steps roll out from states below the track; the work per step is the same (checked against the oracle at steps 0, 50, .., 499: tests/test_parity_gpu.py::test_cfg4_closed_loop_teacher_forced)",
                                         "what": "mppi_step + mppi_sim_step per control step, 64 drones, CUDA events"}},
-            "cpu_baseline": {"value": cpu_rate, "unit": UNIT, "cores": cpu_threads, "kind": "oracle",
-                             "sample": f"{cpu_n} full iterations of {wl.name} ({cpu_s_iter * 1e3:.1f} ms each), float64, OpenMP over samples"},
+            "cpu_baseline": {"value": cpu_rate, "unit": UNIT, "cores": cpu_threads, "kind": "oracle", "cpu": cpu_model(),
+                             "sample": f"{cpu_n} full iterations of {wl.name} ({cpu_s_iter * 1e3:.1f} ms each), float64, OpenMP over samples",
+                             "single_thread": {"value": cpu1_rate, "unit": UNIT, "cores": 1,
+                                               "sample": f"{cpu1_n} full iterations of {wl.name} ({cpu1_s_iter * 1e3:.1f} ms each)"},
+                             "cfg4": {"value": units4 / cpu4_s, "unit": UNIT, "cores": cpu_threads, "s_per_control_step": cpu4_s,
+                                      "extrapolated_s_for_500_control_steps": 500 * cpu4_s,
+                                      "sample": "5 control steps x 64 drones of configs[4] (iteration + plant step), timed in full; the 500-step figure is a linear extrapolation"}},
+            "launch_floor_us": launch_floor_us,
         }
         m4.close()
     m.close()

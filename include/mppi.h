@@ -300,6 +300,18 @@ MPPI_API const char* mppi_last_error(mppi_ctx* ctx);   /* detail of the last fai
 MPPI_API int mppi_measure_fma_peak(int reps, double* tflops, double* sm_clock_mhz);
 MPPI_API int mppi_measure_copy_bw(int64_t bytes, int reps, double* gbs);
 
+/* Issue rates of the instruction classes the rollout loop consists of, for the ceiling of its instruction mix
+ * (DESIGN.md section 7): cycles per warp-instruction per SM sub-partition at saturation, measured with clock64.
+ * cycles_per_instr [n >= 8], host, out: 0 FFMA with three distinct register operands, 1 FFMA with a constant-bank
+ * operand, 2 FFMA2 (packed fp32x2, three register pairs), 3 FMUL, 4 FADD, 5 one Philox half-round (32x32->64
+ * multiply + three-input xor: two instructions), 6 MUFU.EX2, 7 FMNMX.  MPPI_E_RANGE if n < 8.  Synchronises. */
+MPPI_API int mppi_measure_issue_rates(double* cycles_per_instr, int n);
+
+/* Median time, in microseconds, between two CUDA events that bracket an EMPTY kernel of 128 blocks x 256 threads
+ * launched behind a busy GPU (reps launches, 8..4096): the part of any event-timed iteration latency that is the
+ * launch and the events, not the library.  Synchronises. */
+MPPI_API int mppi_measure_launch_floor(int reps, double* median_us);
+
 #ifdef __cplusplus
 }
 #endif

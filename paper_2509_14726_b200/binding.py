@@ -21,7 +21,7 @@ VARIANT_AUTO, VARIANT_THROUGHPUT, VARIANT_LATENCY, VARIANT_PACKED, VARIANT_PIPEL
 EXPORTS = ["mppi_default_params", "mppi_create", "mppi_destroy", "mppi_set_gates",
            "mppi_set_reference", "mppi_set_path", "mppi_step", "mppi_optimize", "mppi_step_host",
            "mppi_sim_step", "mppi_set_prev_front", "mppi_front_flags", "mppi_set_progress", "mppi_sim_step_progress", "mppi_debug_noise", "mppi_get_info", "mppi_launch_count",
-           "mppi_error_string", "mppi_last_error", "mppi_measure_fma_peak", "mppi_measure_copy_bw"]
+           "mppi_error_string", "mppi_last_error", "mppi_measure_fma_peak", "mppi_measure_copy_bw", "mppi_measure_issue_rates", "mppi_measure_launch_floor"]
 
 
 class MppiParams(C.Structure):
@@ -84,6 +84,8 @@ def _load():
     L.mppi_last_error.restype = C.c_char_p
     L.mppi_measure_fma_peak.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.mppi_measure_copy_bw.argtypes = [C.c_int64, C.c_int, C.POINTER(C.c_double)]
+    L.mppi_measure_issue_rates.argtypes = [C.POINTER(C.c_double), C.c_int]
+    L.mppi_measure_launch_floor.argtypes = [C.c_int, C.POINTER(C.c_double)]
     for name in EXPORTS:
         getattr(L, name)            # AttributeError here = the library is stale: rebuild it
     return L
@@ -367,3 +369,24 @@ def measure_copy_bw(nbytes=1 << 30, reps=5):
     if rc:
         raise MppiError(rc)
     return g.value
+
+
+ISSUE_RATE_CLASSES = ("ffma_rrr", "ffma_const", "ffma2_rrr", "fmul", "fadd", "philox_half_round", "mufu", "fmnmx")
+
+
+def measure_issue_rates() -> dict:
+    """cycles per warp-instruction per SM sub-partition at saturation, by instruction class (mppi_measure_issue_rates)."""
+    a = (C.c_double * len(ISSUE_RATE_CLASSES))()
+    rc = lib.mppi_measure_issue_rates(a, len(ISSUE_RATE_CLASSES))
+    if rc:
+        raise MppiError(rc)
+    return dict(zip(ISSUE_RATE_CLASSES, (float(v) for v in a)))
+
+
+def measure_launch_floor(reps=400) -> float:
+    """median event-to-event time of an empty 128 x 256 kernel behind a busy GPU, microseconds."""
+    v = C.c_double()
+    rc = lib.mppi_measure_launch_floor(int(reps), C.byref(v))
+    if rc:
+        raise MppiError(rc)
+    return v.value
