@@ -50,7 +50,8 @@ typedef struct {
     double Qp, Qv, Qq, Qw, R;
     double q_contour, q_lag, mu_progress;
     int32_t window;
-    int32_t pad_;
+    int32_t near_mode;       /* eq.(7): which gate the near term measures against: 0 = the step's own target [R-24],
+                                1 = the horizon's start gate p0_gate, before and after the switch [R-40]        */
     double q_near, r_near;   /* eq.(7): weight and threshold radius [R-24] */
     /* the paper's own input model, PAPER.md:72 and Table I */
     int32_t input_model;     /* 0: rotor thrusts are the inputs (configs); 1: u = dT/dt, thrusts are states */
@@ -338,9 +339,19 @@ double orc_gate_paper_step(const orc_params* P, const orc_track* trk, const doub
     const double d2_prev = dot3(r_prev, r_prev), d2 = dot3(r, r);
 
     double J = d2 - d2_prev;                                     /* eq.(6) */
-    const double d_prev = sqrt(d2_prev);
-    if (d_prev < P->r_near) J += P->q_near * d2_prev;            /* eq.(7) */
-    if (margin && fabs(d_prev - P->r_near) < *margin) *margin = fabs(d_prev - P->r_near);
+    /* eq.(7), on the pre-step state p_k.  near_mode 0 [R-24]: against the step's own target gate.
+     * near_mode 1 [R-40]: "prevent states near the current gate p0_gate ... from deviating too much from it" read
+     * literally -- against the horizon's START gate gate0, also for the states that already target the next gate */
+    double dn2 = d2_prev;
+    if (P->near_mode == 1 && *gate != gate0) {
+        const double* c0 = trk->gates + 11 * gate0;
+        double r0[3];
+        for (int i = 0; i < 3; ++i) r0[i] = p_prev[i] - c0[i];
+        dn2 = dot3(r0, r0);
+    }
+    const double d_near = sqrt(dn2);
+    if (d_near < P->r_near) J += P->q_near * dn2;
+    if (margin && fabs(d_near - P->r_near) < *margin) *margin = fabs(d_near - P->r_near);
 
     const double s_prev = dot3(n, r_prev), s = dot3(n, r);
     if (margin) {

@@ -41,7 +41,7 @@ class _Params(C.Structure):
                 ("gate_miss_penalty", C.c_double), ("gate_pass_bonus", C.c_double),
                 ("Qp", C.c_double), ("Qv", C.c_double), ("Qq", C.c_double), ("Qw", C.c_double),
                 ("R", C.c_double), ("q_contour", C.c_double), ("q_lag", C.c_double),
-                ("mu_progress", C.c_double), ("window", C.c_int32), ("pad_", C.c_int32),
+                ("mu_progress", C.c_double), ("window", C.c_int32), ("near_mode", C.c_int32),
                 ("q_near", C.c_double), ("r_near", C.c_double),
                 ("input_model", C.c_int32), ("pad2_", C.c_int32), ("rate_max", C.c_double),
                 ("drag_x", C.c_double), ("drag_y", C.c_double), ("drag_z", C.c_double),
@@ -58,7 +58,7 @@ class _Track(C.Structure):
 
 
 _PARAM_KEYS = [f for f, _ in _Params._fields_ if f not in ("pad_", "pad2_")]
-_OPTIONAL = {"q_near": 0.0, "r_near": 0.0, "input_model": 0, "rate_max": 0.0, "drag_x": 0.0, "drag_y": 0.0,
+_OPTIONAL = {"near_mode": 0, "q_near": 0.0, "r_near": 0.0, "input_model": 0, "rate_max": 0.0, "drag_x": 0.0, "drag_y": 0.0,
              "drag_z": 0.0, "w_limit": 0.0, "omega_max": 0.0, "sigma_v": 0.0, "dv_max": 0.0, "v_theta_max": 0.0,
              "r_dv": 0.0}
 _dp = C.POINTER(C.c_double)
@@ -155,7 +155,7 @@ def make_params(p: dict) -> _Params:
             else:
                 raise KeyError(f"oracle params: missing '{k}'")
         v = src[k]
-        setattr(s, k, int(v) if k in ("K", "N", "B", "objective", "window", "input_model") else float(v))
+        setattr(s, k, int(v) if k in ("K", "N", "B", "objective", "window", "input_model", "near_mode") else float(v))
     return s
 
 

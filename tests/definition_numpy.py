@@ -203,8 +203,9 @@ def rollout_cost(P, trk, x0, start, u_nom, seed, it, k, b):
             c, n, h, aw, ah = g[0:3], g[3:6], g[6:9], g[9], g[10]
             a, bpt = xs[t][0:3], xs[t + 1][0:3]
             J += np.sum((bpt - c) ** 2) - np.sum((a - c) ** 2)
-            if np.linalg.norm(a - c) < P["r_near"]:
-                J += P["q_near"] * np.sum((a - c) ** 2)
+            cn = gates[g0][0:3] if P.get("near_mode", 0) == 1 else c        # eq.(7): start gate of the horizon, or own target
+            if np.linalg.norm(a - cn) < P["r_near"]:
+                J += P["q_near"] * np.sum((a - cn) ** 2)
             J += P["w_omega"] * np.sum(xs[t + 1][10:13] ** 2)
             sa, sb = n @ (a - c), n @ (bpt - c)
             if sa < 0 <= sb:

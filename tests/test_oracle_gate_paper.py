@@ -144,3 +144,50 @@ def test_stress_case_exercises_registered_and_ignored_passes():
     assert reg.sum() >= 20 and (geo & ~reg).sum() >= 20          # some passes registered, some ignored
     assert not (reg & ~geo).any()                               # the flags can only remove passes
     assert (wl.prev_front == 0).any() and (wl.prev_front == 1).any()
+
+
+# ---- the second reading of eq.(7)'s near term [R-40] (near_mode = 1): "prevent states near the current
+# gate p0_gate ... from deviating too much from it" -- the distance is to the horizon's START gate, also after the
+# target has switched to the next one.
+
+def test_near_term_against_the_start_gate_after_the_switch(P):
+    trk = O.Track(gates=two_gates())                  # gate 0 at the origin, gate 1 at x = 10, normals +x
+    P1 = dict(P, near_mode=1)
+    # a state 0.5 m BEHIND gate 0 that already targets gate 1 (g = 1, g0 = 0): its own target is 9.5 m away
+    a, b = (0.5, 0.25, 0.0), (1.0, 0.25, 0.0)
+    prog = ((1.0 - 10.0) ** 2 + 0.0625) - ((0.5 - 10.0) ** 2 + 0.0625)         # eq.(6) against gate 1
+    J0, *_ = seg(P, trk, a, b, g=1, g0=0)
+    J1, *_ = seg(P1, trk, a, b, g=1, g0=0)
+    assert J0 == pytest.approx(prog, abs=1e-12)                               # [R-24]: the term is dead here
+    assert J1 == pytest.approx(prog + 2.0 * (0.25 + 0.0625), abs=1e-12)       # [R-40]: Q_near |p_k - c_0|^2
+    # before the switch (g = g0) the two readings are the same number
+    for a2, b2 in (((-1.0, 0.5, 0), (-0.5, 0.5, 0)), ((-5, 0, 0), (-4, 0, 0))):
+        assert seg(P, trk, a2, b2)[0] == seg(P1, trk, a2, b2)[0]
+    # beyond r_near of the START gate nothing is added, however close the own target is
+    J1, *_ = seg(P1, trk, (9.0, 0, 0), (9.5, 0, 0), g=1, g0=0)
+    assert J1 == pytest.approx(0.25 - 1.0, abs=1e-12)
+    J0, *_ = seg(P, trk, (9.0, 0, 0), (9.5, 0, 0), g=1, g0=0)
+    assert J0 == pytest.approx(0.25 - 1.0 + 2.0 * 1.0, abs=1e-12)             # [R-24] measures against gate 1 there
+    # the margin follows the gate the term is measured against: | |p_k - c_0| - r_near |
+    *_, mg, _ = O.gate_paper_step(P1, trk, (1.4, 0, 0), (1.6, 0, 0), (0, 0, 0), 1, 0, 1)
+    assert mg == pytest.approx(0.1, abs=1e-12)
+    # the step that registers the pass of gate 0 still measures its pre-step state against gate 0 in both readings
+    Ja, ga, *_ = seg(P, trk, (-0.5, 0, 0), (0.5, 0, 0))
+    Jb, gb, *_ = seg(P1, trk, (-0.5, 0, 0), (0.5, 0, 0))
+    assert ga == gb == 1 and Ja == Jb
+
+
+@pytest.mark.parametrize("name,kw", [("gate_paper", dict(K=4, N=25)), ("stress_gate_paper", dict(K=24, N=30))])
+def test_brute_force_definition_near_mode_1(name, kw):
+    wl = W.ALL[name](**kw)
+    wl.params["near_mode"] = 1
+    trk = O.Track(gates=wl.gates, prev_front=wl.prev_front)
+    r = O.step(wl.params, trk, wl.x0, wl.start, wl.u_nom, 11, 3)
+    J, w, un, du = D.mppi_step(wl.params, _as_dict_track(wl), wl.x0[0].astype(np.float64),
+                               int(wl.start[0]), wl.u_nom[0].astype(np.float64), 11, 3)
+    np.testing.assert_allclose(r["cost"][0], J, rtol=1e-12, atol=1e-11)
+    r0 = O.step(dict(wl.params, near_mode=0), trk, wl.x0, wl.start, wl.u_nom, 11, 3)
+    if name == "stress_gate_paper":                 # passes happen: the two readings really differ on those samples
+        passed = r["ncross"][0] > 0
+        assert passed.any() and (np.abs(r["cost"][0] - r0["cost"][0])[passed] > 1e-6).any()
+        assert np.array_equal(r["cost"][0][~passed], r0["cost"][0][~passed])
