@@ -161,6 +161,11 @@ typedef struct {
     float r_dv;          /* weight of |Delta v_theta|^2 in eq.(9), >= 0                                  */
     float w_limit, omega_max; /* input_model = 1: soft body-rate limit ("external cost"):
                           + w_limit sum_i max(0, |omega_i| - omega_max)^2 on every post-step state */
+    int32_t near_mode;   /* MPPI_OBJ_GATE_PAPER, eq.(7): the gate whose centre the near term measures
+                          against.  0: the target gate of the step (a state that already targets the next gate is far
+                          from it, so the term ends with the switch).  1: the horizon's START gate p0_gate, before and
+                          after the switch ("prevent states near the current gate p0_gate ... from deviating too much
+                          from it", read literally).  DESIGN.md readings R-24 / R-40                       */
 } mppi_params;
 
 #define MPPI_MAX_N 256

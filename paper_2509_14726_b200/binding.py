@@ -40,7 +40,7 @@ class MppiParams(C.Structure):
                 ("r_near", C.c_float), ("input_model", C.c_int32), ("rate_max", C.c_float),
                 ("drag_x", C.c_float), ("drag_y", C.c_float), ("drag_z", C.c_float),
                 ("sigma_v", C.c_float), ("dv_max", C.c_float), ("v_theta_max", C.c_float), ("r_dv", C.c_float),
-                ("w_limit", C.c_float), ("omega_max", C.c_float)]
+                ("w_limit", C.c_float), ("omega_max", C.c_float), ("near_mode", C.c_int32)]
 
 
 class MppiInfo(C.Structure):

@@ -111,6 +111,7 @@ extern "C" int mppi_default_params(mppi_params* p)
     p->input_model = 0; p->rate_max = 0.0f; p->drag_x = p->drag_y = p->drag_z = 0.0f;
     p->w_limit = 0.0f; p->omega_max = 0.0f;
     p->sigma_v = 0.0f; p->dv_max = 0.0f; p->v_theta_max = 0.0f; p->r_dv = 0.0f;
+    p->near_mode = 0;
     return MPPI_OK;
 }
 
@@ -132,6 +133,7 @@ static int validate(const mppi_params* p)
     }
     BAD(!(std::isfinite(p->q_near) && p->q_near >= 0.0f) || !(std::isfinite(p->r_near) && p->r_near >= 0.0f),
         "q_near and r_near must be >= 0");
+    BAD(p->near_mode != 0 && p->near_mode != 1, "near_mode must be 0 or 1");
     BAD(!finite_pos(p->dt), "dt must be > 0");
     BAD(!finite_pos(p->lambda), "lambda must be > 0");
     BAD(!(std::isfinite(p->sigma) && p->sigma >= 0.0f), "sigma must be >= 0");
@@ -333,7 +335,7 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     d.gyy = (float)(((double)p->Jz - p->Jx) / p->Jy);
     d.gyz = (float)(((double)p->Jx - p->Jy) / p->Jz);
     d.w_omega = p->w_omega; d.miss = p->gate_miss_penalty; d.bonus = p->gate_pass_bonus;
-    d.q_near = p->q_near; d.r_near2 = (float)((double)p->r_near * (double)p->r_near);
+    d.q_near = p->q_near; d.r_near2 = (float)((double)p->r_near * (double)p->r_near); d.near_mode = p->near_mode;
     d.input_model = p->input_model; d.rate_max = p->rate_max;
     d.drag_x = p->drag_x; d.drag_y = p->drag_y; d.drag_z = p->drag_z;
     d.drag4_x = 4.0f * p->drag_x; d.drag4_y = 4.0f * p->drag_y; d.drag4_z = 4.0f * p->drag_z;

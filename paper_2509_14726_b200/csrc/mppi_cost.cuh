@@ -124,7 +124,15 @@ struct GatePaperCost {
     __device__ __forceinline__ void step(const DevParams& P, const float4* s_gates, const int* s_front,
                                          const State& x, int t)
     {
-        if (d2_prev < P.r_near2) J = fmaf(P.q_near, d2_prev, J);          // eq.(7), pre-step state
+        // eq.(7) on the pre-step state p_t: against the step's own target [R-24], or (near_mode 1, [R-40]) against
+        // the horizon's start gate also once the target has moved on
+        float dn2 = d2_prev;
+        if (P.near_mode == 1 && gate != gate0) {
+            const float4 c0 = s_gates[4 * gate0];
+            const float ux = ppx - c0.x, uy = ppy - c0.y, uz = ppz - c0.z;
+            dn2 = fmaf(uz, uz, fmaf(uy, uy, ux * ux));
+        }
+        if (dn2 < P.r_near2) J = fmaf(P.q_near, dn2, J);
         const float4 c = s_gates[4 * gate], n = s_gates[4 * gate + 1];
         const float ax = x.px - c.x, ay = x.py - c.y, az = x.pz - c.z;
         const float d2 = fmaf(az, az, fmaf(ay, ay, ax * ax));

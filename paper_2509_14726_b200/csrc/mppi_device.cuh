@@ -24,6 +24,7 @@ struct DevParams {
     float gyx, gyy, gyz;               // (Jy-Jz)/Jx, (Jz-Jx)/Jy, (Jx-Jy)/Jz   (omega x J omega)
     float w_omega, miss, bonus;        // gate objective constants (BASELINE.json configs[0])
     float q_near, r_near2;             // eq.(7): weight, threshold radius squared [R-24]
+    int near_mode;                     // 0: against the step's own target [R-24]; 1: against the horizon's start gate [R-40]
     // the paper's own input model (Table I) [R-27]..[R-32]: u = dT/dt, thrusts are states
     int input_model;
     float rate_max, drag_x, drag_y, drag_z, w_limit, omega_max;

@@ -31,11 +31,11 @@ def base_params(**over) -> dict:
              gate_pass_bonus=5.0, Qp=100.0, Qv=1.0, Qq=10.0, Qw=0.1, R=0.01, q_contour=200.0,
              q_lag=50.0, mu_progress=2.0, window=16, q_near=0.0, r_near=0.0,
              input_model=0, rate_max=0.0, drag_x=0.0, drag_y=0.0, drag_z=0.0, w_limit=0.0, omega_max=0.0,
-             sigma_v=0.0, dv_max=0.0, v_theta_max=0.0, r_dv=0.0)
+             sigma_v=0.0, dv_max=0.0, v_theta_max=0.0, r_dv=0.0, near_mode=0)
     p["lambda"] = 1.0
     p.update(over)
     for k, v in p.items():
-        if k not in ("K", "N", "B", "objective", "window", "input_model"):
+        if k not in ("K", "N", "B", "objective", "window", "input_model", "near_mode"):
             p[k] = _f32(v)
     return p
 

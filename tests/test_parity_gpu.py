@@ -536,14 +536,38 @@ def test_gate_paper_temporal_check_at_scale(pipe):
     assert (np.abs(g_all["cost"] - g["cost"]) > 1.0).mean() > 0.1
 
 
-def test_front_flags_and_closed_loop_feed():
+@pytest.mark.parametrize("pipe", PIPES, ids=PIPE_IDS)
+def test_gate_paper_near_mode_1(pipe):
+    # eq.(7)'s near term measured against the horizon's START gate, before and after the switch [R-40]: the
+    # crossing-heavy case (two thirds of the samples pass gate 0 and then sit within r_near BEHIND it) through
+    # every kernel; the two readings must really differ on the samples that pass
+    wl = W.stress_gate_paper(K=4096, N=30)
+    wl.params["near_mode"] = 1
+    g, o, st = run_case(wl, f"stress_paper near_mode 1 [{pipe}]", **pipe)
+    o0 = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, wl.seed, 0, params=dict(wl.params, near_mode=0))
+    passed = o["ncross"][0] > 0
+    assert passed.mean() > 0.1 and (np.abs(o["cost"][0] - o0["cost"][0])[passed] > 1e-3).mean() > 0.5
+
+
+@pytest.mark.parametrize("pipe", [dict(pipeline=0, variant=4), dict(pipeline=0, variant=1), dict(pipeline=0, variant=3), dict(pipeline=1)],
+                         ids=["fused_pipe", "fused", "fused_pk", "two_pass"])
+def test_gate_paper_near_mode_1_rate_model(pipe):
+    wl = W._rate_model(W.stress_gate_paper(K=2048, N=30), "rate_stress_paper_near1", sigma=np.float32(12.0), rate_max=np.float32(20.0))
+    wl.params["near_mode"] = 1
+    g, o, st = run_case(wl, f"rate stress_paper near_mode 1 [{pipe}]", **pipe)
+    o0 = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, wl.seed, 0, params=dict(wl.params, near_mode=0))
+    assert (np.abs(o["cost"][0] - o0["cost"][0]) > 1e-3).mean() > 0.1
+
+
+@pytest.mark.parametrize("near_mode", [0, 1])
+def test_front_flags_and_closed_loop_feed(near_mode):
     # the flags of the new nominal feed the next control iteration (shifted by the one control step
     # that elapsed); every iteration is compared with the oracle, teacher-forced [R-17]
     import torch
     from oracle import oracle as O
     B, K, N = 4, 1024, 30
     wl = W.stress_gate_paper(K=K, N=N)
-    p = dict(wl.params, B=B)
+    p = dict(wl.params, B=B, near_mode=near_mode)
     rng = np.random.default_rng(2)
     x0 = np.repeat(wl.x0, B, 0); x0[:, 0:3] += rng.uniform(-0.2, 0.2, (B, 3)).astype(np.float32)
     from paper_2509_14726_b200 import binding as Bd
@@ -561,7 +585,7 @@ def test_front_flags_and_closed_loop_feed():
         o = O.step(p, trk, x_in, s_in, u_in, 7, step, want_du=True)
         o["u_nom"] = u_in.astype(np.float64)
         gdict = dict(u_new=u_new.cpu().numpy(), cost=cost.cpu().numpy(), weights=w.cpu().numpy())
-        Pz.compare(f"paper loop step{step}", gdict, o, p["lambda"], True)
+        Pz.compare(f"paper loop near_mode {near_mode} step{step}", gdict, o, p["lambda"], True)
         # flags of the new nominal from the current state, against the oracle's
         f = m.front_flags(x, start, u_new); torch.cuda.synchronize()
         fg = f.cpu().numpy()
