@@ -161,3 +161,66 @@ def contour_rms(log: FlightLog, path: np.ndarray) -> np.ndarray:
         dist2 = ((p[:, None, :] - q) ** 2).sum(-1).min(1)
         out.append(np.sqrt(dist2.mean()))
     return np.array(out)
+
+
+# ---- the experiment as a command: python -m paper_2509_14726_b200.closed_loop [--track circle|figure8] ---------------
+
+def run_table(track: str = "circle", B: int = 8, K: int = 4096, laps: int = 3, horizon_s: float = 40.0):
+    """Flies every objective on one synthetic track and prints the rows of DESIGN.md section 10's table (markdown).
+    Not comparable with the paper's Table II: its tracks and references are not available."""
+    import time
+    import torch
+    from . import binding as Bd
+    from . import workloads as W
+    rows = [("gate", 1), ("gate", 2), ("gate_paper", 1), ("gate_paper", 2), ("contour", 1), ("contour_paper", 1), ("contour_paper", 2)]
+    if track == "circle":
+        rows.insert(4, ("track", 1))
+    print(f"| track | objective | iterations / control step | GPU time / control step | drones finishing {laps} laps in {horizon_s:.0f} s | "
+          "flight time (s) | waypoint distance mean / max (m) | mean / top speed (m/s) | other |")
+    print("|---|---|---|---|---|---|---|---|---|")
+    for kind, iters in rows:
+        wl = W.lap(kind, B=B, K=K, track=track)
+        steps = int(round(horizon_s / wl.params["dt"]))
+        if kind == "track":
+            wl = W.lap(kind, B=B, K=K, steps=steps, track=track)
+        m = Bd.Mppi(wl.params)
+        m.set_track(wl)
+        fly(m, wl, 20, iters_per_step=iters, prev_front_feedback=(kind == "gate_paper"))          # warm-up
+        torch.cuda.synchronize(); t0 = time.perf_counter()
+        log = fly(m, wl, steps, iters_per_step=iters, prev_front_feedback=(kind == "gate_paper"))
+        us = (time.perf_counter() - t0) / steps * 1e6
+        m.close()
+        if kind in ("gate", "gate_paper"):
+            mt = lap_metrics(log, wl.gates, laps=laps)
+            done = [q for q in mt if q["flight_time_s"] is not None]
+            ft = f"{min(q['flight_time_s'] for q in done):.1f} - {max(q['flight_time_s'] for q in done):.1f}" if done else "-"
+            wp = (f"{np.mean([q['wp_dist_mean'] for q in done]):.2f} / {max(q['wp_dist_max'] for q in done):.2f}" if done else "-")
+            sp = f"{np.mean([q['speed_mean'] for q in mt]):.1f} / {max(q['speed_max'] for q in mt):.1f}"
+            print(f"| {track} | {kind} | {iters} | {us:.0f} us | {len(done)} / {B} | {ft} | {wp} | {sp} | passes {min(q['passes'] for q in mt)} - {max(q['passes'] for q in mt)} |", flush=True)
+        elif kind == "track":
+            e = tracking_rmse(log, wl.ref)
+            print(f"| {track} | tracking (Lissajous reference) | {iters} | {us:.0f} us | - | - | - | - | position RMSE {e.min():.2f} - {e.max():.2f} m |", flush=True)
+        elif kind == "contour":
+            e = contour_rms(log, wl.path)
+            sp = np.linalg.norm(log.x[:, :, 7:10].astype(np.float64), axis=-1)
+            print(f"| {track} | contouring (search) | {iters} | {us:.0f} us | - | - | - | {sp.mean():.1f} / {sp.max():.1f} | contour RMS {e.min():.2f} - {e.max():.2f} m |", flush=True)
+        else:
+            pm = progress_metrics(log, wl.path)
+            e = contour_rms(log, wl.path)
+            done = [q for q in pm if len(q["lap_times_s"]) >= laps]
+            ft = f"{min(q['lap_times_s'][laps - 1] for q in done):.1f} - {max(q['lap_times_s'][laps - 1] for q in done):.1f}" if done else "-"
+            print(f"| {track} | the paper's contouring, eq.(9) | {iters} | {us:.0f} us | {len(done)} / {B} (laps of theta) | {ft} | - | "
+                  f"{np.mean([q['speed_mean'] for q in pm]):.1f} / {max(q['speed_max'] for q in pm):.1f} | contour RMS {e.min():.2f} - {e.max():.2f} m; "
+                  f"vehicle <= {max(q['dist_to_progress_point_max'] for q in pm):.2f} m from P(theta); laps {min(q['laps'] for q in pm):.1f} - {max(q['laps'] for q in pm):.1f} |", flush=True)
+
+
+if __name__ == "__main__":
+    import argparse
+    ap = argparse.ArgumentParser(description="closed-loop lap experiment on the synthetic tracks (DESIGN.md section 10)")
+    ap.add_argument("--track", default="circle", choices=["circle", "figure8"])
+    ap.add_argument("--drones", type=int, default=8)
+    ap.add_argument("--samples", type=int, default=4096)
+    ap.add_argument("--laps", type=int, default=3)
+    ap.add_argument("--seconds", type=float, default=40.0)
+    a = ap.parse_args()
+    run_table(a.track, a.drones, a.samples, a.laps, a.seconds)

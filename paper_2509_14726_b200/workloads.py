@@ -307,31 +307,59 @@ def contour_paper(K=4096, N=50) -> Workload:
     return wl
 
 
-def lap(kind="gate", B=8, K=4096, N=50, steps=1500) -> Workload:
+def figure8_start(B, rng, jitter=0.2):
+    """B jittered start states 3 m before gate 0 of the configs[1] lemniscate, flying at 3 m/s towards it [R-16]."""
+    gates = lemniscate_gates()
+    c0 = gates[0, 0:3].astype(np.float64); n0 = gates[0, 3:6].astype(np.float64)
+    x0 = np.tile(_level_state(c0 - 3.0 * n0, 3.0 * n0), (B, 1))
+    x0[:, 0:3] += rng.uniform(-jitter, jitter, (B, 3))
+    return gates, x0.astype(np.float32)
+
+
+def lap(kind="gate", B=8, K=4096, N=50, steps=1500, track="circle") -> Workload:
     """Closed-loop lap experiment (shaped like Table II) on the 4-gate
-    circle of configs[0] / its spline path / the Lissajous reference, B jittered drones.  The noise and
+    circle of configs[0] / its spline path / the Lissajous reference, or (track = "figure8": the stand-in for
+    the paper's Figure-8 track) on the 7-gate lemniscate of configs[1] with gate heights 1-3 m / the
+    spline path through its gate centres; B jittered drones.  The noise and
     temperature are the ones a controller can actually fly with -- sigma 0.5 N, lambda 0.02, w_omega
     0.001: under configs[4]'s sigma 1.5 / lambda 0.5 the closed loop does not stay in the air (measured)."""
     rng = np.random.default_rng(7)
     tune = dict(sigma=_f32(0.5), w_omega=_f32(0.001))
+    if track not in ("circle", "figure8"):
+        raise ValueError("track must be 'circle' or 'figure8'")
+    if kind in ("track",) and track != "circle":
+        raise ValueError("the tracking lap flies the Lissajous reference: track = 'circle' only")
     if kind in ("gate", "gate_paper"):
         wl = cfg4(K=K, N=N, B=B, steps=steps)
+        if track == "figure8":
+            wl.gates, wl.x0 = figure8_start(B, rng)
         p = dict(wl.params, **tune)
         if kind == "gate_paper":
             p.update(objective=OBJ_GATE_PAPER, gate_pass_bonus=0.0, gate_miss_penalty=0.0, q_near=_f32(0.5), r_near=_f32(1.5))
         p["lambda"] = _f32(0.5 if kind == "gate_paper" else 0.02)      # squared distances: larger cost scale
-        return Workload(f"lap_{kind}_B{B}", p, wl.x0, wl.start, wl.u_nom, gates=wl.gates, seed=0, iters=steps)
+        return Workload(f"lap_{kind}_{track}_B{B}", p, wl.x0, wl.start, wl.u_nom, gates=wl.gates, seed=0, iters=steps)
     if kind == "contour_paper":
         # the paper's own contouring under the paper's model; tuned like the other lap workloads so that it flies
         base = contour_paper(K=K, N=N)
+        if track == "figure8":                 # spline path through the lemniscate's gate centres, start on it
+            gates, x13 = figure8_start(1, np.random.default_rng(0), 0.0)
+            base.path = spline_path(gates[:, 0:3], 500)
+            pts = base.path.astype(np.float64)
+            s = np.concatenate([[0.0], np.cumsum(np.linalg.norm(np.diff(pts, axis=0), axis=1))])
+            i = int(np.argmin(np.sum((pts - x13[0, 0:3].astype(np.float64)) ** 2, axis=1)))
+            base.x0 = np.concatenate([x13, base.x0[:, 13:17], np.array([[s[i], 3.0]], np.float32)], axis=1).astype(np.float32)
         p = dict(base.params, B=B, sigma=_f32(3.0), sigma_v=_f32(3.0), w_omega=_f32(0.001), q_contour=_f32(200.0),
                  q_lag=_f32(100.0), mu_progress=_f32(10.0))
         p["lambda"] = _f32(1.0)
         x0 = np.repeat(base.x0, B, 0)
         x0[:, 0:3] += rng.uniform(-0.2, 0.2, (B, 3)).astype(np.float32)
-        return Workload(f"lap_{kind}_B{B}", p, x0.astype(np.float32), np.repeat(base.start, B, 0), np.repeat(base.u_nom, B, 0),
+        return Workload(f"lap_{kind}_{track}_B{B}", p, x0.astype(np.float32), np.repeat(base.start, B, 0), np.repeat(base.u_nom, B, 0),
                         path=base.path, closed=base.closed, v_nom=np.repeat(base.v_nom, B, 0), seed=0, iters=steps)
     base = cfg2(K=K, N=N, extra_rows=steps + 1) if kind == "track" else cfg3(K=K, N=N)
+    if kind == "contour" and track == "figure8":
+        gates, x13 = figure8_start(1, np.random.default_rng(0), 0.0)
+        base.path = spline_path(gates[:, 0:3], 500)
+        base.x0 = x13
     p = dict(base.params, B=B, **tune)
     p["lambda"] = _f32(0.02 if kind == "contour" else 0.5)
     x0 = np.repeat(base.x0, B, 0)

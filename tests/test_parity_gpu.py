@@ -1036,3 +1036,27 @@ def test_lap_experiment_contour_paper():
         assert 3.0 < q["speed_mean"] < 12.0
     assert (CL.contour_rms(log, wl.path) < 0.4).all()
     assert log.x[:, :, 2].min() > 0.5                              # and in the air (the path is at z = 1.5 m)
+
+
+def test_lap_experiment_on_the_figure_eight():
+    # the stand-in for the paper's Figure-8 track: the 7-gate lemniscate of configs[1], gate heights
+    # 1-3 m.  The gate objective must complete a lap through all seven gates in order; the paper's contouring must
+    # carry its progress state once around the spline path through the gate centres, the vehicle staying with it
+    from paper_2509_14726_b200 import closed_loop as CL
+    wl = W.lap("gate", B=4, K=4096, track="figure8")
+    m = Pz.make_ctx(wl)
+    log = CL.fly(m, wl, 700)
+    m.close()
+    assert np.isfinite(log.x).all()
+    for b, q in enumerate(CL.lap_metrics(log, wl.gates, laps=1)):
+        assert q["flight_time_s"] is not None and q["flight_time_s"] < 13.0, (b, q)     # 60 m per lap
+        assert q["wp_dist_max"] <= np.hypot(0.75, 0.75) + 1e-6
+        assert int(log.start[-1, b]) == q["passes"] % wl.gates.shape[0]                 # device counter = float64 replay
+    wl = W.lap("contour_paper", B=4, K=4096, track="figure8")
+    m = Pz.make_ctx(wl)
+    log = CL.fly(m, wl, 700)
+    m.close()
+    for b, q in enumerate(CL.progress_metrics(log, wl.path)):
+        assert q["laps"] > 1.2 and q["dist_to_progress_point_max"] < 2.5, (b, q)
+    assert (CL.contour_rms(log, wl.path) < 0.5).all()
+    assert log.x[:, :, 2].min() > 0.3                                                   # gate heights are 1-3 m
