@@ -25,13 +25,21 @@
  *     gravity (0,0,-g).  Inputs are the four rotor thrusts in newtons.
  *   - All floating-point data is fp32, row-major, densely packed.  "device" pointers are CUDA
  *     device memory owned by the caller (e.g. torch tensors); "host" pointers are ordinary host
- *     memory, copied during the call.  The library never frees or keeps a caller pointer beyond
- *     the call (mppi_step keeps them only until the work it enqueued has run).
+ *     memory, copied during the call.  The library never frees a caller pointer, and keeps one only
+ *     until the work the call enqueued has run -- with three documented exceptions that stay
+ *     registered until replaced: the flags of mppi_set_prev_front and the two columns of
+ *     mppi_set_progress (the caller keeps them alive as long as mppi_step may run).
  *   - Every entry point returns MPPI_OK (0) or a negative mppi_status.  Nothing throws, aborts
  *     or prints.  NaN/Inf in device inputs are not detected; they propagate to the outputs.
+ *     A SAMPLE whose rollout diverges (cost NaN or beyond the fp32 range) is reported with cost
+ *     3.0e38 and gets weight 0; it does not spoil the other samples or u_new.
  *   - A context is not thread-safe; distinct contexts are independent.  All device work is
  *     enqueued on the cudaStream_t passed in (NULL = the legacy default stream) and is
  *     asynchronous with respect to the host unless stated otherwise.
+ *   - A context owns ONE set of scratch buffers (block partials, tickets, staging, the optional dU
+ *     array).  All calls on one context must therefore be stream-ordered: use one stream, or make
+ *     every call wait (event dependency) for the previous call on that context.  Two calls of one
+ *     context in flight on different streams race on that scratch and give wrong results.
  *   - There is no CPU fallback: without a CUDA device mppi_create fails with MPPI_E_CUDA.
  */
 #ifndef MPPI_H_

@@ -740,6 +740,9 @@ int orc_step(const orc_params* P, const orc_track* trk, const double* x0 /*[B][1
             cost[(size_t)b * K + k] =
                 orc_rollout_cost(P, trk, &pa, x0 + (P->objective == ORC_OBJ_CONTOUR_PAPER ? 19 : P->input_model == 1 ? 17 : 13) * b, start[b], un, seed, iter, (uint32_t)k,
                                  (uint32_t)b, du + (size_t)k * N * 4, &mg, &nc, &ae, NULL);
+            /* [R-41] a rollout whose cost is not representable in the fp32 interface (NaN, or beyond 3.0e38: a
+             * diverged sample) counts as cost 3.0e38 -- weight 0 unless every sample diverged (include/mppi.h) */
+            if (!(fabs(cost[(size_t)b * K + k]) <= 3.0e38)) cost[(size_t)b * K + k] = 3.0e38;
             if (margin) margin[(size_t)b * K + k] = mg;
             if (ncross) ncross[(size_t)b * K + k] = nc;
             if (aux_end) aux_end[(size_t)b * K + k] = ae;

@@ -260,6 +260,14 @@ __device__ __forceinline__ void rk4_step(const DevParams& P, State& x, const flo
     x.qw = nw * inv; x.qx = nx * inv; x.qy = ny * inv; x.qz = nz * inv;
 }
 
+// A rollout whose cost is not representable in fp32 -- NaN, or beyond the range: a diverged sample (large noise on a
+// long horizon, Inf - Inf inside the dynamics) -- counts as cost kCostCap: weight exactly 0 unless every sample of
+// the controller diverged (then they all weigh the same and the update stays finite).  Without this one such sample
+// poisons the controller: fminf drops the NaN from the minimum, exp(m - NaN) puts it into Z and from there into every
+// weight and every entry of u_new.  [R-41]; the oracle applies the same cap.
+constexpr float kCostCap = 3.0e38f;
+__device__ __forceinline__ float sanitize_cost(const float J) { return fabsf(J) <= kCostCap ? J : kCostCap; }
+
 __device__ __forceinline__ State load_state(const float* __restrict__ x0)
 {
     State x;

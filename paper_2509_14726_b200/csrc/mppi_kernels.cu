@@ -124,6 +124,7 @@ __global__ void __launch_bounds__(MPPI_PK_THREADS, MPPI_PK_MINB) rollout2_kernel
         rollout_cost2<OBJ, MATH, true>(P, A, s_unom, s_trk, splat_state(x0), start, i0, (uint32_t)k0, (uint32_t)b, du_out, Ja, Jb);
     else
         rollout_cost2<OBJ, MATH, false>(P, A, s_unom, s_trk, splat_state(x0), start, i0, (uint32_t)k0, (uint32_t)b, du_out, Ja, Jb);
+    Ja = sanitize_cost(Ja); Jb = sanitize_cost(Jb);
     *reinterpret_cast<float2*>(A.cost + (size_t)b * P.K + k0) = make_float2(Ja, Jb);
 
     if (!FUSED) return;
@@ -175,7 +176,7 @@ __global__ void rollout_kernel(const DevParams P, const StepArgs A)
     const int i0 = OBJ == OBJ_CONTOUR ? contour_start_index(P, s_trk, start, x0, s_red) : 0;
     const bool stored = FUSED ? keeps_du<STORE_DU>(A, b) : STORE_DU;
     DrawThrust<MATH> src{P, A, s_unom, (uint32_t)k, (uint32_t)b, stored ? A.du + (size_t)b * N * P.K + k : nullptr};
-    const float J = rollout_cost<OBJ, MATH>(P, s_trk, x0, start, i0, src);
+    const float J = sanitize_cost(rollout_cost<OBJ, MATH>(P, s_trk, x0, start, i0, src));
     A.cost[(size_t)b * P.K + k] = J;
 
     if (!FUSED) return;
@@ -240,7 +241,7 @@ __global__ void __launch_bounds__(kLatThreads, 2) rollout_lat_kernel(const DevPa
     float J = __int_as_float(0x7f800000);
     if (warp < C) {
         SmemThrust src{s_T + tid, RS};
-        J = rollout_cost<OBJ, MATH>(P, s_trk, x0, start, i0, src);
+        J = sanitize_cost(rollout_cost<OBJ, MATH>(P, s_trk, x0, start, i0, src));
         A.cost[(size_t)b * P.K + kbase + tid] = J;
     }
     const float m = block_min(J, s_red);

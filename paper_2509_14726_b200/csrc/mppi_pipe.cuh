@@ -288,6 +288,7 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
     if (OBJ == OBJ_GATE || OBJ == OBJ_GATE_PAPER) J = fmaf(P.w_omega, jw, jp);   // = finish() with W's sum |omega|^2
     else if (OBJ == OBJ_TRACK) J = (jp + jq) + jw;
     else J = jp + jw;
+    J = sanitize_cost(J);
     if (warp == 0) A.cost[(size_t)b * P.K + kbase + lane] = J;
     const float m = warp_min(J);
     const float e = exp_weight<MATH>((m - J) * P.inv_lambda);

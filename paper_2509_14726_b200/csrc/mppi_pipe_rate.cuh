@@ -347,6 +347,7 @@ __global__ void __launch_bounds__(kPipeRateThreads, SHALLOW ? 2 : 1) rollout_pip
         if (OBJ == OBJ_GATE || OBJ == OBJ_GATE_PAPER) J = fmaf(P.w_omega, jw, jp) + jl;
         else if (OBJ == OBJ_CONTOUR_PAPER) J = (jp + jw) + jl;
         else J = ((jp + jq) + jw) + jl;
+        J = sanitize_cost(J);
         A.cost[(size_t)b * P.K + kbase + lane] = J;
         m = warp_min(J);
         const float e = exp_weight<MATH>((m - J) * P.inv_lambda);

@@ -82,6 +82,7 @@ __global__ void __launch_bounds__(256, 3) rollout_rate_kernel(const DevParams P,
     if (OBJ == OBJ_GATE) J += gc.finish<MATH>(P, s_trk, x);
     if (OBJ == OBJ_GATE_PAPER) J += gp.finish(P);
     if (OBJ == OBJ_TRACK) J += track_state_term(P, s_trk + 4 * N, x);
+    J = sanitize_cost(J);
     A.cost[(size_t)b * P.K + k] = J;
 
     if (!FUSED) return;
@@ -157,6 +158,7 @@ __global__ void __launch_bounds__(128, 3) rollout_rate2_kernel(const DevParams P
         Ja += track_state_term(P, s_trk + 4 * N, lane_state<0>(x));
         Jb += track_state_term(P, s_trk + 4 * N, lane_state<1>(x));
     }
+    Ja = sanitize_cost(Ja); Jb = sanitize_cost(Jb);
     *reinterpret_cast<float2*>(A.cost + (size_t)b * P.K + k0) = make_float2(Ja, Jb);
 
     if (!FUSED) return;

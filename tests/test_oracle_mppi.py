@@ -348,3 +348,31 @@ def test_start_index_is_clamped_or_wrapped_as_the_interface_states():
     Jg = lambda s: O.step(wl.params, trk, wl.x0, [s], wl.u_nom, 1, 0)["cost"]
     np.testing.assert_array_equal(Jg(G + 1), Jg(1)); np.testing.assert_array_equal(Jg(-1), Jg(G - 1))
     assert not np.array_equal(Jg(0), Jg(1))
+
+
+def test_unrepresentable_costs_are_capped_and_get_no_weight():
+    # [R-41] (include/mppi.h conventions): a rollout whose cost is NaN or beyond the fp32 range counts as 3.0e38.
+    # A miss penalty of 3e38 pushes every sample that misses the gate over the cap; the samples that pass keep their
+    # costs and share the whole weight
+    wl = W.stress_gate(K=256, N=30)
+    p = dict(wl.params, gate_miss_penalty=3.0e38)
+    trk = O.Track(gates=wl.gates)
+    r = O.step(p, trk, wl.x0, wl.start, wl.u_nom, wl.seed, 0, want_du=True)
+    r0 = O.step(wl.params, trk, wl.x0, wl.start, wl.u_nom, wl.seed, 0)
+    J, J0 = r["cost"][0], r0["cost"][0]
+    missed = np.abs(J - J0) > 1.0                                  # the samples whose cost holds a miss penalty
+    assert missed.sum() >= 20 and (~missed).sum() >= 20
+    assert (J[missed] == 3.0e38).all() and np.isfinite(J).all()
+    np.testing.assert_array_equal(J[~missed], J0[~missed])
+    w = r["weights"][0]
+    assert (w[missed] == 0.0).all() and w.sum() == pytest.approx(1.0, abs=1e-12)
+    z = np.exp(-(J[~missed] - J[~missed].min()) / p["lambda"])
+    np.testing.assert_allclose(w[~missed], z / z.sum(), rtol=1e-12)
+    # every sample over the cap: all weigh the same, the update is the plain mean of the clamped samples
+    wl2 = W.cfg2(K=32, N=4)
+    p2 = dict(wl2.params, Qp=3.0e38)
+    x0 = wl2.x0.copy(); x0[0, 0] += 10.0
+    r2 = O.step(p2, O.Track(ref=wl2.ref), x0, wl2.start, wl2.u_nom, 1, 0, want_du=True)
+    assert (r2["cost"] == 3.0e38).all()
+    np.testing.assert_allclose(r2["weights"], 1.0 / 32, rtol=1e-12)
+    np.testing.assert_allclose(r2["u_new"][0], wl2.u_nom[0] + r2["du"][0].mean(0), atol=1e-12)

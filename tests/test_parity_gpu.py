@@ -465,6 +465,46 @@ def test_auto_falls_back_when_the_latency_kernels_do_not_fit(case):
         m.close()
 
 
+@pytest.mark.parametrize("pipe", PIPES, ids=PIPE_IDS)
+def test_diverged_samples_get_no_weight(pipe):
+    # [R-41] a sample whose cost is not representable (here: a miss penalty of 3e38 on a third of the samples) is
+    # reported as 3.0e38 and gets weight 0; the others are untouched and the update stays finite
+    wl = W.stress_gate(K=2048, N=30)
+    wl.params["gate_miss_penalty"] = 3.0e38
+    m = Pz.make_ctx(wl, **pipe)
+    x0, start, u = Pz.to_dev(wl)
+    g = Pz.gpu_step(m, x0, start, u, wl.seed, 0)
+    m.close()
+    o = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, wl.seed, 0, want_du=True)
+    capped = o["cost"][0] == 3.0e38
+    assert capped.mean() > 0.1 and (~capped).mean() > 0.1
+    flagged = o["margin"][0] < Pz.MARGIN
+    assert np.isfinite(g["cost"]).all() and np.isfinite(g["u_new"]).all() and np.isfinite(g["weights"]).all()
+    same = (g["cost"][0] == np.float32(3.0e38)) == capped
+    assert same[~flagged].all()
+    assert (g["weights"][0][capped & ~flagged] == 0.0).all()
+    ok = ~capped & ~flagged
+    assert (np.abs(g["cost"][0][ok] - o["cost"][0][ok]) <= 1e-4 * np.maximum(np.abs(o["cost"][0][ok]), 1.0)).all()
+    assert abs(g["weights"].sum() - 1.0) < 2e-5
+    if not flagged.any():
+        assert np.abs(g["u_new"] - o["u_new"]).max() <= Pz.U_ATOL
+
+
+def test_rate_model_divergent_rollouts_stay_finite():
+    # sigma = 60 N/s on the thrust rates: the explicit RK4 itself diverges on the tumbling samples (DESIGN.md section
+    # 10): fp32 costs overflow to Inf and Inf - Inf.  Outputs must stay finite, weights normalised, u_new in range
+    wl = W.rate_stress(K=2048, N=50)
+    wl.params.update(sigma=float(np.float32(60.0)), rate_max=float(np.float32(100.0)))
+    for opts in (dict(variant=1), dict(variant=3), dict(variant=4), dict(pipeline=1)):
+        m = Pz.make_ctx(wl, **opts)
+        x0, start, u = Pz.to_dev(wl)
+        g = Pz.gpu_step(m, x0, start, u, wl.seed, 0)
+        m.close()
+        assert np.isfinite(g["cost"]).all() and np.isfinite(g["weights"]).all() and np.isfinite(g["u_new"]).all(), opts
+        assert abs(g["weights"].sum() - 1.0) < 2e-5 and np.abs(g["u_new"]).max() <= 100.0
+        assert (g["cost"] == np.float32(3.0e38)).any(), "the case is meant to contain diverged samples"
+
+
 def test_seed_high_word_reaches_the_key():
     wl = W.cfg0(K=64, N=5)
     wl.seed = (0xDEADBEEF << 32) | 0x12345678
