@@ -111,8 +111,8 @@ typedef enum {
                                     throughput kernel)                                                      */
     MPPI_VARIANT_PACKED = 3      /* throughput kernel with TWO samples per thread held in packed fp32x2
                                     registers (sm_100a FFMA2); needs K % 64 == 0; costs are bit-identical
-                                    to MPPI_VARIANT_THROUGHPUT.  Under input_model = 1: objectives gate,
-                                    gate_paper and tracking, block_threads <= 128 (else MPPI_E_PARAM); AUTO
+                                    to MPPI_VARIANT_THROUGHPUT.  Under input_model = 1: every objective but the
+                                    search-based contouring, block_threads <= 128 (else MPPI_E_PARAM); AUTO
                                     takes it when B K / 32 >= 8 x the SM count                             */
 } mppi_variant;
 

@@ -166,8 +166,8 @@ static int validate(const mppi_params* p)
                 p->variant != MPPI_VARIANT_PACKED,
             "input_model = 1 has scalar and packed throughput kernels and a pipelined latency kernel: variant must not be LATENCY");
         BAD(p->variant == MPPI_VARIANT_PACKED &&
-                (p->K % 64 != 0 || (p->objective != MPPI_OBJ_GATE && p->objective != MPPI_OBJ_GATE_PAPER && p->objective != MPPI_OBJ_TRACK)),
-            "input_model = 1, PACKED: K % 64 == 0, objective gate / gate_paper / track");
+                (p->K % 64 != 0 || p->objective == MPPI_OBJ_CONTOUR),
+            "input_model = 1, PACKED: K % 64 == 0, not the search-based contouring");
         BAD(p->variant == MPPI_VARIANT_PIPELINED &&
                 (p->pipeline != MPPI_PIPE_FUSED || p->block_threads != 0 || p->N > 100 || p->K % 32 != 0 ||
                  p->objective == MPPI_OBJ_CONTOUR),
@@ -210,7 +210,7 @@ static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, i
     if (p->input_model == 1) {                     // thrust-rate model: its own kernels (mppi_rate.cu)
         // the scalar shape; whether the pipelined latency kernel takes over is decided in prepare(), once the
         // track (and with it the shared-memory footprint) is known -- see rate_pipe_candidate
-        const bool pk_obj = p->objective == MPPI_OBJ_GATE || p->objective == MPPI_OBJ_GATE_PAPER || p->objective == MPPI_OBJ_TRACK;
+        const bool pk_obj = p->objective != MPPI_OBJ_CONTOUR;
         // packed fp32x2 throughput kernel (rollout_rate2_kernel): when the grid covers the chip
         if (pk_obj && p->K % 64 == 0 && (p->variant == MPPI_VARIANT_PACKED ||
                                          (p->variant == MPPI_VARIANT_AUTO && warps >= 8 * (int64_t)sm_count))) {

@@ -337,7 +337,8 @@ __global__ void sim_kernel(const DevParams P, float* __restrict__ xs, int* __res
             if (P.input_model == 1) {
                 const float4 u = make_float4(fminf(fmaxf(T.x, -P.rate_max), P.rate_max), fminf(fmaxf(T.y, -P.rate_max), P.rate_max),
                                              fminf(fmaxf(T.z, -P.rate_max), P.rate_max), fminf(fmaxf(T.w, -P.rate_max), P.rate_max));
-                rk4_rate_step(P, x, Ts, u);
+                ThrustDiff D = thrust_diff(Ts);
+                rk4_rate_step(P, x, Ts, D, u);
             } else {
                 rk4_step(P, x, T);
             }
@@ -405,7 +406,8 @@ __global__ void sim_progress_kernel(const DevParams P, float* __restrict__ xs, c
         const float4 u = make_float4(fminf(fmaxf(T.x, -P.rate_max), P.rate_max), fminf(fmaxf(T.y, -P.rate_max), P.rate_max),
                                      fminf(fmaxf(T.z, -P.rate_max), P.rate_max), fminf(fmaxf(T.w, -P.rate_max), P.rate_max));
         const float dv = fminf(fmaxf(v_new[(size_t)b * N], -P.dv_max), P.dv_max);
-        rk4_rate_step(P, x, Ts, u);
+        ThrustDiff D = thrust_diff(Ts);
+        rk4_rate_step(P, x, Ts, D, u);
         float* o = xb;
         o[0] = x.px; o[1] = x.py; o[2] = x.pz; o[3] = x.qw; o[4] = x.qx; o[5] = x.qy; o[6] = x.qz;
         o[7] = x.vx; o[8] = x.vy; o[9] = x.vz; o[10] = x.ox; o[11] = x.oy; o[12] = x.oz;
@@ -444,6 +446,7 @@ __global__ void front_flags_kernel(const DevParams P, const float* __restrict__ 
     State x = load_state(xb);
     float4 Ts = make_float4(0.f, 0.f, 0.f, 0.f);
     if (P.input_model == 1) Ts = make_float4(xb[13], xb[14], xb[15], xb[16]);
+    ThrustDiff D = thrust_diff(Ts);
     const int g = wrap_index(start[b], P.G);
     const float4 c = P.gates[4 * g], n = P.gates[4 * g + 1];
     const float4* ub = reinterpret_cast<const float4*>(u) + (size_t)b * P.N;
@@ -456,7 +459,7 @@ __global__ void front_flags_kernel(const DevParams P, const float* __restrict__ 
         const float lo = P.input_model == 1 ? -P.rate_max : P.T_min, hi = P.input_model == 1 ? P.rate_max : P.T_max;
         T.x = fminf(fmaxf(T.x, lo), hi); T.y = fminf(fmaxf(T.y, lo), hi);
         T.z = fminf(fmaxf(T.z, lo), hi); T.w = fminf(fmaxf(T.w, lo), hi);
-        if (P.input_model == 1) rk4_rate_step(P, x, Ts, T);
+        if (P.input_model == 1) rk4_rate_step(P, x, Ts, D, T);
         else rk4_step(P, x, T);
     }
 }

@@ -136,6 +136,7 @@ __global__ void __launch_bounds__(kPipeRateThreads, SHALLOW ? 2 : 1) rollout_pip
         // ---- W: thrust states [R-27],[R-29] and body rates.  omega' = J^-1 (tau(T) - omega x J omega) ----
         float ox = x0.ox, oy = x0.oy, oz = x0.oz;
         float4 T = make_float4(xb[13], xb[14], xb[15], xb[16]);
+        ThrustDiff TD = thrust_diff(T);            // the torques' thrust combinations, integrated beside T (mppi_rate.cuh)
         float acc = 0.0f, lim = 0.0f;
         for (int c = 0, s = 0, ph = 0; c < nchunks; ++c, ph ^= (s + 1 == D), s = (s + 1 == D) ? 0 : s + 1) {
             const int cnt = min(C, N - c * C);       // s = c % D, ph = (c / D) & 1, kept as running counters
@@ -156,12 +157,11 @@ __global__ void __launch_bounds__(kPipeRateThreads, SHALLOW ? 2 : 1) rollout_pip
                     acc = fmaf(P.R, fmaf(u.w, u.w, fmaf(u.z, u.z, fmaf(u.y, u.y, u.x * u.x))), acc);
                 }
                 // torque accelerations and collective acceleration are linear in the thrusts: value at T and slope along u
-                const float s01 = T.x + T.y, s23 = T.z + T.w, u01 = u.x + u.y, u23 = u.z + u.w;
-                const float ax = P.ltx * (s01 - s23), bx = P.ltx * (u01 - u23);
-                const float d10 = T.y - T.x, d23 = T.z - T.w, e10 = u.y - u.x, e23 = u.z - u.w;
-                const float ay = P.lty * (d10 + d23), by = P.lty * (e10 + e23);
-                const float az = P.ltz * (d23 - d10), bz = P.ltz * (e23 - e10);
-                const float c0 = (s01 + s23) * P.inv_mass, cu = (u01 + u23) * P.inv_mass;
+                const ThrustDiff du = thrust_diff(u);
+                const float ax = P.ltx * TD.x, bx = P.ltx * du.x;
+                const float ay = P.lty * TD.y, by = P.lty * du.y;
+                const float az = P.ltz * TD.z, bz = P.ltz * du.z;
+                const float c0 = ((T.x + T.y) + (T.z + T.w)) * P.inv_mass, cu = ((u.x + u.y) + (u.z + u.w)) * P.inv_mass;
                 const float amx = fmaf(P.h2, bx, ax), amy = fmaf(P.h2, by, ay), amz = fmaf(P.h2, bz, az);
                 const float aex = fmaf(P.dt, bx, ax), aey = fmaf(P.dt, by, ay), aez = fmaf(P.dt, bz, az);
                 float kx = fmaf(P.gyx, oy * oz, ax), ky = fmaf(P.gyy, oz * ox, ay), kz = fmaf(P.gyz, ox * oy, az);
@@ -180,8 +180,15 @@ __global__ void __launch_bounds__(kPipeRateThreads, SHALLOW ? 2 : 1) rollout_pip
                 w[96] = make_float4(c0, fmaf(P.h2, cu, c0), fmaf(P.dt, cu, c0), 0.0f);
                 kx = fmaf(P.gyx, o4y * o4z, aex); ky = fmaf(P.gyy, o4z * o4x, aey); kz = fmaf(P.gyz, o4x * o4y, aez);
                 ox = fmaf(P.h6, kx, nx); oy = fmaf(P.h6, ky, ny); oz = fmaf(P.h6, kz, nz);
-                T.x = fminf(fmaxf(fmaf(P.dt, u.x, T.x), P.T_min), P.T_max); T.y = fminf(fmaxf(fmaf(P.dt, u.y, T.y), P.T_min), P.T_max);
-                T.z = fminf(fmaxf(fmaf(P.dt, u.z, T.z), P.T_min), P.T_max); T.w = fminf(fmaxf(fmaf(P.dt, u.w, T.w), P.T_min), P.T_max);
+                {   // thrust states: T + h u projected onto their range [R-29]; D follows its own rate unless the projection acted
+                    const float4 Te = make_float4(fmaf(P.dt, u.x, T.x), fmaf(P.dt, u.y, T.y), fmaf(P.dt, u.z, T.z), fmaf(P.dt, u.w, T.w));
+                    T.x = fminf(fmaxf(Te.x, P.T_min), P.T_max); T.y = fminf(fmaxf(Te.y, P.T_min), P.T_max);
+                    T.z = fminf(fmaxf(Te.z, P.T_min), P.T_max); T.w = fminf(fmaxf(Te.w, P.T_min), P.T_max);
+                    const bool moved = T.x != Te.x || T.y != Te.y || T.z != Te.z || T.w != Te.w;
+                    const ThrustDiff Dc = thrust_diff(T);
+                    TD.x = moved ? Dc.x : fmaf(P.dt, du.x, TD.x); TD.y = moved ? Dc.y : fmaf(P.dt, du.y, TD.y);
+                    TD.z = moved ? Dc.z : fmaf(P.dt, du.z, TD.z);
+                }
                 {   // soft body-rate limit on the post-step rates [R-31]
                     const float ex = fmaxf(fabsf(ox) - P.omega_max, 0.0f), ey = fmaxf(fabsf(oy) - P.omega_max, 0.0f),
                                 ez = fmaxf(fabsf(oz) - P.omega_max, 0.0f);

@@ -41,6 +41,7 @@ __global__ void __launch_bounds__(256, 3) rollout_rate_kernel(const DevParams P,
     const float* xb = A.x0 + (OBJ == OBJ_CONTOUR_PAPER ? 19 : 17) * b;   // p, q, v, omega, T(4) [, theta, v_theta]
     State x = load_state(xb);
     float4 T = make_float4(xb[13], xb[14], xb[15], xb[16]);
+    ThrustDiff D = thrust_diff(T);                                       // the torques' thrust combinations (mppi_rate.cuh)
     float theta = 0.0f, v_theta = 0.0f;                                  // OBJ_CONTOUR_PAPER: progress states [R-33]
     if (OBJ == OBJ_CONTOUR_PAPER) { theta = xb[17]; v_theta = xb[18]; }
     const int i0 = OBJ == OBJ_CONTOUR ? contour_start_index(P, s_trk, start, x, s_red) : 0;
@@ -71,7 +72,7 @@ __global__ void __launch_bounds__(256, 3) rollout_rate_kernel(const DevParams P,
             theta = fmaf(P.hh2, dv, fmaf(P.dt, v_theta, theta));
             v_theta = fminf(fmaxf(fmaf(P.dt, dv, v_theta), 0.0f), P.v_theta_max);
         }
-        rk4_rate_step<decltype(axi)::value>(P, x, T, u);
+        rk4_rate_step<decltype(axi)::value>(P, x, T, D, u);
         J += rate_limit_cost(P, x);
         if (OBJ == OBJ_GATE) gc.template step<MATH>(P, s_trk, x);
         if (OBJ == OBJ_GATE_PAPER) gp.step(P, s_trk, s_front, x, t);
@@ -95,7 +96,8 @@ __global__ void __launch_bounds__(256, 3) rollout_rate_kernel(const DevParams P,
 // ---------------------------------------------------------------------------------------------
 // packed throughput variant of the rate model: two samples per thread in fp32x2 registers
 // (mppi_rate.cuh: fdyn_general2 / rk4_rate_step2).  grid = (K / (2 blockDim.x), B); thread j of the grid
-// row owns samples 2j and 2j+1.  Objectives: gate, the paper's J_gate, tracking.
+// row owns samples 2j and 2j+1.  Objectives: gate, the paper's J_gate, tracking, the paper's contouring (eq.(9): theta,
+// v_theta as packed states, the path looked up per half, the fifth input's column in the fused partial).
 // ---------------------------------------------------------------------------------------------
 template <int OBJ, int MATH, bool STORE_DU, bool FUSED>
 __global__ void __launch_bounds__(128, 3) rollout_rate2_kernel(const DevParams P, const StepArgs A)
@@ -111,15 +113,23 @@ __global__ void __launch_bounds__(128, 3) rollout_rate2_kernel(const DevParams P
     float* s_red = reinterpret_cast<float*>(s_trk + track_f4(P, OBJ));   // 64 floats
     float4* s_acc = reinterpret_cast<float4*>(s_red + 64);
     float* s_pair = reinterpret_cast<float*>(s_acc + (blockDim.x >> 5) * N);
+    // OBJ_CONTOUR_PAPER: nominal of the fifth input [N] + one accumulator row per warp, after the pair area
+    float* s_vnom = s_pair + 4 * ((3 * P.blocks_per_ctrl + 3) / 4);
+    float* s_acc5 = s_vnom + N;
 
     const int start = A.start[b];
     stage_inputs<OBJ>(P, A, b, start, s_unom, s_trk);
+    if (OBJ == OBJ_CONTOUR_PAPER)
+        for (int t = tid; t < N; t += blockDim.x) s_vnom[t] = A.v_nom[(size_t)b * N + t];
     __syncthreads();
 
-    const float* xb = A.x0 + 17 * b;
+    const float* xb = A.x0 + (OBJ == OBJ_CONTOUR_PAPER ? 19 : 17) * b;   // p, q, v, omega, T(4) [, theta, v_theta]
     const State x0 = load_state(xb);
     State2 x = splat_state(x0);
     float2 T[4] = { bc2(xb[13]), bc2(xb[14]), bc2(xb[15]), bc2(xb[16]) };
+    ThrustDiff2 D = thrust_diff2(T[0], T[1], T[2], T[3]);
+    float2 theta = bc2(0.0f), v_theta = bc2(0.0f);                       // OBJ_CONTOUR_PAPER: progress states [R-33]
+    if (OBJ == OBJ_CONTOUR_PAPER) { theta = bc2(xb[17]); v_theta = bc2(xb[18]); }
     const float lo = -P.rate_max, hi = P.rate_max;
 
     float Ja = 0.0f, Jb = 0.0f;
@@ -128,7 +138,7 @@ __global__ void __launch_bounds__(128, 3) rollout_rate2_kernel(const DevParams P
     const int* s_front = reinterpret_cast<const int*>(s_trk + 4 * P.G);  // OBJ_GATE_PAPER only
     if (OBJ == OBJ_GATE) { ga.init<MATH>(P, s_trk, start, x0); gb = ga; }
     if (OBJ == OBJ_GATE_PAPER) { pa.init(P, s_trk, start, x0); pb = pa; }
-    const bool stored = FUSED ? keeps_du<STORE_DU>(A, b) : STORE_DU;
+    const bool stored = (FUSED && OBJ != OBJ_CONTOUR_PAPER) ? keeps_du<STORE_DU>(A, b) : STORE_DU;
     float4* du_out = stored ? A.du + (size_t)b * N * P.K + k0 : nullptr;
     auto horizon = [&](auto axi) {         // as in rollout_rate_kernel: axisymmetric drag form / general form
     for (int t = 0; t < N; ++t) {
@@ -143,7 +153,18 @@ __global__ void __launch_bounds__(128, 3) rollout_rate2_kernel(const DevParams P
             Ja += fmaf(P.R, ua.x * ua.x + ua.y * ua.y + ua.z * ua.z + ua.w * ua.w, track_state_term(P, s_trk + 4 * t, lane_state<0>(x)));
             Jb += fmaf(P.R, ub.x * ub.x + ub.y * ub.y + ub.z * ub.z + ub.w * ub.w, track_state_term(P, s_trk + 4 * t, lane_state<1>(x)));
         }
-        rk4_rate_step2<decltype(axi)::value>(P, x, T, ua, ub);
+        if (OBJ == OBJ_CONTOUR_PAPER) {            // fifth sampled input, stage cost, progress states [R-34]..[R-37]
+            const float vn = s_vnom[t];
+            const float dva = sample_progress_accel<MATH>(P, A.rk, (uint32_t)k0, (uint32_t)t, A.iter, (uint32_t)b, vn);
+            const float dvb = sample_progress_accel<MATH>(P, A.rk, (uint32_t)k0 + 1u, (uint32_t)t, A.iter, (uint32_t)b, vn);
+            Ja += contour_paper_stage(P, s_trk, lane_state<0>(x), theta.x, v_theta.x, ua, dva);
+            Jb += contour_paper_stage(P, s_trk, lane_state<1>(x), theta.y, v_theta.y, ub, dvb);
+            theta.x = fmaf(P.hh2, dva, fmaf(P.dt, v_theta.x, theta.x));
+            theta.y = fmaf(P.hh2, dvb, fmaf(P.dt, v_theta.y, theta.y));
+            v_theta.x = fminf(fmaxf(fmaf(P.dt, dva, v_theta.x), 0.0f), P.v_theta_max);
+            v_theta.y = fminf(fmaxf(fmaf(P.dt, dvb, v_theta.y), 0.0f), P.v_theta_max);
+        }
+        rk4_rate_step2<decltype(axi)::value>(P, x, T, D, ua, ub);
         const State xa = lane_state<0>(x), xc = lane_state<1>(x);
         Ja += rate_limit_cost(P, xa);
         Jb += rate_limit_cost(P, xc);
@@ -165,8 +186,12 @@ __global__ void __launch_bounds__(128, 3) rollout_rate2_kernel(const DevParams P
 
     // ---- block-local softmax partial over the block's 2 blockDim.x samples + last-block combine (mppi_rollout.cuh) ----
     const float Jv[2] = {Ja, Jb};
-    block_partial_and_combine_n<MATH, 2>(P, A, b, blockIdx.x, (uint32_t)(2 * blockIdx.x * blockDim.x), Jv, lo, hi, stored,
-                                         s_unom, s_red, s_acc, s_pair);
+    if (OBJ == OBJ_CONTOUR_PAPER)
+        block_partial_and_combine_n<MATH, 2>(P, A, b, blockIdx.x, (uint32_t)(2 * blockIdx.x * blockDim.x), Jv, lo, hi, false,
+                                             s_unom, s_red, s_acc, s_pair, s_vnom, s_acc5);
+    else
+        block_partial_and_combine_n<MATH, 2>(P, A, b, blockIdx.x, (uint32_t)(2 * blockIdx.x * blockDim.x), Jv, lo, hi, stored,
+                                             s_unom, s_red, s_acc, s_pair);
 }
 
 // ---- host-side dispatch ------------------------------------------------------------------------------
@@ -231,6 +256,7 @@ static RateFn pick_rate_packed(const LaunchCfg& c)
     switch (c.objective) {
         case OBJ_GATE: return pick_rate2p1<OBJ_GATE>(c);
         case OBJ_GATE_PAPER: return pick_rate2p1<OBJ_GATE_PAPER>(c);
+        case OBJ_CONTOUR_PAPER: return pick_rate2p1<OBJ_CONTOUR_PAPER>(c);
         default: return pick_rate2p1<OBJ_TRACK>(c);
     }
 }

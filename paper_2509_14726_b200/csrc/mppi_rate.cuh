@@ -22,22 +22,21 @@ struct Deriv { float qw, qx, qy, qz, vx, vy, vz, ox, oy, oz; };     // q slots: 
 //   v' = [2 S / m - 4 (d_z - d_x) (e2 . v)] e2 + (k |u|^2 - d_x) v - k (u . v) u - g z,   k = 4 d_x (1 - n).
 // AXI = 1: stage 1, where q is the step's normalised state (n = 1 to rounding, k dropped): 16 operations;
 // AXI = 2: inner stages with the k terms: 29 operations; general form: 43.
+// ax, ay, az: torque accelerations tau_i / J_i of the stage's thrusts (J^-1 folded in); c = 2 S / m.
 template <int AXI = 0>
 __device__ __forceinline__ Deriv fdyn_general(const DevParams& P, const float qw, const float qx, const float qy,
                                               const float qz, const float vx, const float vy, const float vz,
-                                              const float ox, const float oy, const float oz, const float4 T)
+                                              const float ox, const float oy, const float oz, const float ax,
+                                              const float ay, const float az, const float c)
 {
     Deriv d;
     d.qw = fmaf(-qz, oz, fmaf(-qy, oy, -qx * ox));
     d.qx = fmaf(-qz, oy, fmaf(qy, oz, qw * ox));
     d.qy = fmaf(-qx, oz, fmaf(qz, ox, qw * oy));
     d.qz = fmaf(-qy, ox, fmaf(qx, oy, qw * oz));
-    const float s01 = T.x + T.y, s23 = T.z + T.w;
-    d.ox = fmaf(P.gyx, oy * oz, P.ltx * (s01 - s23));                  // PAPER.md:70, J^-1 folded in
-    const float d10 = T.y - T.x, d23 = T.z - T.w;                      // (T1 + T2) - (T0 + T3) = d10 + d23, (T0 + T2) - (T1 + T3) = d23 - d10
-    d.oy = fmaf(P.gyy, oz * ox, P.lty * (d10 + d23));
-    d.oz = fmaf(P.gyz, ox * oy, P.ltz * (d23 - d10));
-    const float c = (s01 + s23) * P.inv_mass2;                         // 2 S / m
+    d.ox = fmaf(P.gyx, oy * oz, ax);
+    d.oy = fmaf(P.gyy, oz * ox, ay);
+    d.oz = fmaf(P.gyz, ox * oy, az);
     if (AXI) {
         const float e2x = fmaf(qx, qz, qw * qy), e2y = fmaf(qy, qz, -qw * qx), e2z = fmaf(-qy, qy, fmaf(-qx, qx, 0.5f));
         const float w = fmaf(-P.drag_dd4, fmaf(e2z, vz, fmaf(e2y, vy, e2x * vx)), c);
@@ -69,16 +68,39 @@ __device__ __forceinline__ Deriv fdyn_general(const DevParams& P, const float qw
     return d;
 }
 
+// The three thrust combinations the torques of PAPER.md:70 are made of, carried NEXT TO the thrust states:
+//   x = (T0 + T1) - (T2 + T3),  y = (T1 - T0) + (T2 - T3),  z = (T2 - T3) - (T1 - T0).
+// Each rotor thrust sits near hover (~2 N, ulp 2.4e-7) and collects a rounding error every step; the torques are
+// DIFFERENCES of them (~0.1 N), so that error reaches the body rates amplified by lever / J ~ 100: measured at the
+// paper's Table I sizes it is what pushed one cost of 8192 beyond rel 1e-4 through the soft body-rate limit
+// (profiles/README_r02a.md).  The differences themselves obey D' = the same combination of the rates, so integrating
+// them directly keeps their rounding error relative to |D|, ten to twenty times smaller.  They are re-derived from
+// the thrusts only when the projection onto [T_min, T_max] actually moved a thrust [R-29].
+struct ThrustDiff { float x, y, z; };
+__device__ __forceinline__ ThrustDiff thrust_diff(const float4 T)
+{
+    const float s01 = T.x + T.y, s23 = T.z + T.w, d10 = T.y - T.x, d23 = T.z - T.w;
+    return ThrustDiff{s01 - s23, d10 + d23, d23 - d10};
+}
+
 // x <- RK4 on the 17-vector [p, q, v, omega, T] with T' = u held over the step; q renormalised; the
-// thrust states projected onto [T_min, T_max] afterwards [R-27],[R-29].
+// thrust states projected onto [T_min, T_max] afterwards [R-27],[R-29].  D: thrust_diff(T), kept by the caller.
 template <bool AXI = false>      // AXI: drag_x == drag_y (see fdyn_general)
-__device__ __forceinline__ void rk4_rate_step(const DevParams& P, State& x, float4& T, const float4 u)
+__device__ __forceinline__ void rk4_rate_step(const DevParams& P, State& x, float4& T, ThrustDiff& D, const float4 u)
 {
     const float h = P.dt, hh = P.h2, hq = P.h4;                       // hq: the q slots of Deriv hold 2 q'
-    const float4 Tm = make_float4(fmaf(hh, u.x, T.x), fmaf(hh, u.y, T.y), fmaf(hh, u.z, T.z), fmaf(hh, u.w, T.w));
     const float4 Te = make_float4(fmaf(h, u.x, T.x), fmaf(h, u.y, T.y), fmaf(h, u.z, T.z), fmaf(h, u.w, T.w));
+    // torque accelerations and collective acceleration of the three distinct stage thrusts T, T + h/2 u, T + h u:
+    // linear in the thrusts, so the value at T and the slope along u give all of them
+    const ThrustDiff du = thrust_diff(u);
+    const float S = (T.x + T.y) + (T.z + T.w), su = (u.x + u.y) + (u.z + u.w);
+    const ThrustDiff Dm{fmaf(hh, du.x, D.x), fmaf(hh, du.y, D.y), fmaf(hh, du.z, D.z)};
+    const ThrustDiff De{fmaf(h, du.x, D.x), fmaf(h, du.y, D.y), fmaf(h, du.z, D.z)};
+    const float a1x = P.ltx * D.x, a1y = P.lty * D.y, a1z = P.ltz * D.z, c1 = S * P.inv_mass2;
+    const float amx = P.ltx * Dm.x, amy = P.lty * Dm.y, amz = P.ltz * Dm.z, cm = fmaf(hh, su, S) * P.inv_mass2;
+    const float aex = P.ltx * De.x, aey = P.lty * De.y, aez = P.ltz * De.z, ce = fmaf(h, su, S) * P.inv_mass2;
     // stage 1
-    Deriv k = fdyn_general<(AXI ? 1 : 0)>(P, x.qw, x.qx, x.qy, x.qz, x.vx, x.vy, x.vz, x.ox, x.oy, x.oz, T);
+    Deriv k = fdyn_general<(AXI ? 1 : 0)>(P, x.qw, x.qx, x.qy, x.qz, x.vx, x.vy, x.vz, x.ox, x.oy, x.oz, a1x, a1y, a1z, c1);
     float apx = x.vx, apy = x.vy, apz = x.vz;                         // sums of p' = v over the stages
     Deriv a = k;
     float vx = fmaf(hh, k.vx, x.vx), vy = fmaf(hh, k.vy, x.vy), vz = fmaf(hh, k.vz, x.vz);
@@ -90,21 +112,21 @@ __device__ __forceinline__ void rk4_rate_step(const DevParams& P, State& x, floa
     a.ox = fmaf(W, k.ox, a.ox); a.oy = fmaf(W, k.oy, a.oy); a.oz = fmaf(W, k.oz, a.oz);
     // stage 2 (state x + h/2 k1, thrusts T + h/2 u)
     apx = fmaf(2.0f, vx, apx); apy = fmaf(2.0f, vy, apy); apz = fmaf(2.0f, vz, apz);
-    k = fdyn_general<(AXI ? 2 : 0)>(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Tm);
+    k = fdyn_general<(AXI ? 2 : 0)>(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, amx, amy, amz, cm);
     MPPI_ACC(2.0f)
     vx = fmaf(hh, k.vx, x.vx); vy = fmaf(hh, k.vy, x.vy); vz = fmaf(hh, k.vz, x.vz);
     qw = fmaf(hq, k.qw, x.qw); qx = fmaf(hq, k.qx, x.qx); qy = fmaf(hq, k.qy, x.qy); qz = fmaf(hq, k.qz, x.qz);
     ox = fmaf(hh, k.ox, x.ox); oy = fmaf(hh, k.oy, x.oy); oz = fmaf(hh, k.oz, x.oz);
     // stage 3
     apx = fmaf(2.0f, vx, apx); apy = fmaf(2.0f, vy, apy); apz = fmaf(2.0f, vz, apz);
-    k = fdyn_general<(AXI ? 2 : 0)>(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Tm);
+    k = fdyn_general<(AXI ? 2 : 0)>(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, amx, amy, amz, cm);
     MPPI_ACC(2.0f)
     vx = fmaf(h, k.vx, x.vx); vy = fmaf(h, k.vy, x.vy); vz = fmaf(h, k.vz, x.vz);
     qw = fmaf(hh, k.qw, x.qw); qx = fmaf(hh, k.qx, x.qx); qy = fmaf(hh, k.qy, x.qy); qz = fmaf(hh, k.qz, x.qz);
     ox = fmaf(h, k.ox, x.ox); oy = fmaf(h, k.oy, x.oy); oz = fmaf(h, k.oz, x.oz);
     // stage 4 (state x + h k3, thrusts T + h u)
     apx += vx; apy += vy; apz += vz;
-    k = fdyn_general<(AXI ? 2 : 0)>(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Te);
+    k = fdyn_general<(AXI ? 2 : 0)>(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, aex, aey, aez, ce);
     MPPI_ACC(1.0f)
 #undef MPPI_ACC
     const float h6 = P.h6;
@@ -117,6 +139,9 @@ __device__ __forceinline__ void rk4_rate_step(const DevParams& P, State& x, floa
     x.qw = nw * inv; x.qx = nx * inv; x.qy = ny * inv; x.qz = nz * inv;
     T.x = fminf(fmaxf(Te.x, P.T_min), P.T_max); T.y = fminf(fmaxf(Te.y, P.T_min), P.T_max);
     T.z = fminf(fmaxf(Te.z, P.T_min), P.T_max); T.w = fminf(fmaxf(Te.w, P.T_min), P.T_max);
+    const bool moved = T.x != Te.x || T.y != Te.y || T.z != Te.z || T.w != Te.w;     // the projection acted
+    const ThrustDiff Dc = thrust_diff(T);
+    D.x = moved ? Dc.x : De.x; D.y = moved ? Dc.y : De.y; D.z = moved ? Dc.z : De.z;
 }
 
 // soft body-rate limit [R-31]
@@ -187,12 +212,12 @@ __device__ __forceinline__ float contour_paper_stage(const DevParams& P, const f
 // ---- two samples per thread in packed fp32x2 registers (see mppi_packed.cuh): the same model ------------
 struct Deriv2 { float2 qw, qx, qy, qz, vx, vy, vz, ox, oy, oz; };
 
-// f_dyn of eq.(2) with drag for two samples; T0..T3: rotor thrusts (halves = the two samples)
+// f_dyn of eq.(2) with drag for two samples; ax, ay, az, c as in fdyn_general (halves = the two samples)
 template <int AXI = 0>
 __device__ __forceinline__ Deriv2 fdyn_general2(const DevParams& P, const float2 qw, const float2 qx, const float2 qy,
                                                 const float2 qz, const float2 vx, const float2 vy, const float2 vz,
-                                                const float2 ox, const float2 oy, const float2 oz, const float2 T0,
-                                                const float2 T1, const float2 T2, const float2 T3)
+                                                const float2 ox, const float2 oy, const float2 oz, const float2 ax,
+                                                const float2 ay, const float2 az, const float2 c)
 {
     Deriv2 d;                                  // same operations, same order as fdyn_general on each half
     const float2 hf = bc2(0.5f);
@@ -200,12 +225,9 @@ __device__ __forceinline__ Deriv2 fdyn_general2(const DevParams& P, const float2
     d.qx = fma2(neg2(qz), oy, fma2(qy, oz, mul2(qw, ox)));
     d.qy = fma2(neg2(qx), oz, fma2(qz, ox, mul2(qw, oy)));
     d.qz = fma2(neg2(qy), ox, fma2(qx, oy, mul2(qw, oz)));
-    const float2 s01 = add2(T0, T1), s23 = add2(T2, T3);
-    d.ox = fma2(P.gyx, mul2(oy, oz), mul2(bc2(P.ltx), sub2(s01, s23)));
-    const float2 d10 = sub2(T1, T0), d23 = sub2(T2, T3);
-    d.oy = fma2(P.gyy, mul2(oz, ox), mul2(bc2(P.lty), add2(d10, d23)));
-    d.oz = fma2(P.gyz, mul2(ox, oy), mul2(bc2(P.ltz), sub2(d23, d10)));
-    const float2 c = mul2(add2(s01, s23), bc2(P.inv_mass2));
+    d.ox = fma2(P.gyx, mul2(oy, oz), ax);
+    d.oy = fma2(P.gyy, mul2(oz, ox), ay);
+    d.oz = fma2(P.gyz, mul2(ox, oy), az);
     if (AXI) {
         const float2 e2x = fma2(qx, qz, mul2(qw, qy)), e2y = fma2(qy, qz, mul2(neg2(qw), qx)),
                      e2z = fma2(neg2(qy), qy, fma2(neg2(qx), qx, hf));
@@ -245,15 +267,31 @@ __device__ __forceinline__ float2 clamp2(const float2 v, const float lo, const f
     return make_float2(fminf(fmaxf(v.x, lo), hi), fminf(fmaxf(v.y, lo), hi));
 }
 
-// rk4_rate_step for two samples: x, T (4 rotor thrust pairs) <- one step with the rates ua / ub held
+struct ThrustDiff2 { float2 x, y, z; };
+__device__ __forceinline__ ThrustDiff2 thrust_diff2(const float2 T0, const float2 T1, const float2 T2, const float2 T3)
+{
+    const float2 s01 = add2(T0, T1), s23 = add2(T2, T3), d10 = sub2(T1, T0), d23 = sub2(T2, T3);
+    return ThrustDiff2{sub2(s01, s23), add2(d10, d23), sub2(d23, d10)};
+}
+
+// rk4_rate_step for two samples: x, T (4 rotor thrust pairs), D (their torque combinations) <- one step with the rates
+// ua / ub held; same operations in the same order as rk4_rate_step on each half
 template <bool AXI = false>
-__device__ __forceinline__ void rk4_rate_step2(const DevParams& P, State2& x, float2 (&T)[4], const float4 ua, const float4 ub)
+__device__ __forceinline__ void rk4_rate_step2(const DevParams& P, State2& x, float2 (&T)[4], ThrustDiff2& D, const float4 ua,
+                                               const float4 ub)
 {
     const float2 h = bc2(P.dt), hh = bc2(P.h2), hq = bc2(P.h4), h6 = bc2(P.h6), h12 = bc2(P.h12), two = bc2(2.0f);
     const float2 u0 = make_float2(ua.x, ub.x), u1 = make_float2(ua.y, ub.y), u2 = make_float2(ua.z, ub.z), u3 = make_float2(ua.w, ub.w);
-    const float2 Tm0 = fma2(hh, u0, T[0]), Tm1 = fma2(hh, u1, T[1]), Tm2 = fma2(hh, u2, T[2]), Tm3 = fma2(hh, u3, T[3]);
     const float2 Te0 = fma2(h, u0, T[0]), Te1 = fma2(h, u1, T[1]), Te2 = fma2(h, u2, T[2]), Te3 = fma2(h, u3, T[3]);
-    Deriv2 k = fdyn_general2<(AXI ? 1 : 0)>(P, x.qw, x.qx, x.qy, x.qz, x.vx, x.vy, x.vz, x.ox, x.oy, x.oz, T[0], T[1], T[2], T[3]);
+    const ThrustDiff2 du = thrust_diff2(u0, u1, u2, u3);
+    const float2 S = add2(add2(T[0], T[1]), add2(T[2], T[3])), su = add2(add2(u0, u1), add2(u2, u3));
+    const ThrustDiff2 Dm{fma2(hh, du.x, D.x), fma2(hh, du.y, D.y), fma2(hh, du.z, D.z)};
+    const ThrustDiff2 De{fma2(h, du.x, D.x), fma2(h, du.y, D.y), fma2(h, du.z, D.z)};
+    const float2 ltx = bc2(P.ltx), lty = bc2(P.lty), ltz = bc2(P.ltz), im2 = bc2(P.inv_mass2);
+    const float2 a1x = mul2(ltx, D.x), a1y = mul2(lty, D.y), a1z = mul2(ltz, D.z), c1 = mul2(S, im2);
+    const float2 amx = mul2(ltx, Dm.x), amy = mul2(lty, Dm.y), amz = mul2(ltz, Dm.z), cm = mul2(fma2(hh, su, S), im2);
+    const float2 aex = mul2(ltx, De.x), aey = mul2(lty, De.y), aez = mul2(ltz, De.z), ce = mul2(fma2(h, su, S), im2);
+    Deriv2 k = fdyn_general2<(AXI ? 1 : 0)>(P, x.qw, x.qx, x.qy, x.qz, x.vx, x.vy, x.vz, x.ox, x.oy, x.oz, a1x, a1y, a1z, c1);
     float2 apx = x.vx, apy = x.vy, apz = x.vz;
     Deriv2 a = k;
 #define MPPI_STAGE2(HS, HQ)                                                                          \
@@ -267,15 +305,15 @@ __device__ __forceinline__ void rk4_rate_step2(const DevParams& P, State2& x, fl
     float2 vx, vy, vz, qw, qx, qy, qz, ox, oy, oz;
     MPPI_STAGE2(hh, hq)
     apx = fma2(two, vx, apx); apy = fma2(two, vy, apy); apz = fma2(two, vz, apz);
-    k = fdyn_general2<(AXI ? 2 : 0)>(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Tm0, Tm1, Tm2, Tm3);
+    k = fdyn_general2<(AXI ? 2 : 0)>(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, amx, amy, amz, cm);
     MPPI_ACC2(two)
     MPPI_STAGE2(hh, hq)
     apx = fma2(two, vx, apx); apy = fma2(two, vy, apy); apz = fma2(two, vz, apz);
-    k = fdyn_general2<(AXI ? 2 : 0)>(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Tm0, Tm1, Tm2, Tm3);
+    k = fdyn_general2<(AXI ? 2 : 0)>(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, amx, amy, amz, cm);
     MPPI_ACC2(two)
     MPPI_STAGE2(h, hh)
     apx = add2(apx, vx); apy = add2(apy, vy); apz = add2(apz, vz);
-    k = fdyn_general2<(AXI ? 2 : 0)>(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, Te0, Te1, Te2, Te3);
+    k = fdyn_general2<(AXI ? 2 : 0)>(P, qw, qx, qy, qz, vx, vy, vz, ox, oy, oz, aex, aey, aez, ce);
     a.qw = add2(a.qw, k.qw); a.qx = add2(a.qx, k.qx); a.qy = add2(a.qy, k.qy); a.qz = add2(a.qz, k.qz);
     a.vx = add2(a.vx, k.vx); a.vy = add2(a.vy, k.vy); a.vz = add2(a.vz, k.vz);
     a.ox = add2(a.ox, k.ox); a.oy = add2(a.oy, k.oy); a.oz = add2(a.oz, k.oz);
@@ -290,6 +328,12 @@ __device__ __forceinline__ void rk4_rate_step2(const DevParams& P, State2& x, fl
     x.qw = mul2(nw, inv); x.qx = mul2(nx, inv); x.qy = mul2(ny, inv); x.qz = mul2(nz, inv);
     T[0] = clamp2(Te0, P.T_min, P.T_max); T[1] = clamp2(Te1, P.T_min, P.T_max);
     T[2] = clamp2(Te2, P.T_min, P.T_max); T[3] = clamp2(Te3, P.T_min, P.T_max);
+    const bool ma = T[0].x != Te0.x || T[1].x != Te1.x || T[2].x != Te2.x || T[3].x != Te3.x;   // the projection acted
+    const bool mb = T[0].y != Te0.y || T[1].y != Te1.y || T[2].y != Te2.y || T[3].y != Te3.y;
+    const ThrustDiff2 Dc = thrust_diff2(T[0], T[1], T[2], T[3]);
+    D.x = make_float2(ma ? Dc.x.x : De.x.x, mb ? Dc.x.y : De.x.y);
+    D.y = make_float2(ma ? Dc.y.x : De.y.x, mb ? Dc.y.y : De.y.y);
+    D.z = make_float2(ma ? Dc.z.x : De.z.x, mb ? Dc.z.y : De.z.y);
 }
 
 }  // namespace mppi
