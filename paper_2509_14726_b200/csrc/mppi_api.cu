@@ -210,7 +210,10 @@ static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, i
     if (p->input_model == 1) {                     // thrust-rate model: its own kernels (mppi_rate.cu)
         // the scalar shape; whether the pipelined latency kernel takes over is decided in prepare(), once the
         // track (and with it the shared-memory footprint) is known -- see rate_pipe_candidate
-        const bool pk_obj = p->objective != MPPI_OBJ_CONTOUR;
+        // objective 4 runs on the packed kernel too, but no faster than on the scalar one (313 vs 307 us x 64: its
+        // two Philox blocks per sample-step, path look-ups and stage costs stay scalar per half): AUTO keeps the scalar
+        const bool pk_obj = p->objective != MPPI_OBJ_CONTOUR &&
+                            (p->variant == MPPI_VARIANT_PACKED || p->objective != MPPI_OBJ_CONTOUR_PAPER);
         // packed fp32x2 throughput kernel (rollout_rate2_kernel): when the grid covers the chip
         if (pk_obj && p->K % 64 == 0 && (p->variant == MPPI_VARIANT_PACKED ||
                                          (p->variant == MPPI_VARIANT_AUTO && warps >= 8 * (int64_t)sm_count))) {
