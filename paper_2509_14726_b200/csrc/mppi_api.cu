@@ -568,7 +568,10 @@ static int prepare(mppi_ctx* c)
             c->cfg.smem_bytes = 0;
         }
     }
+    // latency kernel under search-contouring: the rollout / search split needs a position table in shared memory
+    c->cfg.lat_split = (c->cfg.lat_consumers > 0 && obj == MPPI_OBJ_CONTOUR) ? 1 : 0;
     size_t need = rollout_smem_bytes(c->dp, c->cfg);
+    if (c->cfg.lat_split && need > 227 * 1024) { c->cfg.lat_split = 0; need = rollout_smem_bytes(c->dp, c->cfg); }
     if (need > 227 * 1024 && c->prm.variant == MPPI_VARIANT_AUTO && c->prm.input_model == 0 &&
         (c->cfg.pipe || c->cfg.lat_consumers)) {
         // the kernel picked from the warp count alone does not fit with this track: next choice of pick_shape
@@ -581,6 +584,7 @@ static int prepare(mppi_ctx* c)
             const size_t nn = rollout_smem_bytes(nd, nc);
             if (nn <= 227 * 1024 || avoid == 3) {
                 c->cfg = nc; c->cfg.smem_bytes = 0; c->dp.blocks_per_ctrl = nd.blocks_per_ctrl; need = nn;
+                if (!nc.lat_consumers) c->cfg.lat_split = 0;
                 free_graph(c->g_step); free_graph(c->g_opt);
                 break;
             }
@@ -673,7 +677,7 @@ static int graph_run(mppi_ctx* c, GraphSlot& g, const std::vector<StepArgs>& arg
     cudaGraphNode_t prev = nullptr;
     for (int i = 0; i < n; ++i) {
         StepArgs a = args[i];
-        int lat_c = c->cfg.lat_consumers;
+        int lat_c = c->cfg.lat_consumers | (c->cfg.lat_split << 8);
         void* kp[3] = {&dp, &a, &lat_c};
         cudaKernelNodeParams np;
         for (int pass = 0; pass < (c->cfg.fused ? 1 : 2); ++pass) {

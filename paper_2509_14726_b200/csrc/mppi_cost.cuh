@@ -331,17 +331,24 @@ struct ContourCost {
     template <bool ROT = false>
     __device__ __forceinline__ float step(const DevParams& P, const float4* s_path, const State& x)
     {
-        idx = (ROT && P.window == 16) ? nearest_rot(P, s_path, idx, x.px, x.py, x.pz)
-                                      : nearest_smem(P, s_path, idx, x.px, x.py, x.pz);
+        return step_at<ROT>(P, s_path, x.px, x.py, x.pz, x.ox * x.ox + x.oy * x.oy + x.oz * x.oz);
+    }
+    // the same step from a position and |omega|^2 (what the rollout warps of the latency kernel hand over)
+    template <bool ROT = false>
+    __device__ __forceinline__ float step_at(const DevParams& P, const float4* s_path, const float px, const float py,
+                                             const float pz, const float w2)
+    {
+        idx = (ROT && P.window == 16) ? nearest_rot(P, s_path, idx, px, py, pz)
+                                      : nearest_smem(P, s_path, idx, px, py, pz);
         float e_l, e_c2, theta;
-        project(P, s_path, idx, x.px, x.py, x.pz, e_l, e_c2, theta);
+        project(P, s_path, idx, px, py, pz, e_l, e_c2, theta);
         float d = theta - theta_prev;
         if (P.closed) d -= P.path_L * ceilf((d - 0.5f * P.path_L) * P.inv_path_L);  // (-L/2, L/2]
         theta_prev = theta;
         float J = P.q_c * e_c2;
         J = fmaf(P.q_l, e_l * e_l, J);
         J = fmaf(-P.mu, d, J);
-        return fmaf(P.w_omega, x.ox * x.ox + x.oy * x.oy + x.oz * x.oz, J);
+        return fmaf(P.w_omega, w2, J);
     }
 };
 

@@ -15,6 +15,7 @@ struct LaunchCfg {
     int rate;           // 1: rollout_rate_kernel (thrust-rate input model, mppi_rate.cu)
     int pipe_shallow;   // rollout_pipe_rate_kernel: 1 = rings (2, 2) chunks deep (two blocks per SM), 0 = (4, 3)
     int lat_consumers;  // 0: throughput kernel; 1, 2 or 4: latency kernel with that many rollout warps per block
+    int lat_split;      // latency kernel, search-contouring: 1 = the search runs in warps of its own (when it fits in shared memory)
     size_t smem_bytes;  // dynamic shared memory of the rollout kernel
 };
 

@@ -17,6 +17,9 @@
 
 namespace mppi {
 
+constexpr int kLatChunk = 5;       // steps per hand-over of the contouring split of rollout_lat_kernel
+__host__ __device__ inline int lat_chunks(int N) { return (N + kLatChunk - 1) / kLatChunk; }
+
 // Shared-memory carve-up of rollout_kernel (units: float4).
 //   [0, N)                         nominal thrusts u_nom[b]
 //   [N, N + trk)                   track data of the objective
@@ -29,6 +32,8 @@ size_t rollout_smem_bytes(const DevParams& P, const LaunchCfg& c)
     if (c.pipe) return (f4 + (c.rate ? pipe_rate_extra_f4(P.N, P.blocks_per_ctrl, c.objective == OBJ_CONTOUR_PAPER, P.pipe_d, P.pipe_df) : pipe_extra_f4(P.N, P.blocks_per_ctrl))) * sizeof(float4);
     if (c.lat_consumers > 0) {
         f4 += (size_t)P.N * (32 * c.lat_consumers + 1) + 32 + (3 * P.blocks_per_ctrl + 3) / 4;
+        if (c.objective == OBJ_CONTOUR && c.lat_split)   // rollout warps -> search warps: positions [N][32 C], costs [32 C], mbarriers
+            f4 += (size_t)P.N * 32 * c.lat_consumers + 8 * c.lat_consumers + (c.lat_consumers * lat_chunks(P.N) + 1) / 2;
         return f4 * sizeof(float4);
     }
     if (c.fused) f4 += (size_t)(c.block_threads / 32) * P.N + (3 * P.blocks_per_ctrl + 3) / 4;
@@ -204,8 +209,10 @@ struct SmemThrust {
 constexpr int kLatThreads = 256;
 
 template <int OBJ, int MATH, bool STORE_DU>
-__global__ void __launch_bounds__(kLatThreads, 2) rollout_lat_kernel(const DevParams P, const StepArgs A, const int C)
+__global__ void __launch_bounds__(kLatThreads, 2) rollout_lat_kernel(const DevParams P, const StepArgs A, const int Cflags)
 {
+    const int C = Cflags & 0xff;                  // rollout warps per block
+    const bool split = (Cflags & 0x100) != 0;     // search-contouring: search and cost in warps of their own (host: it fits)
     extern __shared__ float4 smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int b = blockIdx.y, N = P.N;
@@ -239,7 +246,45 @@ __global__ void __launch_bounds__(kLatThreads, 2) rollout_lat_kernel(const DevPa
 
     // ---- phase 2: C warps roll out, one per scheduler ----
     float J = __int_as_float(0x7f800000);
-    if (warp < C) {
+    if (OBJ == OBJ_CONTOUR && split) {
+        // Search-based contouring: the windowed nearest-vertex search (33 shared-memory reads and ~300 instructions
+        // per step) is as long as the RK4 step itself, and nothing of it feeds back into the dynamics.  So the C
+        // rollout warps only integrate and publish (p, |omega|^2) per step; C further warps -- idle otherwise --
+        // follow chunk by chunk (mbarriers), search and accumulate the cost.  The two chains overlap instead of adding up.
+        float4* s_pos = reinterpret_cast<float4*>(s_pair) + (3 * P.blocks_per_ctrl + 3) / 4;      // [N][S]
+        float* s_Jc = reinterpret_cast<float*>(s_pos + (size_t)N * S);                             // [S]
+        uint64_t* bar_p = reinterpret_cast<uint64_t*>(s_Jc + S);                                   // [C][chunks]
+        const int nch = lat_chunks(N);
+        for (int i = tid; i < C * nch; i += kLatThreads) mbar_init(bar_p + i, 32);
+        __syncthreads();
+        if (warp < C) {
+            State x = x0;
+            for (int t = 0; t < N; ++t) {
+                rk4_step(P, x, s_T[t * RS + tid]);
+                s_pos[t * S + tid] = make_float4(x.px, x.py, x.pz, x.ox * x.ox + x.oy * x.oy + x.oz * x.oz);
+                if ((t + 1) % kLatChunk == 0 || t == N - 1) mbar_arrive(bar_p + warp * nch + t / kLatChunk);
+            }
+        } else if (warp < 2 * C) {
+            const int w = warp - C, sid = w * 32 + lane;
+            ContourCost cc;
+            cc.init(P, s_trk, i0, x0);
+            float Jc = 0.0f;
+            for (int c = 0; c < nch; ++c) {
+                mbar_wait(bar_p + w * nch + c, 0);
+                const int t1 = min(N, (c + 1) * kLatChunk);
+                for (int t = c * kLatChunk; t < t1; ++t) {
+                    const float4 q = s_pos[t * S + sid];
+                    Jc += cc.step_at(P, s_trk, q.x, q.y, q.z, q.w);
+                }
+            }
+            s_Jc[sid] = Jc;
+        }
+        __syncthreads();
+        if (warp < C) {
+            J = sanitize_cost(s_Jc[tid]);
+            A.cost[(size_t)b * P.K + kbase + tid] = J;
+        }
+    } else if (warp < C) {
         SmemThrust src{s_T + tid, RS};
         J = sanitize_cost(rollout_cost<OBJ, MATH>(P, s_trk, x0, start, i0, src));
         A.cost[(size_t)b * P.K + kbase + tid] = J;
@@ -543,7 +588,7 @@ cudaError_t launch_rollout(const DevParams& P, const StepArgs& A, const LaunchCf
     const dim3 grid(P.blocks_per_ctrl, P.B), block(c.block_threads);
     if (c.rate) return launch_rate(P, A, c, s);
     if (c.pipe) pick_pipe(c)<<<grid, block, c.smem_bytes, s>>>(P, A);
-    else if (c.lat_consumers > 0) pick_lat(c)<<<grid, block, c.smem_bytes, s>>>(P, A, c.lat_consumers);
+    else if (c.lat_consumers > 0) pick_lat(c)<<<grid, block, c.smem_bytes, s>>>(P, A, c.lat_consumers | (c.lat_split << 8));
     else pick(c)<<<grid, block, c.smem_bytes, s>>>(P, A);
     return cudaGetLastError();
 }
