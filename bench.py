@@ -43,7 +43,7 @@ L2_FLUSH_BYTES = 256 << 20
 # cuobjdump -sass of rollout_kernel<OBJ_GATE, fast math>): 154 FFMA (53 with three register operands, 101 with a
 # constant operand), 67 FMUL, 44 FADD, 20 Philox half-rounds (IMAD.WIDE + LOP3), 11 MUFU, 8 FMNMX, 7 LDS.128.
 GATE_LOOP_MIX = {"ffma_rrr": 53, "ffma_const": 101, "fmul": 67, "fadd": 44, "philox_half_round": 20, "mufu": 11, "fmnmx": 8, "lds": 7}
-NCU_DRAM_BYTES_PER_LAUNCH = 53248     # rollout_pipe_kernel<gate>, cfg1: 53.2 KB read + 0 B written (profiles/README_r01e.md)
+NCU_DRAM_BYTES_PER_LAUNCH = 51968     # rollout_pipe_kernel<gate>, cfg1: 52.0 KB read + 0 B written (profiles/README_r02c.md, ncu_details_pipe_r02.txt)
 
 
 def dist_env():
