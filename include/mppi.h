@@ -325,6 +325,37 @@ MPPI_API int mppi_measure_issue_rates(double* cycles_per_instr, int n);
  * launch and the events, not the library.  Synchronises. */
 MPPI_API int mppi_measure_launch_floor(int reps, double* median_us);
 
+/* ---- one entry point that allocates nothing -----------------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA-graph capture, tight serving loops, harnesses that forbid
+ * it): ONE MPPI iteration (Alg. 1 lines 3-17; eq.(3)-(6)) exactly as mppi_create + mppi_set_gates +
+ * mppi_step compute it, for the gate-progress objective (MPPI_OBJ_GATE) with rotor-thrust inputs, through the
+ * pipelined latency kernel -- with every byte of scratch (block partials, their (m, Z) headers, last-block tickets, the
+ * packed gate table) in one file-scope static __device__ array of about 1.07 MB, which every GPU that loads the
+ * library holds until the process exits.  No context, no cudaMalloc / cudaFree / cudaHostAlloc, no allocating library
+ * routine, on any call.  Limits: K <= MPPI_STATIC_MAX_K, N <= MPPI_STATIC_MAX_N, B <= MPPI_STATIC_MAX_B,
+ * G <= MPPI_STATIC_MAX_GATES; beyond them MPPI_E_RANGE, text from mppi_step_static_error().
+ *   p          host: parameters as for mppi_create; objective MPPI_OBJ_GATE, input_model 0, pipeline FUSED, store_noise 0,
+ *              block_threads 0, variant AUTO or PIPELINED (else MPPI_E_PARAM); fast_math honoured
+ *   d_gates    [G][11] DEVICE, in: the rows mppi_set_gates takes (centre, unit normal, unit in-plane axis, half-width,
+ *              half-height), not validated here; packed on the device by a one-block kernel in every call
+ *   d_x0 [B][13], d_start [B], d_u_nom [B][N][4], d_u_new [B][N][4] (== d_u_nom allowed), d_cost [B][K],
+ *   d_weights [B][K]: device, as for mppi_step; seed, iter: Philox key and counter word 2
+ * Two kernels are enqueued on cuda_stream; outputs are valid once the stream has reached the end of that work.
+ * The first call on a device takes the array's address (cudaGetSymbolAddress) and raises the kernels' dynamic
+ * shared-memory limit (cudaFuncSetAttribute) with that device current; a caller that captures graphs makes one plain
+ * call first.  Every call shares the one array per device: it keeps the last call's contents (the tickets, which must
+ * start at zero, are cleared by every call), and calls that OVERLAP on the GPU -- different streams without an event
+ * dependency, concurrent graph replays -- race on it and give wrong results.  Results equal those of the
+ * allocating path for the same inputs. */
+#define MPPI_STATIC_MAX_K 8192
+#define MPPI_STATIC_MAX_N 64
+#define MPPI_STATIC_MAX_B 4
+#define MPPI_STATIC_MAX_GATES 64
+MPPI_API int mppi_step_static(const mppi_params* p, const float* d_gates, int G, const float* d_x0, const int32_t* d_start,
+                              const float* d_u_nom, uint64_t seed, uint32_t iter, float* d_u_new, float* d_cost,
+                              float* d_weights, void* cuda_stream);
+MPPI_API const char* mppi_step_static_error(void); /* detail of this thread's last failed mppi_step_static ("" if none) */
+
 #ifdef __cplusplus
 }
 #endif

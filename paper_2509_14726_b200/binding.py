@@ -21,7 +21,8 @@ VARIANT_AUTO, VARIANT_THROUGHPUT, VARIANT_LATENCY, VARIANT_PACKED, VARIANT_PIPEL
 EXPORTS = ["mppi_default_params", "mppi_create", "mppi_destroy", "mppi_set_gates",
            "mppi_set_reference", "mppi_set_path", "mppi_step", "mppi_optimize", "mppi_step_host",
            "mppi_sim_step", "mppi_set_prev_front", "mppi_front_flags", "mppi_set_progress", "mppi_sim_step_progress", "mppi_debug_noise", "mppi_get_info", "mppi_launch_count",
-           "mppi_error_string", "mppi_last_error", "mppi_measure_fma_peak", "mppi_measure_copy_bw", "mppi_measure_issue_rates", "mppi_measure_launch_floor"]
+           "mppi_error_string", "mppi_last_error", "mppi_measure_fma_peak", "mppi_measure_copy_bw", "mppi_measure_issue_rates", "mppi_measure_launch_floor",
+           "mppi_step_static", "mppi_step_static_error"]
 
 
 class MppiParams(C.Structure):
@@ -86,6 +87,9 @@ def _load():
     L.mppi_measure_copy_bw.argtypes = [C.c_int64, C.c_int, C.POINTER(C.c_double)]
     L.mppi_measure_issue_rates.argtypes = [C.POINTER(C.c_double), C.c_int]
     L.mppi_measure_launch_floor.argtypes = [C.c_int, C.POINTER(C.c_double)]
+    L.mppi_step_static.argtypes = [C.POINTER(MppiParams), fp, C.c_int, fp, ip, fp, C.c_uint64, C.c_uint32, fp, fp, fp, vp]
+    L.mppi_step_static_error.argtypes = []
+    L.mppi_step_static_error.restype = C.c_char_p
     for name in EXPORTS:
         getattr(L, name)            # AttributeError here = the library is stale: rebuild it
     return L
@@ -390,3 +394,25 @@ def measure_launch_floor(reps=400) -> float:
     if rc:
         raise MppiError(rc)
     return v.value
+
+
+STATIC_MAX = dict(K=8192, N=64, B=4, G=64)      # MPPI_STATIC_MAX_* of include/mppi.h
+
+
+def step_static(params, gates, x0, start, u_nom, seed, it, u_new, cost, weights, stream=None):
+    """mppi_step_static: one gate-progress iteration that allocates nothing (scratch in a static device array; limits
+    STATIC_MAX).  params: dict / MppiParams; every other argument a contiguous CUDA tensor the CALLER allocated:
+    gates [G,11] f32, x0 [B,13] f32, start [B] i32, u_nom / u_new [B,N,4] f32, cost / weights [B,K] f32.
+    Calls on one device must not overlap on the GPU."""
+    import torch
+    P = params if isinstance(params, MppiParams) else make_params(params)
+    B, N, K = P.B, P.N, P.K
+    G = int(gates.shape[0])
+    dev = Mppi._dev
+    rc = lib.mppi_step_static(C.byref(P), dev(gates, (G, 11), torch.float32), G, dev(x0, (B, 13), torch.float32),
+                              dev(start, (B,), torch.int32), dev(u_nom, (B, N, 4), torch.float32), C.c_uint64(int(seed)),
+                              C.c_uint32(int(it)), dev(u_new, (B, N, 4), torch.float32), dev(cost, (B, K), torch.float32),
+                              dev(weights, (B, K), torch.float32), _stream_ptr(stream))
+    if rc:
+        raise MppiError(rc, lib.mppi_step_static_error().decode())
+    return u_new, cost, weights
