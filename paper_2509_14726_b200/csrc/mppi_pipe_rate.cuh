@@ -387,7 +387,7 @@ __global__ void __launch_bounds__(kPipeRateThreads, SHALLOW ? 2 : 1) rollout_pip
             part[4 * N + 4 + t] = acc;
         }
     if (tid == 0) write_partial_header(P, A, b, blockIdx.x, m, Zb);
-    publish_and_combine<MATH, 4>(P, A, b, P.blocks_per_ctrl, s_unom, s_red, s_pair, reinterpret_cast<float*>(s_T),
+    publish_and_combine<MATH, (SHALLOW ? 2 : 4)>(P, A, b, P.blocks_per_ctrl, s_unom, s_red, s_pair, reinterpret_cast<float*>(s_T),
                               OBJ == OBJ_CONTOUR_PAPER ? s_vnom : nullptr);
 }
 

@@ -467,48 +467,27 @@ __device__ __forceinline__ void publish_and_combine(const DevParams& P, const St
     // number of contributing partials; thread-per-column with four loads per round took cnt / 4 round trips).  The
     // warps' sums meet in s_work [nw][group columns] and are added in warp order: deterministic.
     // Column groups: the 4N thrust columns, then (fifth input) the N columns kept after the header.
-    const float* unf = reinterpret_cast<const float*>(s_unom);
-    for (int grp = 0; grp < (s_vnom ? 2 : 1); ++grp) {
-        const int gcol = grp ? N : 4 * N, goff = grp ? 4 * N + 4 : 0;
-        constexpr int CMAX = 8;                        // columns per lane and sweep: 256 columns per sweep
-        for (int c0 = 0; c0 < gcol; c0 += 32 * CMAX) {
-            float acc[CMAX];
+    // The first batch of loads goes out BEFORE the weights are formed and is consumed after them: the weights need
+    // beta and Z only, so their arithmetic and stores fill the L2 round trip of the S rows.
+    constexpr int CMAX = 8;                            // columns per lane and sweep: 256 columns per sweep
+    constexpr int kRows = ROWS;                        // partials per warp and batch, all loads issued before the first
+                                                       // use (4 in the latency kernels, 2 where registers are the rollout's)
+    auto load_batch = [&](const int goff, const int gcol, const int c0, const int i0, float (&v)[kRows][CMAX], float (&sc)[kRows]) {
 #pragma unroll
-            for (int c = 0; c < CMAX; ++c) acc[c] = 0.0f;
-            // batches of kRows partials per warp: all their loads are issued before the first use (ROWS: 4 in the
-            // latency kernels, where the iteration time is this chain; 2 where the register budget is the rollout's)
-            constexpr int kRows = ROWS;
-            for (int i0 = warp; i0 < cnt; i0 += kRows * nw) {
-                float v[kRows][CMAX], sc[kRows];
-#pragma unroll
-                for (int r = 0; r < kRows; ++r) {
-                    const int i = i0 + r * nw;
-                    const bool on = i < cnt;
-                    sc[r] = on ? s_scale[i] : 0.0f;
-                    const float* row = pb + (size_t)(on ? s_list[i] : 0) * stride + goff + c0 + lane;
-#pragma unroll
-                    for (int c = 0; c < CMAX; ++c)
-                        v[r][c] = (on && c0 + 32 * c + lane < gcol) ? __ldcg(row + 32 * c) : 0.0f;
-                }
-#pragma unroll
-                for (int r = 0; r < kRows; ++r)
-#pragma unroll
-                    for (int c = 0; c < CMAX; ++c) acc[c] = fmaf(v[r][c], sc[r], acc[c]);
-            }
+        for (int rr = 0; rr < kRows; ++rr) {
+            const int i = i0 + rr * nw;
+            const bool on = i < cnt;
+            sc[rr] = on ? s_scale[i] : 0.0f;
+            const float* row = pb + (size_t)(on ? s_list[i] : 0) * stride + goff + c0 + lane;
 #pragma unroll
             for (int c = 0; c < CMAX; ++c)
-                if (c0 + 32 * c + lane < gcol) s_work[warp * gcol + c0 + 32 * c + lane] = acc[c];
+                v[rr][c] = (on && c0 + 32 * c + lane < gcol) ? __ldcg(row + 32 * c) : 0.0f;
         }
-        __syncthreads();
-        for (int j = tid; j < gcol; j += nthr) {
-            float s = 0.0f;
-            for (int w = 0; w < nw; ++w) s += s_work[w * gcol + j];
-            if (grp == 0) A.u_new[(size_t)b * 4 * N + j] = fmaf(s, invZ, unf[j]);
-            else A.v_new[(size_t)b * N + j] = fmaf(s, invZ, s_vnom[j]);
-        }
-        if (s_vnom) __syncthreads();                   // s_work is reused by the next group
-    }
-    if (tid == 0) MPPI_STAMP(A, 11);
+    };
+    float v0[kRows][CMAX], sc0[kRows];
+    load_batch(0, 4 * N, 0, warp, v0, sc0);
+
+    // ---- weights w_k = exp(-(J_k - beta) / lambda) / Z ----
     float4* w4 = reinterpret_cast<float4*>(A.weights + (size_t)b * P.K);
     const float nil = -P.inv_lambda;
     int nz = 0;                                // samples of this thread that carry weight
@@ -525,6 +504,45 @@ __device__ __forceinline__ void publish_and_combine(const DevParams& P, const St
     }
 #pragma unroll 4
     for (int i = tid + PRE * nthr; i < n4; i += nthr) w4[i] = weights_of(__ldcg(c4 + i));
+    if (tid == 0) MPPI_STAMP(A, 11);
+
+    const float* unf = reinterpret_cast<const float*>(s_unom);
+    for (int grp = 0; grp < (s_vnom ? 2 : 1); ++grp) {
+        const int gcol = grp ? N : 4 * N, goff = grp ? 4 * N + 4 : 0;
+        for (int c0 = 0; c0 < gcol; c0 += 32 * CMAX) {
+            float acc[CMAX];
+#pragma unroll
+            for (int c = 0; c < CMAX; ++c) acc[c] = 0.0f;
+            for (int i0 = warp; i0 < cnt; i0 += kRows * nw) {
+                float v[kRows][CMAX], sc[kRows];
+                if (grp == 0 && c0 == 0 && i0 == warp) {           // the batch that is already in registers
+#pragma unroll
+                    for (int rr = 0; rr < kRows; ++rr) {
+                        sc[rr] = sc0[rr];
+#pragma unroll
+                        for (int c = 0; c < CMAX; ++c) v[rr][c] = v0[rr][c];
+                    }
+                } else {
+                    load_batch(goff, gcol, c0, i0, v, sc);
+                }
+#pragma unroll
+                for (int rr = 0; rr < kRows; ++rr)
+#pragma unroll
+                    for (int c = 0; c < CMAX; ++c) acc[c] = fmaf(v[rr][c], sc[rr], acc[c]);
+            }
+#pragma unroll
+            for (int c = 0; c < CMAX; ++c)
+                if (c0 + 32 * c + lane < gcol) s_work[warp * gcol + c0 + 32 * c + lane] = acc[c];
+        }
+        __syncthreads();
+        for (int j = tid; j < gcol; j += nthr) {
+            float s = 0.0f;
+            for (int w = 0; w < nw; ++w) s += s_work[w * gcol + j];
+            if (grp == 0) A.u_new[(size_t)b * 4 * N + j] = fmaf(s, invZ, unf[j]);
+            else A.v_new[(size_t)b * N + j] = fmaf(s, invZ, s_vnom[j]);
+        }
+        if (s_vnom) __syncthreads();                   // s_work is reused by the next group
+    }
     if (A.hint) {
         // Hint for the NEXT launch on this controller (keeps_du): did many samples carry weight?  Then the sparse
         // re-derivation of the block partials costs a second pass over the noise stream and storing dU is cheaper.
