@@ -595,7 +595,9 @@ static int prepare(mppi_ctx* c)
     if (c->cfg.fused && !c->cfg.pipe && !c->cfg.lat_consumers && c->prm.objective != MPPI_OBJ_CONTOUR_PAPER && !c->d_du &&
         !c->du_tried) {
         c->du_tried = true;
-        if (dev_alloc(c, &c->d_du, (size_t)c->prm.B * c->prm.N * c->prm.K) != cudaSuccess) { cudaGetLastError(); c->d_du = nullptr; }
+        // at most 1 GiB of such scratch (configs[4]: 210 MB); larger batches keep re-deriving the noise
+        const size_t n_du = (size_t)c->prm.B * c->prm.N * c->prm.K;
+        if (n_du * sizeof(float4) <= ((size_t)1 << 30) && dev_alloc(c, &c->d_du, n_du) != cudaSuccess) { cudaGetLastError(); c->d_du = nullptr; }
     }
     if (need != c->cfg.smem_bytes) {
         if (need > 227 * 1024) return fail(c, MPPI_E_PARAM, "track + horizon do not fit in shared memory");

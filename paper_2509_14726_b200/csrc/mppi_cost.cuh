@@ -340,6 +340,12 @@ struct ContourCost {
     {
         idx = (ROT && P.window == 16) ? nearest_rot(P, s_path, idx, px, py, pz)
                                       : nearest_smem(P, s_path, idx, px, py, pz);
+        return step_found(P, s_path, px, py, pz, w2);
+    }
+    // the cost of the step once idx holds the nearest vertex of this position
+    __device__ __forceinline__ float step_found(const DevParams& P, const float4* s_path, const float px, const float py,
+                                                const float pz, const float w2)
+    {
         float e_l, e_c2, theta;
         project(P, s_path, idx, px, py, pz, e_l, e_c2, theta);
         float d = theta - theta_prev;

@@ -20,6 +20,12 @@ namespace mppi {
 constexpr int kLatChunk = 5;       // steps per hand-over of the contouring split of rollout_lat_kernel
 __host__ __device__ inline int lat_chunks(int N) { return (N + kLatChunk - 1) / kLatChunk; }
 
+// float4 units of the register-pair rows of the contouring candidates (nearest_rot4, packed kernel); 0 = not used
+__host__ __device__ inline int contour_pair_f4(const DevParams& P)
+{
+    return (P.window == 16 && P.P <= 1024) ? 2 * (P.P + 2 * P.window + 14) : 0;
+}
+
 // Shared-memory carve-up of rollout_kernel (units: float4).
 //   [0, N)                         nominal thrusts u_nom[b]
 //   [N, N + trk)                   track data of the objective
@@ -37,6 +43,7 @@ size_t rollout_smem_bytes(const DevParams& P, const LaunchCfg& c)
         return f4 * sizeof(float4);
     }
     if (c.fused) f4 += (size_t)(c.block_threads / 32) * P.N + (3 * P.blocks_per_ctrl + 3) / 4;
+    if (c.packed && c.objective == OBJ_CONTOUR) f4 += contour_pair_f4(P);     // candidate pairs of nearest_rot4
     if (c.objective == OBJ_CONTOUR_PAPER)      // fifth column: its nominal + one accumulator row per warp
         f4 += ((size_t)(c.block_threads / 32 + 1) * P.N + 3) / 4;
     return f4 * sizeof(float4);
@@ -46,10 +53,54 @@ size_t rollout_smem_bytes(const DevParams& P, const LaunchCfg& c)
 // packed throughput variant: two samples per thread in fp32x2 registers (mppi_packed.cuh).
 // grid = (K / (2 blockDim.x), B); thread j of the grid row owns samples 2j and 2j+1.
 // ---------------------------------------------------------------------------------------------
+// ---------------------------------------------------------------------------------------------
+// Windowed nearest-vertex search of objective 2 for the packed kernel, FOUR candidates per round in packed fp32x2
+// arithmetic.  configs[3] x 64 was bound by issue slots (75 % busy) AND by the shared-memory pipe (0.72 wavefronts
+// per SM-cycle), two thirds of both being this search (profiles/README_r02c.md).  The candidates of the padded copy
+// (ContourCost::nearest_ext) are laid out a second time so that register PAIRS come straight out of 128-bit loads:
+//   xy2[j] = (x_j, x_{j+1}, y_j, y_{j+1})      z4[j] = (z_j, z_{j+1}, z_{j+2}, z_{j+3})
+// Per four candidates: 3 LDS.128 (12 bytes per candidate instead of 16), 6 FADD2 + 2 FMUL2 + 4 FFMA2 (instead of 24
+// scalar operations), then the four compare-and-selects in scan order.  Same rotation as nearest_rot (each lane starts
+// at the entry congruent to its lane number mod 8: conflict-free 128-bit loads), same distances (dx dx, then + dy dy,
+// then + dz dz), same strict comparison in the same order: the same minimiser, bit for bit.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ int nearest_rot4(const DevParams& P, const float4* __restrict__ xy2, const float4* __restrict__ z4,
+                                            const int centre, const float px, const float py, const float pz)
+{
+    constexpr int W = 16, n = 2 * W + 1, PAD = ContourCost::kExtPad;
+    const int ws = centre + PAD;                             // window start in the padded copy
+    const int r = (ws - (int)(threadIdx.x & 7)) & 7;
+    const int jb = ws - r;
+    const float2 PX = bc2(px), PY = bc2(py), PZ = bc2(pz);
+    const float inf = __int_as_float(0x7f800000);
+    float best = inf;
+    int ob = W + r;
+#pragma unroll
+    for (int o = 0; o < n + PAD; o += 4) {
+        const float4 a0 = xy2[jb + o], a1 = xy2[jb + o + 2], zz = z4[jb + o];
+        const float2 dx0 = sub2(PX, make_float2(a0.x, a0.y)), dy0 = sub2(PY, make_float2(a0.z, a0.w)), dz0 = sub2(PZ, make_float2(zz.x, zz.y));
+        const float2 dx1 = sub2(PX, make_float2(a1.x, a1.y)), dy1 = sub2(PY, make_float2(a1.z, a1.w)), dz1 = sub2(PZ, make_float2(zz.z, zz.w));
+        const float2 e0 = fma2(dz0, dz0, fma2(dy0, dy0, mul2(dx0, dx0)));
+        const float2 e1 = fma2(dz1, dz1, fma2(dy1, dy1, mul2(dx1, dx1)));
+        float d[4] = {e0.x, e0.y, e1.x, e1.y};
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int oo = o + q;
+            if (oo < PAD) d[q] = oo >= r ? d[q] : inf;
+            if (oo >= n) d[q] = oo <= r + 2 * W ? d[q] : inf;
+            if (d[q] < best) { best = d[q]; ob = oo; }
+        }
+    }
+    int i = centre + (ob - r) - W;
+    if (P.closed) { if (i < 0) i += P.P; else if (i >= P.P) i -= P.P; }
+    return i;
+}
+
 template <int OBJ, int MATH, bool SYMZ>
 __device__ __forceinline__ void rollout_cost2(const DevParams& P, const StepArgs& A, const float4* s_unom,
                                               const float4* s_trk, State2 x, int start, int contour_i0,
-                                              uint32_t k0, uint32_t b, float4* du_out, float& Ja, float& Jb)
+                                              uint32_t k0, uint32_t b, float4* du_out, float& Ja, float& Jb,
+                                              const float4* s_xy2 = nullptr, const float4* s_z4 = nullptr)
 {
     const int N = P.N;
     Ja = 0.0f; Jb = 0.0f;
@@ -82,8 +133,16 @@ __device__ __forceinline__ void rollout_cost2(const DevParams& P, const StepArgs
             pb.step(P, s_trk, s_front, lane_state<1>(x), t);
         }
         if (OBJ == OBJ_CONTOUR) {
-            Ja += ca.template step<true>(P, s_trk, lane_state<0>(x));     // conflict-free scan (nearest_rot)
-            Jb += cb.template step<true>(P, s_trk, lane_state<1>(x));
+            if (s_xy2) {                                                  // four candidates per round (nearest_rot4)
+                const State xa = lane_state<0>(x), xb = lane_state<1>(x);
+                ca.idx = nearest_rot4(P, s_xy2, s_z4, ca.idx, xa.px, xa.py, xa.pz);
+                cb.idx = nearest_rot4(P, s_xy2, s_z4, cb.idx, xb.px, xb.py, xb.pz);
+                Ja += ca.step_found(P, s_trk, xa.px, xa.py, xa.pz, xa.ox * xa.ox + xa.oy * xa.oy + xa.oz * xa.oz);
+                Jb += cb.step_found(P, s_trk, xb.px, xb.py, xb.pz, xb.ox * xb.ox + xb.oy * xb.oy + xb.oz * xb.oz);
+            } else {
+                Ja += ca.template step<true>(P, s_trk, lane_state<0>(x));     // conflict-free scan (nearest_rot)
+                Jb += cb.template step<true>(P, s_trk, lane_state<1>(x));
+            }
         }
     }
     if (OBJ == OBJ_GATE) {
@@ -120,15 +179,30 @@ __global__ void __launch_bounds__(MPPI_PK_THREADS, MPPI_PK_MINB) rollout2_kernel
     stage_inputs<OBJ>(P, A, b, start, s_unom, s_trk);
     __syncthreads();
 
+    // objective 2: the candidates once more as register-pair rows for nearest_rot4 (after the combine scratch)
+    float4* s_xy2 = nullptr; float4* s_z4 = nullptr;
+    if (OBJ == OBJ_CONTOUR && contour_pair_f4(P) > 0) {
+        const int L = P.P + 2 * P.window + 14;
+        const float4* ext = s_trk + 2 * P.P;
+        s_xy2 = FUSED ? reinterpret_cast<float4*>(s_pair) + (3 * P.blocks_per_ctrl + 3) / 4 : s_acc;      // (two-pass: no combine scratch)
+        s_z4 = s_xy2 + L;
+        for (int j = tid; j < L; j += blockDim.x) {
+            const float4 e0 = ext[j], e1 = ext[min(j + 1, L - 1)], e2 = ext[min(j + 2, L - 1)], e3 = ext[min(j + 3, L - 1)];
+            const float far = 1e30f;                                   // beyond the copy: never the minimum
+            s_xy2[j] = make_float4(e0.x, j + 1 < L ? e1.x : far, e0.y, j + 1 < L ? e1.y : far);
+            s_z4[j] = make_float4(e0.z, j + 1 < L ? e1.z : far, j + 2 < L ? e2.z : far, j + 3 < L ? e3.z : far);
+        }
+    }
     const State x0 = load_state(A.x0 + 13 * b);
     const int i0 = OBJ == OBJ_CONTOUR ? contour_start_index(P, s_trk, start, x0, s_red) : 0;
+    if (OBJ == OBJ_CONTOUR) __syncthreads();
     float Ja, Jb;
     const bool stored = FUSED ? keeps_du<STORE_DU>(A, b) : STORE_DU;
     float4* const du_out = stored ? A.du + (size_t)b * N * P.K + k0 : nullptr;
     if (OBJ != OBJ_CONTOUR && P.gyz == 0.0f)       // (the contouring search is bound by shared memory) Jx == Jy: the yaw-rate derivative is constant over the step (rk4_step2<true>)
         rollout_cost2<OBJ, MATH, true>(P, A, s_unom, s_trk, splat_state(x0), start, i0, (uint32_t)k0, (uint32_t)b, du_out, Ja, Jb);
     else
-        rollout_cost2<OBJ, MATH, false>(P, A, s_unom, s_trk, splat_state(x0), start, i0, (uint32_t)k0, (uint32_t)b, du_out, Ja, Jb);
+        rollout_cost2<OBJ, MATH, false>(P, A, s_unom, s_trk, splat_state(x0), start, i0, (uint32_t)k0, (uint32_t)b, du_out, Ja, Jb, s_xy2, s_z4);
     Ja = sanitize_cost(Ja); Jb = sanitize_cost(Jb);
     *reinterpret_cast<float2*>(A.cost + (size_t)b * P.K + k0) = make_float2(Ja, Jb);
 
