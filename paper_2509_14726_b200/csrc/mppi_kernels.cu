@@ -39,7 +39,7 @@ size_t rollout_smem_bytes(const DevParams& P, const LaunchCfg& c)
     if (c.lat_consumers > 0) {
         f4 += (size_t)P.N * (32 * c.lat_consumers + 1) + 32 + (3 * P.blocks_per_ctrl + 3) / 4;
         if (c.objective == OBJ_CONTOUR && c.lat_split)   // rollout warps -> search warps: positions [N][32 C], costs [32 C], mbarriers
-            f4 += (size_t)P.N * 32 * c.lat_consumers + 8 * c.lat_consumers + (c.lat_consumers * lat_chunks(P.N) + 1) / 2;
+            f4 += (size_t)P.N * 32 * c.lat_consumers + 8 * c.lat_consumers + (c.lat_consumers * lat_chunks(P.N) + 1) / 2 + contour_pair_f4(P);
         return f4 * sizeof(float4);
     }
     if (c.fused) f4 += (size_t)(c.block_threads / 32) * P.N + (3 * P.blocks_per_ctrl + 3) / 4;
@@ -330,6 +330,20 @@ __global__ void __launch_bounds__(kLatThreads, 2) rollout_lat_kernel(const DevPa
         uint64_t* bar_p = reinterpret_cast<uint64_t*>(s_Jc + S);                                   // [C][chunks]
         const int nch = lat_chunks(N);
         for (int i = tid; i < C * nch; i += kLatThreads) mbar_init(bar_p + i, 32);
+        // the candidates once more as register-pair rows for nearest_rot4 (after the barriers, 16-byte aligned)
+        float4* s_xy2 = nullptr; float4* s_z4 = nullptr;
+        if (contour_pair_f4(P) > 0) {
+            const int L = P.P + 2 * P.window + 14;
+            const float4* ext = s_trk + 2 * P.P;
+            s_xy2 = reinterpret_cast<float4*>(bar_p + 2 * ((C * nch + 1) / 2));
+            s_z4 = s_xy2 + L;
+            for (int j = tid; j < L; j += kLatThreads) {
+                const float4 e0 = ext[j], e1 = ext[min(j + 1, L - 1)], e2 = ext[min(j + 2, L - 1)], e3 = ext[min(j + 3, L - 1)];
+                const float far = 1e30f;
+                s_xy2[j] = make_float4(e0.x, j + 1 < L ? e1.x : far, e0.y, j + 1 < L ? e1.y : far);
+                s_z4[j] = make_float4(e0.z, j + 1 < L ? e1.z : far, j + 2 < L ? e2.z : far, j + 3 < L ? e3.z : far);
+            }
+        }
         __syncthreads();
         if (warp < C) {
             State x = x0;
@@ -348,7 +362,12 @@ __global__ void __launch_bounds__(kLatThreads, 2) rollout_lat_kernel(const DevPa
                 const int t1 = min(N, (c + 1) * kLatChunk);
                 for (int t = c * kLatChunk; t < t1; ++t) {
                     const float4 q = s_pos[t * S + sid];
-                    Jc += cc.step_at(P, s_trk, q.x, q.y, q.z, q.w);
+                    if (s_xy2) {
+                        cc.idx = nearest_rot4(P, s_xy2, s_z4, cc.idx, q.x, q.y, q.z);
+                        Jc += cc.step_found(P, s_trk, q.x, q.y, q.z, q.w);
+                    } else {
+                        Jc += cc.step_at(P, s_trk, q.x, q.y, q.z, q.w);
+                    }
                 }
             }
             s_Jc[sid] = Jc;
