@@ -43,7 +43,7 @@ L2_FLUSH_BYTES = 256 << 20
 # cuobjdump -sass of rollout_kernel<OBJ_GATE, fast math>): 154 FFMA (53 with three register operands, 101 with a
 # constant operand), 67 FMUL, 44 FADD, 20 Philox half-rounds (IMAD.WIDE + LOP3), 11 MUFU, 8 FMNMX, 7 LDS.128.
 GATE_LOOP_MIX = {"ffma_rrr": 53, "ffma_const": 101, "fmul": 67, "fadd": 44, "philox_half_round": 20, "mufu": 11, "fmnmx": 8, "lds": 7}
-NCU_DRAM_BYTES_PER_LAUNCH = 51968     # rollout_pipe_kernel<gate>, cfg1: 52.0 KB read + 0 B written (profiles/README_r02c.md, ncu_details_pipe_r02.txt)
+NCU_DRAM_BYTES_PER_LAUNCH = 55552     # rollout_pipe_kernel<gate>, cfg1: 55.6 KB read + 0 B written (profiles/README_r02e.md, ncu_details_pipe_r02e.txt)
 
 
 def dist_env():
@@ -444,7 +444,7 @@ def run_ours(args):
                          "peak_how": f"{sm} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 x clocks.max.sm (B200_PROFILING.md)",
                          "peak_measured_ffma_tflops": fma_tflops, "frac_of_measured_ffma": ach / fma_tflops,
                          "regs_per_thread": info["regs_per_thread"], "spill_bytes": info["local_bytes_per_thread"],
-                         "traffic_source": "profiles/README_r02c.md (ncu --set full capture of this kernel, dram__bytes_read.sum + dram__bytes_write.sum per launch; not measured in this run)" if args.pipeline == 0 else None,
+                         "traffic_source": "profiles/README_r02e.md (ncu --set full capture of this kernel, dram__bytes_read.sum + dram__bytes_write.sum per launch; not measured in this run)" if args.pipeline == 0 else None,
                          "note": "K=4096 is 128 warps on 148 SMs: latency-bound by construction; see 'batched'"},
             "batched": {"workload": wl4.name, "K": P4["K"], "N": P4["N"], "B": P4["B"],
                         "value": units4 / (float(ms4.mean()) * 1e-3), "unit": UNIT, "ms_per_step": float(ms4.mean()),
