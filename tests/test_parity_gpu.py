@@ -505,6 +505,21 @@ def test_rate_model_divergent_rollouts_stay_finite():
         assert (g["cost"] == np.float32(3.0e38)).any(), "the case is meant to contain diverged samples"
 
 
+@pytest.mark.parametrize("opts", [dict(variant=4), dict(variant=1, block_threads=32), dict(variant=3, block_threads=32)],
+                         ids=["pipelined_512_blocks", "scalar_512_blocks", "packed_256_blocks"])
+@pytest.mark.parametrize("mixing", [False, True], ids=["lambda_as_stated", "mixing"])
+def test_many_blocks_per_controller(opts, mixing):
+    # more than 256 partials per controller take the block-wide form of the last-block combine (the per-warp form
+    # keeps at most eight (m, Z) pairs per lane); exactly 256 is its boundary
+    wl = W.replicate(W.cfg1(K=16384, N=10), 2, 0.2)
+    if mixing:
+        o0 = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, wl.seed, 0)
+        wl.params["lambda"] = float(np.float32(0.25 * np.median(o0["cost"].std(-1))))
+    g, o, st = run_case(wl, f"many blocks [{opts}, mixing {mixing}]", **opts)
+    if mixing:
+        assert st["ess"] > 100 and st["w"] <= Pz.W_ATOL and st["u"] <= Pz.U_ATOL
+
+
 def test_seed_high_word_reaches_the_key():
     wl = W.cfg0(K=64, N=5)
     wl.seed = (0xDEADBEEF << 32) | 0x12345678
