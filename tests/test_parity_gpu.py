@@ -520,6 +520,47 @@ def test_many_blocks_per_controller(opts, mixing):
         assert st["ess"] > 100 and st["w"] <= Pz.W_ATOL and st["u"] <= Pz.U_ATOL
 
 
+@pytest.mark.parametrize("sweep_seed", [20251105, 7, 99])
+def test_random_small_configurations_against_the_oracle(sweep_seed):
+    # seeded sweep over objective x input model x sizes x kernel variant x pipeline x math mode: every combination the
+    # library accepts must match the oracle; what it rejects must be rejected with MPPI_E_PARAM, not run wrongly
+    from paper_2509_14726_b200 import binding as Bd
+    rng = np.random.default_rng(sweep_seed)
+    ran, rejected = 0, 0
+    for case in range(60):
+        obj = int(rng.integers(0, 4))
+        rate = int(rng.integers(0, 2))
+        K = int(rng.choice([32, 64, 96, 128, 256, 512]))
+        N = int(rng.integers(1, 41))
+        B = int(rng.integers(1, 4))
+        make = (W.stress_gate, W.cfg2, W.cfg3, W.stress_gate_paper)[obj]
+        wl = make(K=K, N=N)
+        if obj == 3:
+            wl.params["near_mode"] = int(rng.integers(0, 2))
+        if rate:
+            wl = W._rate_model(wl, wl.name + "_rate")
+        wl = W.replicate(wl, B, 0.2)
+        if obj == 2:
+            wl.start[:] = rng.integers(-1, 500, B)               # hint or global search
+        opts = dict(variant=int(rng.choice([0, 1, 2, 3, 4])), pipeline=int(rng.integers(0, 2)), fast_math=int(rng.integers(0, 2)))
+        if rng.integers(0, 3) == 0:
+            opts["block_threads"] = int(rng.choice([32, 64, 128]))
+        tag = f"random case {sweep_seed}/{case}: obj {obj} rate {rate} K {K} N {N} B {B} {opts}"
+        try:
+            m = Pz.make_ctx(wl, **opts)
+            x0, start, u = Pz.to_dev(wl)
+            g = Pz.gpu_step(m, x0, start, u, wl.seed, case)
+        except Bd.MppiError as e:
+            assert e.status == -2, tag                           # MPPI_E_PARAM: an unsupported combination
+            rejected += 1
+            continue
+        o = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, wl.seed, case, want_du=True)
+        Pz.compare(tag, g, o, wl.params["lambda"], obj in (0, 3))
+        m.close()
+        ran += 1
+    assert ran >= 30 and rejected >= 3, (ran, rejected)
+
+
 def test_seed_high_word_reaches_the_key():
     wl = W.cfg0(K=64, N=5)
     wl.seed = (0xDEADBEEF << 32) | 0x12345678
