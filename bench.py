@@ -358,6 +358,18 @@ def run_ours(args):
         torch.cuda.synchronize()
         chain_ms = np.array([a.elapsed_time(b) for a, b in zip(ce0, ce1)])
         mg.close()
+        # the same chain as plain launches: the pipelined kernel chains them by programmatic dependent launch
+        for _ in range(5):
+            ug.copy_(u0_dev); m.optimize(x0, start, ug, wl.seed, 0, n_chain, cost=cost, weights=w)
+        torch.cuda.synchronize()
+        for i in range(50):
+            flush()
+            ug.copy_(u0_dev)
+            ce0[i].record()
+            m.optimize(x0, start, ug, wl.seed, 0, n_chain, cost=cost, weights=w)
+            ce1[i].record()
+        torch.cuda.synchronize()
+        chain_pdl_ms = np.array([a.elapsed_time(b) for a, b in zip(ce0, ce1)])
 
         # ---- the batched configuration (configs[4] shape): where the FP32 roofline is reachable
         wl4 = W.cfg4()
@@ -461,6 +473,9 @@ def run_ours(args):
                                               "timer": "the same call returning u_new, the K costs and the K weights (what north_star's mppi_step returns), all written by the kernel into mapped host memory"}},
             "optimize_chain": {"iterations": int(n_chain), "us_per_chain_p50": float(np.median(chain_ms) * 1e3),
                                "us_per_iteration": float(np.median(chain_ms) * 1e3 / n_chain),
+                               "programmatic_dependent_launch": {"us_per_chain_p50": float(np.median(chain_pdl_ms) * 1e3),
+                                                                 "us_per_iteration": float(np.median(chain_pdl_ms) * 1e3 / n_chain),
+                                                                 "what": "the same chain as plain stream launches (use_graph = 0): iteration i + 1 is launched with the programmatic-stream-serialization attribute, starts while iteration i combines, and waits (griddepcontrol.wait) before it reads the nominal"},
                                "what": "configs[1] as stated: 10 warm-started iterations at a fixed x0 through mppi_optimize, one CUDA-graph launch per chain (use_graph = 1), CUDA events around the launch, L2 flushed before each chain"},
             "gpu_launches": int(launches),
             "roofline": {"bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,

@@ -622,7 +622,7 @@ static StepArgs make_args(mppi_ctx* c, const float* x0, const int32_t* start, co
     a.du = c->d_du; a.partials = c->d_partials; a.headers = c->d_headers; a.counters = c->d_counters;
     a.hint = (c->cfg.fused && !c->cfg.pipe && !c->cfg.lat_consumers && c->d_du) ? c->d_hint : nullptr;
     a.prev_front = c->d_prev_front; a.v_nom = c->d_v_nom; a.v_new = c->d_v_new;
-    a.done_flag = nullptr; a.done_value = 0;
+    a.done_flag = nullptr; a.done_value = 0; a.pdl = 0;
 #ifdef MPPI_TIMELINE
     {
         static unsigned long long* tl = nullptr;      // profiling builds only: one buffer, read back by the probe script
@@ -638,9 +638,9 @@ static StepArgs make_args(mppi_ctx* c, const float* x0, const int32_t* start, co
     return a;
 }
 
-static int enqueue_iteration(mppi_ctx* c, const StepArgs& a, cudaStream_t s)
+static int enqueue_iteration(mppi_ctx* c, const StepArgs& a, cudaStream_t s, bool pdl = false)
 {
-    CK(c, launch_rollout(c->dp, a, c->cfg, s));
+    CK(c, launch_rollout(c->dp, a, c->cfg, s, pdl));
     c->launches += 1;
     if (!c->cfg.fused) {
         CK(c, launch_reduce(c->dp, a, s));
@@ -737,8 +737,14 @@ extern "C" int mppi_optimize(mppi_ctx* c, const float* d_x0, const int32_t* d_st
     for (int i = 0; i < n_iters; ++i)
         args.push_back(make_args(c, d_x0, d_start, d_u, seed, iter0 + (uint32_t)i, d_u, d_cost, d_weights));
     if (c->prm.use_graph) return graph_run(c, c->g_opt, args, (cudaStream_t)stream);
+    // plain launches.  The pipelined kernel chains its iterations by programmatic dependent launch: every iteration
+    // lets the next one start on the SMs once its rollouts are done, and the next one stages its track and draws the
+    // state-independent half of its noise while this one publishes and combines, then waits (griddepcontrol.wait)
+    // before it reads the nominal.  Bit-identical results (tests: optimize == chain of steps).
+    const bool pdl = c->cfg.pipe && !c->cfg.rate && c->cfg.fused && n_iters > 1;
     for (int i = 0; i < n_iters; ++i) {
-        rc = enqueue_iteration(c, args[i], (cudaStream_t)stream);
+        if (pdl) args[i].pdl = (i > 0 ? 1 : 0) | (i + 1 < n_iters ? 2 : 0);
+        rc = enqueue_iteration(c, args[i], (cudaStream_t)stream, pdl && i > 0);
         if (rc) return rc;
     }
     return MPPI_OK;

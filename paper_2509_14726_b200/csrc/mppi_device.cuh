@@ -56,6 +56,10 @@ struct StepArgs {
     const float* v_nom;    // [B][N] nominal progress accelerations (OBJ_CONTOUR_PAPER), or nullptr
     float* v_new;          // [B][N] updated ones
     const int* prev_front; // [B][N+1] or nullptr: previous-iteration "in front" flags (paper's J_gate, Fig. 2)
+    int pdl;               // pipelined kernel only: bit 0 = this launch carries the programmatic-stream-serialization
+                           // attribute: do everything that does not depend on the previous kernel in the stream (stage
+                           // the track, draw the normals), then griddepcontrol.wait before touching the nominal; bit 1 =
+                           // let a dependent launch start once this block's body-rate chain is done (mppi_optimize's chain)
     unsigned int* done_flag;   // mapped host word, or nullptr: set to done_value once every output of the
     unsigned int done_value;   // call is visible to the host (mppi_step_host polls it instead of a stream sync)
 #ifdef MPPI_TIMELINE
@@ -119,30 +123,50 @@ __device__ __forceinline__ float mufu_ex2(float x) { float y; asm("ex2.approx.ft
 // MATH = 0: IEEE-accurate library functions, in the oracle's operation order.
 // MATH = 1: MUFU lg2 / rsq / sin / cos.  The angle is taken as 2 pi (u2 - 1/2) in [-pi, pi), where the
 // MUFU error bound holds, and the sign flip cos(x - pi) = -cos x is folded into the final fma.
+// The pair in two halves, so that the pipelined kernel can draw the state-independent part (Philox, radius, angle)
+// before the nominal is known: perturb_pair = perturb_finish(perturb_prepare), operation for operation.
+//   MATH = 0: f0 = rad cos, f1 = rad sin          -> a = fma(sigma, f0, una)
+//   MATH = 1: f0 = sigma rad, f1 = angle          -> a = fma(-f0, MUFU.COS(f1), una)
 template <int MATH>
-__device__ __forceinline__ void perturb_pair(uint32_t ra, uint32_t rb, float sigma, float bm_k, float una, float unb,
-                                             float& a, float& b)
+__device__ __forceinline__ void perturb_prepare(uint32_t ra, uint32_t rb, float bm_k, float& f0, float& f1)
 {
     if (MATH == 0) {
         const float u1 = u01(ra), u2 = u01(rb);
         const float rad = sqrtf(-2.0f * logf(u1));
         float s, c;
         sincospif(2.0f * u2, &s, &c);
-        a = fmaf(sigma, rad * c, una);
-        b = fmaf(sigma, rad * s, unb);
+        f0 = rad * c;
+        f1 = rad * s;
     } else {
         // rad = sigma sqrt(-2 ln u1) = sqrt(bm_k lg2 u1), bm_k = -2 ln2 sigma^2 from the host: one multiply
         // and MUFU.SQRT.
-        const float rad = mufu_sqrt(mufu_lg2(u01(ra)) * bm_k);
+        f0 = mufu_sqrt(mufu_lg2(u01(ra)) * bm_k);
         // ang = 2 pi (u2 - 1/2) = 2 pi m2 - 3 pi + 2 pi 2^-24 with m2 = 1 + (rb >> 9) 2^-23 in [1, 2): ONE fma
         // straight from the mantissa trick.  The additive constant is the float next to
         // -3 pi + 2 pi 2^-24 - 1.5 (fl(2 pi) - 2 pi), which centres the error of fl(2 pi) m2 on m2 = 1.5:
         // |angle error| <= 3.4e-7 rad, below the MUFU.SIN / MUFU.COS error itself.
         const float m2 = __uint_as_float(0x3f800000u | (rb >> 9));
-        const float ang = fmaf(m2, 6.283185307179586f, -9.42477798461914f);
-        a = fmaf(-rad, mufu_cos(ang), una);
-        b = fmaf(-rad, mufu_sin(ang), unb);
+        f1 = fmaf(m2, 6.283185307179586f, -9.42477798461914f);
     }
+}
+template <int MATH>
+__device__ __forceinline__ void perturb_finish(float f0, float f1, float sigma, float una, float unb, float& a, float& b)
+{
+    if (MATH == 0) {
+        a = fmaf(sigma, f0, una);
+        b = fmaf(sigma, f1, unb);
+    } else {
+        a = fmaf(-f0, mufu_cos(f1), una);
+        b = fmaf(-f0, mufu_sin(f1), unb);
+    }
+}
+template <int MATH>
+__device__ __forceinline__ void perturb_pair(uint32_t ra, uint32_t rb, float sigma, float bm_k, float una, float unb,
+                                             float& a, float& b)
+{
+    float f0, f1;
+    perturb_prepare<MATH>(ra, rb, bm_k, f0, f1);
+    perturb_finish<MATH>(f0, f1, sigma, una, unb, a, b);
 }
 
 // Perturbed, clamped rotor thrusts of one (sample, step) [R-8]: T = clamp(u_nom + sigma z).

@@ -27,7 +27,7 @@ const void* rollout_kernel_ptr(const LaunchCfg& c);
 const void* reduce_kernel_ptr();
 const void* sim_kernel_ptr();
 
-cudaError_t launch_rollout(const DevParams& P, const StepArgs& A, const LaunchCfg& c, cudaStream_t s);
+cudaError_t launch_rollout(const DevParams& P, const StepArgs& A, const LaunchCfg& c, cudaStream_t s, bool pdl = false);
 cudaError_t launch_reduce(const DevParams& P, const StepArgs& A, cudaStream_t s);
 cudaError_t launch_sim_progress(const DevParams& P, float* x, const float* u_new, float* u_nom_next,
                                 const float* v_new, float* v_nom_next, cudaStream_t s);

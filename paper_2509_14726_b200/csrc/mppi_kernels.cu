@@ -8,6 +8,7 @@
 //   sim_kernel                                   step 8 (closed-loop glue)
 //
 // No tensor cores: nothing here is a contraction.
+#include <cstring>
 #include "mppi_internal.h"
 #include "mppi_rollout.cuh"
 #include "mppi_packed.cuh"
@@ -676,10 +677,22 @@ const void* rollout_kernel_ptr(const LaunchCfg& c)
 const void* reduce_kernel_ptr() { return reinterpret_cast<const void*>(reduce_kernel); }
 const void* sim_kernel_ptr() { return reinterpret_cast<const void*>(sim_kernel<OBJ_GATE>); }
 
-cudaError_t launch_rollout(const DevParams& P, const StepArgs& A, const LaunchCfg& c, cudaStream_t s)
+cudaError_t launch_rollout(const DevParams& P, const StepArgs& A, const LaunchCfg& c, cudaStream_t s, bool pdl)
 {
     const dim3 grid(P.blocks_per_ctrl, P.B), block(c.block_threads);
     if (c.rate) return launch_rate(P, A, c, s);
+    if (c.pipe && pdl) {
+        // programmatic dependent launch: this kernel may start before the previous kernel of the stream has finished;
+        // it orders itself with griddepcontrol.wait (StepArgs::pdl bit 0 must be set)
+        cudaLaunchConfig_t lc;
+        memset(&lc, 0, sizeof lc);
+        lc.gridDim = grid; lc.blockDim = block; lc.dynamicSmemBytes = c.smem_bytes; lc.stream = s;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        lc.attrs = at; lc.numAttrs = 1;
+        return cudaLaunchKernelEx(&lc, pick_pipe(c), P, A);
+    }
     if (c.pipe) pick_pipe(c)<<<grid, block, c.smem_bytes, s>>>(P, A);
     else if (c.lat_consumers > 0) pick_lat(c)<<<grid, block, c.smem_bytes, s>>>(P, A, c.lat_consumers | (c.lat_split << 8));
     else pick(c)<<<grid, block, c.smem_bytes, s>>>(P, A);

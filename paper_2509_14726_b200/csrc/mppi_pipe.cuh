@@ -107,11 +107,29 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
     uint64_t* bar_qe = bar_qf + D;
 
     if (tid == 0) MPPI_STAMP(A, 0);
+    // Programmatic dependent launch (mppi_optimize's chain): this kernel may have been started while the previous
+    // kernel of the stream is still in its tail.  Everything that kernel neither writes nor reads comes first -- the
+    // track, x0, the barriers and the state-independent half of the noise (Philox, radius, angle) -- then
+    // griddepcontrol.wait, then the nominal (the previous kernel's output) and the rest as always.
+    const bool pdl_wait = (A.pdl & 1) != 0;
     const int start = A.start[b];
-    stage_inputs<OBJ>(P, A, b, start, s_unom, s_trk);
+    if (pdl_wait) stage_track<OBJ>(P, A, b, start, s_trk);
+    else stage_inputs<OBJ>(P, A, b, start, s_unom, s_trk);
     for (int i = tid; i < nchunks + 4 * D; i += kPipeThreads)
         mbar_init(bar_T + i, i < nchunks ? 32 * min(C, N - i * C) : 32);
     const State x0 = load_state(A.x0 + 13 * b);
+    if (pdl_wait) {
+        if (warp >= 3)
+            for (int t = warp - 3; t < N; t += kPipeNoiseWarps) {
+                const uint4 r = philox4x32_10((uint32_t)(kbase + lane), (uint32_t)t, A.iter, (uint32_t)b, A.rk);
+                float4 f;
+                perturb_prepare<MATH>(r.x, r.y, P.bm_k, f.x, f.y);
+                perturb_prepare<MATH>(r.z, r.w, P.bm_k, f.z, f.w);
+                s_T[t * RS + lane] = f;
+            }
+        asm volatile("griddepcontrol.wait;" ::: "memory");
+        stage_nominal(P, A, b, s_unom);
+    }
     __syncthreads();
     const int i0 = OBJ == OBJ_CONTOUR ? contour_start_index(P, s_trk, start, x0, s_red) : 0;
     if (tid == 0) MPPI_STAMP(A, 1);
@@ -120,7 +138,16 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
         // ---- noise producers: step t is drawn by warp 3 + t % 5, one sample per lane (eq.(3)) ----
         for (int t = warp - 3; t < N; t += kPipeNoiseWarps) {
             const float4 un = s_unom[t];
-            const float4 T = sample_thrust<MATH>(P, A.rk, (uint32_t)(kbase + lane), (uint32_t)t, A.iter, (uint32_t)b, un);
+            float4 T;
+            if (pdl_wait) {                        // second half of the pair drawn before the wait: the same operations
+                const float4 f = s_T[t * RS + lane];
+                perturb_finish<MATH>(f.x, f.y, P.sigma, un.x, un.y, T.x, T.y);
+                perturb_finish<MATH>(f.z, f.w, P.sigma, un.z, un.w, T.z, T.w);
+                T.x = fminf(fmaxf(T.x, P.T_min), P.T_max); T.y = fminf(fmaxf(T.y, P.T_min), P.T_max);
+                T.z = fminf(fmaxf(T.z, P.T_min), P.T_max); T.w = fminf(fmaxf(T.w, P.T_min), P.T_max);
+            } else {
+                T = sample_thrust<MATH>(P, A.rk, (uint32_t)(kbase + lane), (uint32_t)t, A.iter, (uint32_t)b, un);
+            }
             s_T[t * RS + lane] = T;
             mbar_arrive(bar_T + t / C);
             if (lane == 0 && t == 0) MPPI_STAMP(A, 2);
@@ -177,6 +204,11 @@ __global__ void __launch_bounds__(kPipeThreads, 2) rollout_pipe_kernel(const Dev
             acc = fmaf(P.Qw, wx * wx + wy * wy + wz * wz, acc);
         }
         s_J[lane] = acc;
+        // the body-rate chain of this block is through: a dependent launch (the next iteration of mppi_optimize's chain)
+        // may start on the SMs.  Measured per iteration of the 10-iteration chain: trigger here 14.0 us, after all
+        // rollouts 14.8 us, at kernel start 15.7 us (its noise warps then compete with this kernel's chains); plain
+        // launches 16.1 us, one graph launch 14.3 us.
+        if (A.pdl & 2) asm volatile("griddepcontrol.launch_dependents;");
         if (lane == 0) MPPI_STAMP(A, 4);
     } else if (warp == 1) {
         // ---- Q: attitude.  q' = 1/2 q (x) (0, omega), renormalised once per step [R-5] ----

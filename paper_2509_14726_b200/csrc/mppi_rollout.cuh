@@ -61,13 +61,25 @@ __host__ __device__ inline int track_f4(const DevParams& P, int objective)
 }
 
 // Stage the nominal sequence of controller b and the objective's track data in shared memory.
+__device__ __forceinline__ void stage_nominal(const DevParams& P, const StepArgs& A, int b, float4* s_unom)
+{
+    const float4* un = reinterpret_cast<const float4*>(A.u_nom) + (size_t)b * P.N;
+    for (int t = threadIdx.x; t < P.N; t += blockDim.x) s_unom[t] = un[t];
+}
+template <int OBJ>
+__device__ __forceinline__ void stage_track(const DevParams& P, const StepArgs& A, int b, int start, float4* s_trk);
 template <int OBJ>
 __device__ __forceinline__ void stage_inputs(const DevParams& P, const StepArgs& A, int b, int start,
                                              float4* s_unom, float4* s_trk)
 {
+    stage_nominal(P, A, b, s_unom);
+    stage_track<OBJ>(P, A, b, start, s_trk);
+}
+// The objective's track data only (constant inputs: nothing a previous kernel of the stream writes).
+template <int OBJ>
+__device__ __forceinline__ void stage_track(const DevParams& P, const StepArgs& A, int b, int start, float4* s_trk)
+{
     const int tid = threadIdx.x, N = P.N;
-    const float4* un = reinterpret_cast<const float4*>(A.u_nom) + (size_t)b * N;
-    for (int t = tid; t < N; t += blockDim.x) s_unom[t] = un[t];
     if (OBJ == OBJ_GATE) {
         for (int i = tid; i < 4 * P.G; i += blockDim.x) s_trk[i] = P.gates[i];
     } else if (OBJ == OBJ_GATE_PAPER) {

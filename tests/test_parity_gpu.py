@@ -88,6 +88,35 @@ def test_cfg1_optimize_graph_equals_step_chain():
     m.close()
 
 
+@pytest.mark.parametrize("name,B", [("cfg1", 1), ("cfg2", 1), ("gate_paper", 2), ("stress_gate", 3)])
+@pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
+def test_optimize_chain_by_programmatic_dependent_launch_equals_the_steps(name, B, math):
+    # mppi_optimize without a graph chains the pipelined kernel's iterations by programmatic dependent launch: iteration
+    # i + 1 starts while iteration i publishes and combines, draws the state-independent half of its noise, then waits
+    # before it reads the nominal.  Must equal the chain of single steps bit for bit, repeatedly (a race would show as a
+    # run-to-run difference), and the last iteration must match the oracle fed with the chain's own nominal.
+    import torch
+    wl = W.replicate(W.ALL[name](), B, 0.2) if B > 1 else W.ALL[name]()
+    x0, start, u0 = Pz.to_dev(wl)
+    m = Pz.make_ctx(wl, variant=4, **math)
+    u = u0.clone()
+    n = 6
+    for it in range(n):
+        if it == n - 1:
+            u_in = u.cpu().numpy()
+        _, c_ref, w_ref = m.step(x0, start, u, wl.seed, it, u_new=u)
+    torch.cuda.synchronize()
+    for rep in range(5):
+        u2 = u0.clone()
+        _, c2, w2 = m.optimize(x0, start, u2, wl.seed, 0, n)
+        torch.cuda.synchronize()
+        assert torch.equal(u2, u) and torch.equal(c2, c_ref) and torch.equal(w2, w_ref), rep
+    o = Pz.oracle_step(wl, wl.x0, wl.start, u_in, wl.seed, n - 1, want_du=True)
+    g = dict(u_new=u2.cpu().numpy(), cost=c2.cpu().numpy(), weights=w2.cpu().numpy())
+    Pz.compare(f"optimize chain (PDL) {name} B{B} {math}", g, o, wl.params["lambda"], wl.params["objective"] in (0, 3))
+    m.close()
+
+
 @pytest.mark.parametrize("pipe", PIPES, ids=PIPE_IDS)
 @pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
 def test_cfg2_tracking(pipe, math):
