@@ -109,11 +109,21 @@ typedef enum {
                                     contouring; under MPPI_OBJ_CONTOUR_PAPER the path must fit in shared memory
                                     beside the rings (else mppi_step -> MPPI_E_PARAM; AUTO then stays on the
                                     throughput kernel)                                                      */
-    MPPI_VARIANT_PACKED = 3      /* throughput kernel with TWO samples per thread held in packed fp32x2
+    MPPI_VARIANT_PACKED = 3,     /* throughput kernel with TWO samples per thread held in packed fp32x2
                                     registers (sm_100a FFMA2); needs K % 64 == 0; costs are bit-identical
                                     to MPPI_VARIANT_THROUGHPUT.  Under input_model = 1: every objective but the
                                     search-based contouring, block_threads <= 128 (else MPPI_E_PARAM); AUTO
                                     takes it when B K / 32 >= 8 x the SM count                             */
+    MPPI_VARIANT_SCAN = 5        /* time-parallel latency kernel (eq.(2) PAPER.md:65-72 as a cascade of linear
+                                    recurrences): 512-thread blocks of 32 samples, every rollout split over 16
+                                    lanes ALONG THE HORIZON; body rates, attitude, velocity and position of the
+                                    chunks are joined by warp-shuffle scans (affine maps, quaternion products,
+                                    sums).  Needs input_model = 0, Jx == Jy (then the body-rate equations are
+                                    linear given the yaw rate), objective MPPI_OBJ_GATE, N <= 64, the fused
+                                    pipeline and block_threads 0 (else MPPI_E_PARAM).  Same RK4, same per-step
+                                    renormalisation, another association order: states equal the other kernels'
+                                    to rounding, not bit for bit.  AUTO takes it for such configurations when
+                                    B K / 32 <= the SM count                                                */
 } mppi_variant;
 
 /* Parameters of Alg. 1 (samples, horizon, lambda, Sigma) plus the model and cost

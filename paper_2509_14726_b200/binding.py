@@ -16,7 +16,7 @@ LIB_PATH = _HERE / "libmppi.so"
 
 OBJ_GATE, OBJ_TRACK, OBJ_CONTOUR, OBJ_GATE_PAPER, OBJ_CONTOUR_PAPER = 0, 1, 2, 3, 4
 PIPE_FUSED, PIPE_TWO_PASS = 0, 1
-VARIANT_AUTO, VARIANT_THROUGHPUT, VARIANT_LATENCY, VARIANT_PACKED, VARIANT_PIPELINED = 0, 1, 2, 3, 4
+VARIANT_AUTO, VARIANT_THROUGHPUT, VARIANT_LATENCY, VARIANT_PACKED, VARIANT_PIPELINED, VARIANT_SCAN = 0, 1, 2, 3, 4, 5
 
 EXPORTS = ["mppi_default_params", "mppi_create", "mppi_destroy", "mppi_set_gates",
            "mppi_set_reference", "mppi_set_path", "mppi_step", "mppi_optimize", "mppi_step_host",

@@ -15,9 +15,9 @@ from pathlib import Path
 HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 LIB = HERE / "libmppi.so"
-SOURCES = ["mppi_kernels.cu", "mppi_rate.cu", "mppi_api.cu", "mppi_peaks.cu", "mppi_static.cu"]
+SOURCES = ["mppi_kernels.cu", "mppi_rate.cu", "mppi_api.cu", "mppi_peaks.cu", "mppi_static.cu", "mppi_scan.cu"]
 HEADERS = [CSRC / "mppi_device.cuh", CSRC / "mppi_cost.cuh", CSRC / "mppi_internal.h",
-           CSRC / "mppi_rollout.cuh", CSRC / "mppi_packed.cuh", CSRC / "mppi_pipe.cuh", CSRC / "mppi_rate.cuh", CSRC / "mppi_pipe_rate.cuh",
+           CSRC / "mppi_rollout.cuh", CSRC / "mppi_packed.cuh", CSRC / "mppi_pipe.cuh", CSRC / "mppi_rate.cuh", CSRC / "mppi_pipe_rate.cuh", CSRC / "mppi_scan.cuh",
            HERE.parent / "include" / "mppi.h"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]

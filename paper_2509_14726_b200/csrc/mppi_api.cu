@@ -117,6 +117,14 @@ extern "C" int mppi_default_params(mppi_params* p)
 
 static bool finite_pos(float v) { return std::isfinite(v) && v > 0.0f; }
 
+// May the time-parallel kernel (mppi_scan.cuh) run this configuration?  Its body-rate scan needs the equations of
+// omega_x, omega_y to be linear given omega_z: Jx == Jy (then (Jx - Jy)/Jz = 0 and (Jy - Jz)/Jx = -(Jz - Jx)/Jy).
+static bool scan_capable(const mppi_params* p)
+{
+    return p->input_model == 0 && p->objective == MPPI_OBJ_GATE && p->Jx == p->Jy && p->N <= 64 &&
+           p->pipeline == MPPI_PIPE_FUSED && p->block_threads == 0 && p->K % 32 == 0;
+}
+
 static int validate(const mppi_params* p)
 {
 #define BAD(cond, msg) if (cond) return fail(nullptr, MPPI_E_PARAM, msg)
@@ -147,7 +155,10 @@ static int validate(const mppi_params* p)
                                   p->K % p->block_threads != 0),
         "block_threads must be 0 or a multiple of 32 in 32..256 that divides K");
     BAD((int64_t)p->K / 32 > 65535, "K too large");
-    BAD(p->variant < 0 || p->variant > 4, "unknown variant");
+    BAD(p->variant < 0 || p->variant > 5, "unknown variant");
+    BAD(p->variant == MPPI_VARIANT_SCAN && !scan_capable(p),
+        "the time-parallel variant needs input_model 0, objective MPPI_OBJ_GATE, Jx == Jy, N <= 64, the fused pipeline, "
+        "block_threads 0");
     BAD(p->variant == MPPI_VARIANT_PACKED &&
             (p->K % 64 != 0 || (p->block_threads && (p->block_threads > 128 || p->K % (2 * p->block_threads) != 0))),
         "the packed variant needs K % 64 == 0, block_threads <= 128 and 2*block_threads dividing K");
@@ -201,12 +212,17 @@ static bool rate_pipe_candidate(const mppi_params* p, int sm_count)
 // `avoid` (prepare(), when the preferred kernel does not fit in shared memory with the track that was set):
 // bit 0 = not the pipelined kernel, bit 1 = not the latency kernel either.
 static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, int* lat_consumers, int* packed, int* pipe,
-                       int avoid = 0)
+                       int* scan, int avoid = 0)
 {
     const int64_t warps = (int64_t)p->B * p->K / 32;
     *lat_consumers = 0;
     *packed = 0;
     *pipe = 0;
+    *scan = 0;
+    if (p->variant == MPPI_VARIANT_SCAN) {          // validate() has checked scan_capable
+        *scan = 1; *block_threads = 512;
+        return;
+    }
     if (p->input_model == 1) {                     // thrust-rate model: its own kernels (mppi_rate.cu)
         // the scalar shape; whether the pipelined latency kernel takes over is decided in prepare(), once the
         // track (and with it the shared-memory footprint) is known -- see rate_pipe_candidate
@@ -267,7 +283,7 @@ static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, i
 
 static int blocks_per_ctrl_of(const mppi_params* p, const LaunchCfg& cfg)
 {
-    return cfg.pipe ? p->K / 32 : cfg.lat_consumers ? p->K / (32 * cfg.lat_consumers)
+    return (cfg.pipe || cfg.scan) ? p->K / 32 : cfg.lat_consumers ? p->K / (32 * cfg.lat_consumers)
                                                     : p->K / (cfg.block_threads * (cfg.packed ? 2 : 1));
 }
 
@@ -353,7 +369,7 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     cfg.objective = p->objective; cfg.fast_math = p->fast_math ? 1 : 0;
     cfg.fused = p->pipeline == MPPI_PIPE_FUSED;
     cfg.store_du = (!cfg.fused || p->store_noise) ? 1 : 0;
-    pick_shape(p, c->sm_count, &cfg.block_threads, &cfg.lat_consumers, &cfg.packed, &cfg.pipe);
+    pick_shape(p, c->sm_count, &cfg.block_threads, &cfg.lat_consumers, &cfg.packed, &cfg.pipe, &cfg.scan);
     cfg.rate = p->input_model == 1;
     c->xdim = p->objective == MPPI_OBJ_CONTOUR_PAPER ? 19 : cfg.rate ? 17 : 13;
     d.blocks_per_ctrl = blocks_per_ctrl_of(p, cfg);
@@ -578,7 +594,7 @@ static int prepare(mppi_ctx* c)
         for (int avoid : {1, 3}) {
             if (avoid == 1 && !c->cfg.pipe) continue;
             LaunchCfg nc = c->cfg;
-            pick_shape(&c->prm, c->sm_count, &nc.block_threads, &nc.lat_consumers, &nc.packed, &nc.pipe, avoid);
+            pick_shape(&c->prm, c->sm_count, &nc.block_threads, &nc.lat_consumers, &nc.packed, &nc.pipe, &nc.scan, avoid);
             DevParams nd = c->dp;
             nd.blocks_per_ctrl = blocks_per_ctrl_of(&c->prm, nc);
             const size_t nn = rollout_smem_bytes(nd, nc);
@@ -592,7 +608,7 @@ static int prepare(mppi_ctx* c)
     }
     // fused throughput kernels: scratch for dU, used only in iterations that follow one with many weight-carrying
     // samples (StepArgs::hint).  If the allocation fails the kernels simply keep re-deriving the noise.
-    if (c->cfg.fused && !c->cfg.pipe && !c->cfg.lat_consumers && c->prm.objective != MPPI_OBJ_CONTOUR_PAPER && !c->d_du &&
+    if (c->cfg.fused && !c->cfg.pipe && !c->cfg.scan && !c->cfg.lat_consumers && c->prm.objective != MPPI_OBJ_CONTOUR_PAPER && !c->d_du &&
         !c->du_tried) {
         c->du_tried = true;
         // at most 1 GiB of such scratch (configs[4]: 210 MB); larger batches keep re-deriving the noise
@@ -620,7 +636,7 @@ static StepArgs make_args(mppi_ctx* c, const float* x0, const int32_t* start, co
     StepArgs a;
     a.x0 = x0; a.start = start; a.u_nom = u_nom; a.u_new = u_new; a.cost = cost; a.weights = w;
     a.du = c->d_du; a.partials = c->d_partials; a.headers = c->d_headers; a.counters = c->d_counters;
-    a.hint = (c->cfg.fused && !c->cfg.pipe && !c->cfg.lat_consumers && c->d_du) ? c->d_hint : nullptr;
+    a.hint = (c->cfg.fused && !c->cfg.pipe && !c->cfg.scan && !c->cfg.lat_consumers && c->d_du) ? c->d_hint : nullptr;
     a.prev_front = c->d_prev_front; a.v_nom = c->d_v_nom; a.v_new = c->d_v_new;
     a.done_flag = nullptr; a.done_value = 0; a.pdl = 0;
 #ifdef MPPI_TIMELINE
@@ -911,7 +927,7 @@ extern "C" int mppi_get_info(mppi_ctx* c, mppi_info* o)
     o->sm_count = c->sm_count;
     o->kernels_per_step = c->cfg.fused ? 1 : 2;
     o->samples_per_thread = c->cfg.packed ? 2 : 1;
-    o->rollout_warps_per_block = c->cfg.pipe ? (c->cfg.rate ? 5 : 3) : c->cfg.lat_consumers ? c->cfg.lat_consumers : c->cfg.block_threads / 32;
+    o->rollout_warps_per_block = c->cfg.scan ? 16 : c->cfg.pipe ? (c->cfg.rate ? 5 : 3) : c->cfg.lat_consumers ? c->cfg.lat_consumers : c->cfg.block_threads / 32;
     o->l2_bytes = c->l2_bytes;
     o->scratch_bytes = c->scratch_bytes;
     return MPPI_OK;

@@ -36,6 +36,7 @@ __host__ __device__ inline int contour_pair_f4(const DevParams& P)
 size_t rollout_smem_bytes(const DevParams& P, const LaunchCfg& c)
 {
     size_t f4 = (size_t)P.N + track_f4(P, c.objective) + 16;
+    if (c.scan) return scan_smem_bytes(P, c);
     if (c.pipe) return (f4 + (c.rate ? pipe_rate_extra_f4(P.N, P.blocks_per_ctrl, c.objective == OBJ_CONTOUR_PAPER, P.pipe_d, P.pipe_df) : pipe_extra_f4(P.N, P.blocks_per_ctrl))) * sizeof(float4);
     if (c.lat_consumers > 0) {
         f4 += (size_t)P.N * (32 * c.lat_consumers + 1) + 32 + (3 * P.blocks_per_ctrl + 3) / 4;
@@ -671,6 +672,7 @@ static PipeFn pick_pipe(const LaunchCfg& c)
 const void* rollout_kernel_ptr(const LaunchCfg& c)
 {
     if (c.rate) return rate_kernel_ptr(c);
+    if (c.scan) return scan_kernel_ptr(c);
     if (c.pipe) return reinterpret_cast<const void*>(pick_pipe(c));
     return c.lat_consumers > 0 ? reinterpret_cast<const void*>(pick_lat(c)) : reinterpret_cast<const void*>(pick(c));
 }
@@ -681,6 +683,7 @@ cudaError_t launch_rollout(const DevParams& P, const StepArgs& A, const LaunchCf
 {
     const dim3 grid(P.blocks_per_ctrl, P.B), block(c.block_threads);
     if (c.rate) return launch_rate(P, A, c, s);
+    if (c.scan) return launch_scan(P, A, c, s);
     if (c.pipe && pdl) {
         // programmatic dependent launch: this kernel may start before the previous kernel of the stream has finished;
         // it orders itself with griddepcontrol.wait (StepArgs::pdl bit 0 must be set)
