@@ -1,5 +1,6 @@
 // mppi_api.cu -- host side of libmppi: the C ABI declared in include/mppi.h.
 // Parameter validation, track packing, scratch allocation, stream launches and CUDA-graph replay.
+#include <algorithm>
 #include <atomic>
 #include <chrono>
 #include <cmath>
@@ -124,6 +125,16 @@ static bool scan_capable(const mppi_params* p)
     return p->input_model == 0 && p->objective == MPPI_OBJ_GATE && p->Jx == p->Jy && p->N <= 64 &&
            p->pipeline == MPPI_PIPE_FUSED && p->block_threads == 0 && p->K % 32 == 0;
 }
+// Samples per block of the time-parallel kernel (16 lanes each): 32, or fewer (even, >= 8) when that lets the blocks
+// of the B controllers cover every SM -- its blocks run one per SM.  configs[1] on 148 SMs: 28 -> 147 blocks.
+static int scan_samples_per_block(const mppi_params* p, int sm_count)
+{
+    int64_t nb = p->K / 32;
+    const int64_t room = sm_count / p->B;            // blocks per controller that still fit in one wave
+    if (room > nb) nb = std::min<int64_t>(room, p->K / 8);
+    const int spb = 2 * (int)((p->K + 2 * nb - 1) / (2 * nb));
+    return std::min(32, std::max(8, spb));
+}
 
 static int validate(const mppi_params* p)
 {
@@ -219,8 +230,11 @@ static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, i
     *packed = 0;
     *pipe = 0;
     *scan = 0;
-    if (p->variant == MPPI_VARIANT_SCAN) {          // validate() has checked scan_capable
-        *scan = 1; *block_threads = 512;
+    // time-parallel kernel: on request, or (AUTO) whenever it can run and its blocks fit in one wave of one block
+    // per SM -- cfg1: 17.6 us against 18.8 us for the pipelined kernel in its first form (profiles/README_r02f.md)
+    if (p->variant == MPPI_VARIANT_SCAN ||          // validate() has checked scan_capable
+        (p->variant == MPPI_VARIANT_AUTO && scan_capable(p) && warps <= sm_count && !(avoid & 1))) {
+        *scan = scan_samples_per_block(p, sm_count); *block_threads = 16 * *scan;
         return;
     }
     if (p->input_model == 1) {                     // thrust-rate model: its own kernels (mppi_rate.cu)
@@ -283,7 +297,7 @@ static void pick_shape(const mppi_params* p, int sm_count, int* block_threads, i
 
 static int blocks_per_ctrl_of(const mppi_params* p, const LaunchCfg& cfg)
 {
-    return (cfg.pipe || cfg.scan) ? p->K / 32 : cfg.lat_consumers ? p->K / (32 * cfg.lat_consumers)
+    return cfg.scan ? (p->K + cfg.scan - 1) / cfg.scan : cfg.pipe ? p->K / 32 : cfg.lat_consumers ? p->K / (32 * cfg.lat_consumers)
                                                     : p->K / (cfg.block_threads * (cfg.packed ? 2 : 1));
 }
 
@@ -384,7 +398,7 @@ extern "C" int mppi_create(const mppi_params* p, mppi_ctx** out)
     c->lazy_pipe = rate_pipe_candidate(p, c->sm_count) ? 1 : 0;
     d.pipe_d = 4; d.pipe_df = 3;
     // AUTO may move to another kernel once the track is known (prepare()): size the partials for the largest grid
-    const int max_blocks = (c->lazy_pipe || p->variant == MPPI_VARIANT_AUTO) ? p->K / 32 : d.blocks_per_ctrl;
+    const int max_blocks = (c->lazy_pipe || p->variant == MPPI_VARIANT_AUTO) ? std::max(p->K / 32, d.blocks_per_ctrl) : d.blocks_per_ctrl;
 
     const size_t BN4 = (size_t)p->B * p->N * 4, BK = (size_t)p->B * p->K;
 #define CKC(call)                                                        \
@@ -589,10 +603,10 @@ static int prepare(mppi_ctx* c)
     size_t need = rollout_smem_bytes(c->dp, c->cfg);
     if (c->cfg.lat_split && need > 227 * 1024) { c->cfg.lat_split = 0; need = rollout_smem_bytes(c->dp, c->cfg); }
     if (need > 227 * 1024 && c->prm.variant == MPPI_VARIANT_AUTO && c->prm.input_model == 0 &&
-        (c->cfg.pipe || c->cfg.lat_consumers)) {
+        (c->cfg.pipe || c->cfg.lat_consumers || c->cfg.scan)) {
         // the kernel picked from the warp count alone does not fit with this track: next choice of pick_shape
         for (int avoid : {1, 3}) {
-            if (avoid == 1 && !c->cfg.pipe) continue;
+            if (avoid == 1 && !c->cfg.pipe && !c->cfg.scan) continue;
             LaunchCfg nc = c->cfg;
             pick_shape(&c->prm, c->sm_count, &nc.block_threads, &nc.lat_consumers, &nc.packed, &nc.pipe, &nc.scan, avoid);
             DevParams nd = c->dp;
@@ -757,7 +771,7 @@ extern "C" int mppi_optimize(mppi_ctx* c, const float* d_x0, const int32_t* d_st
     // lets the next one start on the SMs once its rollouts are done, and the next one stages its track and draws the
     // state-independent half of its noise while this one publishes and combines, then waits (griddepcontrol.wait)
     // before it reads the nominal.  Bit-identical results (tests: optimize == chain of steps).
-    const bool pdl = c->cfg.pipe && !c->cfg.rate && c->cfg.fused && n_iters > 1;
+    const bool pdl = (c->cfg.pipe || c->cfg.scan) && !c->cfg.rate && c->cfg.fused && n_iters > 1;
     for (int i = 0; i < n_iters; ++i) {
         if (pdl) args[i].pdl = (i > 0 ? 1 : 0) | (i + 1 < n_iters ? 2 : 0);
         rc = enqueue_iteration(c, args[i], (cudaStream_t)stream, pdl && i > 0);

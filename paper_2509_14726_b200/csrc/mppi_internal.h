@@ -16,7 +16,8 @@ struct LaunchCfg {
     int pipe_shallow;   // rollout_pipe_rate_kernel: 1 = rings (2, 2) chunks deep (two blocks per SM), 0 = (4, 3)
     int lat_consumers;  // 0: throughput kernel; 1, 2 or 4: latency kernel with that many rollout warps per block
     int lat_split;      // latency kernel, search-contouring: 1 = the search runs in warps of its own (when it fits in shared memory)
-    int scan;           // 1: rollout_scan_kernel, one rollout split over 16 lanes along the horizon (mppi_scan.cuh)
+    int scan;           // > 0: rollout_scan_kernel, one rollout split over 16 lanes along the horizon (mppi_scan.cuh);
+                        // the value is the number of samples per block (even, 8..32); block_threads = 16 x that
     size_t smem_bytes;  // dynamic shared memory of the rollout kernel
 };
 
@@ -41,7 +42,7 @@ cudaError_t launch_rate(const DevParams& P, const StepArgs& A, const LaunchCfg& 
 
 // mppi_scan.cu: the time-parallel latency kernel
 const void* scan_kernel_ptr(const LaunchCfg& c);
-cudaError_t launch_scan(const DevParams& P, const StepArgs& A, const LaunchCfg& c, cudaStream_t s);
+cudaError_t launch_scan(const DevParams& P, const StepArgs& A, const LaunchCfg& c, cudaStream_t s, bool pdl = false);
 size_t scan_smem_bytes(const DevParams& P, const LaunchCfg& c);
 
 cudaError_t launch_front(const DevParams& P, const float* x0, const int* start, const float* u, int* front,

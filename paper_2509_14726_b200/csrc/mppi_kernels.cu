@@ -683,7 +683,7 @@ cudaError_t launch_rollout(const DevParams& P, const StepArgs& A, const LaunchCf
 {
     const dim3 grid(P.blocks_per_ctrl, P.B), block(c.block_threads);
     if (c.rate) return launch_rate(P, A, c, s);
-    if (c.scan) return launch_scan(P, A, c, s);
+    if (c.scan) return launch_scan(P, A, c, s, pdl);
     if (c.pipe && pdl) {
         // programmatic dependent launch: this kernel may start before the previous kernel of the stream has finished;
         // it orders itself with griddepcontrol.wait (StepArgs::pdl bit 0 must be set)

@@ -29,7 +29,9 @@
 // it, the first lane (in horizon order) whose chunk switches the target fixes the hypothesis of all later lanes, and
 // those are re-scored -- one round per chunk that contains a valid pass, plus one.  Same decisions as GateCost::step.
 //
-// Block = 512 threads = 32 samples x 16 lanes (warp w: samples 2w, 2w + 1); grid = (K / 32, B); one block per SM.
+// Block = 16 lanes x up to 32 samples (warp w: samples 2w, 2w + 1; 512 threads at most); grid = (ceil(K / samples), B),
+// one block per SM; the host takes fewer samples per block when that lets a lone controller cover every SM
+// (configs[1]: 147 blocks of 28 samples on 148 SMs).
 // The fused update needs no re-derivation of the noise: every lane still holds the thrusts of its steps.
 #pragma once
 #include "mppi_rollout.cuh"
@@ -38,14 +40,15 @@ namespace mppi {
 
 constexpr int kScanC = 16;                 // lanes per sample = chunks of the horizon
 constexpr int kScanL = 4;                  // steps per chunk at most: N <= kScanC * kScanL = 64
-constexpr int kScanSamples = 32;           // samples per block
+constexpr int kScanSamples = 32;           // samples per block at most (the host may take fewer, even, >= kScanMinSamples,
+constexpr int kScanMinSamples = 8;         // so that a lone controller's blocks cover every SM): blockDim.x = 16 x samples
 constexpr int kScanThreads = kScanSamples * kScanC;
 constexpr int kScanMaxN = kScanC * kScanL;
 
 // float4 units of dynamic shared memory after the nominal + track + 16 float4 of reduction scratch
-__host__ __device__ inline size_t scan_extra_f4(int N, int nb)
+__host__ __device__ inline size_t scan_extra_f4(int N, int nb, int spb)
 {
-    return (size_t)(kScanThreads / 32) * N      // s_acc [16 warps][N]: weighted perturbations / combine scratch
+    return (size_t)(spb / 2) * N                // s_acc [warps][N]: weighted perturbations / combine scratch
            + 8                                  // s_cost [32]
            + (size_t)(3 * nb + 3) / 4;          // combine scratch
 }
@@ -92,30 +95,60 @@ __global__ void __launch_bounds__(kScanThreads, 1) rollout_scan_kernel(const Dev
     static_assert(OBJ == OBJ_GATE, "time-parallel kernel: the gate-progress objective");
     extern __shared__ float4 smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, c = lane & (kScanC - 1), grp = lane >> 4;
-    const int b = blockIdx.y, N = P.N;
-    const int kbase = blockIdx.x * kScanSamples;
+    const int b = blockIdx.y, N = P.N, nthr = blockDim.x, nw = nthr >> 5;
+    const int spb = nthr / kScanC;                     // samples per block
+    const int kbase = blockIdx.x * spb;
     const int sidx = 2 * warp + grp;                   // this lane's sample within the block
     const uint32_t k = (uint32_t)(kbase + sidx);
+    const bool valid = kbase + sidx < P.K;             // the last block of a controller may be ragged
 
     float4* s_unom = smem;
     float4* s_trk = smem + N;
     float* s_red = reinterpret_cast<float*>(s_trk + track_f4(P, OBJ));   // 64 floats
     float4* s_acc = reinterpret_cast<float4*>(s_red + 64);               // [16][N]
-    float* s_cost = reinterpret_cast<float*>(s_acc + (kScanThreads / 32) * N);   // [32]
+    float* s_cost = reinterpret_cast<float*>(s_acc + nw * N);            // [32]
     float* s_pair = s_cost + 32;                                         // 3 nb floats
 
     if (tid == 0) MPPI_STAMP(A, 0);
+    const int L = (N + kScanC - 1) / kScanC;           // steps per chunk (<= kScanL)
+    const int t0 = c * L;
+    const int cnt = valid ? max(0, min(L, N - t0)) : 0;   // this lane's steps: t0 .. t0 + cnt - 1
+
+    // ---- inputs.  The loads go out first and are parked in registers; the state-independent half of the noise
+    //      (Philox, radius, angle: perturb_prepare) is drawn while they are in flight -- after an L2 flush they come
+    //      from HBM -- and only then are they put into shared memory.  Under programmatic dependent launch
+    //      (mppi_optimize's chain, StepArgs::pdl bit 0) the nominal is the previous kernel's output and is loaded after
+    //      griddepcontrol.wait; gates, x0 and the draws do not depend on it.
+    const bool pdl_wait = (A.pdl & 1) != 0;
+    const float4* un_g = reinterpret_cast<const float4*>(A.u_nom) + (size_t)b * N;
     const int start = A.start[b];
-    stage_inputs<OBJ>(P, A, b, start, s_unom, s_trk);
     const State x0 = load_state(A.x0 + 13 * b);
+    const int ng4 = 4 * P.G;                           // <= 4 MPPI_MAX_GATES = 256 <= 2 nthr
+    float4 g_a = make_float4(0.f, 0.f, 0.f, 0.f), g_b = g_a, u_a = g_a;
+    if (tid < ng4) g_a = P.gates[tid];
+    if (tid + nthr < ng4) g_b = P.gates[tid + nthr];
+    if (!pdl_wait && tid < N) u_a = un_g[tid];         // N <= 64 <= nthr
+    float f[kScanL][4];
+#pragma unroll
+    for (int j = 0; j < kScanL; ++j)
+        if (j < cnt) {
+            const uint4 r = philox4x32_10(k, (uint32_t)(t0 + j), A.iter, (uint32_t)b, A.rk);
+            perturb_prepare<MATH>(r.x, r.y, P.bm_k, f[j][0], f[j][1]);
+            perturb_prepare<MATH>(r.z, r.w, P.bm_k, f[j][2], f[j][3]);
+        }
+    if (tid < ng4) s_trk[tid] = g_a;
+    if (tid + nthr < ng4) s_trk[tid + nthr] = g_b;
+    if (tid < 32) s_cost[tid] = __int_as_float(0x7f800000);      // samples this block does not have: cost +inf, weight 0
+    if (pdl_wait) {
+        asm volatile("griddepcontrol.wait;" ::: "memory");
+        if (tid < N) u_a = un_g[tid];
+    }
+    if (tid < N) s_unom[tid] = u_a;
     __syncthreads();
     if (tid == 0) MPPI_STAMP(A, 1);
 
-    const int L = (N + kScanC - 1) / kScanC;           // steps per chunk (<= kScanL)
-    const int t0 = c * L;
-    const int cnt = max(0, min(L, N - t0));            // this lane's steps: t0 .. t0 + cnt - 1
-
-    // ---- eq.(3): the clamped thrusts of this lane's steps, and what the dynamics need of them ----
+    // ---- eq.(3): the clamped thrusts of this lane's steps (second half of the pairs: the operations of
+    //      sample_thrust), and what the dynamics need of them ----
     float4 T[kScanL];
     float ax[kScanL], ay[kScanL], az[kScanL], cm[kScanL];
 #pragma unroll
@@ -123,7 +156,10 @@ __global__ void __launch_bounds__(kScanThreads, 1) rollout_scan_kernel(const Dev
         T[j] = make_float4(0.f, 0.f, 0.f, 0.f);
         if (j < cnt) {
             const float4 un = s_unom[t0 + j];
-            T[j] = sample_thrust<MATH>(P, A.rk, k, (uint32_t)(t0 + j), A.iter, (uint32_t)b, un);
+            perturb_finish<MATH>(f[j][0], f[j][1], P.sigma, un.x, un.y, T[j].x, T[j].y);
+            perturb_finish<MATH>(f[j][2], f[j][3], P.sigma, un.z, un.w, T[j].z, T[j].w);
+            T[j].x = fminf(fmaxf(T[j].x, P.T_min), P.T_max); T[j].y = fminf(fmaxf(T[j].y, P.T_min), P.T_max);
+            T[j].z = fminf(fmaxf(T[j].z, P.T_min), P.T_max); T[j].w = fminf(fmaxf(T[j].w, P.T_min), P.T_max);
             if (STORE_DU)
                 A.du[((size_t)b * N + t0 + j) * P.K + k] = make_float4(T[j].x - un.x, T[j].y - un.y, T[j].z - un.z, T[j].w - un.w);
         }
@@ -394,16 +430,20 @@ __global__ void __launch_bounds__(kScanThreads, 1) rollout_scan_kernel(const Dev
 #pragma unroll
     for (int o = 8; o > 0; o >>= 1) J += __shfl_xor_sync(kFull, J, o);
     J = sanitize_cost(J);
-    if (c == 0) s_cost[sidx] = J;
+    if (c == 0 && valid) s_cost[sidx] = J;
+    // the rollouts of this block are through: a dependent launch (the next iteration of mppi_optimize's chain) may
+    // be brought up; its blocks draw their normals and wait for this grid before they read the nominal
+    if (A.pdl & 2) asm volatile("griddepcontrol.launch_dependents;");
     __syncthreads();
     if (tid == 0) MPPI_STAMP(A, 7);
 
     // ---- block partial of the fused update (eq.(4),(5)): every warp forms the 32 costs' minimum and weights on its
     //      own (same values in every warp), every lane weighs the perturbations of its own steps ----
     const float Jl = s_cost[lane];
-    if (warp == 0) A.cost[(size_t)b * P.K + kbase + lane] = Jl;
+    const bool have = lane < spb && kbase + lane < P.K;
+    if (warp == 0 && have) A.cost[(size_t)b * P.K + kbase + lane] = Jl;
     const float m = warp_min(Jl);
-    const float el = exp_weight<MATH>((m - Jl) * P.inv_lambda);
+    const float el = have ? exp_weight<MATH>((m - Jl) * P.inv_lambda) : 0.0f;
     const float Zb = warp_sum(el);
     const float e = __shfl_sync(kFull, el, sidx);
 #pragma unroll
@@ -417,11 +457,11 @@ __global__ void __launch_bounds__(kScanThreads, 1) rollout_scan_kernel(const Dev
         if (grp == 0 && j < cnt) s_acc[warp * N + t0 + j] = d;
     }
     __syncthreads();
+    if (tid == 0) MPPI_STAMP(A, 3);
     float* part = A.partials + ((size_t)b * P.blocks_per_ctrl + blockIdx.x) * P.part_stride;
-    for (int j = tid; j < 4 * N; j += kScanThreads) {
+    for (int j = tid; j < 4 * N; j += nthr) {
         float s = 0.0f;
-#pragma unroll
-        for (int w = 0; w < kScanThreads / 32; ++w) s += reinterpret_cast<const float*>(s_acc)[w * 4 * N + j];
+        for (int w = 0; w < nw; ++w) s += reinterpret_cast<const float*>(s_acc)[w * 4 * N + j];
         part[j] = s;
     }
     if (tid == 0) write_partial_header(P, A, b, blockIdx.x, m, Zb);

@@ -305,9 +305,13 @@ def test_noise_matches_oracle_and_pipelines_agree():
     import torch
     wl = W.cfg0(K=512, N=37)
     outs = {}
-    for name, opts in dict(fused=dict(pipeline=0, store_noise=1), two=dict(pipeline=1),
+    # "fused" names the pipelined kernel: under AUTO this shape now goes to the time-parallel kernel (variant 5), whose
+    # states equal the others' to rounding only (another association order of the same RK4: mppi_scan.cuh); its noise
+    # is the same stream bit for bit, its costs are compared below with a tolerance
+    for name, opts in dict(fused=dict(pipeline=0, variant=4, store_noise=1), two=dict(pipeline=1),
                            thr=dict(pipeline=0, variant=1, store_noise=1),
-                           pk=dict(pipeline=0, variant=3, store_noise=1)).items():
+                           pk=dict(pipeline=0, variant=3, store_noise=1),
+                           scan=dict(pipeline=0, variant=5, store_noise=1)).items():
         m = Pz.make_ctx(wl, **opts)
         x0, start, u = Pz.to_dev(wl)
         outs[name] = Pz.gpu_step(m, x0, start, u, 5, 7)
@@ -317,6 +321,10 @@ def test_noise_matches_oracle_and_pipelines_agree():
     du_o = np.transpose(o["du"], (0, 2, 1, 3))
     np.testing.assert_allclose(outs["fused"]["du"], du_o, rtol=0, atol=3e-6)
     np.testing.assert_array_equal(outs["fused"]["du"], outs["two"]["du"])
+    np.testing.assert_array_equal(outs["scan"]["du"], outs["two"]["du"])
+    np.testing.assert_allclose(outs["scan"]["cost"], outs["two"]["cost"], rtol=2e-5, atol=2e-5)
+    np.testing.assert_allclose(outs["scan"]["weights"], outs["two"]["weights"], rtol=0, atol=1e-5)
+    np.testing.assert_allclose(outs["scan"]["u_new"], outs["two"]["u_new"], rtol=0, atol=1e-4)
     # the packed fp32x2 kernel performs, per half, the scalar kernel's operations in the same order
     for key in ("du", "cost"):
         np.testing.assert_array_equal(outs["thr"][key], outs["pk"][key])
