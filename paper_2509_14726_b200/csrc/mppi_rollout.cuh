@@ -8,11 +8,14 @@ namespace mppi {
 
 constexpr unsigned kFull = 0xffffffffu;
 
+// minimum over the warp: ONE instruction on sm_100a (redux.sync.min.f32 -> CREDUX.MIN.F32, result in a uniform
+// register) instead of five shuffle + FMNMX rounds; the minimum is exact, so nothing else changes.  NaN inputs are
+// ignored, as by fminf (costs are sanitised before they get here).
 __device__ __forceinline__ float warp_min(float v)
 {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(kFull, v, o));
-    return v;
+    float r;
+    asm volatile("redux.sync.min.f32 %0, %1, 0xffffffff;" : "=f"(r) : "f"(v));
+    return r;
 }
 __device__ __forceinline__ float warp_sum(float v)
 {

@@ -437,31 +437,42 @@ __global__ void __launch_bounds__(kScanThreads, 1) rollout_scan_kernel(const Dev
     __syncthreads();
     if (tid == 0) MPPI_STAMP(A, 7);
 
-    // ---- block partial of the fused update (eq.(4),(5)): every warp forms the 32 costs' minimum and weights on its
-    //      own (same values in every warp), every lane weighs the perturbations of its own steps ----
+    // ---- block partial of the fused update (eq.(4),(5)).  With 14-16 warps on the SM every instruction of this
+    //      tail costs ~4 cycles of wall time, so it is kept short: every warp forms the block minimum and the 32 weights
+    //      on its own (one CREDUX), only the warps that hold a sample with a non-zero weight -- every warp knows which
+    //      those are -- weigh their perturbations and take part in the sum over the warps (in the near-arg-min regime of
+    //      the paper's lambda that is one or two warps), and Z is formed by warp 0 beside the others' stores ----
     const float Jl = s_cost[lane];
     const bool have = lane < spb && kbase + lane < P.K;
     if (warp == 0 && have) A.cost[(size_t)b * P.K + kbase + lane] = Jl;
     const float m = warp_min(Jl);
     const float el = have ? exp_weight<MATH>((m - Jl) * P.inv_lambda) : 0.0f;
-    const float Zb = warp_sum(el);
-    const float e = __shfl_sync(kFull, el, sidx);
+    const unsigned cmask = __ballot_sync(kFull, el != 0.0f);      // samples of the block that carry weight
+    if ((cmask >> (2 * warp)) & 3u) {
+        const float e = __shfl_sync(kFull, el, sidx);
 #pragma unroll
-    for (int j = 0; j < kScanL; ++j) {
-        float4 d = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (j < cnt) {
-            const float4 un = s_unom[t0 + j];
-            d = make_float4(e * (T[j].x - un.x), e * (T[j].y - un.y), e * (T[j].z - un.z), e * (T[j].w - un.w));
+        for (int j = 0; j < kScanL; ++j) {
+            float4 d = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (j < cnt) {
+                const float4 un = s_unom[t0 + j];
+                d = make_float4(e * (T[j].x - un.x), e * (T[j].y - un.y), e * (T[j].z - un.z), e * (T[j].w - un.w));
+            }
+            d = add4(d, shfl_xor4(d, 16));
+            if (grp == 0 && j < cnt) s_acc[warp * N + t0 + j] = d;
         }
-        d = add4(d, shfl_xor4(d, 16));
-        if (grp == 0 && j < cnt) s_acc[warp * N + t0 + j] = d;
     }
+    float Zb = 0.0f;
+    if (warp == 0) Zb = warp_sum(el);
     __syncthreads();
     if (tid == 0) MPPI_STAMP(A, 3);
     float* part = A.partials + ((size_t)b * P.blocks_per_ctrl + blockIdx.x) * P.part_stride;
     for (int j = tid; j < 4 * N; j += nthr) {
         float s = 0.0f;
-        for (int w = 0; w < nw; ++w) s += reinterpret_cast<const float*>(s_acc)[w * 4 * N + j];
+        for (unsigned mm = cmask; mm; ) {              // contributing warps in ascending order: deterministic
+            const int w = (__ffs(mm) - 1) >> 1;
+            mm &= ~(3u << (2 * w));
+            s += reinterpret_cast<const float*>(s_acc)[w * 4 * N + j];
+        }
         part[j] = s;
     }
     if (tid == 0) write_partial_header(P, A, b, blockIdx.x, m, Zb);
