@@ -46,6 +46,25 @@ GATE_LOOP_MIX = {"ffma_rrr": 53, "ffma_const": 101, "fmul": 67, "fadd": 44, "phi
 NCU_DRAM_BYTES_PER_LAUNCH = 55552     # rollout_pipe_kernel<gate>, cfg1: 55.6 KB read + 0 B written (profiles/README_r02e.md, ncu_details_pipe_r02e.txt)
 
 
+def kernel_label(info, P=None) -> str:
+    """Which rollout kernel a context launches, from mppi_get_info (the library states shapes, not names)."""
+    rate = bool(P and P.get("input_model", 0) == 1)
+    if rate:
+        return ("rate-model pipelined" if info["block_threads"] == 320 else
+                "rate-model packed fp32x2" if info["samples_per_thread"] == 2 else "rate-model scalar")
+    if info["rollout_warps_per_block"] == 16:
+        return "time-parallel"
+    if info["rollout_warps_per_block"] == 3 and info["block_threads"] == 256:
+        return "pipelined"
+    if info["samples_per_thread"] == 2:
+        return "packed fp32x2"
+    return "latency" if info["block_threads"] == 256 and info["rollout_warps_per_block"] < 8 else "scalar"
+
+
+KERNEL_SYMBOL = {"time-parallel": "rollout_scan_kernel", "pipelined": "rollout_pipe_kernel", "packed fp32x2": "rollout2_kernel",
+                 "latency": "rollout_lat_kernel", "scalar": "rollout_kernel"}
+
+
 def dist_env():
     return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
 
@@ -459,7 +478,7 @@ def run_ours(args):
                        "l2": "flushed between timed iterations (256 MiB write outside the events)",
                        "pipeline": "fused" if args.pipeline == 0 else "two_pass", "fast_math": args.fast_math,
                        "cuda_graph": bool(args.graph), "block_threads": info["block_threads"],
-                       "kernel": "rollout_pipe_kernel" if info["rollout_warps_per_block"] == 3 and info["block_threads"] == 256 else "rollout",
+                       "kernel": KERNEL_SYMBOL.get(kernel_label(info, P), "rollout"),
                        "grid_blocks": info["grid_blocks"], "replicas": world},
             "clocks": clocks,
             "latency_us": {"p50": float(np.median(ms) * 1e3), "p99": float(np.percentile(ms, 99) * 1e3),
@@ -554,12 +573,7 @@ def run_survey(args):
                 m.step(x0, start, u, wl.seed, it[0], u_new=un, cost=cost, weights=w); it[0] += 1
             ms = time_steps(step, lambda: flush_buf.fill_(float(it[0] & 7)), 40 if B > 1 else 200, 5)
             info = m.info()
-            k = ("rate-model pipelined" if P.get("input_model", 0) == 1 and info["block_threads"] == 320 else
-                 "rate-model packed fp32x2" if P.get("input_model", 0) == 1 and info["samples_per_thread"] == 2 else
-                 "rate-model scalar" if P.get("input_model", 0) == 1 else
-                 "pipelined" if info["rollout_warps_per_block"] == 3 and info["block_threads"] == 256 else
-                 "packed fp32x2" if info["samples_per_thread"] == 2 else
-                 "latency" if info["block_threads"] == 256 and info["rollout_warps_per_block"] < 8 else "scalar")
+            k = kernel_label(info, P)
             units = P["K"] * P["N"] * P["B"]
             print(f"| {name} | {P['objective']} | {P.get('input_model', 0)} | {P['K']} | {P['N']} | {P['B']} | {k} "
                   f"({info['block_threads']} thr x {info['grid_blocks']} blocks, {info['regs_per_thread']} regs) | "
@@ -590,7 +604,7 @@ def _time_workload(Bd, wl, dev, flush_buf, steps, warmup, **opts):
     return ms, info, ess, J
 
 
-VARIANT_NAMES = {0: "AUTO", 1: "scalar", 2: "latency", 3: "packed", 4: "pipelined"}
+VARIANT_NAMES = {0: "AUTO", 1: "scalar", 2: "latency", 3: "packed", 4: "pipelined", 5: "time-parallel"}
 
 
 def run_sweep(args):
@@ -612,20 +626,18 @@ def run_sweep(args):
     print("## (i) batch sweep, us per iteration (median of 60; AUTO's choice in brackets)\n")
     for obj in args.sweep_objectives.split(","):
         print(f"objective: {obj}\n")
-        print("| B | " + " | ".join(VARIANT_NAMES[v] for v in (4, 2, 3, 1, 0)) + " | AUTO vs best |")
-        print("|---|" + "---|" * 6)
+        print("| B | " + " | ".join(VARIANT_NAMES[v] for v in (5, 4, 2, 3, 1, 0)) + " | AUTO vs best |")
+        print("|---|" + "---|" * 7)
         for B in [int(b) for b in args.sweep_batches.split(',')]:
             wl = base[obj](B=B) if obj == "gate" else base[obj](B)
             row, best = [], None
-            for v in (4, 2, 3, 1, 0):
+            for v in (5, 4, 2, 3, 1, 0):
                 try:
                     ms, info, _, _ = _time_workload(Bd, wl, dev, flush_buf, 60, 5, fast_math=args.fast_math, variant=v)
                     t = float(np.median(ms)) * 1e3
                     tag = f"{t:.1f}"
                     if v == 0:
-                        k = ("pipelined" if info["rollout_warps_per_block"] == 3 and info["block_threads"] == 256 else
-                             "packed" if info["samples_per_thread"] == 2 else
-                             "latency" if info["block_threads"] == 256 and info["rollout_warps_per_block"] < 8 else "scalar")
+                        k = kernel_label(info)
                         tag += f" [{k}, {info['block_threads']} thr x {info['grid_blocks']}]"
                         row.append(tag)
                         row.append(f"{t / best:.2f}x")

@@ -579,7 +579,7 @@ def test_random_small_configurations_against_the_oracle(sweep_seed):
         wl = W.replicate(wl, B, 0.2)
         if obj == 2:
             wl.start[:] = rng.integers(-1, 500, B)               # hint or global search
-        opts = dict(variant=int(rng.choice([0, 1, 2, 3, 4])), pipeline=int(rng.integers(0, 2)), fast_math=int(rng.integers(0, 2)))
+        opts = dict(variant=int(rng.choice([0, 1, 2, 3, 4, 5])), pipeline=int(rng.integers(0, 2)), fast_math=int(rng.integers(0, 2)))
         if rng.integers(0, 3) == 0:
             opts["block_threads"] = int(rng.choice([32, 64, 128]))
         tag = f"random case {sweep_seed}/{case}: obj {obj} rate {rate} K {K} N {N} B {B} {opts}"
@@ -595,7 +595,7 @@ def test_random_small_configurations_against_the_oracle(sweep_seed):
         Pz.compare(tag, g, o, wl.params["lambda"], obj in (0, 3))
         m.close()
         ran += 1
-    assert ran >= 30 and rejected >= 3, (ran, rejected)
+    assert ran >= 25 and rejected >= 3, (ran, rejected)        # (variant 5 takes the gate objective with thrust inputs only)
 
 
 def test_seed_high_word_reaches_the_key():
