@@ -93,8 +93,9 @@ typedef enum {
 } mppi_pipeline;
 
 typedef enum {
-    MPPI_VARIANT_AUTO = 0,       /* pipelined kernel when B*K/32 warps cannot fill the chip, else packed (K % 64
-                                    == 0) or scalar throughput                                             */
+    MPPI_VARIANT_AUTO = 0,       /* time-parallel kernel where it applies and B*K/32 <= the SM count, pipelined or
+                                    latency kernel while B*K/32 warps cannot fill the chip, else packed (K % 64
+                                    == 0) or scalar throughput (thresholds from the batch sweep, profiles/)    */
     MPPI_VARIANT_THROUGHPUT = 1, /* one sample per thread, noise drawn inside the horizon loop; block_threads
                                     samples per block                                                      */
     MPPI_VARIANT_LATENCY = 2,    /* 256-thread blocks: all warps draw the noise of 32 C samples into shared
@@ -119,7 +120,7 @@ typedef enum {
                                     lanes ALONG THE HORIZON; body rates, attitude, velocity and position of the
                                     chunks are joined by warp-shuffle scans (affine maps, quaternion products,
                                     sums).  Needs input_model = 0, Jx == Jy (then the body-rate equations are
-                                    linear given the yaw rate), objective MPPI_OBJ_GATE, N <= 64, the fused
+                                    linear given the yaw rate), objective MPPI_OBJ_GATE or MPPI_OBJ_GATE_PAPER, N <= 64, the fused
                                     pipeline and block_threads 0 (else MPPI_E_PARAM).  Same RK4, same per-step
                                     renormalisation, another association order: states equal the other kernels'
                                     to rounding, not bit for bit.  AUTO takes it for such configurations when

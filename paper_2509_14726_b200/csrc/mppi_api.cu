@@ -122,7 +122,7 @@ static bool finite_pos(float v) { return std::isfinite(v) && v > 0.0f; }
 // omega_x, omega_y to be linear given omega_z: Jx == Jy (then (Jx - Jy)/Jz = 0 and (Jy - Jz)/Jx = -(Jz - Jx)/Jy).
 static bool scan_capable(const mppi_params* p)
 {
-    return p->input_model == 0 && p->objective == MPPI_OBJ_GATE && p->Jx == p->Jy && p->N <= 64 &&
+    return p->input_model == 0 && (p->objective == MPPI_OBJ_GATE || p->objective == MPPI_OBJ_GATE_PAPER) && p->Jx == p->Jy && p->N <= 64 &&
            p->pipeline == MPPI_PIPE_FUSED && p->block_threads == 0 && p->K % 32 == 0;
 }
 // Samples per block of the time-parallel kernel (16 lanes each): 32, or fewer (even, >= 8) when that lets the blocks
@@ -168,7 +168,7 @@ static int validate(const mppi_params* p)
     BAD((int64_t)p->K / 32 > 65535, "K too large");
     BAD(p->variant < 0 || p->variant > 5, "unknown variant");
     BAD(p->variant == MPPI_VARIANT_SCAN && !scan_capable(p),
-        "the time-parallel variant needs input_model 0, objective MPPI_OBJ_GATE, Jx == Jy, N <= 64, the fused pipeline, "
+        "the time-parallel variant needs input_model 0, objective MPPI_OBJ_GATE or MPPI_OBJ_GATE_PAPER, Jx == Jy, N <= 64, the fused pipeline, "
         "block_threads 0");
     BAD(p->variant == MPPI_VARIANT_PACKED &&
             (p->K % 64 != 0 || (p->block_threads && (p->block_threads > 128 || p->K % (2 * p->block_threads) != 0))),

@@ -7,10 +7,15 @@ namespace mppi {
 
 typedef void (*ScanFn)(const DevParams, const StepArgs);
 
+template <int OBJ>
+static ScanFn pick_scan1(const LaunchCfg& c)
+{
+    if (c.fast_math) return c.store_du ? rollout_scan_kernel<OBJ, 1, true> : rollout_scan_kernel<OBJ, 1, false>;
+    return c.store_du ? rollout_scan_kernel<OBJ, 0, true> : rollout_scan_kernel<OBJ, 0, false>;
+}
 static ScanFn pick_scan(const LaunchCfg& c)
 {
-    if (c.fast_math) return c.store_du ? rollout_scan_kernel<OBJ_GATE, 1, true> : rollout_scan_kernel<OBJ_GATE, 1, false>;
-    return c.store_du ? rollout_scan_kernel<OBJ_GATE, 0, true> : rollout_scan_kernel<OBJ_GATE, 0, false>;
+    return c.objective == OBJ_GATE_PAPER ? pick_scan1<OBJ_GATE_PAPER>(c) : pick_scan1<OBJ_GATE>(c);
 }
 
 size_t scan_smem_bytes(const DevParams& P, const LaunchCfg& c)

@@ -92,7 +92,7 @@ __device__ __forceinline__ void omega_xy_step(const DevParams& P, float& ox, flo
 template <int OBJ, int MATH, bool STORE_DU>
 __global__ void __launch_bounds__(kScanThreads, 1) rollout_scan_kernel(const DevParams P, const StepArgs A)
 {
-    static_assert(OBJ == OBJ_GATE, "time-parallel kernel: the gate-progress objective");
+    static_assert(OBJ == OBJ_GATE || OBJ == OBJ_GATE_PAPER, "time-parallel kernel: the two gate-progress objectives");
     extern __shared__ float4 smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, c = lane & (kScanC - 1), grp = lane >> 4;
     const int b = blockIdx.y, N = P.N, nthr = blockDim.x, nw = nthr >> 5;
@@ -138,6 +138,8 @@ __global__ void __launch_bounds__(kScanThreads, 1) rollout_scan_kernel(const Dev
         }
     if (tid < ng4) s_trk[tid] = g_a;
     if (tid + nthr < ng4) s_trk[tid + nthr] = g_b;
+    if (OBJ == OBJ_GATE_PAPER && tid <= N)             // previous-iteration "in front" flags (caller's; all ones without)
+        reinterpret_cast<int*>(s_trk + ng4)[tid] = A.prev_front ? A.prev_front[(size_t)b * (N + 1) + tid] : 1;
     if (tid < 32) s_cost[tid] = __int_as_float(0x7f800000);      // samples this block does not have: cost +inf, weight 0
     if (pdl_wait) {
         asm volatile("griddepcontrol.wait;" ::: "memory");
@@ -366,17 +368,72 @@ __global__ void __launch_bounds__(kScanThreads, 1) rollout_scan_kernel(const Dev
 
     // ---- objective ----
     float J;
-    if (OBJ == OBJ_GATE) {
-        // GateCost (mppi_cost.cuh) chunk by chunk.  Across a chunk boundary the state of the machine is the target
-        // index alone (s_prev and the segment's first distance are functions of the boundary position), and a
-        // chunk's progress |p_end - c| - |p_start - c| is its own telescoped segment.
+    {
+        // GateCost / GatePaperCost (mppi_cost.cuh) chunk by chunk.  Across a chunk boundary the state of the machine
+        // is the target index alone (s_prev and the segment's first distance are functions of the boundary position;
+        // the paper's form also looks at the horizon's start gate, a constant), and a chunk's progress
+        // |p_end - c| - |p_start - c| is its own telescoped segment.
         const float4* s_gates = s_trk;
-        int g_in = wrap_index(start, P.G), g_out = g_in, lo = 0;
+        const int* s_front = reinterpret_cast<const int*>(s_trk + 4 * P.G);      // OBJ_GATE_PAPER only
+        const int gate0 = wrap_index(start, P.G);
+        int g_in = gate0, g_out = g_in, lo = 0;
         bool need = true;
         float Jc = 0.0f;
         const unsigned gmask = 0xffffu << (lane & 16);
         for (;;) {
-            if (need) {
+            if (need && OBJ == OBJ_GATE_PAPER) {
+                // eq.(6),(7) with squared distances, the near-gate term on the pre-step state and the temporal
+                // check of Fig. 2 [R-23]..[R-25], [R-40]: GatePaperCost::step, operation for operation
+                int gate = g_in;
+                float4 cg = s_gates[4 * gate], ng = s_gates[4 * gate + 1];
+                float ppx = psx, ppy = psy, ppz = psz;
+                float rx0 = ppx - cg.x, ry0 = ppy - cg.y, rz0 = ppz - cg.z;
+                float d2_0 = fmaf(rz0, rz0, fmaf(ry0, ry0, rx0 * rx0)), d2_prev = d2_0;
+                float s_prev = fmaf(ng.z, rz0, fmaf(ng.y, ry0, ng.x * rx0));
+                float acc = 0.0f;
+#pragma unroll
+                for (int j = 0; j < kScanL; ++j)
+                    if (j < cnt) {
+                        const float px = Px[j], py = Py[j], pz = Pz[j];
+                        float dn2 = d2_prev;
+                        if (P.near_mode == 1 && gate != gate0) {
+                            const float4 c0 = s_gates[4 * gate0];
+                            const float ux = ppx - c0.x, uy = ppy - c0.y, uz = ppz - c0.z;
+                            dn2 = fmaf(uz, uz, fmaf(uy, uy, ux * ux));
+                        }
+                        if (dn2 < P.r_near2) acc = fmaf(P.q_near, dn2, acc);
+                        const float fx = px - cg.x, fy = py - cg.y, fz = pz - cg.z;
+                        const float d2 = fmaf(fz, fz, fmaf(fy, fy, fx * fx));
+                        const float s = fmaf(ng.z, fz, fmaf(ng.y, fy, ng.x * fx));
+                        bool switched = false;
+                        if (s_prev < 0.0f && s >= 0.0f) {                 // front -> back through the plane
+                            const float4 hg = s_gates[4 * gate + 2], vg = s_gates[4 * gate + 3];
+                            const float alpha = s_prev / (s_prev - s);
+                            const float rx = ppx - cg.x, ry = ppy - cg.y, rz = ppz - cg.z;
+                            const float hx = fmaf(alpha, fx - rx, rx), hy = fmaf(alpha, fy - ry, ry), hz = fmaf(alpha, fz - rz, rz);
+                            const float y = fmaf(hg.z, hz, fmaf(hg.y, hy, hg.x * hx));
+                            const float z = fmaf(vg.z, hz, fmaf(vg.y, hy, vg.x * hx));
+                            if (fabsf(y) <= cg.w && fabsf(z) <= ng.w) {
+                                if (gate != gate0 || s_front[t0 + j + 1] != 0) {      // temporally consistent pass
+                                    acc += (d2 - d2_0) - P.bonus;                     // close the segment
+                                    gate = (gate + 1 == P.G) ? 0 : gate + 1;
+                                    cg = s_gates[4 * gate]; ng = s_gates[4 * gate + 1];
+                                    const float qx = px - cg.x, qy = py - cg.y, qz = pz - cg.z;
+                                    d2_0 = fmaf(qz, qz, fmaf(qy, qy, qx * qx)); d2_prev = d2_0;
+                                    s_prev = fmaf(ng.z, qz, fmaf(ng.y, qy, ng.x * qx));
+                                    switched = true;
+                                }
+                            } else {
+                                acc += P.miss;                                        // miss: target unchanged
+                            }
+                        }
+                        if (!switched) { s_prev = s; d2_prev = d2; }
+                        ppx = px; ppy = py; ppz = pz;
+                    }
+                Jc = acc + (d2_prev - d2_0);
+                g_out = gate;
+            }
+            if (need && OBJ == OBJ_GATE) {
                 int gate = g_in;
                 float4 cg = s_gates[4 * gate], ng = s_gates[4 * gate + 1], hg = s_gates[4 * gate + 2];
                 float d0 = GateCost::norm3<MATH>(psx - cg.x, psy - cg.y, psz - cg.z);

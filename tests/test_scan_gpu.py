@@ -87,6 +87,24 @@ def test_crossings_in_every_chunk(math):
     assert (nc >= 3).mean() > 0.5 and nc.max() >= 5, (np.bincount(nc),)
 
 
+@pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
+@pytest.mark.parametrize("near_mode", [0, 1])
+def test_the_papers_own_gate_objective(near_mode, math):
+    # objective 3 (eq.(6),(7) with squared distances, Q_near term, temporal check with previous-iteration flags): on the
+    # configs[1] track at full size, and crossing-heavy with RANDOM flags so that registered and unregistered passes of
+    # the start gate both occur, in both readings of the near term
+    wl = W.gate_paper()
+    wl.params["near_mode"] = near_mode
+    run_case(wl, f"scan gate_paper near{near_mode} {math}", variant=SCAN, **math)
+    for K, N, B in ((2048, 30, 1), (1024, 64, 1), (512, 37, 3)):
+        wl = W.stress_gate_paper(K=K, N=N)
+        wl.params["near_mode"] = near_mode
+        if B > 1:
+            wl = W.replicate(wl, B, 0.2)
+        g, o, st, _ = run_case(wl, f"scan stress_gate_paper K{K} N{N} B{B} near{near_mode} {math}", variant=SCAN, **math)
+        assert int((o["ncross"] > 0).sum()) > 0
+
+
 def test_mixing_weights_strict():
     # many samples carry weight: every warp of every block takes part in the block partial; strict bounds
     wl = W.cfg1(K=2048, N=50)
@@ -171,7 +189,7 @@ def test_what_the_variant_rejects_and_what_auto_picks():
         with pytest.raises(Bd.MppiError) as e:
             Bd.Mppi(wl.params, variant=SCAN, **over)
         assert e.value.status == -2, over                                 # MPPI_E_PARAM
-    for make in (W.cfg2, W.cfg3, W.gate_paper, W.rate_gate_paper):
+    for make in (W.cfg2, W.cfg3, W.rate_gate_paper):
         with pytest.raises(Bd.MppiError) as e:
             Bd.Mppi(make().params, variant=SCAN)
         assert e.value.status == -2
