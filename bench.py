@@ -43,7 +43,10 @@ L2_FLUSH_BYTES = 256 << 20
 # cuobjdump -sass of rollout_kernel<OBJ_GATE, fast math>): 154 FFMA (53 with three register operands, 101 with a
 # constant operand), 67 FMUL, 44 FADD, 20 Philox half-rounds (IMAD.WIDE + LOP3), 11 MUFU, 8 FMNMX, 7 LDS.128.
 GATE_LOOP_MIX = {"ffma_rrr": 53, "ffma_const": 101, "fmul": 67, "fadd": 44, "philox_half_round": 20, "mufu": 11, "fmnmx": 8, "lds": 7}
-NCU_DRAM_BYTES_PER_LAUNCH = 55552     # rollout_pipe_kernel<gate>, cfg1: 55.6 KB read + 0 B written (profiles/README_r02e.md, ncu_details_pipe_r02e.txt)
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the kernel that runs cfg1, from the committed ncu --set full
+# captures (not measured live): rollout_scan_kernel<gate> 75.8 KB read + 0 B written (profiles/README_r02f.md,
+# ncu_details_scan_r02f.txt), rollout_pipe_kernel<gate> 55.6 KB + 0 B (profiles/README_r02e.md, ncu_details_pipe_r02e.txt)
+NCU_DRAM_BYTES_PER_LAUNCH = {"time-parallel": (75776, "profiles/README_r02f.md"), "pipelined": (55552, "profiles/README_r02e.md")}
 
 
 def kernel_label(info, P=None) -> str:
@@ -500,13 +503,14 @@ def run_ours(args):
             "roofline": {"bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
                          # dram__bytes_read.sum + dram__bytes_write.sum of this kernel, per launch, from the
                          # ncu --set full capture summarised in profiles/README_r01e.md (not measured live)
-                         "traffic": NCU_DRAM_BYTES_PER_LAUNCH if args.pipeline == 0 else None, "kernel": "the iteration's single kernel (pipelined rollout + cost + fused softmax update)" if args.pipeline == 0 else "rollout kernel of the two-pass pipeline",
+                         "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(kernel_label(info, P), (None, None))[0] if args.pipeline == 0 else None,
+                         "kernel": f"the iteration's single kernel ({kernel_label(info, P)} rollout + cost + fused softmax update)" if args.pipeline == 0 else "rollout kernel of the two-pass pipeline",
                          "flops_per_sample_step": flops, "units_per_launch": units,
                          "peak_how": f"{sm} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 x clocks.max.sm (B200_PROFILING.md)",
                          "peak_measured_ffma_tflops": fma_tflops, "frac_of_measured_ffma": ach / fma_tflops,
                          "regs_per_thread": info["regs_per_thread"], "spill_bytes": info["local_bytes_per_thread"],
-                         "traffic_source": "profiles/README_r02e.md (ncu --set full capture of this kernel, dram__bytes_read.sum + dram__bytes_write.sum per launch; not measured in this run)" if args.pipeline == 0 else None,
-                         "note": "K=4096 is 128 warps on 148 SMs: latency-bound by construction; see 'batched'"},
+                         "traffic_source": (f"{NCU_DRAM_BYTES_PER_LAUNCH.get(kernel_label(info, P), (None, 'no capture'))[1]} (ncu --set full capture of this kernel, dram__bytes_read.sum + dram__bytes_write.sum per launch; not measured in this run)") if args.pipeline == 0 else None,
+                         "note": "K=4096 rollouts of 50 dependent steps on 148 SMs: latency-bound by construction (the time-parallel kernel splits every rollout over 16 lanes along the horizon); see 'batched' for the FP32 roofline"},
             "batched": {"workload": wl4.name, "K": P4["K"], "N": P4["N"], "B": P4["B"],
                         "value": units4 / (float(ms4.mean()) * 1e-3), "unit": UNIT, "ms_per_step": float(ms4.mean()),
                         "roofline": {"bound": "alu", "achieved": ach4, "peak": peak_tf, "unit": "TFLOP/s",

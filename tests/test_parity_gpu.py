@@ -10,18 +10,6 @@ from paper_2509_14726_b200 import workloads as W
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(scope="module", autouse=True)
-def _report():
-    yield
-    import os
-    out = os.path.join(os.path.dirname(__file__), "..", "gpurun_out")
-    if os.path.isdir(out) and Pz.STATS:
-        with open(os.path.join(out, "parity_stats.txt"), "w") as f:
-            f.write("\n".join(Pz.STATS + ["", "reported separately:"] + Pz.REPORT) + "\n")
-    if Pz.REPORT:
-        print("\n[parity] reported separately:\n  " + "\n  ".join(Pz.REPORT))
-
-
 def run_case(wl, tag, it=0, **opts):
     m = Pz.make_ctx(wl, **opts)
     x0, start, u = Pz.to_dev(wl)
