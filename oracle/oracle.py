@@ -22,14 +22,25 @@ OBJ_GATE, OBJ_TRACK, OBJ_CONTOUR, OBJ_GATE_PAPER, OBJ_CONTOUR_PAPER = 0, 1, 2, 3
 
 
 def build(force: bool = False) -> Path:
-    """Compile the oracle with gcc: -O2, OpenMP over samples, no fast-math, no FMA contraction."""
-    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
-        tmp = _LIB.with_suffix(f".{os.getpid()}.tmp")
-        cmd = ["gcc", "-std=c11", "-O2", "-fopenmp", "-ffp-contract=off", "-fno-fast-math",
+    """Compile the oracle with gcc: -O2, OpenMP over samples, no fast-math, no FMA contraction.
+
+    MPPI_ORACLE_SANITIZE=1 in the environment builds (and loads) an AddressSanitizer + UndefinedBehaviorSanitizer
+    variant instead (same source, -O1 -g; libmppi_oracle_san.so).  The interpreter must then be started with the
+    sanitizer runtimes preloaded:
+        MPPI_ORACLE_SANITIZE=1 ASAN_OPTIONS=detect_leaks=0 \
+        LD_PRELOAD="$(gcc -print-file-name=libasan.so) $(gcc -print-file-name=libubsan.so)" \
+        python -m pytest tests -q -m "not gpu"
+    """
+    san = os.environ.get("MPPI_ORACLE_SANITIZE", "") not in ("", "0")
+    lib = _HERE / "libmppi_oracle_san.so" if san else _LIB
+    if force or not lib.exists() or lib.stat().st_mtime < _SRC.stat().st_mtime:
+        tmp = lib.with_suffix(f".{os.getpid()}.tmp")
+        opt = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"] if san else ["-O2"]
+        cmd = ["gcc", "-std=c11", *opt, "-fopenmp", "-ffp-contract=off", "-fno-fast-math",
                "-shared", "-fPIC", "-Wall", "-Wextra", "-o", str(tmp), str(_SRC), "-lm"]
         subprocess.run(cmd, check=True)
-        os.replace(tmp, _LIB)
-    return _LIB
+        os.replace(tmp, lib)
+    return lib
 
 
 class _Params(C.Structure):
