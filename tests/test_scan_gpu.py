@@ -21,7 +21,7 @@ def run_case(wl, tag, it=0, **opts):
     g = Pz.gpu_step(m, x0, start, u, wl.seed, it)
     o = Pz.oracle_step(wl, wl.x0, wl.start, wl.u_nom, wl.seed, it, want_du=wl.params["K"] * wl.params["N"] * wl.params["B"] <= 1 << 22)
     o["u_nom"] = wl.u_nom.astype(np.float64)
-    st = Pz.compare(tag, g, o, wl.params["lambda"], True)
+    st = Pz.compare(tag, g, o, wl.params["lambda"], wl.params["objective"] in (0, 3))
     info = m.info()
     m.close()
     return g, o, st, info
@@ -125,7 +125,7 @@ def test_unnormalised_start_quaternion_and_spinning_start():
     run_case(wl, "scan q0 x 1.07, spinning, fast", variant=SCAN, fast_math=1)
 
 
-@pytest.mark.parametrize("name,B", [("cfg1", 1), ("stress_gate", 3)])
+@pytest.mark.parametrize("name,B", [("cfg1", 1), ("stress_gate", 3), ("gate_paper", 2)])
 @pytest.mark.parametrize("math", MATH, ids=["accurate", "fast"])
 def test_optimize_chain_equals_the_steps(name, B, math):
     # mppi_optimize: programmatic dependent launch without a graph, one graph launch with use_graph -- both must equal
@@ -151,7 +151,7 @@ def test_optimize_chain_equals_the_steps(name, B, math):
         m2.close()
     o = Pz.oracle_step(wl, wl.x0, wl.start, u_in, wl.seed, n - 1, want_du=True)
     g = dict(u_new=u.cpu().numpy(), cost=c_ref.cpu().numpy(), weights=w_ref.cpu().numpy())
-    Pz.compare(f"scan optimize chain {name} B{B} {math}", g, o, wl.params["lambda"], True)
+    Pz.compare(f"scan optimize chain {name} B{B} {math}", g, o, wl.params["lambda"], wl.params["objective"] in (0, 3))
     m.close()
 
 
