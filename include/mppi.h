@@ -304,7 +304,8 @@ typedef struct {
     int32_t max_blocks_per_sm, sm_count;
     int32_t kernels_per_step; /* launches one mppi_step enqueues */
     int32_t samples_per_thread; /* 2 for the packed fp32x2 rollout kernel, else 1 */
-    int32_t rollout_warps_per_block; /* latency variant: consumer warps C; else block_threads / 32 */
+    int32_t rollout_warps_per_block; /* latency variant: consumer warps C; pipelined: 3 (5 under input_model 1);
+                                        time-parallel: 16 (lanes per rollout); else block_threads / 32 */
     int32_t l2_bytes;
     int64_t scratch_bytes;    /* device memory the context owns */
 } mppi_info;
