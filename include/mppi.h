@@ -116,15 +116,18 @@ typedef enum {
                                     search-based contouring, block_threads <= 128 (else MPPI_E_PARAM); AUTO
                                     takes it when B K / 32 >= 8 x the SM count                             */
     MPPI_VARIANT_SCAN = 5        /* time-parallel latency kernel (eq.(2) PAPER.md:65-72 as a cascade of linear
-                                    recurrences): 512-thread blocks of 32 samples, every rollout split over 16
-                                    lanes ALONG THE HORIZON; body rates, attitude, velocity and position of the
-                                    chunks are joined by warp-shuffle scans (affine maps, quaternion products,
-                                    sums).  Needs input_model = 0, Jx == Jy (then the body-rate equations are
-                                    linear given the yaw rate), objective MPPI_OBJ_GATE or MPPI_OBJ_GATE_PAPER, N <= 64, the fused
-                                    pipeline and block_threads 0 (else MPPI_E_PARAM).  Same RK4, same per-step
+                                    recurrences): blocks of up to 32 samples x 16 lanes, every rollout split over
+                                    16 lanes ALONG THE HORIZON; body rates, attitude, velocity and position of
+                                    the chunks are joined by warp-shuffle scans (affine maps, quaternion
+                                    products, sums).  Needs input_model = 0, Jx == Jy (then the body-rate
+                                    equations are linear given the yaw rate), objective MPPI_OBJ_GATE or
+                                    MPPI_OBJ_GATE_PAPER, N <= 64, the fused pipeline and block_threads 0 (else
+                                    MPPI_E_PARAM).  Same RK4, same per-step
                                     renormalisation, another association order: states equal the other kernels'
-                                    to rounding, not bit for bit.  AUTO takes it for such configurations when
-                                    B K / 32 <= the SM count                                                */
+                                    to rounding, not bit for bit.  Samples per block (28 for K = 4096 on 148
+                                    SMs) follow the SM count, so the summation order of the update -- not the
+                                    costs -- depends on the GPU model; on one GPU every call is deterministic.
+                                    AUTO takes it for such configurations when B K / 32 <= the SM count       */
 } mppi_variant;
 
 /* Parameters of Alg. 1 (samples, horizon, lambda, Sigma) plus the model and cost
