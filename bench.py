@@ -626,14 +626,16 @@ def run_sweep(args):
     dev = torch.device("cuda", 0)
     torch.cuda.set_device(dev)
     flush_buf = torch.empty(L2_FLUSH_BYTES // 4, dtype=torch.float32, device=dev)
-    base = {"gate": W.cfg4, "track": lambda B: W.replicate(W.cfg2(), B, 0.3), "contour": lambda B: W.replicate(W.cfg3(), B, 0.3)}
-    print("## (i) batch sweep, us per iteration (median of 60; AUTO's choice in brackets)\n")
+    K = args.sweep_K
+    base = {"gate": lambda B: W.cfg4(K=K, B=B), "track": lambda B: W.replicate(W.cfg2(K=K), B, 0.3),
+            "contour": lambda B: W.replicate(W.cfg3(K=2 * K), B, 0.3)}
+    print(f"## (i) batch sweep at K = {K} (contouring: {2 * K}), N = 50, us per iteration (median of 60; AUTO's choice in brackets)\n")
     for obj in args.sweep_objectives.split(","):
         print(f"objective: {obj}\n")
         print("| B | " + " | ".join(VARIANT_NAMES[v] for v in (5, 4, 2, 3, 1, 0)) + " | AUTO vs best |")
         print("|---|" + "---|" * 7)
         for B in [int(b) for b in args.sweep_batches.split(',')]:
-            wl = base[obj](B=B) if obj == "gate" else base[obj](B)
+            wl = base[obj](B)
             row, best = [], None
             for v in (5, 4, 2, 3, 1, 0):
                 try:
@@ -652,6 +654,8 @@ def run_sweep(args):
                     row.append("n/a")
             print(f"| {B} | " + " | ".join(row) + " |", flush=True)
         print()
+    if args.sweep_K != 4096:
+        return
     print("## (ii) configs[4] shape (K=4096, N=50, B=64, gate), one-hot vs mixing weights, us per iteration (median of 40)\n")
     print("| weights | lambda | ESS (median over controllers) | fused packed | fused scalar | two-pass packed (rollout + reduce) | two-pass scalar | fused packed, dU also stored |")
     print("|---|---|---|---|---|---|---|---|")
@@ -683,6 +687,7 @@ def main(argv=None):
     ap.add_argument("--sweep", action="store_true", help="batch-size sweep over the rollout kernels and the mixing-weight regime (tables, one GPU)")
     ap.add_argument("--sweep-objectives", dest="sweep_objectives", default="gate", help="--sweep: comma list of gate,track,contour")
     ap.add_argument("--sweep-batches", dest="sweep_batches", default="1,2,3,4,6,8,12,16,32,64")
+    ap.add_argument("--sweep-K", dest="sweep_K", type=int, default=4096, help="--sweep: samples per controller (table (i) only when not 4096)")
     ap.add_argument("--only", default=None, help="--survey: this workload only (a key of workloads.ALL)")
     ap.add_argument("--batch", type=int, default=0, help="--survey: this number of controllers only")
     ap.add_argument("--variant", type=int, default=0, help="--survey: mppi_variant (0 AUTO, 1 THROUGHPUT, 2 LATENCY, 3 PACKED, 4 PIPELINED)")
