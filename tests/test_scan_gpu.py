@@ -217,3 +217,41 @@ def test_run_to_run_determinism_and_host_entry():
     h = m.step_host(wl.x0, wl.start, wl.u_nom, 3, 11)
     np.testing.assert_array_equal(h[0], a["u_new"])
     m.close()
+
+
+@pytest.mark.parametrize("fuzz_seed", [1, 2, 3])
+def test_random_tracks_states_and_sizes(fuzz_seed):
+    # seeded fuzz over what the kernel's special handling depends on: the number of gates (1: the target index never
+    # changes value; 2, 3: it wraps inside a horizon), gates in a row at random spacing so that chunks hold zero to
+    # several passes, random start index, speed, spin and attitude, horizons 1 .. 64, block sizes from K and B, both gate
+    # objectives with random flags and both readings of the near term, both math modes, sigma from small to large
+    rng = np.random.default_rng(1000 + fuzz_seed)
+    crossed, multi = 0, 0
+    for case in range(14):
+        obj = int(rng.choice([0, 3]))
+        K = int(rng.choice([32, 64, 160, 256, 512, 1024])); N = int(rng.integers(1, 65)); B = int(rng.integers(1, 4))
+        G = int(rng.choice([1, 2, 3, 5, 8]))
+        wl = W.stress_gate(K=K, N=N)
+        gates = np.zeros((G, 11), np.float32)
+        gates[:, 0] = 1.0 + np.cumsum(rng.uniform(0.6, 2.2, G)); gates[:, 1] = rng.uniform(-0.15, 0.15, G); gates[:, 2] = 2.0 + rng.uniform(-0.15, 0.15, G)
+        gates[:, 3] = 1.0; gates[:, 7] = 1.0; gates[:, 9] = rng.uniform(0.7, 1.2, G); gates[:, 10] = rng.uniform(0.6, 1.0, G)
+        wl.gates = gates
+        x0 = np.zeros((1, 13), np.float32)
+        x0[0, 0:3] = [0.0, rng.uniform(-0.3, 0.3), 2.0 + rng.uniform(-0.3, 0.3)]
+        q = np.array([1.0, 0, 0, 0]) + rng.normal(0, 0.05, 4); x0[0, 3:7] = q / np.linalg.norm(q)
+        x0[0, 7:10] = [rng.uniform(2.0, 12.0), rng.normal(0, 0.5), rng.normal(0, 0.5)]
+        x0[0, 10:13] = rng.normal(0, 3.0, 3)
+        wl.x0 = x0
+        wl.start[:] = 0 if rng.uniform() < 0.7 else int(rng.integers(-3, 12))
+        wl.params["sigma"] = np.float32(rng.choice([0.3, 1.0, 2.5]))
+        wl.params["lambda"] = np.float32(rng.choice([0.05, 0.5, 5.0]))
+        if obj == 3:
+            wl.params.update(objective=3, q_near=np.float32(2.0), r_near=np.float32(1.5), near_mode=int(rng.integers(0, 2)))
+            wl.prev_front = (rng.uniform(size=(1, N + 1)) < 0.6).astype(np.int32)
+        if B > 1:
+            wl = W.replicate(wl, B, 0.2)
+        math = int(rng.integers(0, 2))
+        tag = f"scan fuzz {fuzz_seed}/{case}: obj {obj} K {K} N {N} B {B} G {G} math {math}"
+        g, o, st, _ = run_case(wl, tag, it=case, variant=SCAN, fast_math=math)
+        crossed += int((o["ncross"] >= 1).sum()); multi += int((o["ncross"] >= 2).sum())
+    assert crossed > 1000 and multi > 100, (crossed, multi)       # the re-scoring rounds really ran
